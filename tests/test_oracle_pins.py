@@ -1,0 +1,317 @@
+"""Pins for the CPU oracle (oracle/kvpool_oracle.c): it is checked against what the paper and the mathematics
+fix, never against itself.  No GPU, no product code.  Each test says which plausible mistake it would catch.
+"""
+import itertools
+import os
+from decimal import Decimal, ROUND_HALF_UP
+from fractions import Fraction
+from math import floor
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import exact
+
+
+def _golden_rows(golden_dir, name):
+    with open(os.path.join(golden_dir, name)) as f:
+        for line in f:
+            line = line.strip()
+            if line and not line.startswith("#"):
+                yield [c.strip() for c in line.split("|")]
+
+
+# ------------------------------------------------------------------------------------------------
+# geometry: values the paper prints
+# ------------------------------------------------------------------------------------------------
+def test_kv_bytes_matches_sizes_printed_in_paper(golden_dir):
+    rows = list(_golden_rows(golden_dir, "paper_kv_sizes.txt"))
+    assert len(rows) == 4
+    for label, L, H, D, e, tokens, printed, decimals, _cite in rows:
+        got = oracle.kv_bytes(int(L), int(H), int(D), int(e), int(tokens))
+        gib = Decimal(got) / Decimal(2 ** 30)
+        q = Decimal(1).scaleb(-int(decimals))
+        assert gib.quantize(q, rounding=ROUND_HALF_UP) == Decimal(printed), label
+
+
+def test_kv_bytes_matches_baseline_config_sizes():
+    # BASELINE.json: 128 MiB @1K and 4 GiB @32K (LLaMA-8B), ~6 GiB (GPT-OSS-20B), ~12 GiB (Qwen3), bf16
+    MiB, GiB = 2 ** 20, 2 ** 30
+    assert oracle.kv_bytes(32, 8, 128, 2, 1024) == 128 * MiB
+    assert oracle.kv_bytes(32, 8, 128, 2, 32768) == 4 * GiB
+    assert oracle.kv_bytes(24, 8, 64, 2, 131072) == 6 * GiB
+    assert oracle.kv_bytes(48, 4, 128, 2, 131072) == 12 * GiB
+    assert sum(oracle.kv_bytes(32, 8, 128, 2, t) for t in (32768, 65536, 98304, 131072)) == 40 * GiB
+
+
+# ------------------------------------------------------------------------------------------------
+# weights: the single floating-point step
+# ------------------------------------------------------------------------------------------------
+def test_weights_are_bandwidth_in_integer_mb_per_s_round_half_up():
+    b = [55.62, 57.26, 21.3, 63.0, 0.001, 2.0, 1.0, 12.3456]
+    w = oracle.weights(b)
+    for bi, wi in zip(b, w):
+        # exact decimal value of the double, then round half up to an integer number of MB/s
+        want = int((Decimal(bi) * 1000).quantize(Decimal(1), rounding=ROUND_HALF_UP))
+        assert int(wi) == want
+    with pytest.raises(ValueError):
+        oracle.weights([1.0, 0.0])
+    with pytest.raises(ValueError):
+        oracle.weights([1.0, -3.0])
+    with pytest.raises(ValueError):
+        oracle.weights([0.0004])
+
+
+# ------------------------------------------------------------------------------------------------
+# counts: Eq. 1-2, Alg. 1 l.4-12
+# ------------------------------------------------------------------------------------------------
+def _random_cases(seed, n_cases, max_n=8, max_k=400, max_w=60000):
+    rng = np.random.default_rng(seed)
+    for _ in range(n_cases):
+        n = int(rng.integers(1, max_n + 1))
+        w = [int(x) for x in rng.integers(1, max_w + 1, size=n)]
+        if rng.random() < 0.3:                       # force ties between weights
+            w = [w[int(rng.integers(0, n))] if rng.random() < 0.5 else x for x in w]
+        K = int(rng.integers(0, max_k + 1))
+        yield w, K
+
+
+def test_counts_invariants_exact_rational():
+    """Catches: ceil/round instead of floor, remainder given to one device or to the wrong ones, float drift."""
+    for w, K in _random_cases(1, 3000):
+        c = [int(x) for x in oracle.counts(w, K)]
+        W = sum(w)
+        p = [Fraction(wi, W) for wi in w]
+        assert sum(c) == K                                              # the constraint at PAPER.md:175
+        fl = [floor(pi * K) for pi in p]
+        assert all(ci in (f, f + 1) for ci, f in zip(c, fl))            # Eq. 2 with r_i in {0,1}
+        assert all(abs(ci - pi * K) < 1 for ci, pi in zip(c, p))        # share within one block (north star)
+        r = K - sum(fl)
+        assert 0 <= r <= len(w) - 1 or (len(w) == 1 and r == 0)
+        extras = {i for i in range(len(w)) if c[i] == fl[i] + 1}
+        order = sorted(range(len(w)), key=lambda i: (-p[i], i))
+        assert extras == set(order[:r])                                 # "devices with larger p_i"
+
+
+def test_counts_unique_solution_by_brute_force():
+    """Enumerate every vector with c_i in {floor, floor+1} and sum K whose +1 set is closed under 'larger p first';
+    exactly one exists and the oracle returns it."""
+    for w, K in _random_cases(2, 300, max_n=6, max_k=60, max_w=9):
+        W = sum(w)
+        fl = [(wi * K) // W for wi in w]
+        # independent floor: compare against Fraction too
+        assert fl == [floor(Fraction(wi, W) * K) for wi in w]
+        sols = []
+        for bits in itertools.product((0, 1), repeat=len(w)):
+            if sum(fl) + sum(bits) != K:
+                continue
+            ok = True
+            for i, j in itertools.permutations(range(len(w)), 2):
+                # j got an extra but i did not although i has priority (larger p, or equal p and lower index)
+                if bits[j] and not bits[i] and (w[i] > w[j] or (w[i] == w[j] and i < j)):
+                    ok = False
+            if ok:
+                sols.append([f + b for f, b in zip(fl, bits)])
+        assert len(sols) == 1
+        assert [int(x) for x in oracle.counts(w, K)] == sols[0]
+
+
+def test_counts_closed_forms():
+    for n in (1, 2, 3, 4, 6, 8):
+        for m in (0, 1, 5, 192, 1024):
+            assert list(oracle.counts([7] * n, n * m)) == [m] * n           # equal weights, N | K
+    assert list(oracle.counts([5], 12345)) == [12345]                       # one device takes everything
+    # scaling all weights by a constant changes nothing (p_i is a ratio)
+    for w, K in _random_cases(3, 200):
+        assert list(oracle.counts(w, K)) == list(oracle.counts([3 * x for x in w], K))
+    # huge weights and K: 128-bit product must not overflow (p*K computed exactly)
+    w = [2 ** 40 + 1, 2 ** 40, 3]
+    K = 2 ** 31 - 1
+    c = [int(x) for x in oracle.counts(w, K)]
+    assert sum(c) == K and all(abs(ci - Fraction(wi, sum(w)) * K) < 1 for ci, wi in zip(c, w))
+
+
+def test_counts_and_wrr_hand_worked_examples(golden_dir):
+    n_counts = n_wrr = 0
+    for row in _golden_rows(golden_dir, "worked_placements.txt"):
+        if row[0] == "counts":
+            w = [int(x) for x in row[1].split(",")]
+            want = [int(x) for x in row[3].split(",")]
+            assert [int(x) for x in oracle.counts(w, int(row[2]))] == want, row
+            n_counts += 1
+        elif row[0] == "wrr":
+            c = [int(x) for x in row[1].split(",")]
+            dev, _ = oracle.wrr(c, sum(c))
+            assert "".join(str(int(d)) for d in dev) == row[2], row
+            n_wrr += 1
+    assert n_counts >= 9 and n_wrr >= 6
+
+
+# ------------------------------------------------------------------------------------------------
+# weighted round-robin: Alg. 1 l.13-16
+# ------------------------------------------------------------------------------------------------
+def test_wrr_bijection_slot_order_and_prefix_fairness():
+    """Catches: a block placed twice or never, slots not in enumeration order, bursty (first-fit) assignment."""
+    for w, K in _random_cases(4, 1500):
+        c = [int(x) for x in oracle.counts(w, K)]
+        dev, slot = oracle.wrr(c, K)
+        dev, slot = [int(x) for x in dev], [int(x) for x in slot]
+        n = len(c)
+        assert sorted(zip(dev, slot)) == [(i, s) for i in range(n) for s in range(c[i])]   # placed exactly once
+        a = [0] * n
+        for j in range(K):
+            assert slot[j] == a[dev[j]]                                  # slots ascend with j within a device
+            a[dev[j]] += 1
+            for i in range(n):                                           # prefix fairness, both sides
+                ideal = Fraction(c[i] * (j + 1), K)
+                assert -1 < a[i] - ideal <= Fraction((n - 1) * c[i], K)
+
+
+def test_wrr_equals_merge_of_sorted_ideal_times():
+    """Independent algorithm: the k-th item of device i has ideal time k/c_i; a global sort of all
+    (k/c_i, i) pairs (a library sort, no greedy loop) must give the same sequence."""
+    for w, K in _random_cases(5, 600):
+        c = [int(x) for x in oracle.counts(w, K)]
+        dev, slot = oracle.wrr(c, K)
+        keys = sorted((Fraction(k, c[i]), i, k - 1) for i in range(len(c)) for k in range(1, c[i] + 1))
+        assert [int(d) for d in dev] == [i for _, i, _ in keys]
+        assert [int(s) for s in slot] == [s for _, _, s in keys]
+
+
+def test_wrr_closed_forms():
+    for n in (1, 2, 4, 8):
+        m = 24
+        dev, slot = oracle.wrr([m] * n, n * m)
+        assert list(dev) == [j % n for j in range(n * m)]                # equal counts: plain round-robin
+        assert list(slot) == [j // n for j in range(n * m)]
+    dev, _ = oracle.wrr([2 * 30, 30], 90)
+    assert list(dev) == [0, 0, 1] * 30                                   # 2:1 with 3 | K
+    dev, slot = oracle.wrr([17], 17)
+    assert list(dev) == [0] * 17 and list(slot) == list(range(17))       # N = 1: identity
+    dev, _ = oracle.wrr([0, 5, 0], 5)
+    assert list(dev) == [1] * 5                                          # devices with c_i = 0 never chosen
+    with pytest.raises(ValueError):
+        oracle.wrr([2, 2], 5)                                            # counts must sum to K
+
+
+def test_c_oracle_equals_exact_rational_statement():
+    for w, K in _random_cases(6, 500, max_k=200):
+        assert [int(x) for x in oracle.counts(w, K)] == exact.counts(w, K)
+        c = exact.counts(w, K)
+        d, s = oracle.wrr(c, K)
+        d2, s2 = exact.wrr(c, K)
+        assert [int(x) for x in d] == d2 and [int(x) for x in s] == s2
+
+
+def test_place_applies_algorithm_per_layer():
+    pls = oracle.place([2.0, 1.0], [64, 0, 8, 3])
+    assert [list(p.counts) for p in pls] == [[43, 21], [0, 0], [6, 2], [2, 1]]   # 8*2/3 = 5.33 -> 5, 8/3 = 2.67 -> 2, 1 left -> dev 0
+    assert [len(p.dev) for p in pls] == [64, 0, 8, 3]
+
+
+# ------------------------------------------------------------------------------------------------
+# gather / scatter: MEMSTORE and retrieval
+# ------------------------------------------------------------------------------------------------
+def _tiny_layer(rng, nphys, kvb):
+    return rng.integers(0, 2 ** 16, size=(2, nphys, kvb // 2), dtype=np.uint16)
+
+
+def test_offload_single_device_is_fancy_indexing():
+    """N = 1: stripe == kv[:, table] with K and V interleaved per block (library routine)."""
+    rng = np.random.default_rng(7)
+    nphys, kvb, K = 37, 64, 23
+    kv = _tiny_layer(rng, nphys, kvb)
+    table = rng.permutation(nphys)[:K].astype(np.int32)
+    pl = oracle.place([3.0], [K])[0]
+    (stripe,) = oracle.offload_layer(kv, table, pl)
+    want = np.stack([kv[0][table], kv[1][table]], axis=1)               # [K, 2, kvb/2]: K block then V block
+    assert stripe.tobytes() == want.tobytes()
+    # identity table over the whole pool: plain memcpy of K plane / V plane, interleaved per block
+    table = np.arange(nphys, dtype=np.int32)
+    pl = oracle.place([3.0], [nphys])[0]
+    (stripe,) = oracle.offload_layer(kv, table, pl)
+    assert stripe.tobytes() == np.stack([kv[0], kv[1]], axis=1).tobytes()
+
+
+def test_retrieve_single_device_is_index_assignment():
+    rng = np.random.default_rng(8)
+    nphys, kvb, K = 29, 32, 11
+    table = rng.permutation(nphys)[:K].astype(np.int32)
+    pl = oracle.place([1.0], [K])[0]
+    stripe = rng.integers(0, 256, size=K * 2 * kvb, dtype=np.uint8)
+    out = np.full((2, nphys, kvb // 2), 0x7FC1, dtype=np.uint16)
+    oracle.retrieve_layer(out, table, pl, [stripe])
+    want = np.full((2, nphys, kvb // 2), 0x7FC1, dtype=np.uint16)
+    pay = stripe.view(np.uint16).reshape(K, 2, kvb // 2)
+    want[0][table] = pay[:, 0]
+    want[1][table] = pay[:, 1]
+    assert out.tobytes() == want.tobytes()
+
+
+def test_offload_retrieve_match_brute_force_search():
+    """Catches: K/V swapped, slot stride wrong, table applied on the wrong side, dev/slot transposed."""
+    rng = np.random.default_rng(9)
+    for _ in range(40):
+        n = int(rng.integers(1, 6))
+        bw = [float(x) for x in rng.integers(1, 9, size=n)]
+        nphys = int(rng.integers(1, 40))
+        K = int(rng.integers(0, nphys + 1))
+        kvb = int(rng.choice([16, 48, 64]))
+        kv = _tiny_layer(rng, nphys, kvb)
+        table = rng.permutation(nphys)[:K].astype(np.int32)
+        pl = oracle.place(bw, [K])[0]
+        stripes = oracle.offload_layer(kv, table, pl)
+        kb = [kv[0, p].tobytes() for p in range(nphys)]
+        vb = [kv[1, p].tobytes() for p in range(nphys)]
+        want = exact.offload_bruteforce(kb, vb, [int(t) for t in table], [int(d) for d in pl.dev],
+                                        [int(s) for s in pl.slot], [int(c) for c in pl.counts])
+        assert [s.tobytes() for s in stripes] == want
+        # retrieve into poison, compare with the brute-force inverse
+        out = np.full_like(kv, 0x7FC1)
+        oracle.retrieve_layer(out, table, pl, stripes)
+        kb2 = [np.full(kvb // 2, 0x7FC1, np.uint16).tobytes()] * nphys
+        vb2 = list(kb2)
+        kb2 = list(kb2)
+        exact.retrieve_bruteforce(kb2, vb2, [int(t) for t in table], [int(d) for d in pl.dev],
+                                  [int(s) for s in pl.slot], want, kvb)
+        assert out[0].tobytes() == b"".join(kb2) and out[1].tobytes() == b"".join(vb2)
+
+
+def test_round_trip_conservation_and_no_stray_writes():
+    rng = np.random.default_rng(10)
+    nphys, kvb, K = 96, 128, 64
+    kv = _tiny_layer(rng, nphys, kvb)
+    table = rng.permutation(nphys)[:K].astype(np.int32)
+    pl = oracle.place([4, 4, 2, 2, 1, 1], [K])[0]
+    stripes = oracle.offload_layer(kv, table, pl)
+    # byte share per device within one block of its bandwidth share (north star invariant)
+    P = 2 * kvb
+    for s, wi in zip(stripes, [4, 4, 2, 2, 1, 1]):
+        assert abs(Fraction(s.nbytes) - Fraction(wi, 14) * K * P) < P
+    # conservation: multiset of payloads == multiset of the request's blocks
+    pays = sorted(s[i * P:(i + 1) * P].tobytes() for s in stripes for i in range(s.nbytes // P))
+    want = sorted(kv[0, t].tobytes() + kv[1, t].tobytes() for t in table)
+    assert pays == want
+    out = np.full_like(kv, 0x7FC1)
+    oracle.retrieve_layer(out, table, pl, stripes)
+    used = np.zeros(nphys, bool)
+    used[table] = True
+    assert np.array_equal(out[:, used], kv[:, used])                    # bit-for-bit round trip
+    assert np.all(out[:, ~used] == 0x7FC1)                              # nothing else touched
+    # worker-thread variant (Alg. 1 l.17) gives the same bytes
+    stripes_mt = oracle.offload_layer(kv, table, pl, parallel=True)
+    assert [a.tobytes() for a in stripes_mt] == [a.tobytes() for a in stripes]
+    out_mt = np.full_like(kv, 0x7FC1)
+    oracle.retrieve_layer(out_mt, table, pl, stripes, parallel=True)
+    assert out_mt.tobytes() == out.tobytes()
+
+
+def test_empty_layer_is_a_noop():
+    kv = np.arange(2 * 4 * 8, dtype=np.uint16).reshape(2, 4, 8)
+    pl = oracle.place([2.0, 1.0], [0])[0]
+    stripes = oracle.offload_layer(kv, np.zeros(0, np.int32), pl)
+    assert [s.nbytes for s in stripes] == [0, 0]
+    out = kv.copy()
+    oracle.retrieve_layer(out, np.zeros(0, np.int32), pl, stripes)
+    assert np.array_equal(out, kv)
