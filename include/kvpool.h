@@ -1,0 +1,185 @@
+/*
+ * kvpool.h — C ABI of the B200-native unified KV pooling hot path (arxiv 2606.14779).
+ *
+ * The library moves a request's *paged* KV cache between GPU HBM and a pool of pinned host buffers
+ * ("pool devices"), assigning each layer's KV blocks to pool devices in proportion to
+ * their measured bandwidth (Eq. 1-2; Algorithm 1) and retrieving
+ * them through a dense global lookup table (Table I; retrieval).
+ *
+ * Conventions
+ *   - Every function returns KVPOOL_OK (0) or a negative KVPOOL_E* code; kvpool_last_error() gives a
+ *     thread-local message for the last failure.  Nothing throws or aborts across the ABI.  A call that
+ *     fails with EINVAL / ENOMEM / ESTATE has had no effect.
+ *   - "host" / "device" after a pointer says where the memory lives.  The caller owns the paged KV
+ *     tensors, block tables and CUDA streams; the library owns pool buffers, staging buffers, its own
+ *     streams/events and the per-placement tables.  The library never frees or keeps caller memory
+ *     beyond the stream work a call enqueues.
+ *   - One "KV cache" of the paper = one paged block of one layer: K block then V block,
+ *     P = 2*kvb bytes with kvb = block_tokens*n_kv_heads*head_dim*elem_bytes (R6).
+ *   - There is no CPU fallback: without a CUDA device kvpool_create fails with KVPOOL_ECUDA.  The
+ *     kvpool_plan_* functions are pure host arithmetic and work anywhere.
+ *   - A pool handle is not thread-safe; use it from one host thread (any number of CUDA streams).
+ */
+#ifndef KVPOOL_H
+#define KVPOOL_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KVPOOL_MAX_DEVICES 32u
+
+#if defined(__GNUC__)
+#define KVPOOL_API __attribute__((visibility("default")))
+#else
+#define KVPOOL_API
+#endif
+
+enum {
+  KVPOOL_OK = 0,
+  KVPOOL_EINVAL = -1, /* bad argument: null pointer, bandwidth <= 0, misaligned base/stride, layer/dev out of range */
+  KVPOOL_ENOMEM = -2, /* a pool device has no room for its stripe, or host/device allocation failed */
+  KVPOOL_ECUDA = -3,  /* a CUDA runtime call failed (message has the CUDA error string) */
+  KVPOOL_ENUMA = -4,  /* KVPOOL_DEV_NUMA_STRICT and the pages could not be bound to the requested node */
+  KVPOOL_ESTATE = -5  /* retrieve of a layer that was never offloaded; release with work in flight; ... */
+};
+
+/* pool-device flags */
+#define KVPOOL_DEV_WRITE_COMBINED 1u /* cudaHostAllocWriteCombined (GPU-read-mostly; CPU reads become slow) */
+#define KVPOOL_DEV_NUMA_STRICT 2u    /* fail with ENUMA instead of falling back when binding is impossible */
+
+/* transfer paths (kvpool_set_path) */
+enum {
+  KVPOOL_PATH_AUTO = 0,     /* staged for layers >= the auto threshold, zero-copy below it            */
+  KVPOOL_PATH_STAGED = 1,   /* pack/unpack kernel <-> device staging + one cudaMemcpyAsync per stripe  */
+  KVPOOL_PATH_ZEROCOPY = 2  /* one kernel reads/writes the mapped host stripes directly over the link  */
+};
+/* kernel variants (kvpool_set_tuning) */
+enum {
+  KVPOOL_KERNEL_VEC16 = 0, /* 16-byte ld.global.nc / st.global, warp-contiguous, unrolled              */
+  KVPOOL_KERNEL_BULK = 1   /* cp.async.bulk global->shared->global rings with mbarrier completion      */
+};
+
+typedef struct kvpool kvpool_t;                     /* opaque pool                                       */
+typedef struct kvpool_placement kvpool_placement_t; /* opaque: one request's GLT + reserved stripes      */
+
+typedef struct {           /* one pool device (MEM type; Table I)                          */
+  double bandwidth_gbps;   /* b_i of Eq. 1, measured, in 1e9 B/s; > 0                                   */
+  uint64_t capacity_bytes; /* size of the pinned, mapped host buffer the library allocates; > 0         */
+  int32_t numa_node;       /* -1 = no preference; else bind the pages to this node (mbind)              */
+  uint32_t flags;          /* KVPOOL_DEV_*                                                              */
+} kvpool_device_desc;
+
+typedef struct { /* geometry of one paged KV block */
+  uint32_t n_layers, block_tokens, n_kv_heads, head_dim, elem_bytes;
+} kvpool_geometry;
+
+typedef struct {         /* kvpool_set_tuning; 0 in any field = library default                          */
+  uint32_t kernel;       /* KVPOOL_KERNEL_*                                                             */
+  uint32_t hbm_ctas;     /* CTAs of an in-device pack/unpack launch (default: a multiple of the SM count) */
+  uint32_t link_ctas;    /* CTAs of a zero-copy launch (few suffice to fill the host link)               */
+  uint32_t bulk_chunk;   /* bytes per cp.async.bulk (power of two, 1 KiB..32 KiB)                        */
+  uint32_t bulk_stages;  /* ring depth per issuing warp                                                 */
+  uint32_t bulk_warps;   /* issuing warps per CTA                                                       */
+  uint32_t stage_slots;  /* staging buffers in the ring of the staged path (default 4)                   */
+  uint64_t auto_threshold_bytes; /* PATH_AUTO: layers moving fewer bytes than this go zero-copy          */
+} kvpool_tuning;
+
+/* ---- pure host arithmetic (no CUDA, no pool) --------------------------------------------------------
+ * Eq. 1: weights.  w_i = floor(b_i*1000 + 0.5) (integer MB/s); p_i = w_i / sum_j w_j exactly.
+ * EINVAL if n == 0, n > KVPOOL_MAX_DEVICES or some w_i < 1.                                            */
+KVPOOL_API int kvpool_plan_weights(const double* bandwidth_gbps /*host[n]*/, uint32_t n, uint64_t* w_out /*host[n]*/);
+/* Eq. 2 / Alg. 1 l.4-16 for one layer of K blocks: counts_out[i] = floor(p_i*K) plus one for the top
+ * (K - sum floors) devices by (p_i desc, i asc); dev_out[j], slot_out[j] = smooth weighted round-robin
+ * position of logical block j (device, index inside that device's stripe).  dev_out/slot_out may be
+ * NULL (counts only).                                                                                  */
+KVPOOL_API int kvpool_plan_layer(const uint64_t* w /*host[n]*/, uint32_t n, uint64_t K, uint32_t* counts_out /*host[n]*/,
+                      uint8_t* dev_out /*host[K] or NULL*/, uint32_t* slot_out /*host[K] or NULL*/);
+
+/* ---- pool life cycle ----------------------------------------------------------------------------------
+ * kvpool_create enumerates the pool devices: allocates one pinned, GPU-mapped host
+ * buffer per device (bound to its NUMA node when asked and possible), per-device CUDA streams, events
+ * and an empty GLT.  Slow (pins memory); not on the hot path.  cuda_device = CUDA ordinal.             */
+KVPOOL_API int kvpool_create(const kvpool_device_desc* devs /*host[n_devs]*/, uint32_t n_devs, const kvpool_geometry* geom /*host*/,
+                  int cuda_device, uint32_t flags /*0*/, kvpool_t** out);
+/* Waits for all work the pool enqueued, frees everything including live placements.                    */
+KVPOOL_API int kvpool_destroy(kvpool_t* pool);
+
+/* Replace the bandwidths ("measured bandwidth") — ESTATE while any placement is live.     */
+KVPOOL_API int kvpool_set_bandwidth(kvpool_t* pool, const double* bandwidth_gbps /*host[n_devs]*/);
+/* Measure pool device `dev`: cudaMemcpyAsync of `bytes` (<= capacity) between the pool buffer and a
+ * scratch device buffer, `iters` times, median, CUDA events.  direction 0 = host->GPU (retrieve
+ * direction), 1 = GPU->host.  Blocking; contents of the first `bytes` of the pool buffer are preserved
+ * for direction 0 and overwritten for direction 1 — ESTATE while any placement is live.                */
+KVPOOL_API int kvpool_measure_bandwidth(kvpool_t* pool, uint32_t dev, int direction, uint64_t bytes, uint32_t iters, double* gbps_out /*host*/);
+
+KVPOOL_API int kvpool_set_path(kvpool_t* pool, int path /*KVPOOL_PATH_**/);
+KVPOOL_API int kvpool_set_tuning(kvpool_t* pool, const kvpool_tuning* t /*host*/);
+KVPOOL_API int kvpool_get_tuning(const kvpool_t* pool, kvpool_tuning* t_out /*host*/);
+
+/* ---- placement: Alg. 1 l.4-16 + stripe allocation + GLT update (a1-a4) ------------------------------
+ * blocks_per_layer[l] = K_l, the number of KV blocks of layer l to offload (may differ per layer and
+ * may be 0).  Host work plus one upload of the per-layer tables.  ENOMEM (nothing reserved) if some pool
+ * device cannot hold its stripes.                                                                      */
+KVPOOL_API int kvpool_place(kvpool_t* pool, const uint32_t* blocks_per_layer /*host[n_layers]*/, kvpool_placement_t** out);
+/* Frees the stripes and tables.  The caller must have synchronised the streams it used with it.        */
+KVPOOL_API int kvpool_release(kvpool_t* pool, kvpool_placement_t* pl);
+
+/* ---- the hot path: one layer ---------------------------------------------------------------------------
+ * k_base / v_base: device pointers to the layer's K and V planes; physical block p is the kvb bytes at
+ * base + p*block_stride_bytes (covers [2,nphys,...] and [nphys,2,...] layouts).  Both bases and the
+ * stride must be multiples of 16.  block_table_dev: device int32[K_l], logical -> physical; entries are
+ * not validated on the device (duplicates / out-of-range are the caller's contract, R12).
+ * Asynchronous: returns once the work is enqueued.
+ *
+ * kvpool_offload  (Alg. 1 l.17-22, MEMSTORE): gathers the K_l blocks into the N stripes.  Work enqueued
+ *   on `stream` after the call may overwrite the source blocks (the gather is ordered on `stream`); the
+ *   stripe bytes are complete once kvpool_wait_offloads/kvpool_synchronize says so (zero-copy path: also
+ *   ordered on `stream`).  A later kvpool_retrieve of the same layer is ordered after it internally.
+ * kvpool_retrieve: scatters the stripes back into the paged layout; complete in
+ *   `stream` order.  ESTATE if the layer was never offloaded.  Host->GPU staging copies may run ahead of
+ *   `stream` (they touch only library memory), which is what overlaps layer l+1's I/O with layer l's
+ *   consumer (layerwise pipelining).                                                       */
+KVPOOL_API int kvpool_offload(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, const void* k_base /*device*/,
+                   const void* v_base /*device*/, uint64_t block_stride_bytes, const int32_t* block_table_dev,
+                   void* cuda_stream);
+KVPOOL_API int kvpool_retrieve(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, void* k_base /*device*/, void* v_base /*device*/,
+                    uint64_t block_stride_bytes, const int32_t* block_table_dev, void* cuda_stream);
+/* Make `stream` wait until every offload enqueued so far with `pl` has landed in the pool.             */
+KVPOOL_API int kvpool_wait_offloads(kvpool_t* pool, kvpool_placement_t* pl, void* cuda_stream);
+/* Block the host until all work the pool enqueued on its own streams is done (not the caller's).       */
+KVPOOL_API int kvpool_synchronize(kvpool_t* pool);
+
+/* In-device halves alone (a5 / a8): gather the layer's blocks into `stage_dev` (device, K_l*P bytes) in
+ * stripe order — device 0's stripe, then device 1's, ... — or scatter them back from it.  Ordered on
+ * `stream`.  These are the kernels whose HBM roofline the bench reports.                                */
+KVPOOL_API int kvpool_pack(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base,
+                uint64_t block_stride_bytes, const int32_t* block_table_dev, void* stage_dev, void* cuda_stream);
+KVPOOL_API int kvpool_unpack(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base,
+                  uint64_t block_stride_bytes, const int32_t* block_table_dev, const void* stage_dev, void* cuda_stream);
+
+/* ---- introspection (GLT, Table I) -----------------------------------------------------------------------*/
+KVPOOL_API int kvpool_n_devices(const kvpool_t* pool, uint32_t* n_out);
+KVPOOL_API int kvpool_weights(const kvpool_t* pool, uint64_t* w_out /*host[n_devs]*/);
+KVPOOL_API int kvpool_device_info(const kvpool_t* pool, uint32_t dev, void** host_base, uint64_t* capacity_bytes, uint64_t* used_bytes,
+                       int32_t* numa_node_actual /* -1 unknown */);
+KVPOOL_API int kvpool_counts(const kvpool_placement_t* pl, uint32_t layer, uint32_t* counts_out /*host[n_devs]*/);
+/* GLT entry of logical block `block` of `layer`: device_id, type (0 = MEM), slot inside that device's
+ * stripe and the host pointer of its payload (Table I "location").                                     */
+KVPOOL_API int kvpool_lookup(const kvpool_placement_t* pl, uint32_t layer, uint32_t block, uint32_t* device_id, uint32_t* type,
+                  uint32_t* slot, void** host_ptr);
+KVPOOL_API int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, void** host_ptr, uint64_t* nbytes);
+/* Whole-layer copies of the dense GLT columns (host[K_l] each; either may be NULL).                    */
+KVPOOL_API int kvpool_layer_map(const kvpool_placement_t* pl, uint32_t layer, uint8_t* dev_out, uint32_t* slot_out);
+/* Work counters since create: kernels launched and cudaMemcpyAsync calls issued by the library.        */
+KVPOOL_API int kvpool_stats(const kvpool_t* pool, uint64_t* kernel_launches, uint64_t* memcpy_calls);
+
+KVPOOL_API const char* kvpool_last_error(void);
+KVPOOL_API const char* kvpool_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KVPOOL_H */

@@ -1,0 +1,286 @@
+"""ctypes binding of libkvpool.so — same names as include/kvpool.h, argument marshalling only.
+
+Every step of the path runs inside the library's CUDA kernels / stream choreography; nothing here
+computes.  There is no fallback: if libkvpool.so is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, byref, c_char_p, c_double, c_int, c_int32, c_uint8, c_uint32, c_uint64, c_void_p
+from typing import List, Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libkvpool.so")
+
+MAX_DEVICES = 32
+OK, EINVAL, ENOMEM, ECUDA, ENUMA, ESTATE = 0, -1, -2, -3, -4, -5
+DEV_WRITE_COMBINED, DEV_NUMA_STRICT = 1, 2
+PATH_AUTO, PATH_STAGED, PATH_ZEROCOPY = 0, 1, 2
+KERNEL_VEC16, KERNEL_BULK = 0, 1
+_ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA", ESTATE: "ESTATE"}
+
+EXPORTS = [
+    "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
+    "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_place", "kvpool_release",
+    "kvpool_offload", "kvpool_retrieve", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack",
+    "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_counts", "kvpool_lookup", "kvpool_stripe",
+    "kvpool_layer_map", "kvpool_stats", "kvpool_last_error", "kvpool_version",
+]
+
+
+class DeviceDesc(ctypes.Structure):
+    _fields_ = [("bandwidth_gbps", c_double), ("capacity_bytes", c_uint64), ("numa_node", c_int32), ("flags", c_uint32)]
+
+
+class Geometry(ctypes.Structure):
+    _fields_ = [("n_layers", c_uint32), ("block_tokens", c_uint32), ("n_kv_heads", c_uint32), ("head_dim", c_uint32),
+                ("elem_bytes", c_uint32)]
+
+
+class Tuning(ctypes.Structure):
+    _fields_ = [("kernel", c_uint32), ("hbm_ctas", c_uint32), ("link_ctas", c_uint32), ("bulk_chunk", c_uint32),
+                ("bulk_stages", c_uint32), ("bulk_warps", c_uint32), ("stage_slots", c_uint32),
+                ("auto_threshold_bytes", c_uint64)]
+
+
+class KvPoolError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"kvpool {_ERRNAMES.get(code, code)}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libkvpool.so (loudly: no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing — build it with `python -m paper_2606_14779_b200.build`; "
+                              "there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        L.kvpool_last_error.restype = c_char_p
+        L.kvpool_version.restype = c_char_p
+        vp = c_void_p
+        sig = {
+            "kvpool_plan_weights": [vp, c_uint32, vp],
+            "kvpool_plan_layer": [vp, c_uint32, c_uint64, vp, vp, vp],
+            "kvpool_create": [vp, c_uint32, vp, c_int, c_uint32, POINTER(vp)],
+            "kvpool_destroy": [vp],
+            "kvpool_set_bandwidth": [vp, vp],
+            "kvpool_measure_bandwidth": [vp, c_uint32, c_int, c_uint64, c_uint32, POINTER(c_double)],
+            "kvpool_set_path": [vp, c_int],
+            "kvpool_set_tuning": [vp, vp],
+            "kvpool_get_tuning": [vp, vp],
+            "kvpool_place": [vp, vp, POINTER(vp)],
+            "kvpool_release": [vp, vp],
+            "kvpool_offload": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp],
+            "kvpool_retrieve": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp],
+            "kvpool_wait_offloads": [vp, vp, vp],
+            "kvpool_synchronize": [vp],
+            "kvpool_pack": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp, vp],
+            "kvpool_unpack": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp, vp],
+            "kvpool_n_devices": [vp, POINTER(c_uint32)],
+            "kvpool_weights": [vp, vp],
+            "kvpool_device_info": [vp, c_uint32, POINTER(vp), POINTER(c_uint64), POINTER(c_uint64), POINTER(c_int32)],
+            "kvpool_counts": [vp, c_uint32, vp],
+            "kvpool_lookup": [vp, c_uint32, c_uint32, POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32), POINTER(vp)],
+            "kvpool_stripe": [vp, c_uint32, c_uint32, POINTER(vp), POINTER(c_uint64)],
+            "kvpool_layer_map": [vp, c_uint32, vp, vp],
+            "kvpool_stats": [vp, POINTER(c_uint64), POINTER(c_uint64)],
+        }
+        for name, argtypes in sig.items():
+            f = getattr(L, name)
+            f.restype = c_int
+            f.argtypes = argtypes
+        _lib = L
+    return _lib
+
+
+def _ck(rc: int) -> None:
+    if rc != 0:
+        raise KvPoolError(rc, lib().kvpool_last_error().decode())
+
+
+def _addr(x) -> int:
+    """Device/host address of a torch tensor, numpy array, int or None."""
+    if x is None:
+        return 0
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    raise TypeError(f"cannot take the address of {type(x)}")
+
+
+def _stream(s) -> int:
+    if s is None:
+        return 0
+    if isinstance(s, int):
+        return s
+    return s.cuda_stream  # torch.cuda.Stream
+
+
+# ---- pure host arithmetic ----------------------------------------------------------------------------
+def kvpool_plan_weights(bandwidth_gbps: Sequence[float]) -> np.ndarray:
+    b = np.ascontiguousarray(bandwidth_gbps, dtype=np.float64)
+    w = np.zeros(b.shape[0], dtype=np.uint64)
+    _ck(lib().kvpool_plan_weights(b.ctypes.data, b.shape[0], w.ctypes.data))
+    return w
+
+
+def kvpool_plan_layer(w: Sequence[int], K: int, with_map: bool = True):
+    w = np.ascontiguousarray(w, dtype=np.uint64)
+    counts = np.zeros(w.shape[0], dtype=np.uint32)
+    dev = np.zeros(int(K), dtype=np.uint8) if with_map else None
+    slot = np.zeros(int(K), dtype=np.uint32) if with_map else None
+    _ck(lib().kvpool_plan_layer(w.ctypes.data, w.shape[0], int(K), counts.ctypes.data,
+                                dev.ctypes.data if with_map else None, slot.ctypes.data if with_map else None))
+    return (counts, dev, slot) if with_map else counts
+
+
+# ---- pool ---------------------------------------------------------------------------------------------
+class Placement:
+    def __init__(self, pool: "KvPool", handle: int, blocks_per_layer: np.ndarray):
+        self.pool, self.handle, self.blocks_per_layer = pool, handle, blocks_per_layer
+
+    def counts(self, layer: int) -> np.ndarray:
+        c = np.zeros(self.pool.n_devices, dtype=np.uint32)
+        _ck(lib().kvpool_counts(self.handle, layer, c.ctypes.data))
+        return c
+
+    def layer_map(self, layer: int) -> Tuple[np.ndarray, np.ndarray]:
+        K = int(self.blocks_per_layer[layer])
+        dev, slot = np.zeros(K, dtype=np.uint8), np.zeros(K, dtype=np.uint32)
+        _ck(lib().kvpool_layer_map(self.handle, layer, dev.ctypes.data, slot.ctypes.data))
+        return dev, slot
+
+    def lookup(self, layer: int, block: int) -> Tuple[int, int, int, int]:
+        d, t, s, p = c_uint32(), c_uint32(), c_uint32(), c_void_p()
+        _ck(lib().kvpool_lookup(self.handle, layer, block, byref(d), byref(t), byref(s), byref(p)))
+        return d.value, t.value, s.value, p.value or 0
+
+    def stripe(self, layer: int, dev: int) -> np.ndarray:
+        """The stripe's bytes as a uint8 numpy VIEW of the pinned pool buffer (no copy)."""
+        p, n = c_void_p(), c_uint64()
+        _ck(lib().kvpool_stripe(self.handle, layer, dev, byref(p), byref(n)))
+        if n.value == 0:
+            return np.zeros(0, dtype=np.uint8)
+        return np.ctypeslib.as_array(ctypes.cast(p.value, POINTER(c_uint8)), shape=(n.value,))
+
+    def release(self) -> None:
+        if self.handle:
+            _ck(lib().kvpool_release(self.pool.handle, self.handle))
+            self.handle = 0
+
+
+class KvPool:
+    """kvpool_create / kvpool_destroy and the per-layer calls, one method per ABI entry point."""
+
+    def __init__(self, bandwidth_gbps: Sequence[float], capacity_bytes: Sequence[int], *, n_layers: int, n_kv_heads: int,
+                 head_dim: int, block_tokens: int = 16, elem_bytes: int = 2, cuda_device: int = 0,
+                 numa_nodes: Optional[Sequence[int]] = None, dev_flags: Optional[Sequence[int]] = None):
+        n = len(bandwidth_gbps)
+        descs = (DeviceDesc * n)()
+        for i in range(n):
+            descs[i] = DeviceDesc(float(bandwidth_gbps[i]), int(capacity_bytes[i]), int(numa_nodes[i]) if numa_nodes else -1,
+                                  int(dev_flags[i]) if dev_flags else 0)
+        self.geometry = Geometry(n_layers, block_tokens, n_kv_heads, head_dim, elem_bytes)
+        self.kvb = block_tokens * n_kv_heads * head_dim * elem_bytes
+        self.payload = 2 * self.kvb
+        h = c_void_p()
+        _ck(lib().kvpool_create(ctypes.addressof(descs), n, ctypes.addressof(self.geometry), cuda_device, 0, byref(h)))
+        self.handle = h.value
+        self.n_devices = n
+
+    def destroy(self) -> None:
+        if getattr(self, "handle", 0):
+            _ck(lib().kvpool_destroy(self.handle))
+            self.handle = 0
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def set_bandwidth(self, bandwidth_gbps: Sequence[float]) -> None:
+        b = np.ascontiguousarray(bandwidth_gbps, dtype=np.float64)
+        assert b.shape[0] == self.n_devices
+        _ck(lib().kvpool_set_bandwidth(self.handle, b.ctypes.data))
+
+    def measure_bandwidth(self, dev: int, direction: int = 0, nbytes: int = 256 << 20, iters: int = 5) -> float:
+        g = c_double()
+        _ck(lib().kvpool_measure_bandwidth(self.handle, dev, direction, nbytes, iters, byref(g)))
+        return g.value
+
+    def set_path(self, path: int) -> None:
+        _ck(lib().kvpool_set_path(self.handle, path))
+
+    def set_tuning(self, **kw) -> None:
+        t = self.get_tuning()
+        cur_kernel = t.kernel
+        t = Tuning()
+        t.kernel = kw.pop("kernel", cur_kernel)
+        for k, v in kw.items():
+            setattr(t, k, v)
+        _ck(lib().kvpool_set_tuning(self.handle, ctypes.addressof(t)))
+
+    def get_tuning(self) -> Tuning:
+        t = Tuning()
+        _ck(lib().kvpool_get_tuning(self.handle, ctypes.addressof(t)))
+        return t
+
+    def place(self, blocks_per_layer: Sequence[int]) -> Placement:
+        b = np.ascontiguousarray(blocks_per_layer, dtype=np.uint32)
+        assert b.shape[0] == self.geometry.n_layers
+        h = c_void_p()
+        _ck(lib().kvpool_place(self.handle, b.ctypes.data, byref(h)))
+        return Placement(self, h.value, b)
+
+    def offload(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_dev, stream=None) -> None:
+        _ck(lib().kvpool_offload(self.handle, pl.handle, layer, _addr(k_base), _addr(v_base), block_stride_bytes,
+                                 _addr(block_table_dev), _stream(stream)))
+
+    def retrieve(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_dev, stream=None) -> None:
+        _ck(lib().kvpool_retrieve(self.handle, pl.handle, layer, _addr(k_base), _addr(v_base), block_stride_bytes,
+                                  _addr(block_table_dev), _stream(stream)))
+
+    def pack(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_dev, stage_dev, stream=None) -> None:
+        _ck(lib().kvpool_pack(self.handle, pl.handle, layer, _addr(k_base), _addr(v_base), block_stride_bytes,
+                              _addr(block_table_dev), _addr(stage_dev), _stream(stream)))
+
+    def unpack(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_dev, stage_dev, stream=None) -> None:
+        _ck(lib().kvpool_unpack(self.handle, pl.handle, layer, _addr(k_base), _addr(v_base), block_stride_bytes,
+                                _addr(block_table_dev), _addr(stage_dev), _stream(stream)))
+
+    def wait_offloads(self, pl: Placement, stream=None) -> None:
+        _ck(lib().kvpool_wait_offloads(self.handle, pl.handle, _stream(stream)))
+
+    def synchronize(self) -> None:
+        _ck(lib().kvpool_synchronize(self.handle))
+
+    def weights(self) -> np.ndarray:
+        w = np.zeros(self.n_devices, dtype=np.uint64)
+        _ck(lib().kvpool_weights(self.handle, w.ctypes.data))
+        return w
+
+    def device_info(self, dev: int) -> dict:
+        base, cap, used, node = c_void_p(), c_uint64(), c_uint64(), c_int32()
+        _ck(lib().kvpool_device_info(self.handle, dev, byref(base), byref(cap), byref(used), byref(node)))
+        return {"host_base": base.value, "capacity": cap.value, "used": used.value, "numa_node": node.value}
+
+    def stats(self) -> Tuple[int, int]:
+        k, m = c_uint64(), c_uint64()
+        _ck(lib().kvpool_stats(self.handle, byref(k), byref(m)))
+        return k.value, m.value
+
+
+def version() -> str:
+    return lib().kvpool_version().decode()

@@ -1,0 +1,202 @@
+// sm_100a pack / unpack kernels for paged KV blocks.
+//
+// Pure data movement: no tensor cores.  Two variants of the same gather/scatter, both templated on the
+// direction, both usable with a device staging buffer (HBM-bound) or with mapped pinned host stripes on
+// the pool side (host-link-bound, "zero-copy"):
+//
+//   kv_copy_vec16 : every warp moves 4 KiB pieces with 8 x 16-byte ld.global.nc.L1::no_allocate per lane
+//                   issued back to back, then 8 x st.global.L1::no_allocate — 512 contiguous bytes per
+//                   warp instruction, 128 B per lane in flight.
+//   kv_copy_bulk  : one elected lane per warp drives a ring of shared-memory stages with
+//                   cp.async.bulk global->shared (mbarrier complete_tx) and cp.async.bulk shared->global
+//                   (bulk groups); whole chunks of a block move without touching registers.
+//
+// Addressing of unit j is described in kernels.cuh (LayerArgs).
+#include "kernels.cuh"
+
+#include "../../include/kvpool.h"
+
+namespace kvp {
+namespace {
+
+constexpr int kVecThreads = 512;
+constexpr int kVecUnroll = 8;
+constexpr uint32_t kVecPiece = kVecUnroll * 32 * 16;  // 4096 bytes per warp iteration
+constexpr uint32_t kBulkBarrierBytes = 1024;          // room for warps*stages mbarriers in front of the ring
+
+__device__ __forceinline__ int4 ld_stream(const void* p) {
+  int4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream(void* p, const int4& v) {
+  asm volatile("st.global.L1::no_allocate.v4.s32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w)
+               : "memory");
+}
+
+// Decode work item t of a layer split into `pieces` pieces per K (or V) block of `piece_bytes` bytes.
+struct Piece {
+  uint8_t* paged;
+  uint8_t* pooled;
+  uint32_t bytes;
+};
+__device__ __forceinline__ Piece decode(const LayerArgs& a, uint64_t t, uint32_t pieces, uint32_t piece_bytes) {
+  const uint32_t per_unit = 2u * pieces;
+  const uint32_t j = static_cast<uint32_t>(t / per_unit);
+  const uint32_t r = static_cast<uint32_t>(t - static_cast<uint64_t>(j) * per_unit);
+  const uint32_t half = r >= pieces ? 1u : 0u;  // 0: K block, 1: V block
+  const uint32_t c = r - half * pieces;
+  const int32_t phys = __ldg(a.table + j);
+  const uint32_t d = __ldg(a.dev + j);
+  const uint32_t s = __ldg(a.slot + j);
+  const uint32_t off = c * piece_bytes;
+  Piece p;
+  p.paged = (half ? a.v_base : a.k_base) + static_cast<uint64_t>(phys) * a.stride + off;
+  p.pooled = reinterpret_cast<uint8_t*>(a.pool_base[d]) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;
+  p.bytes = min(piece_bytes, a.kvb - off);
+  return p;
+}
+
+template <bool PACK>
+__global__ void __launch_bounds__(kVecThreads) kv_copy_vec16(const __grid_constant__ LayerArgs a) {
+  const uint32_t lane = threadIdx.x & 31u;
+  const uint32_t warps_per_cta = blockDim.x >> 5;
+  const uint64_t nwarps = static_cast<uint64_t>(gridDim.x) * warps_per_cta;
+  const uint32_t pieces = (a.kvb + kVecPiece - 1) / kVecPiece;
+  const uint64_t total = static_cast<uint64_t>(a.K) * 2u * pieces;
+  for (uint64_t t = static_cast<uint64_t>(blockIdx.x) * warps_per_cta + (threadIdx.x >> 5); t < total; t += nwarps) {
+    const Piece p = decode(a, t, pieces, kVecPiece);
+    const uint8_t* src = (PACK ? p.paged : p.pooled) + lane * 16u;
+    uint8_t* dst = (PACK ? p.pooled : p.paged) + lane * 16u;
+    int4 v[kVecUnroll];
+    if (p.bytes == kVecPiece) {
+#pragma unroll
+      for (int u = 0; u < kVecUnroll; ++u) v[u] = ld_stream(src + u * 512);
+#pragma unroll
+      for (int u = 0; u < kVecUnroll; ++u) st_stream(dst + u * 512, v[u]);
+    } else {  // ragged last piece of a block (kvb not a multiple of 4 KiB; always a multiple of 16)
+#pragma unroll
+      for (int u = 0; u < kVecUnroll; ++u)
+        if (u * 512u + lane * 16u < p.bytes) v[u] = ld_stream(src + u * 512);
+#pragma unroll
+      for (int u = 0; u < kVecUnroll; ++u)
+        if (u * 512u + lane * 16u < p.bytes) st_stream(dst + u * 512, v[u]);
+    }
+  }
+}
+
+// ---- cp.async.bulk / mbarrier primitives (PTX ISA 8.x, sm_90+; SASS: UBLKCP, SYNCS) ------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "KV_WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra KV_DONE_%=;\n"
+      "bra KV_WAIT_%=;\n"
+      "KV_DONE_%=:\n"
+      "}" ::"r"(bar),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst_smem),
+               "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src_smem, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src_smem), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read_1() { asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+// Each warp's lane 0 owns `stages` shared-memory buffers of `chunk` bytes and walks its share of the
+// layer's chunks: up to stages-1 loads are in flight while the oldest landed chunk is stored out.
+template <bool PACK>
+__global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ LayerArgs a, uint32_t chunk, uint32_t stages) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  if ((threadIdx.x & 31u) != 0) return;
+  const uint32_t warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const uint32_t bar0 = smem_u32(smem) + warp * stages * 8u;
+  const uint32_t buf0 = smem_u32(smem) + kBulkBarrierBytes + warp * stages * chunk;
+  for (uint32_t s = 0; s < stages; ++s) mbar_init(bar0 + 8u * s, 1);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+
+  const uint32_t pieces = a.kvb / chunk;  // host guarantees chunk | kvb
+  const uint64_t total = static_cast<uint64_t>(a.K) * 2u * pieces;
+  const uint64_t gw = static_cast<uint64_t>(blockIdx.x) * nw + warp, ngw = static_cast<uint64_t>(gridDim.x) * nw;
+  const uint64_t mine = gw < total ? (total - gw + ngw - 1) / ngw : 0;
+
+  uint64_t issued = 0;
+  uint8_t* out_ring[8];  // destination of the chunk sitting in each stage (stages <= 8)
+  auto issue = [&](uint64_t n) {
+    const uint32_t s = static_cast<uint32_t>(n % stages);
+    const Piece p = decode(a, gw + n * ngw, pieces, chunk);
+    out_ring[s] = PACK ? p.pooled : p.paged;
+    mbar_arrive_expect_tx(bar0 + 8u * s, chunk);
+    bulk_g2s(buf0 + s * chunk, PACK ? p.paged : p.pooled, chunk, bar0 + 8u * s);
+  };
+  for (; issued < mine && issued + 1 < stages; ++issued) issue(issued);
+  for (uint64_t i = 0; i < mine; ++i) {
+    const uint32_t s = static_cast<uint32_t>(i % stages);
+    mbar_wait(bar0 + 8u * s, static_cast<uint32_t>(i / stages) & 1u);
+    bulk_s2g(out_ring[s], buf0 + s * chunk, chunk);
+    bulk_commit();
+    if (issued < mine) {
+      bulk_wait_read_1();  // the store issued one iteration ago has drained its stage: refill that stage
+      issue(issued);
+      ++issued;
+    }
+  }
+  bulk_wait_all();
+}
+
+uint32_t bulk_chunk_for(uint32_t kvb, uint32_t want) {
+  uint32_t c = 16;
+  while (c * 2 <= want && kvb % (c * 2) == 0) c *= 2;
+  return c;
+}
+
+}  // namespace
+
+cudaError_t kernels_init() {
+  cudaError_t e = cudaFuncSetAttribute(kv_copy_bulk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(kv_copy_bulk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+}
+
+cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream) {
+  if (a.K == 0) return cudaSuccess;
+  if (cfg.kernel == KVPOOL_KERNEL_BULK) {
+    const uint32_t chunk = bulk_chunk_for(a.kvb, cfg.bulk_chunk);
+    const uint32_t stages = cfg.bulk_stages < 2 ? 2 : (cfg.bulk_stages > 8 ? 8 : cfg.bulk_stages);
+    uint32_t warps = cfg.bulk_warps < 1 ? 1 : (cfg.bulk_warps > 8 ? 8 : cfg.bulk_warps);
+    while (warps > 1 && static_cast<uint64_t>(warps) * stages * chunk + kBulkBarrierBytes > 200u * 1024u) --warps;
+    const uint64_t total = static_cast<uint64_t>(a.K) * 2u * (a.kvb / chunk);
+    const uint64_t want = (total + warps - 1) / warps;
+    const uint32_t grid = static_cast<uint32_t>(want < cfg.ctas ? want : cfg.ctas);
+    const size_t smem = kBulkBarrierBytes + static_cast<size_t>(warps) * stages * chunk;
+    if (pack) kv_copy_bulk<true><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
+    else kv_copy_bulk<false><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
+  } else {
+    const uint32_t pieces = (a.kvb + kVecPiece - 1) / kVecPiece;
+    const uint64_t total = static_cast<uint64_t>(a.K) * 2u * pieces;
+    const uint64_t want = (total + (kVecThreads / 32) - 1) / (kVecThreads / 32);
+    const uint32_t grid = static_cast<uint32_t>(want < cfg.ctas ? want : cfg.ctas);
+    if (pack) kv_copy_vec16<true><<<grid, kVecThreads, 0, stream>>>(a);
+    else kv_copy_vec16<false><<<grid, kVecThreads, 0, stream>>>(a);
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace kvp

@@ -1,0 +1,39 @@
+// sm_100a pack / unpack kernels (a5, a8 of DESIGN.md §2; fused with a6/a7 when the pool side is mapped
+// host memory).  Launch interface only; kernels.cu has the device code.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+namespace kvp {
+
+constexpr uint32_t kMaxDev = 32;
+
+// One layer's work.  Unit j (logical block j) has
+//   paged side : K block = kvb bytes at k_base + table[j]*stride, V block likewise at v_base
+//   pool side  : P = 2*kvb bytes (K then V) at pool_base[dev[j]] + slot[j]*P
+// pool_base[i] is any address the GPU can reach: a device staging buffer (in-device pack/unpack) or the
+// device alias of a mapped pinned host stripe (zero-copy offload/retrieve).
+struct LayerArgs {
+  uint8_t* k_base;
+  uint8_t* v_base;
+  uint64_t stride;
+  const int32_t* table;
+  const uint8_t* dev;
+  const uint32_t* slot;
+  uint32_t K;
+  uint32_t kvb;
+  uint64_t pool_base[kMaxDev];
+};
+
+struct LaunchCfg {
+  uint32_t kernel;       // KVPOOL_KERNEL_VEC16 / KVPOOL_KERNEL_BULK
+  uint32_t ctas;         // grid size cap
+  uint32_t bulk_chunk, bulk_stages, bulk_warps;
+};
+
+// pack = true: paged -> pool side (offload direction); false: pool side -> paged (retrieve direction).
+cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream);
+// One-time per-device setup (shared-memory opt-in for the bulk kernels).
+cudaError_t kernels_init();
+
+}  // namespace kvp

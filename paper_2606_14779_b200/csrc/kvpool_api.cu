@@ -1,0 +1,752 @@
+// C ABI of libkvpool (include/kvpool.h): pool life cycle, placement + GLT, and the per-layer
+// offload / retrieve choreography over CUDA streams and events.  Device code lives in kernels.cu.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <memory>
+#include <mutex>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+#include "../../include/kvpool.h"
+#include "kernels.cuh"
+#include "placement.hpp"
+#include "pool_mem.hpp"
+
+using namespace kvp;
+
+static_assert(KVPOOL_MAX_DEVICES == kvp::kMaxDevices && KVPOOL_MAX_DEVICES == kvp::kMaxDev, "device limit mismatch");
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  g_err = buf;
+  return code;
+}
+
+#define CU(call)                                                                              \
+  do {                                                                                        \
+    cudaError_t e__ = (call);                                                                 \
+    if (e__ != cudaSuccess) return fail(KVPOOL_ECUDA, "%s: %s", #call, cudaGetErrorString(e__)); \
+  } while (0)
+
+struct DeviceGuard {  // make the pool's GPU current for the duration of a call
+  int prev = -1;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    if (prev != dev) cudaSetDevice(dev);
+    else prev = -1;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
+// Dense per-layer GLT columns shared by all layers of a placement that move the same number of blocks.
+struct LayerMap {
+  uint64_t K = 0;
+  std::vector<uint32_t> counts;   // [N]
+  std::vector<uint32_t> start;    // [N] first stripe-order position of device i (prefix sum of counts)
+  std::vector<uint8_t> dev;       // [K]
+  std::vector<uint32_t> slot;     // [K]
+  const uint8_t* dev_d = nullptr; // device copies
+  const uint32_t* slot_d = nullptr;
+};
+
+struct LayerState {
+  std::shared_ptr<LayerMap> map;
+  std::vector<uint64_t> stripe_off;  // [N] byte offset of this layer's stripe inside pool buffer i
+  bool offloaded = false;
+  cudaEvent_t landed = nullptr;      // recorded when the layer's stripes are complete in the pool
+  bool landed_pending = false;
+};
+
+struct StageSlot {
+  uint8_t* buf = nullptr;
+  cudaEvent_t kernel_done = nullptr;          // last kernel that read/wrote the slot
+  std::vector<cudaEvent_t> copy_done;         // [N] last memcpy per pool stream that read/wrote the slot
+};
+
+}  // namespace
+
+struct kvpool_placement {
+  kvpool* pool = nullptr;
+  std::vector<LayerState> layers;
+  void* tables_d = nullptr;  // one device allocation holding every LayerMap's dev/slot columns
+  cudaEvent_t join = nullptr;
+};
+
+struct kvpool {
+  int cuda_device = 0;
+  int sm_count = 148;
+  kvpool_geometry geom{};
+  uint64_t kvb = 0, payload = 0;
+  uint32_t n = 0;
+  std::vector<double> bandwidth;
+  std::vector<uint64_t> w;
+  std::vector<HostBuffer> bufs;
+  std::vector<StripeAllocator> alloc;
+  std::vector<cudaStream_t> io;  // one I/O stream per pool device ("independent I/O streams")
+  std::vector<StageSlot> slots;
+  uint64_t slot_bytes = 0;
+  uint64_t slot_cursor = 0;
+  cudaEvent_t fork = nullptr;
+  int path = KVPOOL_PATH_AUTO;
+  kvpool_tuning tune{};
+  std::vector<kvpool_placement*> live;
+  uint64_t n_kernels = 0, n_memcpys = 0;
+  std::mutex mu;
+};
+
+namespace {
+
+void default_tuning(kvpool* p) {
+  p->tune.kernel = KVPOOL_KERNEL_VEC16;
+  p->tune.hbm_ctas = 2u * p->sm_count;
+  p->tune.link_ctas = 16;
+  p->tune.bulk_chunk = 16384;
+  p->tune.bulk_stages = 6;
+  p->tune.bulk_warps = 2;
+  p->tune.stage_slots = 4;
+  p->tune.auto_threshold_bytes = 8ull << 20;
+}
+
+void free_slots(kvpool* p) {
+  for (auto& s : p->slots) {
+    if (s.buf) cudaFree(s.buf);
+    if (s.kernel_done) cudaEventDestroy(s.kernel_done);
+    for (auto e : s.copy_done) cudaEventDestroy(e);
+  }
+  p->slots.clear();
+  p->slot_bytes = 0;
+}
+
+int sync_pool_streams(kvpool* p) {
+  for (auto s : p->io) CU(cudaStreamSynchronize(s));
+  return KVPOOL_OK;
+}
+
+// (Re)build the staging ring so that every slot holds `bytes`.  Not on the hot path (called from place).
+int ensure_slots(kvpool* p, uint64_t bytes) {
+  if (bytes <= p->slot_bytes && p->slots.size() == p->tune.stage_slots) return KVPOOL_OK;
+  CU(cudaDeviceSynchronize());
+  const uint64_t want = std::max(bytes, p->slot_bytes);
+  free_slots(p);
+  p->slots.resize(p->tune.stage_slots);
+  for (auto& s : p->slots) {
+    if (want > 0) {
+      cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&s.buf), want);
+      if (e != cudaSuccess) {
+        cudaGetLastError();
+        free_slots(p);
+        return fail(KVPOOL_ENOMEM, "staging slot of %llu bytes: %s", (unsigned long long)want, cudaGetErrorString(e));
+      }
+    }
+    CU(cudaEventCreateWithFlags(&s.kernel_done, cudaEventDisableTiming));
+    s.copy_done.resize(p->n);
+    for (auto& e : s.copy_done) CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  }
+  p->slot_bytes = want;
+  return KVPOOL_OK;
+}
+
+bool is_live(const kvpool* p, const kvpool_placement* pl) {
+  return std::find(p->live.begin(), p->live.end(), pl) != p->live.end();
+}
+
+void destroy_placement(kvpool* p, kvpool_placement* pl) {
+  for (auto& L : pl->layers) {
+    for (uint32_t i = 0; i < p->n; ++i) p->alloc[i].free(L.stripe_off[i], static_cast<uint64_t>(L.map->counts[i]) * p->payload);
+    if (L.landed) cudaEventDestroy(L.landed);
+  }
+  if (pl->tables_d) cudaFree(pl->tables_d);
+  if (pl->join) cudaEventDestroy(pl->join);
+  delete pl;
+}
+
+int check_layer_call(kvpool* p, kvpool_placement* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
+                     const int32_t* table) {
+  if (!p || !pl) return fail(KVPOOL_EINVAL, "null pool or placement");
+  if (pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "placement does not belong to this pool");
+  if (layer >= p->geom.n_layers) return fail(KVPOOL_EINVAL, "layer %u out of range (n_layers %u)", layer, p->geom.n_layers);
+  if (pl->layers[layer].map->K == 0) return KVPOOL_OK;
+  if (!k_base || !v_base || !table) return fail(KVPOOL_EINVAL, "null k_base / v_base / block table");
+  if ((reinterpret_cast<uintptr_t>(k_base) | reinterpret_cast<uintptr_t>(v_base) | stride) & 15u)
+    return fail(KVPOOL_EINVAL, "k_base, v_base and block_stride_bytes must be multiples of 16");
+  if (stride < p->kvb) return fail(KVPOOL_EINVAL, "block_stride_bytes %llu < block bytes %llu", (unsigned long long)stride,
+                                   (unsigned long long)p->kvb);
+  return KVPOOL_OK;
+}
+
+LayerArgs base_args(const kvpool* p, const LayerState& L, const void* k_base, const void* v_base, uint64_t stride,
+                    const int32_t* table) {
+  LayerArgs a{};
+  a.k_base = static_cast<uint8_t*>(const_cast<void*>(k_base));
+  a.v_base = static_cast<uint8_t*>(const_cast<void*>(v_base));
+  a.stride = stride;
+  a.table = table;
+  a.dev = L.map->dev_d;
+  a.slot = L.map->slot_d;
+  a.K = static_cast<uint32_t>(L.map->K);
+  a.kvb = static_cast<uint32_t>(p->kvb);
+  return a;
+}
+
+LaunchCfg launch_cfg(const kvpool* p, bool link_bound) {
+  LaunchCfg c{};
+  c.kernel = p->tune.kernel;
+  c.ctas = link_bound ? p->tune.link_ctas : p->tune.hbm_ctas;
+  c.bulk_chunk = p->tune.bulk_chunk;
+  c.bulk_stages = p->tune.bulk_stages;
+  c.bulk_warps = p->tune.bulk_warps;
+  return c;
+}
+
+bool use_staged(const kvpool* p, const LayerState& L) {
+  if (p->path == KVPOOL_PATH_STAGED) return true;
+  if (p->path == KVPOOL_PATH_ZEROCOPY) return false;
+  return L.map->K * p->payload >= p->tune.auto_threshold_bytes;
+}
+
+// Make `s` wait until the previous user of a staging slot is done with it.
+int wait_slot_free(kvpool* p, StageSlot& slot, cudaStream_t s) {
+  CU(cudaStreamWaitEvent(s, slot.kernel_done, 0));
+  for (uint32_t i = 0; i < p->n; ++i) CU(cudaStreamWaitEvent(s, slot.copy_done[i], 0));
+  return KVPOOL_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* kvpool_last_error(void) { return g_err.c_str(); }
+const char* kvpool_version(void) { return "kvpool 0.1 (sm_100a)"; }
+
+int kvpool_plan_weights(const double* b, uint32_t n, uint64_t* w_out) {
+  if (!b || !w_out || n == 0 || n > KVPOOL_MAX_DEVICES) return fail(KVPOOL_EINVAL, "plan_weights: bad arguments");
+  if (!quantise_weights(b, n, w_out)) return fail(KVPOOL_EINVAL, "bandwidth must be positive and at least 0.0005 GB/s");
+  return KVPOOL_OK;
+}
+
+int kvpool_plan_layer(const uint64_t* w, uint32_t n, uint64_t K, uint32_t* counts_out, uint8_t* dev_out, uint32_t* slot_out) {
+  if (!w || !counts_out || n == 0 || n > KVPOOL_MAX_DEVICES || K > 0xFFFFFFFFull) return fail(KVPOOL_EINVAL, "plan_layer: bad arguments");
+  if ((dev_out == nullptr) != (slot_out == nullptr)) return fail(KVPOOL_EINVAL, "plan_layer: dev_out and slot_out go together");
+  for (uint32_t i = 0; i < n; ++i)
+    if (w[i] == 0) return fail(KVPOOL_EINVAL, "plan_layer: weight %u is zero", i);
+  target_counts(w, n, K, counts_out);
+  if (dev_out) wrr_closed_form(counts_out, n, K, dev_out, slot_out);
+  return KVPOOL_OK;
+}
+
+int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_geometry* g, int cuda_device, uint32_t flags,
+                  kvpool_t** out) {
+  if (!devs || !g || !out) return fail(KVPOOL_EINVAL, "create: null argument");
+  *out = nullptr;
+  if (flags != 0) return fail(KVPOOL_EINVAL, "create: unknown flags 0x%x", flags);
+  if (n_devs == 0 || n_devs > KVPOOL_MAX_DEVICES) return fail(KVPOOL_EINVAL, "create: n_devs %u not in 1..%u", n_devs, KVPOOL_MAX_DEVICES);
+  if (!g->n_layers || !g->block_tokens || !g->n_kv_heads || !g->head_dim || !g->elem_bytes) return fail(KVPOOL_EINVAL, "create: zero in geometry");
+  const uint64_t kvb = static_cast<uint64_t>(g->block_tokens) * g->n_kv_heads * g->head_dim * g->elem_bytes;
+  if (kvb % 16 != 0 || kvb > (1ull << 30)) return fail(KVPOOL_EINVAL, "create: block bytes %llu must be a multiple of 16 and <= 1 GiB", (unsigned long long)kvb);
+  std::vector<double> bw(n_devs);
+  std::vector<uint64_t> w(n_devs);
+  for (uint32_t i = 0; i < n_devs; ++i) {
+    bw[i] = devs[i].bandwidth_gbps;
+    if (devs[i].capacity_bytes == 0) return fail(KVPOOL_EINVAL, "create: device %u has zero capacity", i);
+    if (devs[i].flags & ~(KVPOOL_DEV_WRITE_COMBINED | KVPOOL_DEV_NUMA_STRICT)) return fail(KVPOOL_EINVAL, "create: device %u unknown flags", i);
+  }
+  if (!quantise_weights(bw.data(), n_devs, w.data())) return fail(KVPOOL_EINVAL, "create: bandwidth must be positive (>= 0.0005 GB/s)");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(KVPOOL_ECUDA, "create: no CUDA device (this library has no CPU fallback)");
+  }
+  if (cuda_device < 0 || cuda_device >= ndev) return fail(KVPOOL_EINVAL, "create: cuda_device %d out of range", cuda_device);
+  DeviceGuard guard(cuda_device);
+  CU(cudaFree(nullptr));
+  CU(kernels_init());
+
+  std::unique_ptr<kvpool> p(new kvpool);
+  p->cuda_device = cuda_device;
+  CU(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, cuda_device));
+  p->geom = *g;
+  p->kvb = kvb;
+  p->payload = 2 * kvb;
+  p->n = n_devs;
+  p->bandwidth = bw;
+  p->w = w;
+  default_tuning(p.get());
+  auto cleanup = [&]() {
+    for (auto& b : p->bufs) host_buffer_free(&b);
+    for (auto s : p->io) cudaStreamDestroy(s);
+    if (p->fork) cudaEventDestroy(p->fork);
+  };
+  p->bufs.resize(n_devs);
+  for (uint32_t i = 0; i < n_devs; ++i) {
+    std::string err;
+    const int rc = host_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes, devs[i].numa_node, devs[i].flags & KVPOOL_DEV_WRITE_COMBINED,
+                                     devs[i].flags & KVPOOL_DEV_NUMA_STRICT, &err);
+    if (rc != KVPOOL_OK) {
+      cleanup();
+      return fail(rc, "create: pool device %u (%llu bytes): %s", i, (unsigned long long)devs[i].capacity_bytes, err.c_str());
+    }
+    p->alloc.emplace_back(devs[i].capacity_bytes);
+  }
+  p->io.resize(n_devs, nullptr);
+  for (auto& s : p->io) {
+    cudaError_t e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { cleanup(); return fail(KVPOOL_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)); }
+  }
+  if (cudaEventCreateWithFlags(&p->fork, cudaEventDisableTiming) != cudaSuccess) { cleanup(); return fail(KVPOOL_ECUDA, "cudaEventCreate failed"); }
+  *out = p.release();
+  return KVPOOL_OK;
+}
+
+int kvpool_destroy(kvpool_t* p) {
+  if (!p) return fail(KVPOOL_EINVAL, "destroy: null pool");
+  DeviceGuard guard(p->cuda_device);
+  cudaDeviceSynchronize();
+  for (auto* pl : p->live) destroy_placement(p, pl);
+  p->live.clear();
+  free_slots(p);
+  for (auto s : p->io) cudaStreamDestroy(s);
+  for (auto& b : p->bufs) host_buffer_free(&b);
+  if (p->fork) cudaEventDestroy(p->fork);
+  delete p;
+  return KVPOOL_OK;
+}
+
+int kvpool_set_bandwidth(kvpool_t* p, const double* bw) {
+  if (!p || !bw) return fail(KVPOOL_EINVAL, "set_bandwidth: null argument");
+  if (!p->live.empty()) return fail(KVPOOL_ESTATE, "set_bandwidth: %zu placements are live", p->live.size());
+  std::vector<uint64_t> w(p->n);
+  if (!quantise_weights(bw, p->n, w.data())) return fail(KVPOOL_EINVAL, "set_bandwidth: bandwidth must be positive (>= 0.0005 GB/s)");
+  p->bandwidth.assign(bw, bw + p->n);
+  p->w = w;
+  return KVPOOL_OK;
+}
+
+int kvpool_measure_bandwidth(kvpool_t* p, uint32_t dev, int direction, uint64_t bytes, uint32_t iters, double* gbps_out) {
+  if (!p || !gbps_out || dev >= p->n || bytes == 0 || iters == 0 || (direction != 0 && direction != 1))
+    return fail(KVPOOL_EINVAL, "measure_bandwidth: bad arguments");
+  if (bytes > p->bufs[dev].bytes) return fail(KVPOOL_EINVAL, "measure_bandwidth: %llu bytes exceed the pool buffer", (unsigned long long)bytes);
+  if (!p->live.empty()) return fail(KVPOOL_ESTATE, "measure_bandwidth: %zu placements are live", p->live.size());
+  DeviceGuard guard(p->cuda_device);
+  void* scratch = nullptr;
+  CU(cudaMalloc(&scratch, bytes));
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  CU(cudaEventCreate(&e1));
+  std::vector<float> ms(iters);
+  cudaStream_t s = p->io[dev];
+  int rc = KVPOOL_OK;
+  for (uint32_t it = 0; it < iters + 1 && rc == KVPOOL_OK; ++it) {  // first pass is a warm-up
+    cudaEventRecord(e0, s);
+    cudaError_t e = direction == 0 ? cudaMemcpyAsync(scratch, p->bufs[dev].host, bytes, cudaMemcpyHostToDevice, s)
+                                   : cudaMemcpyAsync(p->bufs[dev].host, scratch, bytes, cudaMemcpyDeviceToHost, s);
+    cudaEventRecord(e1, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) { rc = fail(KVPOOL_ECUDA, "measure_bandwidth: %s", cudaGetErrorString(e)); break; }
+    p->n_memcpys++;
+    if (it > 0) cudaEventElapsedTime(&ms[it - 1], e0, e1);
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(scratch);
+  if (rc != KVPOOL_OK) return rc;
+  std::sort(ms.begin(), ms.end());
+  *gbps_out = static_cast<double>(bytes) / (ms[iters / 2] * 1.0e6);
+  return KVPOOL_OK;
+}
+
+int kvpool_set_path(kvpool_t* p, int path) {
+  if (!p || path < KVPOOL_PATH_AUTO || path > KVPOOL_PATH_ZEROCOPY) return fail(KVPOOL_EINVAL, "set_path: bad arguments");
+  p->path = path;
+  return KVPOOL_OK;
+}
+
+int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
+  if (!p || !t) return fail(KVPOOL_EINVAL, "set_tuning: null argument");
+  if (t->kernel > KVPOOL_KERNEL_BULK) return fail(KVPOOL_EINVAL, "set_tuning: unknown kernel %u", t->kernel);
+  if (t->bulk_chunk && (t->bulk_chunk < 1024 || t->bulk_chunk > 32768 || (t->bulk_chunk & (t->bulk_chunk - 1))))
+    return fail(KVPOOL_EINVAL, "set_tuning: bulk_chunk must be a power of two in 1 KiB..32 KiB");
+  if (t->bulk_stages > 8 || t->bulk_stages == 1) return fail(KVPOOL_EINVAL, "set_tuning: bulk_stages must be 2..8");
+  if (t->bulk_warps > 8) return fail(KVPOOL_EINVAL, "set_tuning: bulk_warps must be 1..8");
+  if (t->stage_slots > 64) return fail(KVPOOL_EINVAL, "set_tuning: stage_slots must be <= 64");
+  kvpool_tuning d = p->tune;
+  d.kernel = t->kernel;
+  if (t->hbm_ctas) d.hbm_ctas = t->hbm_ctas;
+  if (t->link_ctas) d.link_ctas = t->link_ctas;
+  if (t->bulk_chunk) d.bulk_chunk = t->bulk_chunk;
+  if (t->bulk_stages) d.bulk_stages = t->bulk_stages;
+  if (t->bulk_warps) d.bulk_warps = t->bulk_warps;
+  if (t->auto_threshold_bytes) d.auto_threshold_bytes = t->auto_threshold_bytes;
+  if (t->stage_slots && t->stage_slots != d.stage_slots) {
+    DeviceGuard guard(p->cuda_device);
+    d.stage_slots = t->stage_slots;
+    p->tune = d;
+    const uint64_t bytes = p->slot_bytes;
+    CU(cudaDeviceSynchronize());
+    free_slots(p);
+    if (bytes) return ensure_slots(p, bytes);
+    return KVPOOL_OK;
+  }
+  p->tune = d;
+  return KVPOOL_OK;
+}
+
+int kvpool_get_tuning(const kvpool_t* p, kvpool_tuning* t_out) {
+  if (!p || !t_out) return fail(KVPOOL_EINVAL, "get_tuning: null argument");
+  *t_out = p->tune;
+  return KVPOOL_OK;
+}
+
+int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement_t** out) {
+  if (!p || !blocks_per_layer || !out) return fail(KVPOOL_EINVAL, "place: null argument");
+  *out = nullptr;
+  std::lock_guard<std::mutex> lock(p->mu);
+  DeviceGuard guard(p->cuda_device);
+  const uint32_t L = p->geom.n_layers, N = p->n;
+  std::unique_ptr<kvpool_placement> pl(new kvpool_placement);
+  pl->pool = p;
+  pl->layers.resize(L);
+
+  // a1-a3: counts and weighted round-robin, once per distinct K (layers of equal size share their map)
+  std::unordered_map<uint64_t, std::shared_ptr<LayerMap>> by_k;
+  uint64_t table_bytes = 0, max_layer_bytes = 0;
+  for (uint32_t l = 0; l < L; ++l) {
+    const uint64_t K = blocks_per_layer[l];
+    auto it = by_k.find(K);
+    if (it == by_k.end()) {
+      auto m = std::make_shared<LayerMap>();
+      m->K = K;
+      m->counts.resize(N);
+      m->start.resize(N);
+      m->dev.resize(K);
+      m->slot.resize(K);
+      target_counts(p->w.data(), N, K, m->counts.data());
+      wrr_closed_form(m->counts.data(), N, K, m->dev.data(), m->slot.data());
+      uint32_t acc = 0;
+      for (uint32_t i = 0; i < N; ++i) { m->start[i] = acc; acc += m->counts[i]; }
+      table_bytes += (K * 5 + 255) / 256 * 256 + 256;
+      it = by_k.emplace(K, std::move(m)).first;
+    }
+    pl->layers[l].map = it->second;
+    max_layer_bytes = std::max(max_layer_bytes, K * p->payload);
+  }
+
+  // a4: stripe allocation, all or nothing
+  bool ok = true;
+  uint32_t fail_dev = 0, done_layers = 0;
+  for (uint32_t l = 0; l < L && ok; ++l) {
+    auto& Ls = pl->layers[l];
+    Ls.stripe_off.assign(N, 0);
+    uint32_t i = 0;
+    for (; i < N; ++i)
+      if (!p->alloc[i].alloc(static_cast<uint64_t>(Ls.map->counts[i]) * p->payload, &Ls.stripe_off[i])) break;
+    if (i < N) {
+      ok = false;
+      fail_dev = i;
+      for (uint32_t k = 0; k < i; ++k) p->alloc[k].free(Ls.stripe_off[k], static_cast<uint64_t>(Ls.map->counts[k]) * p->payload);
+    } else {
+      done_layers = l + 1;
+    }
+  }
+  auto rollback = [&]() {
+    for (uint32_t l = 0; l < done_layers; ++l)
+      for (uint32_t i = 0; i < N; ++i)
+        p->alloc[i].free(pl->layers[l].stripe_off[i], static_cast<uint64_t>(pl->layers[l].map->counts[i]) * p->payload);
+    if (pl->tables_d) cudaFree(pl->tables_d);
+    for (auto& Ls : pl->layers)
+      if (Ls.landed) cudaEventDestroy(Ls.landed);
+    if (pl->join) cudaEventDestroy(pl->join);
+  };
+  if (!ok) {
+    rollback();
+    return fail(KVPOOL_ENOMEM, "place: pool device %u is full (capacity %llu, used %llu)", fail_dev,
+                (unsigned long long)p->alloc[fail_dev].capacity(), (unsigned long long)p->alloc[fail_dev].used());
+  }
+
+  // GLT upload: dense (device_id, slot) columns, one device allocation per placement
+  if (table_bytes) {
+    cudaError_t e = cudaMalloc(&pl->tables_d, table_bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); rollback(); return fail(KVPOOL_ENOMEM, "place: table upload buffer: %s", cudaGetErrorString(e)); }
+    std::vector<uint8_t> host(table_bytes);
+    uint64_t off = 0;
+    for (auto& kv : by_k) {
+      LayerMap& m = *kv.second;
+      if (m.K == 0) continue;
+      m.slot_d = reinterpret_cast<const uint32_t*>(static_cast<uint8_t*>(pl->tables_d) + off);
+      memcpy(host.data() + off, m.slot.data(), m.K * 4);
+      off += (m.K * 4 + 255) / 256 * 256;
+      m.dev_d = static_cast<const uint8_t*>(pl->tables_d) + off;
+      memcpy(host.data() + off, m.dev.data(), m.K);
+      off += (m.K + 255) / 256 * 256;
+    }
+    e = cudaMemcpy(pl->tables_d, host.data(), off, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: table upload: %s", cudaGetErrorString(e)); }
+  }
+  for (auto& Ls : pl->layers) {
+    cudaError_t e = cudaEventCreateWithFlags(&Ls.landed, cudaEventDisableTiming);
+    if (e != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: cudaEventCreate: %s", cudaGetErrorString(e)); }
+  }
+  if (cudaEventCreateWithFlags(&pl->join, cudaEventDisableTiming) != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: cudaEventCreate failed"); }
+  if (p->path != KVPOOL_PATH_ZEROCOPY) {
+    const int rc = ensure_slots(p, max_layer_bytes);
+    if (rc != KVPOOL_OK) { rollback(); return rc; }
+  }
+  p->live.push_back(pl.get());
+  *out = pl.release();
+  return KVPOOL_OK;
+}
+
+int kvpool_release(kvpool_t* p, kvpool_placement_t* pl) {
+  if (!p || !pl) return fail(KVPOOL_EINVAL, "release: null argument");
+  std::lock_guard<std::mutex> lock(p->mu);
+  auto it = std::find(p->live.begin(), p->live.end(), pl);
+  if (it == p->live.end()) return fail(KVPOOL_EINVAL, "release: placement does not belong to this pool");
+  DeviceGuard guard(p->cuda_device);
+  const int rc = sync_pool_streams(p);  // the library's own transfers for it must be over
+  if (rc != KVPOOL_OK) return rc;
+  p->live.erase(it);
+  destroy_placement(p, pl);
+  return KVPOOL_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------
+// hot path
+// ---------------------------------------------------------------------------------------------------
+extern "C" {
+
+int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
+                   const int32_t* table, void* cuda_stream) {
+  int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
+  if (rc != KVPOOL_OK) return rc;
+  LayerState& L = pl->layers[layer];
+  L.offloaded = true;
+  if (L.map->K == 0) return KVPOOL_OK;
+  DeviceGuard guard(p->cuda_device);
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const uint32_t N = p->n;
+  LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
+
+  if (!use_staged(p, L)) {
+    // zero-copy: one kernel gathers the paged blocks and stores them straight into the mapped host stripes
+    for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
+    if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));  // an earlier staged offload of this layer still in flight
+    CU(launch_layer_copy(a, true, launch_cfg(p, true), s));
+    p->n_kernels++;
+    CU(cudaEventRecord(L.landed, s));
+    L.landed_pending = true;
+    return KVPOOL_OK;
+  }
+
+  // staged: pack kernel -> device staging slot (stripe order), then one D2H copy per stripe on the
+  // per-device I/O streams; `stream` is released as soon as the pack is enqueued.
+  StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
+  rc = wait_slot_free(p, slot, s);
+  if (rc != KVPOOL_OK) return rc;
+  for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload);
+  CU(launch_layer_copy(a, true, launch_cfg(p, false), s));
+  p->n_kernels++;
+  CU(cudaEventRecord(slot.kernel_done, s));
+  for (uint32_t i = 0; i < N; ++i) {
+    const uint64_t bytes = static_cast<uint64_t>(L.map->counts[i]) * p->payload;
+    if (bytes == 0) continue;
+    CU(cudaStreamWaitEvent(p->io[i], slot.kernel_done, 0));
+    if (L.landed_pending) CU(cudaStreamWaitEvent(p->io[i], L.landed, 0));
+    CU(cudaMemcpyAsync(static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i], slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload,
+                       bytes, cudaMemcpyDeviceToHost, p->io[i]));
+    p->n_memcpys++;
+    CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+  }
+  // `landed` must mean "all stripes done": record it on a stream that has waited for every copy
+  {
+    cudaStream_t js = nullptr;
+    for (uint32_t i = 0; i < N; ++i) {
+      if (static_cast<uint64_t>(L.map->counts[i]) == 0) continue;
+      if (!js) { js = p->io[i]; continue; }
+      CU(cudaStreamWaitEvent(js, slot.copy_done[i], 0));
+    }
+    if (js) {
+      CU(cudaEventRecord(L.landed, js));
+      L.landed_pending = true;
+    }
+  }
+  return KVPOOL_OK;
+}
+
+int kvpool_retrieve(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
+                    const int32_t* table, void* cuda_stream) {
+  int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
+  if (rc != KVPOOL_OK) return rc;
+  LayerState& L = pl->layers[layer];
+  if (!L.offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", layer);
+  if (L.map->K == 0) return KVPOOL_OK;
+  DeviceGuard guard(p->cuda_device);
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const uint32_t N = p->n;
+  LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
+
+  if (!use_staged(p, L)) {
+    for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
+    if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
+    CU(launch_layer_copy(a, false, launch_cfg(p, true), s));
+    p->n_kernels++;
+    return KVPOOL_OK;
+  }
+
+  // staged: one H2D copy per stripe on the per-device I/O streams (these may run ahead of `stream`),
+  // then the unpack kernel on `stream` once all of them have landed in the staging slot.
+  StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
+  for (uint32_t i = 0; i < N; ++i) {
+    const uint64_t bytes = static_cast<uint64_t>(L.map->counts[i]) * p->payload;
+    if (bytes == 0) continue;
+    rc = wait_slot_free(p, slot, p->io[i]);
+    if (rc != KVPOOL_OK) return rc;
+    if (L.landed_pending) CU(cudaStreamWaitEvent(p->io[i], L.landed, 0));
+  }
+  for (uint32_t i = 0; i < N; ++i) {
+    const uint64_t bytes = static_cast<uint64_t>(L.map->counts[i]) * p->payload;
+    if (bytes == 0) continue;
+    CU(cudaMemcpyAsync(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload, static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i],
+                       bytes, cudaMemcpyHostToDevice, p->io[i]));
+    p->n_memcpys++;
+    CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+    CU(cudaStreamWaitEvent(s, slot.copy_done[i], 0));
+    a.pool_base[i] = reinterpret_cast<uint64_t>(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload);
+  }
+  CU(launch_layer_copy(a, false, launch_cfg(p, false), s));
+  p->n_kernels++;
+  CU(cudaEventRecord(slot.kernel_done, s));
+  return KVPOOL_OK;
+}
+
+int kvpool_wait_offloads(kvpool_t* p, kvpool_placement_t* pl, void* cuda_stream) {
+  if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "wait_offloads: bad arguments");
+  DeviceGuard guard(p->cuda_device);
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  for (auto& L : pl->layers)
+    if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
+  return KVPOOL_OK;
+}
+
+int kvpool_synchronize(kvpool_t* p) {
+  if (!p) return fail(KVPOOL_EINVAL, "synchronize: null pool");
+  DeviceGuard guard(p->cuda_device);
+  return sync_pool_streams(p);
+}
+
+int kvpool_pack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
+                const int32_t* table, void* stage_dev, void* cuda_stream) {
+  int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
+  if (rc != KVPOOL_OK) return rc;
+  LayerState& L = pl->layers[layer];
+  if (L.map->K == 0) return KVPOOL_OK;
+  if (!stage_dev || (reinterpret_cast<uintptr_t>(stage_dev) & 15u)) return fail(KVPOOL_EINVAL, "pack: stage_dev must be a 16-byte aligned device pointer");
+  DeviceGuard guard(p->cuda_device);
+  LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
+  for (uint32_t i = 0; i < p->n; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(stage_dev) + static_cast<uint64_t>(L.map->start[i]) * p->payload);
+  CU(launch_layer_copy(a, true, launch_cfg(p, false), static_cast<cudaStream_t>(cuda_stream)));
+  p->n_kernels++;
+  return KVPOOL_OK;
+}
+
+int kvpool_unpack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
+                  const int32_t* table, const void* stage_dev, void* cuda_stream) {
+  int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
+  if (rc != KVPOOL_OK) return rc;
+  LayerState& L = pl->layers[layer];
+  if (L.map->K == 0) return KVPOOL_OK;
+  if (!stage_dev || (reinterpret_cast<uintptr_t>(stage_dev) & 15u)) return fail(KVPOOL_EINVAL, "unpack: stage_dev must be a 16-byte aligned device pointer");
+  DeviceGuard guard(p->cuda_device);
+  LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
+  for (uint32_t i = 0; i < p->n; ++i)
+    a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(const_cast<void*>(stage_dev)) + static_cast<uint64_t>(L.map->start[i]) * p->payload);
+  CU(launch_layer_copy(a, false, launch_cfg(p, false), static_cast<cudaStream_t>(cuda_stream)));
+  p->n_kernels++;
+  return KVPOOL_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// introspection
+// ---------------------------------------------------------------------------------------------------
+int kvpool_n_devices(const kvpool_t* p, uint32_t* n_out) {
+  if (!p || !n_out) return fail(KVPOOL_EINVAL, "n_devices: null argument");
+  *n_out = p->n;
+  return KVPOOL_OK;
+}
+
+int kvpool_weights(const kvpool_t* p, uint64_t* w_out) {
+  if (!p || !w_out) return fail(KVPOOL_EINVAL, "weights: null argument");
+  std::copy(p->w.begin(), p->w.end(), w_out);
+  return KVPOOL_OK;
+}
+
+int kvpool_device_info(const kvpool_t* p, uint32_t dev, void** host_base, uint64_t* capacity, uint64_t* used, int32_t* numa_actual) {
+  if (!p || dev >= p->n) return fail(KVPOOL_EINVAL, "device_info: bad arguments");
+  if (host_base) *host_base = p->bufs[dev].host;
+  if (capacity) *capacity = p->bufs[dev].bytes;
+  if (used) *used = p->alloc[dev].used();
+  if (numa_actual) *numa_actual = p->bufs[dev].numa_actual;
+  return KVPOOL_OK;
+}
+
+int kvpool_counts(const kvpool_placement_t* pl, uint32_t layer, uint32_t* counts_out) {
+  if (!pl || !counts_out || layer >= pl->layers.size()) return fail(KVPOOL_EINVAL, "counts: bad arguments");
+  const auto& c = pl->layers[layer].map->counts;
+  std::copy(c.begin(), c.end(), counts_out);
+  return KVPOOL_OK;
+}
+
+int kvpool_lookup(const kvpool_placement_t* pl, uint32_t layer, uint32_t block, uint32_t* device_id, uint32_t* type, uint32_t* slot,
+                  void** host_ptr) {
+  if (!pl || layer >= pl->layers.size()) return fail(KVPOOL_EINVAL, "lookup: bad arguments");
+  const LayerState& L = pl->layers[layer];
+  if (block >= L.map->K) return fail(KVPOOL_EINVAL, "lookup: block %u out of range (K %llu)", block, (unsigned long long)L.map->K);
+  const uint32_t d = L.map->dev[block], s = L.map->slot[block];
+  if (device_id) *device_id = d;
+  if (type) *type = 0;
+  if (slot) *slot = s;
+  if (host_ptr) *host_ptr = static_cast<uint8_t*>(pl->pool->bufs[d].host) + L.stripe_off[d] + static_cast<uint64_t>(s) * pl->pool->payload;
+  return KVPOOL_OK;
+}
+
+int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, void** host_ptr, uint64_t* nbytes) {
+  if (!pl || layer >= pl->layers.size() || dev >= pl->pool->n) return fail(KVPOOL_EINVAL, "stripe: bad arguments");
+  const LayerState& L = pl->layers[layer];
+  const uint64_t bytes = static_cast<uint64_t>(L.map->counts[dev]) * pl->pool->payload;
+  if (host_ptr) *host_ptr = bytes ? static_cast<uint8_t*>(pl->pool->bufs[dev].host) + L.stripe_off[dev] : nullptr;
+  if (nbytes) *nbytes = bytes;
+  return KVPOOL_OK;
+}
+
+int kvpool_layer_map(const kvpool_placement_t* pl, uint32_t layer, uint8_t* dev_out, uint32_t* slot_out) {
+  if (!pl || layer >= pl->layers.size()) return fail(KVPOOL_EINVAL, "layer_map: bad arguments");
+  const LayerMap& m = *pl->layers[layer].map;
+  if (dev_out) std::copy(m.dev.begin(), m.dev.end(), dev_out);
+  if (slot_out) std::copy(m.slot.begin(), m.slot.end(), slot_out);
+  return KVPOOL_OK;
+}
+
+int kvpool_stats(const kvpool_t* p, uint64_t* kernel_launches, uint64_t* memcpy_calls) {
+  if (!p) return fail(KVPOOL_EINVAL, "stats: null pool");
+  if (kernel_launches) *kernel_launches = p->n_kernels;
+  if (memcpy_calls) *memcpy_calls = p->n_memcpys;
+  return KVPOOL_OK;
+}
+
+}  // extern "C"

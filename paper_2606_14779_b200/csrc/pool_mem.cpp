@@ -1,0 +1,96 @@
+// Pinned, GPU-mapped, optionally NUMA-bound host buffers.  libnuma is not in the image, so binding
+// uses the raw mbind / move_pages syscalls and /sys/devices/system/node.
+#include "pool_mem.hpp"
+
+#include <cuda_runtime.h>
+#include <dirent.h>
+#include <errno.h>
+#include <string.h>
+#include <sys/mman.h>
+#include <sys/syscall.h>
+#include <unistd.h>
+
+#include "../../include/kvpool.h"
+
+namespace kvp {
+
+int numa_node_count() {
+  int n = 0;
+  if (DIR* d = opendir("/sys/devices/system/node")) {
+    while (dirent* e = readdir(d))
+      if (strncmp(e->d_name, "node", 4) == 0 && e->d_name[4] >= '0' && e->d_name[4] <= '9') ++n;
+    closedir(d);
+  }
+  return n > 0 ? n : 1;
+}
+
+static int query_node(void* page) {
+  int status = -1;
+  void* pages[1] = {page};
+  if (syscall(SYS_move_pages, 0, 1ul, pages, nullptr, &status, 0) != 0) return -1;
+  return status >= 0 ? status : -1;
+}
+
+int host_buffer_alloc(HostBuffer* hb, uint64_t bytes, int numa_node, bool write_combined, bool strict_numa, std::string* err) {
+  *hb = HostBuffer{};
+  hb->bytes = bytes;
+  hb->numa_requested = numa_node;
+  bool want_bind = numa_node >= 0;
+  if (want_bind && numa_node >= numa_node_count()) {
+    if (strict_numa) { *err = "NUMA node " + std::to_string(numa_node) + " does not exist"; return KVPOOL_ENUMA; }
+    want_bind = false;  // fall back to first-touch placement; numa_actual reports where the pages landed
+  }
+  if (want_bind && !write_combined) {
+    void* m = mmap(nullptr, bytes, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS, -1, 0);
+    if (m == MAP_FAILED) { *err = std::string("mmap: ") + strerror(errno); return KVPOOL_ENOMEM; }
+    unsigned long mask[16] = {0};
+    mask[numa_node / 64] = 1ul << (numa_node % 64);
+    const long rc = syscall(SYS_mbind, m, bytes, 2 /*MPOL_BIND*/, mask, sizeof(mask) * 8, 0);
+    if (rc != 0 && strict_numa) {
+      *err = std::string("mbind: ") + strerror(errno);
+      munmap(m, bytes);
+      return KVPOOL_ENUMA;
+    }
+    // touch one byte per page so the pages exist on the bound node before they are pinned
+    volatile char* p = static_cast<volatile char*>(m);
+    for (uint64_t off = 0; off < bytes; off += 4096) p[off] = 0;
+    const cudaError_t e = cudaHostRegister(m, bytes, cudaHostRegisterMapped | cudaHostRegisterPortable);
+    if (e != cudaSuccess) {
+      *err = std::string("cudaHostRegister: ") + cudaGetErrorString(e);
+      munmap(m, bytes);
+      return e == cudaErrorMemoryAllocation ? KVPOOL_ENOMEM : KVPOOL_ECUDA;
+    }
+    hb->host = m;
+    hb->registered = true;
+  } else {
+    unsigned flags = cudaHostAllocMapped | cudaHostAllocPortable | (write_combined ? cudaHostAllocWriteCombined : 0);
+    void* m = nullptr;
+    const cudaError_t e = cudaHostAlloc(&m, bytes, flags);
+    if (e != cudaSuccess) {
+      *err = std::string("cudaHostAlloc: ") + cudaGetErrorString(e);
+      return e == cudaErrorMemoryAllocation ? KVPOOL_ENOMEM : KVPOOL_ECUDA;
+    }
+    hb->host = m;
+  }
+  const cudaError_t e = cudaHostGetDevicePointer(&hb->dev_alias, hb->host, 0);
+  if (e != cudaSuccess) {
+    *err = std::string("cudaHostGetDevicePointer: ") + cudaGetErrorString(e);
+    host_buffer_free(hb);
+    return KVPOOL_ECUDA;
+  }
+  hb->numa_actual = write_combined ? -1 : query_node(hb->host);
+  return KVPOOL_OK;
+}
+
+void host_buffer_free(HostBuffer* hb) {
+  if (!hb->host) return;
+  if (hb->registered) {
+    cudaHostUnregister(hb->host);
+    munmap(hb->host, hb->bytes);
+  } else {
+    cudaFreeHost(hb->host);
+  }
+  *hb = HostBuffer{};
+}
+
+}  // namespace kvp

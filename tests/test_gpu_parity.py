@@ -1,0 +1,190 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the CPU oracle on the same seeded inputs.
+Bit-exact on placement (counts, dev[], slot[]), on every stripe byte after offload and on the whole paged
+tensor after retrieve into a poison-filled pool (tolerance: none — integer and byte work only)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_14779_b200 import binding as kv
+from paper_2606_14779_b200 import build as kvbuild
+from paper_2606_14779_b200 import workloads as W
+
+from parity_util import check_placement, make_pool, run_parity
+
+pytestmark = pytest.mark.gpu
+
+PATHS = {"staged": kv.PATH_STAGED, "zerocopy": kv.PATH_ZEROCOPY, "auto": kv.PATH_AUTO}
+KERNELS = {"vec16": kv.KERNEL_VEC16, "bulk": kv.KERNEL_BULK}
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    kvbuild.build()
+    assert torch.cuda.is_available()
+    kv.lib()                                    # raises if libkvpool.so is missing: no fallback
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+@pytest.mark.parametrize("path", ["staged", "zerocopy"])
+def test_config1_llama_1k_all_paths(path, kernel):
+    wl = W.make_workload(1)                     # the full config: 32 layers x 64 blocks, 2 buffers 2:1
+    out = run_parity(wl, path=PATHS[path], kernel=KERNELS[kernel])
+    assert out["bytes_compared"] == 128 << 20
+    assert out["kernels"] == 64 and out["memcpys"] == (128 if path == "staged" else 0)
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_config2_llama_32k_measured_weights(kernel):
+    wl = W.make_workload(2, n_layers=3)         # full 32K context (2048 of 4096 blocks), 4 buffers
+    probe = make_pool(wl)
+    try:                                        # weights = measured per-buffer H2D bandwidth (R10)
+        bw = [probe.measure_bandwidth(i, 0, 64 << 20, 3) for i in range(4)]
+    finally:
+        probe.destroy()
+    assert all(b > 1.0 for b in bw)
+    run_parity(wl, path=kv.PATH_STAGED, kernel=KERNELS[kernel], bandwidth=bw)
+    run_parity(wl, path=kv.PATH_ZEROCOPY, kernel=KERNELS[kernel], bandwidth=bw)
+
+
+@pytest.mark.parametrize("path", ["staged", "zerocopy", "auto"])
+def test_config3_gptoss_sliding_window_layers(path):
+    wl = W.make_workload(3, scale=1 / 8, n_layers=6)     # 1024 blocks; even layers move only the last 8
+    assert list(wl.blocks_per_layer(0)) == [8, 1024, 8, 1024, 8, 1024]
+    run_parity(wl, path=PATHS[path], kernel=kv.KERNEL_VEC16)
+    run_parity(wl, path=PATHS[path], kernel=kv.KERNEL_BULK)
+
+
+@pytest.mark.parametrize("path", ["staged", "zerocopy"])
+def test_config4_qwen3_heterogeneous_weights(path):
+    wl = W.make_workload(4, scale=1 / 8, n_layers=4)     # 1024 of 1536 blocks, 6 buffers 4:4:2:2:1:1
+    run_parity(wl, path=PATHS[path], kernel=kv.KERNEL_VEC16)
+    run_parity(wl, path=PATHS[path], kernel=kv.KERNEL_BULK)
+
+
+@pytest.mark.parametrize("path", ["staged", "zerocopy"])
+def test_config5_four_requests_four_streams_retained_prefix(path):
+    wl = W.make_workload(5, scale=1 / 16, n_layers=3)    # 128..512 blocks, 25% prefix kept, 8 buffers
+    run_parity(wl, path=PATHS[path], kernel=kv.KERNEL_VEC16, streams=4)
+    run_parity(wl, path=PATHS[path], kernel=kv.KERNEL_BULK, streams=4, tuning={"stage_slots": 2})
+
+
+def _custom(geom, nphys, tables, n_dev, weights, cfg=77):
+    return W.Workload(cfg, "custom", geom, (0,), nphys, [W.Request(np.asarray(t, dtype=np.int32)) for t in tables], n_dev, weights)
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+@pytest.mark.parametrize("path", ["staged", "zerocopy"])
+def test_edge_cases_ragged_blocks_small_k_and_layouts(path, kernel):
+    rng = np.random.default_rng(5)
+    # ragged block size: 16 tokens x 1 head x 80 dims x 2 B = 2560 B (not a multiple of the 4 KiB warp piece)
+    g = W.Geometry(n_layers=2, n_kv_heads=1, head_dim=80)
+    run_parity(_custom(g, 301, [rng.permutation(301)[:257]], 3, (3.0, 2.0, 1.0)), path=PATHS[path], kernel=KERNELS[kernel])
+    # 12 KiB + ragged tail: 16 x 3 x 136 x 2 = 13056 B
+    g = W.Geometry(n_layers=1, n_kv_heads=3, head_dim=136)
+    run_parity(_custom(g, 97, [rng.permutation(97)[:61]], 5, (5.0, 1.0, 1.0, 3.0, 2.0)), path=PATHS[path], kernel=KERNELS[kernel])
+    # smallest legal block (16 B), K < N, one device left empty
+    g = W.Geometry(n_layers=1, n_kv_heads=1, head_dim=8, block_tokens=1)
+    run_parity(_custom(g, 9, [[7, 2, 5]], 6, (4.0, 4.0, 2.0, 2.0, 1.0, 1.0)), path=PATHS[path], kernel=KERNELS[kernel])
+    # one block, one device; identity table over the whole pool; [nphys, 2, ...] layout
+    g = W.Geometry(n_layers=1, n_kv_heads=2, head_dim=64)
+    run_parity(_custom(g, 4, [[3]], 1, (1.0,)), path=PATHS[path], kernel=KERNELS[kernel])
+    run_parity(_custom(g, 128, [np.arange(128)], 2, (1.0, 1.0)), path=PATHS[path], kernel=KERNELS[kernel])
+    run_parity(_custom(g, 200, [rng.permutation(200)[:150]], 4, (9.0, 1.0, 1.0, 1.0)), path=PATHS[path], kernel=KERNELS[kernel],
+               interleaved_layout=True)
+    # the maximum number of pool devices
+    run_parity(_custom(g, 700, [rng.permutation(700)[:555]], 32, tuple(float(1 + (i * 7) % 5) for i in range(32))),
+               path=PATHS[path], kernel=KERNELS[kernel])
+
+
+def test_empty_layers_and_state_errors():
+    g = W.Geometry(n_layers=3, n_kv_heads=2, head_dim=64)
+    wl = _custom(g, 16, [np.arange(16)], 2, (2.0, 1.0))
+    pool = make_pool(wl)
+    try:
+        pl = pool.place([0, 5, 0])
+        opl = oracle.place([2.0, 1.0], [0, 5, 0])
+        check_placement(pl, opl)
+        kvt = W.kv_layer_torch(wl, 1, "cuda:0")
+        table = torch.arange(5, dtype=torch.int32, device="cuda:0")
+        pool.offload(pl, 0, None, None, g.kvb, None)                        # K_l = 0: no-op, null pointers fine
+        pool.retrieve(pl, 0, None, None, g.kvb, None)
+        with pytest.raises(kv.KvPoolError) as e:                            # never offloaded
+            pool.retrieve(pl, 1, kvt[0], kvt[1], g.kvb, table)
+        assert e.value.code == kv.ESTATE
+        with pytest.raises(kv.KvPoolError) as e:                            # misaligned base
+            pool.offload(pl, 1, kvt[0].data_ptr() + 2, kvt[1], g.kvb, table)
+        assert e.value.code == kv.EINVAL
+        with pytest.raises(kv.KvPoolError) as e:                            # stride not a multiple of 16
+            pool.offload(pl, 1, kvt[0], kvt[1], g.kvb + 8, table)
+        assert e.value.code == kv.EINVAL
+        with pytest.raises(kv.KvPoolError) as e:                            # layer out of range
+            pool.offload(pl, 3, kvt[0], kvt[1], g.kvb, table)
+        assert e.value.code == kv.EINVAL
+        with pytest.raises(kv.KvPoolError) as e:                            # weights are frozen while placements live
+            pool.set_bandwidth([1.0, 1.0])
+        assert e.value.code == kv.ESTATE
+        pl.release()
+        pool.set_bandwidth([1.0, 1.0])
+        assert list(pool.weights()) == [1000, 1000]
+    finally:
+        pool.destroy()
+
+
+def test_pool_full_is_enomem_with_no_partial_reservation():
+    g = W.Geometry(n_layers=4, n_kv_heads=2, head_dim=64)
+    pool = kv.KvPool([1.0, 1.0], [64 * g.payload, 64 * g.payload], n_layers=4, n_kv_heads=2, head_dim=64)
+    try:
+        a = pool.place([32, 32, 32, 32])                                    # 16 blocks per layer per device: fits exactly
+        assert [pool.device_info(i)["used"] for i in range(2)] == [64 * g.payload] * 2
+        with pytest.raises(kv.KvPoolError) as e:
+            pool.place([2, 0, 0, 0])
+        assert e.value.code == kv.ENOMEM
+        assert [pool.device_info(i)["used"] for i in range(2)] == [64 * g.payload] * 2
+        a.release()
+        with pytest.raises(kv.KvPoolError) as e:                            # layer 3 does not fit: layers 0-2 rolled back
+            pool.place([40, 40, 40, 40])
+        assert e.value.code == kv.ENOMEM
+        assert [pool.device_info(i)["used"] for i in range(2)] == [0, 0]
+        b = pool.place([128, 0, 0, 0])                                      # freed space coalesced back into one range
+        b.release()
+    finally:
+        pool.destroy()
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_pack_unpack_in_device_stripe_order(kernel):
+    """a5 / a8 alone: the staging buffer is the N stripes concatenated in device order."""
+    wl = W.make_workload(4, scale=1 / 16, n_layers=2)
+    g = wl.geom
+    bw = list(wl.default_weights())
+    pool = make_pool(wl)
+    try:
+        pool.set_tuning(kernel=KERNELS[kernel])
+        pl = pool.place(wl.blocks_per_layer(0))
+        opl = oracle.place(bw, wl.blocks_per_layer(0))
+        for l in range(g.n_layers):
+            table_np = wl.layer_table(0, l)
+            table = torch.from_numpy(np.ascontiguousarray(table_np)).cuda()
+            src = W.kv_layer_torch(wl, l, "cuda:0")
+            stage = torch.zeros(len(table_np) * g.payload, dtype=torch.uint8, device="cuda:0")
+            pool.pack(pl, l, src[0], src[1], g.kvb, table, stage)
+            torch.cuda.synchronize()
+            want = np.concatenate(oracle.offload_layer(W.kv_layer_numpy(wl, l), table_np, opl[l]))
+            assert np.array_equal(stage.cpu().numpy(), want)
+            dst = W.poison_torch((2, wl.nphys, g.kvb // 2), "cuda:0")
+            pool.unpack(pl, l, dst[0], dst[1], g.kvb, table, stage)
+            torch.cuda.synchronize()
+            ref = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+            oracle.retrieve_layer(ref, table_np, opl[l], oracle.offload_layer(W.kv_layer_numpy(wl, l), table_np, opl[l]))
+            assert np.array_equal(dst.cpu().numpy().view(np.uint16), ref)
+    finally:
+        pool.destroy()
+
+
+def test_kv_stream_is_identical_on_cpu_and_gpu():
+    wl = W.make_workload(2, n_layers=1)
+    a = W.kv_layer_torch(wl, 0, "cuda:0").cpu().numpy().view(np.uint16)
+    rng = np.random.default_rng(3)
+    for plane, phys in [(0, 0), (1, wl.nphys - 1)] + [(int(rng.integers(0, 2)), int(rng.integers(0, wl.nphys))) for _ in range(32)]:
+        assert np.array_equal(a[plane, phys], W.kv_block_numpy(wl, 0, plane, phys))

@@ -1,0 +1,124 @@
+"""CPU-only checks of the product's host side: the C-ABI library loads and exports every symbol the header
+declares, the pure-host placement entry points agree bit-for-bit with the oracle, and argument errors come back
+as codes.  No kernel runs here."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_14779_b200 import binding as kv
+from paper_2606_14779_b200 import build as kvbuild
+from paper_2606_14779_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    kvbuild.build()
+
+
+def test_library_exports_every_symbol_declared_in_header():
+    header = open(os.path.join(ROOT, "include", "kvpool.h")).read()
+    declared = sorted(set(re.findall(r"KVPOOL_API\s+(?:const\s+char\*|int)\s+(kvpool_\w+)\s*\(", header)))
+    assert len(declared) >= 27 and "kvpool_create" in declared and "kvpool_retrieve" in declared
+    lib = ctypes.CDLL(kv.LIB_PATH)
+    for name in declared:
+        assert hasattr(lib, name), f"{name} declared in kvpool.h but not exported"
+    assert sorted(kv.EXPORTS) == declared                      # the Python binding mirrors the header one to one
+    assert kv.version().startswith("kvpool")
+
+
+def _cases(seed, n_cases, max_n=8, max_k=3000, max_w=60000):
+    rng = np.random.default_rng(seed)
+    for _ in range(n_cases):
+        n = int(rng.integers(1, max_n + 1))
+        w = rng.integers(1, max_w + 1, size=n)
+        if rng.random() < 0.3:
+            w[rng.integers(0, n, size=n // 2 + 1)] = w[0]
+        yield [int(x) for x in w], int(rng.integers(0, max_k + 1))
+
+
+def test_plan_layer_matches_oracle_bit_for_bit():
+    for w, K in _cases(21, 1500):
+        c, dev, slot = kv.kvpool_plan_layer(w, K)
+        oc = oracle.counts(w, K)
+        od, os_ = oracle.wrr(oc, K)
+        assert np.array_equal(c, oc)
+        assert np.array_equal(dev.astype(np.uint32), od) and np.array_equal(slot, os_)
+    # many devices, large K, extreme weight ratios
+    for w, K in _cases(22, 40, max_n=32, max_k=40000, max_w=10 ** 9):
+        c, dev, slot = kv.kvpool_plan_layer(w, K)
+        oc = oracle.counts(w, K)
+        od, os_ = oracle.wrr(oc, K)
+        assert np.array_equal(c, oc) and np.array_equal(dev.astype(np.uint32), od) and np.array_equal(slot, os_)
+
+
+def test_plan_matches_oracle_on_all_baseline_configs():
+    for cfg in (1, 2, 3, 4, 5, 6):
+        wl = W.make_workload(cfg)
+        bw = wl.default_weights()
+        w = kv.kvpool_plan_weights(bw)
+        assert np.array_equal(w, oracle.weights(bw))
+        for r in range(len(wl.requests)):
+            for K in sorted(set(int(k) for k in wl.blocks_per_layer(r))):
+                c, dev, slot = kv.kvpool_plan_layer(w, K)
+                oc = oracle.counts(w, K)
+                od, os_ = oracle.wrr(oc, K)
+                assert np.array_equal(c, oc) and np.array_equal(dev.astype(np.uint32), od) and np.array_equal(slot, os_)
+    c = kv.kvpool_plan_layer(kv.kvpool_plan_weights((4, 4, 2, 2, 1, 1)), 8192, with_map=False)
+    assert list(c) == [2341, 2341, 1170, 1170, 585, 585]
+
+
+def test_plan_weights_quantisation_and_errors():
+    b = [55.62, 57.26, 21.3, 0.001, 12.3456]
+    assert np.array_equal(kv.kvpool_plan_weights(b), oracle.weights(b))
+    for bad in ([1.0, 0.0], [-1.0], [0.0004], [float("nan")], [float("inf")], []):
+        with pytest.raises(kv.KvPoolError) as e:
+            kv.kvpool_plan_weights(bad)
+        assert e.value.code == kv.EINVAL
+    with pytest.raises(kv.KvPoolError):
+        kv.kvpool_plan_weights([1.0] * 33)                     # more than KVPOOL_MAX_DEVICES
+    with pytest.raises(kv.KvPoolError):
+        kv.kvpool_plan_layer([1, 0, 1], 5)                     # zero weight
+
+
+def test_create_without_gpu_fails_loudly_with_ecuda():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(kv.KvPoolError) as e:
+        kv.KvPool([1.0], [1 << 20], n_layers=1, n_kv_heads=1, head_dim=64)
+    assert e.value.code == kv.ECUDA and "no CPU fallback" in str(e.value)
+
+
+def test_create_argument_validation_precedes_cuda():
+    for kwargs in (dict(n_layers=0, n_kv_heads=1, head_dim=64), dict(n_layers=1, n_kv_heads=1, head_dim=3, elem_bytes=1, block_tokens=1)):
+        with pytest.raises(kv.KvPoolError) as e:
+            kv.KvPool([1.0], [1 << 20], **kwargs)
+        assert e.value.code == kv.EINVAL
+    with pytest.raises(kv.KvPoolError) as e:
+        kv.KvPool([1.0, -2.0], [1 << 20, 1 << 20], n_layers=1, n_kv_heads=1, head_dim=64)
+    assert e.value.code == kv.EINVAL
+    with pytest.raises(kv.KvPoolError) as e:
+        kv.KvPool([1.0], [0], n_layers=1, n_kv_heads=1, head_dim=64)
+    assert e.value.code == kv.EINVAL
+
+
+def test_product_does_not_import_oracle_and_oracle_does_not_import_product():
+    pkg = os.path.join(ROOT, "paper_2606_14779_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cpp", ".hpp", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", src, re.M), f
+                assert "kvpool_oracle" not in src and "liboracle" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_2606_14779_b200" not in src.replace("paper_2606_14779_b200/", "") or f == "__init__.py"
+            assert not re.search(r"^\s*(from|import)\s+paper_2606_14779_b200", src, re.M), f
+            assert "kvpool.h" not in src, f
