@@ -84,6 +84,8 @@ typedef struct {         /* kvpool_set_tuning; 0 in any field = library default 
   uint32_t bulk_stages;  /* ring depth per issuing warp                                                 */
   uint32_t bulk_warps;   /* issuing warps per CTA                                                       */
   uint32_t stage_slots;  /* staging buffers in the ring of the staged path (default 4)                   */
+  uint32_t vec_threads;  /* threads per CTA of the vec16 kernel (multiple of 32, 64..512)                */
+  uint32_t vec_unroll;   /* 16-byte loads in flight per lane in the vec16 kernel: 4, 8 or 16             */
   uint64_t auto_threshold_bytes; /* PATH_AUTO: layers moving fewer bytes than this go zero-copy          */
 } kvpool_tuning;
 
@@ -175,6 +177,14 @@ KVPOOL_API int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint3
 KVPOOL_API int kvpool_layer_map(const kvpool_placement_t* pl, uint32_t layer, uint8_t* dev_out, uint32_t* slot_out);
 /* Work counters since create: kernels launched and cudaMemcpyAsync calls issued by the library.        */
 KVPOOL_API int kvpool_stats(const kvpool_t* pool, uint64_t* kernel_launches, uint64_t* memcpy_calls);
+
+/* Per-kernel timing for the roofline report.  While enabled, every kernel the library launches is bracketed by a
+ * CUDA event pair recorded on the launching stream after all of the launch's stream waits (so a pair spans the
+ * kernel alone, not the transfers it waited for).  kvpool_profile_read blocks until the recorded pairs of `kind`
+ * have completed, returns their summed duration, count and algorithmic bytes (K_l*P per launch), and clears them.
+ * kind: 0 = in-device pack, 1 = in-device unpack, 2 = zero-copy offload, 3 = zero-copy retrieve.               */
+KVPOOL_API int kvpool_set_profiling(kvpool_t* pool, int enabled);
+KVPOOL_API int kvpool_profile_read(kvpool_t* pool, int kind, double* total_ms, uint64_t* launches, uint64_t* bytes);
 
 KVPOOL_API const char* kvpool_last_error(void);
 KVPOOL_API const char* kvpool_version(void);

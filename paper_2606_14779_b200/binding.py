@@ -27,7 +27,7 @@ EXPORTS = [
     "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_place", "kvpool_release",
     "kvpool_offload", "kvpool_retrieve", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_counts", "kvpool_lookup", "kvpool_stripe",
-    "kvpool_layer_map", "kvpool_stats", "kvpool_last_error", "kvpool_version",
+    "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_last_error", "kvpool_version",
 ]
 
 
@@ -43,7 +43,7 @@ class Geometry(ctypes.Structure):
 class Tuning(ctypes.Structure):
     _fields_ = [("kernel", c_uint32), ("hbm_ctas", c_uint32), ("link_ctas", c_uint32), ("bulk_chunk", c_uint32),
                 ("bulk_stages", c_uint32), ("bulk_warps", c_uint32), ("stage_slots", c_uint32),
-                ("auto_threshold_bytes", c_uint64)]
+                ("vec_threads", c_uint32), ("vec_unroll", c_uint32), ("auto_threshold_bytes", c_uint64)]
 
 
 class KvPoolError(RuntimeError):
@@ -92,6 +92,8 @@ def lib():
             "kvpool_stripe": [vp, c_uint32, c_uint32, POINTER(vp), POINTER(c_uint64)],
             "kvpool_layer_map": [vp, c_uint32, vp, vp],
             "kvpool_stats": [vp, POINTER(c_uint64), POINTER(c_uint64)],
+            "kvpool_set_profiling": [vp, c_int],
+            "kvpool_profile_read": [vp, c_int, POINTER(c_double), POINTER(c_uint64), POINTER(c_uint64)],
         }
         for name, argtypes in sig.items():
             f = getattr(L, name)
@@ -280,6 +282,18 @@ class KvPool:
         k, m = c_uint64(), c_uint64()
         _ck(lib().kvpool_stats(self.handle, byref(k), byref(m)))
         return k.value, m.value
+
+
+    PROF_PACK, PROF_UNPACK, PROF_ZC_OFFLOAD, PROF_ZC_RETRIEVE = 0, 1, 2, 3
+
+    def set_profiling(self, enabled: bool) -> None:
+        _ck(lib().kvpool_set_profiling(self.handle, int(enabled)))
+
+    def profile_read(self, kind: int) -> Tuple[float, int, int]:
+        """(total ms, launches, algorithmic bytes) of the profiled kernels of `kind` since the last read."""
+        ms, n, b = c_double(), c_uint64(), c_uint64()
+        _ck(lib().kvpool_profile_read(self.handle, kind, byref(ms), byref(n), byref(b)))
+        return ms.value, n.value, b.value
 
 
 def version() -> str:

@@ -19,9 +19,7 @@
 namespace kvp {
 namespace {
 
-constexpr int kVecThreads = 512;
-constexpr int kVecUnroll = 8;
-constexpr uint32_t kVecPiece = kVecUnroll * 32 * 16;  // 4096 bytes per warp iteration
+constexpr int kVecMaxThreads = 512;
 constexpr uint32_t kBulkBarrierBytes = 1024;          // room for warps*stages mbarriers in front of the ring
 
 __device__ __forceinline__ int4 ld_stream(const void* p) {
@@ -59,8 +57,9 @@ __device__ __forceinline__ Piece decode(const LayerArgs& a, uint64_t t, uint32_t
   return p;
 }
 
-template <bool PACK>
-__global__ void __launch_bounds__(kVecThreads) kv_copy_vec16(const __grid_constant__ LayerArgs a) {
+template <bool PACK, int kVecUnroll>
+__global__ void __launch_bounds__(kVecMaxThreads) kv_copy_vec16(const __grid_constant__ LayerArgs a) {
+  constexpr uint32_t kVecPiece = kVecUnroll * 32 * 16;  // bytes per warp iteration (4 KiB at unroll 8)
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t warps_per_cta = blockDim.x >> 5;
   const uint64_t nwarps = static_cast<uint64_t>(gridDim.x) * warps_per_cta;
@@ -184,17 +183,31 @@ cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cf
     while (warps > 1 && static_cast<uint64_t>(warps) * stages * chunk + kBulkBarrierBytes > 200u * 1024u) --warps;
     const uint64_t total = static_cast<uint64_t>(a.K) * 2u * (a.kvb / chunk);
     const uint64_t want = (total + warps - 1) / warps;
-    const uint32_t grid = static_cast<uint32_t>(want < cfg.ctas ? want : cfg.ctas);
     const size_t smem = kBulkBarrierBytes + static_cast<size_t>(warps) * stages * chunk;
+    // persistent ring: never launch more CTAs than are co-resident (shared memory bounds CTAs per SM)
+    const uint64_t per_sm = (227u * 1024u) / (smem + 1024u) ? (227u * 1024u) / (smem + 1024u) : 1;
+    const uint64_t resident = static_cast<uint64_t>(cfg.sm_count ? cfg.sm_count : 148u) * (per_sm > 32 ? 32 : per_sm);
+    uint64_t cap = cfg.ctas < resident ? cfg.ctas : resident;
+    const uint32_t grid = static_cast<uint32_t>(want < cap ? want : cap);
     if (pack) kv_copy_bulk<true><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
     else kv_copy_bulk<false><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
   } else {
-    const uint32_t pieces = (a.kvb + kVecPiece - 1) / kVecPiece;
+    const uint32_t unroll = cfg.vec_unroll == 4 ? 4 : (cfg.vec_unroll == 16 ? 16 : 8);
+    const uint32_t threads = cfg.vec_threads ? cfg.vec_threads : kVecMaxThreads;
+    const uint32_t piece = unroll * 512;
+    const uint32_t pieces = (a.kvb + piece - 1) / piece;
     const uint64_t total = static_cast<uint64_t>(a.K) * 2u * pieces;
-    const uint64_t want = (total + (kVecThreads / 32) - 1) / (kVecThreads / 32);
+    const uint64_t want = (total + (threads / 32) - 1) / (threads / 32);
     const uint32_t grid = static_cast<uint32_t>(want < cfg.ctas ? want : cfg.ctas);
-    if (pack) kv_copy_vec16<true><<<grid, kVecThreads, 0, stream>>>(a);
-    else kv_copy_vec16<false><<<grid, kVecThreads, 0, stream>>>(a);
+#define KV_LAUNCH_VEC(U)                                                       \
+  do {                                                                         \
+    if (pack) kv_copy_vec16<true, U><<<grid, threads, 0, stream>>>(a);         \
+    else kv_copy_vec16<false, U><<<grid, threads, 0, stream>>>(a);             \
+  } while (0)
+    if (unroll == 4) KV_LAUNCH_VEC(4);
+    else if (unroll == 16) KV_LAUNCH_VEC(16);
+    else KV_LAUNCH_VEC(8);
+#undef KV_LAUNCH_VEC
   }
   return cudaGetLastError();
 }

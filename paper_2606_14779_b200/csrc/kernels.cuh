@@ -29,6 +29,8 @@ struct LaunchCfg {
   uint32_t kernel;       // KVPOOL_KERNEL_VEC16 / KVPOOL_KERNEL_BULK
   uint32_t ctas;         // grid size cap
   uint32_t bulk_chunk, bulk_stages, bulk_warps;
+  uint32_t vec_threads, vec_unroll;
+  uint32_t sm_count;
 };
 
 // pack = true: paged -> pool side (offload direction); false: pool side -> paged (retrieve direction).

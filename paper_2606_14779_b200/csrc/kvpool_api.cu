@@ -72,6 +72,12 @@ struct LayerState {
   bool landed_pending = false;
 };
 
+struct ProfRec {  // one profiled kernel launch
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  uint64_t bytes = 0;
+  int kind = 0;
+};
+
 struct StageSlot {
   uint8_t* buf = nullptr;
   cudaEvent_t kernel_done = nullptr;          // last kernel that read/wrote the slot
@@ -106,6 +112,9 @@ struct kvpool {
   kvpool_tuning tune{};
   std::vector<kvpool_placement*> live;
   uint64_t n_kernels = 0, n_memcpys = 0;
+  bool profiling = false;
+  std::vector<ProfRec> prof;
+  std::vector<cudaEvent_t> prof_free;  // timing events ready for reuse
   std::mutex mu;
 };
 
@@ -113,12 +122,14 @@ namespace {
 
 void default_tuning(kvpool* p) {
   p->tune.kernel = KVPOOL_KERNEL_VEC16;
-  p->tune.hbm_ctas = 2u * p->sm_count;
+  p->tune.hbm_ctas = 16u * p->sm_count;  // many short CTAs balance the tail better than a persistent grid here (profiles/r1_sweep_hbm.txt)
   p->tune.link_ctas = 16;
   p->tune.bulk_chunk = 16384;
   p->tune.bulk_stages = 6;
   p->tune.bulk_warps = 2;
   p->tune.stage_slots = 4;
+  p->tune.vec_threads = 512;
+  p->tune.vec_unroll = 8;
   p->tune.auto_threshold_bytes = 8ull << 20;
 }
 
@@ -210,6 +221,9 @@ LaunchCfg launch_cfg(const kvpool* p, bool link_bound) {
   c.bulk_chunk = p->tune.bulk_chunk;
   c.bulk_stages = p->tune.bulk_stages;
   c.bulk_warps = p->tune.bulk_warps;
+  c.vec_threads = p->tune.vec_threads;
+  c.vec_unroll = p->tune.vec_unroll;
+  c.sm_count = static_cast<uint32_t>(p->sm_count);
   return c;
 }
 
@@ -217,6 +231,30 @@ bool use_staged(const kvpool* p, const LayerState& L) {
   if (p->path == KVPOOL_PATH_STAGED) return true;
   if (p->path == KVPOOL_PATH_ZEROCOPY) return false;
   return L.map->K * p->payload >= p->tune.auto_threshold_bytes;
+}
+
+cudaError_t prof_event(kvpool* p, cudaEvent_t* e) {
+  if (!p->prof_free.empty()) { *e = p->prof_free.back(); p->prof_free.pop_back(); return cudaSuccess; }
+  return cudaEventCreate(e);
+}
+
+// Launch one layer kernel, counted and (when profiling) bracketed by an event pair on `s`.
+int launch_counted(kvpool* p, const LayerArgs& a, bool pack, bool link_bound, cudaStream_t s) {
+  ProfRec r;
+  if (p->profiling) {
+    CU(prof_event(p, &r.e0));
+    CU(prof_event(p, &r.e1));
+    r.bytes = static_cast<uint64_t>(a.K) * p->payload;
+    r.kind = (link_bound ? 2 : 0) + (pack ? 0 : 1);
+    CU(cudaEventRecord(r.e0, s));
+  }
+  CU(launch_layer_copy(a, pack, launch_cfg(p, link_bound), s));
+  p->n_kernels++;
+  if (p->profiling) {
+    CU(cudaEventRecord(r.e1, s));
+    p->prof.push_back(r);
+  }
+  return KVPOOL_OK;
 }
 
 // Make `s` wait until the previous user of a staging slot is done with it.
@@ -323,6 +361,8 @@ int kvpool_destroy(kvpool_t* p) {
   for (auto s : p->io) cudaStreamDestroy(s);
   for (auto& b : p->bufs) host_buffer_free(&b);
   if (p->fork) cudaEventDestroy(p->fork);
+  for (auto& r : p->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+  for (auto e : p->prof_free) cudaEventDestroy(e);
   delete p;
   return KVPOOL_OK;
 }
@@ -384,6 +424,10 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
   if (t->bulk_stages > 8 || t->bulk_stages == 1) return fail(KVPOOL_EINVAL, "set_tuning: bulk_stages must be 2..8");
   if (t->bulk_warps > 8) return fail(KVPOOL_EINVAL, "set_tuning: bulk_warps must be 1..8");
   if (t->stage_slots > 64) return fail(KVPOOL_EINVAL, "set_tuning: stage_slots must be <= 64");
+  if (t->vec_threads && (t->vec_threads % 32 || t->vec_threads < 64 || t->vec_threads > 512))
+    return fail(KVPOOL_EINVAL, "set_tuning: vec_threads must be a multiple of 32 in 64..512");
+  if (t->vec_unroll && t->vec_unroll != 4 && t->vec_unroll != 8 && t->vec_unroll != 16)
+    return fail(KVPOOL_EINVAL, "set_tuning: vec_unroll must be 4, 8 or 16");
   kvpool_tuning d = p->tune;
   d.kernel = t->kernel;
   if (t->hbm_ctas) d.hbm_ctas = t->hbm_ctas;
@@ -391,6 +435,8 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
   if (t->bulk_chunk) d.bulk_chunk = t->bulk_chunk;
   if (t->bulk_stages) d.bulk_stages = t->bulk_stages;
   if (t->bulk_warps) d.bulk_warps = t->bulk_warps;
+  if (t->vec_threads) d.vec_threads = t->vec_threads;
+  if (t->vec_unroll) d.vec_unroll = t->vec_unroll;
   if (t->auto_threshold_bytes) d.auto_threshold_bytes = t->auto_threshold_bytes;
   if (t->stage_slots && t->stage_slots != d.stage_slots) {
     DeviceGuard guard(p->cuda_device);
@@ -547,8 +593,8 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
     // zero-copy: one kernel gathers the paged blocks and stores them straight into the mapped host stripes
     for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));  // an earlier staged offload of this layer still in flight
-    CU(launch_layer_copy(a, true, launch_cfg(p, true), s));
-    p->n_kernels++;
+    rc = launch_counted(p, a, true, true, s);
+    if (rc != KVPOOL_OK) return rc;
     CU(cudaEventRecord(L.landed, s));
     L.landed_pending = true;
     return KVPOOL_OK;
@@ -560,8 +606,8 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
   rc = wait_slot_free(p, slot, s);
   if (rc != KVPOOL_OK) return rc;
   for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload);
-  CU(launch_layer_copy(a, true, launch_cfg(p, false), s));
-  p->n_kernels++;
+  rc = launch_counted(p, a, true, false, s);
+  if (rc != KVPOOL_OK) return rc;
   CU(cudaEventRecord(slot.kernel_done, s));
   for (uint32_t i = 0; i < N; ++i) {
     const uint64_t bytes = static_cast<uint64_t>(L.map->counts[i]) * p->payload;
@@ -604,8 +650,8 @@ int kvpool_retrieve(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k
   if (!use_staged(p, L)) {
     for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
-    CU(launch_layer_copy(a, false, launch_cfg(p, true), s));
-    p->n_kernels++;
+    rc = launch_counted(p, a, false, true, s);
+    if (rc != KVPOOL_OK) return rc;
     return KVPOOL_OK;
   }
 
@@ -629,8 +675,8 @@ int kvpool_retrieve(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k
     CU(cudaStreamWaitEvent(s, slot.copy_done[i], 0));
     a.pool_base[i] = reinterpret_cast<uint64_t>(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload);
   }
-  CU(launch_layer_copy(a, false, launch_cfg(p, false), s));
-  p->n_kernels++;
+  rc = launch_counted(p, a, false, false, s);
+  if (rc != KVPOOL_OK) return rc;
   CU(cudaEventRecord(slot.kernel_done, s));
   return KVPOOL_OK;
 }
@@ -660,9 +706,7 @@ int kvpool_pack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void*
   DeviceGuard guard(p->cuda_device);
   LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
   for (uint32_t i = 0; i < p->n; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(stage_dev) + static_cast<uint64_t>(L.map->start[i]) * p->payload);
-  CU(launch_layer_copy(a, true, launch_cfg(p, false), static_cast<cudaStream_t>(cuda_stream)));
-  p->n_kernels++;
-  return KVPOOL_OK;
+  return launch_counted(p, a, true, false, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int kvpool_unpack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
@@ -676,9 +720,7 @@ int kvpool_unpack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_b
   LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
   for (uint32_t i = 0; i < p->n; ++i)
     a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(const_cast<void*>(stage_dev)) + static_cast<uint64_t>(L.map->start[i]) * p->payload);
-  CU(launch_layer_copy(a, false, launch_cfg(p, false), static_cast<cudaStream_t>(cuda_stream)));
-  p->n_kernels++;
-  return KVPOOL_OK;
+  return launch_counted(p, a, false, false, static_cast<cudaStream_t>(cuda_stream));
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -739,6 +781,36 @@ int kvpool_layer_map(const kvpool_placement_t* pl, uint32_t layer, uint8_t* dev_
   const LayerMap& m = *pl->layers[layer].map;
   if (dev_out) std::copy(m.dev.begin(), m.dev.end(), dev_out);
   if (slot_out) std::copy(m.slot.begin(), m.slot.end(), slot_out);
+  return KVPOOL_OK;
+}
+
+int kvpool_set_profiling(kvpool_t* p, int enabled) {
+  if (!p) return fail(KVPOOL_EINVAL, "set_profiling: null pool");
+  p->profiling = enabled != 0;
+  return KVPOOL_OK;
+}
+
+int kvpool_profile_read(kvpool_t* p, int kind, double* total_ms, uint64_t* launches, uint64_t* bytes) {
+  if (!p || kind < 0 || kind > 3) return fail(KVPOOL_EINVAL, "profile_read: bad arguments");
+  DeviceGuard guard(p->cuda_device);
+  double ms_sum = 0;
+  uint64_t n = 0, b = 0;
+  std::vector<ProfRec> keep;
+  for (auto& r : p->prof) {
+    if (r.kind != kind) { keep.push_back(r); continue; }
+    CU(cudaEventSynchronize(r.e1));
+    float ms = 0;
+    CU(cudaEventElapsedTime(&ms, r.e0, r.e1));
+    ms_sum += ms;
+    n += 1;
+    b += r.bytes;
+    p->prof_free.push_back(r.e0);
+    p->prof_free.push_back(r.e1);
+  }
+  p->prof.swap(keep);
+  if (total_ms) *total_ms = ms_sum;
+  if (launches) *launches = n;
+  if (bytes) *bytes = b;
   return KVPOOL_OK;
 }
 
