@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--hbm-ctas", type=int, default=0)
     ap.add_argument("--stage-slots", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", choices=["hbm", "link"], default=None,
+                    help="tuning sweep instead of the benchmark: in-device pack/unpack (hbm) or zero-copy transfer (link) GB/s over launch shapes")
     ap.add_argument("--detail", default=None, help="write per-layer latencies and side measurements to this JSON file")
     return ap.parse_args()
 
@@ -254,7 +256,7 @@ def run_kvpool(args) -> dict:
     pool.set_path({"auto": kv.PATH_AUTO, "staged": kv.PATH_STAGED, "zerocopy": kv.PATH_ZEROCOPY}[args.path])
     tune = {}
     if args.kernel:
-        tune["kernel"] = {"vec16": kv.KERNEL_VEC16, "bulk": kv.KERNEL_BULK}[args.kernel]
+        tune["kernel"] = tune["link_kernel"] = {"vec16": kv.KERNEL_VEC16, "bulk": kv.KERNEL_BULK}[args.kernel]
     for k, v in (("link_ctas", args.link_ctas), ("hbm_ctas", args.hbm_ctas), ("stage_slots", args.stage_slots)):
         if v:
             tune[k] = v
@@ -439,6 +441,22 @@ def run_kvpool(args) -> dict:
                 if it >= 2:
                     times.append(e0.elapsed_time(e1))
             hbm[f"{op}_{kname}_gbps"] = 2 * Kbig * g.payload / (statistics.median(times) * 1e6)
+            # the same launches back to back (16 per event pair): amortises the ~10 us an event pair adds around one launch
+            times = []
+            for it in range(5):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(main)
+                for i in range(16):
+                    l = full_layers[i % len(full_layers)]
+                    if op == "pack":
+                        pool.pack(pls[R - 1], l, src[l][0], src[l][1], g.kvb, tables[R - 1][l], stage, main)
+                    else:
+                        pool.unpack(pls[R - 1], l, dst[l][0], dst[l][1], g.kvb, tables[R - 1][l], stage, main)
+                e1.record(main)
+                main.synchronize()
+                if it >= 1:
+                    times.append(e0.elapsed_time(e1) / 16)
+            hbm[f"{op}_{kname}_back_to_back_gbps"] = 2 * Kbig * g.payload / (statistics.median(times) * 1e6)
     pool.set_tuning(kernel=tn.kernel)
     for pl in pls:
         pl.release()
@@ -467,10 +485,18 @@ def run_kvpool(args) -> dict:
     link_roof = {"bound": "host_link", "what": "retrieve leg (all layers back to back)", "achieved": value / world, "peak": link_h2d,
                  "unit": "GB/s", "frac": value / world / link_h2d, "offload_achieved": moved / (off_ms * 1e6), "offload_peak": link_d2h,
                  "offload_frac": moved / (off_ms * 1e6) / link_d2h, "peak_source": "1 GiB pinned cudaMemcpyAsync measured in this run"}
-    best_unpack = max(hbm["unpack_vec16_gbps"], hbm["unpack_bulk_gbps"])
-    hbm_roof = {"bound": "hbm", "what": f"in-device pack/unpack of one {Kbig * g.payload / 2**20:.0f} MiB layer, 2*bytes/time", **hbm,
-                "peak": peaks["hbm_gbs"], "frac_unpack": best_unpack / peaks["hbm_gbs"],
-                "frac_pack": max(hbm["pack_vec16_gbps"], hbm["pack_bulk_gbps"]) / peaks["hbm_gbs"], "frac_unpack_of_8TBs_nominal": best_unpack / 8000.0}
+    best_unpack = max(hbm["unpack_vec16_back_to_back_gbps"], hbm["unpack_bulk_back_to_back_gbps"])
+    best_pack = max(hbm["pack_vec16_back_to_back_gbps"], hbm["pack_bulk_back_to_back_gbps"])
+    hbm_roof = {"bound": "hbm", "what": f"in-device pack/unpack of one {Kbig * g.payload / 2**20:.0f} MiB layer launched alone, 2*bytes/time; "
+                "*_gbps = one launch per event pair, *_back_to_back_gbps = 16 launches per event pair", **hbm,
+                "peak": peaks["hbm_gbs"], "frac_unpack": best_unpack / peaks["hbm_gbs"], "frac_pack": best_pack / peaks["hbm_gbs"],
+                "frac_unpack_of_8TBs_nominal": best_unpack / 8000.0, "frac_pack_of_8TBs_nominal": best_pack / 8000.0}
+    if dom < 2:
+        kn = "vec16" if tn.kernel == kv.KERNEL_VEC16 else "bulk"
+        roof["achieved_back_to_back"] = hbm[f"{'pack' if dom == 0 else 'unpack'}_{kn}_back_to_back_gbps"]
+        roof["frac_back_to_back"] = roof["achieved_back_to_back"] / peaks["hbm_gbs"]
+        roof["note"] = ("achieved = per-launch event pairs inside the timed step, where every launch follows ~4 ms of SM idle time "
+                        "(link-bound pipeline) and carries ~10 us of event-pair overhead; achieved_back_to_back = same kernel, 16 launches per pair")
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms,
@@ -478,6 +504,7 @@ def run_kvpool(args) -> dict:
         "config": {"workload": wl.name, "cfg": args.config, "context_tokens": list(wl.context_tokens), "layers": L, "requests": R,
                    "moved_bytes_per_leg": moved, "pool_buffers": N, "weights": weights_kind, "bandwidth_gbps": [round(float(x), 3) for x in bw],
                    "numa_nodes": numa_actual, "path": args.path, "kernel": "vec16" if tn.kernel == kv.KERNEL_VEC16 else "bulk",
+                   "link_kernel": "vec16" if tn.link_kernel == kv.KERNEL_VEC16 else "bulk",
                    "link_ctas": tn.link_ctas, "hbm_ctas": tn.hbm_ctas, "stage_slots": tn.stage_slots, "streams": len(streams),
                    "l2": f"inputs larger than L2: each leg moves {moved / 2**30:.1f} GiB through {L} distinct layers (L2 is 126 MB); no flush needed",
                    "step": "kvpool_place + kvpool_offload x layers + kvpool_retrieve x layers; value = retrieve leg"},
@@ -505,10 +532,83 @@ def run_kvpool(args) -> dict:
     return out if rank == 0 else None
 
 
+def run_sweep(args) -> None:
+    """Tuning sweeps on a 4-layer cut of the workload (text table on stdout)."""
+    import itertools
+    import torch
+    from paper_2606_14779_b200 import binding as kv
+    from paper_2606_14779_b200 import workloads as W
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    wl = W.make_workload(args.config, n_layers=4)
+    wl.sliding_layers = ()
+    g, R = wl.geom, len(wl.requests) - 1
+    bw = list(wl.default_weights())
+    K = int(wl.blocks_per_layer(R)[0])
+    share = np.array(bw) / np.sum(bw)
+    caps = [int(wl.moved_bytes() * s * 1.25) + 64 * (g.payload + 4096) for s in share]
+    pool = kv.KvPool(bw, caps, n_layers=4, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim)
+    probe_h2d = pool.measure_bandwidth(0, 0, min(256 << 20, caps[0]), 5)
+    probe_d2h = pool.measure_bandwidth(0, 1, min(256 << 20, caps[0]), 5)
+    pl = pool.place(wl.blocks_per_layer(R))
+    src = [W.kv_layer_torch(wl, l, dev) for l in range(4)]
+    tables = [torch.from_numpy(np.ascontiguousarray(wl.layer_table(R, l))).to(dev) for l in range(4)]
+    stage = torch.empty(K * g.payload, dtype=torch.uint8, device=dev)
+    main_s = torch.cuda.Stream(device=dev)
+    nbytes = K * g.payload
+
+    def timed(fn, reps, per_pair):
+        ts = []
+        for it in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(main_s)
+            for i in range(per_pair):
+                fn((it * per_pair + i) % 4)
+            e1.record(main_s)
+            main_s.synchronize()
+            if it >= 2:
+                ts.append(e0.elapsed_time(e1) / per_pair)
+        return statistics.median(ts)
+
+    print(f"# bench.py --sweep {args.sweep} --config {args.config}: {wl.name}, K={K} blocks of P={g.payload} B = {nbytes / 2**20:.0f} MiB per launch")
+    if args.sweep == "hbm":
+        print("# in-device pack / unpack, GB/s = 2*bytes/time, 8 launches per event pair, median of 6; measured HBM copy peak "
+              f"{measured_peaks()['hbm_gbs']:.0f} GB/s")
+        for threads, unroll, ctas in itertools.product((128, 256, 512), (4, 8, 16), (148, 296, 592, 1184, 2368, 4736)):
+            pool.set_tuning(kernel=kv.KERNEL_VEC16, vec_threads=threads, vec_unroll=unroll, hbm_ctas=ctas)
+            p = timed(lambda l: pool.pack(pl, l, src[l][0], src[l][1], g.kvb, tables[l], stage, main_s), 8, 8)
+            u = timed(lambda l: pool.unpack(pl, l, src[l][0], src[l][1], g.kvb, tables[l], stage, main_s), 8, 8)
+            print(f"vec16 threads {threads:4d} unroll {unroll:2d} ctas {ctas:5d}: pack {2 * nbytes / p / 1e6:6.0f}  unpack {2 * nbytes / u / 1e6:6.0f}", flush=True)
+        for warps, stages, chunk, ctas in [(1, 8, 16384, 148), (2, 6, 16384, 148), (2, 4, 16384, 148), (4, 6, 8192, 148), (4, 4, 8192, 296),
+                                           (2, 3, 16384, 296), (2, 3, 32768, 148), (4, 3, 16384, 148), (8, 3, 8192, 148), (8, 6, 4096, 148)]:
+            pool.set_tuning(kernel=kv.KERNEL_BULK, bulk_warps=warps, bulk_stages=stages, bulk_chunk=chunk, hbm_ctas=ctas)
+            p = timed(lambda l: pool.pack(pl, l, src[l][0], src[l][1], g.kvb, tables[l], stage, main_s), 8, 8)
+            u = timed(lambda l: pool.unpack(pl, l, src[l][0], src[l][1], g.kvb, tables[l], stage, main_s), 8, 8)
+            print(f"bulk warps {warps} stages {stages} chunk {chunk:5d} ctas {ctas:4d}: pack {2 * nbytes / p / 1e6:6.0f}  unpack {2 * nbytes / u / 1e6:6.0f}", flush=True)
+    else:
+        print(f"# zero-copy offload / retrieve of one layer, GB/s = bytes/time, 1 launch per event pair, median of 4; cudaMemcpyAsync 256 MiB: "
+              f"H2D {probe_h2d:.2f} D2H {probe_d2h:.2f} GB/s")
+        pool.set_path(kv.PATH_ZEROCOPY)
+        cases = [(kv.KERNEL_VEC16, "vec16", dict(vec_threads=t)) for t in (128, 256, 512)] + \
+                [(kv.KERNEL_BULK, "bulk", dict(bulk_warps=w, bulk_stages=s_, bulk_chunk=c)) for w, s_, c in ((1, 4, 16384), (1, 8, 16384), (2, 6, 16384), (4, 6, 8192))]
+        for kid, name, extra in cases:
+            for ctas in (1, 2, 4, 8, 16, 32, 148):
+                pool.set_tuning(link_kernel=kid, link_ctas=ctas, **extra)
+                o = timed(lambda l: pool.offload(pl, l, src[l][0], src[l][1], g.kvb, tables[l], main_s), 6, 1)
+                r = timed(lambda l: pool.retrieve(pl, l, src[l][0], src[l][1], g.kvb, tables[l], main_s), 6, 1)
+                print(f"{name} {extra} ctas {ctas:4d}: offload {nbytes / o / 1e6:6.2f}  retrieve {nbytes / r / 1e6:6.2f}", flush=True)
+    pl.release()
+    pool.destroy()
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         print(json.dumps(run_reference(args)), flush=True)
+        return
+    if args.sweep:
+        run_sweep(args)
         return
     out = run_kvpool(args)
     if out is None:

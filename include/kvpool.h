@@ -77,9 +77,10 @@ typedef struct { /* geometry of one paged KV block */
 } kvpool_geometry;
 
 typedef struct {         /* kvpool_set_tuning; 0 in any field = library default                          */
-  uint32_t kernel;       /* KVPOOL_KERNEL_*                                                             */
+  uint32_t kernel;       /* KVPOOL_KERNEL_* for HBM-bound launches (staged path, kvpool_pack/unpack); always applied */
+  uint32_t link_kernel;  /* KVPOOL_KERNEL_* for zero-copy launches (default BULK: 2 CTAs fill the link); always applied */
   uint32_t hbm_ctas;     /* CTAs of an in-device pack/unpack launch (default: a multiple of the SM count) */
-  uint32_t link_ctas;    /* CTAs of a zero-copy launch (few suffice to fill the host link)               */
+  uint32_t link_ctas;    /* CTAs of a zero-copy launch (default 4; profiles/r1_sweep_link.txt)           */
   uint32_t bulk_chunk;   /* bytes per cp.async.bulk (power of two, 1 KiB..32 KiB)                        */
   uint32_t bulk_stages;  /* ring depth per issuing warp                                                 */
   uint32_t bulk_warps;   /* issuing warps per CTA                                                       */

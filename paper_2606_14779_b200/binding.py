@@ -41,7 +41,7 @@ class Geometry(ctypes.Structure):
 
 
 class Tuning(ctypes.Structure):
-    _fields_ = [("kernel", c_uint32), ("hbm_ctas", c_uint32), ("link_ctas", c_uint32), ("bulk_chunk", c_uint32),
+    _fields_ = [("kernel", c_uint32), ("link_kernel", c_uint32), ("hbm_ctas", c_uint32), ("link_ctas", c_uint32), ("bulk_chunk", c_uint32),
                 ("bulk_stages", c_uint32), ("bulk_warps", c_uint32), ("stage_slots", c_uint32),
                 ("vec_threads", c_uint32), ("vec_unroll", c_uint32), ("auto_threshold_bytes", c_uint64)]
 
@@ -226,10 +226,10 @@ class KvPool:
         _ck(lib().kvpool_set_path(self.handle, path))
 
     def set_tuning(self, **kw) -> None:
-        t = self.get_tuning()
-        cur_kernel = t.kernel
+        cur = self.get_tuning()
         t = Tuning()
-        t.kernel = kw.pop("kernel", cur_kernel)
+        t.kernel = kw.pop("kernel", cur.kernel)
+        t.link_kernel = kw.pop("link_kernel", cur.link_kernel)
         for k, v in kw.items():
             setattr(t, k, v)
         _ck(lib().kvpool_set_tuning(self.handle, ctypes.addressof(t)))

@@ -122,8 +122,9 @@ namespace {
 
 void default_tuning(kvpool* p) {
   p->tune.kernel = KVPOOL_KERNEL_VEC16;
+  p->tune.link_kernel = KVPOOL_KERNEL_BULK;  // 2 CTAs already saturate the link (profiles/r1_sweep_link.txt)
   p->tune.hbm_ctas = 16u * p->sm_count;  // many short CTAs balance the tail better than a persistent grid here (profiles/r1_sweep_hbm.txt)
-  p->tune.link_ctas = 16;
+  p->tune.link_ctas = 4;
   p->tune.bulk_chunk = 16384;
   p->tune.bulk_stages = 6;
   p->tune.bulk_warps = 2;
@@ -216,7 +217,7 @@ LayerArgs base_args(const kvpool* p, const LayerState& L, const void* k_base, co
 
 LaunchCfg launch_cfg(const kvpool* p, bool link_bound) {
   LaunchCfg c{};
-  c.kernel = p->tune.kernel;
+  c.kernel = link_bound ? p->tune.link_kernel : p->tune.kernel;
   c.ctas = link_bound ? p->tune.link_ctas : p->tune.hbm_ctas;
   c.bulk_chunk = p->tune.bulk_chunk;
   c.bulk_stages = p->tune.bulk_stages;
@@ -418,7 +419,8 @@ int kvpool_set_path(kvpool_t* p, int path) {
 
 int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
   if (!p || !t) return fail(KVPOOL_EINVAL, "set_tuning: null argument");
-  if (t->kernel > KVPOOL_KERNEL_BULK) return fail(KVPOOL_EINVAL, "set_tuning: unknown kernel %u", t->kernel);
+  if (t->kernel > KVPOOL_KERNEL_BULK || t->link_kernel > KVPOOL_KERNEL_BULK)
+    return fail(KVPOOL_EINVAL, "set_tuning: unknown kernel %u / link_kernel %u", t->kernel, t->link_kernel);
   if (t->bulk_chunk && (t->bulk_chunk < 1024 || t->bulk_chunk > 32768 || (t->bulk_chunk & (t->bulk_chunk - 1))))
     return fail(KVPOOL_EINVAL, "set_tuning: bulk_chunk must be a power of two in 1 KiB..32 KiB");
   if (t->bulk_stages > 8 || t->bulk_stages == 1) return fail(KVPOOL_EINVAL, "set_tuning: bulk_stages must be 2..8");
@@ -430,6 +432,7 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
     return fail(KVPOOL_EINVAL, "set_tuning: vec_unroll must be 4, 8 or 16");
   kvpool_tuning d = p->tune;
   d.kernel = t->kernel;
+  d.link_kernel = t->link_kernel;
   if (t->hbm_ctas) d.hbm_ctas = t->hbm_ctas;
   if (t->link_ctas) d.link_ctas = t->link_ctas;
   if (t->bulk_chunk) d.bulk_chunk = t->bulk_chunk;

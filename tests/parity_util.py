@@ -54,7 +54,7 @@ def run_parity(wl: W.Workload, *, path: int, kernel: int, bandwidth=None, tuning
     pool = make_pool(wl, bw)
     try:
         pool.set_path(path)
-        pool.set_tuning(kernel=kernel, **(tuning or {}))
+        pool.set_tuning(kernel=kernel, link_kernel=kernel, **(tuning or {}))
         cuda_streams = [torch.cuda.Stream(device=dev) for _ in range(streams)]
         R = len(wl.requests)
         pls = [pool.place(wl.blocks_per_layer(r)) for r in range(R)]
