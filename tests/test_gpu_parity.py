@@ -188,3 +188,53 @@ def test_kv_stream_is_identical_on_cpu_and_gpu():
     rng = np.random.default_rng(3)
     for plane, phys in [(0, 0), (1, wl.nphys - 1)] + [(int(rng.integers(0, 2)), int(rng.integers(0, wl.nphys))) for _ in range(32)]:
         assert np.array_equal(a[plane, phys], W.kv_block_numpy(wl, 0, plane, phys))
+
+
+@pytest.mark.parametrize("cfg", [4, 3])
+def test_full_size_configs_sampled_against_oracle(cfg):
+    """BASELINE.json's full sizes in bench.py's launch configuration (path auto, default tuning): placement is
+    compared in full; stripe payloads and retrieved blocks are compared on samples the oracle side computes one
+    by one (the counter-based KV stream regenerates any block on the CPU); round trip and untouched poison are
+    checked over the whole tensors on the GPU."""
+    wl = W.make_workload(cfg)
+    g, dev = wl.geom, torch.device("cuda:0")
+    bw = list(wl.default_weights())
+    bpl = wl.blocks_per_layer(0)
+    pool = make_pool(wl)
+    try:
+        pl = pool.place(bpl)
+        opl = oracle.place(bw, bpl)
+        check_placement(pl, opl)
+        table_np = [np.ascontiguousarray(wl.layer_table(0, l)) for l in range(g.n_layers)]
+        tables = [torch.from_numpy(t).to(dev) for t in table_np]
+        src = [W.kv_layer_torch(wl, l, dev) for l in range(g.n_layers)]
+        dst = [W.poison_torch((2, wl.nphys, g.kvb // 2), dev) for l in range(g.n_layers)]
+        s = torch.cuda.Stream()
+        for l in range(g.n_layers):
+            pool.offload(pl, l, src[l][0], src[l][1], g.kvb, tables[l], s)
+        pool.wait_offloads(pl, s)
+        for l in range(g.n_layers):
+            pool.retrieve(pl, l, dst[l][0], dst[l][1], g.kvb, tables[l], s)
+        s.synchronize()
+        rng = np.random.default_rng(cfg)
+        poison = np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item()
+        for l in range(g.n_layers):
+            K = len(table_np[l])
+            for j in sorted(set([0, K - 1] + [int(x) for x in rng.integers(0, K, size=6)])):
+                phys = int(table_np[l][j])
+                want = np.concatenate([W.kv_block_numpy(wl, l, 0, phys), W.kv_block_numpy(wl, l, 1, phys)]).view(np.uint8)
+                d, sl = int(opl[l].dev[j]), int(opl[l].slot[j])
+                got = pl.stripe(l, d)[sl * g.payload:(sl + 1) * g.payload]
+                assert np.array_equal(got, want), f"stripe payload differs: layer {l} block {j}"
+                back = dst[l][:, phys].cpu().numpy().view(np.uint16).reshape(-1)
+                assert np.array_equal(back, want.view(np.uint16)), f"retrieved block differs: layer {l} block {j}"
+            used = torch.zeros(wl.nphys, dtype=torch.bool, device=dev)
+            used[tables[l].long()] = True
+            assert torch.equal(dst[l][:, used], src[l][:, used])
+            assert bool((dst[l][:, ~used] == poison).all())
+            # byte share of every device within one block of its bandwidth share (north star invariant)
+            for i, wi in enumerate(bw):
+                assert abs(pl.stripe(l, i).nbytes - wi / sum(bw) * K * g.payload) < g.payload
+        pl.release()
+    finally:
+        pool.destroy()
