@@ -324,6 +324,10 @@ def run_kvpool(args) -> dict:
         ev[0].record(main)
         do_offload(pls)
         ev[1].record(main)
+        # the legs are timed apart: without this the retrieve's host->GPU copies (which may run ahead of the caller's
+        # stream) would start under the tail of the offload leg and borrow the link's other direction
+        main.synchronize()
+        pool.synchronize()
         ev[2].record(main)
         do_retrieve(pls)
         ev[3].record(main)
@@ -470,7 +474,7 @@ def run_kvpool(args) -> dict:
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
         with open(tp) as f:
-            traffic = json.load(f).get(kinds[dom])
+            traffic = json.load(f).get(str(args.config), {}).get(kinds[dom])     # captured per config; null where not captured
     if dom < 2:
         ach = 2 * b / (ms * 1e6) if ms > 0 else 0.0
         roof = {"bound": "hbm", "kernel": kinds[dom], "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],

@@ -89,8 +89,9 @@ struct StageSlot {
 struct kvpool_placement {
   kvpool* pool = nullptr;
   std::vector<LayerState> layers;
-  void* tables_d = nullptr;  // one device allocation holding every LayerMap's dev/slot columns
-  cudaEvent_t join = nullptr;
+  uint8_t* tables_d = nullptr;   // every LayerMap's dev/slot columns, contiguous
+  uint64_t tables_bytes = 0;
+  bool tables_in_arena = false;  // carved out of the pool's table arena (else a private cudaMalloc)
 };
 
 struct kvpool {
@@ -107,7 +108,9 @@ struct kvpool {
   std::vector<StageSlot> slots;
   uint64_t slot_bytes = 0;
   uint64_t slot_cursor = 0;
-  cudaEvent_t fork = nullptr;
+  uint8_t* table_arena = nullptr;  // device memory for placements' GLT columns: no cudaMalloc/cudaFree per request
+  StripeAllocator table_alloc;
+  std::vector<cudaEvent_t> ev_free;  // recycled cudaEventDisableTiming events
   int path = KVPOOL_PATH_AUTO;
   kvpool_tuning tune{};
   std::vector<kvpool_placement*> live;
@@ -177,13 +180,26 @@ bool is_live(const kvpool* p, const kvpool_placement* pl) {
   return std::find(p->live.begin(), p->live.end(), pl) != p->live.end();
 }
 
+constexpr uint64_t kTableArenaBytes = 8ull << 20;
+
+void free_tables(kvpool* p, kvpool_placement* pl) {
+  if (!pl->tables_d) return;
+  if (pl->tables_in_arena) p->table_alloc.free(static_cast<uint64_t>(pl->tables_d - p->table_arena), pl->tables_bytes);
+  else cudaFree(pl->tables_d);
+  pl->tables_d = nullptr;
+}
+
+cudaError_t take_event(kvpool* p, cudaEvent_t* e) {
+  if (!p->ev_free.empty()) { *e = p->ev_free.back(); p->ev_free.pop_back(); return cudaSuccess; }
+  return cudaEventCreateWithFlags(e, cudaEventDisableTiming);
+}
+
 void destroy_placement(kvpool* p, kvpool_placement* pl) {
   for (auto& L : pl->layers) {
     for (uint32_t i = 0; i < p->n; ++i) p->alloc[i].free(L.stripe_off[i], static_cast<uint64_t>(L.map->counts[i]) * p->payload);
-    if (L.landed) cudaEventDestroy(L.landed);
+    if (L.landed) p->ev_free.push_back(L.landed);
   }
-  if (pl->tables_d) cudaFree(pl->tables_d);
-  if (pl->join) cudaEventDestroy(pl->join);
+  free_tables(p, pl);
   delete pl;
 }
 
@@ -329,7 +345,7 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
   auto cleanup = [&]() {
     for (auto& b : p->bufs) host_buffer_free(&b);
     for (auto s : p->io) cudaStreamDestroy(s);
-    if (p->fork) cudaEventDestroy(p->fork);
+    if (p->table_arena) cudaFree(p->table_arena);
   };
   p->bufs.resize(n_devs);
   for (uint32_t i = 0; i < n_devs; ++i) {
@@ -347,7 +363,12 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     cudaError_t e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
     if (e != cudaSuccess) { cleanup(); return fail(KVPOOL_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)); }
   }
-  if (cudaEventCreateWithFlags(&p->fork, cudaEventDisableTiming) != cudaSuccess) { cleanup(); return fail(KVPOOL_ECUDA, "cudaEventCreate failed"); }
+  if (cudaMalloc(reinterpret_cast<void**>(&p->table_arena), kTableArenaBytes) != cudaSuccess) {
+    cudaGetLastError();
+    cleanup();
+    return fail(KVPOOL_ENOMEM, "create: table arena");
+  }
+  p->table_alloc = StripeAllocator(kTableArenaBytes, 256);
   *out = p.release();
   return KVPOOL_OK;
 }
@@ -361,7 +382,8 @@ int kvpool_destroy(kvpool_t* p) {
   free_slots(p);
   for (auto s : p->io) cudaStreamDestroy(s);
   for (auto& b : p->bufs) host_buffer_free(&b);
-  if (p->fork) cudaEventDestroy(p->fork);
+  if (p->table_arena) cudaFree(p->table_arena);
+  for (auto e : p->ev_free) cudaEventDestroy(e);
   for (auto& r : p->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   for (auto e : p->prof_free) cudaEventDestroy(e);
   delete p;
@@ -516,10 +538,9 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
     for (uint32_t l = 0; l < done_layers; ++l)
       for (uint32_t i = 0; i < N; ++i)
         p->alloc[i].free(pl->layers[l].stripe_off[i], static_cast<uint64_t>(pl->layers[l].map->counts[i]) * p->payload);
-    if (pl->tables_d) cudaFree(pl->tables_d);
+    free_tables(p, pl.get());
     for (auto& Ls : pl->layers)
-      if (Ls.landed) cudaEventDestroy(Ls.landed);
-    if (pl->join) cudaEventDestroy(pl->join);
+      if (Ls.landed) p->ev_free.push_back(Ls.landed);
   };
   if (!ok) {
     rollback();
@@ -529,17 +550,25 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
 
   // GLT upload: dense (device_id, slot) columns, one device allocation per placement
   if (table_bytes) {
-    cudaError_t e = cudaMalloc(&pl->tables_d, table_bytes);
-    if (e != cudaSuccess) { cudaGetLastError(); rollback(); return fail(KVPOOL_ENOMEM, "place: table upload buffer: %s", cudaGetErrorString(e)); }
+    cudaError_t e = cudaSuccess;
+    uint64_t arena_off = 0;
+    pl->tables_bytes = table_bytes;
+    if (p->table_alloc.alloc(table_bytes, &arena_off)) {
+      pl->tables_d = p->table_arena + arena_off;
+      pl->tables_in_arena = true;
+    } else {
+      e = cudaMalloc(reinterpret_cast<void**>(&pl->tables_d), table_bytes);  // arena exhausted: private allocation
+      if (e != cudaSuccess) { cudaGetLastError(); pl->tables_d = nullptr; rollback(); return fail(KVPOOL_ENOMEM, "place: table upload buffer: %s", cudaGetErrorString(e)); }
+    }
     std::vector<uint8_t> host(table_bytes);
     uint64_t off = 0;
     for (auto& kv : by_k) {
       LayerMap& m = *kv.second;
       if (m.K == 0) continue;
-      m.slot_d = reinterpret_cast<const uint32_t*>(static_cast<uint8_t*>(pl->tables_d) + off);
+      m.slot_d = reinterpret_cast<const uint32_t*>(pl->tables_d + off);
       memcpy(host.data() + off, m.slot.data(), m.K * 4);
       off += (m.K * 4 + 255) / 256 * 256;
-      m.dev_d = static_cast<const uint8_t*>(pl->tables_d) + off;
+      m.dev_d = pl->tables_d + off;
       memcpy(host.data() + off, m.dev.data(), m.K);
       off += (m.K + 255) / 256 * 256;
     }
@@ -547,10 +576,9 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
     if (e != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: table upload: %s", cudaGetErrorString(e)); }
   }
   for (auto& Ls : pl->layers) {
-    cudaError_t e = cudaEventCreateWithFlags(&Ls.landed, cudaEventDisableTiming);
+    cudaError_t e = take_event(p, &Ls.landed);
     if (e != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: cudaEventCreate: %s", cudaGetErrorString(e)); }
   }
-  if (cudaEventCreateWithFlags(&pl->join, cudaEventDisableTiming) != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: cudaEventCreate failed"); }
   if (p->path != KVPOOL_PATH_ZEROCOPY) {
     const int rc = ensure_slots(p, max_layer_bytes);
     if (rc != KVPOOL_OK) { rollback(); return rc; }
