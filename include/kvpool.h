@@ -150,6 +150,14 @@ KVPOOL_API int kvpool_offload(kvpool_t* pool, kvpool_placement_t* pl, uint32_t l
                    void* cuda_stream);
 KVPOOL_API int kvpool_retrieve(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, void* k_base /*device*/, void* v_base /*device*/,
                     uint64_t block_stride_bytes, const int32_t* block_table_dev, void* cuda_stream);
+/* Partial retrieval (prefix reuse, chunked prefetch): like kvpool_retrieve for logical blocks
+ * [first_block, first_block + n_blocks) of the layer only.  block_table_dev is still the LAYER's table (indexed by
+ * logical block, as at offload); only the entries of the range are read and only their physical blocks written.
+ * Because placement is a smooth weighted round-robin (R3), any contiguous range draws on all pool devices
+ * in proportion to their bandwidth, within N-1 blocks.  EINVAL if the range exceeds K_l; n_blocks = 0 is a no-op.    */
+KVPOOL_API int kvpool_retrieve_range(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks,
+                          void* k_base /*device*/, void* v_base /*device*/, uint64_t block_stride_bytes,
+                          const int32_t* block_table_dev, void* cuda_stream);
 /* Make `stream` wait until every offload enqueued so far with `pl` has landed in the pool.             */
 KVPOOL_API int kvpool_wait_offloads(kvpool_t* pool, kvpool_placement_t* pl, void* cuda_stream);
 /* Block the host until all work the pool enqueued on its own streams is done (not the caller's).       */

@@ -47,6 +47,8 @@ def _load():
         for f in (lib.orc_offload_layer, lib.orc_retrieve_layer):
             f.restype = None
             f.argtypes = [vp, vp, u64, u64, vp, u64, vp, vp, vp]
+        lib.orc_retrieve_range.restype = None
+        lib.orc_retrieve_range.argtypes = [vp, vp, u64, u64, vp, u64, u64, vp, vp, vp]
         lib.orc_layer_parallel.restype = ctypes.c_int
         lib.orc_layer_parallel.argtypes = [ctypes.c_int, vp, vp, u64, u64, vp, u64, vp, vp, vp, u32]
         _lib = lib
@@ -153,3 +155,12 @@ def retrieve_layer(kv_layer_out: np.ndarray, table: np.ndarray, pl: LayerPlaceme
     else:
         lib.orc_retrieve_layer(kp, vp_, stride, kvb, _ptr(table), table.shape[0], _ptr(pl.dev), _ptr(pl.slot),
                                ctypes.addressof(ptrs))
+
+
+def retrieve_range(kv_layer_out: np.ndarray, table: np.ndarray, pl: LayerPlacement, stripes: List[np.ndarray], first: int, n: int) -> None:
+    """Partial retrieval of logical blocks [first, first+n) of one layer into kv_layer_out (in place)."""
+    kp, vp_, stride, kvb = _planes(kv_layer_out)
+    table = np.ascontiguousarray(table, dtype=np.int32)
+    assert 0 <= first and first + n <= table.shape[0]
+    ptrs = _stripe_ptrs(stripes)
+    _load().orc_retrieve_range(kp, vp_, stride, kvb, _ptr(table), int(first), int(n), _ptr(pl.dev), _ptr(pl.slot), ctypes.addressof(ptrs))

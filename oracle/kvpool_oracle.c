@@ -19,6 +19,8 @@
  *                             independent exact-rational restatement, hand-worked example
  *   orc_offload/orc_retrieve— N=1 reduces to numpy fancy indexing / index assignment, identity table
  *                             reduces to memcpy, O(K^2) brute-force search, round trip, conservation
+ *   orc_retrieve_range      — (0, K) equals orc_retrieve_layer; disjoint ranges compose to the full retrieve; numpy
+ *                             index assignment on the range; nothing outside the range's physical blocks is written
  *   stripe offsets inside a pool buffer: PARITY UNPINNED (implementation detail; not produced here).
  *
  * Build: gcc -O2 -shared -fPIC -pthread -o liboracle.so kvpool_oracle.c   (oracle/__init__.py does it)
@@ -135,6 +137,20 @@ void orc_retrieve_layer(uint8_t *k_plane, uint8_t *v_plane, uint64_t stride, uin
                         const int32_t *table, uint64_t K, const uint32_t *dev, const uint32_t *slot,
                         const uint8_t *const *stripes) {
     for (uint64_t j = 0; j < K; ++j) {
+        const uint8_t *src = stripes[dev[j]] + (uint64_t)slot[j] * 2u * kvb;
+        memcpy(k_plane + (uint64_t)table[j] * stride, src, kvb);
+        memcpy(v_plane + (uint64_t)table[j] * stride, src + kvb, kvb);
+    }
+}
+
+/* ---- partial retrieval -------------------------------------------------------------------------
+ * "When a decoding step requests offloaded KV caches, the allocator first looks up their GLT entries"
+ * (PAPER.md:241): the request may name any subset; here a contiguous range [first, first+n) of the
+ * layer's logical blocks.  Same per-block procedure as orc_retrieve_layer, restricted to the range. */
+void orc_retrieve_range(uint8_t *k_plane, uint8_t *v_plane, uint64_t stride, uint64_t kvb, const int32_t *table,
+                        uint64_t first, uint64_t n, const uint32_t *dev, const uint32_t *slot,
+                        const uint8_t *const *stripes) {
+    for (uint64_t j = first; j < first + n; ++j) {
         const uint8_t *src = stripes[dev[j]] + (uint64_t)slot[j] * 2u * kvb;
         memcpy(k_plane + (uint64_t)table[j] * stride, src, kvb);
         memcpy(v_plane + (uint64_t)table[j] * stride, src + kvb, kvb);

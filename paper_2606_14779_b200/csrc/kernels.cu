@@ -42,8 +42,9 @@ struct Piece {
 };
 __device__ __forceinline__ Piece decode(const LayerArgs& a, uint64_t t, uint32_t pieces, uint32_t piece_bytes) {
   const uint32_t per_unit = 2u * pieces;
-  const uint32_t j = static_cast<uint32_t>(t / per_unit);
-  const uint32_t r = static_cast<uint32_t>(t - static_cast<uint64_t>(j) * per_unit);
+  const uint32_t local = static_cast<uint32_t>(t / per_unit);
+  const uint32_t r = static_cast<uint32_t>(t - static_cast<uint64_t>(local) * per_unit);
+  const uint32_t j = a.j0 + local;
   const uint32_t half = r >= pieces ? 1u : 0u;  // 0: K block, 1: V block
   const uint32_t c = r - half * pieces;
   const int32_t phys = __ldg(a.table + j);

@@ -20,7 +20,8 @@ struct LayerArgs {
   const int32_t* table;
   const uint8_t* dev;
   const uint32_t* slot;
-  uint32_t K;
+  uint32_t K;    // number of units this launch moves ...
+  uint32_t j0;   // ... starting at logical block j0 (table/dev/slot are indexed by j0 + local index)
   uint32_t kvb;
   uint64_t pool_base[kMaxDev];
 };

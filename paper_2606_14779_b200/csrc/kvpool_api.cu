@@ -60,6 +60,7 @@ struct LayerMap {
   std::vector<uint32_t> start;    // [N] first stripe-order position of device i (prefix sum of counts)
   std::vector<uint8_t> dev;       // [K]
   std::vector<uint32_t> slot;     // [K]
+  std::vector<uint32_t> order;    // [K] order[start[i] + s] = logical block stored at slot s of device i (ascending in s)
   const uint8_t* dev_d = nullptr; // device copies
   const uint32_t* slot_d = nullptr;
 };
@@ -227,6 +228,7 @@ LayerArgs base_args(const kvpool* p, const LayerState& L, const void* k_base, co
   a.dev = L.map->dev_d;
   a.slot = L.map->slot_d;
   a.K = static_cast<uint32_t>(L.map->K);
+  a.j0 = 0;
   a.kvb = static_cast<uint32_t>(p->kvb);
   return a;
 }
@@ -510,6 +512,8 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
       wrr_closed_form(m->counts.data(), N, K, m->dev.data(), m->slot.data());
       uint32_t acc = 0;
       for (uint32_t i = 0; i < N; ++i) { m->start[i] = acc; acc += m->counts[i]; }
+      m->order.resize(K);
+      for (uint64_t j = 0; j < K; ++j) m->order[m->start[m->dev[j]] + m->slot[j]] = static_cast<uint32_t>(j);
       table_bytes += (K * 5 + 255) / 256 * 256 + 256;
       it = by_k.emplace(K, std::move(m)).first;
     }
@@ -666,50 +670,71 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
   return KVPOOL_OK;
 }
 
-int kvpool_retrieve(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
-                    const int32_t* table, void* cuda_stream) {
+// Slots of device i that hold logical blocks [first, first+n): a contiguous range because slots ascend with j.
+static void slot_range(const LayerMap& m, uint32_t i, uint32_t first, uint32_t n, uint32_t* lo, uint32_t* hi) {
+  const auto b = m.order.begin() + m.start[i], e = b + m.counts[i];
+  *lo = static_cast<uint32_t>(std::lower_bound(b, e, first) - b);
+  *hi = static_cast<uint32_t>(std::lower_bound(b, e, first + n) - b);
+}
+
+int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks, void* k_base,
+                          void* v_base, uint64_t stride, const int32_t* table, void* cuda_stream) {
   int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
   if (rc != KVPOOL_OK) return rc;
   LayerState& L = pl->layers[layer];
+  if (static_cast<uint64_t>(first_block) + n_blocks > L.map->K)
+    return fail(KVPOOL_EINVAL, "retrieve: blocks [%u, %u) exceed the layer's %llu blocks", first_block, first_block + n_blocks,
+                (unsigned long long)L.map->K);
   if (!L.offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", layer);
-  if (L.map->K == 0) return KVPOOL_OK;
+  if (n_blocks == 0) return KVPOOL_OK;
   DeviceGuard guard(p->cuda_device);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const uint32_t N = p->n;
   LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
+  a.j0 = first_block;
+  a.K = n_blocks;
+  const uint64_t range_bytes = static_cast<uint64_t>(n_blocks) * p->payload;
+  const bool staged = p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && range_bytes >= p->tune.auto_threshold_bytes);
 
-  if (!use_staged(p, L)) {
+  if (!staged) {
     for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
-    rc = launch_counted(p, a, false, true, s);
-    if (rc != KVPOOL_OK) return rc;
-    return KVPOOL_OK;
+    return launch_counted(p, a, false, true, s);
   }
 
-  // staged: one H2D copy per stripe on the per-device I/O streams (these may run ahead of `stream`),
-  // then the unpack kernel on `stream` once all of them have landed in the staging slot.
+  // staged: one H2D copy per stripe (only the slots the range touches) on the per-device I/O streams — these may run
+  // ahead of `stream` — then the unpack kernel on `stream` once all of them have landed in the staging slot.
   StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
+  uint32_t lo[KVPOOL_MAX_DEVICES], hi[KVPOOL_MAX_DEVICES];
   for (uint32_t i = 0; i < N; ++i) {
-    const uint64_t bytes = static_cast<uint64_t>(L.map->counts[i]) * p->payload;
-    if (bytes == 0) continue;
+    if (n_blocks == L.map->K) { lo[i] = 0; hi[i] = L.map->counts[i]; }
+    else slot_range(*L.map, i, first_block, n_blocks, &lo[i], &hi[i]);
+    if (hi[i] == lo[i]) continue;
     rc = wait_slot_free(p, slot, p->io[i]);
     if (rc != KVPOOL_OK) return rc;
     if (L.landed_pending) CU(cudaStreamWaitEvent(p->io[i], L.landed, 0));
   }
   for (uint32_t i = 0; i < N; ++i) {
-    const uint64_t bytes = static_cast<uint64_t>(L.map->counts[i]) * p->payload;
-    if (bytes == 0) continue;
-    CU(cudaMemcpyAsync(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload, static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i],
-                       bytes, cudaMemcpyHostToDevice, p->io[i]));
+    uint8_t* stage_i = slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload;   // same layout as a full layer
+    a.pool_base[i] = reinterpret_cast<uint64_t>(stage_i);
+    if (hi[i] == lo[i]) continue;
+    const uint64_t off = static_cast<uint64_t>(lo[i]) * p->payload, bytes = static_cast<uint64_t>(hi[i] - lo[i]) * p->payload;
+    CU(cudaMemcpyAsync(stage_i + off, static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i] + off, bytes, cudaMemcpyHostToDevice, p->io[i]));
     p->n_memcpys++;
     CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
     CU(cudaStreamWaitEvent(s, slot.copy_done[i], 0));
-    a.pool_base[i] = reinterpret_cast<uint64_t>(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload);
   }
   rc = launch_counted(p, a, false, false, s);
   if (rc != KVPOOL_OK) return rc;
   CU(cudaEventRecord(slot.kernel_done, s));
   return KVPOOL_OK;
+}
+
+int kvpool_retrieve(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
+                    const int32_t* table, void* cuda_stream) {
+  if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "retrieve: bad pool or placement");
+  if (layer >= p->geom.n_layers) return fail(KVPOOL_EINVAL, "layer %u out of range (n_layers %u)", layer, p->geom.n_layers);
+  return kvpool_retrieve_range(p, pl, layer, 0, static_cast<uint32_t>(pl->layers[layer].map->K), k_base, v_base, stride, table, cuda_stream);
 }
 
 int kvpool_wait_offloads(kvpool_t* p, kvpool_placement_t* pl, void* cuda_stream) {

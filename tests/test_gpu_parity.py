@@ -238,3 +238,47 @@ def test_full_size_configs_sampled_against_oracle(cfg):
         pl.release()
     finally:
         pool.destroy()
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+@pytest.mark.parametrize("path", ["staged", "zerocopy"])
+def test_retrieve_range_partial_and_prefix(path, kernel):
+    """kvpool_retrieve_range against the oracle's partial retrieval: prefix, middle, tail, empty and whole ranges."""
+    wl = W.make_workload(4, scale=1 / 16, n_layers=2)          # 512 of 768 blocks, 6 buffers 4:4:2:2:1:1
+    g, dev = wl.geom, torch.device("cuda:0")
+    bw = list(wl.default_weights())
+    pool = make_pool(wl)
+    try:
+        pool.set_path(PATHS[path])
+        pool.set_tuning(kernel=KERNELS[kernel], link_kernel=KERNELS[kernel])
+        pl = pool.place(wl.blocks_per_layer(0))
+        opl = oracle.place(bw, wl.blocks_per_layer(0))
+        rng = np.random.default_rng(13)
+        for l in range(g.n_layers):
+            table_np = np.ascontiguousarray(wl.layer_table(0, l))
+            K = len(table_np)
+            table = torch.from_numpy(table_np).to(dev)
+            src = W.kv_layer_torch(wl, l, dev)
+            src_cpu = W.kv_layer_numpy(wl, l)
+            with pytest.raises(kv.KvPoolError) as e:                               # not offloaded yet
+                pool.retrieve_range(pl, l, 0, 4, src[0], src[1], g.kvb, table)
+            assert e.value.code == kv.ESTATE
+            pool.offload(pl, l, src[0], src[1], g.kvb, table)
+            pool.wait_offloads(pl)
+            torch.cuda.synchronize()
+            stripes = oracle.offload_layer(src_cpu, table_np, opl[l])
+            ranges = [(0, K // 4), (K // 4, K // 2), (K - 1, 1), (0, K), (7, 0), (K, 0), (0, 1)]
+            ranges += [(int(a), int(b)) for a, b in ((rng.integers(0, K), rng.integers(0, 64)) for _ in range(6)) if a + b <= K]
+            for first, n in ranges:
+                dst = W.poison_torch((2, wl.nphys, g.kvb // 2), dev)
+                pool.retrieve_range(pl, l, first, n, dst[0], dst[1], g.kvb, table)
+                torch.cuda.synchronize()
+                want = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+                oracle.retrieve_range(want, table_np, opl[l], stripes, first, n)
+                assert np.array_equal(dst.cpu().numpy().view(np.uint16), want), (l, first, n)
+            with pytest.raises(kv.KvPoolError) as e:                               # range past the end
+                pool.retrieve_range(pl, l, K - 2, 3, src[0], src[1], g.kvb, table)
+            assert e.value.code == kv.EINVAL
+        pl.release()
+    finally:
+        pool.destroy()

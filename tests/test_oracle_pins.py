@@ -315,3 +315,34 @@ def test_empty_layer_is_a_noop():
     out = kv.copy()
     oracle.retrieve_layer(out, np.zeros(0, np.int32), pl, stripes)
     assert np.array_equal(out, kv)
+
+
+def test_retrieve_range_composes_and_touches_only_its_blocks():
+    """Partial retrieval: (0, K) is the full retrieve; disjoint ranges compose to it; a range equals numpy index
+    assignment of exactly its blocks; a prefix draws on every device within N-1 blocks of its share."""
+    rng = np.random.default_rng(11)
+    nphys, kvb, K = 120, 64, 90
+    kv = _tiny_layer(rng, nphys, kvb)
+    table = rng.permutation(nphys)[:K].astype(np.int32)
+    w = [4, 4, 2, 2, 1, 1]
+    pl = oracle.place(w, [K])[0]
+    stripes = oracle.offload_layer(kv, table, pl)
+    full = np.full_like(kv, 0x7FC1)
+    oracle.retrieve_layer(full, table, pl, stripes)
+    a = np.full_like(kv, 0x7FC1)
+    oracle.retrieve_range(a, table, pl, stripes, 0, K)
+    assert np.array_equal(a, full)
+    b = np.full_like(kv, 0x7FC1)
+    cuts = [0, 1, 17, 17, 50, 89, 90]
+    for lo, hi in zip(cuts[:-1], cuts[1:]):
+        oracle.retrieve_range(b, table, pl, stripes, lo, hi - lo)
+    assert np.array_equal(b, full)
+    for first, n in ((0, 23), (23, 40), (89, 1), (40, 0)):
+        c = np.full_like(kv, 0x7FC1)
+        oracle.retrieve_range(c, table, pl, stripes, first, n)
+        want = np.full_like(kv, 0x7FC1)
+        want[:, table[first:first + n]] = kv[:, table[first:first + n]]      # library routine on exactly the range
+        assert np.array_equal(c, want)
+        for i, wi in enumerate(w):                                            # every device serves its share of the range
+            took = int(np.sum(pl.dev[first:first + n] == i))
+            assert abs(took - Fraction(int(pl.counts[i]) * n, K)) <= len(w) - 1 + 1
