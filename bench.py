@@ -56,6 +56,10 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", choices=["hbm", "link"], default=None,
                     help="tuning sweep instead of the benchmark: in-device pack/unpack (hbm) or zero-copy transfer (link) GB/s over launch shapes")
+    ap.add_argument("--blocked-io", action="store_true",
+                    help="blocked-I/O-time analog (PAPER.md:70-72, Fig. 2/4): retrieve + consumer stand-in per layer, serial vs layerwise "
+                         "pipelined, over context lengths 1K..128K for the three model shapes")
+    ap.add_argument("--compute-us", type=float, default=0.0, help="--blocked-io: extra calibrated compute per layer (kvpool_spin), microseconds")
     ap.add_argument("--detail", default=None, help="write per-layer latencies and side measurements to this JSON file")
     return ap.parse_args()
 
@@ -606,6 +610,107 @@ def run_sweep(args) -> None:
     pool.destroy()
 
 
+def run_blocked_io(args) -> None:
+    """Blocked I/O time = time during which only KV retrieval proceeds, with no overlapping GPU computation.
+    Consumer stand-in per layer = kvpool_checksum over the layer's retrieved blocks (reads K_l*P bytes through the block
+    table, as decode attention does) plus an optional kvpool_spin.  Text table on stdout."""
+    import torch
+    from paper_2606_14779_b200 import binding as kv
+    from paper_2606_14779_b200 import workloads as W
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    spin_ns = int(args.compute_us * 1000)
+    print(f"# bench.py --blocked-io --compute-us {args.compute_us}: per-layer consumer = kvpool_checksum"
+          f"{' + kvpool_spin' if spin_ns else ''}; times in ms; blocked = total - consumer-alone (PAPER.md:72)")
+    print("# serial = retrieve(l); consume(l); host sync, layer by layer (Fig. 2a).  pipelined = all retrieves enqueued on one stream, "
+          "consume(l) on another after layer l's event (Fig. 2b)")
+    print(f"{'shape':22s} {'ctx':>7s} {'MiB':>8s} {'io_alone':>9s} {'consume':>8s} {'serial':>8s} {'blocked':>8s} {'pipelined':>9s} {'blocked':>8s} {'GB/s':>6s}")
+    rows = []
+    for cfg in (6, 3, 4):
+        for ctx in (1024, 4096, 16384, 32768, 65536, 131072):
+            wl = W.make_workload(cfg, scale=ctx / 131072)
+            g, L = wl.geom, wl.geom.n_layers
+            bw = list(wl.default_weights())
+            share = np.array(bw) / np.sum(bw)
+            moved = wl.moved_bytes()
+            caps = [int(moved * sh * 1.25) + (L + 4) * (g.payload + 4096) for sh in share]
+            pool = kv.KvPool(bw, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim)
+            bpl = wl.blocks_per_layer(0)
+            pl = pool.place(bpl)
+            elems = g.kvb // 2
+            src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+            dst = [W.poison_torch((2, wl.nphys, elems), dev) for l in range(L)]
+            tables = [torch.from_numpy(np.ascontiguousarray(wl.layer_table(0, l))).to(dev) for l in range(L)]
+            sa, sb = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+            sums = torch.zeros((3, L), dtype=torch.int64, device=dev)
+            for l in range(L):
+                pool.offload(pl, l, src[l][0], src[l][1], g.kvb, tables[l], sa)
+                pool.checksum(src[l][0], src[l][1], g.kvb, tables[l], int(bpl[l]), sums[0, l:l + 1], sa)
+            pool.wait_offloads(pl, sa)
+            sa.synchronize()
+
+            def consume(l, row, stream):
+                pool.checksum(dst[l][0], dst[l][1], g.kvb, tables[l], int(bpl[l]), sums[row, l:l + 1], stream)
+                if spin_ns:
+                    pool.spin(spin_ns, stream)
+
+            def wall(fn, reps=3):
+                ts = []
+                for _ in range(reps):
+                    torch.cuda.synchronize()
+                    pool.synchronize()
+                    t0 = time.perf_counter()
+                    fn()
+                    torch.cuda.synchronize()
+                    ts.append(1e3 * (time.perf_counter() - t0))
+                return statistics.median(ts)
+
+            def io_alone():
+                for l in range(L):
+                    pool.retrieve(pl, l, dst[l][0], dst[l][1], g.kvb, tables[l], sa)
+
+            def consume_alone():
+                sums[1].zero_()
+                for l in range(L):
+                    consume(l, 1, sb)
+
+            def serial():
+                sums[1].zero_()
+                for l in range(L):
+                    pool.retrieve(pl, l, dst[l][0], dst[l][1], g.kvb, tables[l], sa)
+                    consume(l, 1, sa)
+                    sa.synchronize()
+
+            def pipelined():
+                sums[2].zero_()
+                for l in range(L):
+                    pool.retrieve(pl, l, dst[l][0], dst[l][1], g.kvb, tables[l], sa)
+                    e = torch.cuda.Event()
+                    e.record(sa)
+                    sb.wait_event(e)
+                    consume(l, 2, sb)
+
+            t_io, t_c = wall(io_alone), wall(consume_alone)
+            t_ser, t_pipe = wall(serial), wall(pipelined)
+            torch.cuda.synchronize()
+            ok = bool(torch.equal(sums[0], sums[1]) and torch.equal(sums[0], sums[2]))
+            if not ok:
+                raise RuntimeError(f"checksum of retrieved KV differs from the source (cfg {cfg}, ctx {ctx})")
+            row = {"shape": wl.name.split("@")[0], "ctx": ctx, "mib": moved / 2**20, "io_alone_ms": t_io, "consume_ms": t_c, "serial_ms": t_ser,
+                   "serial_blocked_ms": t_ser - t_c, "pipelined_ms": t_pipe, "pipelined_blocked_ms": t_pipe - t_c, "pipelined_gbps": moved / t_pipe / 1e6}
+            rows.append(row)
+            print(f"{row['shape']:22s} {ctx:7d} {row['mib']:8.0f} {t_io:9.3f} {t_c:8.3f} {t_ser:8.3f} {t_ser - t_c:8.3f} {t_pipe:9.3f} {t_pipe - t_c:8.3f} "
+                  f"{row['pipelined_gbps']:6.2f}", flush=True)
+            pl.release()
+            pool.destroy()
+            del src, dst
+            torch.cuda.empty_cache()
+    if args.detail:
+        with open(args.detail, "w") as f:
+            json.dump(rows, f, indent=1)
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -613,6 +718,9 @@ def main():
         return
     if args.sweep:
         run_sweep(args)
+        return
+    if args.blocked_io:
+        run_blocked_io(args)
         return
     out = run_kvpool(args)
     if out is None:

@@ -171,6 +171,17 @@ KVPOOL_API int kvpool_pack(kvpool_t* pool, kvpool_placement_t* pl, uint32_t laye
 KVPOOL_API int kvpool_unpack(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base,
                   uint64_t block_stride_bytes, const int32_t* block_table_dev, const void* stage_dev, void* cuda_stream);
 
+/* Consumer stand-in and integrity check (the "GPU computation" box of Fig. 2, for pipeline
+ * experiments; not part of the paper's method).  Adds to *sum_dev (device uint64, caller zeroes it) the checksum
+ *     sum over logical blocks j < n_blocks, halves h (0 = K, 1 = V), 64-bit little-endian words i of
+ *         word(j, h, i) * (2*idx + 1)   mod 2^64,      idx = (j*2 + h)*(kvb/8) + i
+ * of the paged blocks named by block_table_dev, reading them through the table as decode attention would
+ * (n_blocks*P bytes of HBM reads).  kvb must be a multiple of 16.  Ordered on `stream`.                          */
+KVPOOL_API int kvpool_checksum(kvpool_t* pool, const void* k_base /*device*/, const void* v_base /*device*/, uint64_t block_stride_bytes,
+                    const int32_t* block_table_dev, uint32_t n_blocks, uint64_t* sum_dev /*device*/, void* cuda_stream);
+/* Occupy `stream` for `nanoseconds` with a one-thread kernel (calibrated compute stand-in).                        */
+KVPOOL_API int kvpool_spin(kvpool_t* pool, uint64_t nanoseconds, void* cuda_stream);
+
 /* ---- introspection (GLT, Table I) -----------------------------------------------------------------------*/
 KVPOOL_API int kvpool_n_devices(const kvpool_t* pool, uint32_t* n_out);
 KVPOOL_API int kvpool_weights(const kvpool_t* pool, uint64_t* w_out /*host[n_devs]*/);

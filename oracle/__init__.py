@@ -49,6 +49,8 @@ def _load():
             f.argtypes = [vp, vp, u64, u64, vp, u64, vp, vp, vp]
         lib.orc_retrieve_range.restype = None
         lib.orc_retrieve_range.argtypes = [vp, vp, u64, u64, vp, u64, u64, vp, vp, vp]
+        lib.orc_checksum.restype = u64
+        lib.orc_checksum.argtypes = [vp, vp, u64, u64, vp, u64]
         lib.orc_layer_parallel.restype = ctypes.c_int
         lib.orc_layer_parallel.argtypes = [ctypes.c_int, vp, vp, u64, u64, vp, u64, vp, vp, vp, u32]
         _lib = lib
@@ -164,3 +166,10 @@ def retrieve_range(kv_layer_out: np.ndarray, table: np.ndarray, pl: LayerPlaceme
     assert 0 <= first and first + n <= table.shape[0]
     ptrs = _stripe_ptrs(stripes)
     _load().orc_retrieve_range(kp, vp_, stride, kvb, _ptr(table), int(first), int(n), _ptr(pl.dev), _ptr(pl.slot), ctypes.addressof(ptrs))
+
+
+def checksum(kv_layer: np.ndarray, table: np.ndarray) -> int:
+    """Position-weighted 64-bit checksum of the blocks table[0..n) of one layer (see orc_checksum)."""
+    kp, vp_, stride, kvb = _planes(kv_layer)
+    table = np.ascontiguousarray(table, dtype=np.int32)
+    return int(_load().orc_checksum(kp, vp_, stride, kvb, _ptr(table), table.shape[0]))

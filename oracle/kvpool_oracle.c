@@ -21,6 +21,8 @@
  *                             reduces to memcpy, O(K^2) brute-force search, round trip, conservation
  *   orc_retrieve_range      — (0, K) equals orc_retrieve_layer; disjoint ranges compose to the full retrieve; numpy
  *                             index assignment on the range; nothing outside the range's physical blocks is written
+ *   orc_checksum            — closed form n_words^2 * c for constant words, python big-int restatement, sensitivity
+ *                             to swapping two blocks
  *   stripe offsets inside a pool buffer: PARITY UNPINNED (implementation detail; not produced here).
  *
  * Build: gcc -O2 -shared -fPIC -pthread -o liboracle.so kvpool_oracle.c   (oracle/__init__.py does it)
@@ -155,6 +157,26 @@ void orc_retrieve_range(uint8_t *k_plane, uint8_t *v_plane, uint64_t stride, uin
         memcpy(k_plane + (uint64_t)table[j] * stride, src, kvb);
         memcpy(v_plane + (uint64_t)table[j] * stride, src + kvb, kvb);
     }
+}
+
+/* ---- consumer stand-in checksum (not in the paper; defined in include-free words here) ---------------
+ * sum over logical blocks j < n, halves h (0 = K block, 1 = V block), 64-bit little-endian words i of
+ *     word(j,h,i) * (2*idx + 1)  mod 2^64,   idx = (j*2 + h)*(kvb/8) + i
+ * where the blocks are read through the table: physical block table[j].  Order-independent (a sum),
+ * position-sensitive (odd multipliers), so any misplaced, swapped or stale block changes it. */
+uint64_t orc_checksum(const uint8_t *k_plane, const uint8_t *v_plane, uint64_t stride, uint64_t kvb,
+                      const int32_t *table, uint64_t n) {
+    uint64_t sum = 0, words = kvb / 8;
+    for (uint64_t j = 0; j < n; ++j)
+        for (uint64_t h = 0; h < 2; ++h) {
+            const uint8_t *blk = (h ? v_plane : k_plane) + (uint64_t)table[j] * stride;
+            for (uint64_t i = 0; i < words; ++i) {
+                uint64_t w;
+                memcpy(&w, blk + 8 * i, 8);
+                sum += w * (2 * ((j * 2 + h) * words + i) + 1);
+            }
+        }
+    return sum;
 }
 
 /* ---- "for all u_i in U in parallel" (Alg. 1 l.17; "each pool device has its own worker thread",

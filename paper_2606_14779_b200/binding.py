@@ -25,7 +25,7 @@ _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA",
 EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
     "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_place", "kvpool_release",
-    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack",
+    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_counts", "kvpool_lookup", "kvpool_stripe",
     "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_last_error", "kvpool_version",
 ]
@@ -85,6 +85,8 @@ def lib():
             "kvpool_synchronize": [vp],
             "kvpool_pack": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp, vp],
             "kvpool_unpack": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp, vp],
+            "kvpool_checksum": [vp, vp, vp, c_uint64, vp, c_uint32, vp, vp],
+            "kvpool_spin": [vp, c_uint64, vp],
             "kvpool_n_devices": [vp, POINTER(c_uint32)],
             "kvpool_weights": [vp, vp],
             "kvpool_device_info": [vp, c_uint32, POINTER(vp), POINTER(c_uint64), POINTER(c_uint64), POINTER(c_int32)],
@@ -267,6 +269,13 @@ class KvPool:
     def unpack(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_dev, stage_dev, stream=None) -> None:
         _ck(lib().kvpool_unpack(self.handle, pl.handle, layer, _addr(k_base), _addr(v_base), block_stride_bytes,
                                 _addr(block_table_dev), _addr(stage_dev), _stream(stream)))
+
+    def checksum(self, k_base, v_base, block_stride_bytes: int, block_table_dev, n_blocks: int, sum_dev, stream=None) -> None:
+        _ck(lib().kvpool_checksum(self.handle, _addr(k_base), _addr(v_base), block_stride_bytes, _addr(block_table_dev), n_blocks,
+                                  _addr(sum_dev), _stream(stream)))
+
+    def spin(self, nanoseconds: int, stream=None) -> None:
+        _ck(lib().kvpool_spin(self.handle, int(nanoseconds), _stream(stream)))
 
     def wait_offloads(self, pl: Placement, stream=None) -> None:
         _ck(lib().kvpool_wait_offloads(self.handle, pl.handle, _stream(stream)))

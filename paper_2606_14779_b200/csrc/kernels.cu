@@ -161,6 +161,49 @@ __global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Laye
   bulk_wait_all();
 }
 
+// ---- consumer stand-in: position-weighted 64-bit checksum of the blocks named by a table ---------------------------
+__global__ void __launch_bounds__(256) kv_checksum(const uint8_t* __restrict__ k_base, const uint8_t* __restrict__ v_base, uint64_t stride,
+                                                   const int32_t* __restrict__ table, uint32_t n_blocks, uint32_t kvb,
+                                                   unsigned long long* __restrict__ out) {
+  constexpr uint32_t kUnroll = 4, kPiece = kUnroll * 512;   // 2 KiB per warp iteration, 16 B per lane per load
+  const uint32_t lane = threadIdx.x & 31u, warps_per_cta = blockDim.x >> 5;
+  const uint64_t nwarps = static_cast<uint64_t>(gridDim.x) * warps_per_cta;
+  const uint32_t pieces = (kvb + kPiece - 1) / kPiece, words_per_half = kvb / 8;
+  const uint64_t total = static_cast<uint64_t>(n_blocks) * 2u * pieces;
+  unsigned long long acc = 0;
+  for (uint64_t t = static_cast<uint64_t>(blockIdx.x) * warps_per_cta + (threadIdx.x >> 5); t < total; t += nwarps) {
+    const uint32_t j = static_cast<uint32_t>(t / (2u * pieces));
+    const uint32_t r = static_cast<uint32_t>(t - static_cast<uint64_t>(j) * 2u * pieces);
+    const uint32_t half = r >= pieces ? 1u : 0u, c = r - half * pieces;
+    const uint8_t* src = (half ? v_base : k_base) + static_cast<uint64_t>(__ldg(table + j)) * stride + c * kPiece + lane * 16u;
+    const uint32_t left = kvb - c * kPiece;
+    const uint64_t idx0 = (static_cast<uint64_t>(j) * 2u + half) * words_per_half + (c * kPiece + lane * 16u) / 8u;
+    int4 v[kUnroll];
+#pragma unroll
+    for (uint32_t u = 0; u < kUnroll; ++u)
+      if (u * 512u + lane * 16u < left) v[u] = ld_stream(src + u * 512u);
+#pragma unroll
+    for (uint32_t u = 0; u < kUnroll; ++u)
+      if (u * 512u + lane * 16u < left) {
+        const unsigned long long w0 = (static_cast<unsigned long long>(static_cast<uint32_t>(v[u].y)) << 32) | static_cast<uint32_t>(v[u].x);
+        const unsigned long long w1 = (static_cast<unsigned long long>(static_cast<uint32_t>(v[u].w)) << 32) | static_cast<uint32_t>(v[u].z);
+        const unsigned long long idx = idx0 + u * 64u;
+        acc += w0 * (2ull * idx + 1ull) + w1 * (2ull * idx + 3ull);
+      }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (lane == 0 && acc != 0) atomicAdd(out, acc);
+}
+
+__global__ void kv_spin(uint64_t ns) {
+  uint64_t t0, t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+  do {
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  } while (t - t0 < ns);
+}
+
 uint32_t bulk_chunk_for(uint32_t kvb, uint32_t want) {
   uint32_t c = 16;
   while (c * 2 <= want && kvb % (c * 2) == 0) c *= 2;
@@ -173,6 +216,20 @@ cudaError_t kernels_init() {
   cudaError_t e = cudaFuncSetAttribute(kv_copy_bulk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(kv_copy_bulk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+}
+
+cudaError_t launch_checksum(const uint8_t* k_base, const uint8_t* v_base, uint64_t stride, const int32_t* table, uint32_t n_blocks,
+                            uint32_t kvb, unsigned long long* out, uint32_t ctas, cudaStream_t stream) {
+  if (n_blocks == 0) return cudaSuccess;
+  const uint64_t total = static_cast<uint64_t>(n_blocks) * 2u * ((kvb + 2047u) / 2048u);
+  const uint64_t want = (total + 7) / 8;
+  kv_checksum<<<static_cast<uint32_t>(want < ctas ? want : ctas), 256, 0, stream>>>(k_base, v_base, stride, table, n_blocks, kvb, out);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_spin(uint64_t ns, cudaStream_t stream) {
+  kv_spin<<<1, 1, 0, stream>>>(ns);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream) {

@@ -36,6 +36,13 @@ struct LaunchCfg {
 
 // pack = true: paged -> pool side (offload direction); false: pool side -> paged (retrieve direction).
 cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream);
+// Consumer stand-in / integrity check: *out += sum over logical blocks j < n, halves h (0 = K, 1 = V) and 64-bit
+// words i of  word * (2*idx + 1)  (mod 2^64),  idx = (j*2 + h)*(kvb/8) + i.  Reads the blocks through the table
+// exactly as a decode-attention kernel would (K_l*P bytes of HBM reads); `out` must be zeroed by the caller.
+cudaError_t launch_checksum(const uint8_t* k_base, const uint8_t* v_base, uint64_t stride, const int32_t* table, uint32_t n_blocks,
+                            uint32_t kvb, unsigned long long* out, uint32_t ctas, cudaStream_t stream);
+// One thread spins on %globaltimer for `ns` nanoseconds: a calibrated compute stand-in for pipeline experiments.
+cudaError_t launch_spin(uint64_t ns, cudaStream_t stream);
 // One-time per-device setup (shared-memory opt-in for the bulk kernels).
 cudaError_t kernels_init();
 

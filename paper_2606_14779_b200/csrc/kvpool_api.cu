@@ -779,6 +779,31 @@ int kvpool_unpack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_b
   return launch_counted(p, a, false, false, static_cast<cudaStream_t>(cuda_stream));
 }
 
+int kvpool_checksum(kvpool_t* p, const void* k_base, const void* v_base, uint64_t stride, const int32_t* table, uint32_t n_blocks,
+                    uint64_t* sum_dev, void* cuda_stream) {
+  if (!p || !sum_dev) return fail(KVPOOL_EINVAL, "checksum: null argument");
+  if (n_blocks == 0) return KVPOOL_OK;
+  if (!k_base || !v_base || !table) return fail(KVPOOL_EINVAL, "checksum: null k_base / v_base / block table");
+  if ((reinterpret_cast<uintptr_t>(k_base) | reinterpret_cast<uintptr_t>(v_base) | stride) & 15u)
+    return fail(KVPOOL_EINVAL, "checksum: k_base, v_base and block_stride_bytes must be multiples of 16");
+  if (reinterpret_cast<uintptr_t>(sum_dev) & 7u) return fail(KVPOOL_EINVAL, "checksum: sum_dev must be 8-byte aligned");
+  DeviceGuard guard(p->cuda_device);
+  CU(launch_checksum(static_cast<const uint8_t*>(k_base), static_cast<const uint8_t*>(v_base), stride, table, n_blocks,
+                     static_cast<uint32_t>(p->kvb), reinterpret_cast<unsigned long long*>(sum_dev), p->tune.hbm_ctas,
+                     static_cast<cudaStream_t>(cuda_stream)));
+  p->n_kernels++;
+  return KVPOOL_OK;
+}
+
+int kvpool_spin(kvpool_t* p, uint64_t ns, void* cuda_stream) {
+  if (!p) return fail(KVPOOL_EINVAL, "spin: null pool");
+  if (ns > 10ull * 1000 * 1000 * 1000) return fail(KVPOOL_EINVAL, "spin: more than 10 s");
+  DeviceGuard guard(p->cuda_device);
+  CU(launch_spin(ns, static_cast<cudaStream_t>(cuda_stream)));
+  p->n_kernels++;
+  return KVPOOL_OK;
+}
+
 // ---------------------------------------------------------------------------------------------------
 // introspection
 // ---------------------------------------------------------------------------------------------------

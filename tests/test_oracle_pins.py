@@ -346,3 +346,30 @@ def test_retrieve_range_composes_and_touches_only_its_blocks():
         for i, wi in enumerate(w):                                            # every device serves its share of the range
             took = int(np.sum(pl.dev[first:first + n] == i))
             assert abs(took - Fraction(int(pl.counts[i]) * n, K)) <= len(w) - 1 + 1
+
+
+def test_checksum_closed_form_python_restatement_and_sensitivity():
+    rng = np.random.default_rng(12)
+    nphys, kvb, n = 19, 48, 11
+    # constant words c: sum_idx c*(2*idx+1) = c * n_words^2
+    c = 0x0123456789ABCDEF
+    kv = np.full((2, nphys, kvb // 2), 0, dtype=np.uint16)
+    kv.view(np.uint64)[...] = c
+    table = rng.permutation(nphys)[:n].astype(np.int32)
+    n_words = n * 2 * (kvb // 8)
+    assert oracle.checksum(kv, table) == (c * n_words * n_words) % 2 ** 64
+    # python big-int restatement on random data
+    kv = _tiny_layer(rng, nphys, kvb)
+    want, idx = 0, 0
+    for j in range(n):
+        for h in range(2):
+            for w in kv[h, table[j]].view(np.uint64):
+                want += int(w) * (2 * idx + 1)
+                idx += 1
+    assert oracle.checksum(kv, table) == want % 2 ** 64
+    # swapping two table entries (two blocks trade places) or K with V changes it; an empty table sums to 0
+    t2 = table.copy()
+    t2[[0, 5]] = t2[[5, 0]]
+    assert oracle.checksum(kv, t2) != oracle.checksum(kv, table)
+    assert oracle.checksum(np.ascontiguousarray(kv[::-1]), table) != oracle.checksum(kv, table)
+    assert oracle.checksum(kv, table[:0]) == 0
