@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--link-ctas", type=int, default=0)
     ap.add_argument("--hbm-ctas", type=int, default=0)
     ap.add_argument("--stage-slots", type=int, default=0)
+    ap.add_argument("--per-layer", action="store_true",
+                    help="issue one kvpool_offload / kvpool_retrieve call per layer in the timed step instead of the batched *_layers calls")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", choices=["hbm", "link"], default=None,
                     help="tuning sweep instead of the benchmark: in-device pack/unpack (hbm) or zero-copy transfer (link) GB/s over launch shapes")
@@ -296,17 +298,29 @@ def run_kvpool(args) -> dict:
                 e.record(s)
                 main.wait_event(e)
 
+    src_k, src_v = [x[0] for x in src], [x[1] for x in src]
+    dst_k, dst_v = [x[0] for x in dst], [x[1] for x in dst]
+
     def do_offload(pls):
         fork()
-        for l in range(L):
+        if args.per_layer:
+            for l in range(L):
+                for r in range(R):
+                    pool.offload(pls[r], l, src[l][0], src[l][1], g.kvb, tables[r][l], streams[r % len(streams)])
+        else:
             for r in range(R):
-                pool.offload(pls[r], l, src[l][0], src[l][1], g.kvb, tables[r][l], streams[r % len(streams)])
+                pool.offload_layers(pls[r], 0, src_k, src_v, g.kvb, tables[r], streams[r % len(streams)])
         for r in range(R):
             pool.wait_offloads(pls[r], streams[r % len(streams)])
         join()
 
     def do_retrieve(pls, layer_events=None, upload_tables=False):
         fork()
+        if layer_events is None and not upload_tables and not args.per_layer:
+            for r in range(R):
+                pool.retrieve_layers(pls[r], 0, dst_k, dst_v, g.kvb, tables[r], streams[r % len(streams)])
+            join()
+            return
         for l in range(L):
             for r in range(R):
                 s = streams[r % len(streams)]
@@ -515,7 +529,8 @@ def run_kvpool(args) -> dict:
                    "link_kernel": "vec16" if tn.link_kernel == kv.KERNEL_VEC16 else "bulk",
                    "link_ctas": tn.link_ctas, "hbm_ctas": tn.hbm_ctas, "stage_slots": tn.stage_slots, "streams": len(streams),
                    "l2": f"inputs larger than L2: each leg moves {moved / 2**30:.1f} GiB through {L} distinct layers (L2 is 126 MB); no flush needed",
-                   "step": "kvpool_place + kvpool_offload x layers + kvpool_retrieve x layers; value = retrieve leg"},
+                   "calls": "per-layer" if args.per_layer else "batched (kvpool_offload_layers / kvpool_retrieve_layers, one call per request)",
+                   "step": "kvpool_place + offload of every layer + retrieve of every layer; value = retrieve leg"},
         "retrieve_ms_per_step": ret_ms, "offload_ms_per_step": off_ms, "offload_gbps": world * moved / (off_ms * 1e6),
         "place_ms_per_step": statistics.mean(rec["place_ms"]), "verified_bit_exact_round_trip": verified,
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": moved + table_bytes, "d2h_bytes_per_step": d2h_bytes,

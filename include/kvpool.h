@@ -150,6 +150,18 @@ KVPOOL_API int kvpool_offload(kvpool_t* pool, kvpool_placement_t* pl, uint32_t l
                    void* cuda_stream);
 KVPOOL_API int kvpool_retrieve(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, void* k_base /*device*/, void* v_base /*device*/,
                     uint64_t block_stride_bytes, const int32_t* block_table_dev, void* cuda_stream);
+/* Batched forms: layers [first_layer, first_layer + n_layers) in one call, equivalent to the per-layer calls in
+ * ascending order.  k_bases / v_bases / block_tables are HOST arrays of n_layers DEVICE pointers (entries of layers
+ * with K_l = 0 may be NULL).  Consecutive layers that take the zero-copy path are fused into single kernel launches
+ * (up to 64 layers each): a request made of small layers pays one launch latency and one pipeline ramp instead of
+ * one per layer (the launch-latency regime of 1K-token contexts and sliding-window layers).  All arguments are
+ * validated before anything is enqueued.                                                                            */
+KVPOOL_API int kvpool_offload_layers(kvpool_t* pool, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers,
+                          const void* const* k_bases /*host[n_layers]*/, const void* const* v_bases /*host[n_layers]*/,
+                          uint64_t block_stride_bytes, const int32_t* const* block_tables /*host[n_layers]*/, void* cuda_stream);
+KVPOOL_API int kvpool_retrieve_layers(kvpool_t* pool, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers,
+                           void* const* k_bases /*host[n_layers]*/, void* const* v_bases /*host[n_layers]*/,
+                           uint64_t block_stride_bytes, const int32_t* const* block_tables /*host[n_layers]*/, void* cuda_stream);
 /* Partial retrieval (prefix reuse, chunked prefetch): like kvpool_retrieve for logical blocks
  * [first_block, first_block + n_blocks) of the layer only.  block_table_dev is still the LAYER's table (indexed by
  * logical block, as at offload); only the entries of the range are read and only their physical blocks written.

@@ -58,14 +58,41 @@ __device__ __forceinline__ Piece decode(const LayerArgs& a, uint64_t t, uint32_t
   return p;
 }
 
-template <bool PACK, int kVecUnroll>
-__global__ void __launch_bounds__(kVecMaxThreads) kv_copy_vec16(const __grid_constant__ LayerArgs a) {
+__device__ __forceinline__ Piece decode(const MultiArgs& a, uint64_t t, uint32_t pieces, uint32_t piece_bytes) {
+  const uint32_t per_unit = 2u * pieces;
+  const uint32_t unit = static_cast<uint32_t>(t / per_unit);
+  const uint32_t r = static_cast<uint32_t>(t - static_cast<uint64_t>(unit) * per_unit);
+  uint32_t lo = 0, hi = a.n;  // last layer with first_unit <= unit
+  while (hi - lo > 1) {
+    const uint32_t mid = (lo + hi) >> 1;
+    if (a.d[mid].first_unit <= unit) lo = mid;
+    else hi = mid;
+  }
+  const MultiDesc& L = a.d[lo];
+  const uint32_t j = unit - L.first_unit;
+  const uint32_t half = r >= pieces ? 1u : 0u;
+  const uint32_t c = r - half * pieces;
+  const int32_t phys = __ldg(L.table + j);
+  const uint32_t d = __ldg(L.dev + j);
+  const uint32_t s = __ldg(L.slot + j);
+  const uint32_t off = c * piece_bytes;
+  Piece p;
+  p.paged = (half ? L.v_base : L.k_base) + static_cast<uint64_t>(phys) * a.stride + off;
+  p.pooled = reinterpret_cast<uint8_t*>(__ldg(L.pool_base + d)) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;
+  p.bytes = min(piece_bytes, a.kvb - off);
+  return p;
+}
+__device__ __forceinline__ uint32_t units(const LayerArgs& a) { return a.K; }
+__device__ __forceinline__ uint32_t units(const MultiArgs& a) { return a.total_units; }
+
+template <bool PACK, int kVecUnroll, class Args>
+__global__ void __launch_bounds__(kVecMaxThreads) kv_copy_vec16(const __grid_constant__ Args a) {
   constexpr uint32_t kVecPiece = kVecUnroll * 32 * 16;  // bytes per warp iteration (4 KiB at unroll 8)
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t warps_per_cta = blockDim.x >> 5;
   const uint64_t nwarps = static_cast<uint64_t>(gridDim.x) * warps_per_cta;
   const uint32_t pieces = (a.kvb + kVecPiece - 1) / kVecPiece;
-  const uint64_t total = static_cast<uint64_t>(a.K) * 2u * pieces;
+  const uint64_t total = static_cast<uint64_t>(units(a)) * 2u * pieces;
   for (uint64_t t = static_cast<uint64_t>(blockIdx.x) * warps_per_cta + (threadIdx.x >> 5); t < total; t += nwarps) {
     const Piece p = decode(a, t, pieces, kVecPiece);
     const uint8_t* src = (PACK ? p.paged : p.pooled) + lane * 16u;
@@ -122,8 +149,8 @@ __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wa
 
 // Each warp's lane 0 owns `stages` shared-memory buffers of `chunk` bytes and walks its share of the
 // layer's chunks: up to stages-1 loads are in flight while the oldest landed chunk is stored out.
-template <bool PACK>
-__global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ LayerArgs a, uint32_t chunk, uint32_t stages) {
+template <bool PACK, class Args>
+__global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Args a, uint32_t chunk, uint32_t stages) {
   extern __shared__ __align__(128) uint8_t smem[];
   if ((threadIdx.x & 31u) != 0) return;
   const uint32_t warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
@@ -133,7 +160,7 @@ __global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Laye
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 
   const uint32_t pieces = a.kvb / chunk;  // host guarantees chunk | kvb
-  const uint64_t total = static_cast<uint64_t>(a.K) * 2u * pieces;
+  const uint64_t total = static_cast<uint64_t>(units(a)) * 2u * pieces;
   const uint64_t gw = static_cast<uint64_t>(blockIdx.x) * nw + warp, ngw = static_cast<uint64_t>(gridDim.x) * nw;
   const uint64_t mine = gw < total ? (total - gw + ngw - 1) / ngw : 0;
 
@@ -213,9 +240,11 @@ uint32_t bulk_chunk_for(uint32_t kvb, uint32_t want) {
 }  // namespace
 
 cudaError_t kernels_init() {
-  cudaError_t e = cudaFuncSetAttribute(kv_copy_bulk<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(kv_copy_bulk<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  cudaError_t e = cudaFuncSetAttribute(kv_copy_bulk<true, LayerArgs>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(kv_copy_bulk<false, LayerArgs>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(kv_copy_bulk<true, MultiArgs>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(kv_copy_bulk<false, MultiArgs>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  return e;
 }
 
 cudaError_t launch_checksum(const uint8_t* k_base, const uint8_t* v_base, uint64_t stride, const int32_t* table, uint32_t n_blocks,
@@ -232,14 +261,15 @@ cudaError_t launch_spin(uint64_t ns, cudaStream_t stream) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream) {
-  if (a.K == 0) return cudaSuccess;
+template <class Args>
+static cudaError_t launch_copy(const Args& a, uint32_t n_units, bool pack, const LaunchCfg& cfg, cudaStream_t stream) {
+  if (n_units == 0) return cudaSuccess;
   if (cfg.kernel == KVPOOL_KERNEL_BULK) {
     const uint32_t chunk = bulk_chunk_for(a.kvb, cfg.bulk_chunk);
     const uint32_t stages = cfg.bulk_stages < 2 ? 2 : (cfg.bulk_stages > 8 ? 8 : cfg.bulk_stages);
     uint32_t warps = cfg.bulk_warps < 1 ? 1 : (cfg.bulk_warps > 8 ? 8 : cfg.bulk_warps);
     while (warps > 1 && static_cast<uint64_t>(warps) * stages * chunk + kBulkBarrierBytes > 200u * 1024u) --warps;
-    const uint64_t total = static_cast<uint64_t>(a.K) * 2u * (a.kvb / chunk);
+    const uint64_t total = static_cast<uint64_t>(n_units) * 2u * (a.kvb / chunk);
     const uint64_t want = (total + warps - 1) / warps;
     const size_t smem = kBulkBarrierBytes + static_cast<size_t>(warps) * stages * chunk;
     // persistent ring: never launch more CTAs than are co-resident (shared memory bounds CTAs per SM)
@@ -247,20 +277,20 @@ cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cf
     const uint64_t resident = static_cast<uint64_t>(cfg.sm_count ? cfg.sm_count : 148u) * (per_sm > 32 ? 32 : per_sm);
     uint64_t cap = cfg.ctas < resident ? cfg.ctas : resident;
     const uint32_t grid = static_cast<uint32_t>(want < cap ? want : cap);
-    if (pack) kv_copy_bulk<true><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
-    else kv_copy_bulk<false><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
+    if (pack) kv_copy_bulk<true, Args><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
+    else kv_copy_bulk<false, Args><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
   } else {
     const uint32_t unroll = cfg.vec_unroll == 4 ? 4 : (cfg.vec_unroll == 16 ? 16 : 8);
     const uint32_t threads = cfg.vec_threads ? cfg.vec_threads : kVecMaxThreads;
     const uint32_t piece = unroll * 512;
     const uint32_t pieces = (a.kvb + piece - 1) / piece;
-    const uint64_t total = static_cast<uint64_t>(a.K) * 2u * pieces;
+    const uint64_t total = static_cast<uint64_t>(n_units) * 2u * pieces;
     const uint64_t want = (total + (threads / 32) - 1) / (threads / 32);
     const uint32_t grid = static_cast<uint32_t>(want < cfg.ctas ? want : cfg.ctas);
-#define KV_LAUNCH_VEC(U)                                                       \
-  do {                                                                         \
-    if (pack) kv_copy_vec16<true, U><<<grid, threads, 0, stream>>>(a);         \
-    else kv_copy_vec16<false, U><<<grid, threads, 0, stream>>>(a);             \
+#define KV_LAUNCH_VEC(U)                                                             \
+  do {                                                                               \
+    if (pack) kv_copy_vec16<true, U, Args><<<grid, threads, 0, stream>>>(a);         \
+    else kv_copy_vec16<false, U, Args><<<grid, threads, 0, stream>>>(a);             \
   } while (0)
     if (unroll == 4) KV_LAUNCH_VEC(4);
     else if (unroll == 16) KV_LAUNCH_VEC(16);
@@ -268,6 +298,14 @@ cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cf
 #undef KV_LAUNCH_VEC
   }
   return cudaGetLastError();
+}
+
+cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream) {
+  return launch_copy(a, a.K, pack, cfg, stream);
+}
+
+cudaError_t launch_multi_copy(const MultiArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream) {
+  return launch_copy(a, a.total_units, pack, cfg, stream);
 }
 
 }  // namespace kvp

@@ -26,6 +26,29 @@ struct LayerArgs {
   uint64_t pool_base[kMaxDev];
 };
 
+// Several layers in one launch (tiny layers: one launch latency and one pipeline ramp for the whole batch).  Units are
+// numbered across the batch; layer i owns units [first_unit, first_unit + K).  pool_base points at N device-visible
+// stripe addresses in global memory (uploaded once per placement).
+constexpr uint32_t kMaxBatch = 64;
+struct MultiDesc {
+  uint8_t* k_base;
+  uint8_t* v_base;
+  const int32_t* table;
+  const uint8_t* dev;
+  const uint32_t* slot;
+  const uint64_t* pool_base;
+  uint32_t K;
+  uint32_t first_unit;
+};
+struct MultiArgs {
+  uint64_t stride;
+  uint32_t kvb;
+  uint32_t n;            // layers in this launch, <= kMaxBatch
+  uint32_t total_units;  // sum of K
+  uint32_t pad;
+  MultiDesc d[kMaxBatch];
+};
+
 struct LaunchCfg {
   uint32_t kernel;       // KVPOOL_KERNEL_VEC16 / KVPOOL_KERNEL_BULK
   uint32_t ctas;         // grid size cap
@@ -36,6 +59,7 @@ struct LaunchCfg {
 
 // pack = true: paged -> pool side (offload direction); false: pool side -> paged (retrieve direction).
 cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream);
+cudaError_t launch_multi_copy(const MultiArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream);
 // Consumer stand-in / integrity check: *out += sum over logical blocks j < n, halves h (0 = K, 1 = V) and 64-bit
 // words i of  word * (2*idx + 1)  (mod 2^64),  idx = (j*2 + h)*(kvb/8) + i.  Reads the blocks through the table
 // exactly as a decode-attention kernel would (K_l*P bytes of HBM reads); `out` must be zeroed by the caller.

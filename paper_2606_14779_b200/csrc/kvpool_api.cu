@@ -68,6 +68,7 @@ struct LayerMap {
 struct LayerState {
   std::shared_ptr<LayerMap> map;
   std::vector<uint64_t> stripe_off;  // [N] byte offset of this layer's stripe inside pool buffer i
+  const uint64_t* base_d = nullptr;  // device: [N] GPU-visible addresses of this layer's stripes (for batched launches)
   bool offloaded = false;
   cudaEvent_t landed = nullptr;      // recorded when the layer's stripes are complete in the pool
   bool landed_pending = false;
@@ -521,6 +522,9 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
     max_layer_bytes = std::max(max_layer_bytes, K * p->payload);
   }
 
+  const uint64_t bases_bytes = (static_cast<uint64_t>(L) * N * 8 + 255) / 256 * 256;
+  table_bytes += bases_bytes;
+
   // a4: stripe allocation, all or nothing
   bool ok = true;
   uint32_t fail_dev = 0, done_layers = 0;
@@ -576,6 +580,13 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
       memcpy(host.data() + off, m.dev.data(), m.K);
       off += (m.K + 255) / 256 * 256;
     }
+    for (uint32_t l = 0; l < L; ++l) {  // GPU-visible stripe addresses, one row per layer
+      uint64_t* row = reinterpret_cast<uint64_t*>(host.data() + off) + static_cast<uint64_t>(l) * N;
+      for (uint32_t i = 0; i < N; ++i)
+        row[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + pl->layers[l].stripe_off[i]);
+      pl->layers[l].base_d = reinterpret_cast<const uint64_t*>(pl->tables_d + off) + static_cast<uint64_t>(l) * N;
+    }
+    off += bases_bytes;
     e = cudaMemcpy(pl->tables_d, host.data(), off, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: table upload: %s", cudaGetErrorString(e)); }
   }
@@ -735,6 +746,98 @@ int kvpool_retrieve(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k
   if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "retrieve: bad pool or placement");
   if (layer >= p->geom.n_layers) return fail(KVPOOL_EINVAL, "layer %u out of range (n_layers %u)", layer, p->geom.n_layers);
   return kvpool_retrieve_range(p, pl, layer, 0, static_cast<uint32_t>(pl->layers[layer].map->K), k_base, v_base, stride, table, cuda_stream);
+}
+
+// Layers [first, first+n): consecutive layers that take the zero-copy path are fused into launches of up to kMaxBatch
+// layers; the others go through the per-layer call.
+static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32_t first, uint32_t n, const void* const* k_bases,
+                          const void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream) {
+  if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "layers: bad pool or placement");
+  if (static_cast<uint64_t>(first) + n > p->geom.n_layers) return fail(KVPOOL_EINVAL, "layers [%u, %u) out of range (n_layers %u)", first, first + n, p->geom.n_layers);
+  if (n == 0) return KVPOOL_OK;
+  if (!k_bases || !v_bases || !tables) return fail(KVPOOL_EINVAL, "layers: null pointer array");
+  for (uint32_t q = 0; q < n; ++q) {  // validate everything first: no partial effects on EINVAL / ESTATE
+    const int rc = check_layer_call(p, pl, first + q, k_bases[q], v_bases[q], stride, tables[q]);
+    if (rc != KVPOOL_OK) return rc;
+    if (!pack && !pl->layers[first + q].offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", first + q);
+  }
+  DeviceGuard guard(p->cuda_device);
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  MultiArgs ma{};
+  ma.stride = stride;
+  ma.kvb = static_cast<uint32_t>(p->kvb);
+  uint32_t batch_layers[kMaxBatch];
+  auto flush = [&]() -> int {
+    if (ma.n == 0) return KVPOOL_OK;
+    for (uint32_t b = 0; b < ma.n; ++b) {
+      LayerState& L = pl->layers[batch_layers[b]];
+      if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
+    }
+    ProfRec r;
+    if (p->profiling) {
+      CU(prof_event(p, &r.e0));
+      CU(prof_event(p, &r.e1));
+      r.bytes = static_cast<uint64_t>(ma.total_units) * p->payload;
+      r.kind = pack ? 2 : 3;
+      CU(cudaEventRecord(r.e0, s));
+    }
+    CU(launch_multi_copy(ma, pack, launch_cfg(p, true), s));
+    p->n_kernels++;
+    if (p->profiling) {
+      CU(cudaEventRecord(r.e1, s));
+      p->prof.push_back(r);
+    }
+    if (pack)
+      for (uint32_t b = 0; b < ma.n; ++b) {
+        LayerState& L = pl->layers[batch_layers[b]];
+        CU(cudaEventRecord(L.landed, s));
+        L.landed_pending = true;
+      }
+    ma.n = 0;
+    ma.total_units = 0;
+    return KVPOOL_OK;
+  };
+  for (uint32_t q = 0; q < n; ++q) {
+    const uint32_t layer = first + q;
+    LayerState& L = pl->layers[layer];
+    if (pack) L.offloaded = true;
+    if (L.map->K == 0) continue;
+    if (use_staged(p, L)) {
+      int rc = flush();
+      if (rc != KVPOOL_OK) return rc;
+      rc = pack ? kvpool_offload(p, pl, layer, k_bases[q], v_bases[q], stride, tables[q], cuda_stream)
+                : kvpool_retrieve(p, pl, layer, const_cast<void*>(k_bases[q]), const_cast<void*>(v_bases[q]), stride, tables[q], cuda_stream);
+      if (rc != KVPOOL_OK) return rc;
+      continue;
+    }
+    if (ma.n == kMaxBatch || static_cast<uint64_t>(ma.total_units) + L.map->K > 0x7fffffffull) {
+      const int rc = flush();
+      if (rc != KVPOOL_OK) return rc;
+    }
+    MultiDesc& d = ma.d[ma.n];
+    d.k_base = static_cast<uint8_t*>(const_cast<void*>(k_bases[q]));
+    d.v_base = static_cast<uint8_t*>(const_cast<void*>(v_bases[q]));
+    d.table = tables[q];
+    d.dev = L.map->dev_d;
+    d.slot = L.map->slot_d;
+    d.pool_base = L.base_d;
+    d.K = static_cast<uint32_t>(L.map->K);
+    d.first_unit = ma.total_units;
+    batch_layers[ma.n] = layer;
+    ma.total_units += d.K;
+    ma.n += 1;
+  }
+  return flush();
+}
+
+int kvpool_offload_layers(kvpool_t* p, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers, const void* const* k_bases,
+                          const void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream) {
+  return layers_batched(p, pl, true, first_layer, n_layers, k_bases, v_bases, stride, tables, cuda_stream);
+}
+
+int kvpool_retrieve_layers(kvpool_t* p, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers, void* const* k_bases,
+                           void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream) {
+  return layers_batched(p, pl, false, first_layer, n_layers, k_bases, v_bases, stride, tables, cuda_stream);
 }
 
 int kvpool_wait_offloads(kvpool_t* p, kvpool_placement_t* pl, void* cuda_stream) {

@@ -313,3 +313,63 @@ def test_checksum_consumer_matches_oracle_and_detects_round_trip():
             pl.release()
         finally:
             pool.destroy()
+
+
+def _run_batched(wl, path, kernel, expect_kernels=None):
+    """Offload and retrieve ALL layers with one kvpool_offload_layers / kvpool_retrieve_layers call each and compare
+    every stripe and every retrieved layer with the oracle."""
+    dev = torch.device("cuda:0")
+    g, L = wl.geom, wl.geom.n_layers
+    bw = list(wl.default_weights())
+    pool = make_pool(wl)
+    try:
+        pool.set_path(path)
+        pool.set_tuning(kernel=kernel, link_kernel=kernel)
+        bpl = wl.blocks_per_layer(0)
+        pl = pool.place(bpl)
+        opl = oracle.place(bw, bpl)
+        check_placement(pl, opl)
+        tables_np = [np.ascontiguousarray(wl.layer_table(0, l)) for l in range(L)]
+        tables = [torch.from_numpy(t).to(dev) if len(t) else None for t in tables_np]
+        src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+        dst = [W.poison_torch((2, wl.nphys, g.kvb // 2), dev) for l in range(L)]
+        s = torch.cuda.Stream()
+        with pytest.raises(kv.KvPoolError) as e:                                  # nothing offloaded yet: ESTATE, nothing enqueued
+            pool.retrieve_layers(pl, 0, [d[0] for d in dst], [d[1] for d in dst], g.kvb, tables, s)
+        assert e.value.code == kv.ESTATE
+        k0, _ = pool.stats()
+        pool.offload_layers(pl, 0, [x[0] for x in src], [x[1] for x in src], g.kvb, tables, s)
+        pool.wait_offloads(pl, s)
+        pool.retrieve_layers(pl, 0, [d[0] for d in dst], [d[1] for d in dst], g.kvb, tables, s)
+        s.synchronize()
+        k1, _ = pool.stats()
+        if expect_kernels is not None:
+            assert k1 - k0 == expect_kernels
+        for l in range(L):
+            src_cpu = W.kv_layer_numpy(wl, l)
+            want = oracle.offload_layer(src_cpu, tables_np[l], opl[l])
+            for i in range(pool.n_devices):
+                assert np.array_equal(pl.stripe(l, i), want[i]), f"stripe differs: layer {l} device {i}"
+            ref = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+            oracle.retrieve_layer(ref, tables_np[l], opl[l], want)
+            assert np.array_equal(dst[l].cpu().numpy().view(np.uint16), ref), f"retrieved layer {l} differs"
+        pl.release()
+    finally:
+        pool.destroy()
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_batched_layers_fused_launches(kernel):
+    # config 1, whole request: 32 layers x 4 MiB, auto path -> zero-copy, fused into ONE launch per direction
+    _run_batched(W.make_workload(1), kv.PATH_AUTO, KERNELS[kernel], expect_kernels=2)
+    # sliding-window + full layers (config 3 scaled): tiny layers fuse, 16 MiB layers go staged in between
+    wl = W.make_workload(3, scale=1 / 8, n_layers=6)
+    _run_batched(wl, kv.PATH_AUTO, KERNELS[kernel], expect_kernels=2 * (3 + 3))
+    _run_batched(wl, kv.PATH_ZEROCOPY, KERNELS[kernel], expect_kernels=2)
+    _run_batched(wl, kv.PATH_STAGED, KERNELS[kernel], expect_kernels=12)
+    # more layers than one launch holds (64), ragged block size, some empty layers
+    g = W.Geometry(n_layers=150, n_kv_heads=1, head_dim=80)
+    rng = np.random.default_rng(23)
+    wl = W.Workload(78, "many-tiny-layers", g, (0,), 40, [W.Request(rng.permutation(40)[:29].astype(np.int32))], 3, (3.0, 2.0, 1.0),
+                    sliding_layers=tuple(range(0, 150, 7)))
+    _run_batched(wl, kv.PATH_ZEROCOPY, KERNELS[kernel], expect_kernels=2 * 3)
