@@ -579,6 +579,7 @@ def run_sweep(args) -> None:
     tables = [torch.from_numpy(np.ascontiguousarray(wl.layer_table(R, l))).to(dev) for l in range(4)]
     stage = torch.empty(K * g.payload, dtype=torch.uint8, device=dev)
     main_s = torch.cuda.Stream(device=dev)
+    torch.cuda.synchronize()
     nbytes = K * g.payload
 
     def timed(fn, reps, per_pair):
@@ -659,6 +660,7 @@ def run_blocked_io(args) -> None:
             tables = [torch.from_numpy(np.ascontiguousarray(wl.layer_table(0, l))).to(dev) for l in range(L)]
             sa, sb = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
             sums = torch.zeros((3, L), dtype=torch.int64, device=dev)
+            torch.cuda.synchronize()        # inputs were generated on the default stream; sa / sb do not wait for it
             for l in range(L):
                 pool.offload(pl, l, src[l][0], src[l][1], g.kvb, tables[l], sa)
                 pool.checksum(src[l][0], src[l][1], g.kvb, tables[l], int(bpl[l]), sums[0, l:l + 1], sa)

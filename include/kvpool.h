@@ -152,10 +152,11 @@ KVPOOL_API int kvpool_retrieve(kvpool_t* pool, kvpool_placement_t* pl, uint32_t 
                     uint64_t block_stride_bytes, const int32_t* block_table_dev, void* cuda_stream);
 /* Batched forms: layers [first_layer, first_layer + n_layers) in one call, equivalent to the per-layer calls in
  * ascending order.  k_bases / v_bases / block_tables are HOST arrays of n_layers DEVICE pointers (entries of layers
- * with K_l = 0 may be NULL).  Consecutive layers that take the zero-copy path are fused into single kernel launches
- * (up to 64 layers each): a request made of small layers pays one launch latency and one pipeline ramp instead of
- * one per layer (the launch-latency regime of 1K-token contexts and sliding-window layers).  All arguments are
- * validated before anything is enqueued.                                                                            */
+ * with K_l = 0 may be NULL).  The layers that take the zero-copy path are issued first, fused into single kernel
+ * launches (up to 64 layers each): small layers pay one launch latency and one pipeline ramp per batch instead of
+ * one per layer (the launch-latency regime of 1K-token contexts and sliding-window layers); the staged layers
+ * follow in ascending order.  Layers touch disjoint memory, so the result equals that of the per-layer calls.  All
+ * arguments are validated before anything is enqueued.                                                                            */
 KVPOOL_API int kvpool_offload_layers(kvpool_t* pool, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers,
                           const void* const* k_bases /*host[n_layers]*/, const void* const* v_bases /*host[n_layers]*/,
                           uint64_t block_stride_bytes, const int32_t* const* block_tables /*host[n_layers]*/, void* cuda_stream);

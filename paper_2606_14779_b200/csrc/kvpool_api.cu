@@ -797,19 +797,13 @@ static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32
     ma.total_units = 0;
     return KVPOOL_OK;
   };
+  // pass 1: every layer that takes the zero-copy path, fused (layers touch disjoint memory, so issuing the small
+  // ones first changes no result); pass 2 below: the staged layers in ascending order
   for (uint32_t q = 0; q < n; ++q) {
     const uint32_t layer = first + q;
     LayerState& L = pl->layers[layer];
     if (pack) L.offloaded = true;
-    if (L.map->K == 0) continue;
-    if (use_staged(p, L)) {
-      int rc = flush();
-      if (rc != KVPOOL_OK) return rc;
-      rc = pack ? kvpool_offload(p, pl, layer, k_bases[q], v_bases[q], stride, tables[q], cuda_stream)
-                : kvpool_retrieve(p, pl, layer, const_cast<void*>(k_bases[q]), const_cast<void*>(v_bases[q]), stride, tables[q], cuda_stream);
-      if (rc != KVPOOL_OK) return rc;
-      continue;
-    }
+    if (L.map->K == 0 || use_staged(p, L)) continue;
     if (ma.n == kMaxBatch || static_cast<uint64_t>(ma.total_units) + L.map->K > 0x7fffffffull) {
       const int rc = flush();
       if (rc != KVPOOL_OK) return rc;
@@ -827,7 +821,17 @@ static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32
     ma.total_units += d.K;
     ma.n += 1;
   }
-  return flush();
+  int rc = flush();
+  if (rc != KVPOOL_OK) return rc;
+  for (uint32_t q = 0; q < n; ++q) {
+    const uint32_t layer = first + q;
+    LayerState& L = pl->layers[layer];
+    if (L.map->K == 0 || !use_staged(p, L)) continue;
+    rc = pack ? kvpool_offload(p, pl, layer, k_bases[q], v_bases[q], stride, tables[q], cuda_stream)
+              : kvpool_retrieve(p, pl, layer, const_cast<void*>(k_bases[q]), const_cast<void*>(v_bases[q]), stride, tables[q], cuda_stream);
+    if (rc != KVPOOL_OK) return rc;
+  }
+  return KVPOOL_OK;
 }
 
 int kvpool_offload_layers(kvpool_t* p, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers, const void* const* k_bases,
