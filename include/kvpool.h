@@ -87,7 +87,8 @@ typedef struct {         /* kvpool_set_tuning; 0 in any field = library default 
   uint32_t stage_slots;  /* staging buffers in the ring of the staged path (default 4)                   */
   uint32_t vec_threads;  /* threads per CTA of the vec16 kernel (multiple of 32, 64..512)                */
   uint32_t vec_unroll;   /* 16-byte loads in flight per lane in the vec16 kernel: 4, 8 or 16             */
-  uint64_t auto_threshold_bytes; /* PATH_AUTO: layers moving fewer bytes than this go zero-copy          */
+  uint64_t auto_threshold_bytes; /* PATH_AUTO: layers (or groups) moving fewer bytes than this go zero-copy */
+  uint64_t group_bytes;  /* batched calls: consecutive layers are grouped until a group moves at least this much */
 } kvpool_tuning;
 
 /* ---- pure host arithmetic (no CUDA, no pool) --------------------------------------------------------
@@ -152,11 +153,12 @@ KVPOOL_API int kvpool_retrieve(kvpool_t* pool, kvpool_placement_t* pl, uint32_t 
                     uint64_t block_stride_bytes, const int32_t* block_table_dev, void* cuda_stream);
 /* Batched forms: layers [first_layer, first_layer + n_layers) in one call, equivalent to the per-layer calls in
  * ascending order.  k_bases / v_bases / block_tables are HOST arrays of n_layers DEVICE pointers (entries of layers
- * with K_l = 0 may be NULL).  The layers that take the zero-copy path are issued first, fused into single kernel
- * launches (up to 64 layers each): small layers pay one launch latency and one pipeline ramp per batch instead of
- * one per layer (the launch-latency regime of 1K-token contexts and sliding-window layers); the staged layers
- * follow in ascending order.  Layers touch disjoint memory, so the result equals that of the per-layer calls.  All
- * arguments are validated before anything is enqueued.                                                                            */
+ * with K_l = 0 may be NULL).  Consecutive layers are gathered into groups of at least `group_bytes` (default 64 MiB,
+ * at most 64 layers; a large layer travels with the small ones before it) and each group moves as one unit: one
+ * fused kernel launch on the zero-copy path, or one pack/unpack launch plus ONE cudaMemcpyAsync per pool device on
+ * the staged path (a placement's stripes are contiguous per device across layers).  Small layers thus pay one
+ * launch latency and one DMA ramp per group instead of one per layer (1K-token contexts, sliding-window layers).
+ * All arguments are validated before anything is enqueued.                                                                            */
 KVPOOL_API int kvpool_offload_layers(kvpool_t* pool, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers,
                           const void* const* k_bases /*host[n_layers]*/, const void* const* v_bases /*host[n_layers]*/,
                           uint64_t block_stride_bytes, const int32_t* const* block_tables /*host[n_layers]*/, void* cuda_stream);

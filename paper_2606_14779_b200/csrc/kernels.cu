@@ -78,7 +78,7 @@ __device__ __forceinline__ Piece decode(const MultiArgs& a, uint64_t t, uint32_t
   const uint32_t off = c * piece_bytes;
   Piece p;
   p.paged = (half ? L.v_base : L.k_base) + static_cast<uint64_t>(phys) * a.stride + off;
-  p.pooled = reinterpret_cast<uint8_t*>(__ldg(L.pool_base + d)) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;
+  p.pooled = reinterpret_cast<uint8_t*>(__ldg(L.pool_base + d) + a.delta[d]) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;
   p.bytes = min(piece_bytes, a.kvb - off);
   return p;
 }

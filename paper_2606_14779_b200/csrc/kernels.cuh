@@ -46,6 +46,8 @@ struct MultiArgs {
   uint32_t n;            // layers in this launch, <= kMaxBatch
   uint32_t total_units;  // sum of K
   uint32_t pad;
+  uint64_t delta[kMaxDev];  // added (mod 2^64) to pool_base[i]: 0 for the mapped host stripes themselves, or the
+                            // displacement that maps device i's span of stripes onto its copy in a staging slot
   MultiDesc d[kMaxBatch];
 };
 

@@ -8,6 +8,7 @@
 #include <cstring>
 #include <memory>
 #include <mutex>
+#include <numeric>
 #include <string>
 #include <unordered_map>
 #include <vector>
@@ -83,6 +84,7 @@ struct ProfRec {  // one profiled kernel launch
 struct StageSlot {
   uint8_t* buf = nullptr;
   cudaEvent_t kernel_done = nullptr;          // last kernel that read/wrote the slot
+  cudaEvent_t gate = nullptr;                 // scratch: fans one stream's waits out to the other I/O streams
   std::vector<cudaEvent_t> copy_done;         // [N] last memcpy per pool stream that read/wrote the slot
 };
 
@@ -91,6 +93,7 @@ struct StageSlot {
 struct kvpool_placement {
   kvpool* pool = nullptr;
   std::vector<LayerState> layers;
+  std::vector<uint64_t> region_off, region_bytes;  // [N] one contiguous region per pool device holds all layers' stripes
   uint8_t* tables_d = nullptr;   // every LayerMap's dev/slot columns, contiguous
   uint64_t tables_bytes = 0;
   bool tables_in_arena = false;  // carved out of the pool's table arena (else a private cudaMalloc)
@@ -136,6 +139,7 @@ void default_tuning(kvpool* p) {
   p->tune.stage_slots = 4;
   p->tune.vec_threads = 512;
   p->tune.vec_unroll = 8;
+  p->tune.group_bytes = 64ull << 20;
   p->tune.auto_threshold_bytes = 8ull << 20;
 }
 
@@ -143,6 +147,7 @@ void free_slots(kvpool* p) {
   for (auto& s : p->slots) {
     if (s.buf) cudaFree(s.buf);
     if (s.kernel_done) cudaEventDestroy(s.kernel_done);
+    if (s.gate) cudaEventDestroy(s.gate);
     for (auto e : s.copy_done) cudaEventDestroy(e);
   }
   p->slots.clear();
@@ -171,6 +176,7 @@ int ensure_slots(kvpool* p, uint64_t bytes) {
       }
     }
     CU(cudaEventCreateWithFlags(&s.kernel_done, cudaEventDisableTiming));
+    CU(cudaEventCreateWithFlags(&s.gate, cudaEventDisableTiming));
     s.copy_done.resize(p->n);
     for (auto& e : s.copy_done) CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   }
@@ -197,10 +203,9 @@ cudaError_t take_event(kvpool* p, cudaEvent_t* e) {
 }
 
 void destroy_placement(kvpool* p, kvpool_placement* pl) {
-  for (auto& L : pl->layers) {
-    for (uint32_t i = 0; i < p->n; ++i) p->alloc[i].free(L.stripe_off[i], static_cast<uint64_t>(L.map->counts[i]) * p->payload);
+  for (uint32_t i = 0; i < p->n && i < pl->region_off.size(); ++i) p->alloc[i].free(pl->region_off[i], pl->region_bytes[i]);
+  for (auto& L : pl->layers)
     if (L.landed) p->ev_free.push_back(L.landed);
-  }
   free_tables(p, pl);
   delete pl;
 }
@@ -466,6 +471,7 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
   if (t->vec_threads) d.vec_threads = t->vec_threads;
   if (t->vec_unroll) d.vec_unroll = t->vec_unroll;
   if (t->auto_threshold_bytes) d.auto_threshold_bytes = t->auto_threshold_bytes;
+  if (t->group_bytes) d.group_bytes = t->group_bytes;
   if (t->stage_slots && t->stage_slots != d.stage_slots) {
     DeviceGuard guard(p->cuda_device);
     d.stage_slots = t->stage_slots;
@@ -525,36 +531,41 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
   const uint64_t bases_bytes = (static_cast<uint64_t>(L) * N * 8 + 255) / 256 * 256;
   table_bytes += bases_bytes;
 
-  // a4: stripe allocation, all or nothing
-  bool ok = true;
-  uint32_t fail_dev = 0, done_layers = 0;
-  for (uint32_t l = 0; l < L && ok; ++l) {
+  // a4: stripe allocation, all or nothing.  Each pool device gets ONE contiguous region per placement in which the
+  // layers' stripes follow each other in layer order (256-byte aligned), so that a run of consecutive layers is also
+  // one contiguous span per device — what lets the batched calls move several small layers with one copy per device.
+  constexpr uint64_t kStripeAlign = 256;
+  pl->region_off.assign(N, 0);
+  pl->region_bytes.assign(N, 0);
+  for (uint32_t l = 0; l < L; ++l) {
     auto& Ls = pl->layers[l];
     Ls.stripe_off.assign(N, 0);
-    uint32_t i = 0;
-    for (; i < N; ++i)
-      if (!p->alloc[i].alloc(static_cast<uint64_t>(Ls.map->counts[i]) * p->payload, &Ls.stripe_off[i])) break;
-    if (i < N) {
-      ok = false;
-      fail_dev = i;
-      for (uint32_t k = 0; k < i; ++k) p->alloc[k].free(Ls.stripe_off[k], static_cast<uint64_t>(Ls.map->counts[k]) * p->payload);
-    } else {
-      done_layers = l + 1;
+    for (uint32_t i = 0; i < N; ++i) {
+      Ls.stripe_off[i] = pl->region_bytes[i];  // relative for now
+      pl->region_bytes[i] += (static_cast<uint64_t>(Ls.map->counts[i]) * p->payload + kStripeAlign - 1) / kStripeAlign * kStripeAlign;
     }
   }
+  bool ok = true;
+  uint32_t fail_dev = 0, done_devs = 0;
+  for (uint32_t i = 0; i < N; ++i) {
+    if (!p->alloc[i].alloc(pl->region_bytes[i], &pl->region_off[i])) { ok = false; fail_dev = i; break; }
+    done_devs = i + 1;
+  }
   auto rollback = [&]() {
-    for (uint32_t l = 0; l < done_layers; ++l)
-      for (uint32_t i = 0; i < N; ++i)
-        p->alloc[i].free(pl->layers[l].stripe_off[i], static_cast<uint64_t>(pl->layers[l].map->counts[i]) * p->payload);
+    for (uint32_t i = 0; i < done_devs; ++i) p->alloc[i].free(pl->region_off[i], pl->region_bytes[i]);
+    pl->region_off.clear();
     free_tables(p, pl.get());
     for (auto& Ls : pl->layers)
       if (Ls.landed) p->ev_free.push_back(Ls.landed);
   };
   if (!ok) {
     rollback();
-    return fail(KVPOOL_ENOMEM, "place: pool device %u is full (capacity %llu, used %llu)", fail_dev,
-                (unsigned long long)p->alloc[fail_dev].capacity(), (unsigned long long)p->alloc[fail_dev].used());
+    return fail(KVPOOL_ENOMEM, "place: pool device %u has no contiguous %llu bytes (capacity %llu, used %llu)", fail_dev,
+                (unsigned long long)pl->region_bytes[fail_dev], (unsigned long long)p->alloc[fail_dev].capacity(),
+                (unsigned long long)p->alloc[fail_dev].used());
   }
+  for (auto& Ls : pl->layers)
+    for (uint32_t i = 0; i < N; ++i) Ls.stripe_off[i] += pl->region_off[i];
 
   // GLT upload: dense (device_id, slot) columns, one device allocation per placement
   if (table_bytes) {
@@ -595,7 +606,10 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
     if (e != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: cudaEventCreate: %s", cudaGetErrorString(e)); }
   }
   if (p->path != KVPOOL_PATH_ZEROCOPY) {
-    const int rc = ensure_slots(p, max_layer_bytes);
+    // a slot holds the largest layer, or a group of small layers (plus the 256-byte alignment gaps between stripes)
+    const uint64_t total_bytes = std::accumulate(pl->region_bytes.begin(), pl->region_bytes.end(), uint64_t{0});
+    const uint64_t group_cap = std::min<uint64_t>(std::max<uint64_t>(max_layer_bytes, p->tune.group_bytes), total_bytes);
+    const int rc = ensure_slots(p, std::max(max_layer_bytes, group_cap) + static_cast<uint64_t>(N) * 256 * (kMaxBatch + 1));
     if (rc != KVPOOL_OK) { rollback(); return rc; }
   }
   p->live.push_back(pl.get());
@@ -648,6 +662,8 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
 
   // staged: pack kernel -> device staging slot (stripe order), then one D2H copy per stripe on the
   // per-device I/O streams; `stream` is released as soon as the pack is enqueued.
+  if (p->slots.empty() || L.map->K * p->payload > p->slot_bytes)
+    return fail(KVPOOL_ESTATE, "offload: no staging slot large enough (the placement was made while the path was zero-copy)");
   StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
   rc = wait_slot_free(p, slot, s);
   if (rc != KVPOOL_OK) return rc;
@@ -715,6 +731,8 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
 
   // staged: one H2D copy per stripe (only the slots the range touches) on the per-device I/O streams — these may run
   // ahead of `stream` — then the unpack kernel on `stream` once all of them have landed in the staging slot.
+  if (p->slots.empty() || L.map->K * p->payload > p->slot_bytes)
+    return fail(KVPOOL_ESTATE, "retrieve: no staging slot large enough (the placement was made while the path was zero-copy)");
   StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
   uint32_t lo[KVPOOL_MAX_DEVICES], hi[KVPOOL_MAX_DEVICES];
   for (uint32_t i = 0; i < N; ++i) {
@@ -748,8 +766,184 @@ int kvpool_retrieve(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k
   return kvpool_retrieve_range(p, pl, layer, 0, static_cast<uint32_t>(pl->layers[layer].map->K), k_base, v_base, stride, table, cuda_stream);
 }
 
-// Layers [first, first+n): consecutive layers that take the zero-copy path are fused into launches of up to kMaxBatch
-// layers; the others go through the per-layer call.
+// One multi-layer launch, counted and (when profiling) bracketed by an event pair on `s`.
+static int launch_multi_counted(kvpool* p, const MultiArgs& ma, bool pack, bool link_bound, cudaStream_t s) {
+  ProfRec r;
+  if (p->profiling) {
+    CU(prof_event(p, &r.e0));
+    CU(prof_event(p, &r.e1));
+    r.bytes = static_cast<uint64_t>(ma.total_units) * p->payload;
+    r.kind = (link_bound ? 2 : 0) + (pack ? 0 : 1);
+    CU(cudaEventRecord(r.e0, s));
+  }
+  CU(launch_multi_copy(ma, pack, launch_cfg(p, link_bound), s));
+  p->n_kernels++;
+  if (p->profiling) {
+    CU(cudaEventRecord(r.e1, s));
+    p->prof.push_back(r);
+  }
+  return KVPOOL_OK;
+}
+
+namespace {
+struct LayerGroup {  // a run of layers of one batched call that moves as one unit
+  uint32_t q[kMaxBatch];  // indices into the call's pointer arrays (layer = first + q)
+  uint32_t n = 0;
+  uint64_t bytes = 0;
+};
+struct BatchCall {
+  kvpool* p;
+  kvpool_placement* pl;
+  bool pack;
+  uint32_t first;
+  const void* const* k_bases;
+  const void* const* v_bases;
+  const int32_t* const* tables;
+  uint64_t stride;
+  cudaStream_t s;
+};
+
+void fill_descs(const BatchCall& c, const LayerGroup& g, MultiArgs* ma) {
+  ma->stride = c.stride;
+  ma->kvb = static_cast<uint32_t>(c.p->kvb);
+  ma->n = g.n;
+  ma->total_units = 0;
+  for (uint32_t b = 0; b < g.n; ++b) {
+    const LayerState& L = c.pl->layers[c.first + g.q[b]];
+    MultiDesc& d = ma->d[b];
+    d.k_base = static_cast<uint8_t*>(const_cast<void*>(c.k_bases[g.q[b]]));
+    d.v_base = static_cast<uint8_t*>(const_cast<void*>(c.v_bases[g.q[b]]));
+    d.table = c.tables[g.q[b]];
+    d.dev = L.map->dev_d;
+    d.slot = L.map->slot_d;
+    d.pool_base = L.base_d;
+    d.K = static_cast<uint32_t>(L.map->K);
+    d.first_unit = ma->total_units;
+    ma->total_units += d.K;
+  }
+}
+
+// Zero-copy: one kernel moves the whole group straight between the paged blocks and the mapped host stripes.
+int issue_zero_copy_group(const BatchCall& c, const LayerGroup& g) {
+  kvpool* p = c.p;
+  MultiArgs ma{};
+  fill_descs(c, g, &ma);
+  for (uint32_t b = 0; b < g.n; ++b) {
+    LayerState& L = c.pl->layers[c.first + g.q[b]];
+    if (L.landed_pending) CU(cudaStreamWaitEvent(c.s, L.landed, 0));
+  }
+  const int rc = launch_multi_counted(p, ma, c.pack, true, c.s);
+  if (rc != KVPOOL_OK) return rc;
+  if (c.pack)
+    for (uint32_t b = 0; b < g.n; ++b) {
+      LayerState& L = c.pl->layers[c.first + g.q[b]];
+      CU(cudaEventRecord(L.landed, c.s));
+      L.landed_pending = true;
+    }
+  return KVPOOL_OK;
+}
+
+// Staged: the group's stripes are one contiguous span per pool device (region allocation in kvpool_place), so the
+// whole group moves with ONE cudaMemcpyAsync per device and ONE pack / unpack launch.  Returns 1 if the group does
+// not fit a staging slot (the caller then falls back to per-layer calls).
+int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
+  kvpool* p = c.p;
+  const uint32_t N = p->n;
+  const LayerState& A = c.pl->layers[c.first + g.q[0]];
+  const LayerState& Z = c.pl->layers[c.first + g.q[g.n - 1]];
+  uint64_t span_lo[KVPOOL_MAX_DEVICES], span[KVPOOL_MAX_DEVICES], dev_start[KVPOOL_MAX_DEVICES], total = 0;
+  for (uint32_t i = 0; i < N; ++i) {
+    span_lo[i] = A.stripe_off[i];
+    span[i] = Z.stripe_off[i] + static_cast<uint64_t>(Z.map->counts[i]) * p->payload - span_lo[i];
+    dev_start[i] = total;
+    total += (span[i] + 255) / 256 * 256;
+  }
+  if (total > p->slot_bytes || p->slots.empty()) return 1;
+  StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
+  MultiArgs ma{};
+  fill_descs(c, g, &ma);
+  for (uint32_t i = 0; i < N; ++i)
+    ma.delta[i] = reinterpret_cast<uint64_t>(slot.buf + dev_start[i]) - reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + span_lo[i]);
+
+  // an earlier offload of these layers that is still in flight must land before their stripes are touched again:
+  // gather those waits on the first I/O stream that has work and fan out through one event
+  cudaStream_t lead = nullptr;
+  for (uint32_t i = 0; i < N && !lead; ++i)
+    if (span[i]) lead = p->io[i];
+  if (!lead) return KVPOOL_OK;
+  bool gated = false;
+  for (uint32_t b = 0; b < g.n; ++b) {
+    LayerState& L = c.pl->layers[c.first + g.q[b]];
+    if (L.landed_pending) { CU(cudaStreamWaitEvent(lead, L.landed, 0)); gated = true; }
+  }
+
+  int rc;
+  if (c.pack) {
+    rc = wait_slot_free(p, slot, c.s);
+    if (rc != KVPOOL_OK) return rc;
+    rc = launch_multi_counted(p, ma, true, false, c.s);
+    if (rc != KVPOOL_OK) return rc;
+    CU(cudaEventRecord(slot.kernel_done, c.s));
+    if (gated) CU(cudaEventRecord(slot.gate, lead));
+    for (uint32_t i = 0; i < N; ++i) {
+      if (!span[i]) continue;
+      CU(cudaStreamWaitEvent(p->io[i], slot.kernel_done, 0));
+      if (gated && p->io[i] != lead) CU(cudaStreamWaitEvent(p->io[i], slot.gate, 0));
+      CU(cudaMemcpyAsync(static_cast<uint8_t*>(p->bufs[i].host) + span_lo[i], slot.buf + dev_start[i], span[i], cudaMemcpyDeviceToHost, p->io[i]));
+      p->n_memcpys++;
+      CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+    }
+    for (uint32_t i = 0; i < N; ++i)
+      if (span[i] && p->io[i] != lead) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
+    for (uint32_t b = 0; b < g.n; ++b) {
+      LayerState& L = c.pl->layers[c.first + g.q[b]];
+      CU(cudaEventRecord(L.landed, lead));
+      L.landed_pending = true;
+    }
+    return KVPOOL_OK;
+  }
+  for (uint32_t i = 0; i < N; ++i) {
+    if (!span[i]) continue;
+    rc = wait_slot_free(p, slot, p->io[i]);
+    if (rc != KVPOOL_OK) return rc;
+  }
+  if (gated) CU(cudaEventRecord(slot.gate, lead));
+  for (uint32_t i = 0; i < N; ++i) {
+    if (!span[i]) continue;
+    if (gated && p->io[i] != lead) CU(cudaStreamWaitEvent(p->io[i], slot.gate, 0));
+    CU(cudaMemcpyAsync(slot.buf + dev_start[i], static_cast<uint8_t*>(p->bufs[i].host) + span_lo[i], span[i], cudaMemcpyHostToDevice, p->io[i]));
+    p->n_memcpys++;
+    CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+    CU(cudaStreamWaitEvent(c.s, slot.copy_done[i], 0));
+  }
+  rc = launch_multi_counted(p, ma, false, false, c.s);
+  if (rc != KVPOOL_OK) return rc;
+  CU(cudaEventRecord(slot.kernel_done, c.s));
+  return KVPOOL_OK;
+}
+
+int issue_group(const BatchCall& c, const LayerGroup& g) {
+  kvpool* p = c.p;
+  if (g.n == 0) return KVPOOL_OK;
+  const bool staged = p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && g.bytes >= p->tune.auto_threshold_bytes);
+  if (!staged) return issue_zero_copy_group(c, g);
+  if (g.n > 1) {
+    const int rc = issue_staged_group(c, g);
+    if (rc != 1) return rc;
+  }
+  for (uint32_t b = 0; b < g.n; ++b) {  // a single layer, or a group too large for a staging slot: the per-layer path
+    const uint32_t q = g.q[b], layer = c.first + q;
+    const int rc = c.pack ? kvpool_offload(p, c.pl, layer, c.k_bases[q], c.v_bases[q], c.stride, c.tables[q], c.s)
+                          : kvpool_retrieve(p, c.pl, layer, const_cast<void*>(c.k_bases[q]), const_cast<void*>(c.v_bases[q]), c.stride, c.tables[q], c.s);
+    if (rc != KVPOOL_OK) return rc;
+  }
+  return KVPOOL_OK;
+}
+}  // namespace
+
+// Layers [first, first+n) in one call.  Consecutive layers are gathered into groups of at least tune.group_bytes (a
+// layer at least that large travels with whatever small layers precede it); each group moves as one unit: one fused
+// zero-copy launch, or one pack/unpack launch plus one copy per pool device.
 static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32_t first, uint32_t n, const void* const* k_bases,
                           const void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream) {
   if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "layers: bad pool or placement");
@@ -762,76 +956,32 @@ static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32
     if (!pack && !pl->layers[first + q].offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", first + q);
   }
   DeviceGuard guard(p->cuda_device);
-  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  MultiArgs ma{};
-  ma.stride = stride;
-  ma.kvb = static_cast<uint32_t>(p->kvb);
-  uint32_t batch_layers[kMaxBatch];
-  auto flush = [&]() -> int {
-    if (ma.n == 0) return KVPOOL_OK;
-    for (uint32_t b = 0; b < ma.n; ++b) {
-      LayerState& L = pl->layers[batch_layers[b]];
-      if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
-    }
-    ProfRec r;
-    if (p->profiling) {
-      CU(prof_event(p, &r.e0));
-      CU(prof_event(p, &r.e1));
-      r.bytes = static_cast<uint64_t>(ma.total_units) * p->payload;
-      r.kind = pack ? 2 : 3;
-      CU(cudaEventRecord(r.e0, s));
-    }
-    CU(launch_multi_copy(ma, pack, launch_cfg(p, true), s));
-    p->n_kernels++;
-    if (p->profiling) {
-      CU(cudaEventRecord(r.e1, s));
-      p->prof.push_back(r);
-    }
-    if (pack)
-      for (uint32_t b = 0; b < ma.n; ++b) {
-        LayerState& L = pl->layers[batch_layers[b]];
-        CU(cudaEventRecord(L.landed, s));
-        L.landed_pending = true;
-      }
-    ma.n = 0;
-    ma.total_units = 0;
-    return KVPOOL_OK;
-  };
-  // pass 1: every layer that takes the zero-copy path, fused (layers touch disjoint memory, so issuing the small
-  // ones first changes no result); pass 2 below: the staged layers in ascending order
+  const BatchCall c{p, pl, pack, first, k_bases, v_bases, tables, stride, static_cast<cudaStream_t>(cuda_stream)};
+  const uint64_t cap = std::max<uint64_t>(p->tune.group_bytes, 1);
+  LayerGroup g;
+  uint64_t units = 0;
   for (uint32_t q = 0; q < n; ++q) {
-    const uint32_t layer = first + q;
-    LayerState& L = pl->layers[layer];
+    LayerState& L = pl->layers[first + q];
     if (pack) L.offloaded = true;
-    if (L.map->K == 0 || use_staged(p, L)) continue;
-    if (ma.n == kMaxBatch || static_cast<uint64_t>(ma.total_units) + L.map->K > 0x7fffffffull) {
-      const int rc = flush();
+    if (L.map->K == 0) continue;
+    const uint64_t bytes = L.map->K * p->payload;
+    if (g.n && (g.n == kMaxBatch || units + L.map->K > 0x7fffffffull || (p->path != KVPOOL_PATH_ZEROCOPY && g.bytes + bytes > std::max(cap, bytes)))) {
+      const int rc = issue_group(c, g);
       if (rc != KVPOOL_OK) return rc;
+      g = LayerGroup{};
+      units = 0;
     }
-    MultiDesc& d = ma.d[ma.n];
-    d.k_base = static_cast<uint8_t*>(const_cast<void*>(k_bases[q]));
-    d.v_base = static_cast<uint8_t*>(const_cast<void*>(v_bases[q]));
-    d.table = tables[q];
-    d.dev = L.map->dev_d;
-    d.slot = L.map->slot_d;
-    d.pool_base = L.base_d;
-    d.K = static_cast<uint32_t>(L.map->K);
-    d.first_unit = ma.total_units;
-    batch_layers[ma.n] = layer;
-    ma.total_units += d.K;
-    ma.n += 1;
+    g.q[g.n++] = q;
+    g.bytes += bytes;
+    units += L.map->K;
+    if (p->path != KVPOOL_PATH_ZEROCOPY && g.bytes >= cap) {
+      const int rc = issue_group(c, g);
+      if (rc != KVPOOL_OK) return rc;
+      g = LayerGroup{};
+      units = 0;
+    }
   }
-  int rc = flush();
-  if (rc != KVPOOL_OK) return rc;
-  for (uint32_t q = 0; q < n; ++q) {
-    const uint32_t layer = first + q;
-    LayerState& L = pl->layers[layer];
-    if (L.map->K == 0 || !use_staged(p, L)) continue;
-    rc = pack ? kvpool_offload(p, pl, layer, k_bases[q], v_bases[q], stride, tables[q], cuda_stream)
-              : kvpool_retrieve(p, pl, layer, const_cast<void*>(k_bases[q]), const_cast<void*>(v_bases[q]), stride, tables[q], cuda_stream);
-    if (rc != KVPOOL_OK) return rc;
-  }
-  return KVPOOL_OK;
+  return issue_group(c, g);
 }
 
 int kvpool_offload_layers(kvpool_t* p, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers, const void* const* k_bases,

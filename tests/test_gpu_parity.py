@@ -316,7 +316,7 @@ def test_checksum_consumer_matches_oracle_and_detects_round_trip():
             pool.destroy()
 
 
-def _run_batched(wl, path, kernel, expect_kernels=None):
+def _run_batched(wl, path, kernel, expect_kernels=None, expect_memcpys=None, tuning=None):
     """Offload and retrieve ALL layers with one kvpool_offload_layers / kvpool_retrieve_layers call each and compare
     every stripe and every retrieved layer with the oracle."""
     dev = torch.device("cuda:0")
@@ -325,7 +325,7 @@ def _run_batched(wl, path, kernel, expect_kernels=None):
     pool = make_pool(wl)
     try:
         pool.set_path(path)
-        pool.set_tuning(kernel=kernel, link_kernel=kernel)
+        pool.set_tuning(kernel=kernel, link_kernel=kernel, **(tuning or {}))
         bpl = wl.blocks_per_layer(0)
         pl = pool.place(bpl)
         opl = oracle.place(bw, bpl)
@@ -339,14 +339,16 @@ def _run_batched(wl, path, kernel, expect_kernels=None):
         with pytest.raises(kv.KvPoolError) as e:                                  # nothing offloaded yet: ESTATE, nothing enqueued
             pool.retrieve_layers(pl, 0, [d[0] for d in dst], [d[1] for d in dst], g.kvb, tables, s)
         assert e.value.code == kv.ESTATE
-        k0, _ = pool.stats()
+        k0, m0 = pool.stats()
         pool.offload_layers(pl, 0, [x[0] for x in src], [x[1] for x in src], g.kvb, tables, s)
         pool.wait_offloads(pl, s)
         pool.retrieve_layers(pl, 0, [d[0] for d in dst], [d[1] for d in dst], g.kvb, tables, s)
         s.synchronize()
-        k1, _ = pool.stats()
+        k1, m1 = pool.stats()
         if expect_kernels is not None:
             assert k1 - k0 == expect_kernels
+        if expect_memcpys is not None:
+            assert m1 - m0 == expect_memcpys
         for l in range(L):
             src_cpu = W.kv_layer_numpy(wl, l)
             want = oracle.offload_layer(src_cpu, tables_np[l], opl[l])
@@ -361,17 +363,22 @@ def _run_batched(wl, path, kernel, expect_kernels=None):
 
 
 @pytest.mark.parametrize("kernel", list(KERNELS))
-def test_batched_layers_fused_launches(kernel):
-    # config 1, whole request: 32 layers x 4 MiB, auto path -> zero-copy, fused into ONE launch per direction
-    _run_batched(W.make_workload(1), kv.PATH_AUTO, KERNELS[kernel], expect_kernels=2)
-    # sliding-window + full layers (config 3 scaled): tiny layers fuse, 16 MiB layers go staged in between
+def test_batched_layers_grouped_launches(kernel):
+    k = KERNELS[kernel]
+    # config 1, whole request (32 layers x 4 MiB): two 64 MiB groups, each ONE pack/unpack launch + one copy per device
+    _run_batched(W.make_workload(1), kv.PATH_AUTO, k, expect_kernels=4, expect_memcpys=8)
+    _run_batched(W.make_workload(1), kv.PATH_ZEROCOPY, k, expect_kernels=2, expect_memcpys=0)
+    _run_batched(W.make_workload(1), kv.PATH_AUTO, k, expect_kernels=2, expect_memcpys=0, tuning={"group_bytes": 1 << 30, "auto_threshold_bytes": 1 << 30})   # one group, below the staged threshold
+    # sliding-window + full layers (config 3 scaled: 256 KiB and 32 MiB layers alternate): groups {0,1,2} {3,4} {5}
     wl = W.make_workload(3, scale=1 / 8, n_layers=6)
-    _run_batched(wl, kv.PATH_AUTO, KERNELS[kernel], expect_kernels=2 * (1 + 3))       # 3 tiny layers in one launch + 3 staged
-    _run_batched(wl, kv.PATH_ZEROCOPY, KERNELS[kernel], expect_kernels=2)
-    _run_batched(wl, kv.PATH_STAGED, KERNELS[kernel], expect_kernels=12)
-    # more layers than one launch holds (64), ragged block size, some empty layers
-    g = W.Geometry(n_layers=150, n_kv_heads=1, head_dim=80)
+    _run_batched(wl, kv.PATH_AUTO, k, expect_kernels=6, expect_memcpys=24)
+    _run_batched(wl, kv.PATH_STAGED, k, expect_kernels=6, expect_memcpys=24)
+    _run_batched(wl, kv.PATH_ZEROCOPY, k, expect_kernels=2, expect_memcpys=0)
+    _run_batched(wl, kv.PATH_STAGED, k, expect_kernels=12, expect_memcpys=48, tuning={"group_bytes": 1})      # every layer alone
+    # more layers than one launch holds (64), 160-byte payloads (stripes need alignment padding inside a group)
+    g = W.Geometry(n_layers=150, n_kv_heads=1, head_dim=40, block_tokens=1)
     rng = np.random.default_rng(23)
     wl = W.Workload(78, "many-tiny-layers", g, (0,), 40, [W.Request(rng.permutation(40)[:29].astype(np.int32))], 3, (3.0, 2.0, 1.0),
                     sliding_layers=tuple(range(0, 150, 7)))
-    _run_batched(wl, kv.PATH_ZEROCOPY, KERNELS[kernel], expect_kernels=2 * 3)
+    _run_batched(wl, kv.PATH_ZEROCOPY, k, expect_kernels=2 * 3)
+    _run_batched(wl, kv.PATH_STAGED, k, expect_kernels=2 * 3, expect_memcpys=2 * 3 * 3)
