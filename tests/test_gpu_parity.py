@@ -382,3 +382,43 @@ def test_batched_layers_grouped_launches(kernel):
                     sliding_layers=tuple(range(0, 150, 7)))
     _run_batched(wl, kv.PATH_ZEROCOPY, k, expect_kernels=2 * 3)
     _run_batched(wl, kv.PATH_STAGED, k, expect_kernels=2 * 3, expect_memcpys=2 * 3 * 3)
+
+
+def test_numa_bound_registered_and_write_combined_pool_buffers():
+    """Pool-device flavours: mmap + mbind(node 0) + cudaHostRegister, a node that does not exist (falls back unless
+    KVPOOL_DEV_NUMA_STRICT, then ENUMA), and write-combined buffers — all bit-exact through both paths."""
+    g = W.Geometry(n_layers=2, n_kv_heads=2, head_dim=64)
+    rng = np.random.default_rng(29)
+    wl = _custom(g, 300, [rng.permutation(300)[:256]], 3, (2.0, 1.0, 1.0))
+    cap = [8 << 20] * 3
+    with pytest.raises(kv.KvPoolError) as e:
+        kv.KvPool([2.0, 1.0, 1.0], cap, n_layers=2, n_kv_heads=2, head_dim=64, numa_nodes=[0, 977, 0], dev_flags=[0, kv.DEV_NUMA_STRICT, 0])
+    assert e.value.code == kv.ENUMA
+    for numa, flags in (([0, 0, -1], [kv.DEV_NUMA_STRICT, 0, 0]), ([0, 977, -1], [0, 0, 0]), (None, [kv.DEV_WRITE_COMBINED] * 3)):
+        pool = kv.KvPool([2.0, 1.0, 1.0], cap, n_layers=2, n_kv_heads=2, head_dim=64, numa_nodes=numa, dev_flags=flags)
+        try:
+            if numa is not None:
+                assert pool.device_info(0)["numa_node"] == 0                         # pages really sit on the bound node
+            opl = oracle.place([2.0, 1.0, 1.0], wl.blocks_per_layer(0))
+            for path in (kv.PATH_STAGED, kv.PATH_ZEROCOPY):
+                pool.set_path(path)
+                pl = pool.place(wl.blocks_per_layer(0))
+                for l in range(2):
+                    table_np = np.ascontiguousarray(wl.layer_table(0, l))
+                    table = torch.from_numpy(table_np).cuda()
+                    src = W.kv_layer_torch(wl, l, "cuda:0")
+                    pool.offload(pl, l, src[0], src[1], g.kvb, table)
+                    pool.wait_offloads(pl)
+                    torch.cuda.synchronize()
+                    want = oracle.offload_layer(W.kv_layer_numpy(wl, l), table_np, opl[l])
+                    for i in range(3):
+                        assert np.array_equal(np.array(pl.stripe(l, i)), want[i])
+                    dst = W.poison_torch((2, wl.nphys, g.kvb // 2), "cuda:0")
+                    pool.retrieve(pl, l, dst[0], dst[1], g.kvb, table)
+                    torch.cuda.synchronize()
+                    ref = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+                    oracle.retrieve_layer(ref, table_np, opl[l], want)
+                    assert np.array_equal(dst.cpu().numpy().view(np.uint16), ref)
+                pl.release()
+        finally:
+            pool.destroy()
