@@ -85,6 +85,9 @@ struct StageSlot {
   uint8_t* buf = nullptr;
   cudaEvent_t kernel_done = nullptr;          // last kernel that read/wrote the slot
   cudaEvent_t gate = nullptr;                 // scratch: fans one stream's waits out to the other I/O streams
+  uint32_t copies_after_kernel = 0;           // devices whose copy_done must also be awaited before reuse: set by an
+                                              // offload (D2H copies follow the pack); a retrieve's copies precede its
+                                              // unpack, so kernel_done alone covers them
   std::vector<cudaEvent_t> copy_done;         // [N] last memcpy per pool stream that read/wrote the slot
 };
 
@@ -285,8 +288,16 @@ int launch_counted(kvpool* p, const LayerArgs& a, bool pack, bool link_bound, cu
 // Make `s` wait until the previous user of a staging slot is done with it.
 int wait_slot_free(kvpool* p, StageSlot& slot, cudaStream_t s) {
   CU(cudaStreamWaitEvent(s, slot.kernel_done, 0));
-  for (uint32_t i = 0; i < p->n; ++i) CU(cudaStreamWaitEvent(s, slot.copy_done[i], 0));
+  for (uint32_t i = 0; i < p->n; ++i)
+    if (slot.copies_after_kernel >> i & 1u) CU(cudaStreamWaitEvent(s, slot.copy_done[i], 0));
   return KVPOOL_OK;
+}
+
+// An offload that has certainly landed needs no further stream waits.
+void settle_landed(LayerState& L) {
+  if (!L.landed_pending) return;
+  if (cudaEventQuery(L.landed) == cudaSuccess) L.landed_pending = false;
+  else cudaGetLastError();  // cudaErrorNotReady is not an error
 }
 
 }  // namespace
@@ -667,6 +678,7 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
   StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
   rc = wait_slot_free(p, slot, s);
   if (rc != KVPOOL_OK) return rc;
+  slot.copies_after_kernel = 0;
   for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload);
   rc = launch_counted(p, a, true, false, s);
   if (rc != KVPOOL_OK) return rc;
@@ -680,6 +692,7 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
                        bytes, cudaMemcpyDeviceToHost, p->io[i]));
     p->n_memcpys++;
     CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+    slot.copies_after_kernel |= 1u << i;
   }
   // `landed` must mean "all stripes done": record it on a stream that has waited for every copy
   {
@@ -725,6 +738,7 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
 
   if (!staged) {
     for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
+    settle_landed(L);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
     return launch_counted(p, a, false, true, s);
   }
@@ -734,6 +748,7 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   if (p->slots.empty() || L.map->K * p->payload > p->slot_bytes)
     return fail(KVPOOL_ESTATE, "retrieve: no staging slot large enough (the placement was made while the path was zero-copy)");
   StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
+  settle_landed(L);
   uint32_t lo[KVPOOL_MAX_DEVICES], hi[KVPOOL_MAX_DEVICES];
   for (uint32_t i = 0; i < N; ++i) {
     if (n_blocks == L.map->K) { lo[i] = 0; hi[i] = L.map->counts[i]; }
@@ -743,6 +758,7 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
     if (rc != KVPOOL_OK) return rc;
     if (L.landed_pending) CU(cudaStreamWaitEvent(p->io[i], L.landed, 0));
   }
+  slot.copies_after_kernel = 0;
   for (uint32_t i = 0; i < N; ++i) {
     uint8_t* stage_i = slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload;   // same layout as a full layer
     a.pool_base[i] = reinterpret_cast<uint64_t>(stage_i);
@@ -874,6 +890,7 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   bool gated = false;
   for (uint32_t b = 0; b < g.n; ++b) {
     LayerState& L = c.pl->layers[c.first + g.q[b]];
+    settle_landed(L);
     if (L.landed_pending) { CU(cudaStreamWaitEvent(lead, L.landed, 0)); gated = true; }
   }
 
@@ -881,6 +898,7 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   if (c.pack) {
     rc = wait_slot_free(p, slot, c.s);
     if (rc != KVPOOL_OK) return rc;
+    slot.copies_after_kernel = 0;
     rc = launch_multi_counted(p, ma, true, false, c.s);
     if (rc != KVPOOL_OK) return rc;
     CU(cudaEventRecord(slot.kernel_done, c.s));
@@ -892,6 +910,7 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
       CU(cudaMemcpyAsync(static_cast<uint8_t*>(p->bufs[i].host) + span_lo[i], slot.buf + dev_start[i], span[i], cudaMemcpyDeviceToHost, p->io[i]));
       p->n_memcpys++;
       CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+      slot.copies_after_kernel |= 1u << i;
     }
     for (uint32_t i = 0; i < N; ++i)
       if (span[i] && p->io[i] != lead) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
@@ -907,6 +926,7 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
     rc = wait_slot_free(p, slot, p->io[i]);
     if (rc != KVPOOL_OK) return rc;
   }
+  slot.copies_after_kernel = 0;
   if (gated) CU(cudaEventRecord(slot.gate, lead));
   for (uint32_t i = 0; i < N; ++i) {
     if (!span[i]) continue;
