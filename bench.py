@@ -58,6 +58,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", choices=["hbm", "link"], default=None,
                     help="tuning sweep instead of the benchmark: in-device pack/unpack (hbm) or zero-copy transfer (link) GB/s over launch shapes")
+    ap.add_argument("--variants", action="store_true",
+                    help="time the transfer variants side by side on --config (default 2): per-block cudaMemcpyAsync, staged, zero-copy")
     ap.add_argument("--blocked-io", action="store_true",
                     help="blocked-I/O-time analog (PAPER.md:70-72, Fig. 2/4): retrieve + consumer stand-in per layer, serial vs layerwise "
                          "pipelined, over context lengths 1K..128K for the three model shapes")
@@ -626,6 +628,88 @@ def run_sweep(args) -> None:
     pool.destroy()
 
 
+def run_variants(args) -> None:
+    """V0 per-block cudaMemcpyAsync (what an engine without a gather kernel does), V2 pack/unpack kernel + one
+    cudaMemcpyAsync per stripe (the north star's baseline path), V3 zero-copy 16-byte vector kernel, V4 zero-copy
+    cp.async.bulk kernel.  Whole request, per-layer calls, legs timed apart with CUDA events.  Text table on stdout."""
+    import torch
+    from paper_2606_14779_b200 import binding as kv
+    from paper_2606_14779_b200 import workloads as W
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    cfg = args.config if args.config != 4 or "--config" in sys.argv else 2
+    wl = W.make_workload(cfg)
+    g, L = wl.geom, wl.geom.n_layers
+    bw = list(wl.default_weights())
+    share = np.array(bw) / np.sum(bw)
+    moved = int(wl.blocks_per_layer(0).sum()) * g.payload
+    caps = [int(moved * sh * 1.25) + (L + 4) * (g.payload + 4096) for sh in share]
+    pool = kv.KvPool(bw, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim)
+    h2d = pool.measure_bandwidth(0, 0, min(256 << 20, caps[0]), 5)
+    d2h = pool.measure_bandwidth(0, 1, min(256 << 20, caps[0]), 5)
+    bpl = wl.blocks_per_layer(0)
+    elems = g.kvb // 2
+    src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+    dst = [W.poison_torch((2, wl.nphys, elems), dev) for l in range(L)]
+    tables_np = [np.ascontiguousarray(wl.layer_table(0, l)) for l in range(L)]
+    tables = [torch.from_numpy(t).to(dev) for t in tables_np]
+    s = torch.cuda.Stream(device=dev)
+    torch.cuda.synchronize()
+    print(f"# bench.py --variants --config {cfg}: {wl.name}, {moved / 2**20:.0f} MiB per leg over {L} layers, {wl.n_pool_devices} pool buffers; "
+          f"cudaMemcpyAsync 256 MiB: H2D {h2d:.2f} D2H {d2h:.2f} GB/s; median of 3")
+    print(f"{'variant':58s} {'offload GB/s':>12s} {'retrieve GB/s':>13s} {'x H2D peak':>10s} {'kernels':>8s} {'memcpys':>8s}")
+    variants = [
+        ("V0 per-block cudaMemcpyAsync (2*K_l calls per layer)", "naive", {}),
+        ("V2 staged: vec16 pack/unpack + 1 memcpy per stripe", kv.PATH_STAGED, dict(kernel=kv.KERNEL_VEC16)),
+        ("V2 staged: bulk pack/unpack + 1 memcpy per stripe", kv.PATH_STAGED, dict(kernel=kv.KERNEL_BULK)),
+        ("V3 zero-copy vec16 kernel, 8 CTAs", kv.PATH_ZEROCOPY, dict(link_kernel=kv.KERNEL_VEC16, link_ctas=8)),
+        ("V4 zero-copy cp.async.bulk kernel, 4 CTAs", kv.PATH_ZEROCOPY, dict(link_kernel=kv.KERNEL_BULK, link_ctas=4)),
+        ("V4 zero-copy cp.async.bulk kernel, 2 CTAs", kv.PATH_ZEROCOPY, dict(link_kernel=kv.KERNEL_BULK, link_ctas=2)),
+    ]
+    for name, path, tune in variants:
+        if path != "naive":
+            pool.set_path(path)
+            pool.set_tuning(**tune)
+        offs, rets = [], []
+        k0, m0 = pool.stats()
+        for it in range(4):
+            for d in dst:
+                d.fill_(np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item())
+            pl = pool.place(bpl)
+            torch.cuda.synchronize()
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            ev[0].record(s)
+            for l in range(L):
+                if path == "naive":
+                    pool.offload_naive(pl, l, src[l][0], src[l][1], g.kvb, tables_np[l], s)
+                else:
+                    pool.offload(pl, l, src[l][0], src[l][1], g.kvb, tables[l], s)
+            pool.wait_offloads(pl, s)
+            ev[1].record(s)
+            s.synchronize()
+            pool.synchronize()
+            ev[2].record(s)
+            for l in range(L):
+                if path == "naive":
+                    pool.retrieve_naive(pl, l, dst[l][0], dst[l][1], g.kvb, tables_np[l], s)
+                else:
+                    pool.retrieve(pl, l, dst[l][0], dst[l][1], g.kvb, tables[l], s)
+            ev[3].record(s)
+            s.synchronize()
+            pl.release()
+            if it > 0:
+                offs.append(ev[0].elapsed_time(ev[1]))
+                rets.append(ev[2].elapsed_time(ev[3]))
+        k1, m1 = pool.stats()
+        for l in range(L):
+            if not torch.equal(dst[l][:, tables[l].long()], src[l][:, tables[l].long()]):
+                raise RuntimeError(f"{name}: retrieved KV differs from the source")
+        o, r = moved / statistics.median(offs) / 1e6, moved / statistics.median(rets) / 1e6
+        print(f"{name:58s} {o:12.2f} {r:13.2f} {r / h2d:10.3f} {(k1 - k0) // 4:8d} {(m1 - m0) // 4:8d}", flush=True)
+    pool.destroy()
+
+
 def run_blocked_io(args) -> None:
     """Blocked I/O time = time during which only KV retrieval proceeds, with no overlapping GPU computation.
     Consumer stand-in per layer = kvpool_checksum over the layer's retrieved blocks (reads K_l*P bytes through the block
@@ -738,6 +822,9 @@ def main():
         return
     if args.blocked_io:
         run_blocked_io(args)
+        return
+    if args.variants:
+        run_variants(args)
         return
     out = run_kvpool(args)
     if out is None:

@@ -173,6 +173,14 @@ KVPOOL_API int kvpool_retrieve_layers(kvpool_t* pool, kvpool_placement_t* pl, ui
 KVPOOL_API int kvpool_retrieve_range(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks,
                           void* k_base /*device*/, void* v_base /*device*/, uint64_t block_stride_bytes,
                           const int32_t* block_table_dev, void* cuda_stream);
+/* Comparison baseline, not a product path: what an engine without a gather kernel does — one cudaMemcpyAsync per
+ * K block and per V block (2*K_l calls) straight between the paged blocks and the stripes, all on `stream`.
+ * block_table_host is the HOST copy of the layer's table.  Same results as kvpool_offload / kvpool_retrieve;
+ * exists so that bench.py --variants can time it next to the kernel paths.                                        */
+KVPOOL_API int kvpool_offload_naive(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, const void* k_base /*device*/,
+                         const void* v_base /*device*/, uint64_t block_stride_bytes, const int32_t* block_table_host, void* cuda_stream);
+KVPOOL_API int kvpool_retrieve_naive(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, void* k_base /*device*/, void* v_base /*device*/,
+                          uint64_t block_stride_bytes, const int32_t* block_table_host, void* cuda_stream);
 /* Make `stream` wait until every offload enqueued so far with `pl` has landed in the pool.             */
 KVPOOL_API int kvpool_wait_offloads(kvpool_t* pool, kvpool_placement_t* pl, void* cuda_stream);
 /* Block the host until all work the pool enqueued on its own streams is done (not the caller's).       */

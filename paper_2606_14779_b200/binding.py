@@ -25,7 +25,7 @@ _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA",
 EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
     "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_place", "kvpool_release",
-    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
+    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_counts", "kvpool_lookup", "kvpool_stripe",
     "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_last_error", "kvpool_version",
 ]
@@ -83,6 +83,8 @@ def lib():
             "kvpool_retrieve_range": [vp, vp, c_uint32, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_offload_layers": [vp, vp, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_retrieve_layers": [vp, vp, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
+            "kvpool_offload_naive": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp],
+            "kvpool_retrieve_naive": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_wait_offloads": [vp, vp, vp],
             "kvpool_synchronize": [vp],
             "kvpool_pack": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp, vp],
@@ -279,6 +281,14 @@ class KvPool:
         ka, va, ta = self._ptr_array(k_bases), self._ptr_array(v_bases), self._ptr_array(block_tables)
         _ck(lib().kvpool_retrieve_layers(self.handle, pl.handle, first_layer, n, ctypes.addressof(ka), ctypes.addressof(va),
                                          block_stride_bytes, ctypes.addressof(ta), _stream(stream)))
+
+    def offload_naive(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_host: np.ndarray, stream=None) -> None:
+        t = np.ascontiguousarray(block_table_host, dtype=np.int32)
+        _ck(lib().kvpool_offload_naive(self.handle, pl.handle, layer, _addr(k_base), _addr(v_base), block_stride_bytes, t.ctypes.data, _stream(stream)))
+
+    def retrieve_naive(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_host: np.ndarray, stream=None) -> None:
+        t = np.ascontiguousarray(block_table_host, dtype=np.int32)
+        _ck(lib().kvpool_retrieve_naive(self.handle, pl.handle, layer, _addr(k_base), _addr(v_base), block_stride_bytes, t.ctypes.data, _stream(stream)))
 
     def pack(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_dev, stage_dev, stream=None) -> None:
         _ck(lib().kvpool_pack(self.handle, pl.handle, layer, _addr(k_base), _addr(v_base), block_stride_bytes,

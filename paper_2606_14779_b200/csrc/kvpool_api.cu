@@ -1014,6 +1014,48 @@ int kvpool_retrieve_layers(kvpool_t* p, kvpool_placement_t* pl, uint32_t first_l
   return layers_batched(p, pl, false, first_layer, n_layers, k_bases, v_bases, stride, tables, cuda_stream);
 }
 
+// Baseline for comparison: 2*K_l individual cudaMemcpyAsync calls per layer, no kernel.
+static int naive_layer(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, bool pack, const void* k_base, const void* v_base, uint64_t stride,
+                       const int32_t* table_host, void* cuda_stream) {
+  int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table_host);
+  if (rc != KVPOOL_OK) return rc;
+  LayerState& L = pl->layers[layer];
+  if (!pack && !L.offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", layer);
+  if (pack) L.offloaded = true;
+  DeviceGuard guard(p->cuda_device);
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
+  for (uint64_t j = 0; j < L.map->K; ++j) {
+    const uint32_t d = L.map->dev[j];
+    uint8_t* pooled = static_cast<uint8_t*>(p->bufs[d].host) + L.stripe_off[d] + static_cast<uint64_t>(L.map->slot[j]) * p->payload;
+    uint8_t* kb = static_cast<uint8_t*>(const_cast<void*>(k_base)) + static_cast<uint64_t>(table_host[j]) * stride;
+    uint8_t* vb = static_cast<uint8_t*>(const_cast<void*>(v_base)) + static_cast<uint64_t>(table_host[j]) * stride;
+    if (pack) {
+      CU(cudaMemcpyAsync(pooled, kb, p->kvb, cudaMemcpyDeviceToHost, s));
+      CU(cudaMemcpyAsync(pooled + p->kvb, vb, p->kvb, cudaMemcpyDeviceToHost, s));
+    } else {
+      CU(cudaMemcpyAsync(kb, pooled, p->kvb, cudaMemcpyHostToDevice, s));
+      CU(cudaMemcpyAsync(vb, pooled + p->kvb, p->kvb, cudaMemcpyHostToDevice, s));
+    }
+    p->n_memcpys += 2;
+  }
+  if (pack && L.map->K) {
+    CU(cudaEventRecord(L.landed, s));
+    L.landed_pending = true;
+  }
+  return KVPOOL_OK;
+}
+
+int kvpool_offload_naive(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
+                         const int32_t* table_host, void* cuda_stream) {
+  return naive_layer(p, pl, layer, true, k_base, v_base, stride, table_host, cuda_stream);
+}
+
+int kvpool_retrieve_naive(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
+                          const int32_t* table_host, void* cuda_stream) {
+  return naive_layer(p, pl, layer, false, k_base, v_base, stride, table_host, cuda_stream);
+}
+
 int kvpool_wait_offloads(kvpool_t* p, kvpool_placement_t* pl, void* cuda_stream) {
   if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "wait_offloads: bad arguments");
   DeviceGuard guard(p->cuda_device);

@@ -422,3 +422,31 @@ def test_numa_bound_registered_and_write_combined_pool_buffers():
                 pl.release()
         finally:
             pool.destroy()
+
+
+def test_naive_per_block_memcpy_baseline_matches_oracle():
+    """The comparison baseline (one cudaMemcpyAsync per K/V block) produces the same stripes and the same retrieve."""
+    wl = W.make_workload(4, scale=1 / 32, n_layers=2)
+    g, dev = wl.geom, torch.device("cuda:0")
+    bw = list(wl.default_weights())
+    pool = make_pool(wl)
+    try:
+        pl = pool.place(wl.blocks_per_layer(0))
+        opl = oracle.place(bw, wl.blocks_per_layer(0))
+        for l in range(g.n_layers):
+            table_np = np.ascontiguousarray(wl.layer_table(0, l))
+            src = W.kv_layer_torch(wl, l, dev)
+            pool.offload_naive(pl, l, src[0], src[1], g.kvb, table_np)
+            torch.cuda.synchronize()
+            want = oracle.offload_layer(W.kv_layer_numpy(wl, l), table_np, opl[l])
+            for i in range(pool.n_devices):
+                assert np.array_equal(pl.stripe(l, i), want[i])
+            dst = W.poison_torch((2, wl.nphys, g.kvb // 2), dev)
+            pool.retrieve_naive(pl, l, dst[0], dst[1], g.kvb, table_np)
+            torch.cuda.synchronize()
+            ref = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+            oracle.retrieve_layer(ref, table_np, opl[l], want)
+            assert np.array_equal(dst.cpu().numpy().view(np.uint16), ref)
+        pl.release()
+    finally:
+        pool.destroy()
