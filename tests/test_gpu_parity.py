@@ -450,3 +450,15 @@ def test_naive_per_block_memcpy_baseline_matches_oracle():
         pl.release()
     finally:
         pool.destroy()
+
+
+def test_plain_c_client_creates_a_pool_on_the_gpu(tmp_path):
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    exe, lib_dir = str(tmp_path / "c_abi_client"), os.path.dirname(kv.LIB_PATH)
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-I", os.path.join(root, "include"), os.path.join(root, "tests", "c_abi_client.c"),
+                    "-o", exe, "-L", lib_dir, "-lkvpool", f"-Wl,-rpath,{lib_dir}"], check=True)
+    out = subprocess.run([exe, "gpu"], check=True, capture_output=True, text=True).stdout.splitlines()
+    d, s = oracle.wrr(oracle.counts([2000, 1000], 64), 64)
+    assert out[-1] == f"glt block 63: device {int(d[63])} type 0 slot {int(s[63])} ptr set"

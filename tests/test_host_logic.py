@@ -122,3 +122,17 @@ def test_product_does_not_import_oracle_and_oracle_does_not_import_product():
             assert "paper_2606_14779_b200" not in src.replace("paper_2606_14779_b200/", "") or f == "__init__.py"
             assert not re.search(r"^\s*(from|import)\s+paper_2606_14779_b200", src, re.M), f
             assert "kvpool.h" not in src, f
+
+
+def test_plain_c_client_compiles_against_header_and_runs(tmp_path):
+    """include/kvpool.h is valid C99 and the library is usable from C with nothing but pointers and sizes."""
+    import subprocess
+    exe = str(tmp_path / "c_abi_client")
+    lib_dir = os.path.dirname(kv.LIB_PATH)
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"),
+                    os.path.join(ROOT, "tests", "c_abi_client.c"), "-o", exe, "-L", lib_dir, "-lkvpool", f"-Wl,-rpath,{lib_dir}"], check=True)
+    out = subprocess.run([exe], check=True, capture_output=True, text=True).stdout.splitlines()
+    assert out[0] == "counts 2341 2341 1170 1170 585 585"
+    od, _ = oracle.wrr(oracle.counts([4000, 4000, 2000, 2000, 1000, 1000], 64), 64)
+    assert out[1] == "dev " + " ".join(str(int(d)) for d in od[:16])
+    assert out[2].startswith('error "plan_weights') and out[3].startswith("kvpool")
