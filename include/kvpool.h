@@ -43,7 +43,8 @@ enum {
   KVPOOL_ENOMEM = -2, /* a pool device has no room for its stripe, or host/device allocation failed */
   KVPOOL_ECUDA = -3,  /* a CUDA runtime call failed (message has the CUDA error string) */
   KVPOOL_ENUMA = -4,  /* KVPOOL_DEV_NUMA_STRICT and the pages could not be bound to the requested node */
-  KVPOOL_ESTATE = -5  /* retrieve of a layer that was never offloaded; release with work in flight; ... */
+  KVPOOL_ESTATE = -5, /* retrieve of a layer that was never offloaded; release with work in flight; ... */
+  KVPOOL_ENOENT = -6  /* kvpool_glt_find: no KV cache with that identifier */
 };
 
 /* pool-device flags */
@@ -216,6 +217,16 @@ KVPOOL_API int kvpool_counts(const kvpool_placement_t* pl, uint32_t layer, uint3
 KVPOOL_API int kvpool_lookup(const kvpool_placement_t* pl, uint32_t layer, uint32_t block, uint32_t* device_id, uint32_t* type,
                   uint32_t* slot, void** host_ptr);
 KVPOOL_API int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, void** host_ptr, uint64_t* nbytes);
+/* Keyed GLT (Table I `key` = "hash of the KV cache identifier"): give the K_l KV caches of a layer
+ * caller-chosen 64-bit identifiers (e.g. the prefix-hash of the tokens a block covers, mixed with the layer), after
+ * which any of them is found by identifier alone, across placements — what cross-request prefix reuse needs.
+ * kvpool_glt_bind: EINVAL, nothing bound, if an identifier is already bound or repeats.  Identifiers die with their
+ * placement (kvpool_release).  kvpool_glt_find returns the Table I fields plus where the entry lives: key (the
+ * 64-bit hash the table is indexed by), device_id, type (0 = MEM), location (host pointer of the payload), and the
+ * (placement, layer, block) to hand to kvpool_retrieve_range.  Any out pointer may be NULL.  ENOENT if absent.      */
+KVPOOL_API int kvpool_glt_bind(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, const uint64_t* ids /*host[K_l]*/);
+KVPOOL_API int kvpool_glt_find(kvpool_t* pool, uint64_t id, uint64_t* key, uint32_t* device_id, uint32_t* type, void** location,
+                    kvpool_placement_t** pl, uint32_t* layer, uint32_t* block);
 /* Whole-layer copies of the dense GLT columns (host[K_l] each; either may be NULL).                    */
 KVPOOL_API int kvpool_layer_map(const kvpool_placement_t* pl, uint32_t layer, uint8_t* dev_out, uint32_t* slot_out);
 /* Work counters since create: kernels launched and cudaMemcpyAsync calls issued by the library.        */

@@ -16,18 +16,18 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libkvpool.so")
 
 MAX_DEVICES = 32
-OK, EINVAL, ENOMEM, ECUDA, ENUMA, ESTATE = 0, -1, -2, -3, -4, -5
+OK, EINVAL, ENOMEM, ECUDA, ENUMA, ESTATE, ENOENT = 0, -1, -2, -3, -4, -5, -6
 DEV_WRITE_COMBINED, DEV_NUMA_STRICT = 1, 2
 PATH_AUTO, PATH_STAGED, PATH_ZEROCOPY = 0, 1, 2
 KERNEL_VEC16, KERNEL_BULK = 0, 1
-_ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA", ESTATE: "ESTATE"}
+_ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA", ESTATE: "ESTATE", ENOENT: "ENOENT"}
 
 EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
     "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_place", "kvpool_release",
     "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_counts", "kvpool_lookup", "kvpool_stripe",
-    "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_last_error", "kvpool_version",
+    "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_last_error", "kvpool_version",
 ]
 
 
@@ -97,6 +97,9 @@ def lib():
             "kvpool_counts": [vp, c_uint32, vp],
             "kvpool_lookup": [vp, c_uint32, c_uint32, POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32), POINTER(vp)],
             "kvpool_stripe": [vp, c_uint32, c_uint32, POINTER(vp), POINTER(c_uint64)],
+            "kvpool_glt_bind": [vp, vp, c_uint32, vp],
+            "kvpool_glt_find": [vp, c_uint64, POINTER(c_uint64), POINTER(c_uint32), POINTER(c_uint32), POINTER(vp), POINTER(vp),
+                                POINTER(c_uint32), POINTER(c_uint32)],
             "kvpool_layer_map": [vp, c_uint32, vp, vp],
             "kvpool_stats": [vp, POINTER(c_uint64), POINTER(c_uint64)],
             "kvpool_set_profiling": [vp, c_int],
@@ -310,6 +313,17 @@ class KvPool:
 
     def synchronize(self) -> None:
         _ck(lib().kvpool_synchronize(self.handle))
+
+    def glt_bind(self, pl: Placement, layer: int, ids) -> None:
+        a = np.ascontiguousarray(ids, dtype=np.uint64)
+        assert a.shape[0] == int(pl.blocks_per_layer[layer])
+        _ck(lib().kvpool_glt_bind(self.handle, pl.handle, layer, a.ctypes.data))
+
+    def glt_find(self, ident: int) -> dict:
+        key, d, t, loc, ph, layer, block = c_uint64(), c_uint32(), c_uint32(), c_void_p(), c_void_p(), c_uint32(), c_uint32()
+        _ck(lib().kvpool_glt_find(self.handle, int(ident), byref(key), byref(d), byref(t), byref(loc), byref(ph), byref(layer), byref(block)))
+        return {"key": key.value, "device_id": d.value, "type": t.value, "location": loc.value or 0, "placement": ph.value,
+                "layer": layer.value, "block": block.value}
 
     def weights(self) -> np.ndarray:
         w = np.zeros(self.n_devices, dtype=np.uint64)

@@ -93,8 +93,23 @@ struct StageSlot {
 
 }  // namespace
 
+struct GltHash {  // Table I `key`: splitmix64 finaliser of the identifier
+  static uint64_t mix(uint64_t z) {
+    z += 0x9E3779B97F4A7C15ull;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    return z ^ (z >> 31);
+  }
+  size_t operator()(uint64_t id) const { return static_cast<size_t>(mix(id)); }
+};
+struct GltRef {
+  kvpool_placement* pl;
+  uint32_t layer, block;
+};
+
 struct kvpool_placement {
   kvpool* pool = nullptr;
+  std::vector<uint64_t> bound_ids;  // identifiers bound through kvpool_glt_bind, erased at release
   std::vector<LayerState> layers;
   std::vector<uint64_t> region_off, region_bytes;  // [N] one contiguous region per pool device holds all layers' stripes
   uint8_t* tables_d = nullptr;   // every LayerMap's dev/slot columns, contiguous
@@ -122,6 +137,7 @@ struct kvpool {
   int path = KVPOOL_PATH_AUTO;
   kvpool_tuning tune{};
   std::vector<kvpool_placement*> live;
+  std::unordered_map<uint64_t, GltRef, GltHash> glt;  // keyed GLT: identifier -> (placement, layer, block)
   uint64_t n_kernels = 0, n_memcpys = 0;
   bool profiling = false;
   std::vector<ProfRec> prof;
@@ -206,6 +222,7 @@ cudaError_t take_event(kvpool* p, cudaEvent_t* e) {
 }
 
 void destroy_placement(kvpool* p, kvpool_placement* pl) {
+  for (uint64_t id : pl->bound_ids) p->glt.erase(id);
   for (uint32_t i = 0; i < p->n && i < pl->region_off.size(); ++i) p->alloc[i].free(pl->region_off[i], pl->region_bytes[i]);
   for (auto& L : pl->layers)
     if (L.landed) p->ev_free.push_back(L.landed);
@@ -1174,6 +1191,39 @@ int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, vo
   if (host_ptr) *host_ptr = bytes ? static_cast<uint8_t*>(pl->pool->bufs[dev].host) + L.stripe_off[dev] : nullptr;
   if (nbytes) *nbytes = bytes;
   return KVPOOL_OK;
+}
+
+int kvpool_glt_bind(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const uint64_t* ids) {
+  if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "glt_bind: bad pool or placement");
+  if (layer >= pl->layers.size()) return fail(KVPOOL_EINVAL, "glt_bind: layer %u out of range", layer);
+  const uint64_t K = pl->layers[layer].map->K;
+  if (K == 0) return KVPOOL_OK;
+  if (!ids) return fail(KVPOOL_EINVAL, "glt_bind: null ids");
+  std::lock_guard<std::mutex> lock(p->mu);
+  std::unordered_map<uint64_t, GltRef, GltHash> fresh;
+  fresh.reserve(K);
+  for (uint64_t j = 0; j < K; ++j) {
+    if (p->glt.count(ids[j])) return fail(KVPOOL_EINVAL, "glt_bind: identifier 0x%llx is already bound", (unsigned long long)ids[j]);
+    if (!fresh.emplace(ids[j], GltRef{pl, layer, static_cast<uint32_t>(j)}).second)
+      return fail(KVPOOL_EINVAL, "glt_bind: identifier 0x%llx repeats", (unsigned long long)ids[j]);
+  }
+  p->glt.insert(fresh.begin(), fresh.end());
+  pl->bound_ids.insert(pl->bound_ids.end(), ids, ids + K);
+  return KVPOOL_OK;
+}
+
+int kvpool_glt_find(kvpool_t* p, uint64_t id, uint64_t* key, uint32_t* device_id, uint32_t* type, void** location, kvpool_placement_t** pl,
+                    uint32_t* layer, uint32_t* block) {
+  if (!p) return fail(KVPOOL_EINVAL, "glt_find: null pool");
+  std::lock_guard<std::mutex> lock(p->mu);
+  const auto it = p->glt.find(id);
+  if (it == p->glt.end()) return fail(KVPOOL_ENOENT, "glt_find: identifier 0x%llx is not in the table", (unsigned long long)id);
+  const GltRef& r = it->second;
+  if (key) *key = GltHash::mix(id);
+  if (pl) *pl = r.pl;
+  if (layer) *layer = r.layer;
+  if (block) *block = r.block;
+  return kvpool_lookup(r.pl, r.layer, r.block, device_id, type, nullptr, location);
 }
 
 int kvpool_layer_map(const kvpool_placement_t* pl, uint32_t layer, uint8_t* dev_out, uint32_t* slot_out) {

@@ -462,3 +462,56 @@ def test_plain_c_client_creates_a_pool_on_the_gpu(tmp_path):
     out = subprocess.run([exe, "gpu"], check=True, capture_output=True, text=True).stdout.splitlines()
     d, s = oracle.wrr(oracle.counts([2000, 1000], 64), 64)
     assert out[-1] == f"glt block 63: device {int(d[63])} type 0 slot {int(s[63])} ptr set"
+
+
+def test_keyed_glt_finds_blocks_across_placements_and_forgets_them_on_release():
+    """Table I with its `key` column: identifiers bound to the blocks of two requests are found by identifier alone
+    and give the same (device_id, type, location) as the dense lookup; a found run retrieves through
+    kvpool_retrieve_range; release forgets the identifiers.  (Semantics only: parity unpinned, R15.)"""
+    g = W.Geometry(n_layers=2, n_kv_heads=2, head_dim=64)
+    rng = np.random.default_rng(31)
+    wl = _custom(g, 200, [rng.permutation(200)[:96]], 3, (3.0, 2.0, 1.0))
+    pool = make_pool(wl, slack=4.0)
+    try:
+        a, b = pool.place([96, 96]), pool.place([40, 0])
+        ids_a = [rng.integers(0, 2 ** 63, size=96, dtype=np.uint64) for _ in range(2)]
+        ids_b = rng.integers(0, 2 ** 63, size=40, dtype=np.uint64)
+        for l in range(2):
+            pool.glt_bind(a, l, ids_a[l])
+        pool.glt_bind(b, 0, ids_b)
+        pool.glt_bind(b, 1, [])                                                       # K_l = 0
+        for pl, l, ids in ((a, 0, ids_a[0]), (a, 1, ids_a[1]), (b, 0, ids_b)):
+            for j in (0, len(ids) - 1, 17):
+                f = pool.glt_find(int(ids[j]))
+                d, t, s, ptr = pl.lookup(l, j)
+                assert (f["placement"], f["layer"], f["block"], f["device_id"], f["type"], f["location"]) == (pl.handle, l, j, d, t, ptr)
+        assert len({pool.glt_find(int(i))["key"] for i in ids_b}) == 40                # distinct hash keys
+        for bad in ([int(ids_b[3])] + [1, 2, 3] * 13, [5] * 40):                     # already bound / repeating: nothing bound
+            with pytest.raises(kv.KvPoolError) as e:
+                pool.glt_bind(b, 0, bad[:40])
+            assert e.value.code == kv.EINVAL
+        with pytest.raises(kv.KvPoolError) as e:
+            pool.glt_find(1)
+        assert e.value.code == kv.ENOENT
+        # prefix reuse: find a run of request a's layer-0 blocks by identifier, then fetch exactly that run
+        table_np = np.ascontiguousarray(wl.layer_table(0, 0))
+        table = torch.from_numpy(table_np).cuda()
+        src = W.kv_layer_torch(wl, 0, "cuda:0")
+        pool.offload(a, 0, src[0], src[1], g.kvb, table)
+        first = pool.glt_find(int(ids_a[0][8]))
+        assert (first["layer"], first["block"]) == (0, 8)
+        dst = W.poison_torch((2, wl.nphys, g.kvb // 2), "cuda:0")
+        pool.retrieve_range(a, 0, first["block"], 24, dst[0], dst[1], g.kvb, table)
+        torch.cuda.synchronize()
+        opl = oracle.place([3.0, 2.0, 1.0], [96])[0]
+        ref = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+        oracle.retrieve_range(ref, table_np, opl, oracle.offload_layer(W.kv_layer_numpy(wl, 0), table_np, opl), 8, 24)
+        assert np.array_equal(dst.cpu().numpy().view(np.uint16), ref)
+        b.release()
+        with pytest.raises(kv.KvPoolError) as e:
+            pool.glt_find(int(ids_b[0]))
+        assert e.value.code == kv.ENOENT
+        assert pool.glt_find(int(ids_a[1][95]))["block"] == 95
+        a.release()
+    finally:
+        pool.destroy()
