@@ -66,6 +66,9 @@ def parse_args():
     ap.add_argument("--interference", action="store_true",
                     help="in-device pack/unpack and a plain torch copy of the same size, alone and under a concurrent cudaMemcpyAsync over "
                          "the host link (explains the in-step kernel time of the staged path)")
+    ap.add_argument("--mixed-pool", action="store_true",
+                    help="HBM-type pool devices (KVPOOL_DEV_HBM; the pool's own GPU standing in for an NVLink peer) next to a pinned "
+                         "host device: bandwidth-proportional split by measured weights, offload / retrieve GB/s (DESIGN.md §11)")
     ap.add_argument("--compute-us", type=float, default=0.0, help="--blocked-io: extra calibrated compute per layer (kvpool_spin), microseconds")
     ap.add_argument("--detail", default=None, help="write per-layer latencies and side measurements to this JSON file")
     return ap.parse_args()
@@ -828,6 +831,76 @@ def run_interference(args) -> None:
     pool.destroy()
 
 
+def run_mixed_pool(args) -> None:
+    """Eq. 1-2 at work on devices of very different speed: one pinned host buffer (PCIe) and one HBM-type device, alone and
+    together, weights = kvpool_measure_bandwidth of each.  Whole request (16 layers of --config), batched calls, legs
+    timed apart with CUDA events; every run is verified bit-exact against the source.  Text table on stdout."""
+    import torch
+    from paper_2606_14779_b200 import binding as kv
+    from paper_2606_14779_b200 import workloads as W
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    L = 16
+    wl = W.make_workload(args.config, n_layers=L)
+    wl.sliding_layers = ()
+    g = wl.geom
+    bpl = wl.blocks_per_layer(0)
+    K, moved = int(bpl[0]), int(bpl.sum()) * g.payload
+    elems = g.kvb // 2
+    src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+    dst = [W.poison_torch((2, wl.nphys, elems), dev) for l in range(L)]
+    tables = [torch.from_numpy(np.ascontiguousarray(wl.layer_table(0, l))).to(dev) for l in range(L)]
+    src_k, src_v, dst_k, dst_v = [x[0] for x in src], [x[1] for x in src], [x[0] for x in dst], [x[1] for x in dst]
+    s = torch.cuda.Stream(device=dev)
+    torch.cuda.synchronize()
+    cap = moved + (L + 4) * (g.payload + 4096)
+    print(f"# bench.py --mixed-pool --config {args.config}: {wl.name} cut to {L} layers, {moved / 2**20:.0f} MiB per leg ({K} blocks of {g.payload} B per layer); "
+          "weights = kvpool_measure_bandwidth (256 MiB cudaMemcpyAsync, payload GB/s); median of 3; HBM-type device = this GPU's own memory")
+    print(f"{'pool':34s} {'weights (GB/s)':>22s} {'blocks per layer':>18s} {'offload GB/s':>12s} {'retrieve GB/s':>13s} {'sum of weights':>14s} {'kernels':>8s} {'memcpys':>8s}")
+    for name, flags in (("1 host buffer", [0]), ("1 host buffer + 1 HBM device", [0, kv.DEV_HBM]), ("2 host buffers + 2 HBM devices", [0, 0, kv.DEV_HBM, kv.DEV_HBM]),
+                        ("1 HBM device", [kv.DEV_HBM])):
+        n = len(flags)
+        pool = kv.KvPool([1.0] * n, [cap] * n, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, dev_flags=flags)
+        bw = [pool.measure_bandwidth(i, 0, 256 << 20, 5) for i in range(n)]
+        # devices behind ONE shared resource (the host buffers behind this box's single PCIe link; HBM-type devices in the
+        # same GPU's memory) are each worth their share of it, not the whole of it
+        n_host, n_hbm = sum(1 for f in flags if not f), sum(1 for f in flags if f)
+        bw = [b / (n_hbm if f else n_host) for b, f in zip(bw, flags)]
+        pool.set_bandwidth(bw)
+        offs, rets = [], []
+        k0, m0 = pool.stats()
+        for it in range(4):
+            for d in dst:
+                d.fill_(np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item())
+            pl = pool.place(bpl)
+            counts = list(pl.counts(0))
+            torch.cuda.synchronize()
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            ev[0].record(s)
+            pool.offload_layers(pl, 0, src_k, src_v, g.kvb, tables, s)
+            pool.wait_offloads(pl, s)
+            ev[1].record(s)
+            s.synchronize()
+            pool.synchronize()
+            ev[2].record(s)
+            pool.retrieve_layers(pl, 0, dst_k, dst_v, g.kvb, tables, s)
+            ev[3].record(s)
+            s.synchronize()
+            pl.release()
+            if it > 0:
+                offs.append(ev[0].elapsed_time(ev[1]))
+                rets.append(ev[2].elapsed_time(ev[3]))
+        k1, m1 = pool.stats()
+        for l in range(L):
+            if not torch.equal(dst[l][:, tables[l].long()], src[l][:, tables[l].long()]):
+                raise RuntimeError(f"{name}: retrieved KV differs from the source")
+        o, r = moved / statistics.median(offs) / 1e6, moved / statistics.median(rets) / 1e6
+        print(f"{name:34s} {'/'.join(f'{b:.0f}' for b in bw):>22s} {'/'.join(str(c) for c in counts):>18s} {o:12.1f} {r:13.1f} {sum(bw):14.0f} "
+              f"{(k1 - k0) // 4:8d} {(m1 - m0) // 4:8d}", flush=True)
+        pool.destroy()
+
+
 def run_blocked_io(args) -> None:
     """Blocked I/O time = time during which only KV retrieval proceeds, with no overlapping GPU computation.
     Consumer stand-in per layer = kvpool_checksum over the layer's retrieved blocks (reads K_l*P bytes through the block
@@ -946,6 +1019,9 @@ def main():
         return
     if args.interference:
         run_interference(args)
+        return
+    if args.mixed_pool:
+        run_mixed_pool(args)
         return
     out = run_kvpool(args)
     if out is None:

@@ -50,6 +50,16 @@ enum {
 /* pool-device flags */
 #define KVPOOL_DEV_WRITE_COMBINED 1u /* cudaHostAllocWriteCombined (GPU-read-mostly; CPU reads become slow) */
 #define KVPOOL_DEV_NUMA_STRICT 2u    /* fail with ENUMA instead of falling back when binding is impossible */
+#define KVPOOL_DEV_HBM 4u            /* the pool device is GPU memory, not host memory: HBM of GPU `gpu` — an NVLink / NVSwitch
+                                        peer of the pool's GPU, or that GPU itself.  Its stripes are reached
+                                        by the kernels directly (peer loads / stores); no staging, no copy engine.            */
+
+/* pool-device types (GLT `type`, Table I) */
+enum {
+  KVPOOL_TYPE_MEM = 0, /* pinned host memory; location = host pointer                                     */
+  KVPOOL_TYPE_SSD = 1, /* the paper's second type (location = LBA); not built: no NVMe on the box         */
+  KVPOOL_TYPE_HBM = 2  /* GPU memory (KVPOOL_DEV_HBM); location = device pointer valid on the pool's GPU  */
+};
 
 /* transfer paths (kvpool_set_path) */
 enum {
@@ -66,11 +76,15 @@ enum {
 typedef struct kvpool kvpool_t;                     /* opaque pool                                       */
 typedef struct kvpool_placement kvpool_placement_t; /* opaque: one request's GLT + reserved stripes      */
 
-typedef struct {           /* one pool device (MEM type; Table I)                          */
+typedef struct {           /* one pool device (Table I)                                    */
   double bandwidth_gbps;   /* b_i of Eq. 1, measured, in 1e9 B/s; > 0                                   */
-  uint64_t capacity_bytes; /* size of the pinned, mapped host buffer the library allocates; > 0         */
-  int32_t numa_node;       /* -1 = no preference; else bind the pages to this node (mbind)              */
+  uint64_t capacity_bytes; /* size of the buffer the library allocates (pinned + mapped host memory, or */
+                           /* device memory with KVPOOL_DEV_HBM); > 0                                   */
+  int32_t numa_node;       /* MEM: -1 = no preference; else bind the pages to this node (mbind)         */
   uint32_t flags;          /* KVPOOL_DEV_*                                                              */
+  int32_t gpu;             /* HBM: CUDA ordinal of the GPU that holds the buffer, -1 = the pool's own   */
+                           /* GPU; must be peer-accessible from it (ECUDA otherwise).  MEM: ignored     */
+  uint32_t reserved;       /* 0                                                                         */
 } kvpool_device_desc;
 
 typedef struct { /* geometry of one paged KV block */
@@ -115,8 +129,8 @@ KVPOOL_API int kvpool_destroy(kvpool_t* pool);
 /* Replace the bandwidths ("measured bandwidth") — ESTATE while any placement is live.     */
 KVPOOL_API int kvpool_set_bandwidth(kvpool_t* pool, const double* bandwidth_gbps /*host[n_devs]*/);
 /* Measure pool device `dev`: cudaMemcpyAsync of `bytes` (<= capacity) between the pool buffer and a
- * scratch device buffer, `iters` times, median, CUDA events.  direction 0 = host->GPU (retrieve
- * direction), 1 = GPU->host.  Blocking; contents of the first `bytes` of the pool buffer are preserved
+ * scratch device buffer, `iters` times, median, CUDA events.  direction 0 = pool->GPU (retrieve
+ * direction), 1 = GPU->pool.  GB/s counts the bytes moved once (payload), for HBM devices too.  Blocking; contents of the first `bytes` of the pool buffer are preserved
  * for direction 0 and overwritten for direction 1 — ESTATE while any placement is live.                */
 KVPOOL_API int kvpool_measure_bandwidth(kvpool_t* pool, uint32_t dev, int direction, uint64_t bytes, uint32_t iters, double* gbps_out /*host*/);
 
@@ -211,18 +225,27 @@ KVPOOL_API int kvpool_n_devices(const kvpool_t* pool, uint32_t* n_out);
 KVPOOL_API int kvpool_weights(const kvpool_t* pool, uint64_t* w_out /*host[n_devs]*/);
 KVPOOL_API int kvpool_device_info(const kvpool_t* pool, uint32_t dev, void** host_base, uint64_t* capacity_bytes, uint64_t* used_bytes,
                        int32_t* numa_node_actual /* -1 unknown */);
+/* Type of pool device `dev` (KVPOOL_TYPE_*) and, for HBM devices, the CUDA ordinal that holds it (-1 for MEM).
+ * For an HBM device kvpool_device_info's host_base is NULL.                                              */
+KVPOOL_API int kvpool_device_type(const kvpool_t* pool, uint32_t dev, uint32_t* type, int32_t* gpu);
 KVPOOL_API int kvpool_counts(const kvpool_placement_t* pl, uint32_t layer, uint32_t* counts_out /*host[n_devs]*/);
-/* GLT entry of logical block `block` of `layer`: device_id, type (0 = MEM), slot inside that device's
- * stripe and the host pointer of its payload (Table I "location").                                     */
+/* GLT entry of logical block `block` of `layer`: device_id, type (KVPOOL_TYPE_*), slot inside that device's
+ * stripe and the location of its payload (Table I "location"): a host pointer for MEM, a device pointer for HBM. */
 KVPOOL_API int kvpool_lookup(const kvpool_placement_t* pl, uint32_t layer, uint32_t block, uint32_t* device_id, uint32_t* type,
-                  uint32_t* slot, void** host_ptr);
-KVPOOL_API int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, void** host_ptr, uint64_t* nbytes);
+                  uint32_t* slot, void** location);
+/* Stripe of `layer` on pool device `dev`: its location (host pointer for MEM, device pointer for HBM; NULL when
+ * empty) and size.                                                                                              */
+KVPOOL_API int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, void** location, uint64_t* nbytes);
+/* Copy the first `nbytes` (<= stripe size) of that stripe into host memory, whatever the device type (memcpy for MEM,
+ * blocking cudaMemcpy for HBM).  The caller must have waited for the offload (kvpool_wait_offloads + stream sync).
+ * For inspection and tests; not a hot-path call.                                                                 */
+KVPOOL_API int kvpool_stripe_read(kvpool_t* pool, const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, void* dst_host, uint64_t nbytes);
 /* Keyed GLT (Table I `key` = "hash of the KV cache identifier"): give the K_l KV caches of a layer
  * caller-chosen 64-bit identifiers (e.g. the prefix-hash of the tokens a block covers, mixed with the layer), after
  * which any of them is found by identifier alone, across placements — what cross-request prefix reuse needs.
  * kvpool_glt_bind: EINVAL, nothing bound, if an identifier is already bound or repeats.  Identifiers die with their
  * placement (kvpool_release).  kvpool_glt_find returns the Table I fields plus where the entry lives: key (the
- * 64-bit hash the table is indexed by), device_id, type (0 = MEM), location (host pointer of the payload), and the
+ * 64-bit hash the table is indexed by), device_id, type (KVPOOL_TYPE_*), location (pointer of the payload), and the
  * (placement, layer, block) to hand to kvpool_retrieve_range.  Any out pointer may be NULL.  ENOENT if absent.      */
 KVPOOL_API int kvpool_glt_bind(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, const uint64_t* ids /*host[K_l]*/);
 KVPOOL_API int kvpool_glt_find(kvpool_t* pool, uint64_t id, uint64_t* key, uint32_t* device_id, uint32_t* type, void** location,

@@ -17,7 +17,8 @@ LIB_PATH = os.path.join(_HERE, "libkvpool.so")
 
 MAX_DEVICES = 32
 OK, EINVAL, ENOMEM, ECUDA, ENUMA, ESTATE, ENOENT = 0, -1, -2, -3, -4, -5, -6
-DEV_WRITE_COMBINED, DEV_NUMA_STRICT = 1, 2
+DEV_WRITE_COMBINED, DEV_NUMA_STRICT, DEV_HBM = 1, 2, 4
+TYPE_MEM, TYPE_SSD, TYPE_HBM = 0, 1, 2
 PATH_AUTO, PATH_STAGED, PATH_ZEROCOPY = 0, 1, 2
 KERNEL_VEC16, KERNEL_BULK = 0, 1
 _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA", ESTATE: "ESTATE", ENOENT: "ENOENT"}
@@ -26,13 +27,14 @@ EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
     "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_place", "kvpool_release",
     "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
-    "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_counts", "kvpool_lookup", "kvpool_stripe",
+    "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
     "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_last_error", "kvpool_version",
 ]
 
 
 class DeviceDesc(ctypes.Structure):
-    _fields_ = [("bandwidth_gbps", c_double), ("capacity_bytes", c_uint64), ("numa_node", c_int32), ("flags", c_uint32)]
+    _fields_ = [("bandwidth_gbps", c_double), ("capacity_bytes", c_uint64), ("numa_node", c_int32), ("flags", c_uint32),
+                ("gpu", c_int32), ("reserved", c_uint32)]
 
 
 class Geometry(ctypes.Structure):
@@ -97,6 +99,8 @@ def lib():
             "kvpool_counts": [vp, c_uint32, vp],
             "kvpool_lookup": [vp, c_uint32, c_uint32, POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32), POINTER(vp)],
             "kvpool_stripe": [vp, c_uint32, c_uint32, POINTER(vp), POINTER(c_uint64)],
+            "kvpool_stripe_read": [vp, vp, c_uint32, c_uint32, vp, c_uint64],
+            "kvpool_device_type": [vp, c_uint32, POINTER(c_uint32), POINTER(c_int32)],
             "kvpool_glt_bind": [vp, vp, c_uint32, vp],
             "kvpool_glt_find": [vp, c_uint64, POINTER(c_uint64), POINTER(c_uint32), POINTER(c_uint32), POINTER(vp), POINTER(vp),
                                 POINTER(c_uint32), POINTER(c_uint32)],
@@ -178,13 +182,23 @@ class Placement:
         _ck(lib().kvpool_lookup(self.handle, layer, block, byref(d), byref(t), byref(s), byref(p)))
         return d.value, t.value, s.value, p.value or 0
 
-    def stripe(self, layer: int, dev: int) -> np.ndarray:
-        """The stripe's bytes as a uint8 numpy VIEW of the pinned pool buffer (no copy)."""
+    def stripe_location(self, layer: int, dev: int) -> Tuple[int, int]:
+        """(location, nbytes) of the stripe: a host address for a MEM device, a device address for an HBM device."""
         p, n = c_void_p(), c_uint64()
         _ck(lib().kvpool_stripe(self.handle, layer, dev, byref(p), byref(n)))
-        if n.value == 0:
+        return p.value or 0, n.value
+
+    def stripe(self, layer: int, dev: int) -> np.ndarray:
+        """The stripe's bytes as uint8: a numpy VIEW of the pinned pool buffer for a MEM device (no copy), a host
+        copy made by kvpool_stripe_read for an HBM device."""
+        loc, n = self.stripe_location(layer, dev)
+        if n == 0:
             return np.zeros(0, dtype=np.uint8)
-        return np.ctypeslib.as_array(ctypes.cast(p.value, POINTER(c_uint8)), shape=(n.value,))
+        if self.pool.device_type(dev)[0] == TYPE_HBM:
+            out = np.empty(n, dtype=np.uint8)
+            _ck(lib().kvpool_stripe_read(self.pool.handle, self.handle, layer, dev, out.ctypes.data, n))
+            return out
+        return np.ctypeslib.as_array(ctypes.cast(loc, POINTER(c_uint8)), shape=(n,))
 
     def release(self) -> None:
         if self.handle:
@@ -197,12 +211,13 @@ class KvPool:
 
     def __init__(self, bandwidth_gbps: Sequence[float], capacity_bytes: Sequence[int], *, n_layers: int, n_kv_heads: int,
                  head_dim: int, block_tokens: int = 16, elem_bytes: int = 2, cuda_device: int = 0,
-                 numa_nodes: Optional[Sequence[int]] = None, dev_flags: Optional[Sequence[int]] = None):
+                 numa_nodes: Optional[Sequence[int]] = None, dev_flags: Optional[Sequence[int]] = None,
+                 gpus: Optional[Sequence[int]] = None):
         n = len(bandwidth_gbps)
         descs = (DeviceDesc * n)()
         for i in range(n):
             descs[i] = DeviceDesc(float(bandwidth_gbps[i]), int(capacity_bytes[i]), int(numa_nodes[i]) if numa_nodes else -1,
-                                  int(dev_flags[i]) if dev_flags else 0)
+                                  int(dev_flags[i]) if dev_flags else 0, int(gpus[i]) if gpus else -1, 0)
         self.geometry = Geometry(n_layers, block_tokens, n_kv_heads, head_dim, elem_bytes)
         self.kvb = block_tokens * n_kv_heads * head_dim * elem_bytes
         self.payload = 2 * self.kvb
@@ -334,6 +349,12 @@ class KvPool:
         base, cap, used, node = c_void_p(), c_uint64(), c_uint64(), c_int32()
         _ck(lib().kvpool_device_info(self.handle, dev, byref(base), byref(cap), byref(used), byref(node)))
         return {"host_base": base.value, "capacity": cap.value, "used": used.value, "numa_node": node.value}
+
+    def device_type(self, dev: int) -> Tuple[int, int]:
+        """(TYPE_MEM | TYPE_HBM, CUDA ordinal holding an HBM device or -1)."""
+        t, g = c_uint32(), c_int32()
+        _ck(lib().kvpool_device_type(self.handle, dev, byref(t), byref(g)))
+        return t.value, g.value
 
     def stats(self) -> Tuple[int, int]:
         k, m = c_uint64(), c_uint64()

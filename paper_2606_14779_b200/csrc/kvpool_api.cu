@@ -126,6 +126,7 @@ struct kvpool {
   std::vector<double> bandwidth;
   std::vector<uint64_t> w;
   std::vector<HostBuffer> bufs;
+  uint32_t hbm_mask = 0;  // bit i: pool device i is GPU memory (KVPOOL_DEV_HBM): reached by the kernels directly, never staged or copied
   std::vector<StripeAllocator> alloc;
   std::vector<cudaStream_t> io;  // one I/O stream per pool device ("independent I/O streams")
   std::vector<StageSlot> slots;
@@ -259,7 +260,15 @@ LayerArgs base_args(const kvpool* p, const LayerState& L, const void* k_base, co
   return a;
 }
 
+inline bool is_hbm(const kvpool* p, uint32_t i) { return (p->hbm_mask >> i) & 1u; }
+// Where the CPU / copy engines find pool device i's bytes: the host address, or the device pointer of an HBM device.
+inline uint8_t* pool_bytes(const kvpool* p, uint32_t i) {
+  return static_cast<uint8_t*>(is_hbm(p, i) ? p->bufs[i].dev_alias : p->bufs[i].host);
+}
+
 LaunchCfg launch_cfg(const kvpool* p, bool link_bound) {
+  // a zero-copy launch over a pool with HBM devices moves most of its bytes at HBM / NVLink rates: give it the HBM grid
+  if (p->hbm_mask) link_bound = false;
   LaunchCfg c{};
   c.kernel = link_bound ? p->tune.link_kernel : p->tune.kernel;
   c.ctas = link_bound ? p->tune.link_ctas : p->tune.hbm_ctas;
@@ -354,7 +363,9 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
   for (uint32_t i = 0; i < n_devs; ++i) {
     bw[i] = devs[i].bandwidth_gbps;
     if (devs[i].capacity_bytes == 0) return fail(KVPOOL_EINVAL, "create: device %u has zero capacity", i);
-    if (devs[i].flags & ~(KVPOOL_DEV_WRITE_COMBINED | KVPOOL_DEV_NUMA_STRICT)) return fail(KVPOOL_EINVAL, "create: device %u unknown flags", i);
+    if (devs[i].flags & ~(KVPOOL_DEV_WRITE_COMBINED | KVPOOL_DEV_NUMA_STRICT | KVPOOL_DEV_HBM)) return fail(KVPOOL_EINVAL, "create: device %u unknown flags", i);
+    if ((devs[i].flags & KVPOOL_DEV_HBM) && (devs[i].flags & ~KVPOOL_DEV_HBM)) return fail(KVPOOL_EINVAL, "create: device %u: KVPOOL_DEV_HBM excludes the host-memory flags", i);
+    if (devs[i].reserved != 0) return fail(KVPOOL_EINVAL, "create: device %u: reserved must be 0", i);
   }
   if (!quantise_weights(bw.data(), n_devs, w.data())) return fail(KVPOOL_EINVAL, "create: bandwidth must be positive (>= 0.0005 GB/s)");
 
@@ -386,8 +397,11 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
   p->bufs.resize(n_devs);
   for (uint32_t i = 0; i < n_devs; ++i) {
     std::string err;
-    const int rc = host_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes, devs[i].numa_node, devs[i].flags & KVPOOL_DEV_WRITE_COMBINED,
-                                     devs[i].flags & KVPOOL_DEV_NUMA_STRICT, &err);
+    const bool hbm = devs[i].flags & KVPOOL_DEV_HBM;
+    const int rc = hbm ? device_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes, devs[i].gpu < 0 ? cuda_device : devs[i].gpu, cuda_device, &err)
+                       : host_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes, devs[i].numa_node, devs[i].flags & KVPOOL_DEV_WRITE_COMBINED,
+                                           devs[i].flags & KVPOOL_DEV_NUMA_STRICT, &err);
+    if (rc == KVPOOL_OK && hbm) p->hbm_mask |= 1u << i;
     if (rc != KVPOOL_OK) {
       cleanup();
       return fail(rc, "create: pool device %u (%llu bytes): %s", i, (unsigned long long)devs[i].capacity_bytes, err.c_str());
@@ -452,8 +466,8 @@ int kvpool_measure_bandwidth(kvpool_t* p, uint32_t dev, int direction, uint64_t 
   int rc = KVPOOL_OK;
   for (uint32_t it = 0; it < iters + 1 && rc == KVPOOL_OK; ++it) {  // first pass is a warm-up
     cudaEventRecord(e0, s);
-    cudaError_t e = direction == 0 ? cudaMemcpyAsync(scratch, p->bufs[dev].host, bytes, cudaMemcpyHostToDevice, s)
-                                   : cudaMemcpyAsync(p->bufs[dev].host, scratch, bytes, cudaMemcpyDeviceToHost, s);
+    cudaError_t e = direction == 0 ? cudaMemcpyAsync(scratch, pool_bytes(p, dev), bytes, cudaMemcpyDefault, s)
+                                   : cudaMemcpyAsync(pool_bytes(p, dev), scratch, bytes, cudaMemcpyDefault, s);
     cudaEventRecord(e1, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) { rc = fail(KVPOOL_ECUDA, "measure_bandwidth: %s", cudaGetErrorString(e)); break; }
@@ -696,13 +710,20 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
   rc = wait_slot_free(p, slot, s);
   if (rc != KVPOOL_OK) return rc;
   slot.copies_after_kernel = 0;
-  for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload);
+  bool hbm_blocks = false;
+  for (uint32_t i = 0; i < N; ++i) {
+    // HBM-type devices: the pack kernel stores straight into the stripe; host devices: into the staging slot
+    a.pool_base[i] = is_hbm(p, i) ? reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i])
+                                  : reinterpret_cast<uint64_t>(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload);
+    hbm_blocks |= is_hbm(p, i) && L.map->counts[i];
+  }
+  if (hbm_blocks && L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));  // an earlier offload of this layer still writing the stripe
   rc = launch_counted(p, a, true, false, s);
   if (rc != KVPOOL_OK) return rc;
   CU(cudaEventRecord(slot.kernel_done, s));
   for (uint32_t i = 0; i < N; ++i) {
     const uint64_t bytes = static_cast<uint64_t>(L.map->counts[i]) * p->payload;
-    if (bytes == 0) continue;
+    if (bytes == 0 || is_hbm(p, i)) continue;
     CU(cudaStreamWaitEvent(p->io[i], slot.kernel_done, 0));
     if (L.landed_pending) CU(cudaStreamWaitEvent(p->io[i], L.landed, 0));
     CU(cudaMemcpyAsync(static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i], slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload,
@@ -713,16 +734,14 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
   }
   // `landed` must mean "all stripes done": record it on a stream that has waited for every copy
   {
-    cudaStream_t js = nullptr;
+    cudaStream_t js = nullptr;  // every I/O stream that copies has waited for the pack kernel, so it also covers the HBM stripes
     for (uint32_t i = 0; i < N; ++i) {
-      if (static_cast<uint64_t>(L.map->counts[i]) == 0) continue;
+      if (static_cast<uint64_t>(L.map->counts[i]) == 0 || is_hbm(p, i)) continue;
       if (!js) { js = p->io[i]; continue; }
       CU(cudaStreamWaitEvent(js, slot.copy_done[i], 0));
     }
-    if (js) {
-      CU(cudaEventRecord(L.landed, js));
-      L.landed_pending = true;
-    }
+    CU(cudaEventRecord(L.landed, js ? js : s));  // no host stripe at all: the kernel on `s` was the whole offload
+    L.landed_pending = true;
   }
   return KVPOOL_OK;
 }
@@ -767,19 +786,23 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
   settle_landed(L);
   uint32_t lo[KVPOOL_MAX_DEVICES], hi[KVPOOL_MAX_DEVICES];
+  bool hbm_blocks = false;
   for (uint32_t i = 0; i < N; ++i) {
     if (n_blocks == L.map->K) { lo[i] = 0; hi[i] = L.map->counts[i]; }
     else slot_range(*L.map, i, first_block, n_blocks, &lo[i], &hi[i]);
     if (hi[i] == lo[i]) continue;
+    if (is_hbm(p, i)) { hbm_blocks = true; continue; }  // read in place by the unpack kernel
     rc = wait_slot_free(p, slot, p->io[i]);
     if (rc != KVPOOL_OK) return rc;
     if (L.landed_pending) CU(cudaStreamWaitEvent(p->io[i], L.landed, 0));
   }
+  if (hbm_blocks && L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
   slot.copies_after_kernel = 0;
   for (uint32_t i = 0; i < N; ++i) {
     uint8_t* stage_i = slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload;   // same layout as a full layer
     a.pool_base[i] = reinterpret_cast<uint64_t>(stage_i);
-    if (hi[i] == lo[i]) continue;
+    if (is_hbm(p, i)) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
+    if (hi[i] == lo[i] || is_hbm(p, i)) continue;
     const uint64_t off = static_cast<uint64_t>(lo[i]) * p->payload, bytes = static_cast<uint64_t>(hi[i] - lo[i]) * p->payload;
     CU(cudaMemcpyAsync(stage_i + off, static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i] + off, bytes, cudaMemcpyHostToDevice, p->io[i]));
     p->n_memcpys++;
@@ -884,10 +907,14 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   const uint32_t N = p->n;
   const LayerState& A = c.pl->layers[c.first + g.q[0]];
   const LayerState& Z = c.pl->layers[c.first + g.q[g.n - 1]];
+  // span[i]: bytes device i's copy engine moves for the group.  HBM-type devices move nothing that way — the kernel
+  // reaches their stripes in place (delta 0) — so they take no room in the staging slot either.
   uint64_t span_lo[KVPOOL_MAX_DEVICES], span[KVPOOL_MAX_DEVICES], dev_start[KVPOOL_MAX_DEVICES], total = 0;
+  bool hbm_blocks = false;
   for (uint32_t i = 0; i < N; ++i) {
     span_lo[i] = A.stripe_off[i];
     span[i] = Z.stripe_off[i] + static_cast<uint64_t>(Z.map->counts[i]) * p->payload - span_lo[i];
+    if (is_hbm(p, i)) { hbm_blocks |= span[i] != 0; span[i] = 0; }
     dev_start[i] = total;
     total += (span[i] + 255) / 256 * 256;
   }
@@ -896,19 +923,23 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   MultiArgs ma{};
   fill_descs(c, g, &ma);
   for (uint32_t i = 0; i < N; ++i)
-    ma.delta[i] = reinterpret_cast<uint64_t>(slot.buf + dev_start[i]) - reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + span_lo[i]);
+    ma.delta[i] = is_hbm(p, i) ? 0
+                               : reinterpret_cast<uint64_t>(slot.buf + dev_start[i]) - reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + span_lo[i]);
 
   // an earlier offload of these layers that is still in flight must land before their stripes are touched again:
-  // gather those waits on the first I/O stream that has work and fan out through one event
+  // gather those waits on the first I/O stream that has work and fan out through one event; the kernel's own stream
+  // waits too when it touches HBM-type stripes directly
   cudaStream_t lead = nullptr;
   for (uint32_t i = 0; i < N && !lead; ++i)
     if (span[i]) lead = p->io[i];
-  if (!lead) return KVPOOL_OK;
+  if (!lead && !hbm_blocks) return KVPOOL_OK;
   bool gated = false;
   for (uint32_t b = 0; b < g.n; ++b) {
     LayerState& L = c.pl->layers[c.first + g.q[b]];
     settle_landed(L);
-    if (L.landed_pending) { CU(cudaStreamWaitEvent(lead, L.landed, 0)); gated = true; }
+    if (!L.landed_pending) continue;
+    if (lead) { CU(cudaStreamWaitEvent(lead, L.landed, 0)); gated = true; }
+    if (hbm_blocks) CU(cudaStreamWaitEvent(c.s, L.landed, 0));
   }
 
   int rc;
@@ -931,9 +962,9 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
     }
     for (uint32_t i = 0; i < N; ++i)
       if (span[i] && p->io[i] != lead) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
-    for (uint32_t b = 0; b < g.n; ++b) {
+    for (uint32_t b = 0; b < g.n; ++b) {  // `lead` has waited for the kernel and every copy; with no host stripe the kernel was all
       LayerState& L = c.pl->layers[c.first + g.q[b]];
-      CU(cudaEventRecord(L.landed, lead));
+      CU(cudaEventRecord(L.landed, lead ? lead : c.s));
       L.landed_pending = true;
     }
     return KVPOOL_OK;
@@ -1044,15 +1075,15 @@ static int naive_layer(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, bool
   if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
   for (uint64_t j = 0; j < L.map->K; ++j) {
     const uint32_t d = L.map->dev[j];
-    uint8_t* pooled = static_cast<uint8_t*>(p->bufs[d].host) + L.stripe_off[d] + static_cast<uint64_t>(L.map->slot[j]) * p->payload;
+    uint8_t* pooled = pool_bytes(p, d) + L.stripe_off[d] + static_cast<uint64_t>(L.map->slot[j]) * p->payload;
     uint8_t* kb = static_cast<uint8_t*>(const_cast<void*>(k_base)) + static_cast<uint64_t>(table_host[j]) * stride;
     uint8_t* vb = static_cast<uint8_t*>(const_cast<void*>(v_base)) + static_cast<uint64_t>(table_host[j]) * stride;
     if (pack) {
-      CU(cudaMemcpyAsync(pooled, kb, p->kvb, cudaMemcpyDeviceToHost, s));
-      CU(cudaMemcpyAsync(pooled + p->kvb, vb, p->kvb, cudaMemcpyDeviceToHost, s));
+      CU(cudaMemcpyAsync(pooled, kb, p->kvb, cudaMemcpyDefault, s));
+      CU(cudaMemcpyAsync(pooled + p->kvb, vb, p->kvb, cudaMemcpyDefault, s));
     } else {
-      CU(cudaMemcpyAsync(kb, pooled, p->kvb, cudaMemcpyHostToDevice, s));
-      CU(cudaMemcpyAsync(vb, pooled + p->kvb, p->kvb, cudaMemcpyHostToDevice, s));
+      CU(cudaMemcpyAsync(kb, pooled, p->kvb, cudaMemcpyDefault, s));
+      CU(cudaMemcpyAsync(vb, pooled + p->kvb, p->kvb, cudaMemcpyDefault, s));
     }
     p->n_memcpys += 2;
   }
@@ -1178,9 +1209,9 @@ int kvpool_lookup(const kvpool_placement_t* pl, uint32_t layer, uint32_t block, 
   if (block >= L.map->K) return fail(KVPOOL_EINVAL, "lookup: block %u out of range (K %llu)", block, (unsigned long long)L.map->K);
   const uint32_t d = L.map->dev[block], s = L.map->slot[block];
   if (device_id) *device_id = d;
-  if (type) *type = 0;
+  if (type) *type = is_hbm(pl->pool, d) ? KVPOOL_TYPE_HBM : KVPOOL_TYPE_MEM;
   if (slot) *slot = s;
-  if (host_ptr) *host_ptr = static_cast<uint8_t*>(pl->pool->bufs[d].host) + L.stripe_off[d] + static_cast<uint64_t>(s) * pl->pool->payload;
+  if (host_ptr) *host_ptr = pool_bytes(pl->pool, d) + L.stripe_off[d] + static_cast<uint64_t>(s) * pl->pool->payload;
   return KVPOOL_OK;
 }
 
@@ -1188,8 +1219,32 @@ int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, vo
   if (!pl || layer >= pl->layers.size() || dev >= pl->pool->n) return fail(KVPOOL_EINVAL, "stripe: bad arguments");
   const LayerState& L = pl->layers[layer];
   const uint64_t bytes = static_cast<uint64_t>(L.map->counts[dev]) * pl->pool->payload;
-  if (host_ptr) *host_ptr = bytes ? static_cast<uint8_t*>(pl->pool->bufs[dev].host) + L.stripe_off[dev] : nullptr;
+  if (host_ptr) *host_ptr = bytes ? pool_bytes(pl->pool, dev) + L.stripe_off[dev] : nullptr;
   if (nbytes) *nbytes = bytes;
+  return KVPOOL_OK;
+}
+
+int kvpool_stripe_read(kvpool_t* p, const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, void* dst_host, uint64_t nbytes) {
+  if (!p || !pl || pl->pool != p || !is_live(p, pl) || layer >= pl->layers.size() || dev >= p->n) return fail(KVPOOL_EINVAL, "stripe_read: bad arguments");
+  const LayerState& L = pl->layers[layer];
+  const uint64_t bytes = static_cast<uint64_t>(L.map->counts[dev]) * p->payload;
+  if (nbytes > bytes) return fail(KVPOOL_EINVAL, "stripe_read: %llu bytes exceed the stripe's %llu", (unsigned long long)nbytes, (unsigned long long)bytes);
+  if (nbytes == 0) return KVPOOL_OK;
+  if (!dst_host) return fail(KVPOOL_EINVAL, "stripe_read: null destination");
+  const uint8_t* src = pool_bytes(p, dev) + L.stripe_off[dev];
+  if (is_hbm(p, dev)) {
+    DeviceGuard guard(p->cuda_device);
+    CU(cudaMemcpy(dst_host, src, nbytes, cudaMemcpyDeviceToHost));
+  } else {
+    memcpy(dst_host, src, nbytes);
+  }
+  return KVPOOL_OK;
+}
+
+int kvpool_device_type(const kvpool_t* p, uint32_t dev, uint32_t* type, int32_t* gpu) {
+  if (!p || dev >= p->n) return fail(KVPOOL_EINVAL, "device_type: bad arguments");
+  if (type) *type = is_hbm(p, dev) ? KVPOOL_TYPE_HBM : KVPOOL_TYPE_MEM;
+  if (gpu) *gpu = p->bufs[dev].gpu;
   return KVPOOL_OK;
 }
 

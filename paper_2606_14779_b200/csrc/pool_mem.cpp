@@ -82,7 +82,50 @@ int host_buffer_alloc(HostBuffer* hb, uint64_t bytes, int numa_node, bool write_
   return KVPOOL_OK;
 }
 
+int device_buffer_alloc(HostBuffer* hb, uint64_t bytes, int gpu, int pool_gpu, std::string* err) {
+  *hb = HostBuffer{};
+  hb->bytes = bytes;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || gpu < 0 || gpu >= ndev) {
+    cudaGetLastError();
+    *err = "GPU " + std::to_string(gpu) + " does not exist";
+    return KVPOOL_EINVAL;
+  }
+  if (gpu != pool_gpu) {
+    int can = 0;
+    cudaError_t e = cudaDeviceCanAccessPeer(&can, pool_gpu, gpu);
+    if (e != cudaSuccess || !can) {
+      cudaGetLastError();
+      *err = "GPU " + std::to_string(pool_gpu) + " cannot access GPU " + std::to_string(gpu) + " as a peer";
+      return KVPOOL_ECUDA;
+    }
+    e = cudaDeviceEnablePeerAccess(gpu, 0);  // current device is pool_gpu
+    if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) {
+      *err = std::string("cudaDeviceEnablePeerAccess: ") + cudaGetErrorString(e);
+      return KVPOOL_ECUDA;
+    }
+    cudaGetLastError();
+    cudaSetDevice(gpu);
+  }
+  void* m = nullptr;
+  const cudaError_t e = cudaMalloc(&m, bytes);
+  if (gpu != pool_gpu) cudaSetDevice(pool_gpu);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    *err = std::string("cudaMalloc: ") + cudaGetErrorString(e);
+    return e == cudaErrorMemoryAllocation ? KVPOOL_ENOMEM : KVPOOL_ECUDA;
+  }
+  hb->dev_alias = m;
+  hb->gpu = gpu;
+  return KVPOOL_OK;
+}
+
 void host_buffer_free(HostBuffer* hb) {
+  if (hb->gpu >= 0) {
+    if (hb->dev_alias) cudaFree(hb->dev_alias);  // UVA: cudaFree finds the owning device
+    *hb = HostBuffer{};
+    return;
+  }
   if (!hb->host) return;
   if (hb->registered) {
     cudaHostUnregister(hb->host);

@@ -1,4 +1,5 @@
-// Pinned, GPU-mapped, optionally NUMA-bound host buffers: the MEM-type pool devices.
+// Pool-device buffers: pinned, GPU-mapped, optionally NUMA-bound host memory (the MEM type of PAPER.md:132, 155), or
+// device memory of the pool's GPU / an NVLink peer (the HBM type).
 #pragma once
 #include <cstdint>
 #include <string>
@@ -6,8 +7,9 @@
 namespace kvp {
 
 struct HostBuffer {
-  void* host = nullptr;      // CPU address
-  void* dev_alias = nullptr; // address the GPU uses for the same bytes (UVA: normally equal to host)
+  void* host = nullptr;      // CPU address; nullptr for an HBM-type buffer
+  void* dev_alias = nullptr; // address the pool's GPU uses for the bytes (MEM: UVA alias of host; HBM: the device pointer)
+  int gpu = -1;              // HBM type: CUDA ordinal that holds the buffer; -1 = MEM type
   uint64_t bytes = 0;
   int numa_requested = -1;
   int numa_actual = -1;      // node of the first page after touching, -1 if it cannot be queried
@@ -17,6 +19,9 @@ struct HostBuffer {
 // Returns 0 or a KVPOOL_E* code and fills err.  strict_numa: fail instead of falling back when the
 // pages cannot be bound to numa_node.
 int host_buffer_alloc(HostBuffer* hb, uint64_t bytes, int numa_node, bool write_combined, bool strict_numa, std::string* err);
+// HBM-type buffer: cudaMalloc on `gpu`, peer access enabled from `pool_gpu` when they differ.  The current device is
+// `pool_gpu` on entry and on return.
+int device_buffer_alloc(HostBuffer* hb, uint64_t bytes, int gpu, int pool_gpu, std::string* err);
 void host_buffer_free(HostBuffer* hb);
 int numa_node_count();
 

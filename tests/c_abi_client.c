@@ -22,7 +22,7 @@ int main(int argc, char **argv) {
     printf("error \"%s\"\n", kvpool_last_error());
     printf("%s\n", kvpool_version());
     if (argc > 1 && strcmp(argv[1], "gpu") == 0) {
-        kvpool_device_desc d[2] = {{2.0, 8u << 20, -1, 0}, {1.0, 8u << 20, -1, 0}};
+        kvpool_device_desc d[2] = {{2.0, 8u << 20, -1, 0, -1, 0}, {1.0, 8u << 20, -1, KVPOOL_DEV_HBM, -1, 0}};
         kvpool_geometry g = {2, 16, 2, 64, 2};
         kvpool_t *pool = NULL;
         kvpool_placement_t *pl = NULL;
@@ -32,6 +32,8 @@ int main(int argc, char **argv) {
         if (kvpool_place(pool, bpl, &pl) != KVPOOL_OK) return 3;
         if (kvpool_lookup(pl, 0, 63, &id, &type, &s, &ptr) != KVPOOL_OK) return 3;
         printf("glt block 63: device %u type %u slot %u ptr %s\n", id, type, s, ptr ? "set" : "null");
+        if (kvpool_lookup(pl, 0, 2, &id, &type, &s, &ptr) != KVPOOL_OK) return 3;
+        printf("glt block 2: device %u type %u slot %u ptr %s\n", id, type, s, ptr ? "set" : "null");
         if (kvpool_release(pool, pl) != KVPOOL_OK || kvpool_destroy(pool) != KVPOOL_OK) return 3;
     }
     return 0;

@@ -12,7 +12,8 @@ from paper_2606_14779_b200 import binding as kv
 from paper_2606_14779_b200 import workloads as W
 
 
-def make_pool(wl: W.Workload, bandwidth: Optional[Sequence[float]] = None, slack: float = 1.25) -> kv.KvPool:
+def make_pool(wl: W.Workload, bandwidth: Optional[Sequence[float]] = None, slack: float = 1.25,
+              dev_flags: Optional[Sequence[int]] = None) -> kv.KvPool:
     bw = list(bandwidth) if bandwidth is not None else list(wl.default_weights())
     total = wl.moved_bytes()
     share = np.array(bw) / np.sum(bw)
@@ -20,7 +21,7 @@ def make_pool(wl: W.Workload, bandwidth: Optional[Sequence[float]] = None, slack
     caps = [int(total * s * slack) + (wl.geom.n_layers * len(wl.requests) + 4) * (wl.geom.payload + 4096) for s in share]
     g = wl.geom
     return kv.KvPool(bw, caps, n_layers=g.n_layers, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim,
-                     block_tokens=g.block_tokens, elem_bytes=g.elem_bytes)
+                     block_tokens=g.block_tokens, elem_bytes=g.elem_bytes, dev_flags=dev_flags)
 
 
 def check_placement(pl: kv.Placement, opl: List[oracle.LayerPlacement]) -> None:
@@ -38,20 +39,19 @@ def check_glt(pl: kv.Placement, opl: List[oracle.LayerPlacement], payload: int, 
         K = len(o.dev)
         for j in ([0, K - 1] + list(rng.integers(0, K, size=min(sample, K)))) if K else []:
             d, t, s, ptr = pl.lookup(l, int(j))
-            assert (d, t, s) == (int(o.dev[j]), 0, int(o.slot[j]))
-            stripe = pl.stripe(l, d)
-            assert ptr == stripe.ctypes.data + s * payload
+            assert (d, t, s) == (int(o.dev[j]), pl.pool.device_type(d)[0], int(o.slot[j]))
+            assert ptr == pl.stripe_location(l, d)[0] + s * payload
 
 
 def run_parity(wl: W.Workload, *, path: int, kernel: int, bandwidth=None, tuning: Optional[dict] = None,
-               interleaved_layout: bool = False, streams: int = 1) -> dict:
+               interleaved_layout: bool = False, streams: int = 1, dev_flags: Optional[Sequence[int]] = None) -> dict:
     """Offload every layer of every request, compare stripes with the oracle, retrieve into a poisoned pool,
     compare with the oracle's retrieve and with the source.  Returns a few counters."""
     dev = torch.device("cuda:0")
     g = wl.geom
     elems = g.kvb // 2
     bw = list(bandwidth) if bandwidth is not None else list(wl.default_weights())
-    pool = make_pool(wl, bw)
+    pool = make_pool(wl, bw, dev_flags=dev_flags)
     try:
         pool.set_path(path)
         pool.set_tuning(kernel=kernel, link_kernel=kernel, **(tuning or {}))

@@ -316,13 +316,13 @@ def test_checksum_consumer_matches_oracle_and_detects_round_trip():
             pool.destroy()
 
 
-def _run_batched(wl, path, kernel, expect_kernels=None, expect_memcpys=None, tuning=None):
+def _run_batched(wl, path, kernel, expect_kernels=None, expect_memcpys=None, tuning=None, dev_flags=None):
     """Offload and retrieve ALL layers with one kvpool_offload_layers / kvpool_retrieve_layers call each and compare
     every stripe and every retrieved layer with the oracle."""
     dev = torch.device("cuda:0")
     g, L = wl.geom, wl.geom.n_layers
     bw = list(wl.default_weights())
-    pool = make_pool(wl)
+    pool = make_pool(wl, dev_flags=dev_flags)
     try:
         pool.set_path(path)
         pool.set_tuning(kernel=kernel, link_kernel=kernel, **(tuning or {}))
@@ -461,7 +461,10 @@ def test_plain_c_client_creates_a_pool_on_the_gpu(tmp_path):
                     "-o", exe, "-L", lib_dir, "-lkvpool", f"-Wl,-rpath,{lib_dir}"], check=True)
     out = subprocess.run([exe, "gpu"], check=True, capture_output=True, text=True).stdout.splitlines()
     d, s = oracle.wrr(oracle.counts([2000, 1000], 64), 64)
-    assert out[-1] == f"glt block 63: device {int(d[63])} type 0 slot {int(s[63])} ptr set"
+    # pool device 1 of the client is an HBM-type device (KVPOOL_TYPE_HBM = 2), device 0 pinned host memory (MEM = 0)
+    assert out[-2] == f"glt block 63: device {int(d[63])} type {2 * int(d[63])} slot {int(s[63])} ptr set"
+    assert out[-1] == f"glt block 2: device {int(d[2])} type {2 * int(d[2])} slot {int(s[2])} ptr set"
+    assert {int(d[63]), int(d[2])} == {1}
 
 
 def test_keyed_glt_finds_blocks_across_placements_and_forgets_them_on_release():
@@ -513,5 +516,96 @@ def test_keyed_glt_finds_blocks_across_placements_and_forgets_them_on_release():
         assert e.value.code == kv.ENOENT
         assert pool.glt_find(int(ids_a[1][95]))["block"] == 95
         a.release()
+    finally:
+        pool.destroy()
+
+
+HBM = kv.DEV_HBM
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+@pytest.mark.parametrize("path", ["staged", "zerocopy", "auto"])
+def test_hbm_type_pool_devices_alone_and_mixed_with_host_devices(path, kernel):
+    """KVPOOL_DEV_HBM: pool devices that are GPU memory — here the pool's own GPU, standing in for an
+    NVLink peer — next to pinned host devices.  Same placement, same stripe bytes, same retrieved tensors as the oracle;
+    GLT type = KVPOOL_TYPE_HBM and location = a device pointer for their blocks (checked in run_parity / check_glt)."""
+    p, k = PATHS[path], KERNELS[kernel]
+    # config 1 whole (2 devices 2:1), the slower one in HBM: staged path = 1 pack launch + ONE copy (device 0) per layer
+    out = run_parity(W.make_workload(1), path=p, kernel=k, dev_flags=[0, HBM])
+    assert out["kernels"] == 64 and out["memcpys"] == (64 if path == "staged" else 0)
+    # config 4 cut (6 devices 4:4:2:2:1:1, 16 MiB layers), devices 0 and 3 in HBM
+    out = run_parity(W.make_workload(4, scale=1 / 16, n_layers=3), path=p, kernel=k, dev_flags=[HBM, 0, 0, HBM, 0, 0])
+    assert out["memcpys"] == (0 if path == "zerocopy" else 2 * 3 * 4)
+    # every device in HBM: no copy engine at all, whatever the path
+    out = run_parity(W.make_workload(4, scale=1 / 16, n_layers=2), path=p, kernel=k, dev_flags=[HBM] * 6)
+    assert out["memcpys"] == 0
+    # ragged block size, K < N, sliding-window layers (config 3 scaled: 8-block and 1024-block layers alternate)
+    rng = np.random.default_rng(31)
+    g = W.Geometry(n_layers=2, n_kv_heads=1, head_dim=80)
+    run_parity(_custom(g, 301, [rng.permutation(301)[:257]], 3, (3.0, 2.0, 1.0)), path=p, kernel=k, dev_flags=[HBM, 0, HBM])
+    g = W.Geometry(n_layers=1, n_kv_heads=1, head_dim=8, block_tokens=1)
+    run_parity(_custom(g, 9, [[7, 2, 5]], 6, (4.0, 4.0, 2.0, 2.0, 1.0, 1.0)), path=p, kernel=k, dev_flags=[0, HBM, 0, HBM, 0, HBM])
+    run_parity(W.make_workload(3, scale=1 / 8, n_layers=4), path=p, kernel=k, dev_flags=[0, HBM, HBM, 0])
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_hbm_type_pool_devices_batched_groups_and_ranges(kernel):
+    k = KERNELS[kernel]
+    # batched calls: a group's host stripes travel by one copy per HOST device, its HBM stripes inside the kernel
+    _run_batched(W.make_workload(1), kv.PATH_AUTO, k, expect_kernels=4, expect_memcpys=4, dev_flags=[0, HBM])
+    _run_batched(W.make_workload(1), kv.PATH_STAGED, k, expect_kernels=4, expect_memcpys=0, dev_flags=[HBM, HBM])
+    _run_batched(W.make_workload(1), kv.PATH_ZEROCOPY, k, expect_kernels=2, expect_memcpys=0, dev_flags=[HBM, 0])
+    wl = W.make_workload(3, scale=1 / 8, n_layers=6)                      # groups {0,1,2} {3,4} {5}; 4 devices, 2 of them host
+    _run_batched(wl, kv.PATH_STAGED, k, expect_kernels=6, expect_memcpys=12, dev_flags=[HBM, 0, 0, HBM])
+    # partial retrieval over a mixed pool
+    wl = W.make_workload(4, scale=1 / 16, n_layers=1)
+    g, dev = wl.geom, torch.device("cuda:0")
+    bw = list(wl.default_weights())
+    for path in (kv.PATH_STAGED, kv.PATH_ZEROCOPY):
+        pool = make_pool(wl, dev_flags=[0, HBM, 0, HBM, HBM, 0])
+        try:
+            pool.set_path(path)
+            pool.set_tuning(kernel=k, link_kernel=k)
+            pl = pool.place(wl.blocks_per_layer(0))
+            opl = oracle.place(bw, wl.blocks_per_layer(0))
+            table_np = np.ascontiguousarray(wl.layer_table(0, 0))
+            K, table = len(table_np), torch.from_numpy(table_np).to(dev)
+            src, src_cpu = W.kv_layer_torch(wl, 0, dev), W.kv_layer_numpy(wl, 0)
+            pool.offload(pl, 0, src[0], src[1], g.kvb, table)
+            pool.wait_offloads(pl)
+            torch.cuda.synchronize()
+            stripes = oracle.offload_layer(src_cpu, table_np, opl[0])
+            for first, n in ((0, K // 4), (K // 3, K // 2), (K - 1, 1), (0, K), (5, 0), (17, 3)):
+                dst = W.poison_torch((2, wl.nphys, g.kvb // 2), dev)
+                pool.retrieve_range(pl, 0, first, n, dst[0], dst[1], g.kvb, table)
+                torch.cuda.synchronize()
+                want = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+                oracle.retrieve_range(want, table_np, opl[0], stripes, first, n)
+                assert np.array_equal(dst.cpu().numpy().view(np.uint16), want), (path, first, n)
+            pl.release()
+        finally:
+            pool.destroy()
+
+
+def test_hbm_type_pool_device_introspection_bandwidth_and_errors():
+    g = dict(n_layers=1, n_kv_heads=2, head_dim=64)
+    with pytest.raises(kv.KvPoolError) as e:                                       # HBM excludes the host-memory flags
+        kv.KvPool([1.0], [1 << 20], dev_flags=[HBM | kv.DEV_WRITE_COMBINED], **g)
+    assert e.value.code == kv.EINVAL
+    with pytest.raises(kv.KvPoolError) as e:                                       # a GPU that does not exist
+        kv.KvPool([1.0], [1 << 20], dev_flags=[HBM], gpus=[torch.cuda.device_count() + 3], **g)
+    assert e.value.code == kv.EINVAL
+    pool = kv.KvPool([50.0, 1500.0], [64 << 20, 64 << 20], dev_flags=[0, HBM], gpus=[-1, 0], **g)
+    try:
+        assert pool.device_type(0) == (kv.TYPE_MEM, -1) and pool.device_type(1) == (kv.TYPE_HBM, 0)
+        assert pool.device_info(0)["host_base"] and not pool.device_info(1)["host_base"]
+        host = pool.measure_bandwidth(0, 0, 32 << 20, 3)
+        hbm_r, hbm_w = pool.measure_bandwidth(1, 0, 64 << 20, 3), pool.measure_bandwidth(1, 1, 64 << 20, 3)
+        assert hbm_r > 5 * host and hbm_w > 5 * host                               # a device-to-device copy, not the host link
+        pl = pool.place([31])
+        c = pl.counts(0)
+        assert list(c) == [1, 30]                                                   # 50 : 1500 of 31 blocks
+        assert pl.stripe_location(0, 1)[1] == 30 * pool.payload
+        pl.release()
     finally:
         pool.destroy()
