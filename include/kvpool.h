@@ -198,7 +198,11 @@ KVPOOL_API int kvpool_retrieve_naive(kvpool_t* pool, kvpool_placement_t* pl, uin
                           uint64_t block_stride_bytes, const int32_t* block_table_host, void* cuda_stream);
 /* Make `stream` wait until every offload enqueued so far with `pl` has landed in the pool.             */
 KVPOOL_API int kvpool_wait_offloads(kvpool_t* pool, kvpool_placement_t* pl, void* cuda_stream);
-/* Block the host until all work the pool enqueued on its own streams is done (not the caller's).       */
+/* Block the host until all work the pool enqueued on its own streams is done (not the caller's), and note which
+ * offloads have landed.  After the caller has also synchronised its own streams, later zero-copy calls on those layers
+ * enqueue exactly one kernel on `cuda_stream` and nothing else (no event waits or queries), so a zero-copy
+ * kvpool_retrieve / kvpool_retrieve_layers / kvpool_retrieve_range can be captured into a CUDA graph and replayed
+ * (profiling off; the placement and the tables must outlive the graph).                                           */
 KVPOOL_API int kvpool_synchronize(kvpool_t* pool);
 
 /* In-device halves alone (a5 / a8): gather the layer's blocks into `stage_dev` (device, K_l*P bytes) in

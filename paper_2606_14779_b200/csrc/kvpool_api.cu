@@ -886,7 +886,7 @@ int issue_zero_copy_group(const BatchCall& c, const LayerGroup& g) {
   fill_descs(c, g, &ma);
   for (uint32_t b = 0; b < g.n; ++b) {
     LayerState& L = c.pl->layers[c.first + g.q[b]];
-    if (L.landed_pending) CU(cudaStreamWaitEvent(c.s, L.landed, 0));
+    if (L.landed_pending) CU(cudaStreamWaitEvent(c.s, L.landed, 0));  // settled (no wait) after kvpool_synchronize
   }
   const int rc = launch_multi_counted(p, ma, c.pack, true, c.s);
   if (rc != KVPOOL_OK) return rc;
@@ -1116,7 +1116,13 @@ int kvpool_wait_offloads(kvpool_t* p, kvpool_placement_t* pl, void* cuda_stream)
 int kvpool_synchronize(kvpool_t* p) {
   if (!p) return fail(KVPOOL_EINVAL, "synchronize: null pool");
   DeviceGuard guard(p->cuda_device);
-  return sync_pool_streams(p);
+  const int rc = sync_pool_streams(p);
+  if (rc != KVPOOL_OK) return rc;
+  // offloads that have landed by now need no stream waits any more: later calls on those layers enqueue nothing but
+  // their own work (which is what makes a zero-copy retrieve capturable into a CUDA graph)
+  for (auto* pl : p->live)
+    for (auto& L : pl->layers) settle_landed(L);
+  return KVPOOL_OK;
 }
 
 int kvpool_pack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,

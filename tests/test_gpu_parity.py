@@ -609,3 +609,55 @@ def test_hbm_type_pool_device_introspection_bandwidth_and_errors():
         pl.release()
     finally:
         pool.destroy()
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_zero_copy_retrieve_is_capturable_into_a_cuda_graph(kernel):
+    """Once the offloads have landed (caller's stream synchronised + kvpool_synchronize), a zero-copy retrieve enqueues one
+    kernel and nothing else, so a serving engine can capture it into its decode graph: capture per-layer, range and
+    batched retrieves, replay twice into re-poisoned destinations, compare with the oracle."""
+    wl = W.make_workload(3, scale=1 / 16, n_layers=6)          # sliding-window (8-block) and full (512-block) layers alternate
+    g, L, dev = wl.geom, wl.geom.n_layers, torch.device("cuda:0")
+    bw, bpl = list(wl.default_weights()), wl.blocks_per_layer(0)
+    pool = make_pool(wl)
+    try:
+        pool.set_path(kv.PATH_ZEROCOPY)
+        pool.set_tuning(kernel=KERNELS[kernel], link_kernel=KERNELS[kernel])
+        pl, opl = pool.place(bpl), oracle.place(bw, bpl)
+        tables_np = [np.ascontiguousarray(wl.layer_table(0, l)) for l in range(L)]
+        tables = [torch.from_numpy(t).to(dev) for t in tables_np]
+        src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+        dst = [W.poison_torch((2, wl.nphys, g.kvb // 2), dev) for l in range(L)]
+        torch.cuda.synchronize()
+        s = torch.cuda.Stream()
+        pool.offload_layers(pl, 0, [x[0] for x in src], [x[1] for x in src], g.kvb, tables, s)
+        pool.wait_offloads(pl, s)
+        s.synchronize()
+        pool.synchronize()
+        k0, m0 = pool.stats()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s, capture_error_mode="relaxed"):
+            pool.retrieve_layers(pl, 0, [d[0] for d in dst[:3]], [d[1] for d in dst[:3]], g.kvb, tables[:3], s)    # one fused launch
+            pool.retrieve(pl, 3, dst[3][0], dst[3][1], g.kvb, tables[3], s)
+            pool.retrieve_range(pl, 4, 0, 5, dst[4][0], dst[4][1], g.kvb, tables[4], s)
+            pool.retrieve_range(pl, 5, 100, 300, dst[5][0], dst[5][1], g.kvb, tables[5], s)
+        assert pool.stats() == (k0 + 4, m0)
+        want = []
+        for l in range(L):
+            stripes = oracle.offload_layer(W.kv_layer_numpy(wl, l), tables_np[l], opl[l])
+            ref = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+            first, n = {4: (0, 5), 5: (100, 300)}.get(l, (0, len(tables_np[l])))
+            oracle.retrieve_range(ref, tables_np[l], opl[l], stripes, first, n)
+            want.append(ref)
+        for _ in range(2):
+            for d in dst:
+                d.copy_(W.poison_torch(d.shape, dev))
+            torch.cuda.synchronize()
+            graph.replay()
+            torch.cuda.synchronize()
+            for l in range(L):
+                assert np.array_equal(dst[l].cpu().numpy().view(np.uint16), want[l]), f"graph replay: layer {l} differs"
+        del graph
+        pl.release()
+    finally:
+        pool.destroy()
