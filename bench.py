@@ -69,6 +69,9 @@ def parse_args():
     ap.add_argument("--mixed-pool", action="store_true",
                     help="HBM-type pool devices (KVPOOL_DEV_HBM; the pool's own GPU standing in for an NVLink peer) next to a pinned "
                          "host device: bandwidth-proportional split by measured weights, offload / retrieve GB/s (DESIGN.md §11)")
+    ap.add_argument("--duplex", action="store_true",
+                    help="offload of one request concurrent with retrieve of another (PCIe is full duplex): per-direction and aggregate "
+                         "GB/s against simultaneous cudaMemcpyAsync in both directions")
     ap.add_argument("--compute-us", type=float, default=0.0, help="--blocked-io: extra calibrated compute per layer (kvpool_spin), microseconds")
     ap.add_argument("--detail", default=None, help="write per-layer latencies and side measurements to this JSON file")
     return ap.parse_args()
@@ -901,6 +904,96 @@ def run_mixed_pool(args) -> None:
         pool.destroy()
 
 
+def run_duplex(args) -> None:
+    """A serving engine evicts one request's KV while it fetches another's.  Request A is offloaded on one stream while
+    request B (offloaded beforehand) is retrieved on another; both legs are timed with CUDA events on their own stream and
+    the pair by the wall clock.  Peak = two simultaneous 1 GiB pinned cudaMemcpyAsync, one per direction.  Text table."""
+    import torch
+    from paper_2606_14779_b200 import binding as kv
+    from paper_2606_14779_b200 import workloads as W
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    L = 16
+    wl = W.make_workload(args.config, n_layers=L)
+    wl.sliding_layers = ()
+    g = wl.geom
+    bpl = wl.blocks_per_layer(0)
+    moved = int(bpl.sum()) * g.payload
+    elems = g.kvb // 2
+    bw = list(wl.default_weights())
+    share = np.array(bw) / np.sum(bw)
+    caps = [int(2 * moved * sh * 1.25) + 2 * (L + 4) * (g.payload + 4096) for sh in share]
+    pool = kv.KvPool(bw, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim)
+    src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+    dst = [W.poison_torch((2, wl.nphys, elems), dev) for l in range(L)]
+    tables = [torch.from_numpy(np.ascontiguousarray(wl.layer_table(0, l))).to(dev) for l in range(L)]
+    src_k, src_v, dst_k, dst_v = [x[0] for x in src], [x[1] for x in src], [x[0] for x in dst], [x[1] for x in dst]
+    sa, sb = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+
+    # duplex peak of the link: simultaneous H2D and D2H copies of 1 GiB each
+    hd, dd = torch.empty(1 << 30, dtype=torch.uint8).pin_memory(), torch.empty(1 << 30, dtype=torch.uint8, device=dev)
+    hu, du = torch.empty(1 << 30, dtype=torch.uint8).pin_memory(), torch.empty(1 << 30, dtype=torch.uint8, device=dev)
+    peak = []
+    for it in range(4):
+        torch.cuda.synchronize()
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        with torch.cuda.stream(sa):
+            e[0].record(sa); dd.copy_(hd, non_blocking=True); e[1].record(sa)
+        with torch.cuda.stream(sb):
+            e[2].record(sb); hu.copy_(du, non_blocking=True); e[3].record(sb)
+        torch.cuda.synchronize()
+        if it:
+            peak.append(((1 << 30) / e[0].elapsed_time(e[1]) / 1e6, (1 << 30) / e[2].elapsed_time(e[3]) / 1e6))
+    peak_h2d, peak_d2h = statistics.median(p[0] for p in peak), statistics.median(p[1] for p in peak)
+    del hd, dd, hu, du
+    torch.cuda.synchronize()
+    print(f"# bench.py --duplex --config {args.config}: {wl.name} cut to {L} layers; request A ({moved / 2**20:.0f} MiB) is offloaded while request B "
+          f"({moved / 2**20:.0f} MiB) is retrieved; median of 3")
+    print(f"# simultaneous cudaMemcpyAsync, 1 GiB each way: H2D {peak_h2d:.1f} GB/s + D2H {peak_d2h:.1f} GB/s = {peak_h2d + peak_d2h:.1f} GB/s")
+    print(f"{'path/CTAs':12s} {'offload A GB/s':>15s} {'retrieve B GB/s':>16s} {'aggregate GB/s (wall)':>22s} {'x duplex peak':>14s}")
+    for pname, path, ctas in (("staged", kv.PATH_STAGED, 0), ("zerocopy", kv.PATH_ZEROCOPY, args.link_ctas or 4),
+                              ("zerocopy", kv.PATH_ZEROCOPY, 4 * (args.link_ctas or 4))):
+        pool.set_path(path)
+        if ctas:
+            pool.set_tuning(link_ctas=ctas)
+            pname = f"{pname}/{ctas}"
+        offs, rets, aggs = [], [], []
+        for it in range(4):
+            for d in dst:
+                d.fill_(np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item())
+            pa, pb = pool.place(bpl), pool.place(bpl)
+            torch.cuda.synchronize()
+            pool.offload_layers(pb, 0, src_k, src_v, g.kvb, tables, sb)
+            pool.wait_offloads(pb, sb)
+            sb.synchronize()
+            pool.synchronize()
+            e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            t0 = time.perf_counter()
+            e[0].record(sa)
+            e[2].record(sb)
+            for l in range(L):                      # interleave the two requests layer by layer, as a scheduler would
+                pool.offload(pa, l, src[l][0], src[l][1], g.kvb, tables[l], sa)
+                pool.retrieve(pb, l, dst[l][0], dst[l][1], g.kvb, tables[l], sb)
+            pool.wait_offloads(pa, sa)
+            e[1].record(sa)
+            e[3].record(sb)
+            torch.cuda.synchronize()
+            t1 = time.perf_counter()
+            if it:
+                offs.append(moved / e[0].elapsed_time(e[1]) / 1e6)
+                rets.append(moved / e[2].elapsed_time(e[3]) / 1e6)
+                aggs.append(2 * moved / (t1 - t0) / 1e9)
+            for l in range(L):
+                if not torch.equal(dst[l][:, tables[l].long()], src[l][:, tables[l].long()]):
+                    raise RuntimeError(f"{pname}: retrieved KV differs from the source")
+            pa.release()
+            pb.release()
+        o, r, a = statistics.median(offs), statistics.median(rets), statistics.median(aggs)
+        print(f"{pname:12s} {o:15.1f} {r:16.1f} {a:22.1f} {a / (peak_h2d + peak_d2h):14.3f}", flush=True)
+    pool.destroy()
+
+
 def run_blocked_io(args) -> None:
     """Blocked I/O time = time during which only KV retrieval proceeds, with no overlapping GPU computation.
     Consumer stand-in per layer = kvpool_checksum over the layer's retrieved blocks (reads K_l*P bytes through the block
@@ -1022,6 +1115,9 @@ def main():
         return
     if args.mixed_pool:
         run_mixed_pool(args)
+        return
+    if args.duplex:
+        run_duplex(args)
         return
     out = run_kvpool(args)
     if out is None:

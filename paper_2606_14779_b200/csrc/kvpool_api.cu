@@ -128,7 +128,8 @@ struct kvpool {
   std::vector<HostBuffer> bufs;
   uint32_t hbm_mask = 0;  // bit i: pool device i is GPU memory (KVPOOL_DEV_HBM): reached by the kernels directly, never staged or copied
   std::vector<StripeAllocator> alloc;
-  std::vector<cudaStream_t> io;  // one I/O stream per pool device ("independent I/O streams")
+  std::vector<cudaStream_t> io;      // one I/O stream per pool device ("independent I/O streams"): host -> GPU copies
+  std::vector<cudaStream_t> io_out;  // and one for GPU -> host copies, so that an offload and a retrieve use both directions of the link at once
   std::vector<StageSlot> slots;
   uint64_t slot_bytes = 0;
   uint64_t slot_cursor = 0;
@@ -176,6 +177,7 @@ void free_slots(kvpool* p) {
 
 int sync_pool_streams(kvpool* p) {
   for (auto s : p->io) CU(cudaStreamSynchronize(s));
+  for (auto s : p->io_out) CU(cudaStreamSynchronize(s));
   return KVPOOL_OK;
 }
 
@@ -391,7 +393,8 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
   default_tuning(p.get());
   auto cleanup = [&]() {
     for (auto& b : p->bufs) host_buffer_free(&b);
-    for (auto s : p->io) cudaStreamDestroy(s);
+    for (auto s : p->io) if (s) cudaStreamDestroy(s);
+    for (auto s : p->io_out) if (s) cudaStreamDestroy(s);
     if (p->table_arena) cudaFree(p->table_arena);
   };
   p->bufs.resize(n_devs);
@@ -409,10 +412,12 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     p->alloc.emplace_back(devs[i].capacity_bytes);
   }
   p->io.resize(n_devs, nullptr);
-  for (auto& s : p->io) {
-    cudaError_t e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
-    if (e != cudaSuccess) { cleanup(); return fail(KVPOOL_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)); }
-  }
+  p->io_out.resize(n_devs, nullptr);
+  for (auto* v : {&p->io, &p->io_out})
+    for (auto& s : *v) {
+      cudaError_t e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
+      if (e != cudaSuccess) { cleanup(); return fail(KVPOOL_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)); }
+    }
   if (cudaMalloc(reinterpret_cast<void**>(&p->table_arena), kTableArenaBytes) != cudaSuccess) {
     cudaGetLastError();
     cleanup();
@@ -431,6 +436,7 @@ int kvpool_destroy(kvpool_t* p) {
   p->live.clear();
   free_slots(p);
   for (auto s : p->io) cudaStreamDestroy(s);
+  for (auto s : p->io_out) cudaStreamDestroy(s);
   for (auto& b : p->bufs) host_buffer_free(&b);
   if (p->table_arena) cudaFree(p->table_arena);
   for (auto e : p->ev_free) cudaEventDestroy(e);
@@ -462,7 +468,7 @@ int kvpool_measure_bandwidth(kvpool_t* p, uint32_t dev, int direction, uint64_t 
   CU(cudaEventCreate(&e0));
   CU(cudaEventCreate(&e1));
   std::vector<float> ms(iters);
-  cudaStream_t s = p->io[dev];
+  cudaStream_t s = direction == 0 ? p->io[dev] : p->io_out[dev];
   int rc = KVPOOL_OK;
   for (uint32_t it = 0; it < iters + 1 && rc == KVPOOL_OK; ++it) {  // first pass is a warm-up
     cudaEventRecord(e0, s);
@@ -724,12 +730,12 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
   for (uint32_t i = 0; i < N; ++i) {
     const uint64_t bytes = static_cast<uint64_t>(L.map->counts[i]) * p->payload;
     if (bytes == 0 || is_hbm(p, i)) continue;
-    CU(cudaStreamWaitEvent(p->io[i], slot.kernel_done, 0));
-    if (L.landed_pending) CU(cudaStreamWaitEvent(p->io[i], L.landed, 0));
+    CU(cudaStreamWaitEvent(p->io_out[i], slot.kernel_done, 0));
+    if (L.landed_pending) CU(cudaStreamWaitEvent(p->io_out[i], L.landed, 0));
     CU(cudaMemcpyAsync(static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i], slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload,
-                       bytes, cudaMemcpyDeviceToHost, p->io[i]));
+                       bytes, cudaMemcpyDeviceToHost, p->io_out[i]));
     p->n_memcpys++;
-    CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+    CU(cudaEventRecord(slot.copy_done[i], p->io_out[i]));
     slot.copies_after_kernel |= 1u << i;
   }
   // `landed` must mean "all stripes done": record it on a stream that has waited for every copy
@@ -737,7 +743,7 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
     cudaStream_t js = nullptr;  // every I/O stream that copies has waited for the pack kernel, so it also covers the HBM stripes
     for (uint32_t i = 0; i < N; ++i) {
       if (static_cast<uint64_t>(L.map->counts[i]) == 0 || is_hbm(p, i)) continue;
-      if (!js) { js = p->io[i]; continue; }
+      if (!js) { js = p->io_out[i]; continue; }
       CU(cudaStreamWaitEvent(js, slot.copy_done[i], 0));
     }
     CU(cudaEventRecord(L.landed, js ? js : s));  // no host stripe at all: the kernel on `s` was the whole offload
@@ -905,6 +911,7 @@ int issue_zero_copy_group(const BatchCall& c, const LayerGroup& g) {
 int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   kvpool* p = c.p;
   const uint32_t N = p->n;
+  const std::vector<cudaStream_t>& ios = c.pack ? p->io_out : p->io;  // the copy streams of this direction
   const LayerState& A = c.pl->layers[c.first + g.q[0]];
   const LayerState& Z = c.pl->layers[c.first + g.q[g.n - 1]];
   // span[i]: bytes device i's copy engine moves for the group.  HBM-type devices move nothing that way — the kernel
@@ -931,7 +938,7 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   // waits too when it touches HBM-type stripes directly
   cudaStream_t lead = nullptr;
   for (uint32_t i = 0; i < N && !lead; ++i)
-    if (span[i]) lead = p->io[i];
+    if (span[i]) lead = ios[i];
   if (!lead && !hbm_blocks) return KVPOOL_OK;
   bool gated = false;
   for (uint32_t b = 0; b < g.n; ++b) {
@@ -953,15 +960,15 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
     if (gated) CU(cudaEventRecord(slot.gate, lead));
     for (uint32_t i = 0; i < N; ++i) {
       if (!span[i]) continue;
-      CU(cudaStreamWaitEvent(p->io[i], slot.kernel_done, 0));
-      if (gated && p->io[i] != lead) CU(cudaStreamWaitEvent(p->io[i], slot.gate, 0));
-      CU(cudaMemcpyAsync(static_cast<uint8_t*>(p->bufs[i].host) + span_lo[i], slot.buf + dev_start[i], span[i], cudaMemcpyDeviceToHost, p->io[i]));
+      CU(cudaStreamWaitEvent(ios[i], slot.kernel_done, 0));
+      if (gated && ios[i] != lead) CU(cudaStreamWaitEvent(ios[i], slot.gate, 0));
+      CU(cudaMemcpyAsync(static_cast<uint8_t*>(p->bufs[i].host) + span_lo[i], slot.buf + dev_start[i], span[i], cudaMemcpyDeviceToHost, ios[i]));
       p->n_memcpys++;
-      CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+      CU(cudaEventRecord(slot.copy_done[i], ios[i]));
       slot.copies_after_kernel |= 1u << i;
     }
     for (uint32_t i = 0; i < N; ++i)
-      if (span[i] && p->io[i] != lead) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
+      if (span[i] && ios[i] != lead) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
     for (uint32_t b = 0; b < g.n; ++b) {  // `lead` has waited for the kernel and every copy; with no host stripe the kernel was all
       LayerState& L = c.pl->layers[c.first + g.q[b]];
       CU(cudaEventRecord(L.landed, lead ? lead : c.s));
@@ -971,17 +978,17 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   }
   for (uint32_t i = 0; i < N; ++i) {
     if (!span[i]) continue;
-    rc = wait_slot_free(p, slot, p->io[i]);
+    rc = wait_slot_free(p, slot, ios[i]);
     if (rc != KVPOOL_OK) return rc;
   }
   slot.copies_after_kernel = 0;
   if (gated) CU(cudaEventRecord(slot.gate, lead));
   for (uint32_t i = 0; i < N; ++i) {
     if (!span[i]) continue;
-    if (gated && p->io[i] != lead) CU(cudaStreamWaitEvent(p->io[i], slot.gate, 0));
-    CU(cudaMemcpyAsync(slot.buf + dev_start[i], static_cast<uint8_t*>(p->bufs[i].host) + span_lo[i], span[i], cudaMemcpyHostToDevice, p->io[i]));
+    if (gated && ios[i] != lead) CU(cudaStreamWaitEvent(ios[i], slot.gate, 0));
+    CU(cudaMemcpyAsync(slot.buf + dev_start[i], static_cast<uint8_t*>(p->bufs[i].host) + span_lo[i], span[i], cudaMemcpyHostToDevice, ios[i]));
     p->n_memcpys++;
-    CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+    CU(cudaEventRecord(slot.copy_done[i], ios[i]));
     CU(cudaStreamWaitEvent(c.s, slot.copy_done[i], 0));
   }
   rc = launch_multi_counted(p, ma, false, false, c.s);
