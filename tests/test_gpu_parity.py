@@ -190,53 +190,58 @@ def test_kv_stream_is_identical_on_cpu_and_gpu():
         assert np.array_equal(a[plane, phys], W.kv_block_numpy(wl, 0, plane, phys))
 
 
-@pytest.mark.parametrize("cfg", [4, 3])
+@pytest.mark.parametrize("cfg", [4, 3, 5])
 def test_full_size_configs_sampled_against_oracle(cfg):
-    """BASELINE.json's full sizes in bench.py's launch configuration (path auto, default tuning): placement is
-    compared in full; stripe payloads and retrieved blocks are compared on samples the oracle side computes one
-    by one (the counter-based KV stream regenerates any block on the CPU); round trip and untouched poison are
-    checked over the whole tensors on the GPU."""
+    """BASELINE.json's full sizes in bench.py's launch configuration (path auto, default tuning, batched calls, one
+    stream per request): placement is compared in full; stripe payloads and retrieved blocks are compared on samples
+    the oracle side computes one by one (the counter-based KV stream regenerates any block on the CPU); round trip and
+    untouched poison are checked over the whole tensors on the GPU.  Config 5: four requests (32K..128K, 25 % of each
+    kept in HBM) on four streams over one shared block pool, 30 GiB moved per leg."""
     wl = W.make_workload(cfg)
-    g, dev = wl.geom, torch.device("cuda:0")
+    g, dev, R, L = wl.geom, torch.device("cuda:0"), len(wl.requests), wl.geom.n_layers
     bw = list(wl.default_weights())
-    bpl = wl.blocks_per_layer(0)
     pool = make_pool(wl)
     try:
-        pl = pool.place(bpl)
-        opl = oracle.place(bw, bpl)
-        check_placement(pl, opl)
-        table_np = [np.ascontiguousarray(wl.layer_table(0, l)) for l in range(g.n_layers)]
-        tables = [torch.from_numpy(t).to(dev) for t in table_np]
-        src = [W.kv_layer_torch(wl, l, dev) for l in range(g.n_layers)]
-        dst = [W.poison_torch((2, wl.nphys, g.kvb // 2), dev) for l in range(g.n_layers)]
+        bpl = [wl.blocks_per_layer(r) for r in range(R)]
+        pls = [pool.place(bpl[r]) for r in range(R)]
+        opls = [oracle.place(bw, bpl[r]) for r in range(R)]
+        for r in range(R):
+            check_placement(pls[r], opls[r])
+        table_np = [[np.ascontiguousarray(wl.layer_table(r, l)) for l in range(L)] for r in range(R)]
+        tables = [[torch.from_numpy(t).to(dev) for t in row] for row in table_np]
+        src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+        dst = [W.poison_torch((2, wl.nphys, g.kvb // 2), dev) for l in range(L)]
         torch.cuda.synchronize()                                                  # inputs were generated on the default stream
-        s = torch.cuda.Stream()
-        for l in range(g.n_layers):
-            pool.offload(pl, l, src[l][0], src[l][1], g.kvb, tables[l], s)
-        pool.wait_offloads(pl, s)
-        for l in range(g.n_layers):
-            pool.retrieve(pl, l, dst[l][0], dst[l][1], g.kvb, tables[l], s)
-        s.synchronize()
+        streams = [torch.cuda.Stream() for _ in range(R)]
+        for r in range(R):
+            pool.offload_layers(pls[r], 0, [x[0] for x in src], [x[1] for x in src], g.kvb, tables[r], streams[r])
+        for r in range(R):
+            pool.wait_offloads(pls[r], streams[r])
+        for r in range(R):
+            pool.retrieve_layers(pls[r], 0, [d[0] for d in dst], [d[1] for d in dst], g.kvb, tables[r], streams[r])
+        torch.cuda.synchronize()
         rng = np.random.default_rng(cfg)
         poison = np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item()
-        for l in range(g.n_layers):
-            K = len(table_np[l])
-            for j in sorted(set([0, K - 1] + [int(x) for x in rng.integers(0, K, size=6)])):
-                phys = int(table_np[l][j])
-                want = np.concatenate([W.kv_block_numpy(wl, l, 0, phys), W.kv_block_numpy(wl, l, 1, phys)]).view(np.uint8)
-                d, sl = int(opl[l].dev[j]), int(opl[l].slot[j])
-                got = pl.stripe(l, d)[sl * g.payload:(sl + 1) * g.payload]
-                assert np.array_equal(got, want), f"stripe payload differs: layer {l} block {j}"
-                back = dst[l][:, phys].cpu().numpy().view(np.uint16).reshape(-1)
-                assert np.array_equal(back, want.view(np.uint16)), f"retrieved block differs: layer {l} block {j}"
+        for l in range(L):
             used = torch.zeros(wl.nphys, dtype=torch.bool, device=dev)
-            used[tables[l].long()] = True
+            for r in range(R):
+                K = len(table_np[r][l])
+                for j in sorted(set([0, K - 1] + [int(x) for x in rng.integers(0, K, size=6 if R == 1 else 2)])):
+                    phys = int(table_np[r][l][j])
+                    want = np.concatenate([W.kv_block_numpy(wl, l, 0, phys), W.kv_block_numpy(wl, l, 1, phys)]).view(np.uint8)
+                    d, sl = int(opls[r][l].dev[j]), int(opls[r][l].slot[j])
+                    got = pls[r].stripe(l, d)[sl * g.payload:(sl + 1) * g.payload]
+                    assert np.array_equal(got, want), f"stripe payload differs: request {r} layer {l} block {j}"
+                    back = dst[l][:, phys].cpu().numpy().view(np.uint16).reshape(-1)
+                    assert np.array_equal(back, want.view(np.uint16)), f"retrieved block differs: request {r} layer {l} block {j}"
+                used[tables[r][l].long()] = True
+                # byte share of every device within one block of its bandwidth share (north star invariant)
+                for i, wi in enumerate(bw):
+                    assert abs(pls[r].stripe_location(l, i)[1] - wi / sum(bw) * K * g.payload) < g.payload
             assert torch.equal(dst[l][:, used], src[l][:, used])
-            assert bool((dst[l][:, ~used] == poison).all())
-            # byte share of every device within one block of its bandwidth share (north star invariant)
-            for i, wi in enumerate(bw):
-                assert abs(pl.stripe(l, i).nbytes - wi / sum(bw) * K * g.payload) < g.payload
-        pl.release()
+            assert bool((dst[l][:, ~used] == poison).all())                        # the retained prefixes and free blocks stay untouched
+        for pl in pls:
+            pl.release()
     finally:
         pool.destroy()
 
