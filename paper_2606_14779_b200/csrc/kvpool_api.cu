@@ -283,7 +283,10 @@ LaunchCfg launch_cfg(const kvpool* p, bool link_bound) {
   return c;
 }
 
+inline bool all_hbm(const kvpool* p) { return p->hbm_mask == (p->n >= 32 ? 0xFFFFFFFFu : (1u << p->n) - 1u); }
+
 bool use_staged(const kvpool* p, const LayerState& L) {
+  if (all_hbm(p)) return false;  // nothing to stage: every stripe is reached in place (one kernel, HBM grid)
   if (p->path == KVPOOL_PATH_STAGED) return true;
   if (p->path == KVPOOL_PATH_ZEROCOPY) return false;
   return L.map->K * p->payload >= p->tune.auto_threshold_bytes;
@@ -653,7 +656,7 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
     cudaError_t e = take_event(p, &Ls.landed);
     if (e != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: cudaEventCreate: %s", cudaGetErrorString(e)); }
   }
-  if (p->path != KVPOOL_PATH_ZEROCOPY) {
+  if (p->path != KVPOOL_PATH_ZEROCOPY && !all_hbm(p)) {
     // a slot holds the largest layer, or a group of small layers (plus the 256-byte alignment gaps between stripes)
     const uint64_t total_bytes = std::accumulate(pl->region_bytes.begin(), pl->region_bytes.end(), uint64_t{0});
     const uint64_t group_cap = std::min<uint64_t>(std::max<uint64_t>(max_layer_bytes, p->tune.group_bytes), total_bytes);
@@ -776,7 +779,7 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   a.j0 = first_block;
   a.K = n_blocks;
   const uint64_t range_bytes = static_cast<uint64_t>(n_blocks) * p->payload;
-  const bool staged = p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && range_bytes >= p->tune.auto_threshold_bytes);
+  const bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && range_bytes >= p->tune.auto_threshold_bytes));
 
   if (!staged) {
     for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
@@ -1000,7 +1003,7 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
 int issue_group(const BatchCall& c, const LayerGroup& g) {
   kvpool* p = c.p;
   if (g.n == 0) return KVPOOL_OK;
-  const bool staged = p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && g.bytes >= p->tune.auto_threshold_bytes);
+  const bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && g.bytes >= p->tune.auto_threshold_bytes));
   if (!staged) return issue_zero_copy_group(c, g);
   if (g.n > 1) {
     const int rc = issue_staged_group(c, g);

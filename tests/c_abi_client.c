@@ -21,6 +21,7 @@ int main(int argc, char **argv) {
     if (kvpool_plan_weights(bw, 0, w) != KVPOOL_EINVAL) return 2;
     printf("error \"%s\"\n", kvpool_last_error());
     printf("%s\n", kvpool_version());
+    printf("sizeof %u %u %u\n", (unsigned)sizeof(kvpool_device_desc), (unsigned)sizeof(kvpool_geometry), (unsigned)sizeof(kvpool_tuning));
     if (argc > 1 && strcmp(argv[1], "gpu") == 0) {
         kvpool_device_desc d[2] = {{2.0, 8u << 20, -1, 0, -1, 0}, {1.0, 8u << 20, -1, KVPOOL_DEV_HBM, -1, 0}};
         kvpool_geometry g = {2, 16, 2, 64, 2};

@@ -106,6 +106,10 @@ def test_create_argument_validation_precedes_cuda():
     with pytest.raises(kv.KvPoolError) as e:
         kv.KvPool([1.0], [0], n_layers=1, n_kv_heads=1, head_dim=64)
     assert e.value.code == kv.EINVAL
+    for flags in (8, kv.DEV_HBM | kv.DEV_WRITE_COMBINED, kv.DEV_HBM | kv.DEV_NUMA_STRICT):      # unknown flag; HBM excludes host flags
+        with pytest.raises(kv.KvPoolError) as e:
+            kv.KvPool([1.0], [1 << 20], n_layers=1, n_kv_heads=1, head_dim=64, dev_flags=[flags])
+        assert e.value.code == kv.EINVAL
 
 
 def test_product_does_not_import_oracle_and_oracle_does_not_import_product():
@@ -136,3 +140,5 @@ def test_plain_c_client_compiles_against_header_and_runs(tmp_path):
     od, _ = oracle.wrr(oracle.counts([4000, 4000, 2000, 2000, 1000, 1000], 64), 64)
     assert out[1] == "dev " + " ".join(str(int(d)) for d in od[:16])
     assert out[2].startswith('error "plan_weights') and out[3].startswith("kvpool")
+    import ctypes                                              # the ctypes structs of the binding have the header's C layout
+    assert out[4] == f"sizeof {ctypes.sizeof(kv.DeviceDesc)} {ctypes.sizeof(kv.Geometry)} {ctypes.sizeof(kv.Tuning)}"
