@@ -256,6 +256,8 @@ def run_kvpool(args) -> dict:
     share = np.array(base_w) / np.sum(base_w)
     caps = [int(moved * s * 1.25) + (L * R + 4) * (g.payload + 4096) for s in share]
     numa = [i % 2 for i in range(N)] if args.config == 2 else None      # config 2: "on 2 NUMA nodes" (falls back, reported)
+    if numa is None and world > 1:
+        numa = [kv.NUMA_AUTO] * N       # several ranks on one host: each rank's buffers on the NUMA node its own GPU hangs off
     t0 = time.perf_counter()
     pool = kv.KvPool(base_w, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, block_tokens=g.block_tokens,
                      elem_bytes=g.elem_bytes, cuda_device=local, numa_nodes=numa)
@@ -524,7 +526,7 @@ def run_kvpool(args) -> dict:
                 "*_gbps = one launch per event pair, *_back_to_back_gbps = 16 launches per event pair", **hbm,
                 "peak": peaks["hbm_gbs"], "frac_unpack": best_unpack / peaks["hbm_gbs"], "frac_pack": best_pack / peaks["hbm_gbs"],
                 "frac_unpack_of_8TBs_nominal": best_unpack / 8000.0, "frac_pack_of_8TBs_nominal": best_pack / 8000.0}
-    if dom < 2:
+    if dom < 2 and Kbig * g.payload >= (64 << 20):      # (a 4 MiB launch measures launch latency, not bandwidth: no reference then)
         # the measured peak's own kernel (a contiguous torch copy_ of the same bytes) under the in-step condition: a copy
         # engine streaming over the host link in the direction of that leg (offload: D2H, retrieve: H2D)
         side, big_d = torch.empty(Kbig * g.payload, dtype=torch.uint8, device=dev), torch.empty(1 << 30, dtype=torch.uint8, device=dev)
@@ -544,6 +546,7 @@ def run_kvpool(args) -> dict:
         roof["torch_copy_same_bytes_alone_gbps"] = 2 * Kbig * g.payload / ref_alone_us / 1e3
         roof["frac_of_torch_copy_under_dma"] = ach / roof["torch_copy_same_bytes_under_dma_gbps"]
         del side, big_d, big_h
+    if dom < 2:
         kn = "vec16" if tn.kernel == kv.KERNEL_VEC16 else "bulk"
         roof["achieved_back_to_back"] = hbm[f"{'pack' if dom == 0 else 'unpack'}_{kn}_back_to_back_gbps"]
         roof["frac_back_to_back"] = roof["achieved_back_to_back"] / peaks["hbm_gbs"]

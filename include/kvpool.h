@@ -54,6 +54,8 @@ enum {
                                         peer of the pool's GPU, or that GPU itself.  Its stripes are reached
                                         by the kernels directly (peer loads / stores); no staging, no copy engine.            */
 
+#define KVPOOL_NUMA_AUTO (-2)        /* kvpool_device_desc.numa_node: bind to the NUMA node of the pool's GPU */
+
 /* pool-device types (GLT `type`, Table I) */
 enum {
   KVPOOL_TYPE_MEM = 0, /* pinned host memory; location = host pointer                                     */
@@ -80,7 +82,8 @@ typedef struct {           /* one pool device (Table I)           
   double bandwidth_gbps;   /* b_i of Eq. 1, measured, in 1e9 B/s; > 0                                   */
   uint64_t capacity_bytes; /* size of the buffer the library allocates (pinned + mapped host memory, or */
                            /* device memory with KVPOOL_DEV_HBM); > 0                                   */
-  int32_t numa_node;       /* MEM: -1 = no preference; else bind the pages to this node (mbind)         */
+  int32_t numa_node;       /* MEM: -1 = no preference; KVPOOL_NUMA_AUTO = the node the pool's GPU hangs */
+                           /* off (sysfs; no preference if unknown); else bind the pages to this node   */
   uint32_t flags;          /* KVPOOL_DEV_*                                                              */
   int32_t gpu;             /* HBM: CUDA ordinal of the GPU that holds the buffer, -1 = the pool's own   */
                            /* GPU; must be peer-accessible from it (ECUDA otherwise).  MEM: ignored     */

@@ -19,6 +19,7 @@ MAX_DEVICES = 32
 OK, EINVAL, ENOMEM, ECUDA, ENUMA, ESTATE, ENOENT = 0, -1, -2, -3, -4, -5, -6
 DEV_WRITE_COMBINED, DEV_NUMA_STRICT, DEV_HBM = 1, 2, 4
 TYPE_MEM, TYPE_SSD, TYPE_HBM = 0, 1, 2
+NUMA_AUTO = -2
 PATH_AUTO, PATH_STAGED, PATH_ZEROCOPY = 0, 1, 2
 KERNEL_VEC16, KERNEL_BULK = 0, 1
 _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA", ESTATE: "ESTATE", ENOENT: "ENOENT"}

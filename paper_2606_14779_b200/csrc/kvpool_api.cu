@@ -370,6 +370,7 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     if (devs[i].capacity_bytes == 0) return fail(KVPOOL_EINVAL, "create: device %u has zero capacity", i);
     if (devs[i].flags & ~(KVPOOL_DEV_WRITE_COMBINED | KVPOOL_DEV_NUMA_STRICT | KVPOOL_DEV_HBM)) return fail(KVPOOL_EINVAL, "create: device %u unknown flags", i);
     if ((devs[i].flags & KVPOOL_DEV_HBM) && (devs[i].flags & ~KVPOOL_DEV_HBM)) return fail(KVPOOL_EINVAL, "create: device %u: KVPOOL_DEV_HBM excludes the host-memory flags", i);
+    if (devs[i].numa_node < KVPOOL_NUMA_AUTO) return fail(KVPOOL_EINVAL, "create: device %u: numa_node %d", i, devs[i].numa_node);
     if (devs[i].reserved != 0) return fail(KVPOOL_EINVAL, "create: device %u: reserved must be 0", i);
   }
   if (!quantise_weights(bw.data(), n_devs, w.data())) return fail(KVPOOL_EINVAL, "create: bandwidth must be positive (>= 0.0005 GB/s)");
@@ -405,7 +406,8 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     std::string err;
     const bool hbm = devs[i].flags & KVPOOL_DEV_HBM;
     const int rc = hbm ? device_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes, devs[i].gpu < 0 ? cuda_device : devs[i].gpu, cuda_device, &err)
-                       : host_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes, devs[i].numa_node, devs[i].flags & KVPOOL_DEV_WRITE_COMBINED,
+                       : host_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes,
+                                           devs[i].numa_node == KVPOOL_NUMA_AUTO ? gpu_numa_node(cuda_device) : devs[i].numa_node, devs[i].flags & KVPOOL_DEV_WRITE_COMBINED,
                                            devs[i].flags & KVPOOL_DEV_NUMA_STRICT, &err);
     if (rc == KVPOOL_OK && hbm) p->hbm_mask |= 1u << i;
     if (rc != KVPOOL_OK) {

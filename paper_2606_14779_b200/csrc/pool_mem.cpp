@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <dirent.h>
 #include <errno.h>
+#include <stdio.h>
 #include <string.h>
 #include <sys/mman.h>
 #include <sys/syscall.h>
@@ -22,6 +23,24 @@ int numa_node_count() {
     closedir(d);
   }
   return n > 0 ? n : 1;
+}
+
+// NUMA node the GPU's PCIe root port hangs off, from sysfs; -1 when unknown (single-node boxes report -1 or 0).
+int gpu_numa_node(int cuda_device) {
+  char bdf[32] = {0};
+  if (cudaDeviceGetPCIBusId(bdf, sizeof(bdf), cuda_device) != cudaSuccess) {
+    cudaGetLastError();
+    return -1;
+  }
+  for (char* c = bdf; *c; ++c)
+    if (*c >= 'A' && *c <= 'F') *c = static_cast<char>(*c - 'A' + 'a');  // sysfs spells the address in lower case
+  const std::string path = std::string("/sys/bus/pci/devices/") + bdf + "/numa_node";
+  FILE* f = fopen(path.c_str(), "r");
+  if (!f) return -1;
+  int node = -1;
+  if (fscanf(f, "%d", &node) != 1) node = -1;
+  fclose(f);
+  return node >= 0 && node < numa_node_count() ? node : -1;
 }
 
 static int query_node(void* page) {

@@ -399,11 +399,17 @@ def test_numa_bound_registered_and_write_combined_pool_buffers():
     with pytest.raises(kv.KvPoolError) as e:
         kv.KvPool([2.0, 1.0, 1.0], cap, n_layers=2, n_kv_heads=2, head_dim=64, numa_nodes=[0, 977, 0], dev_flags=[0, kv.DEV_NUMA_STRICT, 0])
     assert e.value.code == kv.ENUMA
-    for numa, flags in (([0, 0, -1], [kv.DEV_NUMA_STRICT, 0, 0]), ([0, 977, -1], [0, 0, 0]), (None, [kv.DEV_WRITE_COMBINED] * 3)):
+    with pytest.raises(kv.KvPoolError) as e:
+        kv.KvPool([2.0, 1.0, 1.0], cap, n_layers=2, n_kv_heads=2, head_dim=64, numa_nodes=[0, -3, 0])
+    assert e.value.code == kv.EINVAL
+    auto = [kv.NUMA_AUTO] * 3               # the node the GPU hangs off, read from sysfs; no preference where sysfs does not say
+    for numa, flags in (([0, 0, -1], [kv.DEV_NUMA_STRICT, 0, 0]), ([0, 977, -1], [0, 0, 0]), (None, [kv.DEV_WRITE_COMBINED] * 3), (auto, [0, 0, 0])):
         pool = kv.KvPool([2.0, 1.0, 1.0], cap, n_layers=2, n_kv_heads=2, head_dim=64, numa_nodes=numa, dev_flags=flags)
         try:
-            if numa is not None:
+            if numa is not None and numa is not auto:
                 assert pool.device_info(0)["numa_node"] == 0                         # pages really sit on the bound node
+            if numa is auto:
+                assert pool.device_info(0)["numa_node"] in (-1, 0)                   # this box has one node
             opl = oracle.place([2.0, 1.0, 1.0], wl.blocks_per_layer(0))
             for path in (kv.PATH_STAGED, kv.PATH_ZEROCOPY):
                 pool.set_path(path)
