@@ -396,7 +396,8 @@ def run_kvpool(args) -> dict:
     pool.set_profiling(False)
     k1, m1 = pool.stats()
     clocks = sampler.stop(t_begin, t_end) if rank == 0 else None
-    prof = {kind: pool.profile_read(kind) for kind in range(4)}
+    prof_clk = {kind: pool.profile_read_clock(kind) for kind in range(4)}
+    prof = {kind: (v[0], v[2], v[4]) for kind, v in prof_clk.items()}
 
     step_ms = 1e3 * (t_end - t_begin) / args.steps
     ret_ms = sum(rec["retrieve_ms"]) / args.steps
@@ -511,6 +512,12 @@ def run_kvpool(args) -> dict:
         roof = {"bound": "hbm", "kernel": kinds[dom], "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
                 "traffic": traffic, "peak_source": peaks["source"], "launches": n, "avg_launch_ms": ms / max(n, 1),
                 "algorithmic_bytes_per_launch": 2 * b // max(n, 1), "frac_of_8TBs_nominal": ach / 8000.0}
+        _, dms, _, nd, _ = prof_clk[dom]
+        if nd:
+            # the same launches of the timed region by the kernels' own clock (%globaltimer: first CTA start to last CTA end)
+            clk = 2 * (b / n) * nd / (dms * 1e6)
+            roof.update({"achieved_kernel_clock": clk, "frac_kernel_clock": clk / peaks["hbm_gbs"], "avg_launch_ms_kernel_clock": dms / nd,
+                         "launches_kernel_clock": nd})
     else:
         peak = link_d2h if dom == 2 else link_h2d
         ach = b / (ms * 1e6) if ms > 0 else 0.0
@@ -542,6 +549,8 @@ def run_kvpool(args) -> dict:
 
         ref_us = time_under_dma(torch, main, other, k_copy, bg)
         ref_alone_us = time_under_dma(torch, main, other, k_copy, None)
+        roof["empty_event_pair_under_dma_us"] = time_under_dma(torch, main, other, lambda i: None, bg)
+        roof["empty_event_pair_alone_us"] = time_under_dma(torch, main, other, lambda i: None, None)
         roof["torch_copy_same_bytes_under_dma_gbps"] = 2 * Kbig * g.payload / ref_us / 1e3
         roof["torch_copy_same_bytes_alone_gbps"] = 2 * Kbig * g.payload / ref_alone_us / 1e3
         roof["frac_of_torch_copy_under_dma"] = ach / roof["torch_copy_same_bytes_under_dma_gbps"]
@@ -550,10 +559,13 @@ def run_kvpool(args) -> dict:
         kn = "vec16" if tn.kernel == kv.KERNEL_VEC16 else "bulk"
         roof["achieved_back_to_back"] = hbm[f"{'pack' if dom == 0 else 'unpack'}_{kn}_back_to_back_gbps"]
         roof["frac_back_to_back"] = roof["achieved_back_to_back"] / peaks["hbm_gbs"]
-        roof["note"] = ("achieved = per-launch event pairs inside the timed step, where every pack/unpack launch runs while the copy engines "
-                        "stream the neighbouring layers over the host link: any HBM-bound kernel (a plain torch copy_ included) loses "
-                        "20-30 us per 512 MiB of traffic under a concurrent cudaMemcpyAsync on this box (bench.py --interference, "
-                        "profiles/r1_interference.txt); achieved_back_to_back = same kernel, 16 launches per event pair, no concurrent copy")
+        roof["note"] = ("achieved = per-launch CUDA event pairs inside the timed step, where every pack/unpack launch runs while the copy "
+                        "engines stream the neighbouring layers over the host link; under such a stream an event pair with NOTHING between "
+                        "its records already reads empty_event_pair_under_dma_us (vs empty_event_pair_alone_us), a fixed cost that does not "
+                        "grow with the kernel (bench.py --interference, profiles/r1_interference.txt), and a plain torch copy_ of the same "
+                        "bytes pays the same; achieved_kernel_clock = the same in-step launches timed by the kernel itself (%globaltimer, "
+                        "first CTA start to last CTA end, stores fenced); achieved_back_to_back = same kernel, 16 launches per event pair, "
+                        "no concurrent copy")
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms,
@@ -819,20 +831,54 @@ def run_interference(args) -> None:
     def measure(fn, bg):
         return time_under_dma(torch, s, o, fn, bg)
 
+    def device_clock_us(fn, bg, kind):
+        """Mean in-kernel span (%globaltimer, first CTA start to last CTA end) of the same launches under the same condition."""
+        for k in range(4):
+            pool.profile_read_clock(k)
+        pool.set_profiling(True)
+        try:
+            measure(fn, bg)
+        finally:
+            pool.set_profiling(False)
+        _, dms, _, nd, _ = pool.profile_read_clock(kind)
+        return 1e3 * dms / max(nd, 1)
+
     peak = measured_peaks()["hbm_gbs"]
     print(f"# bench.py --interference --config {args.config}: {wl.name}, {nbytes / 2**20:.0f} MiB read + {nbytes / 2**20:.0f} MiB written per launch; "
-          f"one CUDA event pair per launch, 16 launches, median, best of 3; GB/s = 2*bytes/time; measured HBM copy peak {peak:.0f} GB/s")
-    print(f"{'kernel':46s} {'alone us':>9s} {'GB/s':>6s} {'+H2D us':>9s} {'GB/s':>6s} {'+D2H us':>9s} {'GB/s':>6s}")
-    rows = [("kv_copy_vec16 unpack (stage -> paged)", k_unpack, kv.KERNEL_VEC16), ("kv_copy_vec16 pack (paged -> stage)", k_pack, kv.KERNEL_VEC16),
-            ("kv_copy_bulk unpack", k_unpack, kv.KERNEL_BULK), ("kv_copy_bulk pack", k_pack, kv.KERNEL_BULK),
-            ("torch copy_ (contiguous D2D kernel, same bytes)", k_copy, None)]
-    for name, fn, kid in rows:
+          f"'us' = one CUDA event pair per launch, 16 launches, median, best of 3; 'clk' = the same launches by the kernels' own clock "
+          f"(%globaltimer span, first CTA start to last CTA end, mean); GB/s = 2*bytes/event time; measured HBM copy peak {peak:.0f} GB/s")
+    print(f"{'kernel':46s} {'alone us':>9s} {'clk':>6s} {'GB/s':>6s} {'+H2D us':>9s} {'clk':>6s} {'GB/s':>6s} {'+D2H us':>9s} {'clk':>6s} {'GB/s':>6s}")
+    rows = [("kv_copy_vec16 unpack (stage -> paged)", k_unpack, kv.KERNEL_VEC16, kv.KvPool.PROF_UNPACK), ("kv_copy_vec16 pack (paged -> stage)", k_pack, kv.KERNEL_VEC16, kv.KvPool.PROF_PACK),
+            ("kv_copy_bulk unpack", k_unpack, kv.KERNEL_BULK, kv.KvPool.PROF_UNPACK), ("kv_copy_bulk pack", k_pack, kv.KERNEL_BULK, kv.KvPool.PROF_PACK),
+            ("torch copy_ (contiguous D2D kernel, same bytes)", k_copy, None, None),
+            ("empty event pair (no kernel between the records)", lambda i: None, None, None)]
+    for name, fn, kid, kind in rows:
         if kid is not None:
             pool.set_tuning(kernel=kid)
         for i in range(4):
             fn(i)
-        a, b, c = measure(fn, None), measure(fn, bg_h2d), measure(fn, bg_d2h)
-        print(f"{name:46s} {a:9.1f} {2 * nbytes / a / 1e3:6.0f} {b:9.1f} {2 * nbytes / b / 1e3:6.0f} {c:9.1f} {2 * nbytes / c / 1e3:6.0f}", flush=True)
+        t = [measure(fn, bg) for bg in (None, bg_h2d, bg_d2h)]
+        c = [device_clock_us(fn, bg, kind) if kind is not None else None for bg in (None, bg_h2d, bg_d2h)]
+        gbs = [f"{2 * nbytes / t[q] / 1e3:6.0f}" if not name.startswith("empty") else "     -" for q in range(3)]
+        cells = "".join(f" {t[q]:9.1f} {(f'{c[q]:6.1f}' if c[q] is not None else '     -')} {gbs[q]}" for q in range(3))
+        print(f"{name:46s}{cells}", flush=True)
+
+    # fixed or proportional?  per launch or per event pair?  (a kernel this repo did not write: contiguous torch copy_)
+    print("# torch copy_ of n MiB (read n + write n), nk launches inside ONE event pair, 8 pairs, median, best of 3: event-pair us alone / +H2D / +D2H "
+          "and the excess over alone")
+    print(f"{'MiB':>6s} {'nk':>3s} {'alone':>9s} {'+H2D':>9s} {'+D2H':>9s} {'dH2D':>7s} {'dD2H':>7s}")
+    del stages, flat_a
+    for mib, nk in [(16, 1), (64, 1), (256, 1), (1024, 1), (2048, 1), (64, 2), (64, 4), (64, 8), (256, 2), (256, 4), (256, 8)]:
+        a_, b_ = torch.empty(mib << 20, dtype=torch.uint8, device=dev), torch.empty(mib << 20, dtype=torch.uint8, device=dev)
+
+        def k_n(i, a_=a_, b_=b_, nk=nk):
+            with torch.cuda.stream(s):
+                for _ in range(nk):
+                    b_.copy_(a_, non_blocking=True)
+
+        t = [time_under_dma(torch, s, o, k_n, bg, launches=8) for bg in (None, bg_h2d, bg_d2h)]
+        print(f"{mib:6d} {nk:3d} {t[0]:9.1f} {t[1]:9.1f} {t[2]:9.1f} {t[1] - t[0]:7.1f} {t[2] - t[0]:7.1f}", flush=True)
+        del a_, b_
     pl.release()
     pool.destroy()
 

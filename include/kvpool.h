@@ -269,6 +269,14 @@ KVPOOL_API int kvpool_stats(const kvpool_t* pool, uint64_t* kernel_launches, uin
  * kind: 0 = in-device pack, 1 = in-device unpack, 2 = zero-copy offload, 3 = zero-copy retrieve.               */
 KVPOOL_API int kvpool_set_profiling(kvpool_t* pool, int enabled);
 KVPOOL_API int kvpool_profile_read(kvpool_t* pool, int kind, double* total_ms, uint64_t* launches, uint64_t* bytes);
+/* The same read plus the kernels' own clock: while profiling is on, every CTA of a launch folds its start and its end
+ * (%globaltimer, after its stores are globally visible) into a per-launch {min start, max end} pair in device memory;
+ * device_ms is the sum of (max end - min start) over the device_launches launches that got such a pair (the first
+ * 16384 between two reads that empty the record list).  The event pairs of total_ms also count what the stream's front
+ * end adds around a launch — ~5 us on an idle GPU, 20-35 us while a copy engine streams over the host link (an empty
+ * event pair measures the same) — device_ms does not.  Any out pointer may be NULL.                   */
+KVPOOL_API int kvpool_profile_read_clock(kvpool_t* pool, int kind, double* total_ms, double* device_ms, uint64_t* launches,
+                              uint64_t* device_launches, uint64_t* bytes);
 
 KVPOOL_API const char* kvpool_last_error(void);
 KVPOOL_API const char* kvpool_version(void);

@@ -29,7 +29,7 @@ EXPORTS = [
     "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_place", "kvpool_release",
     "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
-    "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_last_error", "kvpool_version",
+    "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_last_error", "kvpool_version",
 ]
 
 
@@ -109,6 +109,7 @@ def lib():
             "kvpool_stats": [vp, POINTER(c_uint64), POINTER(c_uint64)],
             "kvpool_set_profiling": [vp, c_int],
             "kvpool_profile_read": [vp, c_int, POINTER(c_double), POINTER(c_uint64), POINTER(c_uint64)],
+            "kvpool_profile_read_clock": [vp, c_int, POINTER(c_double), POINTER(c_double), POINTER(c_uint64), POINTER(c_uint64), POINTER(c_uint64)],
         }
         for name, argtypes in sig.items():
             f = getattr(L, name)
@@ -373,6 +374,12 @@ class KvPool:
         ms, n, b = c_double(), c_uint64(), c_uint64()
         _ck(lib().kvpool_profile_read(self.handle, kind, byref(ms), byref(n), byref(b)))
         return ms.value, n.value, b.value
+
+    def profile_read_clock(self, kind: int) -> Tuple[float, float, int, int, int]:
+        """(event ms, in-kernel %globaltimer ms, launches, launches with a device span, algorithmic bytes) since the last read."""
+        ms, dms, n, nd, b = c_double(), c_double(), c_uint64(), c_uint64(), c_uint64()
+        _ck(lib().kvpool_profile_read_clock(self.handle, kind, byref(ms), byref(dms), byref(n), byref(nd), byref(b)))
+        return ms.value, dms.value, n.value, nd.value, b.value
 
 
 def version() -> str:

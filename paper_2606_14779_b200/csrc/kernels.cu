@@ -34,6 +34,21 @@ __device__ __forceinline__ void st_stream(void* p, const int4& v) {
                : "memory");
 }
 
+// Profiling: the launch's own execution span on the device clock.  Every CTA (vec16) or issuing warp (bulk) folds its
+// start and its end — after its stores are globally visible — into {min, max}; event pairs around a launch also count whatever the
+// stream's front end adds (notably under a concurrent copy-engine stream).
+__device__ __forceinline__ unsigned long long global_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+__device__ __forceinline__ void span_begin(unsigned long long* span) {
+  if (span) atomicMin(span, global_ns());
+}
+__device__ __forceinline__ void span_end(unsigned long long* span) {
+  if (span) atomicMax(span + 1, global_ns());
+}
+
 // Decode work item t of a layer split into `pieces` pieces per K (or V) block of `piece_bytes` bytes.
 struct Piece {
   uint8_t* paged;
@@ -93,6 +108,7 @@ __global__ void __launch_bounds__(kVecMaxThreads) kv_copy_vec16(const __grid_con
   const uint64_t nwarps = static_cast<uint64_t>(gridDim.x) * warps_per_cta;
   const uint32_t pieces = (a.kvb + kVecPiece - 1) / kVecPiece;
   const uint64_t total = static_cast<uint64_t>(units(a)) * 2u * pieces;
+  if (threadIdx.x == 0) span_begin(a.span);
   for (uint64_t t = static_cast<uint64_t>(blockIdx.x) * warps_per_cta + (threadIdx.x >> 5); t < total; t += nwarps) {
     const Piece p = decode(a, t, pieces, kVecPiece);
     const uint8_t* src = (PACK ? p.paged : p.pooled) + lane * 16u;
@@ -111,6 +127,11 @@ __global__ void __launch_bounds__(kVecMaxThreads) kv_copy_vec16(const __grid_con
       for (int u = 0; u < kVecUnroll; ++u)
         if (u * 512u + lane * 16u < p.bytes) st_stream(dst + u * 512, v[u]);
     }
+  }
+  if (a.span) {  // uniform across the grid
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) span_end(a.span);
   }
 }
 
@@ -156,6 +177,7 @@ __global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Args
   const uint32_t warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const uint32_t bar0 = smem_u32(smem) + warp * stages * 8u;
   const uint32_t buf0 = smem_u32(smem) + kBulkBarrierBytes + warp * stages * chunk;
+  span_begin(a.span);
   for (uint32_t s = 0; s < stages; ++s) mbar_init(bar0 + 8u * s, 1);
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 
@@ -186,6 +208,7 @@ __global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Args
     }
   }
   bulk_wait_all();
+  span_end(a.span);
 }
 
 // ---- consumer stand-in: position-weighted 64-bit checksum of the blocks named by a table ---------------------------

@@ -23,6 +23,7 @@ struct LayerArgs {
   uint32_t K;    // number of units this launch moves ...
   uint32_t j0;   // ... starting at logical block j0 (table/dev/slot are indexed by j0 + local index)
   uint32_t kvb;
+  unsigned long long* span;  // profiling only (else null): device {min start, max end} of the launch in %globaltimer ns
   uint64_t pool_base[kMaxDev];
 };
 
@@ -46,6 +47,7 @@ struct MultiArgs {
   uint32_t n;            // layers in this launch, <= kMaxBatch
   uint32_t total_units;  // sum of K
   uint32_t pad;
+  unsigned long long* span;  // as in LayerArgs
   uint64_t delta[kMaxDev];  // added (mod 2^64) to pool_base[i]: 0 for the mapped host stripes themselves, or the
                             // displacement that maps device i's span of stripes onto its copy in a staging slot
   MultiDesc d[kMaxBatch];

@@ -79,6 +79,7 @@ struct ProfRec {  // one profiled kernel launch
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   uint64_t bytes = 0;
   int kind = 0;
+  int32_t span = -1;  // index of the launch's {min start, max end} pair in the pool's span arena, -1 = none left
 };
 
 struct StageSlot {
@@ -144,6 +145,8 @@ struct kvpool {
   bool profiling = false;
   std::vector<ProfRec> prof;
   std::vector<cudaEvent_t> prof_free;  // timing events ready for reuse
+  unsigned long long* span_arena = nullptr;  // device: kSpanCap x {min start, max end} in %globaltimer ns, written by the kernels
+  uint32_t span_cursor = 0;
   std::mutex mu;
 };
 
@@ -292,6 +295,23 @@ bool use_staged(const kvpool* p, const LayerState& L) {
   return L.map->K * p->payload >= p->tune.auto_threshold_bytes;
 }
 
+constexpr uint32_t kSpanCap = 16384;  // profiled launches between two reads that also get a device-clock span
+
+// Hand the next launch its span pair (null once the arena is used up: such launches are timed by events only).
+unsigned long long* take_span(kvpool* p, ProfRec* r) {
+  if (!p->span_arena || p->span_cursor >= kSpanCap) return nullptr;
+  r->span = static_cast<int32_t>(p->span_cursor++);
+  return p->span_arena + 2ull * r->span;
+}
+
+// Spans start out as {UINT64_MAX, 0} so that atomicMin / atomicMax fold into them.
+cudaError_t reset_spans(kvpool* p) {
+  std::vector<unsigned long long> init(2ull * kSpanCap);
+  for (uint32_t i = 0; i < kSpanCap; ++i) { init[2 * i] = ~0ull; init[2 * i + 1] = 0; }
+  p->span_cursor = 0;
+  return cudaMemcpy(p->span_arena, init.data(), init.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice);
+}
+
 cudaError_t prof_event(kvpool* p, cudaEvent_t* e) {
   if (!p->prof_free.empty()) { *e = p->prof_free.back(); p->prof_free.pop_back(); return cudaSuccess; }
   return cudaEventCreate(e);
@@ -307,7 +327,9 @@ int launch_counted(kvpool* p, const LayerArgs& a, bool pack, bool link_bound, cu
     r.kind = (link_bound ? 2 : 0) + (pack ? 0 : 1);
     CU(cudaEventRecord(r.e0, s));
   }
-  CU(launch_layer_copy(a, pack, launch_cfg(p, link_bound), s));
+  LayerArgs timed = a;
+  if (p->profiling) timed.span = take_span(p, &r);
+  CU(launch_layer_copy(timed, pack, launch_cfg(p, link_bound), s));
   p->n_kernels++;
   if (p->profiling) {
     CU(cudaEventRecord(r.e1, s));
@@ -447,6 +469,7 @@ int kvpool_destroy(kvpool_t* p) {
   for (auto e : p->ev_free) cudaEventDestroy(e);
   for (auto& r : p->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   for (auto e : p->prof_free) cudaEventDestroy(e);
+  if (p->span_arena) cudaFree(p->span_arena);
   delete p;
   return KVPOOL_OK;
 }
@@ -843,7 +866,9 @@ static int launch_multi_counted(kvpool* p, const MultiArgs& ma, bool pack, bool 
     r.kind = (link_bound ? 2 : 0) + (pack ? 0 : 1);
     CU(cudaEventRecord(r.e0, s));
   }
-  CU(launch_multi_copy(ma, pack, launch_cfg(p, link_bound), s));
+  MultiArgs timed = ma;
+  if (p->profiling) timed.span = take_span(p, &r);
+  CU(launch_multi_copy(timed, pack, launch_cfg(p, link_bound), s));
   p->n_kernels++;
   if (p->profiling) {
     CU(cudaEventRecord(r.e1, s));
@@ -1309,32 +1334,59 @@ int kvpool_layer_map(const kvpool_placement_t* pl, uint32_t layer, uint8_t* dev_
 
 int kvpool_set_profiling(kvpool_t* p, int enabled) {
   if (!p) return fail(KVPOOL_EINVAL, "set_profiling: null pool");
+  if (enabled && !p->span_arena) {
+    DeviceGuard guard(p->cuda_device);
+    CU(cudaMalloc(reinterpret_cast<void**>(&p->span_arena), 2ull * kSpanCap * sizeof(unsigned long long)));
+    CU(reset_spans(p));
+  }
   p->profiling = enabled != 0;
   return KVPOOL_OK;
 }
 
-int kvpool_profile_read(kvpool_t* p, int kind, double* total_ms, uint64_t* launches, uint64_t* bytes) {
+int kvpool_profile_read_clock(kvpool_t* p, int kind, double* total_ms, double* device_ms, uint64_t* launches, uint64_t* device_launches,
+                              uint64_t* bytes) {
   if (!p || kind < 0 || kind > 3) return fail(KVPOOL_EINVAL, "profile_read: bad arguments");
   DeviceGuard guard(p->cuda_device);
-  double ms_sum = 0;
-  uint64_t n = 0, b = 0;
+  double ms_sum = 0, dev_ms_sum = 0;
+  uint64_t n = 0, n_dev = 0, b = 0;
   std::vector<ProfRec> keep;
+  std::vector<unsigned long long> spans;
+  bool any_span = false;
+  for (auto& r : p->prof)
+    if (r.kind == kind) {
+      CU(cudaEventSynchronize(r.e1));
+      any_span |= r.span >= 0;
+    }
+  if (any_span) {  // every launch of this kind has completed: one read-back of the spans handed out so far
+    spans.resize(2ull * p->span_cursor);
+    CU(cudaMemcpy(spans.data(), p->span_arena, spans.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+  }
   for (auto& r : p->prof) {
     if (r.kind != kind) { keep.push_back(r); continue; }
-    CU(cudaEventSynchronize(r.e1));
     float ms = 0;
     CU(cudaEventElapsedTime(&ms, r.e0, r.e1));
     ms_sum += ms;
     n += 1;
     b += r.bytes;
+    if (r.span >= 0) {
+      const unsigned long long t0 = spans[2ull * r.span], t1 = spans[2ull * r.span + 1];
+      if (t1 >= t0) { dev_ms_sum += static_cast<double>(t1 - t0) * 1e-6; n_dev += 1; }  // (a launch with no work leaves {max, 0})
+    }
     p->prof_free.push_back(r.e0);
     p->prof_free.push_back(r.e1);
   }
   p->prof.swap(keep);
+  if (p->prof.empty() && p->span_arena && p->span_cursor) CU(reset_spans(p));  // all read: the arena starts over
   if (total_ms) *total_ms = ms_sum;
+  if (device_ms) *device_ms = dev_ms_sum;
   if (launches) *launches = n;
+  if (device_launches) *device_launches = n_dev;
   if (bytes) *bytes = b;
   return KVPOOL_OK;
+}
+
+int kvpool_profile_read(kvpool_t* p, int kind, double* total_ms, uint64_t* launches, uint64_t* bytes) {
+  return kvpool_profile_read_clock(p, kind, total_ms, nullptr, launches, nullptr, bytes);
 }
 
 int kvpool_stats(const kvpool_t* p, uint64_t* kernel_launches, uint64_t* memcpy_calls) {

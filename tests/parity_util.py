@@ -44,7 +44,8 @@ def check_glt(pl: kv.Placement, opl: List[oracle.LayerPlacement], payload: int, 
 
 
 def run_parity(wl: W.Workload, *, path: int, kernel: int, bandwidth=None, tuning: Optional[dict] = None,
-               interleaved_layout: bool = False, streams: int = 1, dev_flags: Optional[Sequence[int]] = None) -> dict:
+               interleaved_layout: bool = False, streams: int = 1, dev_flags: Optional[Sequence[int]] = None,
+               profiling: bool = False) -> dict:
     """Offload every layer of every request, compare stripes with the oracle, retrieve into a poisoned pool,
     compare with the oracle's retrieve and with the source.  Returns a few counters."""
     dev = torch.device("cuda:0")
@@ -55,6 +56,7 @@ def run_parity(wl: W.Workload, *, path: int, kernel: int, bandwidth=None, tuning
     try:
         pool.set_path(path)
         pool.set_tuning(kernel=kernel, link_kernel=kernel, **(tuning or {}))
+        pool.set_profiling(profiling)
         cuda_streams = [torch.cuda.Stream(device=dev) for _ in range(streams)]
         R = len(wl.requests)
         pls = [pool.place(wl.blocks_per_layer(r)) for r in range(R)]
@@ -114,9 +116,10 @@ def run_parity(wl: W.Workload, *, path: int, kernel: int, bandwidth=None, tuning
             assert np.array_equal(got[:, used], src_cpu[:, used])                 # round trip, bit for bit
             assert np.all(got[:, ~used] == W.POISON_BITS)                         # nothing else written
         k, m = pool.stats()
+        prof = {kind: pool.profile_read_clock(kind) for kind in range(4)} if profiling else None
         for pl in pls:
             pl.release()
         assert all(pool.device_info(i)["used"] == 0 for i in range(pool.n_devices))
-        return {"bytes_compared": n_bytes, "kernels": k, "memcpys": m}
+        return {"bytes_compared": n_bytes, "kernels": k, "memcpys": m, "prof": prof}
     finally:
         pool.destroy()

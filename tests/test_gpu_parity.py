@@ -182,6 +182,25 @@ def test_pack_unpack_in_device_stripe_order(kernel):
         pool.destroy()
 
 
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_profiling_keeps_parity_and_reports_event_and_kernel_clock_spans(kernel):
+    """With profiling on the kernels also fold their start/end (%globaltimer) into a per-launch span: results must stay
+    bit-exact on both paths, every launch gets a span, and a launch's own span cannot exceed the event pair around it
+    by more than the clocks' granularity."""
+    wl = W.make_workload(4, scale=1 / 8, n_layers=4)
+    for path in (kv.PATH_STAGED, kv.PATH_ZEROCOPY):
+        out = run_parity(wl, path=path, kernel=KERNELS[kernel], profiling=True)
+        prof = out["prof"]
+        pack_kind, unpack_kind = (kv.KvPool.PROF_PACK, kv.KvPool.PROF_UNPACK) if path == kv.PATH_STAGED else (kv.KvPool.PROF_ZC_OFFLOAD, kv.KvPool.PROF_ZC_RETRIEVE)
+        for kind in range(4):
+            ms, dms, n, nd, b = prof[kind]
+            if kind in (pack_kind, unpack_kind):
+                assert n == nd == wl.geom.n_layers and b == sum(int(k) for k in wl.blocks_per_layer(0)) * wl.geom.payload
+                assert 0.0 < dms <= ms + 0.02 * n, (ms, dms)          # events bracket the kernel; 20 us per launch of clock slack
+            else:
+                assert (ms, dms, n, nd, b) == (0.0, 0.0, 0, 0, 0)
+
+
 def test_kv_stream_is_identical_on_cpu_and_gpu():
     wl = W.make_workload(2, n_layers=1)
     a = W.kv_layer_torch(wl, 0, "cuda:0").cpu().numpy().view(np.uint16)
