@@ -120,6 +120,12 @@ KVPOOL_API int kvpool_plan_weights(const double* bandwidth_gbps /*host[n]*/, uin
 KVPOOL_API int kvpool_plan_layer(const uint64_t* w /*host[n]*/, uint32_t n, uint64_t K, uint32_t* counts_out /*host[n]*/,
                       uint8_t* dev_out /*host[K] or NULL*/, uint32_t* slot_out /*host[K] or NULL*/);
 
+/* The caller's contract on a block table (R12), checked on a HOST copy: K entries, each in [0, nphys), no
+ * physical block named twice (a duplicate would make two KV caches race for one block at retrieve).  The hot path
+ * never validates tables on the device; engines call this in debug builds or tests.  EINVAL with the first offending
+ * entry in kvpool_last_error().  K = 0 is valid.                                                                  */
+KVPOOL_API int kvpool_validate_table(const int32_t* table /*host[K]*/, uint64_t K, uint64_t nphys);
+
 /* ---- pool life cycle ----------------------------------------------------------------------------------
  * kvpool_create enumerates the pool devices: allocates one pinned, GPU-mapped host
  * buffer per device (bound to its NUMA node when asked and possible), per-device CUDA streams, events
@@ -183,6 +189,16 @@ KVPOOL_API int kvpool_offload_layers(kvpool_t* pool, kvpool_placement_t* pl, uin
 KVPOOL_API int kvpool_retrieve_layers(kvpool_t* pool, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers,
                            void* const* k_bases /*host[n_layers]*/, void* const* v_bases /*host[n_layers]*/,
                            uint64_t block_stride_bytes, const int32_t* const* block_tables /*host[n_layers]*/, void* cuda_stream);
+/* kvpool_retrieve_layers for a consumer on ANOTHER stream (layerwise pipelining): layer_ready is a HOST
+ * array of n_layers caller-owned cudaEvent_t (entries may be NULL); layer_ready[q] is recorded on `stream` as soon as layer
+ * first_layer + q is complete in the paged layout, so the consumer does cudaStreamWaitEvent(consumer, layer_ready[q]) and
+ * computes layer q while the pool is still moving layers q+1, ... (the staged path's host->GPU copies run up to
+ * `stage_slots` layers ahead).  Layers that travel as one group (small layers, see above) become ready together; a layer
+ * with K_l = 0 is ready at once.  One host call per request instead of one per layer.                                 */
+KVPOOL_API int kvpool_retrieve_layers_signal(kvpool_t* pool, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers,
+                                  void* const* k_bases /*host[n_layers]*/, void* const* v_bases /*host[n_layers]*/,
+                                  uint64_t block_stride_bytes, const int32_t* const* block_tables /*host[n_layers]*/,
+                                  void* const* layer_ready /*host[n_layers] of cudaEvent_t*/, void* cuda_stream);
 /* Partial retrieval (prefix reuse, chunked prefetch): like kvpool_retrieve for logical blocks
  * [first_block, first_block + n_blocks) of the layer only.  block_table_dev is still the LAYER's table (indexed by
  * logical block, as at offload); only the entries of the range are read and only their physical blocks written.

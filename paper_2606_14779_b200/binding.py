@@ -27,9 +27,9 @@ _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA",
 EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
     "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_place", "kvpool_release",
-    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
+    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
-    "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_last_error", "kvpool_version",
+    "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_validate_table", "kvpool_last_error", "kvpool_version",
 ]
 
 
@@ -72,6 +72,7 @@ def lib():
         sig = {
             "kvpool_plan_weights": [vp, c_uint32, vp],
             "kvpool_plan_layer": [vp, c_uint32, c_uint64, vp, vp, vp],
+            "kvpool_validate_table": [vp, c_uint64, c_uint64],
             "kvpool_create": [vp, c_uint32, vp, c_int, c_uint32, POINTER(vp)],
             "kvpool_destroy": [vp],
             "kvpool_set_bandwidth": [vp, vp],
@@ -86,6 +87,7 @@ def lib():
             "kvpool_retrieve_range": [vp, vp, c_uint32, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_offload_layers": [vp, vp, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_retrieve_layers": [vp, vp, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
+            "kvpool_retrieve_layers_signal": [vp, vp, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp, vp],
             "kvpool_offload_naive": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_retrieve_naive": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_wait_offloads": [vp, vp, vp],
@@ -145,6 +147,17 @@ def _stream(s) -> int:
     return s.cuda_stream  # torch.cuda.Stream
 
 
+def _event(e) -> int:
+    """cudaEvent_t handle of a torch.cuda.Event (created on first use), an int handle, or None."""
+    if e is None:
+        return 0
+    if isinstance(e, int):
+        return e
+    if not e.cuda_event:  # torch creates the CUDA event lazily, on its first record
+        e.record()
+    return e.cuda_event
+
+
 # ---- pure host arithmetic ----------------------------------------------------------------------------
 def kvpool_plan_weights(bandwidth_gbps: Sequence[float]) -> np.ndarray:
     b = np.ascontiguousarray(bandwidth_gbps, dtype=np.float64)
@@ -161,6 +174,12 @@ def kvpool_plan_layer(w: Sequence[int], K: int, with_map: bool = True):
     _ck(lib().kvpool_plan_layer(w.ctypes.data, w.shape[0], int(K), counts.ctypes.data,
                                 dev.ctypes.data if with_map else None, slot.ctypes.data if with_map else None))
     return (counts, dev, slot) if with_map else counts
+
+
+def kvpool_validate_table(table: np.ndarray, nphys: int) -> None:
+    """Raises KvPoolError(EINVAL) unless `table` (host int32) names distinct physical blocks in [0, nphys)."""
+    t = np.ascontiguousarray(table, dtype=np.int32)
+    _ck(lib().kvpool_validate_table(t.ctypes.data, t.shape[0], int(nphys)))
 
 
 # ---- pool ---------------------------------------------------------------------------------------------
@@ -301,6 +320,15 @@ class KvPool:
         ka, va, ta = self._ptr_array(k_bases), self._ptr_array(v_bases), self._ptr_array(block_tables)
         _ck(lib().kvpool_retrieve_layers(self.handle, pl.handle, first_layer, n, ctypes.addressof(ka), ctypes.addressof(va),
                                          block_stride_bytes, ctypes.addressof(ta), _stream(stream)))
+
+    def retrieve_layers_signal(self, pl: Placement, first_layer: int, k_bases, v_bases, block_stride_bytes: int, block_tables, layer_ready,
+                               stream=None) -> None:
+        """layer_ready: one torch.cuda.Event (or raw cudaEvent_t handle, or None) per layer, recorded when that layer is complete."""
+        n = len(k_bases)
+        ka, va, ta = self._ptr_array(k_bases), self._ptr_array(v_bases), self._ptr_array(block_tables)
+        ea = (c_void_p * n)(*[_event(e) for e in layer_ready])
+        _ck(lib().kvpool_retrieve_layers_signal(self.handle, pl.handle, first_layer, n, ctypes.addressof(ka), ctypes.addressof(va),
+                                                block_stride_bytes, ctypes.addressof(ta), ctypes.addressof(ea), _stream(stream)))
 
     def offload_naive(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_host: np.ndarray, stream=None) -> None:
         t = np.ascontiguousarray(block_table_host, dtype=np.int32)

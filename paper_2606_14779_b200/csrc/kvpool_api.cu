@@ -376,6 +376,23 @@ int kvpool_plan_layer(const uint64_t* w, uint32_t n, uint64_t K, uint32_t* count
   return KVPOOL_OK;
 }
 
+int kvpool_validate_table(const int32_t* table, uint64_t K, uint64_t nphys) {
+  if (K == 0) return KVPOOL_OK;
+  if (!table) return fail(KVPOOL_EINVAL, "validate_table: null table");
+  if (nphys == 0 || nphys > 0x7fffffffull) return fail(KVPOOL_EINVAL, "validate_table: nphys %llu not in 1..2^31-1", (unsigned long long)nphys);
+  if (K > nphys) return fail(KVPOOL_EINVAL, "validate_table: %llu entries cannot be distinct among %llu physical blocks", (unsigned long long)K, (unsigned long long)nphys);
+  std::vector<uint64_t> seen((nphys + 63) / 64, 0);
+  for (uint64_t j = 0; j < K; ++j) {
+    const int64_t v = table[j];
+    if (v < 0 || static_cast<uint64_t>(v) >= nphys) return fail(KVPOOL_EINVAL, "validate_table: entry %llu = %lld is outside [0, %llu)", (unsigned long long)j, (long long)v, (unsigned long long)nphys);
+    uint64_t& word = seen[static_cast<uint64_t>(v) >> 6];
+    const uint64_t bit = 1ull << (v & 63);
+    if (word & bit) return fail(KVPOOL_EINVAL, "validate_table: physical block %lld appears twice (second time at entry %llu)", (long long)v, (unsigned long long)j);
+    word |= bit;
+  }
+  return KVPOOL_OK;
+}
+
 int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_geometry* g, int cuda_device, uint32_t flags,
                   kvpool_t** out) {
   if (!devs || !g || !out) return fail(KVPOOL_EINVAL, "create: null argument");
@@ -893,6 +910,7 @@ struct BatchCall {
   const int32_t* const* tables;
   uint64_t stride;
   cudaStream_t s;
+  void* const* ready;  // optional: caller-owned cudaEvent_t per layer of the call, recorded on `s` when that layer is complete
 };
 
 void fill_descs(const BatchCall& c, const LayerGroup& g, MultiArgs* ma) {
@@ -1027,9 +1045,20 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   return KVPOOL_OK;
 }
 
+int issue_group_work(const BatchCall& c, const LayerGroup& g);
+
+// Move one group, then tell the caller's per-layer events: the layers of a group become ready together.
 int issue_group(const BatchCall& c, const LayerGroup& g) {
-  kvpool* p = c.p;
   if (g.n == 0) return KVPOOL_OK;
+  const int rc = issue_group_work(c, g);
+  if (rc != KVPOOL_OK || !c.ready) return rc;
+  for (uint32_t b = 0; b < g.n; ++b)
+    if (c.ready[g.q[b]]) CU(cudaEventRecord(static_cast<cudaEvent_t>(c.ready[g.q[b]]), c.s));
+  return KVPOOL_OK;
+}
+
+int issue_group_work(const BatchCall& c, const LayerGroup& g) {
+  kvpool* p = c.p;
   const bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && g.bytes >= p->tune.auto_threshold_bytes));
   if (!staged) return issue_zero_copy_group(c, g);
   if (g.n > 1) {
@@ -1050,7 +1079,8 @@ int issue_group(const BatchCall& c, const LayerGroup& g) {
 // layer at least that large travels with whatever small layers precede it); each group moves as one unit: one fused
 // zero-copy launch, or one pack/unpack launch plus one copy per pool device.
 static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32_t first, uint32_t n, const void* const* k_bases,
-                          const void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream) {
+                          const void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream,
+                          void* const* ready = nullptr) {
   if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "layers: bad pool or placement");
   if (static_cast<uint64_t>(first) + n > p->geom.n_layers) return fail(KVPOOL_EINVAL, "layers [%u, %u) out of range (n_layers %u)", first, first + n, p->geom.n_layers);
   if (n == 0) return KVPOOL_OK;
@@ -1061,14 +1091,17 @@ static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32
     if (!pack && !pl->layers[first + q].offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", first + q);
   }
   DeviceGuard guard(p->cuda_device);
-  const BatchCall c{p, pl, pack, first, k_bases, v_bases, tables, stride, static_cast<cudaStream_t>(cuda_stream)};
+  const BatchCall c{p, pl, pack, first, k_bases, v_bases, tables, stride, static_cast<cudaStream_t>(cuda_stream), ready};
   const uint64_t cap = std::max<uint64_t>(p->tune.group_bytes, 1);
   LayerGroup g;
   uint64_t units = 0;
   for (uint32_t q = 0; q < n; ++q) {
     LayerState& L = pl->layers[first + q];
     if (pack) L.offloaded = true;
-    if (L.map->K == 0) continue;
+    if (L.map->K == 0) {  // nothing to move: ready in stream order right away
+      if (ready && ready[q]) CU(cudaEventRecord(static_cast<cudaEvent_t>(ready[q]), c.s));
+      continue;
+    }
     const uint64_t bytes = L.map->K * p->payload;
     if (g.n && (g.n == kMaxBatch || units + L.map->K > 0x7fffffffull || (p->path != KVPOOL_PATH_ZEROCOPY && g.bytes + bytes > std::max(cap, bytes)))) {
       const int rc = issue_group(c, g);
@@ -1097,6 +1130,13 @@ int kvpool_offload_layers(kvpool_t* p, kvpool_placement_t* pl, uint32_t first_la
 int kvpool_retrieve_layers(kvpool_t* p, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers, void* const* k_bases,
                            void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream) {
   return layers_batched(p, pl, false, first_layer, n_layers, k_bases, v_bases, stride, tables, cuda_stream);
+}
+
+int kvpool_retrieve_layers_signal(kvpool_t* p, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers, void* const* k_bases,
+                                  void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* const* layer_ready,
+                                  void* cuda_stream) {
+  if (n_layers && !layer_ready) return fail(KVPOOL_EINVAL, "retrieve_layers_signal: null layer_ready array");
+  return layers_batched(p, pl, false, first_layer, n_layers, k_bases, v_bases, stride, tables, cuda_stream, layer_ready);
 }
 
 // Baseline for comparison: 2*K_l individual cudaMemcpyAsync calls per layer, no kernel.

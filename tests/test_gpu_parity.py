@@ -408,6 +408,55 @@ def test_batched_layers_grouped_launches(kernel):
     _run_batched(wl, kv.PATH_STAGED, k, expect_kernels=2 * 3, expect_memcpys=2 * 3 * 3)
 
 
+@pytest.mark.parametrize("path", ["staged", "zerocopy", "auto"])
+def test_retrieve_layers_signal_feeds_a_consumer_on_another_stream(path):
+    """Layerwise pipelining through ONE batched call: the retrieve stream records a caller-owned event per
+    layer; a consumer stream waits on each and checksums that layer straight away.  Every checksum must equal the oracle's
+    for the source layer (a consumer that ran before its layer was complete would read poison), and the retrieved tensors
+    must equal the oracle's retrieve."""
+    dev = torch.device("cuda:0")
+    wl = W.make_workload(3, scale=1 / 8, n_layers=6)       # 256 KiB and 32 MiB layers alternate: groups and single layers
+    g, L = wl.geom, wl.geom.n_layers
+    bw = list(wl.default_weights())
+    pool = make_pool(wl)
+    try:
+        pool.set_path(PATHS[path])
+        bpl = list(wl.blocks_per_layer(0))
+        bpl[4] = 0                                         # an empty layer in the middle: ready at once, nothing moved
+        pl, opl = pool.place(bpl), oracle.place(bw, bpl)
+        tables_np = [np.ascontiguousarray(wl.layer_table(0, l))[:bpl[l]] for l in range(L)]
+        tables = [torch.from_numpy(t).to(dev) if len(t) else None for t in tables_np]
+        src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+        dst = [W.poison_torch((2, wl.nphys, g.kvb // 2), dev) for l in range(L)]
+        sums = torch.zeros(L, dtype=torch.int64, device=dev)
+        torch.cuda.synchronize()
+        io, consumer = torch.cuda.Stream(), torch.cuda.Stream()
+        pool.offload_layers(pl, 0, [x[0] for x in src], [x[1] for x in src], g.kvb, tables, io)
+        pool.wait_offloads(pl, io)
+        ready = [torch.cuda.Event() for _ in range(L)]
+        with pytest.raises(kv.KvPoolError) as e:           # validated before anything is enqueued
+            pool.retrieve_layers_signal(pl, 0, [d[0] for d in dst], [None] + [d[1] for d in dst][1:], g.kvb, tables, ready, io)
+        assert e.value.code == kv.EINVAL
+        pool.retrieve_layers_signal(pl, 0, [d[0] for d in dst], [d[1] for d in dst], g.kvb, tables, ready, io)
+        for l in range(L):                                 # the consumer never synchronises with `io` except through the events
+            consumer.wait_event(ready[l])
+            if bpl[l]:
+                pool.checksum(dst[l][0], dst[l][1], g.kvb, tables[l], bpl[l], sums[l:l + 1], consumer)
+        consumer.synchronize()
+        got = [int(x) % 2 ** 64 for x in sums.cpu().tolist()]
+        want = [oracle.checksum(W.kv_layer_numpy(wl, l), tables_np[l]) if bpl[l] else 0 for l in range(L)]
+        assert got == want
+        io.synchronize()
+        for l in range(L):
+            stripes = oracle.offload_layer(W.kv_layer_numpy(wl, l), tables_np[l], opl[l])
+            ref = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+            oracle.retrieve_layer(ref, tables_np[l], opl[l], stripes)
+            assert np.array_equal(dst[l].cpu().numpy().view(np.uint16), ref), f"retrieved layer {l} differs"
+        pl.release()
+    finally:
+        pool.destroy()
+
+
 def test_numa_bound_registered_and_write_combined_pool_buffers():
     """Pool-device flavours: mmap + mbind(node 0) + cudaHostRegister, a node that does not exist (falls back unless
     KVPOOL_DEV_NUMA_STRICT, then ENUMA), and write-combined buffers — all bit-exact through both paths."""

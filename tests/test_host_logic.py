@@ -86,6 +86,24 @@ def test_plan_weights_quantisation_and_errors():
         kv.kvpool_plan_layer([1, 0, 1], 5)                     # zero weight
 
 
+def test_validate_table_accepts_every_workload_table_and_names_the_offending_entry():
+    """DESIGN.md R12: distinct entries in [0, nphys) are the caller's contract; the host-side checker states it."""
+    for cfg in (1, 3, 5):
+        wl = W.make_workload(cfg, scale=1 / 8) if cfg != 1 else W.make_workload(cfg)
+        for r in range(len(wl.requests)):
+            for l in (0, 1, wl.geom.n_layers - 1):
+                kv.kvpool_validate_table(wl.layer_table(r, l), wl.nphys)
+    kv.kvpool_validate_table(np.zeros(0, np.int32), 1)                       # K = 0 is valid
+    kv.kvpool_validate_table(np.arange(64, dtype=np.int32)[::-1], 64)        # a full permutation
+    for bad, nphys, word in (([0, 1, 64], 64, "outside"), ([0, -1], 64, "outside"), ([3, 5, 3], 64, "twice"), ([0, 1, 2], 2, "distinct")):
+        with pytest.raises(kv.KvPoolError) as e:
+            kv.kvpool_validate_table(np.array(bad, np.int32), nphys)
+        assert e.value.code == kv.EINVAL and word in str(e.value)
+    with pytest.raises(kv.KvPoolError) as e:
+        kv.kvpool_validate_table(np.array([7, 9, 7], np.int32), 16)
+    assert "entry 2" in str(e.value) and "block 7" in str(e.value)
+
+
 def test_create_without_gpu_fails_loudly_with_ecuda():
     import torch
     if torch.cuda.is_available():
