@@ -147,9 +147,18 @@ KVPOOL_API int kvpool_set_path(kvpool_t* pool, int path /*KVPOOL_PATH_**/);
 KVPOOL_API int kvpool_set_tuning(kvpool_t* pool, const kvpool_tuning* t /*host*/);
 KVPOOL_API int kvpool_get_tuning(const kvpool_t* pool, kvpool_tuning* t_out /*host*/);
 
+/* Size the staging ring of the staged path now: `stage_slots` device buffers of `bytes` bytes each.  A placement needs
+ * max(its largest layer K_l * P, min(group_bytes, all its layers together)) — the second term for the groups of small
+ * layers the batched calls form.  kvpool_place grows the ring by itself when a placement needs more, but
+ * growing waits for the whole device (cudaDeviceSynchronize) and reallocates; an engine that knows its largest layer
+ * calls this once at start-up and no later kvpool_place ever waits for GPU work.  ENOMEM if the device is out of memory. */
+KVPOOL_API int kvpool_reserve_staging(kvpool_t* pool, uint64_t bytes);
+
 /* ---- placement: Alg. 1 l.4-16 + stripe allocation + GLT update (a1-a4) ------------------------------
  * blocks_per_layer[l] = K_l, the number of KV blocks of layer l to offload (may differ per layer and
- * may be 0).  Host work plus one upload of the per-layer tables.  ENOMEM (nothing reserved) if some pool
+ * may be 0).  Host work plus one upload of the per-layer tables on the library's own stream: the call does not wait for
+ * work queued on any other stream, the legacy default stream included (unless the staging ring must grow, see
+ * kvpool_reserve_staging).  ENOMEM (nothing reserved) if some pool
  * device cannot hold its stripes.                                                                      */
 KVPOOL_API int kvpool_place(kvpool_t* pool, const uint32_t* blocks_per_layer /*host[n_layers]*/, kvpool_placement_t** out);
 /* Frees the stripes and tables.  The caller must have synchronised the streams it used with it.        */

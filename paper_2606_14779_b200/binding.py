@@ -26,7 +26,7 @@ _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA",
 
 EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
-    "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_place", "kvpool_release",
+    "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release",
     "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
     "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_validate_table", "kvpool_last_error", "kvpool_version",
@@ -79,6 +79,7 @@ def lib():
             "kvpool_measure_bandwidth": [vp, c_uint32, c_int, c_uint64, c_uint32, POINTER(c_double)],
             "kvpool_set_path": [vp, c_int],
             "kvpool_set_tuning": [vp, vp],
+            "kvpool_reserve_staging": [vp, c_uint64],
             "kvpool_get_tuning": [vp, vp],
             "kvpool_place": [vp, vp, POINTER(vp)],
             "kvpool_release": [vp, vp],
@@ -284,6 +285,9 @@ class KvPool:
         t = Tuning()
         _ck(lib().kvpool_get_tuning(self.handle, ctypes.addressof(t)))
         return t
+
+    def reserve_staging(self, nbytes: int) -> None:
+        _ck(lib().kvpool_reserve_staging(self.handle, int(nbytes)))
 
     def place(self, blocks_per_layer: Sequence[int]) -> Placement:
         b = np.ascontiguousarray(blocks_per_layer, dtype=np.uint32)

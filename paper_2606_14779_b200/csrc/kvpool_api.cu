@@ -135,6 +135,10 @@ struct kvpool {
   uint64_t slot_bytes = 0;
   uint64_t slot_cursor = 0;
   uint8_t* table_arena = nullptr;  // device memory for placements' GLT columns: no cudaMalloc/cudaFree per request
+  uint8_t* table_arena_host = nullptr;  // its pinned host mirror: tables are built in place and uploaded on `upload`
+  cudaStream_t upload = nullptr;   // the library's own non-blocking stream for table uploads and small read-backs, so that
+                                   // kvpool_place never touches the legacy default stream (which would make it wait for
+                                   // whatever the application has queued there)
   StripeAllocator table_alloc;
   std::vector<cudaEvent_t> ev_free;  // recycled cudaEventDisableTiming events
   int path = KVPOOL_PATH_AUTO;
@@ -309,7 +313,8 @@ cudaError_t reset_spans(kvpool* p) {
   std::vector<unsigned long long> init(2ull * kSpanCap);
   for (uint32_t i = 0; i < kSpanCap; ++i) { init[2 * i] = ~0ull; init[2 * i + 1] = 0; }
   p->span_cursor = 0;
-  return cudaMemcpy(p->span_arena, init.data(), init.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice);
+  cudaError_t e = cudaMemcpyAsync(p->span_arena, init.data(), init.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, p->upload);
+  return e == cudaSuccess ? cudaStreamSynchronize(p->upload) : e;
 }
 
 cudaError_t prof_event(kvpool* p, cudaEvent_t* e) {
@@ -439,6 +444,8 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     for (auto s : p->io) if (s) cudaStreamDestroy(s);
     for (auto s : p->io_out) if (s) cudaStreamDestroy(s);
     if (p->table_arena) cudaFree(p->table_arena);
+    if (p->table_arena_host) cudaFreeHost(p->table_arena_host);
+    if (p->upload) cudaStreamDestroy(p->upload);
   };
   p->bufs.resize(n_devs);
   for (uint32_t i = 0; i < n_devs; ++i) {
@@ -467,6 +474,12 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     cleanup();
     return fail(KVPOOL_ENOMEM, "create: table arena");
   }
+  if (cudaHostAlloc(reinterpret_cast<void**>(&p->table_arena_host), kTableArenaBytes, cudaHostAllocDefault) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&p->upload, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaGetLastError();
+    cleanup();
+    return fail(KVPOOL_ENOMEM, "create: table arena mirror / upload stream");
+  }
   p->table_alloc = StripeAllocator(kTableArenaBytes, 256);
   *out = p.release();
   return KVPOOL_OK;
@@ -483,6 +496,8 @@ int kvpool_destroy(kvpool_t* p) {
   for (auto s : p->io_out) cudaStreamDestroy(s);
   for (auto& b : p->bufs) host_buffer_free(&b);
   if (p->table_arena) cudaFree(p->table_arena);
+  if (p->table_arena_host) cudaFreeHost(p->table_arena_host);
+  if (p->upload) cudaStreamDestroy(p->upload);
   for (auto e : p->ev_free) cudaEventDestroy(e);
   for (auto& r : p->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   for (auto e : p->prof_free) cudaEventDestroy(e);
@@ -579,6 +594,13 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
   return KVPOOL_OK;
 }
 
+int kvpool_reserve_staging(kvpool_t* p, uint64_t bytes) {
+  if (!p) return fail(KVPOOL_EINVAL, "reserve_staging: null pool");
+  if (all_hbm(p)) return KVPOOL_OK;  // nothing is ever staged
+  DeviceGuard guard(p->cuda_device);
+  return ensure_slots(p, bytes + static_cast<uint64_t>(p->n) * 256 * (kMaxBatch + 1));
+}
+
 int kvpool_get_tuning(const kvpool_t* p, kvpool_tuning* t_out) {
   if (!p || !t_out) return fail(KVPOOL_EINVAL, "get_tuning: null argument");
   *t_out = p->tune;
@@ -672,26 +694,30 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
       e = cudaMalloc(reinterpret_cast<void**>(&pl->tables_d), table_bytes);  // arena exhausted: private allocation
       if (e != cudaSuccess) { cudaGetLastError(); pl->tables_d = nullptr; rollback(); return fail(KVPOOL_ENOMEM, "place: table upload buffer: %s", cudaGetErrorString(e)); }
     }
-    std::vector<uint8_t> host(table_bytes);
+    // built in the pinned mirror of the arena (or, for a private allocation, in pageable memory) and uploaded on the
+    // library's own stream: no use of the legacy default stream, so no implicit wait for the application's work
+    std::vector<uint8_t> pageable(pl->tables_in_arena ? 0 : table_bytes);
+    uint8_t* const host = pl->tables_in_arena ? p->table_arena_host + arena_off : pageable.data();
     uint64_t off = 0;
     for (auto& kv : by_k) {
       LayerMap& m = *kv.second;
       if (m.K == 0) continue;
       m.slot_d = reinterpret_cast<const uint32_t*>(pl->tables_d + off);
-      memcpy(host.data() + off, m.slot.data(), m.K * 4);
+      memcpy(host + off, m.slot.data(), m.K * 4);
       off += (m.K * 4 + 255) / 256 * 256;
       m.dev_d = pl->tables_d + off;
-      memcpy(host.data() + off, m.dev.data(), m.K);
+      memcpy(host + off, m.dev.data(), m.K);
       off += (m.K + 255) / 256 * 256;
     }
     for (uint32_t l = 0; l < L; ++l) {  // GPU-visible stripe addresses, one row per layer
-      uint64_t* row = reinterpret_cast<uint64_t*>(host.data() + off) + static_cast<uint64_t>(l) * N;
+      uint64_t* row = reinterpret_cast<uint64_t*>(host + off) + static_cast<uint64_t>(l) * N;
       for (uint32_t i = 0; i < N; ++i)
         row[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + pl->layers[l].stripe_off[i]);
       pl->layers[l].base_d = reinterpret_cast<const uint64_t*>(pl->tables_d + off) + static_cast<uint64_t>(l) * N;
     }
     off += bases_bytes;
-    e = cudaMemcpy(pl->tables_d, host.data(), off, cudaMemcpyHostToDevice);
+    e = cudaMemcpyAsync(pl->tables_d, host, off, cudaMemcpyHostToDevice, p->upload);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->upload);  // the tables are in place before any launch can name them
     if (e != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: table upload: %s", cudaGetErrorString(e)); }
   }
   for (auto& Ls : pl->layers) {
@@ -1317,7 +1343,8 @@ int kvpool_stripe_read(kvpool_t* p, const kvpool_placement_t* pl, uint32_t layer
   const uint8_t* src = pool_bytes(p, dev) + L.stripe_off[dev];
   if (is_hbm(p, dev)) {
     DeviceGuard guard(p->cuda_device);
-    CU(cudaMemcpy(dst_host, src, nbytes, cudaMemcpyDeviceToHost));
+    CU(cudaMemcpyAsync(dst_host, src, nbytes, cudaMemcpyDeviceToHost, p->upload));
+    CU(cudaStreamSynchronize(p->upload));
   } else {
     memcpy(dst_host, src, nbytes);
   }
@@ -1399,7 +1426,8 @@ int kvpool_profile_read_clock(kvpool_t* p, int kind, double* total_ms, double* d
     }
   if (any_span) {  // every launch of this kind has completed: one read-back of the spans handed out so far
     spans.resize(2ull * p->span_cursor);
-    CU(cudaMemcpy(spans.data(), p->span_arena, spans.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    CU(cudaMemcpyAsync(spans.data(), p->span_arena, spans.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->upload));
+    CU(cudaStreamSynchronize(p->upload));
   }
   for (auto& r : p->prof) {
     if (r.kind != kind) { keep.push_back(r); continue; }

@@ -131,6 +131,31 @@ def test_empty_layers_and_state_errors():
         pool.destroy()
 
 
+def test_place_does_not_wait_for_work_on_the_legacy_default_stream():
+    """kvpool_place uploads its tables on the library's own stream: with the staging ring reserved up front it returns in
+    host time while a long kernel still occupies the legacy default stream (a synchronous cudaMemcpy would wait for it)."""
+    import time
+    g = W.Geometry(n_layers=4, n_kv_heads=2, head_dim=64)
+    wl = _custom(g, 600, [np.random.default_rng(41).permutation(600)[:512]], 2, (2.0, 1.0))
+    pool = make_pool(wl)
+    try:
+        pool.set_path(kv.PATH_STAGED)
+        pool.reserve_staging(64 << 20)                    # >= max(largest layer, group_bytes): no placement below grows the ring
+        torch.cuda.synchronize()
+        pool.spin(400_000_000, None)                      # 0.4 s on the legacy default stream
+        t0 = time.perf_counter()
+        pl = pool.place(wl.blocks_per_layer(0))
+        dt = time.perf_counter() - t0
+        busy = not torch.cuda.default_stream().query()    # the spin kernel must still be running for the timing to mean anything
+        torch.cuda.synchronize()
+        assert busy and dt < 0.1, (busy, dt)
+        check_placement(pl, oracle.place([2.0, 1.0], wl.blocks_per_layer(0)))
+        pl.release()
+    finally:
+        pool.destroy()
+    run_parity(wl, path=kv.PATH_STAGED, kernel=kv.KERNEL_VEC16)
+
+
 def test_pool_full_is_enomem_with_no_partial_reservation():
     g = W.Geometry(n_layers=4, n_kv_heads=2, head_dim=64)
     pool = kv.KvPool([1.0, 1.0], [64 * g.payload, 64 * g.payload], n_layers=4, n_kv_heads=2, head_dim=64)
