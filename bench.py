@@ -56,6 +56,7 @@ def parse_args():
     ap.add_argument("--per-layer", action="store_true",
                     help="issue one kvpool_offload / kvpool_retrieve call per layer in the timed step instead of the batched *_layers calls")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--settle-s", type=float, default=60.0, help="upper bound on the untimed host-settle phase before the timed steps (0 = off)")
     ap.add_argument("--sweep", choices=["hbm", "link"], default=None,
                     help="tuning sweep instead of the benchmark: in-device pack/unpack (hbm) or zero-copy transfer (link) GB/s over launch shapes")
     ap.add_argument("--variants", action="store_true",
@@ -371,8 +372,21 @@ def run_kvpool(args) -> dict:
             rec["retrieve_ms"].append(ev[2].elapsed_time(ev[3]))
 
     rec = {"place_ms": [], "offload_ms": [], "retrieve_ms": []}
+    warm = {"place_ms": [], "offload_ms": [], "retrieve_ms": []}
     for _ in range(args.warmup):
-        step(False, rec)
+        step(True, warm)
+    # Host settle (untimed, disclosed in the JSON): in the first minutes after a GPU VM boots, DMA over a multi-GiB pinned
+    # working set — and plain CPU memcpy — run 10-50 % below their steady state on this pool of boxes (the 1 GiB link probe
+    # does not show it).  If the last warm-up leg is well below the link peak measured a moment ago, keep stepping, for at
+    # most --settle-s seconds, until it is not.  A box that never gets there is timed as it is.
+    settle = {"extra_steps": 0, "seconds": 0.0}
+    t_settle = time.perf_counter()
+    want_gbps = 0.9 * min(link_h2d, 55.0) * (0.92 if args.path == "zerocopy" else 1.0)
+    while (args.settle_s > 0 and moved >= (1 << 30) and warm["retrieve_ms"] and moved / (warm["retrieve_ms"][-1] * 1e6) < want_gbps
+           and time.perf_counter() - t_settle < args.settle_s):
+        step(True, warm)
+        settle["extra_steps"] += 1
+        settle["seconds"] = time.perf_counter() - t_settle
 
     def barrier():
         if world > 1:
@@ -583,7 +597,7 @@ def run_kvpool(args) -> dict:
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": moved + table_bytes, "d2h_bytes_per_step": d2h_bytes,
                 "what": "retrieve leg by host wall clock: pinned block tables H2D + kvpool_retrieve x layers + D2H of one block per layer + sync",
                 "offload_gbps": world * moved / (statistics.median(e2e_off_s) * 1e9)},
-        "gpu_launches": k1 - k0, "memcpy_calls": m1 - m0,
+        "gpu_launches": k1 - k0, "memcpy_calls": m1 - m0, "host_settle": settle,
         "roofline": roof, "roofline_link": link_roof, "roofline_hbm": hbm_roof,
         "clocks": clocks,
     }
