@@ -294,8 +294,11 @@ inline bool all_hbm(const kvpool* p) { return p->hbm_mask == (p->n >= 32 ? 0xFFF
 
 bool use_staged(const kvpool* p, const LayerState& L) {
   if (all_hbm(p)) return false;  // nothing to stage: every stripe is reached in place (one kernel, HBM grid)
-  if (p->path == KVPOOL_PATH_STAGED) return true;
   if (p->path == KVPOOL_PATH_ZEROCOPY) return false;
+  bool host_blocks = false;  // a layer whose blocks all went to HBM-type devices (tiny K, large weights) has nothing to stage
+  for (uint32_t i = 0; i < p->n; ++i) host_blocks |= L.map->counts[i] && !is_hbm(p, i);
+  if (!host_blocks) return false;
+  if (p->path == KVPOOL_PATH_STAGED) return true;
   return L.map->K * p->payload >= p->tune.auto_threshold_bytes;
 }
 
@@ -847,7 +850,18 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   a.j0 = first_block;
   a.K = n_blocks;
   const uint64_t range_bytes = static_cast<uint64_t>(n_blocks) * p->payload;
-  const bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && range_bytes >= p->tune.auto_threshold_bytes));
+  bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && range_bytes >= p->tune.auto_threshold_bytes));
+  uint32_t lo[KVPOOL_MAX_DEVICES], hi[KVPOOL_MAX_DEVICES];
+  if (staged) {
+    // a range whose blocks all sit on HBM-type devices has nothing to stage: it must not take (and so recycle) a slot
+    bool host_blocks = false;
+    for (uint32_t i = 0; i < N; ++i) {
+      if (n_blocks == L.map->K) { lo[i] = 0; hi[i] = L.map->counts[i]; }
+      else slot_range(*L.map, i, first_block, n_blocks, &lo[i], &hi[i]);
+      host_blocks |= hi[i] != lo[i] && !is_hbm(p, i);
+    }
+    staged = host_blocks;
+  }
 
   if (!staged) {
     for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
@@ -862,11 +876,8 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
     return fail(KVPOOL_ESTATE, "retrieve: no staging slot large enough (the placement was made while the path was zero-copy)");
   StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
   settle_landed(L);
-  uint32_t lo[KVPOOL_MAX_DEVICES], hi[KVPOOL_MAX_DEVICES];
   bool hbm_blocks = false;
   for (uint32_t i = 0; i < N; ++i) {
-    if (n_blocks == L.map->K) { lo[i] = 0; hi[i] = L.map->counts[i]; }
-    else slot_range(*L.map, i, first_block, n_blocks, &lo[i], &hi[i]);
     if (hi[i] == lo[i]) continue;
     if (is_hbm(p, i)) { hbm_blocks = true; continue; }  // read in place by the unpack kernel
     rc = wait_slot_free(p, slot, p->io[i]);
@@ -1000,6 +1011,7 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
     total += (span[i] + 255) / 256 * 256;
   }
   if (total > p->slot_bytes || p->slots.empty()) return 1;
+  if (total == 0) return issue_zero_copy_group(c, g);  // every block of the group sits on HBM-type devices: nothing to stage, no slot taken
   StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
   MultiArgs ma{};
   fill_descs(c, g, &ma);
@@ -1013,7 +1025,6 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   cudaStream_t lead = nullptr;
   for (uint32_t i = 0; i < N && !lead; ++i)
     if (span[i]) lead = ios[i];
-  if (!lead && !hbm_blocks) return KVPOOL_OK;
   bool gated = false;
   for (uint32_t b = 0; b < g.n; ++b) {
     LayerState& L = c.pl->layers[c.first + g.q[b]];

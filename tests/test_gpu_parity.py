@@ -650,6 +650,11 @@ def test_hbm_type_pool_devices_alone_and_mixed_with_host_devices(path, kernel):
     g = W.Geometry(n_layers=1, n_kv_heads=1, head_dim=8, block_tokens=1)
     run_parity(_custom(g, 9, [[7, 2, 5]], 6, (4.0, 4.0, 2.0, 2.0, 1.0, 1.0)), path=p, kernel=k, dev_flags=[0, HBM, 0, HBM, 0, HBM])
     run_parity(W.make_workload(3, scale=1 / 8, n_layers=4), path=p, kernel=k, dev_flags=[0, HBM, HBM, 0])
+    # a slow host device next to a fast HBM one, few blocks: counts (0, 8) — nothing to stage, so no copy and no staging
+    # slot is taken whatever the path (a slot recycled without waits could be overwritten under an earlier offload's copy)
+    g = W.Geometry(n_layers=2, n_kv_heads=1, head_dim=64)
+    out = run_parity(_custom(g, 16, [rng.permutation(16)[:8]], 2, (1.0, 50.0)), path=p, kernel=k, dev_flags=[0, HBM])
+    assert out["memcpys"] == 0
 
 
 @pytest.mark.parametrize("kernel", list(KERNELS))
