@@ -73,6 +73,9 @@ def parse_args():
     ap.add_argument("--duplex", action="store_true",
                     help="offload of one request concurrent with retrieve of another (PCIe is full duplex): per-direction and aggregate "
                          "GB/s against simultaneous cudaMemcpyAsync in both directions")
+    ap.add_argument("--pool-create", action="store_true",
+                    help="side mode: time kvpool_create of one pool buffer, default (huge pages faulted in in parallel + cudaHostRegister) "
+                         "vs KVPOOL_DEV_CUDA_HOSTALLOC, and the link bandwidth from each, pass by pass; text table")
     ap.add_argument("--compute-us", type=float, default=0.0, help="--blocked-io: extra calibrated compute per layer (kvpool_spin), microseconds")
     ap.add_argument("--detail", default=None, help="write per-layer latencies and side measurements to this JSON file")
     return ap.parse_args()
@@ -594,6 +597,8 @@ def run_kvpool(args) -> dict:
                    "step": "kvpool_place + offload of every layer + retrieve of every layer; value = retrieve leg"},
         "retrieve_ms_per_step": ret_ms, "offload_ms_per_step": off_ms, "offload_gbps": world * moved / (off_ms * 1e6),
         "place_ms_per_step": statistics.mean(rec["place_ms"]), "verified_bit_exact_round_trip": verified,
+        "pool_create": {"seconds": create_s, "pinned_bytes": int(sum(caps)), "gbps": sum(caps) / create_s / 1e9,
+                        "what": "kvpool_create: huge-page mapping faulted in by up to 16 threads + cudaHostRegister (outside the timed region)"},
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": moved + table_bytes, "d2h_bytes_per_step": d2h_bytes,
                 "what": "retrieve leg by host wall clock: pinned block tables H2D + kvpool_retrieve x layers + D2H of one block per layer + sync",
                 "offload_gbps": world * moved / (statistics.median(e2e_off_s) * 1e9)},
@@ -1057,6 +1062,48 @@ def run_duplex(args) -> None:
     pool.destroy()
 
 
+def run_pool_create(args) -> None:
+    """kvpool_create pins the pool ("at model initialization"; 20 GB of host memory in the paper's setup,
+    PAPER.md:106).  Times the creation of ONE pool buffer of 1, 8 and 32 GiB both ways, then the link from a fresh buffer
+    pass by pass: pages the CPU has just zeroed read ~5 % slow host->GPU until a DMA write has claimed them (every stripe is
+    written by an offload before a retrieve reads it; kvpool_measure_bandwidth does the same before it measures)."""
+    import torch
+    from paper_2606_14779_b200 import binding as kv
+
+    torch.cuda.set_device(0)
+    torch.cuda.init()
+    import ctypes
+    rt = ctypes.CDLL("libcudart.so.12")          # the runtime already in the process; only for the raw passes below
+    rt.cudaMemcpy.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int]
+    scratch = torch.empty(1 << 30, dtype=torch.uint8, device="cuda:0")
+
+    def raw_pass(host_ptr: int, to_gpu: bool) -> float:     # one blocking 1 GiB cudaMemcpy, no warm-up, host clock
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        rc = rt.cudaMemcpy(scratch.data_ptr(), host_ptr, 1 << 30, 1) if to_gpu else rt.cudaMemcpy(host_ptr, scratch.data_ptr(), 1 << 30, 2)
+        assert rc == 0, rc
+        return (1 << 30) / (time.perf_counter() - t0) / 1e9
+
+    flavours = (("default: 2 MiB-aligned mmap + MADV_HUGEPAGE + parallel first touch + cudaHostRegister", 0),
+                ("KVPOOL_DEV_CUDA_HOSTALLOC: cudaHostAlloc", kv.DEV_CUDA_HOSTALLOC))
+    print(f"kvpool_create of one pool buffer ({len(os.sched_getaffinity(0))} host cores)")
+    for gib in (1, 8, 32):
+        for name, flags in flavours:
+            t0 = time.perf_counter()
+            pool = kv.KvPool([1.0], [gib << 30], n_layers=1, n_kv_heads=4, head_dim=128, dev_flags=[flags])
+            dt = time.perf_counter() - t0
+            line = f"  {gib:3d} GiB  {dt:6.2f} s  {gib * 2**30 / dt / 1e9:6.2f} GB/s  {name}"
+            if gib == 1:
+                host = pool.device_info(0)["host_base"]
+                h = [raw_pass(host, True) for _ in range(8)]
+                d = [raw_pass(host, False) for _ in range(2)]
+                h2 = [raw_pass(host, True) for _ in range(3)]
+                line += ("\n           host->GPU passes over the fresh buffer " + " ".join(f"{x:.1f}" for x in h) +
+                         "; GPU->host " + " ".join(f"{x:.1f}" for x in d) + "; host->GPU again " + " ".join(f"{x:.1f}" for x in h2) + " GB/s")
+            print(line, flush=True)
+            pool.destroy()
+
+
 def run_blocked_io(args) -> None:
     """Blocked I/O time = time during which only KV retrieval proceeds, with no overlapping GPU computation.
     Consumer stand-in per layer = kvpool_checksum over the layer's retrieved blocks (reads K_l*P bytes through the block
@@ -1192,6 +1239,9 @@ def main():
         return
     if args.duplex:
         run_duplex(args)
+        return
+    if args.pool_create:
+        run_pool_create(args)
         return
     out = run_kvpool(args)
     if out is None:

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libkvpool.so")
 
 MAX_DEVICES = 32
 OK, EINVAL, ENOMEM, ECUDA, ENUMA, ESTATE, ENOENT = 0, -1, -2, -3, -4, -5, -6
-DEV_WRITE_COMBINED, DEV_NUMA_STRICT, DEV_HBM = 1, 2, 4
+DEV_WRITE_COMBINED, DEV_NUMA_STRICT, DEV_HBM, DEV_CUDA_HOSTALLOC = 1, 2, 4, 8
 TYPE_MEM, TYPE_SSD, TYPE_HBM = 0, 1, 2
 NUMA_AUTO = -2
 PATH_AUTO, PATH_STAGED, PATH_ZEROCOPY = 0, 1, 2

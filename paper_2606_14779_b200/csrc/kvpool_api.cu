@@ -415,7 +415,7 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
   for (uint32_t i = 0; i < n_devs; ++i) {
     bw[i] = devs[i].bandwidth_gbps;
     if (devs[i].capacity_bytes == 0) return fail(KVPOOL_EINVAL, "create: device %u has zero capacity", i);
-    if (devs[i].flags & ~(KVPOOL_DEV_WRITE_COMBINED | KVPOOL_DEV_NUMA_STRICT | KVPOOL_DEV_HBM)) return fail(KVPOOL_EINVAL, "create: device %u unknown flags", i);
+    if (devs[i].flags & ~(KVPOOL_DEV_WRITE_COMBINED | KVPOOL_DEV_NUMA_STRICT | KVPOOL_DEV_HBM | KVPOOL_DEV_CUDA_HOSTALLOC)) return fail(KVPOOL_EINVAL, "create: device %u unknown flags", i);
     if ((devs[i].flags & KVPOOL_DEV_HBM) && (devs[i].flags & ~KVPOOL_DEV_HBM)) return fail(KVPOOL_EINVAL, "create: device %u: KVPOOL_DEV_HBM excludes the host-memory flags", i);
     if (devs[i].numa_node < KVPOOL_NUMA_AUTO) return fail(KVPOOL_EINVAL, "create: device %u: numa_node %d", i, devs[i].numa_node);
     if (devs[i].reserved != 0) return fail(KVPOOL_EINVAL, "create: device %u: reserved must be 0", i);
@@ -457,7 +457,7 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     const int rc = hbm ? device_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes, devs[i].gpu < 0 ? cuda_device : devs[i].gpu, cuda_device, &err)
                        : host_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes,
                                            devs[i].numa_node == KVPOOL_NUMA_AUTO ? gpu_numa_node(cuda_device) : devs[i].numa_node, devs[i].flags & KVPOOL_DEV_WRITE_COMBINED,
-                                           devs[i].flags & KVPOOL_DEV_NUMA_STRICT, &err);
+                                           devs[i].flags & KVPOOL_DEV_NUMA_STRICT, devs[i].flags & KVPOOL_DEV_CUDA_HOSTALLOC, &err);
     if (rc == KVPOOL_OK && hbm) p->hbm_mask |= 1u << i;
     if (rc != KVPOOL_OK) {
       cleanup();
@@ -533,6 +533,13 @@ int kvpool_measure_bandwidth(kvpool_t* p, uint32_t dev, int direction, uint64_t 
   std::vector<float> ms(iters);
   cudaStream_t s = direction == 0 ? p->io[dev] : p->io_out[dev];
   int rc = KVPOOL_OK;
+  if (direction == 0 && !is_hbm(p, dev)) {
+    // Pages the CPU has just zeroed sit partly in its caches; host->GPU DMA reads of such lines run 5 % slow until a DMA
+    // write has claimed them (measured: 52 -> 55.6 GB/s after one pass).  Stripes are always written by an offload
+    // before a retrieve reads them, so that is the state to measure: write the region once (no placement is live).
+    CU(cudaMemcpyAsync(pool_bytes(p, dev), scratch, bytes, cudaMemcpyDefault, s));
+    p->n_memcpys++;
+  }
   for (uint32_t it = 0; it < iters + 1 && rc == KVPOOL_OK; ++it) {  // first pass is a warm-up
     cudaEventRecord(e0, s);
     cudaError_t e = direction == 0 ? cudaMemcpyAsync(scratch, pool_bytes(p, dev), bytes, cudaMemcpyDefault, s)

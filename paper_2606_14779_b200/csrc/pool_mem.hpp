@@ -14,11 +14,15 @@ struct HostBuffer {
   int numa_requested = -1;
   int numa_actual = -1;      // node of the first page after touching, -1 if it cannot be queried
   bool registered = false;   // true: mmap + cudaHostRegister; false: cudaHostAlloc
+  void* map_base = nullptr;  // registered: the mapping that holds `host` (2 MiB-aligned inside it) and its length
+  uint64_t map_bytes = 0;
 };
 
 // Returns 0 or a KVPOOL_E* code and fills err.  strict_numa: fail instead of falling back when the
-// pages cannot be bound to numa_node.
-int host_buffer_alloc(HostBuffer* hb, uint64_t bytes, int numa_node, bool write_combined, bool strict_numa, std::string* err);
+// pages cannot be bound to numa_node.  cuda_hostalloc: take the buffer from cudaHostAlloc instead of faulting huge
+// pages in in parallel and registering them (kept for comparison; a NUMA request still goes through mbind + register).
+int host_buffer_alloc(HostBuffer* hb, uint64_t bytes, int numa_node, bool write_combined, bool strict_numa, bool cuda_hostalloc,
+                      std::string* err);
 // HBM-type buffer: cudaMalloc on `gpu`, peer access enabled from `pool_gpu` when they differ.  The current device is
 // `pool_gpu` on entry and on return.
 int device_buffer_alloc(HostBuffer* hb, uint64_t bytes, int gpu, int pool_gpu, std::string* err);

@@ -484,7 +484,8 @@ def test_retrieve_layers_signal_feeds_a_consumer_on_another_stream(path):
 
 def test_numa_bound_registered_and_write_combined_pool_buffers():
     """Pool-device flavours: mmap + mbind(node 0) + cudaHostRegister, a node that does not exist (falls back unless
-    KVPOOL_DEV_NUMA_STRICT, then ENUMA), and write-combined buffers — all bit-exact through both paths."""
+    KVPOOL_DEV_NUMA_STRICT, then ENUMA), write-combined buffers, and cudaHostAlloc buffers next to the default ones
+    (2 MiB-aligned mapping faulted in in parallel, then cudaHostRegister) — all bit-exact through both paths."""
     g = W.Geometry(n_layers=2, n_kv_heads=2, head_dim=64)
     rng = np.random.default_rng(29)
     wl = _custom(g, 300, [rng.permutation(300)[:256]], 3, (2.0, 1.0, 1.0))
@@ -496,7 +497,8 @@ def test_numa_bound_registered_and_write_combined_pool_buffers():
         kv.KvPool([2.0, 1.0, 1.0], cap, n_layers=2, n_kv_heads=2, head_dim=64, numa_nodes=[0, -3, 0])
     assert e.value.code == kv.EINVAL
     auto = [kv.NUMA_AUTO] * 3               # the node the GPU hangs off, read from sysfs; no preference where sysfs does not say
-    for numa, flags in (([0, 0, -1], [kv.DEV_NUMA_STRICT, 0, 0]), ([0, 977, -1], [0, 0, 0]), (None, [kv.DEV_WRITE_COMBINED] * 3), (auto, [0, 0, 0])):
+    for numa, flags in (([0, 0, -1], [kv.DEV_NUMA_STRICT, 0, 0]), ([0, 977, -1], [0, 0, 0]), (None, [kv.DEV_WRITE_COMBINED] * 3), (auto, [0, 0, 0]),
+                        (None, [kv.DEV_CUDA_HOSTALLOC, 0, kv.DEV_CUDA_HOSTALLOC])):   # cudaHostAlloc next to the default (huge pages + register)
         pool = kv.KvPool([2.0, 1.0, 1.0], cap, n_layers=2, n_kv_heads=2, head_dim=64, numa_nodes=numa, dev_flags=flags)
         try:
             if numa is not None and numa is not auto:

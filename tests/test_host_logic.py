@@ -124,7 +124,7 @@ def test_create_argument_validation_precedes_cuda():
     with pytest.raises(kv.KvPoolError) as e:
         kv.KvPool([1.0], [0], n_layers=1, n_kv_heads=1, head_dim=64)
     assert e.value.code == kv.EINVAL
-    for flags in (8, kv.DEV_HBM | kv.DEV_WRITE_COMBINED, kv.DEV_HBM | kv.DEV_NUMA_STRICT):      # unknown flag; HBM excludes host flags
+    for flags in (16, kv.DEV_HBM | kv.DEV_CUDA_HOSTALLOC, kv.DEV_HBM | kv.DEV_WRITE_COMBINED, kv.DEV_HBM | kv.DEV_NUMA_STRICT):      # unknown flag; HBM excludes host flags
         with pytest.raises(kv.KvPoolError) as e:
             kv.KvPool([1.0], [1 << 20], n_layers=1, n_kv_heads=1, head_dim=64, dev_flags=[flags])
         assert e.value.code == kv.EINVAL
