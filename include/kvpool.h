@@ -18,7 +18,11 @@
  *     P = 2*kvb bytes with kvb = block_tokens*n_kv_heads*head_dim*elem_bytes (R6).
  *   - There is no CPU fallback: without a CUDA device kvpool_create fails with KVPOOL_ECUDA.  The
  *     kvpool_plan_* functions are pure host arithmetic and work anywhere.
- *   - A pool handle is not thread-safe; use it from one host thread (any number of CUDA streams).
+ *   - A pool handle may be used from several host threads at once (one per request, say), each with
+ *     its own CUDA streams: every call that touches pool state takes the pool's lock, and calls only
+ *     enqueue work, so the lock is held for microseconds (kvpool_release, kvpool_synchronize and
+ *     kvpool_measure_bandwidth hold it while they wait).  A placement is used by one thread at a time;
+ *     kvpool_destroy must not race with any other call.
  */
 #ifndef KVPOOL_H
 #define KVPOOL_H

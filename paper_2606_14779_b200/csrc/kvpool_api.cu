@@ -54,6 +54,13 @@ struct DeviceGuard {  // make the pool's GPU current for the duration of a call
   }
 };
 
+// Serialises host threads on one pool (null-tolerant so that it can precede the argument checks; recursive because the
+// batched calls go through the per-layer entry points).
+struct PoolLock {
+  std::unique_lock<std::recursive_mutex> l;
+  explicit PoolLock(kvpool* p);
+};
+
 // Dense per-layer GLT columns shared by all layers of a placement that move the same number of blocks.
 struct LayerMap {
   uint64_t K = 0;
@@ -151,10 +158,14 @@ struct kvpool {
   std::vector<cudaEvent_t> prof_free;  // timing events ready for reuse
   unsigned long long* span_arena = nullptr;  // device: kSpanCap x {min start, max end} in %globaltimer ns, written by the kernels
   uint32_t span_cursor = 0;
-  std::mutex mu;
+  std::recursive_mutex mu;  // every entry point that touches pool state holds it: calls only enqueue work, so the lock is short
 };
 
 namespace {
+
+PoolLock::PoolLock(kvpool* p) {
+  if (p) l = std::unique_lock<std::recursive_mutex>(p->mu);
+}
 
 void default_tuning(kvpool* p) {
   p->tune.kernel = KVPOOL_KERNEL_VEC16;
@@ -510,6 +521,7 @@ int kvpool_destroy(kvpool_t* p) {
 }
 
 int kvpool_set_bandwidth(kvpool_t* p, const double* bw) {
+  PoolLock lock__(p);
   if (!p || !bw) return fail(KVPOOL_EINVAL, "set_bandwidth: null argument");
   if (!p->live.empty()) return fail(KVPOOL_ESTATE, "set_bandwidth: %zu placements are live", p->live.size());
   std::vector<uint64_t> w(p->n);
@@ -520,6 +532,7 @@ int kvpool_set_bandwidth(kvpool_t* p, const double* bw) {
 }
 
 int kvpool_measure_bandwidth(kvpool_t* p, uint32_t dev, int direction, uint64_t bytes, uint32_t iters, double* gbps_out) {
+  PoolLock lock__(p);
   if (!p || !gbps_out || dev >= p->n || bytes == 0 || iters == 0 || (direction != 0 && direction != 1))
     return fail(KVPOOL_EINVAL, "measure_bandwidth: bad arguments");
   if (bytes > p->bufs[dev].bytes) return fail(KVPOOL_EINVAL, "measure_bandwidth: %llu bytes exceed the pool buffer", (unsigned long long)bytes);
@@ -560,12 +573,14 @@ int kvpool_measure_bandwidth(kvpool_t* p, uint32_t dev, int direction, uint64_t 
 }
 
 int kvpool_set_path(kvpool_t* p, int path) {
+  PoolLock lock__(p);
   if (!p || path < KVPOOL_PATH_AUTO || path > KVPOOL_PATH_ZEROCOPY) return fail(KVPOOL_EINVAL, "set_path: bad arguments");
   p->path = path;
   return KVPOOL_OK;
 }
 
 int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
+  PoolLock lock__(p);
   if (!p || !t) return fail(KVPOOL_EINVAL, "set_tuning: null argument");
   if (t->kernel > KVPOOL_KERNEL_BULK || t->link_kernel > KVPOOL_KERNEL_BULK)
     return fail(KVPOOL_EINVAL, "set_tuning: unknown kernel %u / link_kernel %u", t->kernel, t->link_kernel);
@@ -605,6 +620,7 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
 }
 
 int kvpool_reserve_staging(kvpool_t* p, uint64_t bytes) {
+  PoolLock lock__(p);
   if (!p) return fail(KVPOOL_EINVAL, "reserve_staging: null pool");
   if (all_hbm(p)) return KVPOOL_OK;  // nothing is ever staged
   DeviceGuard guard(p->cuda_device);
@@ -620,7 +636,7 @@ int kvpool_get_tuning(const kvpool_t* p, kvpool_tuning* t_out) {
 int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement_t** out) {
   if (!p || !blocks_per_layer || !out) return fail(KVPOOL_EINVAL, "place: null argument");
   *out = nullptr;
-  std::lock_guard<std::mutex> lock(p->mu);
+  std::lock_guard<std::recursive_mutex> lock(p->mu);
   DeviceGuard guard(p->cuda_device);
   const uint32_t L = p->geom.n_layers, N = p->n;
   std::unique_ptr<kvpool_placement> pl(new kvpool_placement);
@@ -748,7 +764,7 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
 
 int kvpool_release(kvpool_t* p, kvpool_placement_t* pl) {
   if (!p || !pl) return fail(KVPOOL_EINVAL, "release: null argument");
-  std::lock_guard<std::mutex> lock(p->mu);
+  std::lock_guard<std::recursive_mutex> lock(p->mu);
   auto it = std::find(p->live.begin(), p->live.end(), pl);
   if (it == p->live.end()) return fail(KVPOOL_EINVAL, "release: placement does not belong to this pool");
   DeviceGuard guard(p->cuda_device);
@@ -768,6 +784,7 @@ extern "C" {
 
 int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
                    const int32_t* table, void* cuda_stream) {
+  PoolLock lock__(p);
   int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
   if (rc != KVPOOL_OK) return rc;
   LayerState& L = pl->layers[layer];
@@ -842,6 +859,7 @@ static void slot_range(const LayerMap& m, uint32_t i, uint32_t first, uint32_t n
 
 int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks, void* k_base,
                           void* v_base, uint64_t stride, const int32_t* table, void* cuda_stream) {
+  PoolLock lock__(p);
   int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
   if (rc != KVPOOL_OK) return rc;
   LayerState& L = pl->layers[layer];
@@ -912,6 +930,7 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
 
 int kvpool_retrieve(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
                     const int32_t* table, void* cuda_stream) {
+  PoolLock lock__(p);
   if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "retrieve: bad pool or placement");
   if (layer >= p->geom.n_layers) return fail(KVPOOL_EINVAL, "layer %u out of range (n_layers %u)", layer, p->geom.n_layers);
   return kvpool_retrieve_range(p, pl, layer, 0, static_cast<uint32_t>(pl->layers[layer].map->K), k_base, v_base, stride, table, cuda_stream);
@@ -1125,6 +1144,7 @@ int issue_group_work(const BatchCall& c, const LayerGroup& g) {
 static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32_t first, uint32_t n, const void* const* k_bases,
                           const void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream,
                           void* const* ready = nullptr) {
+  PoolLock lock__(p);
   if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "layers: bad pool or placement");
   if (static_cast<uint64_t>(first) + n > p->geom.n_layers) return fail(KVPOOL_EINVAL, "layers [%u, %u) out of range (n_layers %u)", first, first + n, p->geom.n_layers);
   if (n == 0) return KVPOOL_OK;
@@ -1186,6 +1206,7 @@ int kvpool_retrieve_layers_signal(kvpool_t* p, kvpool_placement_t* pl, uint32_t 
 // Baseline for comparison: 2*K_l individual cudaMemcpyAsync calls per layer, no kernel.
 static int naive_layer(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, bool pack, const void* k_base, const void* v_base, uint64_t stride,
                        const int32_t* table_host, void* cuda_stream) {
+  PoolLock lock__(p);
   int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table_host);
   if (rc != KVPOOL_OK) return rc;
   LayerState& L = pl->layers[layer];
@@ -1226,6 +1247,7 @@ int kvpool_retrieve_naive(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, v
 }
 
 int kvpool_wait_offloads(kvpool_t* p, kvpool_placement_t* pl, void* cuda_stream) {
+  PoolLock lock__(p);
   if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "wait_offloads: bad arguments");
   DeviceGuard guard(p->cuda_device);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
@@ -1235,6 +1257,7 @@ int kvpool_wait_offloads(kvpool_t* p, kvpool_placement_t* pl, void* cuda_stream)
 }
 
 int kvpool_synchronize(kvpool_t* p) {
+  PoolLock lock__(p);
   if (!p) return fail(KVPOOL_EINVAL, "synchronize: null pool");
   DeviceGuard guard(p->cuda_device);
   const int rc = sync_pool_streams(p);
@@ -1248,6 +1271,7 @@ int kvpool_synchronize(kvpool_t* p) {
 
 int kvpool_pack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
                 const int32_t* table, void* stage_dev, void* cuda_stream) {
+  PoolLock lock__(p);
   int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
   if (rc != KVPOOL_OK) return rc;
   LayerState& L = pl->layers[layer];
@@ -1261,6 +1285,7 @@ int kvpool_pack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void*
 
 int kvpool_unpack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
                   const int32_t* table, const void* stage_dev, void* cuda_stream) {
+  PoolLock lock__(p);
   int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
   if (rc != KVPOOL_OK) return rc;
   LayerState& L = pl->layers[layer];
@@ -1275,6 +1300,7 @@ int kvpool_unpack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_b
 
 int kvpool_checksum(kvpool_t* p, const void* k_base, const void* v_base, uint64_t stride, const int32_t* table, uint32_t n_blocks,
                     uint64_t* sum_dev, void* cuda_stream) {
+  PoolLock lock__(p);
   if (!p || !sum_dev) return fail(KVPOOL_EINVAL, "checksum: null argument");
   if (n_blocks == 0) return KVPOOL_OK;
   if (!k_base || !v_base || !table) return fail(KVPOOL_EINVAL, "checksum: null k_base / v_base / block table");
@@ -1290,6 +1316,7 @@ int kvpool_checksum(kvpool_t* p, const void* k_base, const void* v_base, uint64_
 }
 
 int kvpool_spin(kvpool_t* p, uint64_t ns, void* cuda_stream) {
+  PoolLock lock__(p);
   if (!p) return fail(KVPOOL_EINVAL, "spin: null pool");
   if (ns > 10ull * 1000 * 1000 * 1000) return fail(KVPOOL_EINVAL, "spin: more than 10 s");
   DeviceGuard guard(p->cuda_device);
@@ -1352,6 +1379,7 @@ int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, vo
 }
 
 int kvpool_stripe_read(kvpool_t* p, const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, void* dst_host, uint64_t nbytes) {
+  PoolLock lock__(p);
   if (!p || !pl || pl->pool != p || !is_live(p, pl) || layer >= pl->layers.size() || dev >= p->n) return fail(KVPOOL_EINVAL, "stripe_read: bad arguments");
   const LayerState& L = pl->layers[layer];
   const uint64_t bytes = static_cast<uint64_t>(L.map->counts[dev]) * p->payload;
@@ -1382,7 +1410,7 @@ int kvpool_glt_bind(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const u
   const uint64_t K = pl->layers[layer].map->K;
   if (K == 0) return KVPOOL_OK;
   if (!ids) return fail(KVPOOL_EINVAL, "glt_bind: null ids");
-  std::lock_guard<std::mutex> lock(p->mu);
+  std::lock_guard<std::recursive_mutex> lock(p->mu);
   std::unordered_map<uint64_t, GltRef, GltHash> fresh;
   fresh.reserve(K);
   for (uint64_t j = 0; j < K; ++j) {
@@ -1398,7 +1426,7 @@ int kvpool_glt_bind(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const u
 int kvpool_glt_find(kvpool_t* p, uint64_t id, uint64_t* key, uint32_t* device_id, uint32_t* type, void** location, kvpool_placement_t** pl,
                     uint32_t* layer, uint32_t* block) {
   if (!p) return fail(KVPOOL_EINVAL, "glt_find: null pool");
-  std::lock_guard<std::mutex> lock(p->mu);
+  std::lock_guard<std::recursive_mutex> lock(p->mu);
   const auto it = p->glt.find(id);
   if (it == p->glt.end()) return fail(KVPOOL_ENOENT, "glt_find: identifier 0x%llx is not in the table", (unsigned long long)id);
   const GltRef& r = it->second;
@@ -1418,6 +1446,7 @@ int kvpool_layer_map(const kvpool_placement_t* pl, uint32_t layer, uint8_t* dev_
 }
 
 int kvpool_set_profiling(kvpool_t* p, int enabled) {
+  PoolLock lock__(p);
   if (!p) return fail(KVPOOL_EINVAL, "set_profiling: null pool");
   if (enabled && !p->span_arena) {
     DeviceGuard guard(p->cuda_device);
@@ -1430,6 +1459,7 @@ int kvpool_set_profiling(kvpool_t* p, int enabled) {
 
 int kvpool_profile_read_clock(kvpool_t* p, int kind, double* total_ms, double* device_ms, uint64_t* launches, uint64_t* device_launches,
                               uint64_t* bytes) {
+  PoolLock lock__(p);
   if (!p || kind < 0 || kind > 3) return fail(KVPOOL_EINVAL, "profile_read: bad arguments");
   DeviceGuard guard(p->cuda_device);
   double ms_sum = 0, dev_ms_sum = 0;

@@ -772,3 +772,72 @@ def test_zero_copy_retrieve_is_capturable_into_a_cuda_graph(kernel):
         pl.release()
     finally:
         pool.destroy()
+
+
+def test_host_threads_share_one_pool():
+    """Four host threads, one request each (config 5 scaled: interleaved block tables over one shared paged pool), drive one
+    pool handle concurrently — place, offload every layer, retrieve every layer, release, three times over, each on its
+    own stream.  ctypes drops the GIL inside the library, so the calls really interleave; staging slots, events, the table
+    arena and the allocators are shared.  Every request's stripes and retrieved blocks must equal the oracle's."""
+    import threading
+    wl = W.make_workload(5, scale=1 / 16, n_layers=4)
+    g, dev = wl.geom, torch.device("cuda:0")
+    R, L, elems = len(wl.requests), wl.geom.n_layers, wl.geom.kvb // 2
+    bw = list(wl.default_weights())
+    pool = make_pool(wl, bw)
+    src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+    src_cpu = [W.kv_layer_numpy(wl, l) for l in range(L)]
+    dst = [W.poison_torch((2, wl.nphys, elems), dev) for l in range(L)]      # requests own disjoint physical blocks
+    torch.cuda.synchronize()
+    errors, stripes_ok = [], [0] * R
+    barrier = threading.Barrier(R)
+
+    def worker(r: int) -> None:
+        try:
+            torch.cuda.set_device(dev)
+            s = torch.cuda.Stream(device=dev)
+            bpl = wl.blocks_per_layer(r)
+            opl = oracle.place(bw, bpl)
+            tables_np = [np.ascontiguousarray(wl.layer_table(r, l)) for l in range(L)]
+            with torch.cuda.stream(s):
+                tables = [torch.from_numpy(t).to(dev) for t in tables_np]
+            s.synchronize()
+            barrier.wait()
+            for rep in range(3):
+                pool.set_path((kv.PATH_STAGED, kv.PATH_AUTO, kv.PATH_STAGED)[rep] if r % 2 == 0 else kv.PATH_STAGED)
+                pl = pool.place(bpl)
+                check_placement(pl, opl)
+                for l in range(L):
+                    pool.offload(pl, l, src[l][0], src[l][1], g.kvb, tables[l], s)
+                pool.wait_offloads(pl, s)
+                s.synchronize()
+                for l in range(L):
+                    want = oracle.offload_layer(src_cpu[l], tables_np[l], opl[l])
+                    for i in range(pool.n_devices):
+                        assert np.array_equal(pl.stripe(l, i), want[i]), (r, rep, l, i)
+                        stripes_ok[r] += 1
+                for l in range(L):
+                    pool.retrieve(pl, l, dst[l][0], dst[l][1], g.kvb, tables[l], s)
+                s.synchronize()
+                pl.release()
+        except BaseException as e:        # noqa: BLE001 - reported by the main thread
+            errors.append((r, repr(e)))
+            barrier.abort()
+
+    threads = [threading.Thread(target=worker, args=(r,)) for r in range(R)]
+    try:
+        for t in threads:
+            t.start()
+        for t in threads:
+            t.join()
+        assert not errors, errors
+        assert all(n == 3 * L * pool.n_devices for n in stripes_ok)
+        torch.cuda.synchronize()
+        for l in range(L):                # every request's blocks came back; everything else is still poison
+            want = W.poison_numpy((2, wl.nphys, elems))
+            for r in range(R):
+                t = wl.layer_table(r, l)
+                want[:, t] = src_cpu[l][:, t]
+            assert np.array_equal(dst[l].cpu().numpy().view(np.uint16), want), l
+    finally:
+        pool.destroy()
