@@ -73,6 +73,8 @@ def parse_args():
     ap.add_argument("--duplex", action="store_true",
                     help="offload of one request concurrent with retrieve of another (PCIe is full duplex): per-direction and aggregate "
                          "GB/s against simultaneous cudaMemcpyAsync in both directions")
+    ap.add_argument("--hostalloc", action="store_true", help="pool buffers from cudaHostAlloc (KVPOOL_DEV_CUDA_HOSTALLOC) instead of the default "
+                    "huge-page mapping + cudaHostRegister; main run and --duplex")
     ap.add_argument("--pool-create", action="store_true",
                     help="side mode: time kvpool_create of one pool buffer, default (huge pages faulted in in parallel + cudaHostRegister) "
                          "vs KVPOOL_DEV_CUDA_HOSTALLOC, and the link bandwidth from each, pass by pass; text table")
@@ -264,7 +266,8 @@ def run_kvpool(args) -> dict:
         numa = [kv.NUMA_AUTO] * N       # several ranks on one host: each rank's buffers on the NUMA node its own GPU hangs off
     t0 = time.perf_counter()
     pool = kv.KvPool(base_w, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, block_tokens=g.block_tokens,
-                     elem_bytes=g.elem_bytes, cuda_device=local, numa_nodes=numa)
+                     elem_bytes=g.elem_bytes, cuda_device=local, numa_nodes=numa,
+                     dev_flags=[kv.DEV_CUDA_HOSTALLOC] * N if args.hostalloc else None)
     create_s = time.perf_counter() - t0
     weights_kind = args.weights
     if args.weights == "measured" or (args.weights == "config" and wl.weights is None):
@@ -992,7 +995,8 @@ def run_duplex(args) -> None:
     bw = list(wl.default_weights())
     share = np.array(bw) / np.sum(bw)
     caps = [int(2 * moved * sh * 1.25) + 2 * (L + 4) * (g.payload + 4096) for sh in share]
-    pool = kv.KvPool(bw, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim)
+    pool = kv.KvPool(bw, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim,
+                     dev_flags=[kv.DEV_CUDA_HOSTALLOC] * len(bw) if args.hostalloc else None)
     src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
     dst = [W.poison_torch((2, wl.nphys, elems), dev) for l in range(L)]
     tables = [torch.from_numpy(np.ascontiguousarray(wl.layer_table(0, l))).to(dev) for l in range(L)]
@@ -1002,6 +1006,7 @@ def run_duplex(args) -> None:
     # duplex peak of the link: simultaneous H2D and D2H copies of 1 GiB each
     hd, dd = torch.empty(1 << 30, dtype=torch.uint8).pin_memory(), torch.empty(1 << 30, dtype=torch.uint8, device=dev)
     hu, du = torch.empty(1 << 30, dtype=torch.uint8).pin_memory(), torch.empty(1 << 30, dtype=torch.uint8, device=dev)
+    hd.copy_(dd)          # freshly zeroed host pages read slow over the link until a DMA write has claimed them
     peak = []
     for it in range(4):
         torch.cuda.synchronize()
@@ -1020,6 +1025,8 @@ def run_duplex(args) -> None:
           f"({moved / 2**20:.0f} MiB) is retrieved; median of 3")
     print(f"# simultaneous cudaMemcpyAsync, 1 GiB each way: H2D {peak_h2d:.1f} GB/s + D2H {peak_d2h:.1f} GB/s = {peak_h2d + peak_d2h:.1f} GB/s")
     print(f"{'path/CTAs':12s} {'offload A GB/s':>15s} {'retrieve B GB/s':>16s} {'aggregate GB/s (wall)':>22s} {'x duplex peak':>14s}")
+    if args.stage_slots:
+        pool.set_tuning(stage_slots=args.stage_slots)
     for pname, path, ctas in (("staged", kv.PATH_STAGED, 0), ("zerocopy", kv.PATH_ZEROCOPY, args.link_ctas or 4),
                               ("zerocopy", kv.PATH_ZEROCOPY, 4 * (args.link_ctas or 4))):
         pool.set_path(path)
