@@ -6,6 +6,7 @@
 #include <dirent.h>
 #include <errno.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 #include <sys/mman.h>
 #include <sys/syscall.h>
@@ -78,9 +79,42 @@ static void first_touch(char* m, uint64_t bytes) {
   for (auto& t : pool) t.join();
 }
 
+// Host memory a new buffer can still take: MemAvailable, capped by the cgroup's limit where there is one.  Faulting in
+// more than that would wake the OOM killer instead of failing the call, so registered_alloc refuses first.
+static uint64_t read_u64_after(const char* path, const char* key) {
+  FILE* f = fopen(path, "r");
+  if (!f) return ~0ull;
+  char line[256];
+  uint64_t v = ~0ull;
+  while (fgets(line, sizeof(line), f)) {
+    if (key) {
+      if (strncmp(line, key, strlen(key)) == 0) { v = strtoull(line + strlen(key), nullptr, 10); break; }
+    } else {
+      if (line[0] >= '0' && line[0] <= '9') v = strtoull(line, nullptr, 10);  // "max" stays ~0
+      break;
+    }
+  }
+  fclose(f);
+  return v;
+}
+
+uint64_t available_host_bytes() {
+  uint64_t avail = read_u64_after("/proc/meminfo", "MemAvailable:");
+  if (avail != ~0ull) avail *= 1024;  // kB
+  const uint64_t cg_max = read_u64_after("/sys/fs/cgroup/memory.max", nullptr);
+  const uint64_t cg_cur = read_u64_after("/sys/fs/cgroup/memory.current", nullptr);
+  if (cg_max != ~0ull && cg_cur != ~0ull) avail = std::min(avail, cg_max > cg_cur ? cg_max - cg_cur : 0);
+  return avail;
+}
+
 // mmap (2 MiB aligned, MADV_HUGEPAGE) + optional mbind + parallel first touch + cudaHostRegister.  Returns KVPOOL_OK,
 // or a code with *err set and nothing left allocated.
 static int registered_alloc(HostBuffer* hb, uint64_t bytes, int bind_node, bool strict_numa, std::string* err) {
+  const uint64_t avail = available_host_bytes();
+  if (avail != ~0ull && bytes > avail) {
+    *err = "host memory: " + std::to_string(bytes) + " bytes wanted, " + std::to_string(avail) + " available";
+    return KVPOOL_ENOMEM;
+  }
   const uint64_t span = bytes + kHugePage;
   void* raw = mmap(nullptr, span, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS | MAP_NORESERVE, -1, 0);
   if (raw == MAP_FAILED) { *err = std::string("mmap: ") + strerror(errno); return KVPOOL_ENOMEM; }
@@ -127,7 +161,7 @@ int host_buffer_alloc(HostBuffer* hb, uint64_t bytes, int numa_node, bool write_
   int rc = KVPOOL_ECUDA;
   if (!write_combined && !(cuda_hostalloc && !want_bind)) {
     rc = registered_alloc(hb, bytes, want_bind ? numa_node : -1, strict_numa, err);
-    if (rc == KVPOOL_ENUMA) return rc;  // strict binding refused; anything else falls back to cudaHostAlloc (first-touch placement)
+    if (rc == KVPOOL_ENUMA || rc == KVPOOL_ENOMEM) return rc;  // strict binding refused / no room; a refused registration falls back to cudaHostAlloc
   }
   if (rc != KVPOOL_OK) {
     unsigned flags = cudaHostAllocMapped | cudaHostAllocPortable | (write_combined ? cudaHostAllocWriteCombined : 0);

@@ -28,6 +28,7 @@ int host_buffer_alloc(HostBuffer* hb, uint64_t bytes, int numa_node, bool write_
 int device_buffer_alloc(HostBuffer* hb, uint64_t bytes, int gpu, int pool_gpu, std::string* err);
 void host_buffer_free(HostBuffer* hb);
 int numa_node_count();
+uint64_t available_host_bytes();  // MemAvailable capped by the cgroup limit; ~0 when unknown
 int gpu_numa_node(int cuda_device);  // -1 when sysfs does not say
 
 }  // namespace kvp

@@ -496,6 +496,9 @@ def test_numa_bound_registered_and_write_combined_pool_buffers():
     with pytest.raises(kv.KvPoolError) as e:
         kv.KvPool([2.0, 1.0, 1.0], cap, n_layers=2, n_kv_heads=2, head_dim=64, numa_nodes=[0, -3, 0])
     assert e.value.code == kv.EINVAL
+    with pytest.raises(kv.KvPoolError) as e:   # more than the host has: refused before a page is touched, not left to the OOM killer
+        kv.KvPool([2.0, 1.0, 1.0], [8 << 20, 1 << 46, 8 << 20], n_layers=2, n_kv_heads=2, head_dim=64)
+    assert e.value.code == kv.ENOMEM and "available" in str(e.value)
     auto = [kv.NUMA_AUTO] * 3               # the node the GPU hangs off, read from sysfs; no preference where sysfs does not say
     for numa, flags in (([0, 0, -1], [kv.DEV_NUMA_STRICT, 0, 0]), ([0, 977, -1], [0, 0, 0]), (None, [kv.DEV_WRITE_COMBINED] * 3), (auto, [0, 0, 0]),
                         (None, [kv.DEV_CUDA_HOSTALLOC, 0, kv.DEV_CUDA_HOSTALLOC])):   # cudaHostAlloc next to the default (huge pages + register)
