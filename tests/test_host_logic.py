@@ -160,3 +160,14 @@ def test_plain_c_client_compiles_against_header_and_runs(tmp_path):
     assert out[2].startswith('error "plan_weights') and out[3].startswith("kvpool")
     import ctypes                                              # the ctypes structs of the binding have the header's C layout
     assert out[4] == f"sizeof {ctypes.sizeof(kv.DeviceDesc)} {ctypes.sizeof(kv.Geometry)} {ctypes.sizeof(kv.Tuning)}"
+
+
+def test_stripe_allocator_against_a_page_bitmap_model(tmp_path):
+    """a4: the first-fit, coalescing allocator that hands placements their regions (csrc/placement.cpp, plain C++) against a
+    bitmap model on random alloc/free sequences — aligned, disjoint, lowest fitting gap, exact accounting, full coalescing."""
+    import subprocess
+    exe = str(tmp_path / "stripe_alloc_check")
+    subprocess.run(["g++", "-std=c++17", "-O1", "-Wall", "-Wextra", "-Werror", os.path.join(ROOT, "tests", "stripe_alloc_check.cpp"),
+                    os.path.join(ROOT, "paper_2606_14779_b200", "csrc", "placement.cpp"), "-o", exe], check=True)
+    out = subprocess.run([exe], capture_output=True, text=True)
+    assert out.returncode == 0 and out.stdout.strip() == "stripe allocator ok", out.stdout
