@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--link-ctas", type=int, default=0)
     ap.add_argument("--hbm-ctas", type=int, default=0)
     ap.add_argument("--stage-slots", type=int, default=0)
+    ap.add_argument("--stage-chunk-mib", type=float, default=0.0,
+                    help="staged path: cap a staging slot at this many MiB; larger layers travel in chunks (tune.stage_chunk_bytes)")
     ap.add_argument("--per-layer", action="store_true",
                     help="issue one kvpool_offload / kvpool_retrieve call per layer in the timed step instead of the batched *_layers calls")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -286,6 +288,8 @@ def run_kvpool(args) -> dict:
     for k, v in (("link_ctas", args.link_ctas), ("hbm_ctas", args.hbm_ctas), ("stage_slots", args.stage_slots)):
         if v:
             tune[k] = v
+    if args.stage_chunk_mib:
+        tune["stage_chunk_bytes"] = int(args.stage_chunk_mib * 2**20)
     if tune:
         pool.set_tuning(**tune)
     tn = pool.get_tuning()
@@ -594,7 +598,7 @@ def run_kvpool(args) -> dict:
                    "moved_bytes_per_leg": moved, "pool_buffers": N, "weights": weights_kind, "bandwidth_gbps": [round(float(x), 3) for x in bw],
                    "numa_nodes": numa_actual, "path": args.path, "kernel": "vec16" if tn.kernel == kv.KERNEL_VEC16 else "bulk",
                    "link_kernel": "vec16" if tn.link_kernel == kv.KERNEL_VEC16 else "bulk",
-                   "link_ctas": tn.link_ctas, "hbm_ctas": tn.hbm_ctas, "stage_slots": tn.stage_slots, "streams": len(streams),
+                   "link_ctas": tn.link_ctas, "hbm_ctas": tn.hbm_ctas, "stage_slots": tn.stage_slots, "stage_chunk_bytes": tn.stage_chunk_bytes, "streams": len(streams),
                    "l2": f"inputs larger than L2: each leg moves {moved / 2**30:.1f} GiB through {L} distinct layers (L2 is 126 MB); no flush needed",
                    "calls": "per-layer" if args.per_layer else "batched (kvpool_offload_layers / kvpool_retrieve_layers, one call per request)",
                    "step": "kvpool_place + offload of every layer + retrieve of every layer; value = retrieve leg"},

@@ -117,6 +117,10 @@ typedef struct {         /* kvpool_set_tuning; 0 in any field = library default 
   uint32_t vec_unroll;   /* 16-byte loads in flight per lane in the vec16 kernel: 4, 8 or 16             */
   uint64_t auto_threshold_bytes; /* PATH_AUTO: layers (or groups) moving fewer bytes than this go zero-copy */
   uint64_t group_bytes;  /* batched calls: consecutive layers are grouped until a group moves at least this much */
+  uint64_t stage_chunk_bytes; /* staged path: a staging slot holds at most this much; a larger layer travels in chunks of
+                            consecutive logical blocks (copies of chunk c+1 overlap the pack/unpack of chunk c), so the
+                            staging ring (stage_slots x this) does not grow with the context length.  Default: off (a slot
+                            holds the largest layer); UINT64_MAX turns it off again; at least one block per chunk           */
 } kvpool_tuning;
 
 /* ---- pure host arithmetic (no CUDA, no pool) --------------------------------------------------------

@@ -46,7 +46,8 @@ class Geometry(ctypes.Structure):
 class Tuning(ctypes.Structure):
     _fields_ = [("kernel", c_uint32), ("link_kernel", c_uint32), ("hbm_ctas", c_uint32), ("link_ctas", c_uint32), ("bulk_chunk", c_uint32),
                 ("bulk_stages", c_uint32), ("bulk_warps", c_uint32), ("stage_slots", c_uint32),
-                ("vec_threads", c_uint32), ("vec_unroll", c_uint32), ("auto_threshold_bytes", c_uint64), ("group_bytes", c_uint64)]
+                ("vec_threads", c_uint32), ("vec_unroll", c_uint32), ("auto_threshold_bytes", c_uint64), ("group_bytes", c_uint64),
+                ("stage_chunk_bytes", c_uint64)]
 
 
 class KvPoolError(RuntimeError):

@@ -605,6 +605,7 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
   if (t->vec_unroll) d.vec_unroll = t->vec_unroll;
   if (t->auto_threshold_bytes) d.auto_threshold_bytes = t->auto_threshold_bytes;
   if (t->group_bytes) d.group_bytes = t->group_bytes;
+  if (t->stage_chunk_bytes) d.stage_chunk_bytes = t->stage_chunk_bytes == ~0ull ? 0 : t->stage_chunk_bytes;
   if (t->stage_slots && t->stage_slots != d.stage_slots) {
     DeviceGuard guard(p->cuda_device);
     d.stage_slots = t->stage_slots;
@@ -754,7 +755,9 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
     // a slot holds the largest layer, or a group of small layers (plus the 256-byte alignment gaps between stripes)
     const uint64_t total_bytes = std::accumulate(pl->region_bytes.begin(), pl->region_bytes.end(), uint64_t{0});
     const uint64_t group_cap = std::min<uint64_t>(std::max<uint64_t>(max_layer_bytes, p->tune.group_bytes), total_bytes);
-    const int rc = ensure_slots(p, std::max(max_layer_bytes, group_cap) + static_cast<uint64_t>(N) * 256 * (kMaxBatch + 1));
+    uint64_t want = std::max(max_layer_bytes, group_cap);
+    if (p->tune.stage_chunk_bytes) want = std::min(want, std::max<uint64_t>(p->tune.stage_chunk_bytes, p->payload));  // larger layers travel in chunks
+    const int rc = ensure_slots(p, want + static_cast<uint64_t>(N) * 256 * (kMaxBatch + 1));
     if (rc != KVPOOL_OK) { rollback(); return rc; }
   }
   p->live.push_back(pl.get());
@@ -782,22 +785,65 @@ int kvpool_release(kvpool_t* p, kvpool_placement_t* pl) {
 // ---------------------------------------------------------------------------------------------------
 extern "C" {
 
+// Slots of device i that hold logical blocks [first, first+n): a contiguous range because slots ascend with j.
+static void slot_range(const LayerMap& m, uint32_t i, uint32_t first, uint32_t n, uint32_t* lo, uint32_t* hi) {
+  if (first == 0 && n == m.K) { *lo = 0; *hi = m.counts[i]; return; }
+  const auto b = m.order.begin() + m.start[i], e = b + m.counts[i];
+  *lo = static_cast<uint32_t>(std::lower_bound(b, e, first) - b);
+  *hi = static_cast<uint32_t>(std::lower_bound(b, e, first + n) - b);
+}
+
+// Blocks one staging slot can take: the slot's size, capped by tune.stage_chunk_bytes (layers larger than that travel
+// in chunks of consecutive logical blocks, so the staging ring does not grow with the context length).
+static uint64_t blocks_per_slot(const kvpool* p) {
+  const uint64_t cap = p->tune.stage_chunk_bytes ? std::max<uint64_t>(p->tune.stage_chunk_bytes, p->payload) : ~0ull;
+  return std::min(p->slot_bytes, cap) / p->payload;
+}
+
+// One chunk [first, first+n) of a layer through a staging slot.  The slot is compact: device 0's share of the chunk,
+// then device 1's, ...; pool_base[i] is displaced so that slot index s of device i lands on its place in that share.
+struct ChunkPlan {
+  uint32_t lo[KVPOOL_MAX_DEVICES], hi[KVPOOL_MAX_DEVICES];
+  uint64_t off[KVPOOL_MAX_DEVICES];  // byte offset of device i's share inside the slot
+  bool host_blocks = false, hbm_blocks = false;
+};
+static ChunkPlan plan_chunk(const kvpool* p, const LayerState& L, uint32_t first, uint32_t n) {
+  ChunkPlan c;
+  uint64_t acc = 0;
+  for (uint32_t i = 0; i < p->n; ++i) {
+    slot_range(*L.map, i, first, n, &c.lo[i], &c.hi[i]);
+    c.off[i] = acc;
+    if (c.hi[i] == c.lo[i]) continue;
+    if (is_hbm(p, i)) { c.hbm_blocks = true; continue; }
+    c.host_blocks = true;
+    acc += static_cast<uint64_t>(c.hi[i] - c.lo[i]) * p->payload;
+  }
+  return c;
+}
+static void chunk_bases(const kvpool* p, const LayerState& L, const ChunkPlan& c, const StageSlot* slot, LayerArgs* a) {
+  for (uint32_t i = 0; i < p->n; ++i) {
+    // HBM-type devices: the kernel reaches the stripe in place; host devices: their share of the staging slot
+    if (is_hbm(p, i) || !slot) a->pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
+    else a->pool_base[i] = reinterpret_cast<uint64_t>(slot->buf) + c.off[i] - static_cast<uint64_t>(c.lo[i]) * p->payload;
+  }
+}
+
 int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
                    const int32_t* table, void* cuda_stream) {
   PoolLock lock__(p);
   int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
   if (rc != KVPOOL_OK) return rc;
   LayerState& L = pl->layers[layer];
-  L.offloaded = true;
-  if (L.map->K == 0) return KVPOOL_OK;
+  if (L.map->K == 0) { L.offloaded = true; return KVPOOL_OK; }
   DeviceGuard guard(p->cuda_device);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  const uint32_t N = p->n;
+  const uint32_t N = p->n, K = static_cast<uint32_t>(L.map->K);
   LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
 
   if (!use_staged(p, L)) {
     // zero-copy: one kernel gathers the paged blocks and stores them straight into the mapped host stripes
-    for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
+    L.offloaded = true;
+    chunk_bases(p, L, ChunkPlan{}, nullptr, &a);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));  // an earlier staged offload of this layer still in flight
     rc = launch_counted(p, a, true, true, s);
     if (rc != KVPOOL_OK) return rc;
@@ -806,55 +852,55 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
     return KVPOOL_OK;
   }
 
-  // staged: pack kernel -> device staging slot (stripe order), then one D2H copy per stripe on the
-  // per-device I/O streams; `stream` is released as soon as the pack is enqueued.
-  if (p->slots.empty() || L.map->K * p->payload > p->slot_bytes)
-    return fail(KVPOOL_ESTATE, "offload: no staging slot large enough (the placement was made while the path was zero-copy)");
-  StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
-  rc = wait_slot_free(p, slot, s);
-  if (rc != KVPOOL_OK) return rc;
-  slot.copies_after_kernel = 0;
-  bool hbm_blocks = false;
-  for (uint32_t i = 0; i < N; ++i) {
-    // HBM-type devices: the pack kernel stores straight into the stripe; host devices: into the staging slot
-    a.pool_base[i] = is_hbm(p, i) ? reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i])
-                                  : reinterpret_cast<uint64_t>(slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload);
-    hbm_blocks |= is_hbm(p, i) && L.map->counts[i];
-  }
-  if (hbm_blocks && L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));  // an earlier offload of this layer still writing the stripe
-  rc = launch_counted(p, a, true, false, s);
-  if (rc != KVPOOL_OK) return rc;
-  CU(cudaEventRecord(slot.kernel_done, s));
-  for (uint32_t i = 0; i < N; ++i) {
-    const uint64_t bytes = static_cast<uint64_t>(L.map->counts[i]) * p->payload;
-    if (bytes == 0 || is_hbm(p, i)) continue;
-    CU(cudaStreamWaitEvent(p->io_out[i], slot.kernel_done, 0));
-    if (L.landed_pending) CU(cudaStreamWaitEvent(p->io_out[i], L.landed, 0));
-    CU(cudaMemcpyAsync(static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i], slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload,
-                       bytes, cudaMemcpyDeviceToHost, p->io_out[i]));
-    p->n_memcpys++;
-    CU(cudaEventRecord(slot.copy_done[i], p->io_out[i]));
-    slot.copies_after_kernel |= 1u << i;
-  }
-  // `landed` must mean "all stripes done": record it on a stream that has waited for every copy
-  {
-    cudaStream_t js = nullptr;  // every I/O stream that copies has waited for the pack kernel, so it also covers the HBM stripes
-    for (uint32_t i = 0; i < N; ++i) {
-      if (static_cast<uint64_t>(L.map->counts[i]) == 0 || is_hbm(p, i)) continue;
-      if (!js) { js = p->io_out[i]; continue; }
-      CU(cudaStreamWaitEvent(js, slot.copy_done[i], 0));
+  // staged: pack kernel -> device staging slot, then one D2H copy per device on the per-device I/O streams; `stream` is
+  // released as soon as the last pack is enqueued.  A layer larger than a slot travels in chunks of logical blocks.
+  const uint64_t per_slot = p->slots.empty() ? 0 : blocks_per_slot(p);
+  if (per_slot == 0) return fail(KVPOOL_ESTATE, "offload: no staging slot (the placement was made while the path was zero-copy)");
+  L.offloaded = true;
+  cudaStream_t lead = nullptr;  // gathers every copy of the layer, so that `landed` can mean "all stripes complete"
+  for (uint32_t i = 0; i < N && !lead; ++i)
+    if (L.map->counts[i] && !is_hbm(p, i)) lead = p->io_out[i];
+  bool first_kernel = true;
+  for (uint32_t first = 0; first < K;) {
+    const uint32_t n = static_cast<uint32_t>(std::min<uint64_t>(per_slot, K - first));
+    const ChunkPlan c = plan_chunk(p, L, first, n);
+    a.j0 = first;
+    a.K = n;
+    first += n;
+    // an earlier offload of this layer may still be writing the HBM-type stripes the kernel stores into
+    if (c.hbm_blocks && first_kernel && L.landed_pending) { CU(cudaStreamWaitEvent(s, L.landed, 0)); first_kernel = false; }
+    if (!c.host_blocks) {  // the whole chunk sits on HBM-type devices: nothing to stage, no slot taken
+      chunk_bases(p, L, c, nullptr, &a);
+      rc = launch_counted(p, a, true, false, s);
+      if (rc != KVPOOL_OK) return rc;
+      continue;
     }
-    CU(cudaEventRecord(L.landed, js ? js : s));  // no host stripe at all: the kernel on `s` was the whole offload
-    L.landed_pending = true;
+    StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
+    rc = wait_slot_free(p, slot, s);
+    if (rc != KVPOOL_OK) return rc;
+    slot.copies_after_kernel = 0;
+    chunk_bases(p, L, c, &slot, &a);
+    rc = launch_counted(p, a, true, false, s);
+    if (rc != KVPOOL_OK) return rc;
+    CU(cudaEventRecord(slot.kernel_done, s));
+    for (uint32_t i = 0; i < N; ++i) {
+      if (c.hi[i] == c.lo[i] || is_hbm(p, i)) continue;
+      const uint64_t bytes = static_cast<uint64_t>(c.hi[i] - c.lo[i]) * p->payload;
+      CU(cudaStreamWaitEvent(p->io_out[i], slot.kernel_done, 0));
+      if (L.landed_pending) CU(cudaStreamWaitEvent(p->io_out[i], L.landed, 0));  // the previous offload of this layer
+      CU(cudaMemcpyAsync(static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i] + static_cast<uint64_t>(c.lo[i]) * p->payload,
+                         slot.buf + c.off[i], bytes, cudaMemcpyDeviceToHost, p->io_out[i]));
+      p->n_memcpys++;
+      CU(cudaEventRecord(slot.copy_done[i], p->io_out[i]));
+      slot.copies_after_kernel |= 1u << i;
+    }
+    CU(cudaStreamWaitEvent(lead, slot.kernel_done, 0));  // covers the HBM-type stripes the kernel wrote
+    for (uint32_t i = 0; i < N; ++i)
+      if ((slot.copies_after_kernel >> i & 1u) && p->io_out[i] != lead) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
   }
+  CU(cudaEventRecord(L.landed, lead));
+  L.landed_pending = true;
   return KVPOOL_OK;
-}
-
-// Slots of device i that hold logical blocks [first, first+n): a contiguous range because slots ascend with j.
-static void slot_range(const LayerMap& m, uint32_t i, uint32_t first, uint32_t n, uint32_t* lo, uint32_t* hi) {
-  const auto b = m.order.begin() + m.start[i], e = b + m.counts[i];
-  *lo = static_cast<uint32_t>(std::lower_bound(b, e, first) - b);
-  *hi = static_cast<uint32_t>(std::lower_bound(b, e, first + n) - b);
 }
 
 int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks, void* k_base,
@@ -872,61 +918,64 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const uint32_t N = p->n;
   LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
-  a.j0 = first_block;
-  a.K = n_blocks;
   const uint64_t range_bytes = static_cast<uint64_t>(n_blocks) * p->payload;
   bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && range_bytes >= p->tune.auto_threshold_bytes));
-  uint32_t lo[KVPOOL_MAX_DEVICES], hi[KVPOOL_MAX_DEVICES];
-  if (staged) {
-    // a range whose blocks all sit on HBM-type devices has nothing to stage: it must not take (and so recycle) a slot
-    bool host_blocks = false;
-    for (uint32_t i = 0; i < N; ++i) {
-      if (n_blocks == L.map->K) { lo[i] = 0; hi[i] = L.map->counts[i]; }
-      else slot_range(*L.map, i, first_block, n_blocks, &lo[i], &hi[i]);
-      host_blocks |= hi[i] != lo[i] && !is_hbm(p, i);
-    }
-    staged = host_blocks;
-  }
+  // a range whose blocks all sit on HBM-type devices has nothing to stage
+  if (staged) staged = plan_chunk(p, L, first_block, n_blocks).host_blocks;
+  settle_landed(L);
 
   if (!staged) {
-    for (uint32_t i = 0; i < N; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
-    settle_landed(L);
+    a.j0 = first_block;
+    a.K = n_blocks;
+    chunk_bases(p, L, ChunkPlan{}, nullptr, &a);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
     return launch_counted(p, a, false, true, s);
   }
 
-  // staged: one H2D copy per stripe (only the slots the range touches) on the per-device I/O streams — these may run
-  // ahead of `stream` — then the unpack kernel on `stream` once all of them have landed in the staging slot.
-  if (p->slots.empty() || L.map->K * p->payload > p->slot_bytes)
-    return fail(KVPOOL_ESTATE, "retrieve: no staging slot large enough (the placement was made while the path was zero-copy)");
-  StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
-  settle_landed(L);
-  bool hbm_blocks = false;
-  for (uint32_t i = 0; i < N; ++i) {
-    if (hi[i] == lo[i]) continue;
-    if (is_hbm(p, i)) { hbm_blocks = true; continue; }  // read in place by the unpack kernel
-    rc = wait_slot_free(p, slot, p->io[i]);
+  // staged: one H2D copy per device (only the slots the range touches) on the per-device I/O streams — these may run
+  // ahead of `stream` — then the unpack kernel on `stream` once all of them have landed in the staging slot.  A range
+  // larger than a slot travels in chunks of logical blocks: the copies of chunk c+1 overlap the unpack of chunk c.
+  const uint64_t per_slot = p->slots.empty() ? 0 : blocks_per_slot(p);
+  if (per_slot == 0) return fail(KVPOOL_ESTATE, "retrieve: no staging slot (the placement was made while the path was zero-copy)");
+  bool first_kernel = true;
+  for (uint32_t first = first_block, end = first_block + n_blocks; first < end;) {
+    const uint32_t n = static_cast<uint32_t>(std::min<uint64_t>(per_slot, end - first));
+    const ChunkPlan c = plan_chunk(p, L, first, n);
+    a.j0 = first;
+    a.K = n;
+    first += n;
+    if (c.hbm_blocks && first_kernel && L.landed_pending) { CU(cudaStreamWaitEvent(s, L.landed, 0)); first_kernel = false; }
+    if (!c.host_blocks) {  // read in place by the unpack kernel: no slot taken (a slot recycled without waits could be
+      chunk_bases(p, L, c, nullptr, &a);  // overwritten under an earlier offload's copy)
+      rc = launch_counted(p, a, false, false, s);
+      if (rc != KVPOOL_OK) return rc;
+      continue;
+    }
+    StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
+    for (uint32_t i = 0; i < N; ++i) {
+      if (c.hi[i] == c.lo[i] || is_hbm(p, i)) continue;
+      rc = wait_slot_free(p, slot, p->io[i]);
+      if (rc != KVPOOL_OK) return rc;
+      if (L.landed_pending) CU(cudaStreamWaitEvent(p->io[i], L.landed, 0));
+    }
+    slot.copies_after_kernel = 0;
+    chunk_bases(p, L, c, &slot, &a);
+    for (uint32_t i = 0; i < N; ++i) {
+      if (c.hi[i] == c.lo[i] || is_hbm(p, i)) continue;
+      const uint64_t bytes = static_cast<uint64_t>(c.hi[i] - c.lo[i]) * p->payload;
+      CU(cudaMemcpyAsync(slot.buf + c.off[i], static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i] + static_cast<uint64_t>(c.lo[i]) * p->payload,
+                         bytes, cudaMemcpyHostToDevice, p->io[i]));
+      p->n_memcpys++;
+      CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+      CU(cudaStreamWaitEvent(s, slot.copy_done[i], 0));
+    }
+    rc = launch_counted(p, a, false, false, s);
     if (rc != KVPOOL_OK) return rc;
-    if (L.landed_pending) CU(cudaStreamWaitEvent(p->io[i], L.landed, 0));
+    CU(cudaEventRecord(slot.kernel_done, s));
   }
-  if (hbm_blocks && L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
-  slot.copies_after_kernel = 0;
-  for (uint32_t i = 0; i < N; ++i) {
-    uint8_t* stage_i = slot.buf + static_cast<uint64_t>(L.map->start[i]) * p->payload;   // same layout as a full layer
-    a.pool_base[i] = reinterpret_cast<uint64_t>(stage_i);
-    if (is_hbm(p, i)) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i]);
-    if (hi[i] == lo[i] || is_hbm(p, i)) continue;
-    const uint64_t off = static_cast<uint64_t>(lo[i]) * p->payload, bytes = static_cast<uint64_t>(hi[i] - lo[i]) * p->payload;
-    CU(cudaMemcpyAsync(stage_i + off, static_cast<uint8_t*>(p->bufs[i].host) + L.stripe_off[i] + off, bytes, cudaMemcpyHostToDevice, p->io[i]));
-    p->n_memcpys++;
-    CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
-    CU(cudaStreamWaitEvent(s, slot.copy_done[i], 0));
-  }
-  rc = launch_counted(p, a, false, false, s);
-  if (rc != KVPOOL_OK) return rc;
-  CU(cudaEventRecord(slot.kernel_done, s));
   return KVPOOL_OK;
 }
+
 
 int kvpool_retrieve(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
                     const int32_t* table, void* cuda_stream) {
@@ -1036,7 +1085,8 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
     dev_start[i] = total;
     total += (span[i] + 255) / 256 * 256;
   }
-  if (total > p->slot_bytes || p->slots.empty()) return 1;
+  if (p->slots.empty() || total > p->slot_bytes || (p->tune.stage_chunk_bytes && total > std::max<uint64_t>(p->tune.stage_chunk_bytes, p->payload) + 256ull * N))
+    return 1;
   if (total == 0) return issue_zero_copy_group(c, g);  // every block of the group sits on HBM-type devices: nothing to stage, no slot taken
   StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
   MultiArgs ma{};

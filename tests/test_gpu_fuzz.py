@@ -107,7 +107,8 @@ def test_random_sequences_match_the_oracle(seed):
     try:
         pool.set_tuning(stage_slots=int(rng.integers(1, 4)), group_bytes=int(rng.choice([1 << 20, 8 << 20, 64 << 20])),
                         auto_threshold_bytes=int(rng.choice([64 << 10, 1 << 20, 8 << 20])),
-                        kernel=int(rng.integers(0, 2)), link_kernel=int(rng.integers(0, 2)))
+                        kernel=int(rng.integers(0, 2)), link_kernel=int(rng.integers(0, 2)),
+                        stage_chunk_bytes=int(rng.choice([2 ** 64 - 1, 2 ** 64 - 1, 96 << 10, 1 << 20, 5 << 20])))   # off, or chunked staging
         pool.set_path(kv.PATH_STAGED)
         pool.reserve_staging(KMAX * 2 * kvb)                                   # zero-copy placements never shrink the ring
         for step in range(90):

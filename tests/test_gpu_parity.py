@@ -844,3 +844,39 @@ def test_host_threads_share_one_pool():
             assert np.array_equal(dst[l].cpu().numpy().view(np.uint16), want), l
     finally:
         pool.destroy()
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_chunked_staging_caps_the_ring_and_keeps_parity(kernel):
+    """tune.stage_chunk_bytes: a layer larger than a staging slot travels in chunks of consecutive logical blocks through
+    compact slots — same stripes, same retrieved tensors, more (smaller) launches and copies, a ring that no longer grows
+    with the layer."""
+    k = KERNELS[kernel]
+    wl = W.make_workload(4, scale=1 / 8, n_layers=3)                      # 1024 blocks x 32 KiB = 32 MiB per layer, 6 devices
+    base = run_parity(wl, path=kv.PATH_STAGED, kernel=k)
+    # 5 MiB chunks: 160 blocks each, 7 chunks per layer (the last one ragged); per-layer calls and 4 streams' worth of slots
+    out = run_parity(wl, path=kv.PATH_STAGED, kernel=k, tuning={"stage_chunk_bytes": 5 << 20})
+    assert out["bytes_compared"] == base["bytes_compared"]
+    assert out["kernels"] == 7 * base["kernels"] and out["memcpys"] == 7 * base["memcpys"]
+    # a chunk smaller than one block still moves one block at a time; 2 slots; mixed host / HBM pool; ragged block size
+    g = W.Geometry(n_layers=2, n_kv_heads=1, head_dim=80)
+    rng = np.random.default_rng(53)
+    run_parity(_custom(g, 301, [rng.permutation(301)[:257]], 3, (3.0, 2.0, 1.0)), path=kv.PATH_STAGED, kernel=k,
+               tuning={"stage_chunk_bytes": 1000, "stage_slots": 2}, dev_flags=[0, HBM, 0])
+    # auto path, sliding-window layers (tiny layers go zero-copy, big ones chunked), several requests on several streams
+    run_parity(W.make_workload(3, scale=1 / 8, n_layers=4), path=kv.PATH_AUTO, kernel=k, tuning={"stage_chunk_bytes": 3 << 20})
+    run_parity(W.make_workload(5, scale=1 / 16, n_layers=2), path=kv.PATH_STAGED, kernel=k, streams=4, tuning={"stage_chunk_bytes": 2 << 20})
+    # batched calls and partial retrieval under a chunk cap
+    _run_batched(W.make_workload(3, scale=1 / 8, n_layers=6), kv.PATH_STAGED, k, expect_kernels=None, expect_memcpys=None,
+                 tuning={"stage_chunk_bytes": 3 << 20})
+    # the ring really is capped: 4 slots of ~5 MiB instead of 4 x 32 MiB
+    pool = make_pool(wl)
+    try:
+        pool.set_path(kv.PATH_STAGED)
+        free0 = torch.cuda.mem_get_info()[0]
+        pool.set_tuning(stage_chunk_bytes=5 << 20)
+        pl = pool.place(wl.blocks_per_layer(0))
+        assert free0 - torch.cuda.mem_get_info()[0] < 4 * (8 << 20)
+        pl.release()
+    finally:
+        pool.destroy()
