@@ -49,6 +49,8 @@ def _load():
             f.argtypes = [vp, vp, u64, u64, vp, u64, vp, vp, vp]
         lib.orc_retrieve_range.restype = None
         lib.orc_retrieve_range.argtypes = [vp, vp, u64, u64, vp, u64, u64, vp, vp, vp]
+        lib.orc_offload_range.restype = None
+        lib.orc_offload_range.argtypes = [vp, vp, u64, u64, vp, u64, u64, vp, vp, vp]
         lib.orc_checksum.restype = u64
         lib.orc_checksum.argtypes = [vp, vp, u64, u64, vp, u64]
         lib.orc_layer_parallel.restype = ctypes.c_int
@@ -166,6 +168,15 @@ def retrieve_range(kv_layer_out: np.ndarray, table: np.ndarray, pl: LayerPlaceme
     assert 0 <= first and first + n <= table.shape[0]
     ptrs = _stripe_ptrs(stripes)
     _load().orc_retrieve_range(kp, vp_, stride, kvb, _ptr(table), int(first), int(n), _ptr(pl.dev), _ptr(pl.slot), ctypes.addressof(ptrs))
+
+
+def offload_range(kv_layer: np.ndarray, table: np.ndarray, pl: LayerPlacement, stripes: List[np.ndarray], first: int, n: int) -> None:
+    """Partial offload: logical blocks [first, first+n) of one layer into the given stripes (in place)."""
+    kp, vp_, stride, kvb = _planes(kv_layer)
+    table = np.ascontiguousarray(table, dtype=np.int32)
+    assert 0 <= first and first + n <= table.shape[0] and table.shape[0] == pl.dev.shape[0]
+    ptrs = _stripe_ptrs(stripes)
+    _load().orc_offload_range(kp, vp_, stride, kvb, _ptr(table), int(first), int(n), _ptr(pl.dev), _ptr(pl.slot), ctypes.addressof(ptrs))
 
 
 def checksum(kv_layer: np.ndarray, table: np.ndarray) -> int:

@@ -21,6 +21,8 @@
  *                             reduces to memcpy, O(K^2) brute-force search, round trip, conservation
  *   orc_retrieve_range      — (0, K) equals orc_retrieve_layer; disjoint ranges compose to the full retrieve; numpy
  *                             index assignment on the range; nothing outside the range's physical blocks is written
+ *   orc_offload_range       — (0, K) equals orc_offload_layer; disjoint ranges compose to the full offload; numpy fancy
+ *                             indexing into the range's slots; stripe bytes outside the range's slots keep their fill
  *   orc_checksum            — closed form n_words^2 * c for constant words, python big-int restatement, sensitivity
  *                             to swapping two blocks
  *   stripe offsets inside a pool buffer: PARITY UNPINNED (implementation detail; not produced here).
@@ -156,6 +158,21 @@ void orc_retrieve_range(uint8_t *k_plane, uint8_t *v_plane, uint64_t stride, uin
         const uint8_t *src = stripes[dev[j]] + (uint64_t)slot[j] * 2u * kvb;
         memcpy(k_plane + (uint64_t)table[j] * stride, src, kvb);
         memcpy(v_plane + (uint64_t)table[j] * stride, src + kvb, kvb);
+    }
+}
+
+/* ---- partial offload ----------------------------------------------------------------------------
+ * "At decoding step t, let K(t) denote the set of KV caches that must be offloaded": a
+ * request's blocks reach the pool in instalments.  Here an instalment is a contiguous range
+ * [first, first+n) of the layer's logical blocks, stored at the places Algorithm 1 gave them when the
+ * layer was placed; same per-block MEMSTORE as orc_offload_layer, nothing outside the range's slots is
+ * written. */
+void orc_offload_range(const uint8_t *k_plane, const uint8_t *v_plane, uint64_t stride, uint64_t kvb, const int32_t *table,
+                       uint64_t first, uint64_t n, const uint32_t *dev, const uint32_t *slot, uint8_t *const *stripes) {
+    for (uint64_t j = first; j < first + n; ++j) {
+        uint8_t *dst = stripes[dev[j]] + (uint64_t)slot[j] * 2u * kvb;
+        memcpy(dst, k_plane + (uint64_t)table[j] * stride, kvb);
+        memcpy(dst + kvb, v_plane + (uint64_t)table[j] * stride, kvb);
     }
 }
 

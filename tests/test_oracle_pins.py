@@ -348,6 +348,50 @@ def test_retrieve_range_composes_and_touches_only_its_blocks():
             assert abs(took - Fraction(int(pl.counts[i]) * n, K)) <= len(w) - 1 + 1
 
 
+def test_offload_range_composes_and_writes_only_its_slots():
+    """Partial offload (instalments of a request's blocks): (0, K) is the full offload; disjoint ranges
+    compose to it in any order; a range equals numpy fancy indexing into exactly the slots Algorithm 1 gave its blocks
+    (found here by an independent search over (dev, slot)); every other stripe byte keeps its fill."""
+    rng = np.random.default_rng(13)
+    nphys, kvb, K = 120, 64, 90
+    kv = _tiny_layer(rng, nphys, kvb)
+    table = rng.permutation(nphys)[:K].astype(np.int32)
+    w = [4, 4, 2, 2, 1, 1]
+    pl = oracle.place(w, [K])[0]
+    full = oracle.offload_layer(kv, table, pl)
+    P = 2 * kvb
+
+    def filled():
+        return [np.full(int(c) * P, 0xA5, dtype=np.uint8) for c in pl.counts]
+
+    a = filled()
+    oracle.offload_range(kv, table, pl, a, 0, K)
+    assert all(np.array_equal(x, y) for x, y in zip(a, full))
+    b = filled()
+    cuts = [0, 1, 17, 17, 50, 89, 90]
+    for lo, hi in reversed(list(zip(cuts[:-1], cuts[1:]))):               # instalments in reverse order
+        oracle.offload_range(kv, table, pl, b, lo, hi - lo)
+    assert all(np.array_equal(x, y) for x, y in zip(b, full))
+    kv8 = kv.view(np.uint8).reshape(2, nphys, kvb)
+    for first, n in ((0, 23), (23, 40), (89, 1), (40, 0)):
+        c = filled()
+        oracle.offload_range(kv, table, pl, c, first, n)
+        want = filled()
+        for i in range(len(w)):                                           # slot s of device i holds the unique j with (dev, slot) = (i, s)
+            js = [j for j in range(first, first + n) if pl.dev[j] == i]
+            for j in js:
+                s_ = int(pl.slot[j])
+                want[i][s_ * P:s_ * P + kvb] = kv8[0, table[j]]
+                want[i][s_ * P + kvb:(s_ + 1) * P] = kv8[1, table[j]]
+        assert all(np.array_equal(x, y) for x, y in zip(c, want)), (first, n)
+    # what was offloaded in instalments comes back whole
+    back = np.full_like(kv, 0x7FC1)
+    oracle.retrieve_layer(back, table, pl, b)
+    ref = np.full_like(kv, 0x7FC1)
+    ref[:, table] = kv[:, table]
+    assert np.array_equal(back, ref)
+
+
 def test_checksum_closed_form_python_restatement_and_sensitivity():
     rng = np.random.default_rng(12)
     nphys, kvb, n = 19, 48, 11
