@@ -235,6 +235,15 @@ KVPOOL_API int kvpool_retrieve_layers_signal(kvpool_t* pool, kvpool_placement_t*
 KVPOOL_API int kvpool_retrieve_range(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks,
                           void* k_base /*device*/, void* v_base /*device*/, uint64_t block_stride_bytes,
                           const int32_t* block_table_dev, void* cuda_stream);
+/* Partial offload — a request's blocks reach the pool in instalments ("at decoding step t, let K(t) denote the set of KV
+ * caches that must be offloaded"): like kvpool_offload for logical blocks [first_block, first_block +
+ * n_blocks) of the layer only, stored at the places Algorithm 1 gave them when the layer was placed (so the split
+ * stays bandwidth-proportional however the layer is cut).  Nothing outside the range's slots is written.  A retrieve
+ * (whole or range) needs every block it names to have been offloaded: ESTATE otherwise.  EINVAL if the range exceeds
+ * K_l; n_blocks = 0 is a no-op.  kvpool_offload is this call over [0, K_l).                                           */
+KVPOOL_API int kvpool_offload_range(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks,
+                         const void* k_base /*device*/, const void* v_base /*device*/, uint64_t block_stride_bytes,
+                         const int32_t* block_table_dev /*device[K_l]*/, void* cuda_stream);
 /* Comparison baseline, not a product path: what an engine without a gather kernel does — one cudaMemcpyAsync per
  * K block and per V block (2*K_l calls) straight between the paged blocks and the stripes, all on `stream`.
  * block_table_host is the HOST copy of the layer's table.  Same results as kvpool_offload / kvpool_retrieve;

@@ -27,7 +27,7 @@ _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA",
 EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
     "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release",
-    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
+    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
     "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_validate_table", "kvpool_last_error", "kvpool_version",
 ]
@@ -87,6 +87,7 @@ def lib():
             "kvpool_offload": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_retrieve": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_retrieve_range": [vp, vp, c_uint32, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
+            "kvpool_offload_range": [vp, vp, c_uint32, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_offload_layers": [vp, vp, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_retrieve_layers": [vp, vp, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_retrieve_layers_signal": [vp, vp, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp, vp],
@@ -309,6 +310,11 @@ class KvPool:
                        block_table_dev, stream=None) -> None:
         _ck(lib().kvpool_retrieve_range(self.handle, pl.handle, layer, first_block, n_blocks, _addr(k_base), _addr(v_base),
                                         block_stride_bytes, _addr(block_table_dev), _stream(stream)))
+
+    def offload_range(self, pl: Placement, layer: int, first_block: int, n_blocks: int, k_base, v_base, block_stride_bytes: int,
+                      block_table_dev, stream=None) -> None:
+        _ck(lib().kvpool_offload_range(self.handle, pl.handle, layer, first_block, n_blocks, _addr(k_base), _addr(v_base),
+                                       block_stride_bytes, _addr(block_table_dev), _stream(stream)))
 
     @staticmethod
     def _ptr_array(items) -> "ctypes.Array":

@@ -77,7 +77,8 @@ struct LayerState {
   std::shared_ptr<LayerMap> map;
   std::vector<uint64_t> stripe_off;  // [N] byte offset of this layer's stripe inside pool buffer i
   const uint64_t* base_d = nullptr;  // device: [N] GPU-visible addresses of this layer's stripes (for batched launches)
-  bool offloaded = false;
+  bool offloaded = false;            // every block of the layer has been offloaded at least once
+  std::vector<uint64_t> have;        // else, once a partial offload has happened: bit j = logical block j is in the pool
   cudaEvent_t landed = nullptr;      // recorded when the layer's stripes are complete in the pool
   bool landed_pending = false;
 };
@@ -785,6 +786,25 @@ int kvpool_release(kvpool_t* p, kvpool_placement_t* pl) {
 // ---------------------------------------------------------------------------------------------------
 extern "C" {
 
+// Which blocks of a layer are in the pool (kvpool_offload_range fills a layer in instalments).
+static void mark_offloaded(LayerState& L, uint32_t first, uint32_t n) {
+  const uint64_t K = L.map->K;
+  if (L.offloaded) return;
+  if (n == K) { L.offloaded = true; L.have.clear(); return; }
+  if (L.have.empty()) L.have.assign((K + 63) / 64, 0);
+  for (uint32_t j = first; j < first + n; ++j) L.have[j >> 6] |= 1ull << (j & 63);
+  uint64_t total = 0;
+  for (uint64_t w : L.have) total += static_cast<uint64_t>(__builtin_popcountll(w));
+  if (total == K) { L.offloaded = true; L.have.clear(); }
+}
+static bool is_offloaded(const LayerState& L, uint32_t first, uint32_t n) {
+  if (L.offloaded) return true;
+  if (L.have.empty()) return false;
+  for (uint32_t j = first; j < first + n; ++j)
+    if (!(L.have[j >> 6] >> (j & 63) & 1ull)) return false;
+  return true;
+}
+
 // Slots of device i that hold logical blocks [first, first+n): a contiguous range because slots ascend with j.
 static void slot_range(const LayerMap& m, uint32_t i, uint32_t first, uint32_t n, uint32_t* lo, uint32_t* hi) {
   if (first == 0 && n == m.K) { *lo = 0; *hi = m.counts[i]; return; }
@@ -828,21 +848,32 @@ static void chunk_bases(const kvpool* p, const LayerState& L, const ChunkPlan& c
   }
 }
 
-int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
-                   const int32_t* table, void* cuda_stream) {
+int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks, const void* k_base,
+                         const void* v_base, uint64_t stride, const int32_t* table, void* cuda_stream) {
   PoolLock lock__(p);
   int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table);
   if (rc != KVPOOL_OK) return rc;
   LayerState& L = pl->layers[layer];
+  if (static_cast<uint64_t>(first_block) + n_blocks > L.map->K)
+    return fail(KVPOOL_EINVAL, "offload: blocks [%u, %u) exceed the layer's %llu blocks", first_block, first_block + n_blocks,
+                (unsigned long long)L.map->K);
   if (L.map->K == 0) { L.offloaded = true; return KVPOOL_OK; }
+  if (n_blocks == 0) return KVPOOL_OK;
   DeviceGuard guard(p->cuda_device);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  const uint32_t N = p->n, K = static_cast<uint32_t>(L.map->K);
+  const uint32_t N = p->n;
   LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
+  bool staged = use_staged(p, L);
+  if (staged && n_blocks != L.map->K) {  // a range is judged by its own size and by where its own blocks sit
+    staged = plan_chunk(p, L, first_block, n_blocks).host_blocks &&
+             (p->path == KVPOOL_PATH_STAGED || static_cast<uint64_t>(n_blocks) * p->payload >= p->tune.auto_threshold_bytes);
+  }
 
-  if (!use_staged(p, L)) {
+  if (!staged) {
     // zero-copy: one kernel gathers the paged blocks and stores them straight into the mapped host stripes
-    L.offloaded = true;
+    mark_offloaded(L, first_block, n_blocks);
+    a.j0 = first_block;
+    a.K = n_blocks;
     chunk_bases(p, L, ChunkPlan{}, nullptr, &a);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));  // an earlier staged offload of this layer still in flight
     rc = launch_counted(p, a, true, true, s);
@@ -856,13 +887,14 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
   // released as soon as the last pack is enqueued.  A layer larger than a slot travels in chunks of logical blocks.
   const uint64_t per_slot = p->slots.empty() ? 0 : blocks_per_slot(p);
   if (per_slot == 0) return fail(KVPOOL_ESTATE, "offload: no staging slot (the placement was made while the path was zero-copy)");
-  L.offloaded = true;
+  mark_offloaded(L, first_block, n_blocks);
   cudaStream_t lead = nullptr;  // gathers every copy of the layer, so that `landed` can mean "all stripes complete"
   for (uint32_t i = 0; i < N && !lead; ++i)
     if (L.map->counts[i] && !is_hbm(p, i)) lead = p->io_out[i];
+  if (L.landed_pending) CU(cudaStreamWaitEvent(lead, L.landed, 0));  // `landed` keeps covering what was offloaded before
   bool first_kernel = true;
-  for (uint32_t first = 0; first < K;) {
-    const uint32_t n = static_cast<uint32_t>(std::min<uint64_t>(per_slot, K - first));
+  for (uint32_t first = first_block, end = first_block + n_blocks; first < end;) {
+    const uint32_t n = static_cast<uint32_t>(std::min<uint64_t>(per_slot, end - first));
     const ChunkPlan c = plan_chunk(p, L, first, n);
     a.j0 = first;
     a.K = n;
@@ -903,6 +935,14 @@ int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const vo
   return KVPOOL_OK;
 }
 
+int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
+                   const int32_t* table, void* cuda_stream) {
+  PoolLock lock__(p);
+  if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "offload: bad pool or placement");
+  if (layer >= p->geom.n_layers) return fail(KVPOOL_EINVAL, "layer %u out of range (n_layers %u)", layer, p->geom.n_layers);
+  return kvpool_offload_range(p, pl, layer, 0, static_cast<uint32_t>(pl->layers[layer].map->K), k_base, v_base, stride, table, cuda_stream);
+}
+
 int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks, void* k_base,
                           void* v_base, uint64_t stride, const int32_t* table, void* cuda_stream) {
   PoolLock lock__(p);
@@ -912,7 +952,9 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   if (static_cast<uint64_t>(first_block) + n_blocks > L.map->K)
     return fail(KVPOOL_EINVAL, "retrieve: blocks [%u, %u) exceed the layer's %llu blocks", first_block, first_block + n_blocks,
                 (unsigned long long)L.map->K);
-  if (!L.offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", layer);
+  if (!L.offloaded && L.have.empty()) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", layer);
+  if (!is_offloaded(L, first_block, n_blocks))
+    return fail(KVPOOL_ESTATE, "retrieve: some of blocks [%u, %u) of layer %u were never offloaded", first_block, first_block + n_blocks, layer);
   if (n_blocks == 0) return KVPOOL_OK;
   DeviceGuard guard(p->cuda_device);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
@@ -1211,7 +1253,7 @@ static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32
   uint64_t units = 0;
   for (uint32_t q = 0; q < n; ++q) {
     LayerState& L = pl->layers[first + q];
-    if (pack) L.offloaded = true;
+    if (pack) { L.offloaded = true; L.have.clear(); }
     if (L.map->K == 0) {  // nothing to move: ready in stream order right away
       if (ready && ready[q]) CU(cudaEventRecord(static_cast<cudaEvent_t>(ready[q]), c.s));
       continue;
@@ -1261,7 +1303,7 @@ static int naive_layer(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, bool
   if (rc != KVPOOL_OK) return rc;
   LayerState& L = pl->layers[layer];
   if (!pack && !L.offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", layer);
-  if (pack) L.offloaded = true;
+  if (pack) { L.offloaded = true; L.have.clear(); }
   DeviceGuard guard(p->cuda_device);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));

@@ -122,6 +122,18 @@ def test_random_sequences_match_the_oracle(seed):
                 l, v = int(rng.integers(0, L)), int(rng.integers(0, 2))
                 pool.offload(r.pl, l, src[v][l][0], src[v][l][1], kvb, r.table, r.stream)
                 r.version[l] = v
+            elif op < 0.36:                                                    # re-offload of a range of a layer already in the pool
+                l = int(rng.integers(0, L))
+                if r.version[l] is None or r.bpl[l] < 2:
+                    continue
+                first = int(rng.integers(0, r.bpl[l])); n = int(rng.integers(1, r.bpl[l] - first + 1))
+                v = int(rng.integers(0, 2))
+                pool.offload_range(r.pl, l, first, n, src[v][l][0], src[v][l][1], kvb, r.table, r.stream)
+                base = stripes_of(r, l)                                        # oracle: the range lands on top of what was there
+                mixed = [x.copy() for x in base]
+                oracle.offload_range(src_np[v][l], r.table_np[:r.bpl[l]], r.opl[l], mixed, first, n)
+                r.version[l] = ("mix", step)
+                r.stripes[(l, r.version[l])] = mixed
             elif op < 0.42:                                                    # batched offload of a run of layers
                 a = int(rng.integers(0, L)); n = int(rng.integers(1, L - a + 1)); v = int(rng.integers(0, 2))
                 pool.offload_layers(r.pl, a, [src[v][l][0] for l in range(a, a + n)], [src[v][l][1] for l in range(a, a + n)], kvb,

@@ -880,3 +880,72 @@ def test_chunked_staging_caps_the_ring_and_keeps_parity(kernel):
         pl.release()
     finally:
         pool.destroy()
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+@pytest.mark.parametrize("path", ["staged", "zerocopy", "auto"])
+def test_offload_range_fills_a_layer_in_instalments(path, kernel):
+    """kvpool_offload_range: a layer placed once and offloaded in instalments, in any order, ends with the
+    oracle's stripes; after each instalment exactly its slots have changed (the rest of the stripes still hold the fill
+    written before), a retrieve of blocks not yet offloaded is ESTATE, and what has arrived can be retrieved at once."""
+    p, k = PATHS[path], KERNELS[kernel]
+    wl = W.make_workload(4, scale=1 / 16, n_layers=1)                    # 512 blocks x 32 KiB, 6 devices 4:4:2:2:1:1
+    g, dev = wl.geom, torch.device("cuda:0")
+    bw = list(wl.default_weights())
+    for flags, tuning in (([0] * 6, {}), ([0, HBM, 0, 0, HBM, 0], {"stage_chunk_bytes": 3 << 20, "stage_slots": 2})):
+        pool = make_pool(wl, dev_flags=flags)
+        try:
+            pool.set_path(p)
+            pool.set_tuning(kernel=k, link_kernel=k, **tuning)
+            bpl = wl.blocks_per_layer(0)
+            K = int(bpl[0])
+            pl = pool.place(bpl)
+            opl = oracle.place(bw, bpl)
+            table_np = np.ascontiguousarray(wl.layer_table(0, 0))
+            table = torch.from_numpy(table_np).to(dev)
+            src, src_cpu = W.kv_layer_torch(wl, 0, dev), W.kv_layer_numpy(wl, 0)
+            fill = torch.full_like(src, 0x1111)                           # a first whole-layer offload of a constant: the stripes' fill
+            fill_cpu = np.full_like(src_cpu, 0x1111)
+            torch.cuda.synchronize()
+            s = torch.cuda.Stream()
+            with pytest.raises(kv.KvPoolError) as e:
+                pool.offload_range(pl, 0, K - 3, 4, src[0], src[1], g.kvb, table, s)
+            assert e.value.code == kv.EINVAL
+            pool.offload_range(pl, 0, 0, 40, fill[0], fill[1], g.kvb, table, s)
+            dst = W.poison_torch((2, wl.nphys, g.kvb // 2), dev)
+            with pytest.raises(kv.KvPoolError) as e:                      # blocks 40.. are not in the pool yet
+                pool.retrieve(pl, 0, dst[0], dst[1], g.kvb, table, s)
+            assert e.value.code == kv.ESTATE
+            with pytest.raises(kv.KvPoolError) as e:
+                pool.retrieve_range(pl, 0, 30, 20, dst[0], dst[1], g.kvb, table, s)
+            assert e.value.code == kv.ESTATE
+            pool.retrieve_range(pl, 0, 5, 30, dst[0], dst[1], g.kvb, table, s)       # these are
+            pool.offload(pl, 0, fill[0], fill[1], g.kvb, table, s)                   # now the whole layer holds the fill
+            want = oracle.offload_layer(fill_cpu, table_np, opl[0])
+            cuts = [0, 1, 130, 130, 131, 400, K]
+            order = [4, 0, 5, 2, 1, 3]
+            for q in order:
+                lo, hi = cuts[q], cuts[q + 1]
+                pool.offload_range(pl, 0, lo, hi - lo, src[0], src[1], g.kvb, table, s)
+                oracle.offload_range(src_cpu, table_np, opl[0], want, lo, hi - lo)
+                if q in (0, 2):                                           # check the intermediate state twice, else keep enqueueing
+                    pool.wait_offloads(pl, s)
+                    s.synchronize()
+                    for i in range(pool.n_devices):
+                        assert np.array_equal(pl.stripe(0, i), want[i]), (path, q, i)
+            pool.wait_offloads(pl, s)
+            dst2 = W.poison_torch((2, wl.nphys, g.kvb // 2), dev)
+            pool.retrieve(pl, 0, dst2[0], dst2[1], g.kvb, table, s)
+            s.synchronize()
+            full = oracle.offload_layer(src_cpu, table_np, opl[0])
+            for i in range(pool.n_devices):
+                assert np.array_equal(pl.stripe(0, i), full[i]) and np.array_equal(want[i], full[i])
+            ref = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+            oracle.retrieve_layer(ref, table_np, opl[0], full)
+            assert np.array_equal(dst2.cpu().numpy().view(np.uint16), ref)
+            ref1 = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+            oracle.retrieve_range(ref1, table_np, opl[0], oracle.offload_layer(fill_cpu, table_np, opl[0]), 5, 30)
+            assert np.array_equal(dst.cpu().numpy().view(np.uint16), ref1)
+            pl.release()
+        finally:
+            pool.destroy()
