@@ -168,7 +168,8 @@ KVPOOL_API int kvpool_get_tuning(const kvpool_t* pool, kvpool_tuning* t_out /*ho
 
 /* Size the staging ring of the staged path now: `stage_slots` device buffers of `bytes` bytes each.  A placement needs
  * max(its largest layer K_l * P, min(group_bytes, all its layers together)) — the second term for the groups of small
- * layers the batched calls form.  kvpool_place grows the ring by itself when a placement needs more, but
+ * layers the batched calls form — capped by tune.stage_chunk_bytes when that is set (larger layers then travel in
+ * chunks).  kvpool_place grows the ring by itself when a placement needs more, but
  * growing waits for the whole device (cudaDeviceSynchronize) and reallocates; an engine that knows its largest layer
  * calls this once at start-up and no later kvpool_place ever waits for GPU work.  ENOMEM if the device is out of memory. */
 KVPOOL_API int kvpool_reserve_staging(kvpool_t* pool, uint64_t bytes);
