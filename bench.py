@@ -527,10 +527,14 @@ def run_kvpool(args) -> dict:
     dom = max(range(4), key=lambda k: prof[k][0])
     ms, n, b = prof[dom]
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")                            # ncu dram bytes per launch (profiles/traffic.md)
     if os.path.exists(tp):
         with open(tp) as f:
-            traffic = json.load(f).get(str(args.config), {}).get(kinds[dom])     # captured per config; null where not captured
+            for row in f.read().splitlines()[1:]:
+                cfg, rest = row.split(",", 1)
+                kind, nbytes = rest.rsplit(",", 1)
+                if cfg == str(args.config) and kind == kinds[dom]:                  # captured per config; null where not captured
+                    traffic = int(nbytes)
     if dom < 2:
         ach = 2 * b / (ms * 1e6) if ms > 0 else 0.0
         roof = {"bound": "hbm", "kernel": kinds[dom], "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
