@@ -1,6 +1,8 @@
 """GPU parity: the CUDA path, called through the C ABI, against the CPU oracle on the same seeded inputs.
 Bit-exact on placement (counts, dev[], slot[]), on every stripe byte after offload and on the whole paged
 tensor after retrieve into a poison-filled pool (tolerance: none — integer and byte work only)."""
+import ctypes
+
 import numpy as np
 import pytest
 import torch
@@ -949,3 +951,81 @@ def test_offload_range_fills_a_layer_in_instalments(path, kernel):
             pl.release()
         finally:
             pool.destroy()
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_red_zones_around_planes_stripes_and_staging_stay_intact(kernel):
+    """compute-sanitizer is closed on this GPU pool, so out-of-bounds writes are hunted with red zones: the K and V planes
+    and a caller staging buffer sit inside larger poison-filled allocations, the table names the first and the last
+    physical block, block sizes are ragged (not a multiple of the kernels' 4 KiB / 16 KiB pieces) — after pack, unpack,
+    offload and retrieve on every path the guards on both sides of each buffer still hold the poison, and so does every
+    pool-buffer byte outside the placement's stripes."""
+    k = KERNELS[kernel]
+    rng = np.random.default_rng(61)
+    dev = torch.device("cuda:0")
+    GUARD = 0x5AA5
+    for g, nphys, n_dev, w in ((W.Geometry(n_layers=1, n_kv_heads=1, head_dim=80), 67, 3, (3.0, 2.0, 1.0)),
+                               (W.Geometry(n_layers=1, n_kv_heads=3, head_dim=136), 41, 2, (2.0, 1.0)),
+                               (W.Geometry(n_layers=1, n_kv_heads=4, head_dim=128), 33, 4, (4.0, 2.0, 1.0, 1.0))):
+        table_np = np.ascontiguousarray(rng.permutation(nphys).astype(np.int32))          # every block, the first and the last included
+        wl = _custom(g, nphys, [table_np], n_dev, w)
+        elems, pad = g.kvb // 2, 3
+        src_cpu = W.kv_layer_numpy(wl, 0)
+        table = torch.from_numpy(table_np).to(dev)
+        opl = oracle.place(list(w), [nphys])
+        want = oracle.offload_layer(src_cpu, table_np, opl[0])
+
+        def guarded(fill_from=None):
+            """Two planes of (pad + nphys + pad) blocks each; returns (buffers, views of the nphys blocks in the middle)."""
+            bufs = [torch.full((nphys + 2 * pad, elems), GUARD, dtype=torch.int16, device=dev) for _ in range(2)]
+            mids = [b[pad:pad + nphys] for b in bufs]
+            for h in range(2):
+                mids[h].copy_(torch.from_numpy(fill_from[h].view(np.int16)).to(dev) if fill_from is not None
+                              else torch.full((nphys, elems), np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item(), dtype=torch.int16, device=dev))
+            return bufs, mids
+
+        def guards_intact(bufs):
+            return all(bool((b[:pad] == GUARD).all()) and bool((b[pad + nphys:] == GUARD).all()) for b in bufs)
+
+        sbufs, smid = guarded(src_cpu)
+        for path in (kv.PATH_STAGED, kv.PATH_ZEROCOPY):
+            pool = make_pool(wl)
+            try:
+                pool.set_path(path)
+                pool.set_tuning(kernel=k, link_kernel=k)
+                caps = [pool.device_info(i)["capacity"] for i in range(n_dev)]
+                hosts = [np.ctypeslib.as_array(ctypes.cast(pool.device_info(i)["host_base"], ctypes.POINTER(ctypes.c_uint8)), shape=(caps[i],))
+                         for i in range(n_dev)]
+                for h in hosts:
+                    h[:] = 0xC3                                                        # every pool byte; the stripes are then the only change
+                pl = pool.place([nphys])
+                # caller staging with red zones: exactly K*P bytes in the middle
+                stage_all = torch.full((nphys * g.payload + 2 * 4096,), 0x77, dtype=torch.uint8, device=dev)
+                stage = stage_all[4096:4096 + nphys * g.payload]
+                pool.pack(pl, 0, smid[0], smid[1], g.kvb, table, stage)
+                dbufs, dmid = guarded()
+                pool.unpack(pl, 0, dmid[0], dmid[1], g.kvb, table, stage)
+                torch.cuda.synchronize()
+                assert bool((stage_all[:4096] == 0x77).all()) and bool((stage_all[4096 + nphys * g.payload:] == 0x77).all())
+                assert np.array_equal(stage.cpu().numpy(), np.concatenate(want))
+                assert guards_intact(dbufs) and guards_intact(sbufs)
+                for h in range(2):
+                    assert np.array_equal(dmid[h].cpu().numpy().view(np.uint16), src_cpu[h])
+                # through the pool
+                pool.offload(pl, 0, smid[0], smid[1], g.kvb, table)
+                pool.wait_offloads(pl)
+                dbufs, dmid = guarded()
+                pool.retrieve(pl, 0, dmid[0], dmid[1], g.kvb, table)
+                torch.cuda.synchronize()
+                assert guards_intact(dbufs) and guards_intact(sbufs)
+                for h in range(2):
+                    assert np.array_equal(dmid[h].cpu().numpy().view(np.uint16), src_cpu[h])
+                for i in range(n_dev):
+                    loc, nb = pl.stripe_location(0, i)
+                    off = loc - pool.device_info(i)["host_base"]
+                    assert np.array_equal(hosts[i][off:off + nb], want[i])
+                    assert bool((hosts[i][:off] == 0xC3).all()) and bool((hosts[i][off + nb:] == 0xC3).all()), (path, i)
+                pl.release()
+            finally:
+                del hosts
+                pool.destroy()
