@@ -138,6 +138,7 @@ struct kvpool {
   uint32_t hbm_mask = 0;  // bit i: pool device i is GPU memory (KVPOOL_DEV_HBM): reached by the kernels directly, never staged or copied
   std::vector<StripeAllocator> alloc;
   std::vector<cudaStream_t> io;      // one I/O stream per pool device ("independent I/O streams"): host -> GPU copies
+  cudaStream_t join_out = nullptr;   // gathers an offload's copies for its `landed` event; carries no work of its own
   std::vector<cudaStream_t> io_out;  // and one for GPU -> host copies, so that an offload and a retrieve use both directions of the link at once
   std::vector<StageSlot> slots;
   uint64_t slot_bytes = 0;
@@ -197,6 +198,7 @@ void free_slots(kvpool* p) {
 int sync_pool_streams(kvpool* p) {
   for (auto s : p->io) CU(cudaStreamSynchronize(s));
   for (auto s : p->io_out) CU(cudaStreamSynchronize(s));
+  if (p->join_out) CU(cudaStreamSynchronize(p->join_out));
   return KVPOOL_OK;
 }
 
@@ -461,6 +463,7 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     if (p->table_arena) cudaFree(p->table_arena);
     if (p->table_arena_host) cudaFreeHost(p->table_arena_host);
     if (p->upload) cudaStreamDestroy(p->upload);
+    if (p->join_out) cudaStreamDestroy(p->join_out);
   };
   p->bufs.resize(n_devs);
   for (uint32_t i = 0; i < n_devs; ++i) {
@@ -490,7 +493,8 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     return fail(KVPOOL_ENOMEM, "create: table arena");
   }
   if (cudaHostAlloc(reinterpret_cast<void**>(&p->table_arena_host), kTableArenaBytes, cudaHostAllocDefault) != cudaSuccess ||
-      cudaStreamCreateWithFlags(&p->upload, cudaStreamNonBlocking) != cudaSuccess) {
+      cudaStreamCreateWithFlags(&p->upload, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&p->join_out, cudaStreamNonBlocking) != cudaSuccess) {
     cudaGetLastError();
     cleanup();
     return fail(KVPOOL_ENOMEM, "create: table arena mirror / upload stream");
@@ -513,6 +517,7 @@ int kvpool_destroy(kvpool_t* p) {
   if (p->table_arena) cudaFree(p->table_arena);
   if (p->table_arena_host) cudaFreeHost(p->table_arena_host);
   if (p->upload) cudaStreamDestroy(p->upload);
+  if (p->join_out) cudaStreamDestroy(p->join_out);
   for (auto e : p->ev_free) cudaEventDestroy(e);
   for (auto& r : p->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   for (auto e : p->prof_free) cudaEventDestroy(e);
@@ -888,9 +893,9 @@ int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, ui
   const uint64_t per_slot = p->slots.empty() ? 0 : blocks_per_slot(p);
   if (per_slot == 0) return fail(KVPOOL_ESTATE, "offload: no staging slot (the placement was made while the path was zero-copy)");
   mark_offloaded(L, first_block, n_blocks);
-  cudaStream_t lead = nullptr;  // gathers every copy of the layer, so that `landed` can mean "all stripes complete"
-  for (uint32_t i = 0; i < N && !lead; ++i)
-    if (L.map->counts[i] && !is_hbm(p, i)) lead = p->io_out[i];
+  // `landed` must mean "all stripes complete": it is recorded on a stream of the pool's own that carries no copies and only
+  // gathers every chunk's kernel and copies — the per-device I/O streams never wait for one another
+  cudaStream_t lead = p->join_out;
   if (L.landed_pending) CU(cudaStreamWaitEvent(lead, L.landed, 0));  // `landed` keeps covering what was offloaded before
   bool first_kernel = true;
   for (uint32_t first = first_block, end = first_block + n_blocks; first < end;) {
@@ -928,7 +933,7 @@ int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, ui
     }
     CU(cudaStreamWaitEvent(lead, slot.kernel_done, 0));  // covers the HBM-type stripes the kernel wrote
     for (uint32_t i = 0; i < N; ++i)
-      if ((slot.copies_after_kernel >> i & 1u) && p->io_out[i] != lead) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
+      if (slot.copies_after_kernel >> i & 1u) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
   }
   CU(cudaEventRecord(L.landed, lead));
   L.landed_pending = true;
