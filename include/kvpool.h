@@ -139,6 +139,15 @@ KVPOOL_API int kvpool_plan_layer(const uint64_t* w /*host[n]*/, uint32_t n, uint
  * never validates tables on the device; engines call this in debug builds or tests.  EINVAL with the first offending
  * entry in kvpool_last_error().  K = 0 is valid.                                                                  */
 KVPOOL_API int kvpool_validate_table(const int32_t* table /*host[K]*/, uint64_t K, uint64_t nphys);
+/* The same contract checked on the DEVICE, opt-in (hardening / debug builds; compute-sanitizer-free): with nphys > 0
+ * every later launch skips table entries outside [0, nphys) — the blocks they name are neither read nor written, so a
+ * corrupt table cannot touch another request's KV — and counts them (after an offload the pool slot of a rejected entry
+ * holds unspecified bytes).  One compare per 4-16 KiB piece: no measurable
+ * cost.  Duplicates are not detected (kvpool_validate_table does that on the host).  nphys = 0 (default) trusts the
+ * table.  kvpool_table_errors returns the number of rejected entries of the launches that have completed since the
+ * last call and resets it (blocking; the caller synchronises the streams it cares about first).                     */
+KVPOOL_API int kvpool_set_table_check(kvpool_t* pool, uint64_t nphys);
+KVPOOL_API int kvpool_table_errors(kvpool_t* pool, uint64_t* count_out /*host*/);
 
 /* ---- pool life cycle ----------------------------------------------------------------------------------
  * kvpool_create enumerates the pool devices: allocates one pinned, GPU-mapped host

@@ -29,7 +29,7 @@ EXPORTS = [
     "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release",
     "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
-    "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_validate_table", "kvpool_last_error", "kvpool_version",
+    "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_validate_table", "kvpool_set_table_check", "kvpool_table_errors", "kvpool_last_error", "kvpool_version",
 ]
 
 
@@ -74,6 +74,8 @@ def lib():
             "kvpool_plan_weights": [vp, c_uint32, vp],
             "kvpool_plan_layer": [vp, c_uint32, c_uint64, vp, vp, vp],
             "kvpool_validate_table": [vp, c_uint64, c_uint64],
+            "kvpool_set_table_check": [vp, c_uint64],
+            "kvpool_table_errors": [vp, vp],
             "kvpool_create": [vp, c_uint32, vp, c_int, c_uint32, POINTER(vp)],
             "kvpool_destroy": [vp],
             "kvpool_set_bandwidth": [vp, vp],
@@ -396,6 +398,14 @@ class KvPool:
         t, g = c_uint32(), c_int32()
         _ck(lib().kvpool_device_type(self.handle, dev, byref(t), byref(g)))
         return t.value, g.value
+
+    def set_table_check(self, nphys: int) -> None:
+        _ck(lib().kvpool_set_table_check(self.handle, int(nphys)))
+
+    def table_errors(self) -> int:
+        n = c_uint64()
+        _ck(lib().kvpool_table_errors(self.handle, byref(n)))
+        return n.value
 
     def stats(self) -> Tuple[int, int]:
         k, m = c_uint64(), c_uint64()

@@ -55,6 +55,15 @@ struct Piece {
   uint8_t* pooled;
   uint32_t bytes;
 };
+// Table check (opt-in, kvpool_set_table_check): a table entry outside the paged pool must neither be read nor written.
+// The piece is turned into a copy of the pool-side bytes onto themselves (harmless in both directions, and the bulk ring
+// keeps its load/store rhythm); the entry is counted once, by the lane that handles the first piece of its K block.
+__device__ __forceinline__ void reject(Piece& p, unsigned long long* bad, bool first_piece) {
+  p.paged = p.pooled;
+  if (first_piece && (threadIdx.x & 31u) == 0 && bad) atomicAdd(bad, 1ull);
+}
+
+template <bool CHECK = true>
 __device__ __forceinline__ Piece decode(const LayerArgs& a, uint64_t t, uint32_t pieces, uint32_t piece_bytes) {
   const uint32_t per_unit = 2u * pieces;
   const uint32_t local = static_cast<uint32_t>(t / per_unit);
@@ -70,9 +79,12 @@ __device__ __forceinline__ Piece decode(const LayerArgs& a, uint64_t t, uint32_t
   p.paged = (half ? a.v_base : a.k_base) + static_cast<uint64_t>(phys) * a.stride + off;
   p.pooled = reinterpret_cast<uint8_t*>(a.pool_base[d]) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;
   p.bytes = min(piece_bytes, a.kvb - off);
+  if constexpr (CHECK)
+    if (a.nphys_check && static_cast<uint32_t>(phys) >= a.nphys_check) reject(p, a.bad, r == 0);
   return p;
 }
 
+template <bool CHECK = true>
 __device__ __forceinline__ Piece decode(const MultiArgs& a, uint64_t t, uint32_t pieces, uint32_t piece_bytes) {
   const uint32_t per_unit = 2u * pieces;
   const uint32_t unit = static_cast<uint32_t>(t / per_unit);
@@ -95,6 +107,8 @@ __device__ __forceinline__ Piece decode(const MultiArgs& a, uint64_t t, uint32_t
   p.paged = (half ? L.v_base : L.k_base) + static_cast<uint64_t>(phys) * a.stride + off;
   p.pooled = reinterpret_cast<uint8_t*>(__ldg(L.pool_base + d) + a.delta[d]) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;
   p.bytes = min(piece_bytes, a.kvb - off);
+  if constexpr (CHECK)
+    if (a.nphys_check && static_cast<uint32_t>(phys) >= a.nphys_check) reject(p, a.bad, r == 0);
   return p;
 }
 __device__ __forceinline__ uint32_t units(const LayerArgs& a) { return a.K; }
@@ -172,7 +186,9 @@ __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wa
 
 // Each warp's lane 0 owns `stages` shared-memory buffers of `chunk` bytes and walks its share of the
 // layer's chunks: up to stages-1 loads are in flight while the oldest landed chunk is stored out.
-template <bool PACK, class Args>
+// CHECK: compiled with the opt-in table check (the single issuing lane is latency-bound: the unchecked build keeps the
+// check's compare and branch out of its loop — 2 % on an HBM-bound launch).
+template <bool PACK, class Args, bool CHECK>
 __global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Args a, uint32_t chunk, uint32_t stages) {
   extern __shared__ __align__(128) uint8_t smem[];
   if ((threadIdx.x & 31u) != 0) return;
@@ -192,7 +208,7 @@ __global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Args
   uint8_t* out_ring[8];  // destination of the chunk sitting in each stage (stages <= 8)
   auto issue = [&](uint64_t n) {
     const uint32_t s = static_cast<uint32_t>(n % stages);
-    const Piece p = decode(a, gw + n * ngw, pieces, chunk);
+    const Piece p = decode<CHECK>(a, gw + n * ngw, pieces, chunk);
     out_ring[s] = PACK ? p.pooled : p.paged;
     mbar_arrive_expect_tx(bar0 + 8u * s, chunk);
     bulk_g2s(buf0 + s * chunk, PACK ? p.paged : p.pooled, chunk, bar0 + 8u * s);
@@ -264,11 +280,20 @@ uint32_t bulk_chunk_for(uint32_t kvb, uint32_t want) {
 
 }  // namespace
 
+template <bool PACK, class Args, bool CHECK>
+static cudaError_t bulk_opt_in() {
+  return cudaFuncSetAttribute(kv_copy_bulk<PACK, Args, CHECK>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+}
+
 cudaError_t kernels_init() {
-  cudaError_t e = cudaFuncSetAttribute(kv_copy_bulk<true, LayerArgs>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(kv_copy_bulk<false, LayerArgs>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(kv_copy_bulk<true, MultiArgs>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(kv_copy_bulk<false, MultiArgs>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+  cudaError_t e = bulk_opt_in<true, LayerArgs, false>();
+  if (e == cudaSuccess) e = bulk_opt_in<false, LayerArgs, false>();
+  if (e == cudaSuccess) e = bulk_opt_in<true, MultiArgs, false>();
+  if (e == cudaSuccess) e = bulk_opt_in<false, MultiArgs, false>();
+  if (e == cudaSuccess) e = bulk_opt_in<true, LayerArgs, true>();
+  if (e == cudaSuccess) e = bulk_opt_in<false, LayerArgs, true>();
+  if (e == cudaSuccess) e = bulk_opt_in<true, MultiArgs, true>();
+  if (e == cudaSuccess) e = bulk_opt_in<false, MultiArgs, true>();
   return e;
 }
 
@@ -302,8 +327,13 @@ static cudaError_t launch_copy(const Args& a, uint32_t n_units, bool pack, const
     const uint64_t resident = static_cast<uint64_t>(cfg.sm_count ? cfg.sm_count : 148u) * (per_sm > 32 ? 32 : per_sm);
     uint64_t cap = cfg.ctas < resident ? cfg.ctas : resident;
     const uint32_t grid = static_cast<uint32_t>(want < cap ? want : cap);
-    if (pack) kv_copy_bulk<true, Args><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
-    else kv_copy_bulk<false, Args><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
+    if (a.nphys_check) {
+      if (pack) kv_copy_bulk<true, Args, true><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
+      else kv_copy_bulk<false, Args, true><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
+    } else {
+      if (pack) kv_copy_bulk<true, Args, false><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
+      else kv_copy_bulk<false, Args, false><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
+    }
   } else {
     const uint32_t unroll = cfg.vec_unroll == 4 ? 4 : (cfg.vec_unroll == 16 ? 16 : 8);
     const uint32_t threads = cfg.vec_threads ? cfg.vec_threads : kVecMaxThreads;

@@ -24,6 +24,8 @@ struct LayerArgs {
   uint32_t j0;   // ... starting at logical block j0 (table/dev/slot are indexed by j0 + local index)
   uint32_t kvb;
   unsigned long long* span;  // profiling only (else null): device {min start, max end} of the launch in %globaltimer ns
+  unsigned long long* bad;   // table check only (else null): counts table entries outside [0, nphys_check)
+  uint32_t nphys_check;      // 0 = the table is trusted (R12); else entries >= this (or negative) are skipped and counted
   uint64_t pool_base[kMaxDev];
 };
 
@@ -48,6 +50,8 @@ struct MultiArgs {
   uint32_t total_units;  // sum of K
   uint32_t pad;
   unsigned long long* span;  // as in LayerArgs
+  unsigned long long* bad;   // as in LayerArgs
+  uint32_t nphys_check, pad2;
   uint64_t delta[kMaxDev];  // added (mod 2^64) to pool_base[i]: 0 for the mapped host stripes themselves, or the
                             // displacement that maps device i's span of stripes onto its copy in a staging slot
   MultiDesc d[kMaxBatch];

@@ -154,6 +154,8 @@ struct kvpool {
   kvpool_tuning tune{};
   std::vector<kvpool_placement*> live;
   std::unordered_map<uint64_t, GltRef, GltHash> glt;  // keyed GLT: identifier -> (placement, layer, block)
+  uint32_t check_nphys = 0;              // kvpool_set_table_check: the kernels skip and count table entries outside [0, check_nphys)
+  unsigned long long* bad_d = nullptr;   // device counter of such entries
   uint64_t n_kernels = 0, n_memcpys = 0;
   bool profiling = false;
   std::vector<ProfRec> prof;
@@ -280,6 +282,8 @@ LayerArgs base_args(const kvpool* p, const LayerState& L, const void* k_base, co
   a.K = static_cast<uint32_t>(L.map->K);
   a.j0 = 0;
   a.kvb = static_cast<uint32_t>(p->kvb);
+  a.nphys_check = p->check_nphys;
+  a.bad = p->bad_d;
   return a;
 }
 
@@ -522,6 +526,7 @@ int kvpool_destroy(kvpool_t* p) {
   for (auto& r : p->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   for (auto e : p->prof_free) cudaEventDestroy(e);
   if (p->span_arena) cudaFree(p->span_arena);
+  if (p->bad_d) cudaFree(p->bad_d);
   delete p;
   return KVPOOL_OK;
 }
@@ -1075,6 +1080,8 @@ struct BatchCall {
 void fill_descs(const BatchCall& c, const LayerGroup& g, MultiArgs* ma) {
   ma->stride = c.stride;
   ma->kvb = static_cast<uint32_t>(c.p->kvb);
+  ma->nphys_check = c.p->check_nphys;
+  ma->bad = c.p->bad_d;
   ma->n = g.n;
   ma->total_units = 0;
   for (uint32_t b = 0; b < g.n; ++b) {
@@ -1600,6 +1607,33 @@ int kvpool_profile_read_clock(kvpool_t* p, int kind, double* total_ms, double* d
 
 int kvpool_profile_read(kvpool_t* p, int kind, double* total_ms, uint64_t* launches, uint64_t* bytes) {
   return kvpool_profile_read_clock(p, kind, total_ms, nullptr, launches, nullptr, bytes);
+}
+
+int kvpool_set_table_check(kvpool_t* p, uint64_t nphys) {
+  PoolLock lock__(p);
+  if (!p || nphys > 0x7fffffffull) return fail(KVPOOL_EINVAL, "set_table_check: null pool or nphys above 2^31-1");
+  DeviceGuard guard(p->cuda_device);
+  if (nphys && !p->bad_d) {
+    CU(cudaMalloc(reinterpret_cast<void**>(&p->bad_d), sizeof(unsigned long long)));
+    CU(cudaMemsetAsync(p->bad_d, 0, sizeof(unsigned long long), p->upload));
+    CU(cudaStreamSynchronize(p->upload));
+  }
+  p->check_nphys = static_cast<uint32_t>(nphys);
+  return KVPOOL_OK;
+}
+
+int kvpool_table_errors(kvpool_t* p, uint64_t* count_out) {
+  PoolLock lock__(p);
+  if (!p || !count_out) return fail(KVPOOL_EINVAL, "table_errors: null argument");
+  *count_out = 0;
+  if (!p->bad_d) return KVPOOL_OK;
+  DeviceGuard guard(p->cuda_device);
+  unsigned long long v = 0;
+  CU(cudaMemcpyAsync(&v, p->bad_d, sizeof(v), cudaMemcpyDeviceToHost, p->upload));
+  CU(cudaMemsetAsync(p->bad_d, 0, sizeof(v), p->upload));
+  CU(cudaStreamSynchronize(p->upload));
+  *count_out = v;
+  return KVPOOL_OK;
 }
 
 int kvpool_stats(const kvpool_t* p, uint64_t* kernel_launches, uint64_t* memcpy_calls) {

@@ -1029,3 +1029,80 @@ def test_red_zones_around_planes_stripes_and_staging_stay_intact(kernel):
             finally:
                 del hosts
                 pool.destroy()
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+@pytest.mark.parametrize("path", ["staged", "zerocopy"])
+def test_device_side_table_check_skips_and_counts_bad_entries(path, kernel):
+    """kvpool_set_table_check (R12, opt-in): table entries outside [0, nphys) are skipped — nothing outside the
+    planes is read or written (red zones intact), the other blocks move exactly as the oracle says — and counted; with
+    a clean table the check changes nothing."""
+    p, k = PATHS[path], KERNELS[kernel]
+    rng = np.random.default_rng(71)
+    dev = torch.device("cuda:0")
+    g = W.Geometry(n_layers=1, n_kv_heads=2, head_dim=80)                 # kvb = 5120 B, ragged against the 4 KiB piece
+    nphys, K, elems, pad, GUARD = 90, 64, g.kvb // 2, 4, 0x5AA5
+    good = np.ascontiguousarray(rng.permutation(nphys)[:K].astype(np.int32))
+    bad = good.copy()
+    bad_at = [3, 17, 40, 63]
+    bad[bad_at] = [nphys, -1, nphys + 2, 2 ** 31 - 1]                     # one past the end, negative, inside the guard, huge
+    wl = _custom(g, nphys, [good], 3, (3.0, 2.0, 1.0))
+    src_cpu = W.kv_layer_numpy(wl, 0)
+    opl = oracle.place([3.0, 2.0, 1.0], [K])
+    pool = make_pool(wl)
+    try:
+        pool.set_path(p)
+        pool.set_tuning(kernel=k, link_kernel=k)
+        pool.set_table_check(nphys)
+        pl = pool.place([K])
+
+        def guarded(fill):
+            bufs = [torch.full((nphys + 2 * pad, elems), GUARD, dtype=torch.int16, device=dev) for _ in range(2)]
+            for h in range(2):
+                bufs[h][pad:pad + nphys].copy_(torch.from_numpy(fill[h].view(np.int16)).to(dev))
+            return bufs, [b[pad:pad + nphys] for b in bufs]
+
+        sbufs, smid = guarded(src_cpu)
+        # clean table: identical to the unchecked path, zero errors
+        pool.offload(pl, 0, smid[0], smid[1], g.kvb, torch.from_numpy(good).to(dev))
+        pool.wait_offloads(pl)
+        torch.cuda.synchronize()
+        want = oracle.offload_layer(src_cpu, good, opl[0])
+        assert all(np.array_equal(pl.stripe(0, i), want[i]) for i in range(3)) and pool.table_errors() == 0
+        # bad table at retrieve: the four entries are skipped, everything else lands, guards intact
+        dbufs, dmid = guarded(W.poison_numpy((2, nphys, elems)))
+        pool.retrieve(pl, 0, dmid[0], dmid[1], g.kvb, torch.from_numpy(bad).to(dev))
+        torch.cuda.synchronize()
+        assert pool.table_errors() == len(bad_at) and pool.table_errors() == 0        # read and reset
+        ref = W.poison_numpy((2, nphys, elems))
+        ok = np.ones(K, bool); ok[bad_at] = False
+        ref[:, good[ok]] = src_cpu[:, good[ok]]
+        for h in range(2):
+            assert np.array_equal(dmid[h].cpu().numpy().view(np.uint16), ref[h])
+            assert bool((dbufs[h][:pad] == GUARD).all()) and bool((dbufs[h][pad + nphys:] == GUARD).all())
+        # bad table at offload: every other block lands; on the zero-copy path the skipped entries' slots keep what they held
+        fill = np.full_like(src_cpu, 0x2222)
+        fbufs, fmid = guarded(fill)
+        pool.offload(pl, 0, fmid[0], fmid[1], g.kvb, torch.from_numpy(good).to(dev))        # whole layer = 0x2222
+        pool.offload(pl, 0, smid[0], smid[1], g.kvb, torch.from_numpy(bad).to(dev))
+        pool.wait_offloads(pl)
+        torch.cuda.synchronize()
+        assert pool.table_errors() == len(bad_at)
+        want2 = oracle.offload_layer(fill, good, opl[0])
+        for j in np.flatnonzero(ok):
+            oracle.offload_range(src_cpu, good, opl[0], want2, int(j), 1)
+        got = [np.array(pl.stripe(0, i)) for i in range(3)]
+        P = g.payload
+        for j in range(K):                                                             # the pool slot of a rejected entry is unspecified on
+            d, sl = int(opl[0].dev[j]), int(opl[0].slot[j])                             # the staged path (its staging bytes were never written)
+            if ok[j] or path == "zerocopy":
+                assert np.array_equal(got[d][sl * P:(sl + 1) * P], want2[d][sl * P:(sl + 1) * P]), j
+        # check off again: trusted tables, counter stays at zero
+        pool.set_table_check(0)
+        pool.offload(pl, 0, smid[0], smid[1], g.kvb, torch.from_numpy(good).to(dev))
+        pool.wait_offloads(pl)
+        torch.cuda.synchronize()
+        assert all(np.array_equal(pl.stripe(0, i), want[i]) for i in range(3)) and pool.table_errors() == 0
+        pl.release()
+    finally:
+        pool.destroy()
