@@ -422,6 +422,17 @@ def run_kvpool(args) -> dict:
     clocks = sampler.stop(t_begin, t_end) if rank == 0 else None
     prof_clk = {kind: pool.profile_read_clock(kind) for kind in range(4)}
     prof = {kind: (v[0], v[2], v[4]) for kind, v in prof_clk.items()}
+    # one more step, untimed, with the timing events recorded on the launching streams themselves (kvpool.h: such a record
+    # holds its stream up for 25-47 us under a concurrent copy-engine transfer): reported beside the side-stream figure
+    pool.set_profiling(kv.PROFILE_INSTREAM)
+    step(True, {"place_ms": [], "offload_ms": [], "retrieve_ms": []})
+    pool.set_profiling(False)
+    prof_in = {kind: pool.profile_read_clock(kind) for kind in range(4)}
+    for kind, name in enumerate(("pack", "unpack", "zero-copy offload", "zero-copy retrieve")):
+        if prof_clk[kind][2]:
+            a, b_ = prof_clk[kind], prof_in[kind]
+            log(f"[rank {rank}] {name}: {a[2]} launches; mean per launch: side-stream events {1e3 * a[0] / a[2]:.1f} us, kernel clock "
+                f"{1e3 * a[1] / max(a[3], 1):.1f} us; in-stream events (extra step) {1e3 * b_[0] / max(b_[2], 1):.1f} us, kernel clock {1e3 * b_[1] / max(b_[3], 1):.1f} us")
 
     step_ms = 1e3 * (t_end - t_begin) / args.steps
     ret_ms = sum(rec["retrieve_ms"]) / args.steps
@@ -540,6 +551,12 @@ def run_kvpool(args) -> dict:
         roof = {"bound": "hbm", "kernel": kinds[dom], "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
                 "traffic": traffic, "peak_source": peaks["source"], "launches": n, "avg_launch_ms": ms / max(n, 1),
                 "algorithmic_bytes_per_launch": 2 * b // max(n, 1), "frac_of_8TBs_nominal": ach / 8000.0}
+        ims, _, inn, _, ib = prof_in[dom]
+        if inn and ims > 0:
+            roof.update({"achieved_instream_events": 2 * ib / (ims * 1e6), "frac_instream_events": 2 * ib / (ims * 1e6) / peaks["hbm_gbs"],
+                         "avg_launch_ms_instream_events": ims / inn})
+        roof["timing"] = ("CUDA timing events on two side streams of the pool, gated by non-timing marker events recorded on the launching "
+                          "stream right before and right after the kernel (kvpool_set_profiling, KVPOOL_PROFILE_SIDE)")
         _, dms, _, nd, _ = prof_clk[dom]
         if nd:
             # the same launches of the timed region by the kernels' own clock (%globaltimer: first CTA start to last CTA end)
@@ -587,13 +604,15 @@ def run_kvpool(args) -> dict:
         kn = "vec16" if tn.kernel == kv.KERNEL_VEC16 else "bulk"
         roof["achieved_back_to_back"] = hbm[f"{'pack' if dom == 0 else 'unpack'}_{kn}_back_to_back_gbps"]
         roof["frac_back_to_back"] = roof["achieved_back_to_back"] / peaks["hbm_gbs"]
-        roof["note"] = ("achieved = per-launch CUDA event pairs inside the timed step, where every pack/unpack launch runs while the copy "
-                        "engines stream the neighbouring layers over the host link; under such a stream an event pair with NOTHING between "
-                        "its records already reads empty_event_pair_under_dma_us (vs empty_event_pair_alone_us), a fixed cost that does not "
-                        "grow with the kernel (bench.py --interference, profiles/r1_interference.txt), and a plain torch copy_ of the same "
-                        "bytes pays the same; achieved_kernel_clock = the same in-step launches timed by the kernel itself (%globaltimer, "
-                        "first CTA start to last CTA end, stores fenced); achieved_back_to_back = same kernel, 16 launches per event pair, "
-                        "no concurrent copy")
+        roof["note"] = ("achieved = per-launch CUDA timing-event pairs inside the timed step, where every pack/unpack launch runs while the "
+                        "copy engines stream the neighbouring layers over the host link; the events sit on side streams behind non-timing "
+                        "markers (see timing) because a timing event recorded on the launching stream holds that stream up until its "
+                        "timestamp is written - empty_event_pair_under_dma_us with nothing between the records, vs "
+                        "empty_event_pair_alone_us - which delays the kernel and counts the delay: achieved_instream_events is that "
+                        "measurement (one extra untimed step), and a plain torch copy_ of the same bytes timed that way pays the same "
+                        "(torch_copy_same_bytes_under_dma_gbps; bench.py --interference, profiles/r1_interference.txt); "
+                        "achieved_kernel_clock = the same in-step launches timed by the kernel itself (%globaltimer, first CTA start to "
+                        "last CTA end, stores fenced); achieved_back_to_back = same kernel, 16 launches per event pair, no concurrent copy")
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms,

@@ -51,6 +51,11 @@ enum {
   KVPOOL_ENOENT = -6  /* kvpool_glt_find: no KV cache with that identifier */
 };
 
+/* kvpool_set_profiling modes */
+#define KVPOOL_PROFILE_OFF 0
+#define KVPOOL_PROFILE_SIDE 1
+#define KVPOOL_PROFILE_INSTREAM 2
+
 /* pool-device flags */
 #define KVPOOL_DEV_WRITE_COMBINED 1u /* cudaHostAllocWriteCombined (GPU-read-mostly; CPU reads become slow) */
 #define KVPOOL_DEV_NUMA_STRICT 2u    /* fail with ENUMA instead of falling back when binding is impossible */
@@ -326,8 +331,12 @@ KVPOOL_API int kvpool_layer_map(const kvpool_placement_t* pl, uint32_t layer, ui
 KVPOOL_API int kvpool_stats(const kvpool_t* pool, uint64_t* kernel_launches, uint64_t* memcpy_calls);
 
 /* Per-kernel timing for the roofline report.  While enabled, every kernel the library launches is bracketed by a
- * CUDA event pair recorded on the launching stream after all of the launch's stream waits (so a pair spans the
- * kernel alone, not the transfers it waited for).  kvpool_profile_read blocks until the recorded pairs of `kind`
+ * CUDA timing-event pair taken after all of the launch's stream waits (so a pair spans the kernel alone, not the
+ * transfers it waited for).  enabled = KVPOOL_PROFILE_SIDE (1): the launching stream only gets two non-timing marker
+ * events and the timing events are recorded on two side streams of the pool behind those markers — a TIMING event
+ * recorded on the launching stream itself holds that stream up until its timestamp is written (3 us on an idle GPU,
+ * 25-47 us under a concurrent copy-engine transfer over the host link), which both delays the kernel and counts the
+ * delay.  KVPOOL_PROFILE_INSTREAM (2) records the pair on the launching stream anyway, for comparison.  kvpool_profile_read blocks until the recorded pairs of `kind`
  * have completed, returns their summed duration, count and algorithmic bytes (K_l*P per launch), and clears them.
  * kind: 0 = in-device pack, 1 = in-device unpack, 2 = zero-copy offload, 3 = zero-copy retrieve.               */
 KVPOOL_API int kvpool_set_profiling(kvpool_t* pool, int enabled);

@@ -20,6 +20,7 @@ OK, EINVAL, ENOMEM, ECUDA, ENUMA, ESTATE, ENOENT = 0, -1, -2, -3, -4, -5, -6
 DEV_WRITE_COMBINED, DEV_NUMA_STRICT, DEV_HBM, DEV_CUDA_HOSTALLOC = 1, 2, 4, 8
 TYPE_MEM, TYPE_SSD, TYPE_HBM = 0, 1, 2
 NUMA_AUTO = -2
+PROFILE_OFF, PROFILE_SIDE, PROFILE_INSTREAM = 0, 1, 2
 PATH_AUTO, PATH_STAGED, PATH_ZEROCOPY = 0, 1, 2
 KERNEL_VEC16, KERNEL_BULK = 0, 1
 _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA", ESTATE: "ESTATE", ENOENT: "ENOENT"}
@@ -415,7 +416,8 @@ class KvPool:
 
     PROF_PACK, PROF_UNPACK, PROF_ZC_OFFLOAD, PROF_ZC_RETRIEVE = 0, 1, 2, 3
 
-    def set_profiling(self, enabled: bool) -> None:
+    def set_profiling(self, enabled) -> None:
+        """False / True (= PROFILE_SIDE: timing events on side streams behind non-timing markers) / PROFILE_INSTREAM."""
         _ck(lib().kvpool_set_profiling(self.handle, int(enabled)))
 
     def profile_read(self, kind: int) -> Tuple[float, int, int]:
