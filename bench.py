@@ -928,6 +928,35 @@ def run_interference(args) -> None:
         t = [time_under_dma(torch, s, o, k_n, bg, launches=8) for bg in (None, bg_h2d, bg_d2h)]
         print(f"{mib:6d} {nk:3d} {t[0]:9.1f} {t[1]:9.1f} {t[2]:9.1f} {t[1] - t[0]:7.1f} {t[2] - t[0]:7.1f}", flush=True)
         del a_, b_
+
+    # what one event record costs its stream: k records back to back inside one timing pair, timing vs non-timing events
+    print("# k event records back to back on one stream inside ONE timing pair, median of 6: us per record = (t(k=64) - t(k=16)) / 48, "
+          "alone / +H2D / +D2H")
+
+    def per_record(timing: bool, bg) -> float:
+        out = {}
+        for k in (16, 64):
+            ts = []
+            for rep in range(8):
+                torch.cuda.synchronize()
+                if bg:
+                    bg()
+                    time.sleep(0.005)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                evs = [torch.cuda.Event(enable_timing=timing) for _ in range(k)]
+                e0.record(s)
+                for e in evs:
+                    e.record(s)
+                e1.record(s)
+                torch.cuda.synchronize()
+                if rep >= 2:
+                    ts.append(1e3 * e0.elapsed_time(e1))
+            out[k] = statistics.median(ts)
+        return (out[64] - out[16]) / 48
+
+    for label, timing in (("timing events (cudaEventDefault)", True), ("non-timing events (cudaEventDisableTiming)", False)):
+        t = [per_record(timing, bg) for bg in (None, bg_h2d, bg_d2h)]
+        print(f"{label:46s} {t[0]:9.2f} {t[1]:9.2f} {t[2]:9.2f}", flush=True)
     pl.release()
     pool.destroy()
 
