@@ -66,9 +66,6 @@ def parse_args():
     ap.add_argument("--blocked-io", action="store_true",
                     help="blocked-I/O-time analog (PAPER.md:70-72, Fig. 2/4): retrieve + consumer stand-in per layer, serial vs layerwise "
                          "pipelined, over context lengths 1K..128K for the three model shapes")
-    ap.add_argument("--interference", action="store_true",
-                    help="in-device pack/unpack and a plain torch copy of the same size, alone and under a concurrent cudaMemcpyAsync over "
-                         "the host link (explains the in-step kernel time of the staged path)")
     ap.add_argument("--mixed-pool", action="store_true",
                     help="HBM-type pool devices (KVPOOL_DEV_HBM; the pool's own GPU standing in for an NVLink peer) next to a pinned "
                          "host device: bandwidth-proportional split by measured weights, offload / retrieve GB/s (DESIGN.md §11)")
@@ -77,9 +74,6 @@ def parse_args():
                          "GB/s against simultaneous cudaMemcpyAsync in both directions")
     ap.add_argument("--hostalloc", action="store_true", help="pool buffers from cudaHostAlloc (KVPOOL_DEV_CUDA_HOSTALLOC) instead of the default "
                     "huge-page mapping + cudaHostRegister; main run and --duplex")
-    ap.add_argument("--pool-create", action="store_true",
-                    help="side mode: time kvpool_create of one pool buffer, default (huge pages faulted in in parallel + cudaHostRegister) "
-                         "vs KVPOOL_DEV_CUDA_HOSTALLOC, and the link bandwidth from each, pass by pass; text table")
     ap.add_argument("--compute-us", type=float, default=0.0, help="--blocked-io: extra calibrated compute per layer (kvpool_spin), microseconds")
     ap.add_argument("--detail", default=None, help="write per-layer latencies and side measurements to this JSON file")
     return ap.parse_args()
@@ -610,7 +604,7 @@ def run_kvpool(args) -> dict:
                         "timestamp is written - empty_event_pair_under_dma_us with nothing between the records, vs "
                         "empty_event_pair_alone_us - which delays the kernel and counts the delay: achieved_instream_events is that "
                         "measurement (one extra untimed step), and a plain torch copy_ of the same bytes timed that way pays the same "
-                        "(torch_copy_same_bytes_under_dma_gbps; bench.py --interference, profiles/r1_interference.txt); "
+                        "(torch_copy_same_bytes_under_dma_gbps; profiles/r1_interference.txt); "
                         "achieved_kernel_clock = the same in-step launches timed by the kernel itself (%globaltimer, first CTA start to "
                         "last CTA end, stores fenced); achieved_back_to_back = same kernel, 16 launches per event pair, no concurrent copy")
 
@@ -831,136 +825,6 @@ def time_under_dma(torch, s, o, fn, bg, launches: int = 16, reps: int = 4):
     return best
 
 
-def run_interference(args) -> None:
-    """The staged path overlaps the unpack (pack) of layer l with the host->GPU (GPU->host) copies of the next layers.  This
-    table times the HBM-bound kernels alone and while a copy engine streams over the host link, next to a plain
-    torch `copy_` of the same bytes (a kernel this repo did not write) under the same conditions.  Text table on stdout."""
-    import torch
-    from paper_2606_14779_b200 import binding as kv
-    from paper_2606_14779_b200 import workloads as W
-
-    dev = torch.device("cuda", 0)
-    torch.cuda.set_device(dev)
-    NL = 8
-    wl = W.make_workload(args.config, n_layers=NL)
-    wl.sliding_layers = ()
-    g, R = wl.geom, len(wl.requests) - 1
-    K = int(wl.blocks_per_layer(R)[0])
-    nbytes = K * g.payload
-    pool = kv.KvPool([1.0], [NL * nbytes + (64 << 20)], n_layers=NL, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim)
-    pool.set_path(kv.PATH_ZEROCOPY)          # only kvpool_pack / kvpool_unpack are called: no staging ring needed
-    pl = pool.place([K] * NL)
-    kvt = [W.kv_layer_torch(wl, l, dev) for l in range(NL)]
-    tables = [torch.from_numpy(np.ascontiguousarray(wl.layer_table(R, l))).to(dev) for l in range(NL)]
-    stages = [torch.empty(nbytes, dtype=torch.uint8, device=dev) for _ in range(4)]
-    flat_a = [torch.empty(nbytes, dtype=torch.uint8, device=dev) for _ in range(4)]
-    big_d = torch.empty(2 << 30, dtype=torch.uint8, device=dev)
-    big_h = torch.empty(2 << 30, dtype=torch.uint8).pin_memory()
-    s, o = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
-    torch.cuda.synchronize()
-
-    def k_unpack(i):
-        pool.unpack(pl, i % NL, kvt[i % NL][0], kvt[i % NL][1], g.kvb, tables[i % NL], stages[i % 4], s)
-
-    def k_pack(i):
-        pool.pack(pl, i % NL, kvt[i % NL][0], kvt[i % NL][1], g.kvb, tables[i % NL], stages[i % 4], s)
-
-    def k_copy(i):
-        with torch.cuda.stream(s):
-            stages[i % 4].copy_(flat_a[(i + 1) % 4], non_blocking=True)
-
-    def bg_h2d():
-        with torch.cuda.stream(o):
-            big_d.copy_(big_h, non_blocking=True)
-
-    def bg_d2h():
-        with torch.cuda.stream(o):
-            big_h.copy_(big_d, non_blocking=True)
-
-    def measure(fn, bg):
-        return time_under_dma(torch, s, o, fn, bg)
-
-    def device_clock_us(fn, bg, kind):
-        """Mean in-kernel span (%globaltimer, first CTA start to last CTA end) of the same launches under the same condition."""
-        for k in range(4):
-            pool.profile_read_clock(k)
-        pool.set_profiling(True)
-        try:
-            measure(fn, bg)
-        finally:
-            pool.set_profiling(False)
-        _, dms, _, nd, _ = pool.profile_read_clock(kind)
-        return 1e3 * dms / max(nd, 1)
-
-    peak = measured_peaks()["hbm_gbs"]
-    print(f"# bench.py --interference --config {args.config}: {wl.name}, {nbytes / 2**20:.0f} MiB read + {nbytes / 2**20:.0f} MiB written per launch; "
-          f"'us' = one CUDA event pair per launch, 16 launches, median, best of 3; 'clk' = the same launches by the kernels' own clock "
-          f"(%globaltimer span, first CTA start to last CTA end, mean); GB/s = 2*bytes/event time; measured HBM copy peak {peak:.0f} GB/s")
-    print(f"{'kernel':46s} {'alone us':>9s} {'clk':>6s} {'GB/s':>6s} {'+H2D us':>9s} {'clk':>6s} {'GB/s':>6s} {'+D2H us':>9s} {'clk':>6s} {'GB/s':>6s}")
-    rows = [("kv_copy_vec16 unpack (stage -> paged)", k_unpack, kv.KERNEL_VEC16, kv.KvPool.PROF_UNPACK), ("kv_copy_vec16 pack (paged -> stage)", k_pack, kv.KERNEL_VEC16, kv.KvPool.PROF_PACK),
-            ("kv_copy_bulk unpack", k_unpack, kv.KERNEL_BULK, kv.KvPool.PROF_UNPACK), ("kv_copy_bulk pack", k_pack, kv.KERNEL_BULK, kv.KvPool.PROF_PACK),
-            ("torch copy_ (contiguous D2D kernel, same bytes)", k_copy, None, None),
-            ("empty event pair (no kernel between the records)", lambda i: None, None, None)]
-    for name, fn, kid, kind in rows:
-        if kid is not None:
-            pool.set_tuning(kernel=kid)
-        for i in range(4):
-            fn(i)
-        t = [measure(fn, bg) for bg in (None, bg_h2d, bg_d2h)]
-        c = [device_clock_us(fn, bg, kind) if kind is not None else None for bg in (None, bg_h2d, bg_d2h)]
-        gbs = [f"{2 * nbytes / t[q] / 1e3:6.0f}" if not name.startswith("empty") else "     -" for q in range(3)]
-        cells = "".join(f" {t[q]:9.1f} {(f'{c[q]:6.1f}' if c[q] is not None else '     -')} {gbs[q]}" for q in range(3))
-        print(f"{name:46s}{cells}", flush=True)
-
-    # fixed or proportional?  per launch or per event pair?  (a kernel this repo did not write: contiguous torch copy_)
-    print("# torch copy_ of n MiB (read n + write n), nk launches inside ONE event pair, 8 pairs, median, best of 3: event-pair us alone / +H2D / +D2H "
-          "and the excess over alone")
-    print(f"{'MiB':>6s} {'nk':>3s} {'alone':>9s} {'+H2D':>9s} {'+D2H':>9s} {'dH2D':>7s} {'dD2H':>7s}")
-    del stages, flat_a
-    for mib, nk in [(16, 1), (64, 1), (256, 1), (1024, 1), (2048, 1), (64, 2), (64, 4), (64, 8), (256, 2), (256, 4), (256, 8)]:
-        a_, b_ = torch.empty(mib << 20, dtype=torch.uint8, device=dev), torch.empty(mib << 20, dtype=torch.uint8, device=dev)
-
-        def k_n(i, a_=a_, b_=b_, nk=nk):
-            with torch.cuda.stream(s):
-                for _ in range(nk):
-                    b_.copy_(a_, non_blocking=True)
-
-        t = [time_under_dma(torch, s, o, k_n, bg, launches=8) for bg in (None, bg_h2d, bg_d2h)]
-        print(f"{mib:6d} {nk:3d} {t[0]:9.1f} {t[1]:9.1f} {t[2]:9.1f} {t[1] - t[0]:7.1f} {t[2] - t[0]:7.1f}", flush=True)
-        del a_, b_
-
-    # what one event record costs its stream: k records back to back inside one timing pair, timing vs non-timing events
-    print("# k event records back to back on one stream inside ONE timing pair, median of 6: us per record = (t(k=64) - t(k=16)) / 48, "
-          "alone / +H2D / +D2H")
-
-    def per_record(timing: bool, bg) -> float:
-        out = {}
-        for k in (16, 64):
-            ts = []
-            for rep in range(8):
-                torch.cuda.synchronize()
-                if bg:
-                    bg()
-                    time.sleep(0.005)
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                evs = [torch.cuda.Event(enable_timing=timing) for _ in range(k)]
-                e0.record(s)
-                for e in evs:
-                    e.record(s)
-                e1.record(s)
-                torch.cuda.synchronize()
-                if rep >= 2:
-                    ts.append(1e3 * e0.elapsed_time(e1))
-            out[k] = statistics.median(ts)
-        return (out[64] - out[16]) / 48
-
-    for label, timing in (("timing events (cudaEventDefault)", True), ("non-timing events (cudaEventDisableTiming)", False)):
-        t = [per_record(timing, bg) for bg in (None, bg_h2d, bg_d2h)]
-        print(f"{label:46s} {t[0]:9.2f} {t[1]:9.2f} {t[2]:9.2f}", flush=True)
-    pl.release()
-    pool.destroy()
-
-
 def run_mixed_pool(args) -> None:
     """Eq. 1-2 at work on devices of very different speed: one pinned host buffer (PCIe) and one HBM-type device, alone and
     together, weights = kvpool_measure_bandwidth of each.  Whole request (16 layers of --config), batched calls, legs
@@ -1125,48 +989,6 @@ def run_duplex(args) -> None:
     pool.destroy()
 
 
-def run_pool_create(args) -> None:
-    """kvpool_create pins the pool ("at model initialization"; 20 GB of host memory in the paper's setup,
-    PAPER.md:106).  Times the creation of ONE pool buffer of 1, 8 and 32 GiB both ways, then the link from a fresh buffer
-    pass by pass: pages the CPU has just zeroed read ~5 % slow host->GPU until a DMA write has claimed them (every stripe is
-    written by an offload before a retrieve reads it; kvpool_measure_bandwidth does the same before it measures)."""
-    import torch
-    from paper_2606_14779_b200 import binding as kv
-
-    torch.cuda.set_device(0)
-    torch.cuda.init()
-    import ctypes
-    rt = ctypes.CDLL("libcudart.so.12")          # the runtime already in the process; only for the raw passes below
-    rt.cudaMemcpy.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int]
-    scratch = torch.empty(1 << 30, dtype=torch.uint8, device="cuda:0")
-
-    def raw_pass(host_ptr: int, to_gpu: bool) -> float:     # one blocking 1 GiB cudaMemcpy, no warm-up, host clock
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        rc = rt.cudaMemcpy(scratch.data_ptr(), host_ptr, 1 << 30, 1) if to_gpu else rt.cudaMemcpy(host_ptr, scratch.data_ptr(), 1 << 30, 2)
-        assert rc == 0, rc
-        return (1 << 30) / (time.perf_counter() - t0) / 1e9
-
-    flavours = (("default: 2 MiB-aligned mmap + MADV_HUGEPAGE + parallel first touch + cudaHostRegister", 0),
-                ("KVPOOL_DEV_CUDA_HOSTALLOC: cudaHostAlloc", kv.DEV_CUDA_HOSTALLOC))
-    print(f"kvpool_create of one pool buffer ({len(os.sched_getaffinity(0))} host cores)")
-    for gib in (1, 8, 32):
-        for name, flags in flavours:
-            t0 = time.perf_counter()
-            pool = kv.KvPool([1.0], [gib << 30], n_layers=1, n_kv_heads=4, head_dim=128, dev_flags=[flags])
-            dt = time.perf_counter() - t0
-            line = f"  {gib:3d} GiB  {dt:6.2f} s  {gib * 2**30 / dt / 1e9:6.2f} GB/s  {name}"
-            if gib == 1:
-                host = pool.device_info(0)["host_base"]
-                h = [raw_pass(host, True) for _ in range(8)]
-                d = [raw_pass(host, False) for _ in range(2)]
-                h2 = [raw_pass(host, True) for _ in range(3)]
-                line += ("\n           host->GPU passes over the fresh buffer " + " ".join(f"{x:.1f}" for x in h) +
-                         "; GPU->host " + " ".join(f"{x:.1f}" for x in d) + "; host->GPU again " + " ".join(f"{x:.1f}" for x in h2) + " GB/s")
-            print(line, flush=True)
-            pool.destroy()
-
-
 def run_blocked_io(args) -> None:
     """Blocked I/O time = time during which only KV retrieval proceeds, with no overlapping GPU computation.
     Consumer stand-in per layer = kvpool_checksum over the layer's retrieved blocks (reads K_l*P bytes through the block
@@ -1294,17 +1116,11 @@ def main():
     if args.variants:
         run_variants(args)
         return
-    if args.interference:
-        run_interference(args)
-        return
     if args.mixed_pool:
         run_mixed_pool(args)
         return
     if args.duplex:
         run_duplex(args)
-        return
-    if args.pool_create:
-        run_pool_create(args)
         return
     out = run_kvpool(args)
     if out is None:
