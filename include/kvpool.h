@@ -47,14 +47,9 @@ enum {
   KVPOOL_ENOMEM = -2, /* a pool device has no room for its stripe, or host/device allocation failed */
   KVPOOL_ECUDA = -3,  /* a CUDA runtime call failed (message has the CUDA error string) */
   KVPOOL_ENUMA = -4,  /* KVPOOL_DEV_NUMA_STRICT and the pages could not be bound to the requested node */
-  KVPOOL_ESTATE = -5, /* retrieve of a layer that was never offloaded; release with work in flight; ... */
+  KVPOOL_ESTATE = -5, /* retrieve of a layer that was never offloaded; set_bandwidth while placements are live; ... */
   KVPOOL_ENOENT = -6  /* kvpool_glt_find: no KV cache with that identifier */
 };
-
-/* kvpool_set_profiling modes */
-#define KVPOOL_PROFILE_OFF 0
-#define KVPOOL_PROFILE_SIDE 1
-#define KVPOOL_PROFILE_INSTREAM 2
 
 /* pool-device flags */
 #define KVPOOL_DEV_WRITE_COMBINED 1u /* cudaHostAllocWriteCombined (GPU-read-mostly; CPU reads become slow) */
@@ -126,6 +121,9 @@ typedef struct {         /* kvpool_set_tuning; 0 in any field = library default 
                             consecutive logical blocks (copies of chunk c+1 overlap the pack/unpack of chunk c), so the
                             staging ring (stage_slots x this) does not grow with the context length.  Default: off (a slot
                             holds the largest layer); UINT64_MAX turns it off again; at least one block per chunk           */
+  uint32_t pdl;          /* programmatic dependent launch of the library's kernels (the next layer's launch latency and
+                            ramp hide under the current layer's kernel): 1 = on (default), 2 = off                          */
+  uint32_t reserved;     /* 0                                                                                             */
 } kvpool_tuning;
 
 /* ---- pure host arithmetic (no CUDA, no pool) --------------------------------------------------------
@@ -195,8 +193,23 @@ KVPOOL_API int kvpool_reserve_staging(kvpool_t* pool, uint64_t bytes);
  * kvpool_reserve_staging).  ENOMEM (nothing reserved) if some pool
  * device cannot hold its stripes.                                                                      */
 KVPOOL_API int kvpool_place(kvpool_t* pool, const uint32_t* blocks_per_layer /*host[n_layers]*/, kvpool_placement_t** out);
-/* Frees the stripes and tables.  The caller must have synchronised the streams it used with it.        */
+/* Frees the stripes and tables.  Waits first (host-blocking) for the library's own transfers and for the last work
+ * each hot-path call enqueued with this placement on the caller's streams, so the stripes cannot be handed to another
+ * request while a kernel still reads or writes them.  (Calls made while a stream was being captured into a CUDA graph
+ * are not tracked: a graph that names the placement must not be launched after the release.)                       */
 KVPOOL_API int kvpool_release(kvpool_t* pool, kvpool_placement_t* pl);
+
+/* A request's block tables in ONE upload (a 1K-token request moves 4 MiB per layer: a separate table copy per layer costs
+ * more than the layer's own transfer time).  tables_host (host; pageable or pinned; free again when the call returns) is
+ * the concatenation, in layer order, of the K_l int32 entries of every layer of the placement — n_entries must equal
+ * sum_l K_l; layers with K_l = 0 contribute nothing.  One cudaMemcpyAsync on `stream` into device memory the placement
+ * owns.  Afterwards every hot-path call on this placement accepts block_table_dev = NULL (per-layer calls) or
+ * block_tables = NULL / NULL entries (batched calls) and then reads the uploaded table of that layer; such a call must be
+ * ordered after the upload (same stream, or an event).  May be called again to replace the tables (it then first waits,
+ * host-blocking, for the work enqueued with the placement so far).
+ * EINVAL on a wrong entry count; entries are not validated (R12).                                          */
+KVPOOL_API int kvpool_set_tables(kvpool_t* pool, kvpool_placement_t* pl, const int32_t* tables_host /*host[sum K_l]*/, uint64_t n_entries,
+                      void* cuda_stream);
 
 /* ---- the hot path: one layer ---------------------------------------------------------------------------
  * k_base / v_base: device pointers to the layer's K and V planes; physical block p is the kvb bytes at
@@ -259,14 +272,6 @@ KVPOOL_API int kvpool_retrieve_range(kvpool_t* pool, kvpool_placement_t* pl, uin
 KVPOOL_API int kvpool_offload_range(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks,
                          const void* k_base /*device*/, const void* v_base /*device*/, uint64_t block_stride_bytes,
                          const int32_t* block_table_dev /*device[K_l]*/, void* cuda_stream);
-/* Comparison baseline, not a product path: what an engine without a gather kernel does — one cudaMemcpyAsync per
- * K block and per V block (2*K_l calls) straight between the paged blocks and the stripes, all on `stream`.
- * block_table_host is the HOST copy of the layer's table.  Same results as kvpool_offload / kvpool_retrieve;
- * exists so that bench.py --variants can time it next to the kernel paths.                                        */
-KVPOOL_API int kvpool_offload_naive(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, const void* k_base /*device*/,
-                         const void* v_base /*device*/, uint64_t block_stride_bytes, const int32_t* block_table_host, void* cuda_stream);
-KVPOOL_API int kvpool_retrieve_naive(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, void* k_base /*device*/, void* v_base /*device*/,
-                          uint64_t block_stride_bytes, const int32_t* block_table_host, void* cuda_stream);
 /* Make `stream` wait until every offload enqueued so far with `pl` has landed in the pool.             */
 KVPOOL_API int kvpool_wait_offloads(kvpool_t* pool, kvpool_placement_t* pl, void* cuda_stream);
 /* Block the host until all work the pool enqueued on its own streams is done (not the caller's), and note which
@@ -283,17 +288,6 @@ KVPOOL_API int kvpool_pack(kvpool_t* pool, kvpool_placement_t* pl, uint32_t laye
                 uint64_t block_stride_bytes, const int32_t* block_table_dev, void* stage_dev, void* cuda_stream);
 KVPOOL_API int kvpool_unpack(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base,
                   uint64_t block_stride_bytes, const int32_t* block_table_dev, const void* stage_dev, void* cuda_stream);
-
-/* Consumer stand-in and integrity check (the "GPU computation" box of Fig. 2, for pipeline
- * experiments; not part of the paper's method).  Adds to *sum_dev (device uint64, caller zeroes it) the checksum
- *     sum over logical blocks j < n_blocks, halves h (0 = K, 1 = V), 64-bit little-endian words i of
- *         word(j, h, i) * (2*idx + 1)   mod 2^64,      idx = (j*2 + h)*(kvb/8) + i
- * of the paged blocks named by block_table_dev, reading them through the table as decode attention would
- * (n_blocks*P bytes of HBM reads).  kvb must be a multiple of 16.  Ordered on `stream`.                          */
-KVPOOL_API int kvpool_checksum(kvpool_t* pool, const void* k_base /*device*/, const void* v_base /*device*/, uint64_t block_stride_bytes,
-                    const int32_t* block_table_dev, uint32_t n_blocks, uint64_t* sum_dev /*device*/, void* cuda_stream);
-/* Occupy `stream` for `nanoseconds` with a one-thread kernel (calibrated compute stand-in).                        */
-KVPOOL_API int kvpool_spin(kvpool_t* pool, uint64_t nanoseconds, void* cuda_stream);
 
 /* ---- introspection (GLT, Table I) -----------------------------------------------------------------------*/
 KVPOOL_API int kvpool_n_devices(const kvpool_t* pool, uint32_t* n_out);
@@ -327,29 +321,6 @@ KVPOOL_API int kvpool_glt_find(kvpool_t* pool, uint64_t id, uint64_t* key, uint3
                     kvpool_placement_t** pl, uint32_t* layer, uint32_t* block);
 /* Whole-layer copies of the dense GLT columns (host[K_l] each; either may be NULL).                    */
 KVPOOL_API int kvpool_layer_map(const kvpool_placement_t* pl, uint32_t layer, uint8_t* dev_out, uint32_t* slot_out);
-/* Work counters since create: kernels launched and cudaMemcpyAsync calls issued by the library.        */
-KVPOOL_API int kvpool_stats(const kvpool_t* pool, uint64_t* kernel_launches, uint64_t* memcpy_calls);
-
-/* Per-kernel timing for the roofline report.  While enabled, every kernel the library launches is bracketed by a
- * CUDA timing-event pair taken after all of the launch's stream waits (so a pair spans the kernel alone, not the
- * transfers it waited for).  enabled = KVPOOL_PROFILE_SIDE (1): the launching stream only gets two non-timing marker
- * events and the timing events are recorded on two side streams of the pool behind those markers — a TIMING event
- * recorded on the launching stream itself holds that stream up until its timestamp is written (3 us on an idle GPU,
- * 25-47 us under a concurrent copy-engine transfer over the host link), which both delays the kernel and counts the
- * delay.  KVPOOL_PROFILE_INSTREAM (2) records the pair on the launching stream anyway, for comparison.  kvpool_profile_read blocks until the recorded pairs of `kind`
- * have completed, returns their summed duration, count and algorithmic bytes (K_l*P per launch), and clears them.
- * kind: 0 = in-device pack, 1 = in-device unpack, 2 = zero-copy offload, 3 = zero-copy retrieve.               */
-KVPOOL_API int kvpool_set_profiling(kvpool_t* pool, int enabled);
-KVPOOL_API int kvpool_profile_read(kvpool_t* pool, int kind, double* total_ms, uint64_t* launches, uint64_t* bytes);
-/* The same read plus the kernels' own clock: while profiling is on, every CTA of a launch folds its start and its end
- * (%globaltimer, after its stores are globally visible) into a per-launch {min start, max end} pair in device memory;
- * device_ms is the sum of (max end - min start) over the device_launches launches that got such a pair (the first
- * 16384 between two reads that empty the record list).  The event pairs of total_ms also count what the stream's front
- * end adds around a launch — ~5 us on an idle GPU, 20-35 us while a copy engine streams over the host link (an empty
- * event pair measures the same) — device_ms does not.  Any out pointer may be NULL.                   */
-KVPOOL_API int kvpool_profile_read_clock(kvpool_t* pool, int kind, double* total_ms, double* device_ms, uint64_t* launches,
-                              uint64_t* device_launches, uint64_t* bytes);
-
 KVPOOL_API const char* kvpool_last_error(void);
 KVPOOL_API const char* kvpool_version(void);
 

@@ -1,4 +1,4 @@
-"""ctypes binding of libkvpool.so — same names as include/kvpool.h, argument marshalling only.
+"""ctypes binding of libkvpool.so — same names as include/kvpool.h (+ include/kvpool_dev.h), argument marshalling only.
 
 Every step of the path runs inside the library's CUDA kernels / stream choreography; nothing here
 computes.  There is no fallback: if libkvpool.so is missing or a call fails, this raises.
@@ -27,7 +27,7 @@ _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA",
 
 EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
-    "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release",
+    "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release", "kvpool_set_tables",
     "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
     "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_validate_table", "kvpool_set_table_check", "kvpool_table_errors", "kvpool_last_error", "kvpool_version",
@@ -48,7 +48,7 @@ class Tuning(ctypes.Structure):
     _fields_ = [("kernel", c_uint32), ("link_kernel", c_uint32), ("hbm_ctas", c_uint32), ("link_ctas", c_uint32), ("bulk_chunk", c_uint32),
                 ("bulk_stages", c_uint32), ("bulk_warps", c_uint32), ("stage_slots", c_uint32),
                 ("vec_threads", c_uint32), ("vec_unroll", c_uint32), ("auto_threshold_bytes", c_uint64), ("group_bytes", c_uint64),
-                ("stage_chunk_bytes", c_uint64)]
+                ("stage_chunk_bytes", c_uint64), ("pdl", c_uint32), ("reserved", c_uint32)]
 
 
 class KvPoolError(RuntimeError):
@@ -87,6 +87,7 @@ def lib():
             "kvpool_get_tuning": [vp, vp],
             "kvpool_place": [vp, vp, POINTER(vp)],
             "kvpool_release": [vp, vp],
+            "kvpool_set_tables": [vp, vp, vp, c_uint64, vp],
             "kvpool_offload": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_retrieve": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp],
             "kvpool_retrieve_range": [vp, vp, c_uint32, c_uint32, c_uint32, vp, vp, c_uint64, vp, vp],
@@ -301,6 +302,13 @@ class KvPool:
         _ck(lib().kvpool_place(self.handle, b.ctypes.data, byref(h)))
         return Placement(self, h.value, b)
 
+    def set_tables(self, pl: Placement, tables_host, stream=None) -> None:
+        """tables_host: int32 numpy array / pinned torch tensor / address holding every layer's table back to back."""
+        n = int(np.sum(pl.blocks_per_layer))
+        if isinstance(tables_host, np.ndarray):
+            assert tables_host.dtype == np.int32 and tables_host.flags["C_CONTIGUOUS"] and tables_host.size == n
+        _ck(lib().kvpool_set_tables(self.handle, pl.handle, _addr(tables_host), n, _stream(stream)))
+
     def offload(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_dev, stream=None) -> None:
         _ck(lib().kvpool_offload(self.handle, pl.handle, layer, _addr(k_base), _addr(v_base), block_stride_bytes,
                                  _addr(block_table_dev), _stream(stream)))
@@ -320,20 +328,22 @@ class KvPool:
                                        block_stride_bytes, _addr(block_table_dev), _stream(stream)))
 
     @staticmethod
-    def _ptr_array(items) -> "ctypes.Array":
+    def _ptr_array(items) -> "Optional[ctypes.Array]":
+        if items is None:               # block_tables=None: the tables uploaded with set_tables
+            return None
         return (c_void_p * len(items))(*[_addr(x) or None for x in items])
 
     def offload_layers(self, pl: Placement, first_layer: int, k_bases, v_bases, block_stride_bytes: int, block_tables, stream=None) -> None:
         n = len(k_bases)
         ka, va, ta = self._ptr_array(k_bases), self._ptr_array(v_bases), self._ptr_array(block_tables)
         _ck(lib().kvpool_offload_layers(self.handle, pl.handle, first_layer, n, ctypes.addressof(ka), ctypes.addressof(va),
-                                        block_stride_bytes, ctypes.addressof(ta), _stream(stream)))
+                                        block_stride_bytes, ctypes.addressof(ta) if ta is not None else None, _stream(stream)))
 
     def retrieve_layers(self, pl: Placement, first_layer: int, k_bases, v_bases, block_stride_bytes: int, block_tables, stream=None) -> None:
         n = len(k_bases)
         ka, va, ta = self._ptr_array(k_bases), self._ptr_array(v_bases), self._ptr_array(block_tables)
         _ck(lib().kvpool_retrieve_layers(self.handle, pl.handle, first_layer, n, ctypes.addressof(ka), ctypes.addressof(va),
-                                         block_stride_bytes, ctypes.addressof(ta), _stream(stream)))
+                                         block_stride_bytes, ctypes.addressof(ta) if ta is not None else None, _stream(stream)))
 
     def retrieve_layers_signal(self, pl: Placement, first_layer: int, k_bases, v_bases, block_stride_bytes: int, block_tables, layer_ready,
                                stream=None) -> None:
@@ -342,7 +352,7 @@ class KvPool:
         ka, va, ta = self._ptr_array(k_bases), self._ptr_array(v_bases), self._ptr_array(block_tables)
         ea = (c_void_p * n)(*[_event(e) for e in layer_ready])
         _ck(lib().kvpool_retrieve_layers_signal(self.handle, pl.handle, first_layer, n, ctypes.addressof(ka), ctypes.addressof(va),
-                                                block_stride_bytes, ctypes.addressof(ta), ctypes.addressof(ea), _stream(stream)))
+                                                block_stride_bytes, ctypes.addressof(ta) if ta is not None else None, ctypes.addressof(ea), _stream(stream)))
 
     def offload_naive(self, pl: Placement, layer: int, k_base, v_base, block_stride_bytes: int, block_table_host: np.ndarray, stream=None) -> None:
         t = np.ascontiguousarray(block_table_host, dtype=np.int32)

@@ -14,6 +14,8 @@
 // Addressing of unit j is described in kernels.cuh (LayerArgs).
 #include "kernels.cuh"
 
+#include <utility>
+
 #include "../../include/kvpool.h"
 
 namespace kvp {
@@ -48,6 +50,15 @@ __device__ __forceinline__ void span_begin(unsigned long long* span) {
 __device__ __forceinline__ void span_end(unsigned long long* span) {
   if (span) atomicMax(span + 1, global_ns());
 }
+
+// Programmatic dependent launch (sm_90+): a launch that carries cudaLaunchAttributeProgrammaticStreamSerialization may
+// start while the kernel before it on the stream is still running.  Every kernel here lets its successor go at once
+// (launch_dependents: the successor's CTAs become resident, set up their barriers and indices) and touches global memory
+// only after griddep_wait(), which returns once the predecessor grid has completed and its writes are visible.  Without
+// the launch attribute both instructions do nothing.  What it buys: the launch latency and the pipeline ramp of layer
+// l+1's kernel hide under layer l's kernel when an engine issues one small zero-copy launch per layer.
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // Decode work item t of a layer split into `pieces` pieces per K (or V) block of `piece_bytes` bytes.
 struct Piece {
@@ -122,6 +133,8 @@ __global__ void __launch_bounds__(kVecMaxThreads) kv_copy_vec16(const __grid_con
   const uint64_t nwarps = static_cast<uint64_t>(gridDim.x) * warps_per_cta;
   const uint32_t pieces = (a.kvb + kVecPiece - 1) / kVecPiece;
   const uint64_t total = static_cast<uint64_t>(units(a)) * 2u * pieces;
+  griddep_launch_dependents();
+  griddep_wait();
   if (threadIdx.x == 0) span_begin(a.span);
   for (uint64_t t = static_cast<uint64_t>(blockIdx.x) * warps_per_cta + (threadIdx.x >> 5); t < total; t += nwarps) {
     const Piece p = decode(a, t, pieces, kVecPiece);
@@ -195,9 +208,11 @@ __global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Args
   const uint32_t warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const uint32_t bar0 = smem_u32(smem) + warp * stages * 8u;
   const uint32_t buf0 = smem_u32(smem) + kBulkBarrierBytes + warp * stages * chunk;
-  span_begin(a.span);
+  griddep_launch_dependents();
   for (uint32_t s = 0; s < stages; ++s) mbar_init(bar0 + 8u * s, 1);
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  griddep_wait();
+  span_begin(a.span);
 
   const uint32_t pieces = a.kvb / chunk;  // host guarantees chunk | kvb
   const uint64_t total = static_cast<uint64_t>(units(a)) * 2u * pieces;
@@ -311,6 +326,23 @@ cudaError_t launch_spin(uint64_t ns, cudaStream_t stream) {
   return cudaGetLastError();
 }
 
+// One launch, optionally as a programmatic dependent of the kernel before it on the stream.
+template <class... Params, class... Given>
+static cudaError_t launch_ex(void (*kernel)(Params...), uint32_t grid, uint32_t block, size_t smem, cudaStream_t stream, bool pdl,
+                             Given&&... args) {
+  cudaLaunchConfig_t c{};
+  c.gridDim = dim3(grid);
+  c.blockDim = dim3(block);
+  c.dynamicSmemBytes = smem;
+  c.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  c.attrs = at;
+  c.numAttrs = pdl ? 1u : 0u;
+  return cudaLaunchKernelEx(&c, kernel, std::forward<Given>(args)...);
+}
+
 template <class Args>
 static cudaError_t launch_copy(const Args& a, uint32_t n_units, bool pack, const LaunchCfg& cfg, cudaStream_t stream) {
   if (n_units == 0) return cudaSuccess;
@@ -328,12 +360,11 @@ static cudaError_t launch_copy(const Args& a, uint32_t n_units, bool pack, const
     uint64_t cap = cfg.ctas < resident ? cfg.ctas : resident;
     const uint32_t grid = static_cast<uint32_t>(want < cap ? want : cap);
     if (a.nphys_check) {
-      if (pack) kv_copy_bulk<true, Args, true><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
-      else kv_copy_bulk<false, Args, true><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
-    } else {
-      if (pack) kv_copy_bulk<true, Args, false><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
-      else kv_copy_bulk<false, Args, false><<<grid, warps * 32, smem, stream>>>(a, chunk, stages);
+      if (pack) return launch_ex(kv_copy_bulk<true, Args, true>, grid, warps * 32, smem, stream, cfg.pdl, a, chunk, stages);
+      return launch_ex(kv_copy_bulk<false, Args, true>, grid, warps * 32, smem, stream, cfg.pdl, a, chunk, stages);
     }
+    if (pack) return launch_ex(kv_copy_bulk<true, Args, false>, grid, warps * 32, smem, stream, cfg.pdl, a, chunk, stages);
+    return launch_ex(kv_copy_bulk<false, Args, false>, grid, warps * 32, smem, stream, cfg.pdl, a, chunk, stages);
   } else {
     const uint32_t unroll = cfg.vec_unroll == 4 ? 4 : (cfg.vec_unroll == 16 ? 16 : 8);
     const uint32_t threads = cfg.vec_threads ? cfg.vec_threads : kVecMaxThreads;
@@ -342,17 +373,14 @@ static cudaError_t launch_copy(const Args& a, uint32_t n_units, bool pack, const
     const uint64_t total = static_cast<uint64_t>(n_units) * 2u * pieces;
     const uint64_t want = (total + (threads / 32) - 1) / (threads / 32);
     const uint32_t grid = static_cast<uint32_t>(want < cfg.ctas ? want : cfg.ctas);
-#define KV_LAUNCH_VEC(U)                                                             \
-  do {                                                                               \
-    if (pack) kv_copy_vec16<true, U, Args><<<grid, threads, 0, stream>>>(a);         \
-    else kv_copy_vec16<false, U, Args><<<grid, threads, 0, stream>>>(a);             \
-  } while (0)
-    if (unroll == 4) KV_LAUNCH_VEC(4);
-    else if (unroll == 16) KV_LAUNCH_VEC(16);
-    else KV_LAUNCH_VEC(8);
+#define KV_LAUNCH_VEC(U)                                                                                          \
+  (pack ? launch_ex(kv_copy_vec16<true, U, Args>, grid, threads, 0, stream, cfg.pdl, a)                           \
+        : launch_ex(kv_copy_vec16<false, U, Args>, grid, threads, 0, stream, cfg.pdl, a))
+    if (unroll == 4) return KV_LAUNCH_VEC(4);
+    if (unroll == 16) return KV_LAUNCH_VEC(16);
+    return KV_LAUNCH_VEC(8);
 #undef KV_LAUNCH_VEC
   }
-  return cudaGetLastError();
 }
 
 cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream) {

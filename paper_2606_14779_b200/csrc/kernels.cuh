@@ -63,6 +63,7 @@ struct LaunchCfg {
   uint32_t bulk_chunk, bulk_stages, bulk_warps;
   uint32_t vec_threads, vec_unroll;
   uint32_t sm_count;
+  bool pdl;              // launch as a programmatic dependent of the kernel before it on the stream
 };
 
 // pack = true: paged -> pool side (offload direction); false: pool side -> paged (retrieve direction).

@@ -1,4 +1,4 @@
-// C ABI of libkvpool (include/kvpool.h): pool life cycle, placement + GLT, and the per-layer
+// C ABI of libkvpool (include/kvpool.h; development entry points: include/kvpool_dev.h): pool life cycle, placement + GLT, and the per-layer
 // offload / retrieve choreography over CUDA streams and events.  Device code lives in kernels.cu.
 #include <cuda_runtime.h>
 
@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "../../include/kvpool.h"
+#include "../../include/kvpool_dev.h"
 #include "kernels.cuh"
 #include "placement.hpp"
 #include "pool_mem.hpp"
@@ -124,6 +125,14 @@ struct kvpool_placement {
   uint8_t* tables_d = nullptr;   // every LayerMap's dev/slot columns, contiguous
   uint64_t tables_bytes = 0;
   bool tables_in_arena = false;  // carved out of the pool's table arena (else a private cudaMalloc)
+  // last work enqueued with this placement on each caller stream (non-timing events): kvpool_release waits for them, so
+  // that stripes never go back to the allocator while a kernel on a caller's stream still reads or writes them
+  std::vector<std::pair<cudaStream_t, cudaEvent_t>> last_use;
+  // kvpool_set_tables: the request's block tables, uploaded in one copy; layer l's table starts at own_table_off[l] entries
+  int32_t* own_tables_d = nullptr;
+  uint64_t own_tables_bytes = 0;
+  bool own_tables_in_arena = false, own_tables_set = false;
+  std::vector<uint64_t> own_table_off;
 };
 
 struct kvpool {
@@ -159,7 +168,9 @@ struct kvpool {
   uint64_t n_kernels = 0, n_memcpys = 0;
   bool profiling = false;
   bool prof_instream = false;            // KVPOOL_PROFILE_INSTREAM: timing events on the launching stream itself (perturbs it, see prof_begin)
-  cudaStream_t prof_s0 = nullptr, prof_s1 = nullptr;  // side streams that carry the timing events of profiled launches
+  // side streams that carry the timing events of profiled launches: one pair per launching stream, so that the e0 of one
+  // caller stream never queues behind another caller stream's marker wait
+  std::unordered_map<cudaStream_t, std::pair<cudaStream_t, cudaStream_t>> prof_side;
   std::vector<ProfRec> prof;
   std::vector<cudaEvent_t> prof_free;  // timing events ready for reuse
   unsigned long long* span_arena = nullptr;  // device: kSpanCap x {min start, max end} in %globaltimer ns, written by the kernels
@@ -186,6 +197,7 @@ void default_tuning(kvpool* p) {
   p->tune.vec_unroll = 8;
   p->tune.group_bytes = 64ull << 20;
   p->tune.auto_threshold_bytes = 8ull << 20;
+  p->tune.pdl = 1;
 }
 
 void free_slots(kvpool* p) {
@@ -238,6 +250,12 @@ bool is_live(const kvpool* p, const kvpool_placement* pl) {
 constexpr uint64_t kTableArenaBytes = 8ull << 20;
 
 void free_tables(kvpool* p, kvpool_placement* pl) {
+  if (pl->own_tables_d) {
+    if (pl->own_tables_in_arena) p->table_alloc.free(static_cast<uint64_t>(reinterpret_cast<uint8_t*>(pl->own_tables_d) - p->table_arena), pl->own_tables_bytes);
+    else cudaFree(pl->own_tables_d);
+    pl->own_tables_d = nullptr;
+    pl->own_tables_set = false;
+  }
   if (!pl->tables_d) return;
   if (pl->tables_in_arena) p->table_alloc.free(static_cast<uint64_t>(pl->tables_d - p->table_arena), pl->tables_bytes);
   else cudaFree(pl->tables_d);
@@ -249,8 +267,24 @@ cudaError_t take_event(kvpool* p, cudaEvent_t* e) {
   return cudaEventCreateWithFlags(e, cudaEventDisableTiming);
 }
 
+// Remember that `s` carries work of this placement (skipped while `s` is being captured into a CUDA graph: a captured
+// event could not be waited for later, and a graph's lifetime is the caller's business, kvpool.h).
+int note_use(kvpool* p, kvpool_placement* pl, cudaStream_t s) {
+  cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(s, &st) != cudaSuccess) { cudaGetLastError(); return KVPOOL_OK; }
+  if (st != cudaStreamCaptureStatusNone) return KVPOOL_OK;
+  for (auto& u : pl->last_use)
+    if (u.first == s) { CU(cudaEventRecord(u.second, s)); return KVPOOL_OK; }
+  cudaEvent_t e = nullptr;
+  CU(take_event(p, &e));
+  pl->last_use.emplace_back(s, e);
+  CU(cudaEventRecord(e, s));
+  return KVPOOL_OK;
+}
+
 void destroy_placement(kvpool* p, kvpool_placement* pl) {
   for (uint64_t id : pl->bound_ids) p->glt.erase(id);
+  for (auto& u : pl->last_use) p->ev_free.push_back(u.second);
   for (uint32_t i = 0; i < p->n && i < pl->region_off.size(); ++i) p->alloc[i].free(pl->region_off[i], pl->region_bytes[i]);
   for (auto& L : pl->layers)
     if (L.landed) p->ev_free.push_back(L.landed);
@@ -264,12 +298,18 @@ int check_layer_call(kvpool* p, kvpool_placement* pl, uint32_t layer, const void
   if (pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "placement does not belong to this pool");
   if (layer >= p->geom.n_layers) return fail(KVPOOL_EINVAL, "layer %u out of range (n_layers %u)", layer, p->geom.n_layers);
   if (pl->layers[layer].map->K == 0) return KVPOOL_OK;
-  if (!k_base || !v_base || !table) return fail(KVPOOL_EINVAL, "null k_base / v_base / block table");
+  if (!k_base || !v_base) return fail(KVPOOL_EINVAL, "null k_base / v_base");
+  if (!table && !pl->own_tables_set) return fail(KVPOOL_EINVAL, "null block table (and no tables uploaded with kvpool_set_tables)");
   if ((reinterpret_cast<uintptr_t>(k_base) | reinterpret_cast<uintptr_t>(v_base) | stride) & 15u)
     return fail(KVPOOL_EINVAL, "k_base, v_base and block_stride_bytes must be multiples of 16");
   if (stride < p->kvb) return fail(KVPOOL_EINVAL, "block_stride_bytes %llu < block bytes %llu", (unsigned long long)stride,
                                    (unsigned long long)p->kvb);
   return KVPOOL_OK;
+}
+
+// The layer's block table on the device: the caller's, or (null) the one kvpool_set_tables uploaded.
+inline const int32_t* table_of(const kvpool_placement* pl, uint32_t layer, const int32_t* given) {
+  return given ? given : pl->own_tables_d + pl->own_table_off[layer];
 }
 
 LayerArgs base_args(const kvpool* p, const LayerState& L, const void* k_base, const void* v_base, uint64_t stride,
@@ -307,6 +347,7 @@ LaunchCfg launch_cfg(const kvpool* p, bool link_bound) {
   c.vec_threads = p->tune.vec_threads;
   c.vec_unroll = p->tune.vec_unroll;
   c.sm_count = static_cast<uint32_t>(p->sm_count);
+  c.pdl = p->tune.pdl != 2;
   return c;
 }
 
@@ -351,27 +392,45 @@ cudaError_t prof_event(kvpool* p, cudaEvent_t* e) {
 // markers (1 us each, unaffected by DMA) and the timing events are recorded on two side streams behind them: e0 on
 // prof_s0 once the marker in front of the kernel has fired, e1 on prof_s1 once the marker behind it has.  The pair then
 // spans the kernel (plus a few us of marker latency) and the launching stream is not held up at all.
+int prof_side_streams(kvpool* p, cudaStream_t s, cudaStream_t* s0, cudaStream_t* s1) {
+  auto it = p->prof_side.find(s);
+  if (it == p->prof_side.end()) {
+    std::pair<cudaStream_t, cudaStream_t> pr{nullptr, nullptr};
+    CU(cudaStreamCreateWithFlags(&pr.first, cudaStreamNonBlocking));
+    CU(cudaStreamCreateWithFlags(&pr.second, cudaStreamNonBlocking));
+    it = p->prof_side.emplace(s, pr).first;
+  }
+  *s0 = it->second.first;
+  *s1 = it->second.second;
+  return KVPOOL_OK;
+}
 int prof_begin(kvpool* p, ProfRec* r, cudaStream_t s) {
   CU(prof_event(p, &r->e0));
   CU(prof_event(p, &r->e1));
   if (p->prof_instream) { CU(cudaEventRecord(r->e0, s)); return KVPOOL_OK; }
+  cudaStream_t s0 = nullptr, s1 = nullptr;
+  const int rc = prof_side_streams(p, s, &s0, &s1);
+  if (rc != KVPOOL_OK) return rc;
   cudaEvent_t m = nullptr;
   CU(take_event(p, &m));
   CU(cudaEventRecord(m, s));
-  CU(cudaStreamWaitEvent(p->prof_s0, m, 0));
+  CU(cudaStreamWaitEvent(s0, m, 0));
   p->ev_free.push_back(m);  // the wait has captured this record; a later re-record does not move it
-  CU(cudaEventRecord(r->e0, p->prof_s0));
+  CU(cudaEventRecord(r->e0, s0));
   return KVPOOL_OK;
 }
 int prof_end(kvpool* p, ProfRec* r, cudaStream_t s) {
   if (p->prof_instream) { CU(cudaEventRecord(r->e1, s)); }
   else {
+    cudaStream_t s0 = nullptr, s1 = nullptr;
+    const int rc = prof_side_streams(p, s, &s0, &s1);
+    if (rc != KVPOOL_OK) return rc;
     cudaEvent_t m = nullptr;
     CU(take_event(p, &m));
     CU(cudaEventRecord(m, s));
-    CU(cudaStreamWaitEvent(p->prof_s1, m, 0));
+    CU(cudaStreamWaitEvent(s1, m, 0));
     p->ev_free.push_back(m);
-    CU(cudaEventRecord(r->e1, p->prof_s1));
+    CU(cudaEventRecord(r->e1, s1));
   }
   p->prof.push_back(*r);
   return KVPOOL_OK;
@@ -552,8 +611,7 @@ int kvpool_destroy(kvpool_t* p) {
   if (p->table_arena_host) cudaFreeHost(p->table_arena_host);
   if (p->upload) cudaStreamDestroy(p->upload);
   if (p->join_out) cudaStreamDestroy(p->join_out);
-  if (p->prof_s0) cudaStreamDestroy(p->prof_s0);
-  if (p->prof_s1) cudaStreamDestroy(p->prof_s1);
+  for (auto& kv : p->prof_side) { cudaStreamDestroy(kv.second.first); cudaStreamDestroy(kv.second.second); }
   for (auto e : p->ev_free) cudaEventDestroy(e);
   for (auto& r : p->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   for (auto e : p->prof_free) cudaEventDestroy(e);
@@ -634,6 +692,7 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
   if (t->stage_slots > 64) return fail(KVPOOL_EINVAL, "set_tuning: stage_slots must be <= 64");
   if (t->vec_threads && (t->vec_threads % 32 || t->vec_threads < 64 || t->vec_threads > 512))
     return fail(KVPOOL_EINVAL, "set_tuning: vec_threads must be a multiple of 32 in 64..512");
+  if (t->pdl > 2) return fail(KVPOOL_EINVAL, "set_tuning: pdl must be 0 (keep), 1 (on) or 2 (off)");
   if (t->vec_unroll && t->vec_unroll != 4 && t->vec_unroll != 8 && t->vec_unroll != 16)
     return fail(KVPOOL_EINVAL, "set_tuning: vec_unroll must be 4, 8 or 16");
   kvpool_tuning d = p->tune;
@@ -646,6 +705,7 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
   if (t->bulk_warps) d.bulk_warps = t->bulk_warps;
   if (t->vec_threads) d.vec_threads = t->vec_threads;
   if (t->vec_unroll) d.vec_unroll = t->vec_unroll;
+  if (t->pdl) d.pdl = t->pdl;
   if (t->auto_threshold_bytes) d.auto_threshold_bytes = t->auto_threshold_bytes;
   if (t->group_bytes) d.group_bytes = t->group_bytes;
   if (t->stage_chunk_bytes) d.stage_chunk_bytes = t->stage_chunk_bytes == ~0ull ? 0 : t->stage_chunk_bytes;
@@ -816,6 +876,7 @@ int kvpool_release(kvpool_t* p, kvpool_placement_t* pl) {
   DeviceGuard guard(p->cuda_device);
   const int rc = sync_pool_streams(p);  // the library's own transfers for it must be over
   if (rc != KVPOOL_OK) return rc;
+  for (auto& u : pl->last_use) CU(cudaEventSynchronize(u.second));  // and so must the kernels it put on the caller's streams
   p->live.erase(it);
   destroy_placement(p, pl);
   return KVPOOL_OK;
@@ -904,7 +965,7 @@ int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, ui
   DeviceGuard guard(p->cuda_device);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const uint32_t N = p->n;
-  LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
+  LayerArgs a = base_args(p, L, k_base, v_base, stride, table_of(pl, layer, table));
   bool staged = use_staged(p, L);
   if (staged && n_blocks != L.map->K) {  // a range is judged by its own size and by where its own blocks sit
     staged = plan_chunk(p, L, first_block, n_blocks).host_blocks &&
@@ -913,23 +974,22 @@ int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, ui
 
   if (!staged) {
     // zero-copy: one kernel gathers the paged blocks and stores them straight into the mapped host stripes
-    mark_offloaded(L, first_block, n_blocks);
     a.j0 = first_block;
     a.K = n_blocks;
     chunk_bases(p, L, ChunkPlan{}, nullptr, &a);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));  // an earlier staged offload of this layer still in flight
     rc = launch_counted(p, a, true, true, s);
     if (rc != KVPOOL_OK) return rc;
+    mark_offloaded(L, first_block, n_blocks);  // only now: a failed launch must not leave the blocks flagged as present
     CU(cudaEventRecord(L.landed, s));
     L.landed_pending = true;
-    return KVPOOL_OK;
+    return note_use(p, pl, s);
   }
 
   // staged: pack kernel -> device staging slot, then one D2H copy per device on the per-device I/O streams; `stream` is
   // released as soon as the last pack is enqueued.  A layer larger than a slot travels in chunks of logical blocks.
   const uint64_t per_slot = p->slots.empty() ? 0 : blocks_per_slot(p);
   if (per_slot == 0) return fail(KVPOOL_ESTATE, "offload: no staging slot (the placement was made while the path was zero-copy)");
-  mark_offloaded(L, first_block, n_blocks);
   // `landed` must mean "all stripes complete": it is recorded on a stream of the pool's own that carries no copies and only
   // gathers every chunk's kernel and copies — the per-device I/O streams never wait for one another
   cudaStream_t lead = p->join_out;
@@ -972,9 +1032,10 @@ int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, ui
     for (uint32_t i = 0; i < N; ++i)
       if (slot.copies_after_kernel >> i & 1u) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
   }
+  mark_offloaded(L, first_block, n_blocks);  // every chunk is enqueued (an error above leaves the range unflagged: retrieve -> ESTATE)
   CU(cudaEventRecord(L.landed, lead));
   L.landed_pending = true;
-  return KVPOOL_OK;
+  return note_use(p, pl, s);
 }
 
 int kvpool_offload(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
@@ -1001,7 +1062,7 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   DeviceGuard guard(p->cuda_device);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const uint32_t N = p->n;
-  LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
+  LayerArgs a = base_args(p, L, k_base, v_base, stride, table_of(pl, layer, table));
   const uint64_t range_bytes = static_cast<uint64_t>(n_blocks) * p->payload;
   bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && range_bytes >= p->tune.auto_threshold_bytes));
   // a range whose blocks all sit on HBM-type devices has nothing to stage
@@ -1013,7 +1074,8 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
     a.K = n_blocks;
     chunk_bases(p, L, ChunkPlan{}, nullptr, &a);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
-    return launch_counted(p, a, false, true, s);
+    rc = launch_counted(p, a, false, true, s);
+    return rc == KVPOOL_OK ? note_use(p, pl, s) : rc;
   }
 
   // staged: one H2D copy per device (only the slots the range touches) on the per-device I/O streams — these may run
@@ -1057,7 +1119,7 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
     if (rc != KVPOOL_OK) return rc;
     CU(cudaEventRecord(slot.kernel_done, s));
   }
-  return KVPOOL_OK;
+  return note_use(p, pl, s);
 }
 
 
@@ -1117,7 +1179,7 @@ void fill_descs(const BatchCall& c, const LayerGroup& g, MultiArgs* ma) {
     MultiDesc& d = ma->d[b];
     d.k_base = static_cast<uint8_t*>(const_cast<void*>(c.k_bases[g.q[b]]));
     d.v_base = static_cast<uint8_t*>(const_cast<void*>(c.v_bases[g.q[b]]));
-    d.table = c.tables[g.q[b]];
+    d.table = table_of(c.pl, c.first + g.q[b], c.tables ? c.tables[g.q[b]] : nullptr);
     d.dev = L.map->dev_d;
     d.slot = L.map->slot_d;
     d.pool_base = L.base_d;
@@ -1141,6 +1203,8 @@ int issue_zero_copy_group(const BatchCall& c, const LayerGroup& g) {
   if (c.pack)
     for (uint32_t b = 0; b < g.n; ++b) {
       LayerState& L = c.pl->layers[c.first + g.q[b]];
+      L.offloaded = true;
+      L.have.clear();
       CU(cudaEventRecord(L.landed, c.s));
       L.landed_pending = true;
     }
@@ -1214,6 +1278,8 @@ int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
       if (span[i] && ios[i] != lead) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
     for (uint32_t b = 0; b < g.n; ++b) {  // `lead` has waited for the kernel and every copy; with no host stripe the kernel was all
       LayerState& L = c.pl->layers[c.first + g.q[b]];
+      L.offloaded = true;
+      L.have.clear();
       CU(cudaEventRecord(L.landed, lead ? lead : c.s));
       L.landed_pending = true;
     }
@@ -1262,8 +1328,8 @@ int issue_group_work(const BatchCall& c, const LayerGroup& g) {
   }
   for (uint32_t b = 0; b < g.n; ++b) {  // a single layer, or a group too large for a staging slot: the per-layer path
     const uint32_t q = g.q[b], layer = c.first + q;
-    const int rc = c.pack ? kvpool_offload(p, c.pl, layer, c.k_bases[q], c.v_bases[q], c.stride, c.tables[q], c.s)
-                          : kvpool_retrieve(p, c.pl, layer, const_cast<void*>(c.k_bases[q]), const_cast<void*>(c.v_bases[q]), c.stride, c.tables[q], c.s);
+    const int rc = c.pack ? kvpool_offload(p, c.pl, layer, c.k_bases[q], c.v_bases[q], c.stride, c.tables ? c.tables[q] : nullptr, c.s)
+                          : kvpool_retrieve(p, c.pl, layer, const_cast<void*>(c.k_bases[q]), const_cast<void*>(c.v_bases[q]), c.stride, c.tables ? c.tables[q] : nullptr, c.s);
     if (rc != KVPOOL_OK) return rc;
   }
   return KVPOOL_OK;
@@ -1280,9 +1346,10 @@ static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32
   if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "layers: bad pool or placement");
   if (static_cast<uint64_t>(first) + n > p->geom.n_layers) return fail(KVPOOL_EINVAL, "layers [%u, %u) out of range (n_layers %u)", first, first + n, p->geom.n_layers);
   if (n == 0) return KVPOOL_OK;
-  if (!k_bases || !v_bases || !tables) return fail(KVPOOL_EINVAL, "layers: null pointer array");
+  if (!k_bases || !v_bases) return fail(KVPOOL_EINVAL, "layers: null pointer array");
+  if (!tables && !pl->own_tables_set) return fail(KVPOOL_EINVAL, "layers: null block_tables (and no tables uploaded with kvpool_set_tables)");
   for (uint32_t q = 0; q < n; ++q) {  // validate everything first: no partial effects on EINVAL / ESTATE
-    const int rc = check_layer_call(p, pl, first + q, k_bases[q], v_bases[q], stride, tables[q]);
+    const int rc = check_layer_call(p, pl, first + q, k_bases[q], v_bases[q], stride, tables ? tables[q] : nullptr);
     if (rc != KVPOOL_OK) return rc;
     if (!pack && !pl->layers[first + q].offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", first + q);
   }
@@ -1293,13 +1360,13 @@ static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32
   uint64_t units = 0;
   for (uint32_t q = 0; q < n; ++q) {
     LayerState& L = pl->layers[first + q];
-    if (pack) { L.offloaded = true; L.have.clear(); }
     if (L.map->K == 0) {  // nothing to move: ready in stream order right away
+      if (pack) L.offloaded = true;
       if (ready && ready[q]) CU(cudaEventRecord(static_cast<cudaEvent_t>(ready[q]), c.s));
       continue;
     }
     const uint64_t bytes = L.map->K * p->payload;
-    if (g.n && (g.n == kMaxBatch || units + L.map->K > 0x7fffffffull || (p->path != KVPOOL_PATH_ZEROCOPY && g.bytes + bytes > std::max(cap, bytes)))) {
+    if (g.n && (g.n == kMaxBatch || units + L.map->K > 0x7fffffffull || g.bytes + bytes > std::max(cap, bytes))) {
       const int rc = issue_group(c, g);
       if (rc != KVPOOL_OK) return rc;
       g = LayerGroup{};
@@ -1308,14 +1375,15 @@ static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32
     g.q[g.n++] = q;
     g.bytes += bytes;
     units += L.map->K;
-    if (p->path != KVPOOL_PATH_ZEROCOPY && g.bytes >= cap) {
+    if (g.bytes >= cap) {  // on every path: a group is also the grain at which a consumer's per-layer events fire
       const int rc = issue_group(c, g);
       if (rc != KVPOOL_OK) return rc;
       g = LayerGroup{};
       units = 0;
     }
   }
-  return issue_group(c, g);
+  const int rc = issue_group(c, g);
+  return rc == KVPOOL_OK ? note_use(p, pl, c.s) : rc;
 }
 
 int kvpool_offload_layers(kvpool_t* p, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers, const void* const* k_bases,
@@ -1365,7 +1433,7 @@ static int naive_layer(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, bool
     CU(cudaEventRecord(L.landed, s));
     L.landed_pending = true;
   }
-  return KVPOOL_OK;
+  return note_use(p, pl, s);
 }
 
 int kvpool_offload_naive(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
@@ -1376,6 +1444,50 @@ int kvpool_offload_naive(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, co
 int kvpool_retrieve_naive(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
                           const int32_t* table_host, void* cuda_stream) {
   return naive_layer(p, pl, layer, false, k_base, v_base, stride, table_host, cuda_stream);
+}
+
+int kvpool_set_tables(kvpool_t* p, kvpool_placement_t* pl, const int32_t* tables_host, uint64_t n_entries, void* cuda_stream) {
+  PoolLock lock__(p);
+  if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "set_tables: bad pool or placement");
+  uint64_t total = 0;
+  for (auto& L : pl->layers) total += L.map->K;
+  if (n_entries != total) return fail(KVPOOL_EINVAL, "set_tables: %llu entries given, the placement's layers hold %llu blocks", (unsigned long long)n_entries, (unsigned long long)total);
+  if (total == 0) { pl->own_tables_set = true; pl->own_table_off.assign(pl->layers.size(), 0); return KVPOOL_OK; }
+  if (!tables_host) return fail(KVPOOL_EINVAL, "set_tables: null tables_host");
+  DeviceGuard guard(p->cuda_device);
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  if (!pl->own_tables_d) {
+    const uint64_t bytes = (total * 4 + 255) / 256 * 256;
+    uint64_t off = 0;
+    if (p->table_alloc.alloc(bytes, &off)) {
+      pl->own_tables_d = reinterpret_cast<int32_t*>(p->table_arena + off);
+      pl->own_tables_in_arena = true;
+    } else {
+      cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&pl->own_tables_d), bytes);
+      if (e != cudaSuccess) { cudaGetLastError(); pl->own_tables_d = nullptr; return fail(KVPOOL_ENOMEM, "set_tables: %s", cudaGetErrorString(e)); }
+      pl->own_tables_in_arena = false;
+    }
+    pl->own_tables_bytes = bytes;
+    pl->own_table_off.resize(pl->layers.size());
+    uint64_t acc = 0;
+    for (size_t l = 0; l < pl->layers.size(); ++l) { pl->own_table_off[l] = acc; acc += pl->layers[l].map->K; }
+  }
+  if (pl->own_tables_in_arena) {
+    // through the pinned mirror of the arena: the caller's buffer (pageable or not) is free again when the call returns,
+    // and the copy is one asynchronous DMA ordered on `stream`.  A re-upload first waits for the work enqueued with the
+    // placement so far (the earlier upload may not have read the mirror yet; kernels may still read the old tables).
+    if (pl->own_tables_set)
+      for (auto& u : pl->last_use) CU(cudaEventSynchronize(u.second));
+    uint8_t* mirror = p->table_arena_host + (reinterpret_cast<uint8_t*>(pl->own_tables_d) - p->table_arena);
+    memcpy(mirror, tables_host, total * 4);
+    CU(cudaMemcpyAsync(pl->own_tables_d, mirror, total * 4, cudaMemcpyHostToDevice, s));
+  } else {
+    CU(cudaMemcpyAsync(pl->own_tables_d, tables_host, total * 4, cudaMemcpyHostToDevice, s));
+    CU(cudaStreamSynchronize(s));  // (arena exhausted: private allocation, no mirror — the caller's buffer must be read before we return)
+  }
+  p->n_memcpys++;
+  pl->own_tables_set = true;
+  return note_use(p, pl, s);
 }
 
 int kvpool_wait_offloads(kvpool_t* p, kvpool_placement_t* pl, void* cuda_stream) {
@@ -1410,9 +1522,10 @@ int kvpool_pack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, const void*
   if (L.map->K == 0) return KVPOOL_OK;
   if (!stage_dev || (reinterpret_cast<uintptr_t>(stage_dev) & 15u)) return fail(KVPOOL_EINVAL, "pack: stage_dev must be a 16-byte aligned device pointer");
   DeviceGuard guard(p->cuda_device);
-  LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
+  LayerArgs a = base_args(p, L, k_base, v_base, stride, table_of(pl, layer, table));
   for (uint32_t i = 0; i < p->n; ++i) a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(stage_dev) + static_cast<uint64_t>(L.map->start[i]) * p->payload);
-  return launch_counted(p, a, true, false, static_cast<cudaStream_t>(cuda_stream));
+  rc = launch_counted(p, a, true, false, static_cast<cudaStream_t>(cuda_stream));
+  return rc == KVPOOL_OK ? note_use(p, pl, static_cast<cudaStream_t>(cuda_stream)) : rc;
 }
 
 int kvpool_unpack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base, uint64_t stride,
@@ -1424,10 +1537,11 @@ int kvpool_unpack(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, void* k_b
   if (L.map->K == 0) return KVPOOL_OK;
   if (!stage_dev || (reinterpret_cast<uintptr_t>(stage_dev) & 15u)) return fail(KVPOOL_EINVAL, "unpack: stage_dev must be a 16-byte aligned device pointer");
   DeviceGuard guard(p->cuda_device);
-  LayerArgs a = base_args(p, L, k_base, v_base, stride, table);
+  LayerArgs a = base_args(p, L, k_base, v_base, stride, table_of(pl, layer, table));
   for (uint32_t i = 0; i < p->n; ++i)
     a.pool_base[i] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(const_cast<void*>(stage_dev)) + static_cast<uint64_t>(L.map->start[i]) * p->payload);
-  return launch_counted(p, a, false, false, static_cast<cudaStream_t>(cuda_stream));
+  rc = launch_counted(p, a, false, false, static_cast<cudaStream_t>(cuda_stream));
+  return rc == KVPOOL_OK ? note_use(p, pl, static_cast<cudaStream_t>(cuda_stream)) : rc;
 }
 
 int kvpool_checksum(kvpool_t* p, const void* k_base, const void* v_base, uint64_t stride, const int32_t* table, uint32_t n_blocks,
@@ -1585,11 +1699,6 @@ int kvpool_set_profiling(kvpool_t* p, int enabled) {
     DeviceGuard guard(p->cuda_device);
     CU(cudaMalloc(reinterpret_cast<void**>(&p->span_arena), 2ull * kSpanCap * sizeof(unsigned long long)));
     CU(reset_spans(p));
-  }
-  if (enabled && !p->prof_s0) {
-    DeviceGuard guard(p->cuda_device);
-    CU(cudaStreamCreateWithFlags(&p->prof_s0, cudaStreamNonBlocking));
-    CU(cudaStreamCreateWithFlags(&p->prof_s1, cudaStreamNonBlocking));
   }
   p->profiling = enabled != 0;
   p->prof_instream = enabled == KVPOOL_PROFILE_INSTREAM;
