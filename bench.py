@@ -55,6 +55,10 @@ def parse_args():
     ap.add_argument("--stage-slots", type=int, default=0)
     ap.add_argument("--stage-chunk-mib", type=float, default=0.0,
                     help="staged path: cap a staging slot at this many MiB; larger layers travel in chunks (tune.stage_chunk_bytes)")
+    ap.add_argument("--link-groups", choices=["shared", "independent"], default="shared",
+                    help="shared (default): every host pool buffer names link group 1 - they all sit behind this GPU's one PCIe link, so the "
+                         "library serves them in request order on one I/O stream per direction; independent: link group 0, one I/O stream "
+                         "pair per pool device (the paper's literal 'independent I/O streams', PAPER.md:177)")
     ap.add_argument("--per-layer", action="store_true",
                     help="issue one kvpool_offload / kvpool_retrieve call per layer in the timed step instead of the batched *_layers calls")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -263,7 +267,8 @@ def run_kvpool(args) -> dict:
     t0 = time.perf_counter()
     pool = kv.KvPool(base_w, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, block_tokens=g.block_tokens,
                      elem_bytes=g.elem_bytes, cuda_device=local, numa_nodes=numa,
-                     dev_flags=[kv.DEV_CUDA_HOSTALLOC] * N if args.hostalloc else None)
+                     dev_flags=[kv.DEV_CUDA_HOSTALLOC] * N if args.hostalloc else None,
+                     link_groups=[1] * N if args.link_groups == "shared" else None)
     create_s = time.perf_counter() - t0
     weights_kind = args.weights
     if args.weights == "measured" or (args.weights == "config" and wl.weights is None):
@@ -615,7 +620,7 @@ def run_kvpool(args) -> dict:
                    "moved_bytes_per_leg": moved, "pool_buffers": N, "weights": weights_kind, "bandwidth_gbps": [round(float(x), 3) for x in bw],
                    "numa_nodes": numa_actual, "path": args.path, "kernel": "vec16" if tn.kernel == kv.KERNEL_VEC16 else "bulk",
                    "link_kernel": "vec16" if tn.link_kernel == kv.KERNEL_VEC16 else "bulk",
-                   "link_ctas": tn.link_ctas, "hbm_ctas": tn.hbm_ctas, "stage_slots": tn.stage_slots, "stage_chunk_bytes": tn.stage_chunk_bytes, "streams": len(streams),
+                   "link_ctas": tn.link_ctas, "hbm_ctas": tn.hbm_ctas, "stage_slots": tn.stage_slots, "stage_chunk_bytes": tn.stage_chunk_bytes, "link_groups": args.link_groups, "streams": len(streams),
                    "l2": f"inputs larger than L2: each leg moves {moved / 2**30:.1f} GiB through {L} distinct layers (L2 is 126 MB); no flush needed",
                    "calls": "per-layer" if args.per_layer else "batched (kvpool_offload_layers / kvpool_retrieve_layers, one call per request)",
                    "step": "kvpool_place + offload of every layer + retrieve of every layer; value = retrieve leg"},
@@ -850,18 +855,18 @@ def run_mixed_pool(args) -> None:
     torch.cuda.synchronize()
     cap = moved + (L + 4) * (g.payload + 4096)
     print(f"# bench.py --mixed-pool --config {args.config}: {wl.name} cut to {L} layers, {moved / 2**20:.0f} MiB per leg ({K} blocks of {g.payload} B per layer); "
-          "weights = kvpool_measure_bandwidth (256 MiB cudaMemcpyAsync, payload GB/s); median of 3; HBM-type device = this GPU's own memory")
+          "weights = kvpool_calibrate (256 MiB per device: cudaMemcpyAsync for the host-only pool, the gather kernel itself for pools with HBM-type devices; link groups "
+          "share; payload GB/s); median of 3; HBM-type device = this GPU's own memory")
     print(f"{'pool':34s} {'weights (GB/s)':>22s} {'blocks per layer':>18s} {'offload GB/s':>12s} {'retrieve GB/s':>13s} {'sum of weights':>14s} {'kernels':>8s} {'memcpys':>8s}")
     for name, flags in (("1 host buffer", [0]), ("1 host buffer + 1 HBM device", [0, kv.DEV_HBM]), ("2 host buffers + 2 HBM devices", [0, 0, kv.DEV_HBM, kv.DEV_HBM]),
                         ("1 HBM device", [kv.DEV_HBM])):
         n = len(flags)
-        pool = kv.KvPool([1.0] * n, [cap] * n, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, dev_flags=flags)
-        bw = [pool.measure_bandwidth(i, 0, 256 << 20, 5) for i in range(n)]
-        # devices behind ONE shared resource (the host buffers behind this box's single PCIe link; HBM-type devices in the
-        # same GPU's memory) are each worth their share of it, not the whole of it
-        n_host, n_hbm = sum(1 for f in flags if not f), sum(1 for f in flags if f)
-        bw = [b / (n_hbm if f else n_host) for b, f in zip(bw, flags)]
-        pool.set_bandwidth(bw)
+        # devices behind ONE shared resource name one link group (the host buffers behind this GPU's single PCIe link: 1; the
+        # HBM-type devices inside one GPU: 2): kvpool_calibrate measures every device and divides what a group shares.  A pool
+        # with HBM-type devices is measured with the library's own kernel, which is what reaches every stripe there.
+        pool = kv.KvPool([1.0] * n, [cap] * n, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, dev_flags=flags,
+                         link_groups=[2 if f else 1 for f in flags])
+        bw = list(pool.calibrate(kv.MEASURE_KERNEL_RETRIEVE if any(flags) else kv.MEASURE_RETRIEVE, 256 << 20, 5))
         offs, rets = [], []
         k0, m0 = pool.stats()
         for it in range(4):

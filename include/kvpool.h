@@ -62,6 +62,9 @@ enum {
                                         peer of the pool's GPU, or that GPU itself.  Its stripes are reached
                                         by the kernels directly (peer loads / stores); no staging, no copy engine.            */
 
+#define KVPOOL_MEASURE_KERNEL_RETRIEVE 2 /* kvpool_measure_bandwidth / kvpool_calibrate `direction`, see there */
+#define KVPOOL_MEASURE_KERNEL_OFFLOAD 3
+
 #define KVPOOL_NUMA_AUTO (-2)        /* kvpool_device_desc.numa_node: bind to the NUMA node of the pool's GPU */
 
 /* pool-device types (GLT `type`, Table I) */
@@ -97,7 +100,14 @@ typedef struct {           /* one pool device (Table I)           
   uint32_t flags;          /* KVPOOL_DEV_*                                                              */
   int32_t gpu;             /* HBM: CUDA ordinal of the GPU that holds the buffer, -1 = the pool's own   */
                            /* GPU; must be peer-accessible from it (ECUDA otherwise).  MEM: ignored     */
-  uint32_t reserved;       /* 0                                                                         */
+  uint32_t link_group;     /* 0 = the device has a transfer resource of its own.  g > 0: it shares one  */
+                           /* with every other device of the pool that names the same g - several host  */
+                           /* buffers behind one PCIe link, several HBM devices inside one GPU.  Such   */
+                           /* devices are served in request order by ONE I/O stream per direction (the  */
+                           /* paper's "independent I/O streams", are per independent      */
+                           /* resource: copies that share a link only slow each other down, and layer   */
+                           /* l+1's copies would delay layer l's), and kvpool_calibrate divides what    */
+                           /* they share.  Placement (Eq. 1-2) is untouched: only b_i changes           */
 } kvpool_device_desc;
 
 typedef struct { /* geometry of one paged KV block */
@@ -112,15 +122,18 @@ typedef struct {         /* kvpool_set_tuning; 0 in any field = library default 
   uint32_t bulk_chunk;   /* bytes per cp.async.bulk (power of two, 1 KiB..32 KiB)                        */
   uint32_t bulk_stages;  /* ring depth per issuing warp                                                 */
   uint32_t bulk_warps;   /* issuing warps per CTA                                                       */
-  uint32_t stage_slots;  /* staging buffers in the ring of the staged path (default 4)                   */
+  uint32_t stage_slots;  /* staging buffers in the ring of the staged path (default 2: one fills while the other drains) */
   uint32_t vec_threads;  /* threads per CTA of the vec16 kernel (multiple of 32, 64..512)                */
   uint32_t vec_unroll;   /* 16-byte loads in flight per lane in the vec16 kernel: 4, 8 or 16             */
   uint64_t auto_threshold_bytes; /* PATH_AUTO: layers (or groups) moving fewer bytes than this go zero-copy */
   uint64_t group_bytes;  /* batched calls: consecutive layers are grouped until a group moves at least this much */
-  uint64_t stage_chunk_bytes; /* staged path: a staging slot holds at most this much; a larger layer travels in chunks of
-                            consecutive logical blocks (copies of chunk c+1 overlap the pack/unpack of chunk c), so the
-                            staging ring (stage_slots x this) does not grow with the context length.  Default: off (a slot
-                            holds the largest layer); UINT64_MAX turns it off again; at least one block per chunk           */
+  uint64_t stage_chunk_bytes; /* staged path: a staging slot holds at most this much (default 256 MiB, so the ring is at most
+                            stage_slots x 256 MiB = 512 MiB of HBM whatever the context length).  A larger layer travels in
+                            DEVICE-MAJOR chunks: a chunk is a run of consecutive slots of ONE pool device's stripe, i.e. one
+                            contiguous piece of that stripe - ONE cudaMemcpyAsync - gathered / scattered by a launch that finds
+                            its logical blocks through the device's inverse map (uploaded with the placement); the copy of
+                            chunk c+1 overlaps the pack / unpack of chunk c.  Placement and stripe bytes are the same as
+                            without chunking.  UINT64_MAX: no cap (a slot holds the largest layer); at least one block per chunk */
   uint32_t pdl;          /* programmatic dependent launch of the library's kernels (the next layer's launch latency and
                             ramp hide under the current layer's kernel): 1 = on (default), 2 = off                          */
   uint32_t reserved;     /* 0                                                                                             */
@@ -168,11 +181,32 @@ KVPOOL_API int kvpool_set_bandwidth(kvpool_t* pool, const double* bandwidth_gbps
 /* Measure pool device `dev`: cudaMemcpyAsync of `bytes` (<= capacity) between the pool buffer and a
  * scratch device buffer, `iters` times, median, CUDA events.  direction 0 = pool->GPU (retrieve
  * direction), 1 = GPU->pool.  GB/s counts the bytes moved once (payload), for HBM devices too.  Blocking.
+ * direction KVPOOL_MEASURE_KERNEL_RETRIEVE (2) / KVPOOL_MEASURE_KERNEL_OFFLOAD (3): the same bytes moved by the
+ * library's own gather / scatter kernel between the device's memory, reached in place (mapped host memory over the
+ * link, or HBM), and a scratch paged layout — the rate that counts where the kernels reach the stripes themselves:
+ * every device of a pool with HBM-type devices, and the zero-copy path (SM-issued transfers over PCIe run ~8 %
+ * below the copy engines).  Measure with the mechanism that will move the bytes.
  * The first `bytes` of the pool buffer are overwritten in either direction (a host buffer measured in
  * direction 0 is first written once by DMA: stripes are always written by an offload before a retrieve
  * reads them, and freshly zeroed pages still held in CPU caches read ~5 % slow until then) — ESTATE
  * while any placement is live.                                                                          */
 KVPOOL_API int kvpool_measure_bandwidth(kvpool_t* pool, uint32_t dev, int direction, uint64_t bytes, uint32_t iters, double* gbps_out /*host*/);
+/* What each device can count on when the members of a link group run together (pure host arithmetic, no pool):
+ * out[i] = alone[i] for link_group[i] == 0, else alone[i] * max_g / sum_g over the members of its group, evaluated
+ * left to right in IEEE double - m equal members get 1/m of the shared rate each, unequal members split the best
+ * member's rate in proportion to their own, and a group's shares add up to that best rate.  Eq. 1 presumes every
+ * device delivers b_i concurrently; bandwidths measured one device at a time over-count devices
+ * that share a link.  EINVAL if n == 0, n > KVPOOL_MAX_DEVICES or some alone[i] is not positive and finite.       */
+KVPOOL_API int kvpool_share_bandwidth(const double* alone_gbps /*host[n]*/, const uint32_t* link_group /*host[n]*/, uint32_t n,
+                           double* out_gbps /*host[n]*/);
+/* "Measured bandwidth" of Eq. 1 in one call: kvpool_measure_bandwidth on every pool device in turn
+ * (min(bytes, capacity) each), kvpool_share_bandwidth over the pool's link groups, kvpool_set_bandwidth with the
+ * result.  bandwidth_out (host[n_devs], may be NULL) receives the installed b_i.  Blocking; ESTATE while any
+ * placement is live.                                                                                              */
+KVPOOL_API int kvpool_calibrate(kvpool_t* pool, int direction, uint64_t bytes, uint32_t iters, double* bandwidth_out /*host[n_devs]*/);
+/* The b_i the pool currently places by (as given to kvpool_create / kvpool_set_bandwidth, or installed by
+ * kvpool_calibrate) and each device's link group.  Either out pointer may be NULL.                                */
+KVPOOL_API int kvpool_bandwidths(const kvpool_t* pool, double* bandwidth_out /*host[n_devs]*/, uint32_t* link_group_out /*host[n_devs]*/);
 
 KVPOOL_API int kvpool_set_path(kvpool_t* pool, int path /*KVPOOL_PATH_**/);
 KVPOOL_API int kvpool_set_tuning(kvpool_t* pool, const kvpool_tuning* t /*host*/);

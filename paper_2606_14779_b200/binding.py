@@ -20,6 +20,7 @@ OK, EINVAL, ENOMEM, ECUDA, ENUMA, ESTATE, ENOENT = 0, -1, -2, -3, -4, -5, -6
 DEV_WRITE_COMBINED, DEV_NUMA_STRICT, DEV_HBM, DEV_CUDA_HOSTALLOC = 1, 2, 4, 8
 TYPE_MEM, TYPE_SSD, TYPE_HBM = 0, 1, 2
 NUMA_AUTO = -2
+MEASURE_RETRIEVE, MEASURE_OFFLOAD, MEASURE_KERNEL_RETRIEVE, MEASURE_KERNEL_OFFLOAD = 0, 1, 2, 3
 PROFILE_OFF, PROFILE_SIDE, PROFILE_INSTREAM = 0, 1, 2
 PATH_AUTO, PATH_STAGED, PATH_ZEROCOPY = 0, 1, 2
 KERNEL_VEC16, KERNEL_BULK = 0, 1
@@ -27,7 +28,7 @@ _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA",
 
 EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
-    "kvpool_measure_bandwidth", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release", "kvpool_set_tables",
+    "kvpool_measure_bandwidth", "kvpool_share_bandwidth", "kvpool_calibrate", "kvpool_bandwidths", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release", "kvpool_set_tables",
     "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
     "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_validate_table", "kvpool_set_table_check", "kvpool_table_errors", "kvpool_last_error", "kvpool_version",
@@ -36,7 +37,7 @@ EXPORTS = [
 
 class DeviceDesc(ctypes.Structure):
     _fields_ = [("bandwidth_gbps", c_double), ("capacity_bytes", c_uint64), ("numa_node", c_int32), ("flags", c_uint32),
-                ("gpu", c_int32), ("reserved", c_uint32)]
+                ("gpu", c_int32), ("link_group", c_uint32)]
 
 
 class Geometry(ctypes.Structure):
@@ -81,6 +82,9 @@ def lib():
             "kvpool_destroy": [vp],
             "kvpool_set_bandwidth": [vp, vp],
             "kvpool_measure_bandwidth": [vp, c_uint32, c_int, c_uint64, c_uint32, POINTER(c_double)],
+            "kvpool_share_bandwidth": [vp, vp, c_uint32, vp],
+            "kvpool_calibrate": [vp, c_int, c_uint64, c_uint32, vp],
+            "kvpool_bandwidths": [vp, vp, vp],
             "kvpool_set_path": [vp, c_int],
             "kvpool_set_tuning": [vp, vp],
             "kvpool_reserve_staging": [vp, c_uint64],
@@ -183,6 +187,15 @@ def kvpool_plan_layer(w: Sequence[int], K: int, with_map: bool = True):
     return (counts, dev, slot) if with_map else counts
 
 
+def kvpool_share_bandwidth(alone_gbps: Sequence[float], link_group: Sequence[int]) -> np.ndarray:
+    a = np.ascontiguousarray(alone_gbps, dtype=np.float64)
+    g = np.ascontiguousarray(link_group, dtype=np.uint32)
+    assert a.shape == g.shape
+    out = np.zeros(a.shape[0], dtype=np.float64)
+    _ck(lib().kvpool_share_bandwidth(a.ctypes.data, g.ctypes.data, a.shape[0], out.ctypes.data))
+    return out
+
+
 def kvpool_validate_table(table: np.ndarray, nphys: int) -> None:
     """Raises KvPoolError(EINVAL) unless `table` (host int32) names distinct physical blocks in [0, nphys)."""
     t = np.ascontiguousarray(table, dtype=np.int32)
@@ -240,12 +253,13 @@ class KvPool:
     def __init__(self, bandwidth_gbps: Sequence[float], capacity_bytes: Sequence[int], *, n_layers: int, n_kv_heads: int,
                  head_dim: int, block_tokens: int = 16, elem_bytes: int = 2, cuda_device: int = 0,
                  numa_nodes: Optional[Sequence[int]] = None, dev_flags: Optional[Sequence[int]] = None,
-                 gpus: Optional[Sequence[int]] = None):
+                 gpus: Optional[Sequence[int]] = None, link_groups: Optional[Sequence[int]] = None):
         n = len(bandwidth_gbps)
         descs = (DeviceDesc * n)()
         for i in range(n):
             descs[i] = DeviceDesc(float(bandwidth_gbps[i]), int(capacity_bytes[i]), int(numa_nodes[i]) if numa_nodes else -1,
-                                  int(dev_flags[i]) if dev_flags else 0, int(gpus[i]) if gpus else -1, 0)
+                                  int(dev_flags[i]) if dev_flags else 0, int(gpus[i]) if gpus else -1,
+                                  int(link_groups[i]) if link_groups else 0)
         self.geometry = Geometry(n_layers, block_tokens, n_kv_heads, head_dim, elem_bytes)
         self.kvb = block_tokens * n_kv_heads * head_dim * elem_bytes
         self.payload = 2 * self.kvb
@@ -274,6 +288,18 @@ class KvPool:
         g = c_double()
         _ck(lib().kvpool_measure_bandwidth(self.handle, dev, direction, nbytes, iters, byref(g)))
         return g.value
+
+    def calibrate(self, direction: int = 0, nbytes: int = 256 << 20, iters: int = 5) -> np.ndarray:
+        """Measure every device, divide what link groups share, install the result as the pool's bandwidths; returns them."""
+        out = np.zeros(self.n_devices, dtype=np.float64)
+        _ck(lib().kvpool_calibrate(self.handle, direction, int(nbytes), iters, out.ctypes.data))
+        return out
+
+    def bandwidths(self) -> Tuple[np.ndarray, np.ndarray]:
+        """(b_i the pool places by, link group of each device)."""
+        b, g = np.zeros(self.n_devices, dtype=np.float64), np.zeros(self.n_devices, dtype=np.uint32)
+        _ck(lib().kvpool_bandwidths(self.handle, b.ctypes.data, g.ctypes.data))
+        return b, g
 
     def set_path(self, path: int) -> None:
         _ck(lib().kvpool_set_path(self.handle, path))

@@ -79,13 +79,20 @@ __device__ __forceinline__ Piece decode(const LayerArgs& a, uint64_t t, uint32_t
   const uint32_t per_unit = 2u * pieces;
   const uint32_t local = static_cast<uint32_t>(t / per_unit);
   const uint32_t r = static_cast<uint32_t>(t - static_cast<uint64_t>(local) * per_unit);
-  const uint32_t j = a.j0 + local;
   const uint32_t half = r >= pieces ? 1u : 0u;  // 0: K block, 1: V block
   const uint32_t c = r - half * pieces;
-  const int32_t phys = __ldg(a.table + j);
-  const uint32_t d = __ldg(a.dev + j);
-  const uint32_t s = __ldg(a.slot + j);
   const uint32_t off = c * piece_bytes;
+  uint32_t j, d, s;
+  if (a.order) {  // device-major chunk: unit `local` of one device's slot range (uniform across the launch)
+    j = __ldg(a.order + a.j0 + local);
+    d = 0;
+    s = local;
+  } else {
+    j = a.j0 + local;
+    d = __ldg(a.dev + j);
+    s = __ldg(a.slot + j);
+  }
+  const int32_t phys = __ldg(a.table + j);
   Piece p;
   p.paged = (half ? a.v_base : a.k_base) + static_cast<uint64_t>(phys) * a.stride + off;
   p.pooled = reinterpret_cast<uint8_t*>(a.pool_base[d]) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;

@@ -22,6 +22,11 @@ struct LayerArgs {
   const uint32_t* slot;
   uint32_t K;    // number of units this launch moves ...
   uint32_t j0;   // ... starting at logical block j0 (table/dev/slot are indexed by j0 + local index)
+  // Device-major chunk (staged path, layers larger than a staging slot): when `order` is set the launch moves K
+  // consecutive SLOTS of ONE pool device instead of K consecutive logical blocks: unit u is logical block
+  // order[j0 + u] (the inverse map of that device, ascending in slot) and its pool side is pool_base[0] + u*P, so the
+  // chunk is one contiguous piece of that device's stripe: ONE copy per chunk.  dev / slot are not read.
+  const uint32_t* order;
   uint32_t kvb;
   unsigned long long* span;  // profiling only (else null): device {min start, max end} of the launch in %globaltimer ns
   unsigned long long* bad;   // table check only (else null): counts table entries outside [0, nphys_check)

@@ -72,6 +72,8 @@ struct LayerMap {
   std::vector<uint32_t> order;    // [K] order[start[i] + s] = logical block stored at slot s of device i (ascending in s)
   const uint8_t* dev_d = nullptr; // device copies
   const uint32_t* slot_d = nullptr;
+  const uint32_t* order_d = nullptr;
+  uint64_t host_blocks = 0;       // blocks of the layer that sit on host-memory devices (the rest: HBM-type devices)
 };
 
 struct LayerState {
@@ -144,6 +146,8 @@ struct kvpool {
   std::vector<double> bandwidth;
   std::vector<uint64_t> w;
   std::vector<HostBuffer> bufs;
+  std::vector<uint32_t> link_group;  // [N] kvpool_device_desc.link_group: devices of one group share io / io_out streams
+  std::vector<cudaStream_t> own_streams;  // every stream created for io / io_out, once (members of a group alias one)
   uint32_t hbm_mask = 0;  // bit i: pool device i is GPU memory (KVPOOL_DEV_HBM): reached by the kernels directly, never staged or copied
   std::vector<StripeAllocator> alloc;
   std::vector<cudaStream_t> io;      // one I/O stream per pool device ("independent I/O streams"): host -> GPU copies
@@ -192,7 +196,8 @@ void default_tuning(kvpool* p) {
   p->tune.bulk_chunk = 16384;
   p->tune.bulk_stages = 6;
   p->tune.bulk_warps = 2;
-  p->tune.stage_slots = 4;
+  p->tune.stage_slots = 2;                   // one slot fills while the other drains; the kernels take ~2 % of a copy's time
+  p->tune.stage_chunk_bytes = 256ull << 20;  // ring <= 512 MiB whatever the context length (larger layers: device-major chunks)
   p->tune.vec_threads = 512;
   p->tune.vec_unroll = 8;
   p->tune.group_bytes = 64ull << 20;
@@ -212,8 +217,7 @@ void free_slots(kvpool* p) {
 }
 
 int sync_pool_streams(kvpool* p) {
-  for (auto s : p->io) CU(cudaStreamSynchronize(s));
-  for (auto s : p->io_out) CU(cudaStreamSynchronize(s));
+  for (auto s : p->own_streams) CU(cudaStreamSynchronize(s));
   if (p->join_out) CU(cudaStreamSynchronize(p->join_out));
   return KVPOOL_OK;
 }
@@ -360,7 +364,10 @@ bool use_staged(const kvpool* p, const LayerState& L) {
   for (uint32_t i = 0; i < p->n; ++i) host_blocks |= L.map->counts[i] && !is_hbm(p, i);
   if (!host_blocks) return false;
   if (p->path == KVPOOL_PATH_STAGED) return true;
-  return L.map->K * p->payload >= p->tune.auto_threshold_bytes;
+  // judged by what would travel through the copy engines: in a pool with HBM-type devices the host devices' share of a
+  // layer is small (Eq. 1 gives a 55 GB/s link 2 % next to 3 TB/s of HBM); below the threshold the same kernel that
+  // reaches the HBM stripes in place also stores / loads the mapped host stripes, instead of a few latency-bound copies
+  return L.map->host_blocks * p->payload >= p->tune.auto_threshold_bytes;
 }
 
 constexpr uint32_t kSpanCap = 16384;  // profiled launches between two reads that also get a device-clock span
@@ -525,7 +532,6 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     if (devs[i].flags & ~(KVPOOL_DEV_WRITE_COMBINED | KVPOOL_DEV_NUMA_STRICT | KVPOOL_DEV_HBM | KVPOOL_DEV_CUDA_HOSTALLOC)) return fail(KVPOOL_EINVAL, "create: device %u unknown flags", i);
     if ((devs[i].flags & KVPOOL_DEV_HBM) && (devs[i].flags & ~KVPOOL_DEV_HBM)) return fail(KVPOOL_EINVAL, "create: device %u: KVPOOL_DEV_HBM excludes the host-memory flags", i);
     if (devs[i].numa_node < KVPOOL_NUMA_AUTO) return fail(KVPOOL_EINVAL, "create: device %u: numa_node %d", i, devs[i].numa_node);
-    if (devs[i].reserved != 0) return fail(KVPOOL_EINVAL, "create: device %u: reserved must be 0", i);
   }
   if (!quantise_weights(bw.data(), n_devs, w.data())) return fail(KVPOOL_EINVAL, "create: bandwidth must be positive (>= 0.0005 GB/s)");
 
@@ -551,8 +557,7 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
   default_tuning(p.get());
   auto cleanup = [&]() {
     for (auto& b : p->bufs) host_buffer_free(&b);
-    for (auto s : p->io) if (s) cudaStreamDestroy(s);
-    for (auto s : p->io_out) if (s) cudaStreamDestroy(s);
+    for (auto s : p->own_streams) cudaStreamDestroy(s);
     if (p->table_arena) cudaFree(p->table_arena);
     if (p->table_arena_host) cudaFreeHost(p->table_arena_host);
     if (p->upload) cudaStreamDestroy(p->upload);
@@ -573,13 +578,23 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     }
     p->alloc.emplace_back(devs[i].capacity_bytes);
   }
+  // one I/O stream per direction and per independent resource: a device of its own (link_group 0) gets its own pair, the
+  // members of a link group share the pair of the group's first member, so their copies run in the order they were asked for
   p->io.resize(n_devs, nullptr);
   p->io_out.resize(n_devs, nullptr);
-  for (auto* v : {&p->io, &p->io_out})
-    for (auto& s : *v) {
-      cudaError_t e = cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking);
+  p->link_group.resize(n_devs);
+  for (uint32_t i = 0; i < n_devs; ++i) {
+    p->link_group[i] = devs[i].link_group;
+    uint32_t first = i;
+    for (uint32_t j = 0; j < i && devs[i].link_group; ++j)
+      if (devs[j].link_group == devs[i].link_group) { first = j; break; }
+    if (first != i) { p->io[i] = p->io[first]; p->io_out[i] = p->io_out[first]; continue; }
+    for (auto* v : {&p->io, &p->io_out}) {
+      cudaError_t e = cudaStreamCreateWithFlags(&(*v)[i], cudaStreamNonBlocking);
       if (e != cudaSuccess) { cleanup(); return fail(KVPOOL_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)); }
+      p->own_streams.push_back((*v)[i]);
     }
+  }
   if (cudaMalloc(reinterpret_cast<void**>(&p->table_arena), kTableArenaBytes) != cudaSuccess) {
     cudaGetLastError();
     cleanup();
@@ -604,8 +619,7 @@ int kvpool_destroy(kvpool_t* p) {
   for (auto* pl : p->live) destroy_placement(p, pl);
   p->live.clear();
   free_slots(p);
-  for (auto s : p->io) cudaStreamDestroy(s);
-  for (auto s : p->io_out) cudaStreamDestroy(s);
+  for (auto s : p->own_streams) cudaStreamDestroy(s);
   for (auto& b : p->bufs) host_buffer_free(&b);
   if (p->table_arena) cudaFree(p->table_arena);
   if (p->table_arena_host) cudaFreeHost(p->table_arena_host);
@@ -634,7 +648,7 @@ int kvpool_set_bandwidth(kvpool_t* p, const double* bw) {
 
 int kvpool_measure_bandwidth(kvpool_t* p, uint32_t dev, int direction, uint64_t bytes, uint32_t iters, double* gbps_out) {
   PoolLock lock__(p);
-  if (!p || !gbps_out || dev >= p->n || bytes == 0 || iters == 0 || (direction != 0 && direction != 1))
+  if (!p || !gbps_out || dev >= p->n || bytes == 0 || iters == 0 || direction < 0 || direction > KVPOOL_MEASURE_KERNEL_OFFLOAD)
     return fail(KVPOOL_EINVAL, "measure_bandwidth: bad arguments");
   if (bytes > p->bufs[dev].bytes) return fail(KVPOOL_EINVAL, "measure_bandwidth: %llu bytes exceed the pool buffer", (unsigned long long)bytes);
   if (!p->live.empty()) return fail(KVPOOL_ESTATE, "measure_bandwidth: %zu placements are live", p->live.size());
@@ -645,9 +659,32 @@ int kvpool_measure_bandwidth(kvpool_t* p, uint32_t dev, int direction, uint64_t 
   CU(cudaEventCreate(&e0));
   CU(cudaEventCreate(&e1));
   std::vector<float> ms(iters);
-  cudaStream_t s = direction == 0 ? p->io[dev] : p->io_out[dev];
+  const bool by_kernel = direction >= KVPOOL_MEASURE_KERNEL_RETRIEVE, towards_gpu = direction == 0 || direction == KVPOOL_MEASURE_KERNEL_RETRIEVE;
+  cudaStream_t s = towards_gpu ? p->io[dev] : p->io_out[dev];
   int rc = KVPOOL_OK;
-  if (direction == 0 && !is_hbm(p, dev)) {
+  // kernel modes: K blocks, block u at slot u of the device's buffer and at physical block u of the scratch paged layout
+  // (K plane then V plane): one device-major launch whose inverse map and block table are both the identity
+  const uint32_t K = static_cast<uint32_t>(std::min<uint64_t>(bytes / p->payload, 0x7fffffffull));
+  uint32_t* ident = nullptr;
+  LayerArgs ka{};
+  if (by_kernel) {
+    if (K == 0) { cudaFree(scratch); cudaEventDestroy(e0); cudaEventDestroy(e1); return fail(KVPOOL_EINVAL, "measure_bandwidth: fewer bytes than one KV cache (%llu)", (unsigned long long)p->payload); }
+    bytes = static_cast<uint64_t>(K) * p->payload;
+    std::vector<uint32_t> h(K);
+    std::iota(h.begin(), h.end(), 0u);
+    CU(cudaMalloc(reinterpret_cast<void**>(&ident), static_cast<uint64_t>(K) * 4));
+    CU(cudaMemcpyAsync(ident, h.data(), static_cast<uint64_t>(K) * 4, cudaMemcpyHostToDevice, s));
+    CU(cudaStreamSynchronize(s));
+    ka.k_base = static_cast<uint8_t*>(scratch);
+    ka.v_base = static_cast<uint8_t*>(scratch) + static_cast<uint64_t>(K) * p->kvb;
+    ka.stride = p->kvb;
+    ka.table = reinterpret_cast<const int32_t*>(ident);
+    ka.order = ident;
+    ka.K = K;
+    ka.kvb = static_cast<uint32_t>(p->kvb);
+    ka.pool_base[0] = reinterpret_cast<uint64_t>(p->bufs[dev].dev_alias);
+  }
+  if (towards_gpu && !is_hbm(p, dev)) {
     // Pages the CPU has just zeroed sit partly in its caches; host->GPU DMA reads of such lines run 5 % slow until a DMA
     // write has claimed them (measured: 52 -> 55.6 GB/s after one pass).  Stripes are always written by an offload
     // before a retrieve reads them, so that is the state to measure: write the region once (no placement is live).
@@ -656,20 +693,64 @@ int kvpool_measure_bandwidth(kvpool_t* p, uint32_t dev, int direction, uint64_t 
   }
   for (uint32_t it = 0; it < iters + 1 && rc == KVPOOL_OK; ++it) {  // first pass is a warm-up
     cudaEventRecord(e0, s);
-    cudaError_t e = direction == 0 ? cudaMemcpyAsync(scratch, pool_bytes(p, dev), bytes, cudaMemcpyDefault, s)
-                                   : cudaMemcpyAsync(pool_bytes(p, dev), scratch, bytes, cudaMemcpyDefault, s);
+    cudaError_t e;
+    if (by_kernel) {
+      e = launch_layer_copy(ka, !towards_gpu, launch_cfg(p, !is_hbm(p, dev)), s);
+      p->n_kernels++;
+    } else {
+      e = towards_gpu ? cudaMemcpyAsync(scratch, pool_bytes(p, dev), bytes, cudaMemcpyDefault, s)
+                      : cudaMemcpyAsync(pool_bytes(p, dev), scratch, bytes, cudaMemcpyDefault, s);
+      p->n_memcpys++;
+    }
     cudaEventRecord(e1, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) { rc = fail(KVPOOL_ECUDA, "measure_bandwidth: %s", cudaGetErrorString(e)); break; }
-    p->n_memcpys++;
     if (it > 0) cudaEventElapsedTime(&ms[it - 1], e0, e1);
   }
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   cudaFree(scratch);
+  if (ident) cudaFree(ident);
   if (rc != KVPOOL_OK) return rc;
   std::sort(ms.begin(), ms.end());
   *gbps_out = static_cast<double>(bytes) / (ms[iters / 2] * 1.0e6);
+  return KVPOOL_OK;
+}
+
+int kvpool_share_bandwidth(const double* alone, const uint32_t* link_group, uint32_t n, double* out) {
+  if (!alone || !link_group || !out || n == 0 || n > KVPOOL_MAX_DEVICES) return fail(KVPOOL_EINVAL, "share_bandwidth: bad arguments");
+  for (uint32_t i = 0; i < n; ++i)
+    if (!(alone[i] > 0.0) || !(alone[i] < 1e300)) return fail(KVPOOL_EINVAL, "share_bandwidth: bandwidth %u is not positive and finite", i);
+  for (uint32_t i = 0; i < n; ++i) {
+    if (link_group[i] == 0) { out[i] = alone[i]; continue; }
+    double best = 0.0, sum = 0.0;  // summed in index order
+    for (uint32_t j = 0; j < n; ++j)
+      if (link_group[j] == link_group[i]) { best = std::max(best, alone[j]); sum += alone[j]; }
+    out[i] = alone[i] * best / sum;
+  }
+  return KVPOOL_OK;
+}
+
+int kvpool_calibrate(kvpool_t* p, int direction, uint64_t bytes, uint32_t iters, double* bandwidth_out) {
+  PoolLock lock__(p);
+  if (!p || bytes == 0 || iters == 0 || direction < 0 || direction > KVPOOL_MEASURE_KERNEL_OFFLOAD) return fail(KVPOOL_EINVAL, "calibrate: bad arguments");
+  if (!p->live.empty()) return fail(KVPOOL_ESTATE, "calibrate: %zu placements are live", p->live.size());
+  std::vector<double> alone(p->n), shared(p->n);
+  for (uint32_t i = 0; i < p->n; ++i) {
+    const int rc = kvpool_measure_bandwidth(p, i, direction, std::min<uint64_t>(bytes, p->bufs[i].bytes), iters, &alone[i]);
+    if (rc != KVPOOL_OK) return rc;
+  }
+  int rc = kvpool_share_bandwidth(alone.data(), p->link_group.data(), p->n, shared.data());
+  if (rc == KVPOOL_OK) rc = kvpool_set_bandwidth(p, shared.data());
+  if (rc != KVPOOL_OK) return rc;
+  if (bandwidth_out) std::copy(shared.begin(), shared.end(), bandwidth_out);
+  return KVPOOL_OK;
+}
+
+int kvpool_bandwidths(const kvpool_t* p, double* bandwidth_out, uint32_t* link_group_out) {
+  if (!p) return fail(KVPOOL_EINVAL, "bandwidths: null pool");
+  if (bandwidth_out) std::copy(p->bandwidth.begin(), p->bandwidth.end(), bandwidth_out);
+  if (link_group_out) std::copy(p->link_group.begin(), p->link_group.end(), link_group_out);
   return KVPOOL_OK;
 }
 
@@ -766,7 +847,9 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
       for (uint32_t i = 0; i < N; ++i) { m->start[i] = acc; acc += m->counts[i]; }
       m->order.resize(K);
       for (uint64_t j = 0; j < K; ++j) m->order[m->start[m->dev[j]] + m->slot[j]] = static_cast<uint32_t>(j);
-      table_bytes += (K * 5 + 255) / 256 * 256 + 256;
+      for (uint32_t i = 0; i < N; ++i)
+        if (!is_hbm(p, i)) m->host_blocks += m->counts[i];
+      table_bytes += 2 * ((K * 4 + 255) / 256 * 256) + (K + 255) / 256 * 256;
       it = by_k.emplace(K, std::move(m)).first;
     }
     pl->layers[l].map = it->second;
@@ -834,6 +917,9 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
       if (m.K == 0) continue;
       m.slot_d = reinterpret_cast<const uint32_t*>(pl->tables_d + off);
       memcpy(host + off, m.slot.data(), m.K * 4);
+      off += (m.K * 4 + 255) / 256 * 256;
+      m.order_d = reinterpret_cast<const uint32_t*>(pl->tables_d + off);  // per-device inverse map, for device-major chunks
+      memcpy(host + off, m.order.data(), m.K * 4);
       off += (m.K * 4 + 255) / 256 * 256;
       m.dev_d = pl->tables_d + off;
       memcpy(host + off, m.dev.data(), m.K);
@@ -928,6 +1014,7 @@ static uint64_t blocks_per_slot(const kvpool* p) {
 struct ChunkPlan {
   uint32_t lo[KVPOOL_MAX_DEVICES], hi[KVPOOL_MAX_DEVICES];
   uint64_t off[KVPOOL_MAX_DEVICES];  // byte offset of device i's share inside the slot
+  uint64_t host_bytes = 0;           // what the chunk moves to / from host-memory devices
   bool host_blocks = false, hbm_blocks = false;
 };
 static ChunkPlan plan_chunk(const kvpool* p, const LayerState& L, uint32_t first, uint32_t n) {
@@ -941,7 +1028,18 @@ static ChunkPlan plan_chunk(const kvpool* p, const LayerState& L, uint32_t first
     c.host_blocks = true;
     acc += static_cast<uint64_t>(c.hi[i] - c.lo[i]) * p->payload;
   }
+  c.host_bytes = acc;
   return c;
+}
+
+// Make `waiter` wait for everything enqueued on `s` so far (a pooled non-timing event; the wait captures the record).
+static int stream_after(kvpool* p, cudaStream_t waiter, cudaStream_t s) {
+  cudaEvent_t m = nullptr;
+  CU(take_event(p, &m));
+  CU(cudaEventRecord(m, s));
+  CU(cudaStreamWaitEvent(waiter, m, 0));
+  p->ev_free.push_back(m);
+  return KVPOOL_OK;
 }
 static void chunk_bases(const kvpool* p, const LayerState& L, const ChunkPlan& c, const StageSlot* slot, LayerArgs* a) {
   for (uint32_t i = 0; i < p->n; ++i) {
@@ -967,10 +1065,9 @@ int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, ui
   const uint32_t N = p->n;
   LayerArgs a = base_args(p, L, k_base, v_base, stride, table_of(pl, layer, table));
   bool staged = use_staged(p, L);
-  if (staged && n_blocks != L.map->K) {  // a range is judged by its own size and by where its own blocks sit
-    staged = plan_chunk(p, L, first_block, n_blocks).host_blocks &&
-             (p->path == KVPOOL_PATH_STAGED || static_cast<uint64_t>(n_blocks) * p->payload >= p->tune.auto_threshold_bytes);
-  }
+  const ChunkPlan whole = plan_chunk(p, L, first_block, n_blocks);
+  if (staged && n_blocks != L.map->K)  // a range is judged by its own size and by where its own blocks sit
+    staged = whole.host_blocks && (p->path == KVPOOL_PATH_STAGED || whole.host_bytes >= p->tune.auto_threshold_bytes);
 
   if (!staged) {
     // zero-copy: one kernel gathers the paged blocks and stores them straight into the mapped host stripes
@@ -994,21 +1091,53 @@ int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, ui
   // gathers every chunk's kernel and copies — the per-device I/O streams never wait for one another
   cudaStream_t lead = p->join_out;
   if (L.landed_pending) CU(cudaStreamWaitEvent(lead, L.landed, 0));  // `landed` keeps covering what was offloaded before
-  bool first_kernel = true;
-  for (uint32_t first = first_block, end = first_block + n_blocks; first < end;) {
-    const uint32_t n = static_cast<uint32_t>(std::min<uint64_t>(per_slot, end - first));
-    const ChunkPlan c = plan_chunk(p, L, first, n);
-    a.j0 = first;
-    a.K = n;
-    first += n;
-    // an earlier offload of this layer may still be writing the HBM-type stripes the kernel stores into
-    if (c.hbm_blocks && first_kernel && L.landed_pending) { CU(cudaStreamWaitEvent(s, L.landed, 0)); first_kernel = false; }
-    if (!c.host_blocks) {  // the whole chunk sits on HBM-type devices: nothing to stage, no slot taken
+  // an earlier offload of this layer may still be writing the HBM-type stripes the kernel stores into
+  if (whole.hbm_blocks && L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
+  if (n_blocks > per_slot) {
+    // DEVICE-MAJOR chunks: a chunk is a run of consecutive slots of one device's stripe, gathered by a launch that finds its
+    // logical blocks through that device's inverse map, and leaves the slot as ONE copy.  An HBM-type device's share is
+    // gathered in place by one launch.
+    a.order = L.map->order_d;
+    for (uint32_t i = 0; i < N; ++i) {
+      for (uint32_t lo = whole.lo[i]; lo < whole.hi[i];) {
+        const uint32_t n = is_hbm(p, i) ? whole.hi[i] - lo : static_cast<uint32_t>(std::min<uint64_t>(per_slot, whole.hi[i] - lo));
+        a.j0 = L.map->start[i] + lo;
+        a.K = n;
+        uint8_t* const stripe_at = static_cast<uint8_t*>(p->bufs[i].dev_alias) + L.stripe_off[i] + static_cast<uint64_t>(lo) * p->payload;
+        lo += n;
+        if (is_hbm(p, i)) {
+          a.pool_base[0] = reinterpret_cast<uint64_t>(stripe_at);
+          rc = launch_counted(p, a, true, false, s);
+          if (rc != KVPOOL_OK) return rc;
+          continue;
+        }
+        StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
+        rc = wait_slot_free(p, slot, s);
+        if (rc != KVPOOL_OK) return rc;
+        slot.copies_after_kernel = 0;
+        a.pool_base[0] = reinterpret_cast<uint64_t>(slot.buf);
+        rc = launch_counted(p, a, true, false, s);
+        if (rc != KVPOOL_OK) return rc;
+        CU(cudaEventRecord(slot.kernel_done, s));
+        CU(cudaStreamWaitEvent(p->io_out[i], slot.kernel_done, 0));
+        if (L.landed_pending) CU(cudaStreamWaitEvent(p->io_out[i], L.landed, 0));  // the previous offload of this layer
+        CU(cudaMemcpyAsync(static_cast<uint8_t*>(p->bufs[i].host) + (stripe_at - static_cast<uint8_t*>(p->bufs[i].dev_alias)), slot.buf,
+                           static_cast<uint64_t>(n) * p->payload, cudaMemcpyDeviceToHost, p->io_out[i]));
+        p->n_memcpys++;
+        CU(cudaEventRecord(slot.copy_done[i], p->io_out[i]));
+        slot.copies_after_kernel = 1u << i;
+        CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
+      }
+    }
+  } else {
+    const ChunkPlan& c = whole;  // the range fits one staging slot: one pack launch, one copy per device
+    a.j0 = first_block;
+    a.K = n_blocks;
+    if (!c.host_blocks) {  // the whole range sits on HBM-type devices: nothing to stage, no slot taken
       chunk_bases(p, L, c, nullptr, &a);
       rc = launch_counted(p, a, true, false, s);
       if (rc != KVPOOL_OK) return rc;
-      continue;
-    }
+    } else {
     StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
     rc = wait_slot_free(p, slot, s);
     if (rc != KVPOOL_OK) return rc;
@@ -1028,9 +1157,13 @@ int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, ui
       CU(cudaEventRecord(slot.copy_done[i], p->io_out[i]));
       slot.copies_after_kernel |= 1u << i;
     }
-    CU(cudaStreamWaitEvent(lead, slot.kernel_done, 0));  // covers the HBM-type stripes the kernel wrote
     for (uint32_t i = 0; i < N; ++i)
       if (slot.copies_after_kernel >> i & 1u) CU(cudaStreamWaitEvent(lead, slot.copy_done[i], 0));
+    }
+  }
+  if (whole.hbm_blocks) {  // `landed` also covers the HBM-type stripes the kernels on `s` wrote in place
+    rc = stream_after(p, lead, s);
+    if (rc != KVPOOL_OK) return rc;
   }
   mark_offloaded(L, first_block, n_blocks);  // every chunk is enqueued (an error above leaves the range unflagged: retrieve -> ESTATE)
   CU(cudaEventRecord(L.landed, lead));
@@ -1063,10 +1196,11 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const uint32_t N = p->n;
   LayerArgs a = base_args(p, L, k_base, v_base, stride, table_of(pl, layer, table));
-  const uint64_t range_bytes = static_cast<uint64_t>(n_blocks) * p->payload;
-  bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && range_bytes >= p->tune.auto_threshold_bytes));
-  // a range whose blocks all sit on HBM-type devices has nothing to stage
-  if (staged) staged = plan_chunk(p, L, first_block, n_blocks).host_blocks;
+  const ChunkPlan whole = plan_chunk(p, L, first_block, n_blocks);
+  // staged only if something travels through the copy engines (a range whose blocks all sit on HBM-type devices has
+  // nothing to stage) and, on the auto path, enough of it (use_staged)
+  const bool staged = !all_hbm(p) && whole.host_blocks &&
+                      (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && whole.host_bytes >= p->tune.auto_threshold_bytes));
   settle_landed(L);
 
   if (!staged) {
@@ -1083,20 +1217,45 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   // larger than a slot travels in chunks of logical blocks: the copies of chunk c+1 overlap the unpack of chunk c.
   const uint64_t per_slot = p->slots.empty() ? 0 : blocks_per_slot(p);
   if (per_slot == 0) return fail(KVPOOL_ESTATE, "retrieve: no staging slot (the placement was made while the path was zero-copy)");
-  bool first_kernel = true;
-  for (uint32_t first = first_block, end = first_block + n_blocks; first < end;) {
-    const uint32_t n = static_cast<uint32_t>(std::min<uint64_t>(per_slot, end - first));
-    const ChunkPlan c = plan_chunk(p, L, first, n);
-    a.j0 = first;
-    a.K = n;
-    first += n;
-    if (c.hbm_blocks && first_kernel && L.landed_pending) { CU(cudaStreamWaitEvent(s, L.landed, 0)); first_kernel = false; }
-    if (!c.host_blocks) {  // read in place by the unpack kernel: no slot taken (a slot recycled without waits could be
-      chunk_bases(p, L, c, nullptr, &a);  // overwritten under an earlier offload's copy)
-      rc = launch_counted(p, a, false, false, s);
-      if (rc != KVPOOL_OK) return rc;
-      continue;
+  if (whole.hbm_blocks && L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));  // HBM-type stripes are read in place
+  if (n_blocks > per_slot) {
+    // DEVICE-MAJOR chunks (see kvpool_offload_range): one copy fills a slot with a run of one device's slots, one launch
+    // scatters them through that device's inverse map; the copy of the next chunk overlaps it
+    a.order = L.map->order_d;
+    for (uint32_t i = 0; i < N; ++i) {
+      for (uint32_t lo = whole.lo[i]; lo < whole.hi[i];) {
+        const uint32_t n = is_hbm(p, i) ? whole.hi[i] - lo : static_cast<uint32_t>(std::min<uint64_t>(per_slot, whole.hi[i] - lo));
+        a.j0 = L.map->start[i] + lo;
+        a.K = n;
+        const uint64_t at = L.stripe_off[i] + static_cast<uint64_t>(lo) * p->payload;
+        lo += n;
+        if (is_hbm(p, i)) {
+          a.pool_base[0] = reinterpret_cast<uint64_t>(static_cast<uint8_t*>(p->bufs[i].dev_alias) + at);
+          rc = launch_counted(p, a, false, false, s);
+          if (rc != KVPOOL_OK) return rc;
+          continue;
+        }
+        StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
+        rc = wait_slot_free(p, slot, p->io[i]);
+        if (rc != KVPOOL_OK) return rc;
+        if (L.landed_pending) CU(cudaStreamWaitEvent(p->io[i], L.landed, 0));
+        slot.copies_after_kernel = 0;
+        CU(cudaMemcpyAsync(slot.buf, static_cast<uint8_t*>(p->bufs[i].host) + at, static_cast<uint64_t>(n) * p->payload, cudaMemcpyHostToDevice, p->io[i]));
+        p->n_memcpys++;
+        CU(cudaEventRecord(slot.copy_done[i], p->io[i]));
+        CU(cudaStreamWaitEvent(s, slot.copy_done[i], 0));
+        a.pool_base[0] = reinterpret_cast<uint64_t>(slot.buf);
+        rc = launch_counted(p, a, false, false, s);
+        if (rc != KVPOOL_OK) return rc;
+        CU(cudaEventRecord(slot.kernel_done, s));
+      }
     }
+    return note_use(p, pl, s);
+  }
+  {
+    const ChunkPlan& c = whole;  // the range fits one staging slot: one copy per device, one unpack launch
+    a.j0 = first_block;
+    a.K = n_blocks;
     StageSlot& slot = p->slots[p->slot_cursor++ % p->slots.size()];
     for (uint32_t i = 0; i < N; ++i) {
       if (c.hi[i] == c.lo[i] || is_hbm(p, i)) continue;
@@ -1153,6 +1312,7 @@ struct LayerGroup {  // a run of layers of one batched call that moves as one un
   uint32_t q[kMaxBatch];  // indices into the call's pointer arrays (layer = first + q)
   uint32_t n = 0;
   uint64_t bytes = 0;
+  uint64_t host_bytes = 0;  // of which on host-memory devices (what the staged path would send through the copy engines)
 };
 struct BatchCall {
   kvpool* p;
@@ -1320,7 +1480,7 @@ int issue_group(const BatchCall& c, const LayerGroup& g) {
 
 int issue_group_work(const BatchCall& c, const LayerGroup& g) {
   kvpool* p = c.p;
-  const bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && g.bytes >= p->tune.auto_threshold_bytes));
+  const bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && g.host_bytes >= p->tune.auto_threshold_bytes));
   if (!staged) return issue_zero_copy_group(c, g);
   if (g.n > 1) {
     const int rc = issue_staged_group(c, g);
@@ -1374,6 +1534,7 @@ static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32
     }
     g.q[g.n++] = q;
     g.bytes += bytes;
+    g.host_bytes += L.map->host_blocks * p->payload;
     units += L.map->K;
     if (g.bytes >= cap) {  // on every path: a group is also the grain at which a consumer's per-layer events fire
       const int rc = issue_group(c, g);

@@ -58,7 +58,10 @@ def test_random_sequences_match_the_oracle(seed):
     flags = [kv.DEV_HBM if rng.random() < 0.3 else 0 for _ in range(n_dev)]
     flags[int(rng.integers(0, n_dev))] = 0                                     # at least one host device
     cap = 4 * L * KMAX * 2 * ELEMS * 2                                         # room for 4 placements on any one device
-    pool = kv.KvPool(bw, [cap] * n_dev, n_layers=L, dev_flags=flags, **GEOM)
+    # link groups (devices of one group share an I/O stream per direction) from a generator of their own, so that the
+    # operation sequences of the seeds stay what they were before groups existed
+    groups = [int(x) for x in np.random.default_rng(977 + seed).integers(0, 3, size=n_dev)]
+    pool = kv.KvPool(bw, [cap] * n_dev, n_layers=L, dev_flags=flags, link_groups=groups, **GEOM)
     src_np = [[rng.integers(0, 0x7F80, size=(2, NPHYS, ELEMS), dtype=np.uint16) for _ in range(L)] for _ in range(2)]
     src = [[torch.from_numpy(a.view(np.int16)).to(dev) for a in vs] for vs in src_np]
     torch.cuda.synchronize()

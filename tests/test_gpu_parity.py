@@ -318,13 +318,24 @@ def test_full_size_configs_every_byte_against_oracle(cfg, path, kernel):
 @pytest.mark.parametrize("path", ["staged", "zerocopy"])
 def test_retrieve_range_partial_and_prefix(path, kernel):
     """kvpool_retrieve_range against the oracle's partial retrieval: prefix, middle, tail, empty and whole ranges."""
+    _retrieve_ranges(path, kernel, {}, None)
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_retrieve_range_larger_than_a_staging_slot_in_device_major_chunks(kernel):
+    """The same ranges under a 2 MiB chunk cap (64 blocks per slot; ranges of 128, 256 and 512 blocks travel device-major),
+    with the pool devices in link groups (shared I/O streams)."""
+    _retrieve_ranges("staged", kernel, {"stage_chunk_bytes": 2 << 20}, [1, 1, 1, 2, 2, 0])
+
+
+def _retrieve_ranges(path, kernel, tuning, link_groups):
     wl = W.make_workload(4, scale=1 / 16, n_layers=2)          # 512 of 768 blocks, 6 buffers 4:4:2:2:1:1
     g, dev = wl.geom, torch.device("cuda:0")
     bw = list(wl.default_weights())
-    pool = make_pool(wl)
+    pool = make_pool(wl, link_groups=link_groups)
     try:
         pool.set_path(PATHS[path])
-        pool.set_tuning(kernel=KERNELS[kernel], link_kernel=KERNELS[kernel])
+        pool.set_tuning(kernel=KERNELS[kernel], link_kernel=KERNELS[kernel], **tuning)
         pl = pool.place(wl.blocks_per_layer(0))
         opl = oracle.place(bw, wl.blocks_per_layer(0))
         rng = np.random.default_rng(13)
@@ -806,7 +817,7 @@ def test_hbm_type_pool_devices_batched_groups_and_ranges(kernel):
     # batched calls: a group's host stripes travel by one copy per HOST device, its HBM stripes inside the kernel
     _run_batched(W.make_workload(1), kv.PATH_AUTO, k, expect_kernels=4, expect_memcpys=4, dev_flags=[0, HBM])
     _run_batched(W.make_workload(1), kv.PATH_STAGED, k, expect_kernels=4, expect_memcpys=0, dev_flags=[HBM, HBM])
-    _run_batched(W.make_workload(1), kv.PATH_ZEROCOPY, k, expect_kernels=2, expect_memcpys=0, dev_flags=[HBM, 0])
+    _run_batched(W.make_workload(1), kv.PATH_ZEROCOPY, k, expect_kernels=4, expect_memcpys=0, dev_flags=[HBM, 0])   # two 64 MiB groups per leg
     wl = W.make_workload(3, scale=1 / 8, n_layers=6)                      # groups {0,1,2} {3,4} {5}; 4 devices, 2 of them host
     _run_batched(wl, kv.PATH_STAGED, k, expect_kernels=6, expect_memcpys=12, dev_flags=[HBM, 0, 0, HBM])
     # partial retrieval over a mixed pool
@@ -986,16 +997,22 @@ def test_host_threads_share_one_pool():
 
 @pytest.mark.parametrize("kernel", list(KERNELS))
 def test_chunked_staging_caps_the_ring_and_keeps_parity(kernel):
-    """tune.stage_chunk_bytes: a layer larger than a staging slot travels in chunks of consecutive logical blocks through
-    compact slots — same stripes, same retrieved tensors, more (smaller) launches and copies, a ring that no longer grows
-    with the layer."""
+    """tune.stage_chunk_bytes: a layer larger than a staging slot travels in DEVICE-MAJOR chunks — runs of consecutive slots
+    of one pool device's stripe, one copy and one launch each (the launch finds its logical blocks through the device's
+    inverse map) — same stripes, same retrieved tensors, a ring that no longer grows with the layer."""
     k = KERNELS[kernel]
     wl = W.make_workload(4, scale=1 / 8, n_layers=3)                      # 1024 blocks x 32 KiB = 32 MiB per layer, 6 devices
     base = run_parity(wl, path=kv.PATH_STAGED, kernel=k)
-    # 5 MiB chunks: 160 blocks each, 7 chunks per layer (the last one ragged); per-layer calls and 4 streams' worth of slots
+    # 5 MiB chunks = 160 slots: stripes of 293, 293, 146, 146, 73, 73 blocks travel as 2 + 2 + 1 + 1 + 1 + 1 chunks
+    counts = oracle.place(list(wl.default_weights()), wl.blocks_per_layer(0))[0].counts
+    chunks = sum(-(-int(c) // 160) for c in counts)
+    assert chunks == 8
     out = run_parity(wl, path=kv.PATH_STAGED, kernel=k, tuning={"stage_chunk_bytes": 5 << 20})
     assert out["bytes_compared"] == base["bytes_compared"]
-    assert out["kernels"] == 7 * base["kernels"] and out["memcpys"] == 7 * base["memcpys"]
+    assert out["kernels"] == chunks * base["kernels"] and out["memcpys"] * 6 == chunks * base["memcpys"]
+    # the same with the devices in link groups (shared I/O streams: {0,1,2} on one, {3,4} on another, 5 alone) and 3 slots
+    out = run_parity(wl, path=kv.PATH_STAGED, kernel=k, tuning={"stage_chunk_bytes": 5 << 20, "stage_slots": 3}, link_groups=[7, 7, 7, 2, 2, 0])
+    assert out["kernels"] == chunks * base["kernels"] and out["memcpys"] * 6 == chunks * base["memcpys"]
     # a chunk smaller than one block still moves one block at a time; 2 slots; mixed host / HBM pool; ragged block size
     g = W.Geometry(n_layers=2, n_kv_heads=1, head_dim=80)
     rng = np.random.default_rng(53)
@@ -1012,7 +1029,7 @@ def test_chunked_staging_caps_the_ring_and_keeps_parity(kernel):
     try:
         pool.set_path(kv.PATH_STAGED)
         free0 = torch.cuda.mem_get_info()[0]
-        pool.set_tuning(stage_chunk_bytes=5 << 20)
+        pool.set_tuning(stage_chunk_bytes=5 << 20, stage_slots=4)
         pl = pool.place(wl.blocks_per_layer(0))
         assert free0 - torch.cuda.mem_get_info()[0] < 4 * (8 << 20)
         pl.release()

@@ -92,6 +92,36 @@ def test_plan_weights_quantisation_and_errors():
         kv.kvpool_plan_layer([1, 0, 1], 5)                     # zero weight
 
 
+def test_share_bandwidth_divides_what_a_link_group_shares():
+    """kvpool_share_bandwidth (include/kvpool.h): host arithmetic in front of Eq. 1, not part of the paper's method — checked
+    against exact rational arithmetic: ungrouped devices keep their bandwidth, a group's shares add up to its best member's
+    rate and keep the members' proportions, m equal members get 1/m each."""
+    from fractions import Fraction
+    rng = np.random.default_rng(5)
+    for _ in range(200):
+        n = int(rng.integers(1, 9))
+        alone = [float(rng.integers(1, 4000)) / 8.0 for _ in range(n)]          # exactly representable
+        groups = [int(x) for x in rng.integers(0, 4, size=n)]
+        out = kv.kvpool_share_bandwidth(alone, groups)
+        for g in set(groups):
+            members = [i for i in range(n) if groups[i] == g]
+            if g == 0:
+                assert all(out[i] == alone[i] for i in members)
+                continue
+            best, total = max(Fraction(alone[i]) for i in members), sum(Fraction(alone[i]) for i in members)
+            for i in members:
+                exact = Fraction(alone[i]) * best / total
+                assert abs(Fraction(float(out[i])) - exact) <= exact * Fraction(1, 2 ** 50)
+                assert out[i] == alone[i] * float(best) / float(total)               # the header's left-to-right double formula
+            assert abs(sum(Fraction(float(out[i])) for i in members) - best) <= best * Fraction(1, 2 ** 48)
+    assert list(kv.kvpool_share_bandwidth([56.0, 56.0, 3000.0, 3000.0], [1, 1, 2, 2])) == [28.0, 28.0, 1500.0, 1500.0]
+    assert list(kv.kvpool_share_bandwidth([56.0, 3000.0], [0, 0])) == [56.0, 3000.0]
+    for bad in ([1.0, 0.0], [float("nan")], [float("inf")]):
+        with pytest.raises(kv.KvPoolError) as e:
+            kv.kvpool_share_bandwidth(bad, [1] * len(bad))
+        assert e.value.code == kv.EINVAL
+
+
 def test_validate_table_accepts_every_workload_table_and_names_the_offending_entry():
     """DESIGN.md R12: distinct entries in [0, nphys) are the caller's contract; the host-side checker states it."""
     for cfg in (1, 3, 5):
