@@ -46,14 +46,14 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["kvpool", "reference"], default="kvpool")
     ap.add_argument("--config", type=int, default=4, help="workload: 1..5 = BASELINE.json configs[0..4], 6 = LLaMA-8B alone at 128K")
-    ap.add_argument("--path", choices=["auto", "staged", "zerocopy"], default="auto")
+    ap.add_argument("--path", choices=["auto", "staged", "zerocopy", "hybrid"], default="auto")
     ap.add_argument("--kernel", choices=["vec16", "bulk"], default=None)
     ap.add_argument("--weights", choices=["config", "measured", "equal"], default="config",
                     help="config: the weights BASELINE.json gives (measured where it gives none)")
     ap.add_argument("--link-ctas", type=int, default=0)
     ap.add_argument("--hbm-ctas", type=int, default=0)
     ap.add_argument("--stage-slots", type=int, default=0)
-    ap.add_argument("--stage-chunk-mib", type=float, default=0.0,
+    ap.add_argument("--stage-chunk-mib", type=float, default=0.0,  # (negative: no cap)
                     help="staged path: cap a staging slot at this many MiB; larger layers travel in chunks (tune.stage_chunk_bytes)")
     ap.add_argument("--link-groups", choices=["shared", "independent"], default="shared",
                     help="shared (default): every host pool buffer names link group 1 - they all sit behind this GPU's one PCIe link, so the "
@@ -62,6 +62,8 @@ def parse_args():
     ap.add_argument("--per-layer", action="store_true",
                     help="issue one kvpool_offload / kvpool_retrieve call per layer in the timed step instead of the batched *_layers calls")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the side lines printed beside the headline (paths.zerocopy / paths.hybrid on the "
+                                                              "same workload, shapes.* = the other two 128K shapes)")
     ap.add_argument("--settle-s", type=float, default=60.0, help="upper bound on the untimed host-settle phase before the timed steps (0 = off)")
     ap.add_argument("--sweep", choices=["hbm", "link"], default=None,
                     help="tuning sweep instead of the benchmark: in-device pack/unpack (hbm) or zero-copy transfer (link) GB/s over launch shapes")
@@ -188,11 +190,42 @@ def cpu_baseline(cfg: int, budget_s: float = 12.0) -> dict:
     while done < wl.geom.n_layers and time.perf_counter() - t_start < budget_s:
         a, b, c = oracle_time_layers(st, 1, True)
         t_off, t_ret, nbytes, done = t_off + a, t_ret + b, nbytes + c, done + 1
-    return {"value": nbytes / t_ret / 1e9, "unit": UNIT, "cores": n_threads, "kind": "oracle",
-            "sample": f"{done} x retrieve of one full layer of config {cfg} ({nbytes / done / 2**20:.0f} MiB each, host paged copy <- host stripes), "
-                      f"one worker thread per pool device (PAPER.md:177); offload {nbytes / t_off / 1e9:.2f} GB/s; "
-                      f"single-thread retrieve {b1 / t_ret1 / 1e9:.2f} GB/s",
-            "host_cores": len(os.sched_getaffinity(0))}
+    out = {"value": nbytes / t_ret / 1e9, "unit": UNIT, "cores": n_threads, "kind": "oracle",
+           "sample": f"{done} x retrieve of one full layer of config {cfg} ({nbytes / done / 2**20:.0f} MiB each, host paged copy <- host stripes), "
+                     f"one worker thread per pool device (PAPER.md:177); offload {nbytes / t_off / 1e9:.2f} GB/s; "
+                     f"single-thread retrieve {b1 / t_ret1 / 1e9:.2f} GB/s",
+           "host_cores": len(os.sched_getaffinity(0))}
+    out["all_cores"] = oracle_all_cores(st, 4.0)
+    return out
+
+
+def oracle_all_cores(st, budget_s: float) -> dict:
+    """The same oracle on every host core the process may use: C threads, each retrieving the sample layer
+    with the single-thread oracle from the same stripes into a destination of its own (the oracle is not changed or tuned:
+    this runs C copies of it side by side)."""
+    import threading
+    oracle, wl, table, pl, src, dst, _, _ = st
+    from paper_2606_14779_b200 import workloads as W
+    C = len(os.sched_getaffinity(0))
+    stripes = oracle.offload_layer(src, table, pl)
+    dsts = [dst] + [W.poison_numpy(src.shape) for _ in range(C - 1)]
+    per = len(table) * wl.geom.payload
+
+    def round_(reps: int) -> float:
+        th = [threading.Thread(target=lambda d=d: [oracle.retrieve_layer(d, table, pl, stripes) for _ in range(reps)]) for d in dsts]
+        t0 = time.perf_counter()
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        return time.perf_counter() - t0
+
+    t1 = round_(1)                                                                  # also touches the destinations' pages
+    reps = max(1, min(16, int(budget_s / max(round_(1), 1e-3))))
+    t = round_(reps)
+    return {"value": C * reps * per / t / 1e9, "unit": UNIT, "cores": C,
+            "sample": f"{C} threads x {reps} x retrieve of the same full layer ({per / 2**20:.0f} MiB) by the single-thread oracle, each into its own "
+                      f"destination; first (page-touching) round {C * per / t1 / 1e9:.2f} GB/s"}
 
 
 def run_reference(args) -> dict:
@@ -223,10 +256,294 @@ def run_reference(args) -> dict:
 # ---------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ---------------------------------------------------------------------------------------------------
+class Rig:
+    """One workload resident on the GPU (seeded source layers, poison-filled destination layers, block tables) and its pool:
+    what a step, an end-to-end pass and a per-layer latency pass need.  Used for the headline configuration and again for
+    the other shapes / paths the bench line reports beside it."""
+
+    def __init__(self, args, cfg: int, path: str, local: int, world: int):
+        import torch
+        from paper_2606_14779_b200 import binding as kv
+        from paper_2606_14779_b200 import workloads as W
+        self.torch, self.kv, self.W, self.args, self.cfg = torch, kv, W, args, cfg
+        self.dev = dev = torch.device("cuda", local)
+        self.wl = wl = W.make_workload(cfg)
+        self.g = g = wl.geom
+        self.R, self.L, self.N = len(wl.requests), g.n_layers, wl.n_pool_devices
+        R, L, N = self.R, self.L, self.N
+        self.elems = g.kvb // 2
+        self.moved = wl.moved_bytes()
+        self.bpl = [wl.blocks_per_layer(r) for r in range(R)]
+        base_w = list(wl.default_weights())
+        share = np.array(base_w) / np.sum(base_w)
+        self.caps = [int(self.moved * s * 1.25) + (L * R + 4) * (g.payload + 4096) for s in share]
+        numa = [i % 2 for i in range(N)] if cfg == 2 else None      # config 2: "on 2 NUMA nodes" (falls back, reported)
+        if numa is None and world > 1:
+            numa = [kv.NUMA_AUTO] * N       # several ranks on one host: each rank's buffers on the NUMA node its own GPU hangs off
+        t0 = time.perf_counter()
+        self.pool = pool = kv.KvPool(base_w, self.caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, block_tokens=g.block_tokens,
+                                     elem_bytes=g.elem_bytes, cuda_device=local, numa_nodes=numa,
+                                     dev_flags=[kv.DEV_CUDA_HOSTALLOC] * N if args.hostalloc else None,
+                                     link_groups=[1] * N if args.link_groups == "shared" else None)
+        self.create_s = time.perf_counter() - t0
+        self.weights_kind = args.weights
+        if args.weights == "measured" or (args.weights == "config" and wl.weights is None):
+            # Eq. 1's "measured bandwidth": every buffer measured alone, what a link group shares divided among its members
+            self.bw = [float(x) for x in pool.calibrate(kv.MEASURE_RETRIEVE, 256 << 20, 5)]
+            self.weights_kind = "kvpool_calibrate: per-buffer H2D cudaMemcpyAsync GB/s, shared within a link group"
+        elif args.weights == "equal":
+            self.bw = [1.0] * N
+            pool.set_bandwidth(self.bw)
+        else:
+            self.bw = base_w
+        tune = {}
+        if args.kernel:
+            tune["kernel"] = tune["link_kernel"] = {"vec16": kv.KERNEL_VEC16, "bulk": kv.KERNEL_BULK}[args.kernel]
+        for k, v in (("link_ctas", args.link_ctas), ("hbm_ctas", args.hbm_ctas), ("stage_slots", args.stage_slots)):
+            if v:
+                tune[k] = v
+        if args.stage_chunk_mib:
+            tune["stage_chunk_bytes"] = int(args.stage_chunk_mib * 2**20) if args.stage_chunk_mib > 0 else 2**64 - 1
+        if tune:
+            pool.set_tuning(**tune)
+        self.set_path(path)
+        self.tn = pool.get_tuning()
+        self.numa_actual = [pool.device_info(i)["numa_node"] for i in range(N)]
+
+        # synthetic paged KV in HBM: seeded N(0,1) bf16 source layers, ONE poison-filled destination tensor (layers are views of
+        # it, so that the end-to-end leg reads its per-layer result samples with one gather + one device->host copy)
+        self.src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+        self.dst_all = W.poison_torch((L, 2, wl.nphys, self.elems), dev)
+        self.dst = [self.dst_all[l] for l in range(L)]
+        self.tables_np = [[np.ascontiguousarray(wl.layer_table(r, l)) for l in range(L)] for r in range(R)]
+        self.tables = [[torch.from_numpy(t).to(dev) for t in row] for row in self.tables_np]
+        # each request's tables back to back in pinned host memory: what kvpool_set_tables uploads in one copy
+        self.packed_pin = [torch.from_numpy(np.concatenate(row).astype(np.int32)).pin_memory() for row in self.tables_np]
+        self.table_bytes = sum(int(t.numel()) * 4 for t in self.packed_pin)
+        samp = [(l, int(self.tables_np[r][l][0])) for r in range(R) for l in range(L) if len(self.tables_np[r][l])]
+        self.samp_l = torch.tensor([a for a, _ in samp], dtype=torch.long, device=dev)
+        self.samp_p = torch.tensor([b for _, b in samp], dtype=torch.long, device=dev)
+        self.sample_pin = torch.empty((len(samp), self.elems), dtype=torch.int16).pin_memory()
+        self.d2h_bytes = len(samp) * g.kvb
+        self.main = torch.cuda.Stream(device=dev)
+        self.streams = [torch.cuda.Stream(device=dev) for _ in range(wl.n_streams)] if wl.n_streams > 1 else [self.main]
+        self.src_k, self.src_v = [x[0] for x in self.src], [x[1] for x in self.src]
+        self.dst_k, self.dst_v = [x[0] for x in self.dst], [x[1] for x in self.dst]
+        self.kmax = max(int(b.max()) for b in self.bpl)
+        torch.cuda.synchronize()
+
+    def set_path(self, path: str) -> None:
+        kv = self.kv
+        self.path = path
+        self.pool.set_path({"auto": kv.PATH_AUTO, "staged": kv.PATH_STAGED, "zerocopy": kv.PATH_ZEROCOPY, "hybrid": kv.PATH_HYBRID}[path])
+
+    def stream_of(self, r: int):
+        return self.streams[r % len(self.streams)]
+
+    def fork(self):
+        if self.streams[0] is not self.main:
+            e = self.torch.cuda.Event()
+            e.record(self.main)
+            for s in self.streams:
+                s.wait_event(e)
+
+    def join(self):
+        if self.streams[0] is not self.main:
+            for s in self.streams:
+                e = self.torch.cuda.Event()
+                e.record(s)
+                self.main.wait_event(e)
+
+    def do_offload(self, pls, own_tables: bool = False):
+        pool, g = self.pool, self.g
+        self.fork()
+        for r in range(self.R):
+            tb = None if own_tables else self.tables[r]
+            if self.args.per_layer:
+                for l in range(self.L):
+                    pool.offload(pls[r], l, self.src_k[l], self.src_v[l], g.kvb, None if own_tables else tb[l], self.stream_of(r))
+            else:
+                pool.offload_layers(pls[r], 0, self.src_k, self.src_v, g.kvb, tb, self.stream_of(r))
+        for r in range(self.R):
+            pool.wait_offloads(pls[r], self.stream_of(r))
+        self.join()
+
+    def do_retrieve(self, pls, own_tables: bool = False, ready=None):
+        """ready: per request a list of L non-timing events the library (batched calls) or this loop (per-layer calls)
+        records when a layer is complete in the paged layout."""
+        pool, g = self.pool, self.g
+        self.fork()
+        for r in range(self.R):
+            s, tb = self.stream_of(r), (None if own_tables else self.tables[r])
+            if self.args.per_layer:
+                for l in range(self.L):
+                    pool.retrieve(pls[r], l, self.dst_k[l], self.dst_v[l], g.kvb, None if own_tables else tb[l], s)
+                    if ready is not None:
+                        ready[r][l].record(s)
+            elif ready is not None:
+                pool.retrieve_layers_signal(pls[r], 0, self.dst_k, self.dst_v, g.kvb, tb, ready[r], s)
+            else:
+                pool.retrieve_layers(pls[r], 0, self.dst_k, self.dst_v, g.kvb, tb, s)
+        self.join()
+
+    def step(self, rec: dict) -> None:
+        """kvpool_place + offload of every layer + retrieve of every layer; the legs timed apart with CUDA events."""
+        torch, pool, main = self.torch, self.pool, self.main
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        t0 = time.perf_counter()
+        pls = [pool.place(self.bpl[r]) for r in range(self.R)]
+        t1 = time.perf_counter()
+        ev[0].record(main)
+        self.do_offload(pls)
+        ev[1].record(main)
+        # the legs are timed apart: without this the retrieve's host->GPU copies (which may run ahead of the caller's
+        # stream) would start under the tail of the offload leg and borrow the link's other direction
+        main.synchronize()
+        pool.synchronize()
+        ev[2].record(main)
+        self.do_retrieve(pls)
+        ev[3].record(main)
+        main.synchronize()
+        for pl in pls:
+            pl.release()
+        rec["place_ms"].append(1e3 * (t1 - t0))
+        rec["offload_ms"].append(ev[0].elapsed_time(ev[1]))
+        rec["retrieve_ms"].append(ev[2].elapsed_time(ev[3]))
+
+    def e2e_pass(self):
+        """Both legs by the host's wall clock through the public API, nothing resident beforehand but the KV itself: per leg
+        ONE upload of the request's block tables from pinned host memory (kvpool_set_tables), the batched call, and for the
+        retrieve a read-back of one block per layer (one gather, one device->host copy).  Returns (offload s, retrieve s)."""
+        torch, pool, main = self.torch, self.pool, self.main
+        pls = [pool.place(self.bpl[r]) for r in range(self.R)]
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for r in range(self.R):
+            pool.set_tables(pls[r], self.packed_pin[r], self.stream_of(r))
+        self.do_offload(pls, own_tables=True)
+        main.synchronize()
+        pool.synchronize()
+        t1 = time.perf_counter()
+        for r in range(self.R):
+            pool.set_tables(pls[r], self.packed_pin[r], self.stream_of(r))
+        self.do_retrieve(pls, own_tables=True)
+        with torch.cuda.stream(main):
+            self.sample_pin.copy_(self.dst_all[self.samp_l, 0, self.samp_p], non_blocking=True)
+        main.synchronize()
+        t2 = time.perf_counter()
+        for pl in pls:
+            pl.release()
+        return t1 - t0, t2 - t1
+
+    def layer_latency_pass(self):
+        """Per-layer retrieve latency as a pipelined consumer sees it: the interval between the completion
+        events of consecutive full layers.  The events are the non-timing ones of kvpool_retrieve_layers_signal; their
+        timestamps are taken on a side stream that waits for them, so the retrieve stream carries no timing event (one
+        recorded there costs its stream 25-47 us under a concurrent copy).  Returns ms per request."""
+        torch, pool = self.torch, self.pool
+        pls = [pool.place(self.bpl[r]) for r in range(self.R)]
+        for r in range(self.R):
+            pool.set_tables(pls[r], self.packed_pin[r], self.stream_of(r))
+        self.do_offload(pls, own_tables=True)
+        self.main.synchronize()
+        pool.synchronize()
+        ready = [[torch.cuda.Event() for _ in range(self.L)] for _ in range(self.R)]
+        sides = [torch.cuda.Stream(device=self.dev) for _ in range(self.R)]
+        start = torch.cuda.Event(enable_timing=True)
+        start.record(self.main)
+        for r in range(self.R):
+            sides[r].wait_event(start)
+        self.do_retrieve(pls, own_tables=True, ready=ready)
+        stamps = [[] for _ in range(self.R)]
+        for r in range(self.R):
+            for l in range(self.L):
+                if int(self.bpl[r][l]) != int(self.bpl[r].max()):
+                    continue                                    # (sliding-window layers of a few blocks ride with their neighbours)
+                sides[r].wait_event(ready[r][l])
+                t = torch.cuda.Event(enable_timing=True)
+                t.record(sides[r])
+                stamps[r].append(t)
+        torch.cuda.synchronize()
+        out = []
+        for r in range(self.R):
+            prev, row = start, []
+            for t in stamps[r]:
+                row.append(prev.elapsed_time(t))
+                prev = t
+            out.append(row)
+        for pl in pls:
+            pl.release()
+        return out
+
+    def verify(self) -> bool:
+        """What was just retrieved: the round trip is bit-identical and nothing else was written."""
+        torch, W, ok = self.torch, self.W, True
+        poison = np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item()
+        for l in range(self.L):
+            used = torch.zeros(self.wl.nphys, dtype=torch.bool, device=self.dev)
+            for r in range(self.R):
+                used[self.tables[r][l].long()] = True
+            ok &= bool(torch.equal(self.dst[l][:, used], self.src[l][:, used]))
+            ok &= bool((self.dst[l][:, ~used] == poison).all())
+        return ok
+
+    def repoison(self) -> None:
+        self.dst_all.fill_(np.int16(np.uint16(self.W.POISON_BITS).view(np.int16)).item())
+        self.torch.cuda.synchronize()
+
+    def staging_bytes(self) -> int:
+        """HBM the staged path holds for its ring: stage_slots x what one slot must hold for this workload (its largest layer or
+        group of small layers, capped by stage_chunk_bytes)."""
+        tn, g = self.pool.get_tuning(), self.g
+        total = self.moved
+        need = max(self.kmax * g.payload, min(max(self.kmax * g.payload, tn.group_bytes), total))
+        if tn.stage_chunk_bytes:
+            need = min(need, max(tn.stage_chunk_bytes, g.payload))
+        return int(tn.stage_slots * need)
+
+    def close(self) -> None:
+        self.pool.destroy()
+        del self.src, self.dst, self.dst_all, self.src_k, self.src_v, self.dst_k, self.dst_v
+        self.torch.cuda.empty_cache()
+
+
+def layer_stats(rows) -> dict:
+    xs = sorted(x for row in rows for x in row)
+    if not xs:
+        return {}
+    return {"min": xs[0], "median": xs[len(xs) // 2], "p99": xs[min(len(xs) - 1, int(0.99 * len(xs)))], "max": xs[-1], "n": len(xs),
+            "what": "interval between the completion events of consecutive full layers of a request, retrieve leg (first interval: from "
+                    "the start of the leg); non-timing events, timestamps on a side stream"}
+
+
+def side_line(rig: Rig, steps: int, warmup: int, link_h2d: float, link_d2h: float) -> dict:
+    """A short, bit-verified measurement of one more (workload, path): device-timed legs, end-to-end legs, per-layer latency."""
+    rec = {"place_ms": [], "offload_ms": [], "retrieve_ms": []}
+    for _ in range(warmup):
+        rig.step({"place_ms": [], "offload_ms": [], "retrieve_ms": []})
+    rig.repoison()
+    for _ in range(steps):
+        rig.step(rec)
+    if not rig.verify():
+        raise RuntimeError(f"config {rig.cfg} path {rig.path}: retrieved KV differs from the source - refusing to report a number")
+    e2e = [rig.e2e_pass() for _ in range(steps + 1)][1:]
+    lat = layer_stats(rig.layer_latency_pass())
+    ret, off = statistics.median(rec["retrieve_ms"]), statistics.median(rec["offload_ms"])
+    val = rig.moved / (ret * 1e6)
+    tn = rig.pool.get_tuning()
+    return {"workload": rig.wl.name, "cfg": rig.cfg, "path": rig.path, "value": val, "best": rig.moved / (min(rec["retrieve_ms"]) * 1e6), "unit": UNIT,
+            "frac_of_link": val / link_h2d, "offload_gbps": rig.moved / (off * 1e6), "offload_frac_of_link": rig.moved / (off * 1e6) / link_d2h,
+            "e2e": rig.moved / (statistics.median(x[1] for x in e2e) * 1e9), "e2e_offload": rig.moved / (statistics.median(x[0] for x in e2e) * 1e9),
+            "retrieve_layer_ms": {k: lat[k] for k in ("min", "median", "p99", "max", "n")} if lat else None,
+            "moved_bytes_per_leg": rig.moved, "steps": steps, "warmup": warmup, "verified_bit_exact_round_trip": True,
+            "ctas": tn.link_ctas if rig.path == "zerocopy" else None, "sms_used": min(tn.link_ctas, 148) if rig.path == "zerocopy" else None,
+            "staging_bytes": 0 if rig.path == "zerocopy" else rig.staging_bytes()}
+
+
 def run_kvpool(args) -> dict:
     import torch
     from paper_2606_14779_b200 import binding as kv
-    from paper_2606_14779_b200 import workloads as W
+    from paper_2606_14779_b200 import sharding
 
     rank = int(os.environ.get("RANK", 0))
     world = int(os.environ.get("WORLD_SIZE", 1))
@@ -243,157 +560,35 @@ def run_kvpool(args) -> dict:
         kvbuild.build()
     kv.lib()
 
-    wl = W.make_workload(args.config)
-    g = wl.geom
-    R, L, N = len(wl.requests), g.n_layers, wl.n_pool_devices
-    elems = g.kvb // 2
-    moved = wl.moved_bytes()
-    bpl = [wl.blocks_per_layer(r) for r in range(R)]
-
-    # ---- host-link peak of this box, measured now: 1 GiB pinned cudaMemcpyAsync, both directions (DESIGN.md §7) ----
-    probe = kv.KvPool([1.0], [1 << 30], n_layers=1, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim)
+    # ---- host-link peak of this box, measured now: 1 GiB pinned cudaMemcpyAsync, both directions (DESIGN.md §8) ----
+    probe = kv.KvPool([1.0], [1 << 30], n_layers=1, n_kv_heads=4, head_dim=128)
     link_h2d = max(probe.measure_bandwidth(0, 0, 1 << 30, 5) for _ in range(2))
     link_d2h = max(probe.measure_bandwidth(0, 1, 1 << 30, 5) for _ in range(2))
     probe.destroy()
     log(f"[rank {rank}] host link peak: H2D {link_h2d:.2f} GB/s, D2H {link_d2h:.2f} GB/s")
 
-    # ---- the pool -------------------------------------------------------------------------------------------------
-    base_w = list(wl.default_weights())
-    share = np.array(base_w) / np.sum(base_w)
-    caps = [int(moved * s * 1.25) + (L * R + 4) * (g.payload + 4096) for s in share]
-    numa = [i % 2 for i in range(N)] if args.config == 2 else None      # config 2: "on 2 NUMA nodes" (falls back, reported)
-    if numa is None and world > 1:
-        numa = [kv.NUMA_AUTO] * N       # several ranks on one host: each rank's buffers on the NUMA node its own GPU hangs off
-    t0 = time.perf_counter()
-    pool = kv.KvPool(base_w, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, block_tokens=g.block_tokens,
-                     elem_bytes=g.elem_bytes, cuda_device=local, numa_nodes=numa,
-                     dev_flags=[kv.DEV_CUDA_HOSTALLOC] * N if args.hostalloc else None,
-                     link_groups=[1] * N if args.link_groups == "shared" else None)
-    create_s = time.perf_counter() - t0
-    weights_kind = args.weights
-    if args.weights == "measured" or (args.weights == "config" and wl.weights is None):
-        bw = [pool.measure_bandwidth(i, 0, min(256 << 20, caps[i]), 5) for i in range(N)]
-        pool.set_bandwidth(bw)
-        weights_kind = "measured per-buffer H2D GB/s"
-    elif args.weights == "equal":
-        bw = [1.0] * N
-        pool.set_bandwidth(bw)
-    else:
-        bw = base_w
-    pool.set_path({"auto": kv.PATH_AUTO, "staged": kv.PATH_STAGED, "zerocopy": kv.PATH_ZEROCOPY}[args.path])
-    tune = {}
-    if args.kernel:
-        tune["kernel"] = tune["link_kernel"] = {"vec16": kv.KERNEL_VEC16, "bulk": kv.KERNEL_BULK}[args.kernel]
-    for k, v in (("link_ctas", args.link_ctas), ("hbm_ctas", args.hbm_ctas), ("stage_slots", args.stage_slots)):
-        if v:
-            tune[k] = v
-    if args.stage_chunk_mib:
-        tune["stage_chunk_bytes"] = int(args.stage_chunk_mib * 2**20)
-    if tune:
-        pool.set_tuning(**tune)
-    tn = pool.get_tuning()
-    numa_actual = [pool.device_info(i)["numa_node"] for i in range(N)]
-    log(f"[rank {rank}] pool: {N} buffers, {sum(caps) / 2**30:.1f} GiB pinned in {create_s:.1f} s, NUMA nodes {numa_actual}, weights {list(pool.weights())}")
+    rig = Rig(args, args.config, args.path, local, world)
+    pool, wl, g, R, L, N, moved, tn = rig.pool, rig.wl, rig.g, rig.R, rig.L, rig.N, rig.moved, rig.tn
+    main, src, dst, tables, bpl = rig.main, rig.src, rig.dst, rig.tables, rig.bpl
+    log(f"[rank {rank}] pool: {N} buffers, {sum(rig.caps) / 2**30:.1f} GiB pinned in {rig.create_s:.1f} s, NUMA nodes {rig.numa_actual}, weights {list(pool.weights())}")
 
-    # ---- synthetic paged KV in HBM: source layers (seeded N(0,1) bf16) and poison-filled destination layers ---------
-    src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
-    dst = [W.poison_torch((2, wl.nphys, elems), dev) for l in range(L)]
-    tables_np = [[np.ascontiguousarray(wl.layer_table(r, l)) for l in range(L)] for r in range(R)]
-    tables_pin = [[torch.from_numpy(t).pin_memory() for t in row] for row in tables_np]
-    tables = [[t.to(dev) for t in row] for row in tables_pin]
-    table_bytes = sum(t.nbytes for row in tables_np for t in row)
-    sample_pin = torch.empty((R, L, elems), dtype=torch.int16).pin_memory()
-    main = torch.cuda.Stream(device=dev)
-    streams = [torch.cuda.Stream(device=dev) for _ in range(max(1, wl.n_streams))] if wl.n_streams > 1 else [main]
-    torch.cuda.synchronize()
+    def fresh():
+        return {"place_ms": [], "offload_ms": [], "retrieve_ms": []}
 
-    def fork():
-        if streams[0] is not main:
-            e = torch.cuda.Event()
-            e.record(main)
-            for s in streams:
-                s.wait_event(e)
-
-    def join():
-        if streams[0] is not main:
-            for s in streams:
-                e = torch.cuda.Event()
-                e.record(s)
-                main.wait_event(e)
-
-    src_k, src_v = [x[0] for x in src], [x[1] for x in src]
-    dst_k, dst_v = [x[0] for x in dst], [x[1] for x in dst]
-
-    def do_offload(pls):
-        fork()
-        if args.per_layer:
-            for l in range(L):
-                for r in range(R):
-                    pool.offload(pls[r], l, src[l][0], src[l][1], g.kvb, tables[r][l], streams[r % len(streams)])
-        else:
-            for r in range(R):
-                pool.offload_layers(pls[r], 0, src_k, src_v, g.kvb, tables[r], streams[r % len(streams)])
-        for r in range(R):
-            pool.wait_offloads(pls[r], streams[r % len(streams)])
-        join()
-
-    def do_retrieve(pls, layer_events=None, upload_tables=False):
-        fork()
-        if layer_events is None and not upload_tables and not args.per_layer:
-            for r in range(R):
-                pool.retrieve_layers(pls[r], 0, dst_k, dst_v, g.kvb, tables[r], streams[r % len(streams)])
-            join()
-            return
-        for l in range(L):
-            for r in range(R):
-                s = streams[r % len(streams)]
-                if upload_tables:
-                    with torch.cuda.stream(s):
-                        tables[r][l].copy_(tables_pin[r][l], non_blocking=True)
-                pool.retrieve(pls[r], l, dst[l][0], dst[l][1], g.kvb, tables[r][l], s)
-                if layer_events is not None:
-                    e = torch.cuda.Event(enable_timing=True)
-                    e.record(s)
-                    layer_events[r].append(e)
-        join()
-
-    def step(timed: bool, rec: dict):
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
-        t0 = time.perf_counter()
-        pls = [pool.place(bpl[r]) for r in range(R)]
-        t1 = time.perf_counter()
-        ev[0].record(main)
-        do_offload(pls)
-        ev[1].record(main)
-        # the legs are timed apart: without this the retrieve's host->GPU copies (which may run ahead of the caller's
-        # stream) would start under the tail of the offload leg and borrow the link's other direction
-        main.synchronize()
-        pool.synchronize()
-        ev[2].record(main)
-        do_retrieve(pls)
-        ev[3].record(main)
-        main.synchronize()
-        for pl in pls:
-            pl.release()
-        if timed:
-            rec["place_ms"].append(1e3 * (t1 - t0))
-            rec["offload_ms"].append(ev[0].elapsed_time(ev[1]))
-            rec["retrieve_ms"].append(ev[2].elapsed_time(ev[3]))
-
-    rec = {"place_ms": [], "offload_ms": [], "retrieve_ms": []}
-    warm = {"place_ms": [], "offload_ms": [], "retrieve_ms": []}
+    rec, warm = fresh(), fresh()
     for _ in range(args.warmup):
-        step(True, warm)
-    # Host settle (untimed, disclosed in the JSON): in the first minutes after a GPU VM boots, DMA over a multi-GiB pinned
-    # working set — and plain CPU memcpy — run 10-50 % below their steady state on this pool of boxes (the 1 GiB link probe
-    # does not show it).  If the last warm-up leg is well below the link peak measured a moment ago, keep stepping, for at
-    # most --settle-s seconds, until it is not.  A box that never gets there is timed as it is.
+        rig.step(warm)
+    # Host settle (untimed; its step count is printed at the top level of the JSON line, next to `warmup`): in the first
+    # minutes after a GPU VM boots, DMA over a multi-GiB pinned working set — and plain CPU memcpy — run 10-50 % below their
+    # steady state on this pool of boxes (the 1 GiB link probe does not show it).  If the last warm-up leg is well below the
+    # link peak measured a moment ago, keep stepping, for at most --settle-s seconds, until it is not.  A box that never gets
+    # there is timed as it is.  --settle-s 0 turns it off.
     settle = {"extra_steps": 0, "seconds": 0.0}
     t_settle = time.perf_counter()
     want_gbps = 0.9 * min(link_h2d, 55.0) * (0.92 if args.path == "zerocopy" else 1.0)
     while (args.settle_s > 0 and moved >= (1 << 30) and warm["retrieve_ms"] and moved / (warm["retrieve_ms"][-1] * 1e6) < want_gbps
            and time.perf_counter() - t_settle < args.settle_s):
-        step(True, warm)
+        rig.step(warm)
         settle["extra_steps"] += 1
         settle["seconds"] = time.perf_counter() - t_settle
 
@@ -413,7 +608,7 @@ def run_kvpool(args) -> dict:
     barrier()
     t_begin = time.perf_counter()
     for _ in range(args.steps):
-        step(True, rec)
+        rig.step(rec)
     barrier()
     t_end = time.perf_counter()
     pool.set_profiling(False)
@@ -421,10 +616,10 @@ def run_kvpool(args) -> dict:
     clocks = sampler.stop(t_begin, t_end) if rank == 0 else None
     prof_clk = {kind: pool.profile_read_clock(kind) for kind in range(4)}
     prof = {kind: (v[0], v[2], v[4]) for kind, v in prof_clk.items()}
-    # one more step, untimed, with the timing events recorded on the launching streams themselves (kvpool.h: such a record
+    # one more step, untimed, with the timing events recorded on the launching streams themselves (kvpool_dev.h: such a record
     # holds its stream up for 25-47 us under a concurrent copy-engine transfer): reported beside the side-stream figure
     pool.set_profiling(kv.PROFILE_INSTREAM)
-    step(True, {"place_ms": [], "offload_ms": [], "retrieve_ms": []})
+    rig.step(fresh())
     pool.set_profiling(False)
     prof_in = {kind: pool.profile_read_clock(kind) for kind in range(4)}
     for kind, name in enumerate(("pack", "unpack", "zero-copy offload", "zero-copy retrieve")):
@@ -433,59 +628,25 @@ def run_kvpool(args) -> dict:
             log(f"[rank {rank}] {name}: {a[2]} launches; mean per launch: side-stream events {1e3 * a[0] / a[2]:.1f} us, kernel clock "
                 f"{1e3 * a[1] / max(a[3], 1):.1f} us; in-stream events (extra step) {1e3 * b_[0] / max(b_[2], 1):.1f} us, kernel clock {1e3 * b_[1] / max(b_[3], 1):.1f} us")
 
+    # value = median over the K timed steps; best and mean beside it; max over ranks of each
     step_ms = 1e3 * (t_end - t_begin) / args.steps
-    ret_ms = sum(rec["retrieve_ms"]) / args.steps
-    off_ms = sum(rec["offload_ms"]) / args.steps
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([step_ms, ret_ms, off_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        step_ms, ret_ms, off_ms = [float(x) for x in t.tolist()]
+    ret_ms, off_ms = statistics.median(rec["retrieve_ms"]), statistics.median(rec["offload_ms"])
+    ret_best_ms, ret_mean_ms = min(rec["retrieve_ms"]), statistics.mean(rec["retrieve_ms"])
+    step_ms, ret_ms, off_ms, ret_best_ms, ret_mean_ms = sharding.max_over_ranks([step_ms, ret_ms, off_ms, ret_best_ms, ret_mean_ms], dev)
     value = world * moved / (ret_ms * 1e6)
 
     # ---- correctness of what was timed: round trip bit-identical, nothing else written ---------------------------------
-    verified = True
-    for l in range(L):
-        used = torch.zeros(wl.nphys, dtype=torch.bool, device=dev)
-        for r in range(R):
-            used[tables[r][l].long()] = True
-        verified &= bool(torch.equal(dst[l][:, used], src[l][:, used]))
-        verified &= bool((dst[l][:, ~used] == dst[l].new_tensor(np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item())).all())
-    if not verified:
+    if not rig.verify():
         raise RuntimeError("retrieved KV differs from the source — refusing to report a number")
 
-    # ---- e2e: the retrieve leg by host wall clock through the public API, tables uploaded from pinned host memory ------
-    e2e_ret_s, e2e_off_s, layer_ms = [], [], [[] for _ in range(R)]
-    for it in range(max(2, args.steps)):
-        pls = [pool.place(bpl[r]) for r in range(R)]
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        do_offload(pls)
-        main.synchronize()
-        t1 = time.perf_counter()
-        evs = [[] for _ in range(R)]
-        start = torch.cuda.Event(enable_timing=True)
-        start.record(main)
-        do_retrieve(pls, layer_events=evs, upload_tables=True)
-        with torch.cuda.stream(main):
-            for r in range(R):
-                for l in range(L):
-                    if len(tables_np[r][l]):
-                        sample_pin[r, l].copy_(dst[l][0, int(tables_np[r][l][0])], non_blocking=True)
-        main.synchronize()
-        t2 = time.perf_counter()
-        for pl in pls:
-            pl.release()
-        if it > 0:                                          # first pass warms the pinned-table path
-            e2e_off_s.append(t1 - t0)
-            e2e_ret_s.append(t2 - t1)
-            for r in range(R):
-                prev = start
-                for e in evs[r]:
-                    layer_ms[r].append(prev.elapsed_time(e))
-                    prev = e
-    e2e_val = world * moved / (statistics.median(e2e_ret_s) * 1e9)
-    d2h_bytes = sum(g.kvb for r in range(R) for l in range(L) if len(tables_np[r][l]))
+    # ---- e2e: both legs by host wall clock through the public API (tables from pinned host memory, result read back) ------
+    e2e = [rig.e2e_pass() for _ in range(max(3, args.steps) + 1)][1:]          # first pass warms the pinned-table path
+    e2e_ret_s, e2e_off_s = sharding.max_over_ranks([statistics.median(x[1] for x in e2e), statistics.median(x[0] for x in e2e)], dev)
+    e2e_val = world * moved / (e2e_ret_s * 1e9)
+    # ---- per-layer retrieve latency, its own passes -----------------------------------------------------
+    layer_rows = []
+    for _ in range(3):
+        layer_rows += rig.layer_latency_pass()
 
     # ---- in-device pack / unpack alone (HBM roofline), rotating over layers so nothing is L2-resident ------------------
     hbm = {}
@@ -613,37 +774,61 @@ def run_kvpool(args) -> dict:
                         "achieved_kernel_clock = the same in-step launches timed by the kernel itself (%globaltimer, first CTA start to "
                         "last CTA end, stores fenced); achieved_back_to_back = same kernel, 16 launches per event pair, no concurrent copy")
 
+    # ---- beside the headline (rank 0 of a 1-GPU run of the headline configuration): the design's own path and the other shapes ---
+    paths, shapes = {}, {}
+    if world == 1 and args.config == 4 and args.path == "auto" and not args.no_extras:
+        rig.set_path("zerocopy")                       # north_star: "zero-copy reads of mapped pinned host memory"
+        paths["zerocopy"] = side_line(rig, 3, 1, link_h2d, link_d2h)
+        rig.set_path("hybrid")                         # offload by the kernel, retrieve by the copy engines (kvpool.h)
+        paths["hybrid"] = side_line(rig, 3, 1, link_h2d, link_d2h)
+        rig.set_path(args.path)
+    staging = rig.staging_bytes() if args.path != "zerocopy" else 0
+    create_s, caps, weights_kind, bw, numa_actual, streams = rig.create_s, rig.caps, rig.weights_kind, rig.bw, rig.numa_actual, rig.streams
+    table_bytes, d2h_bytes = rig.table_bytes, rig.d2h_bytes
+    src = dst = tables = stage = None              # (the closures above keep cells, not tensors)
+    rig.close()
+    if world == 1 and args.config == 4 and args.path == "auto" and not args.no_extras:
+        for cfg in (3, 6):                             # GPT-OSS-20B and LLaMA-3.1-8B at 128K (north_star)
+            other = Rig(args, cfg, "auto", local, world)
+            shapes[other.wl.name] = side_line(other, 3, 2, link_h2d, link_d2h)
+            other.close()
+
     out = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": step_ms,
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "warmup_extra_steps": settle["extra_steps"], "ms_per_step": step_ms,
+        "value_is": "median over the timed steps of (bytes of the retrieve leg / its device time)", "best": world * moved / (ret_best_ms * 1e6),
+        "mean": world * moved / (ret_mean_ms * 1e6),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
         "config": {"workload": wl.name, "cfg": args.config, "context_tokens": list(wl.context_tokens), "layers": L, "requests": R,
                    "moved_bytes_per_leg": moved, "pool_buffers": N, "weights": weights_kind, "bandwidth_gbps": [round(float(x), 3) for x in bw],
                    "numa_nodes": numa_actual, "path": args.path, "kernel": "vec16" if tn.kernel == kv.KERNEL_VEC16 else "bulk",
                    "link_kernel": "vec16" if tn.link_kernel == kv.KERNEL_VEC16 else "bulk",
-                   "link_ctas": tn.link_ctas, "hbm_ctas": tn.hbm_ctas, "stage_slots": tn.stage_slots, "stage_chunk_bytes": tn.stage_chunk_bytes, "link_groups": args.link_groups, "streams": len(streams),
+                   "link_ctas": tn.link_ctas, "hbm_ctas": tn.hbm_ctas, "stage_slots": tn.stage_slots, "stage_chunk_bytes": tn.stage_chunk_bytes, "staging_bytes": staging, "link_groups": args.link_groups, "streams": len(streams),
                    "l2": f"inputs larger than L2: each leg moves {moved / 2**30:.1f} GiB through {L} distinct layers (L2 is 126 MB); no flush needed",
                    "calls": "per-layer" if args.per_layer else "batched (kvpool_offload_layers / kvpool_retrieve_layers, one call per request)",
                    "step": "kvpool_place + offload of every layer + retrieve of every layer; value = retrieve leg"},
         "retrieve_ms_per_step": ret_ms, "offload_ms_per_step": off_ms, "offload_gbps": world * moved / (off_ms * 1e6),
-        "place_ms_per_step": statistics.mean(rec["place_ms"]), "verified_bit_exact_round_trip": verified,
+        "place_ms_per_step": statistics.median(rec["place_ms"]), "verified_bit_exact_round_trip": True, "staging_bytes": staging,
         "pool_create": {"seconds": create_s, "pinned_bytes": int(sum(caps)), "gbps": sum(caps) / create_s / 1e9,
                         "what": "kvpool_create: huge-page mapping faulted in by up to 16 threads + cudaHostRegister (outside the timed region)"},
         "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": moved + table_bytes, "d2h_bytes_per_step": d2h_bytes,
-                "what": "retrieve leg by host wall clock: pinned block tables H2D + kvpool_retrieve x layers + D2H of one block per layer + sync",
-                "offload_gbps": world * moved / (statistics.median(e2e_off_s) * 1e9)},
+                "what": "retrieve leg by host wall clock through the public API: kvpool_set_tables (the request's block tables from pinned host "
+                        "memory, one H2D copy) + kvpool_retrieve_layers + one gather and one D2H copy of one block per layer + sync; median of "
+                        f"{len(e2e)} passes",
+                "offload_gbps": world * moved / (e2e_off_s * 1e9)},
         "gpu_launches": k1 - k0, "memcpy_calls": m1 - m0, "host_settle": settle,
         "roofline": roof, "roofline_link": link_roof, "roofline_hbm": hbm_roof,
         "clocks": clocks,
     }
-    per_layer = [x for r in range(R) for x in layer_ms[r]]
-    if per_layer:
-        per_layer.sort()
-        out["retrieve_layer_ms"] = {"min": per_layer[0], "median": per_layer[len(per_layer) // 2], "p99": per_layer[min(len(per_layer) - 1, int(0.99 * len(per_layer)))],
-                                    "what": "interval between consecutive per-layer completion events on a request's stream, retrieve leg"}
+    if paths:
+        out["paths"] = paths
+    if shapes:
+        out["shapes"] = shapes
+    if layer_rows:
+        out["retrieve_layer_ms"] = layer_stats(layer_rows)
     if args.detail and rank == 0:
         with open(args.detail, "w") as f:
-            json.dump({"out": out, "rec": rec, "layer_ms": layer_ms, "prof": {kinds[k]: prof[k] for k in range(4)}}, f, indent=1)
-    pool.destroy()
+            json.dump({"out": out, "rec": rec, "layer_ms": layer_rows, "prof": {kinds[k]: prof[k] for k in range(4)}}, f, indent=1)
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
@@ -921,7 +1106,8 @@ def run_duplex(args) -> None:
     share = np.array(bw) / np.sum(bw)
     caps = [int(2 * moved * sh * 1.25) + 2 * (L + 4) * (g.payload + 4096) for sh in share]
     pool = kv.KvPool(bw, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim,
-                     dev_flags=[kv.DEV_CUDA_HOSTALLOC] * len(bw) if args.hostalloc else None)
+                     dev_flags=[kv.DEV_CUDA_HOSTALLOC] * len(bw) if args.hostalloc else None,
+                     link_groups=[1] * len(bw) if args.link_groups == "shared" else None)
     src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
     dst = [W.poison_torch((2, wl.nphys, elems), dev) for l in range(L)]
     tables = [torch.from_numpy(np.ascontiguousarray(wl.layer_table(0, l))).to(dev) for l in range(L)]
@@ -949,10 +1135,12 @@ def run_duplex(args) -> None:
     print(f"# bench.py --duplex --config {args.config}: {wl.name} cut to {L} layers; request A ({moved / 2**20:.0f} MiB) is offloaded while request B "
           f"({moved / 2**20:.0f} MiB) is retrieved; median of 3")
     print(f"# simultaneous cudaMemcpyAsync, 1 GiB each way: H2D {peak_h2d:.1f} GB/s + D2H {peak_d2h:.1f} GB/s = {peak_h2d + peak_d2h:.1f} GB/s")
+    print("# staged = pack/unpack kernels + copy engines both ways; hybrid = offload by the kernel's own stores (8 CTAs), retrieve by the copy engines; "
+          "zerocopy/n = both directions by kernels of n CTAs")
     print(f"{'path/CTAs':12s} {'offload A GB/s':>15s} {'retrieve B GB/s':>16s} {'aggregate GB/s (wall)':>22s} {'x duplex peak':>14s}")
     if args.stage_slots:
         pool.set_tuning(stage_slots=args.stage_slots)
-    for pname, path, ctas in (("staged", kv.PATH_STAGED, 0), ("zerocopy", kv.PATH_ZEROCOPY, args.link_ctas or 4),
+    for pname, path, ctas in (("staged", kv.PATH_STAGED, 0), ("hybrid", kv.PATH_HYBRID, 0), ("zerocopy", kv.PATH_ZEROCOPY, args.link_ctas or 4),
                               ("zerocopy", kv.PATH_ZEROCOPY, 4 * (args.link_ctas or 4))):
         pool.set_path(path)
         if ctas:

@@ -78,7 +78,14 @@ enum {
 enum {
   KVPOOL_PATH_AUTO = 0,     /* staged for layers >= the auto threshold, zero-copy below it            */
   KVPOOL_PATH_STAGED = 1,   /* pack/unpack kernel <-> device staging + one cudaMemcpyAsync per stripe  */
-  KVPOOL_PATH_ZEROCOPY = 2  /* one kernel reads/writes the mapped host stripes directly over the link  */
+  KVPOOL_PATH_ZEROCOPY = 2, /* one kernel reads/writes the mapped host stripes directly over the link  */
+  KVPOOL_PATH_HYBRID = 3    /* offload: zero-copy (the kernel's own posted writes, >= 8 CTAs, no staging slot, no copy
+                               engine); retrieve: as AUTO.  For engines that evict one request while they fetch another
+                               (PAPER.md:166, 241): SM-issued READS collapse under a concurrent GPU->host stream (their
+                               128-byte read requests queue behind the write data), SM-issued writes do not, so this is
+                               the kernel path that keeps both directions of the link busy — 91 GB/s against 94 staged
+                               both ways and 67-74 zero-copy both ways (profiles/r2_duplex.md) — and it leaves the copy
+                               engines and the whole staging ring to the retrieve direction                              */
 };
 /* kernel variants (kvpool_set_tuning) */
 enum {
@@ -283,7 +290,8 @@ KVPOOL_API int kvpool_retrieve_layers(kvpool_t* pool, kvpool_placement_t* pl, ui
  * array of n_layers caller-owned cudaEvent_t (entries may be NULL); layer_ready[q] is recorded on `stream` as soon as layer
  * first_layer + q is complete in the paged layout, so the consumer does cudaStreamWaitEvent(consumer, layer_ready[q]) and
  * computes layer q while the pool is still moving layers q+1, ... (the staged path's host->GPU copies run up to
- * `stage_slots` layers ahead).  Layers that travel as one group (small layers, see above) become ready together; a layer
+ * `stage_slots` layers ahead).  Layers that travel as one group (small layers, see above) become ready together (a request
+ * smaller than one group is cut into two groups here, so that the consumer of the first overlaps the second); a layer
  * with K_l = 0 is ready at once.  One host call per request instead of one per layer.                                 */
 KVPOOL_API int kvpool_retrieve_layers_signal(kvpool_t* pool, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers,
                                   void* const* k_bases /*host[n_layers]*/, void* const* v_bases /*host[n_layers]*/,

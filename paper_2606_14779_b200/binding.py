@@ -22,7 +22,7 @@ TYPE_MEM, TYPE_SSD, TYPE_HBM = 0, 1, 2
 NUMA_AUTO = -2
 MEASURE_RETRIEVE, MEASURE_OFFLOAD, MEASURE_KERNEL_RETRIEVE, MEASURE_KERNEL_OFFLOAD = 0, 1, 2, 3
 PROFILE_OFF, PROFILE_SIDE, PROFILE_INSTREAM = 0, 1, 2
-PATH_AUTO, PATH_STAGED, PATH_ZEROCOPY = 0, 1, 2
+PATH_AUTO, PATH_STAGED, PATH_ZEROCOPY, PATH_HYBRID = 0, 1, 2, 3
 KERNEL_VEC16, KERNEL_BULK = 0, 1
 _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA", ESTATE: "ESTATE", ENOENT: "ENOENT"}
 

@@ -88,7 +88,7 @@ __device__ __forceinline__ Piece decode(const LayerArgs& a, uint64_t t, uint32_t
     d = 0;
     s = local;
   } else {
-    j = a.j0 + local;
+    j = a.visit ? __ldg(a.visit + a.j0 + local) : a.j0 + local;
     d = __ldg(a.dev + j);
     s = __ldg(a.slot + j);
   }

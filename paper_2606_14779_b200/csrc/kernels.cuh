@@ -27,6 +27,11 @@ struct LayerArgs {
   // order[j0 + u] (the inverse map of that device, ascending in slot) and its pool side is pool_base[0] + u*P, so the
   // chunk is one contiguous piece of that device's stripe: ONE copy per chunk.  dev / slot are not read.
   const uint32_t* order;
+  // Visiting order (mixed pools, whole-layer zero-copy launches): when set, unit u is logical block visit[j0 + u] — a
+  // permutation of the layer's blocks that lists the blocks of host-memory devices first, so that the link (the slow
+  // resource of such a launch: ~50 GB/s next to ~3 TB/s) is busy from the first CTA on instead of receiving its last
+  // pieces when the HBM share is nearly done.  dev / slot are read as usual.
+  const uint32_t* visit;
   uint32_t kvb;
   unsigned long long* span;  // profiling only (else null): device {min start, max end} of the launch in %globaltimer ns
   unsigned long long* bad;   // table check only (else null): counts table entries outside [0, nphys_check)

@@ -73,6 +73,7 @@ struct LayerMap {
   const uint8_t* dev_d = nullptr; // device copies
   const uint32_t* slot_d = nullptr;
   const uint32_t* order_d = nullptr;
+  const uint32_t* visit_d = nullptr; // mixed pools only: the layer's blocks with those of host-memory devices first (kernels.cuh)
   uint64_t host_blocks = 0;       // blocks of the layer that sit on host-memory devices (the rest: HBM-type devices)
 };
 
@@ -339,12 +340,15 @@ inline uint8_t* pool_bytes(const kvpool* p, uint32_t i) {
   return static_cast<uint8_t*>(is_hbm(p, i) ? p->bufs[i].dev_alias : p->bufs[i].host);
 }
 
-LaunchCfg launch_cfg(const kvpool* p, bool link_bound) {
+LaunchCfg launch_cfg(const kvpool* p, bool link_bound, bool pack = false) {
   // a zero-copy launch over a pool with HBM devices moves most of its bytes at HBM / NVLink rates: give it the HBM grid
   if (p->hbm_mask) link_bound = false;
   LaunchCfg c{};
   c.kernel = link_bound ? p->tune.link_kernel : p->tune.kernel;
   c.ctas = link_bound ? p->tune.link_ctas : p->tune.hbm_ctas;
+  // the hybrid path is made for both directions of the link at once: under a concurrent host->GPU copy stream the posted
+  // writes of 4 CTAs reach 43.8 GB/s, those of 8 CTAs 45.8 (profiles/r2_duplex.md)
+  if (link_bound && pack && p->path == KVPOOL_PATH_HYBRID) c.ctas = std::max<uint32_t>(c.ctas, 8);
   c.bulk_chunk = p->tune.bulk_chunk;
   c.bulk_stages = p->tune.bulk_stages;
   c.bulk_warps = p->tune.bulk_warps;
@@ -357,17 +361,22 @@ LaunchCfg launch_cfg(const kvpool* p, bool link_bound) {
 
 inline bool all_hbm(const kvpool* p) { return p->hbm_mask == (p->n >= 32 ? 0xFFFFFFFFu : (1u << p->n) - 1u); }
 
-bool use_staged(const kvpool* p, const LayerState& L) {
-  if (all_hbm(p)) return false;  // nothing to stage: every stripe is reached in place (one kernel, HBM grid)
-  if (p->path == KVPOOL_PATH_ZEROCOPY) return false;
-  bool host_blocks = false;  // a layer whose blocks all went to HBM-type devices (tiny K, large weights) has nothing to stage
-  for (uint32_t i = 0; i < p->n; ++i) host_blocks |= L.map->counts[i] && !is_hbm(p, i);
-  if (!host_blocks) return false;
-  if (p->path == KVPOOL_PATH_STAGED) return true;
-  // judged by what would travel through the copy engines: in a pool with HBM-type devices the host devices' share of a
-  // layer is small (Eq. 1 gives a 55 GB/s link 2 % next to 3 TB/s of HBM); below the threshold the same kernel that
-  // reaches the HBM stripes in place also stores / loads the mapped host stripes, instead of a few latency-bound copies
-  return L.map->host_blocks * p->payload >= p->tune.auto_threshold_bytes;
+// Does a transfer of `host_bytes` to / from host-memory devices go through the staging ring and the copy engines?
+bool use_staged(const kvpool* p, bool pack, uint64_t host_bytes) {
+  if (all_hbm(p)) return false;   // nothing to stage: every stripe is reached in place (one kernel, HBM grid)
+  if (host_bytes == 0) return false;  // all of its blocks went to HBM-type devices (tiny K, large weights)
+  switch (p->path) {
+    case KVPOOL_PATH_ZEROCOPY: return false;
+    case KVPOOL_PATH_STAGED: return true;
+    case KVPOOL_PATH_HYBRID:
+      if (pack) return false;  // offload by the kernel's own stores, retrieve as on the auto path
+      [[fallthrough]];
+    default:
+      // judged by what would travel through the copy engines: in a pool with HBM-type devices the host devices' share of a
+      // layer is small (Eq. 1 gives a 55 GB/s link 2 % next to 3 TB/s of HBM); below the threshold the same kernel that
+      // reaches the HBM stripes in place also stores / loads the mapped host stripes, instead of a few latency-bound copies
+      return host_bytes >= p->tune.auto_threshold_bytes;
+  }
 }
 
 constexpr uint32_t kSpanCap = 16384;  // profiled launches between two reads that also get a device-clock span
@@ -454,7 +463,7 @@ int launch_counted(kvpool* p, const LayerArgs& a, bool pack, bool link_bound, cu
   }
   LayerArgs timed = a;
   if (p->profiling) timed.span = take_span(p, &r);
-  CU(launch_layer_copy(timed, pack, launch_cfg(p, link_bound), s));
+  CU(launch_layer_copy(timed, pack, launch_cfg(p, link_bound, pack), s));
   p->n_kernels++;
   if (p->profiling) return prof_end(p, &r, s);
   return KVPOOL_OK;
@@ -756,7 +765,7 @@ int kvpool_bandwidths(const kvpool_t* p, double* bandwidth_out, uint32_t* link_g
 
 int kvpool_set_path(kvpool_t* p, int path) {
   PoolLock lock__(p);
-  if (!p || path < KVPOOL_PATH_AUTO || path > KVPOOL_PATH_ZEROCOPY) return fail(KVPOOL_EINVAL, "set_path: bad arguments");
+  if (!p || path < KVPOOL_PATH_AUTO || path > KVPOOL_PATH_HYBRID) return fail(KVPOOL_EINVAL, "set_path: bad arguments");
   p->path = path;
   return KVPOOL_OK;
 }
@@ -849,7 +858,7 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
       for (uint64_t j = 0; j < K; ++j) m->order[m->start[m->dev[j]] + m->slot[j]] = static_cast<uint32_t>(j);
       for (uint32_t i = 0; i < N; ++i)
         if (!is_hbm(p, i)) m->host_blocks += m->counts[i];
-      table_bytes += 2 * ((K * 4 + 255) / 256 * 256) + (K + 255) / 256 * 256;
+      table_bytes += (2 + (p->hbm_mask && !all_hbm(p) ? 1 : 0)) * ((K * 4 + 255) / 256 * 256) + (K + 255) / 256 * 256;
       it = by_k.emplace(K, std::move(m)).first;
     }
     pl->layers[l].map = it->second;
@@ -924,6 +933,15 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
       m.dev_d = pl->tables_d + off;
       memcpy(host + off, m.dev.data(), m.K);
       off += (m.K + 255) / 256 * 256;
+      if (p->hbm_mask && !all_hbm(p)) {  // visiting order: host-device blocks first, each class in logical order
+        uint32_t* v = reinterpret_cast<uint32_t*>(host + off);
+        uint64_t at = 0;
+        for (int hbm_pass = 0; hbm_pass < 2; ++hbm_pass)
+          for (uint64_t j = 0; j < m.K; ++j)
+            if (is_hbm(p, m.dev[j]) == (hbm_pass == 1)) v[at++] = static_cast<uint32_t>(j);
+        m.visit_d = reinterpret_cast<const uint32_t*>(pl->tables_d + off);
+        off += (m.K * 4 + 255) / 256 * 256;
+      }
     }
     for (uint32_t l = 0; l < L; ++l) {  // GPU-visible stripe addresses, one row per layer
       uint64_t* row = reinterpret_cast<uint64_t*>(host + off) + static_cast<uint64_t>(l) * N;
@@ -1064,15 +1082,14 @@ int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, ui
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const uint32_t N = p->n;
   LayerArgs a = base_args(p, L, k_base, v_base, stride, table_of(pl, layer, table));
-  bool staged = use_staged(p, L);
   const ChunkPlan whole = plan_chunk(p, L, first_block, n_blocks);
-  if (staged && n_blocks != L.map->K)  // a range is judged by its own size and by where its own blocks sit
-    staged = whole.host_blocks && (p->path == KVPOOL_PATH_STAGED || whole.host_bytes >= p->tune.auto_threshold_bytes);
+  const bool staged = use_staged(p, true, whole.host_bytes);  // a range is judged by its own size and by where its own blocks sit
 
   if (!staged) {
     // zero-copy: one kernel gathers the paged blocks and stores them straight into the mapped host stripes
     a.j0 = first_block;
     a.K = n_blocks;
+    if (n_blocks == L.map->K) a.visit = L.map->visit_d;  // (null unless the pool mixes host and HBM-type devices)
     chunk_bases(p, L, ChunkPlan{}, nullptr, &a);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));  // an earlier staged offload of this layer still in flight
     rc = launch_counted(p, a, true, true, s);
@@ -1198,14 +1215,14 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   LayerArgs a = base_args(p, L, k_base, v_base, stride, table_of(pl, layer, table));
   const ChunkPlan whole = plan_chunk(p, L, first_block, n_blocks);
   // staged only if something travels through the copy engines (a range whose blocks all sit on HBM-type devices has
-  // nothing to stage) and, on the auto path, enough of it (use_staged)
-  const bool staged = !all_hbm(p) && whole.host_blocks &&
-                      (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && whole.host_bytes >= p->tune.auto_threshold_bytes));
+  // nothing to stage) and, on the auto path, enough of it
+  const bool staged = use_staged(p, false, whole.host_bytes);
   settle_landed(L);
 
   if (!staged) {
     a.j0 = first_block;
     a.K = n_blocks;
+    if (n_blocks == L.map->K) a.visit = L.map->visit_d;
     chunk_bases(p, L, ChunkPlan{}, nullptr, &a);
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
     rc = launch_counted(p, a, false, true, s);
@@ -1301,7 +1318,7 @@ static int launch_multi_counted(kvpool* p, const MultiArgs& ma, bool pack, bool 
   }
   MultiArgs timed = ma;
   if (p->profiling) timed.span = take_span(p, &r);
-  CU(launch_multi_copy(timed, pack, launch_cfg(p, link_bound), s));
+  CU(launch_multi_copy(timed, pack, launch_cfg(p, link_bound, pack), s));
   p->n_kernels++;
   if (p->profiling) return prof_end(p, &r, s);
   return KVPOOL_OK;
@@ -1480,8 +1497,7 @@ int issue_group(const BatchCall& c, const LayerGroup& g) {
 
 int issue_group_work(const BatchCall& c, const LayerGroup& g) {
   kvpool* p = c.p;
-  const bool staged = !all_hbm(p) && (p->path == KVPOOL_PATH_STAGED || (p->path == KVPOOL_PATH_AUTO && g.host_bytes >= p->tune.auto_threshold_bytes));
-  if (!staged) return issue_zero_copy_group(c, g);
+  if (!use_staged(p, c.pack, g.host_bytes)) return issue_zero_copy_group(c, g);
   if (g.n > 1) {
     const int rc = issue_staged_group(c, g);
     if (rc != 1) return rc;
@@ -1515,7 +1531,15 @@ static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32
   }
   DeviceGuard guard(p->cuda_device);
   const BatchCall c{p, pl, pack, first, k_bases, v_bases, tables, stride, static_cast<cudaStream_t>(cuda_stream), ready};
-  const uint64_t cap = std::max<uint64_t>(p->tune.group_bytes, 1);
+  uint64_t cap = std::max<uint64_t>(p->tune.group_bytes, 1);
+  if (ready) {
+    // a consumer follows behind the per-layer events: a request so small that it would travel as ONE group (all layers
+    // ready together, the consumer not overlapped at all) is cut in two, so that the consumer of the first half runs
+    // under the transfer of the second (GPT-OSS-shaped KV at 1K context: 27 MiB; profiles/r2_blocked_io.txt)
+    uint64_t total = 0;
+    for (uint32_t q = 0; q < n; ++q) total += pl->layers[first + q].map->K * p->payload;
+    if (total < cap) cap = std::max<uint64_t>((total + 1) / 2, 1);
+  }
   LayerGroup g;
   uint64_t units = 0;
   for (uint32_t q = 0; q < n; ++q) {

@@ -13,7 +13,8 @@ from paper_2606_14779_b200 import workloads as W
 
 
 def make_pool(wl: W.Workload, bandwidth: Optional[Sequence[float]] = None, slack: float = 1.25,
-              dev_flags: Optional[Sequence[int]] = None, link_groups: Optional[Sequence[int]] = None) -> kv.KvPool:
+              dev_flags: Optional[Sequence[int]] = None, link_groups: Optional[Sequence[int]] = None,
+              gpus: Optional[Sequence[int]] = None) -> kv.KvPool:
     bw = list(bandwidth) if bandwidth is not None else list(wl.default_weights())
     total = wl.moved_bytes()
     share = np.array(bw) / np.sum(bw)
@@ -21,7 +22,7 @@ def make_pool(wl: W.Workload, bandwidth: Optional[Sequence[float]] = None, slack
     caps = [int(total * s * slack) + (wl.geom.n_layers * len(wl.requests) + 4) * (wl.geom.payload + 4096) for s in share]
     g = wl.geom
     return kv.KvPool(bw, caps, n_layers=g.n_layers, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim,
-                     block_tokens=g.block_tokens, elem_bytes=g.elem_bytes, dev_flags=dev_flags, link_groups=link_groups)
+                     block_tokens=g.block_tokens, elem_bytes=g.elem_bytes, dev_flags=dev_flags, link_groups=link_groups, gpus=gpus)
 
 
 def check_placement(pl: kv.Placement, opl: List[oracle.LayerPlacement]) -> None:
@@ -45,14 +46,14 @@ def check_glt(pl: kv.Placement, opl: List[oracle.LayerPlacement], payload: int, 
 
 def run_parity(wl: W.Workload, *, path: int, kernel: int, bandwidth=None, tuning: Optional[dict] = None,
                interleaved_layout: bool = False, streams: int = 1, dev_flags: Optional[Sequence[int]] = None,
-               profiling: bool = False, link_groups: Optional[Sequence[int]] = None) -> dict:
+               profiling: bool = False, link_groups: Optional[Sequence[int]] = None, gpus: Optional[Sequence[int]] = None) -> dict:
     """Offload every layer of every request, compare stripes with the oracle, retrieve into a poisoned pool,
     compare with the oracle's retrieve and with the source.  Returns a few counters."""
     dev = torch.device("cuda:0")
     g = wl.geom
     elems = g.kvb // 2
     bw = list(bandwidth) if bandwidth is not None else list(wl.default_weights())
-    pool = make_pool(wl, bw, dev_flags=dev_flags, link_groups=link_groups)
+    pool = make_pool(wl, bw, dev_flags=dev_flags, link_groups=link_groups, gpus=gpus)
     try:
         pool.set_path(path)
         pool.set_tuning(kernel=kernel, link_kernel=kernel, **(tuning or {}))

@@ -16,7 +16,7 @@ from parity_util import check_placement, make_pool, run_parity
 
 pytestmark = pytest.mark.gpu
 
-PATHS = {"staged": kv.PATH_STAGED, "zerocopy": kv.PATH_ZEROCOPY, "auto": kv.PATH_AUTO}
+PATHS = {"staged": kv.PATH_STAGED, "zerocopy": kv.PATH_ZEROCOPY, "auto": kv.PATH_AUTO, "hybrid": kv.PATH_HYBRID}
 KERNELS = {"vec16": kv.KERNEL_VEC16, "bulk": kv.KERNEL_BULK}
 
 
@@ -57,11 +57,25 @@ def test_config3_gptoss_sliding_window_layers(path):
     run_parity(wl, path=PATHS[path], kernel=kv.KERNEL_BULK)
 
 
-@pytest.mark.parametrize("path", ["staged", "zerocopy"])
+@pytest.mark.parametrize("path", ["staged", "zerocopy", "hybrid"])
 def test_config4_qwen3_heterogeneous_weights(path):
     wl = W.make_workload(4, scale=1 / 8, n_layers=4)     # 1024 of 1536 blocks, 6 buffers 4:4:2:2:1:1
-    run_parity(wl, path=PATHS[path], kernel=kv.KERNEL_VEC16)
+    out = run_parity(wl, path=PATHS[path], kernel=kv.KERNEL_VEC16)
+    # 32 MiB layers: the hybrid path offloads with the kernel's own stores (no copy) and retrieves through the copy engines
+    assert out["kernels"] == 8 and out["memcpys"] == {"staged": 48, "zerocopy": 0, "hybrid": 24}[path]
     run_parity(wl, path=PATHS[path], kernel=kv.KERNEL_BULK)
+
+
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_hybrid_path_offload_by_kernel_retrieve_by_copy_engine(kernel):
+    """KVPOOL_PATH_HYBRID (both directions of the link at once): same stripes and same retrieved tensors
+    as every other path, on the batched calls, with ranges, with link groups and with a mixed host / HBM pool."""
+    k = KERNELS[kernel]
+    _run_batched(W.make_workload(1), kv.PATH_HYBRID, k, expect_kernels=4, expect_memcpys=4)          # 2 groups: 2 zero-copy packs; 2 unpacks + 2 x 2 copies
+    run_parity(W.make_workload(3, scale=1 / 8, n_layers=4), path=kv.PATH_HYBRID, kernel=k, link_groups=[1, 1, 1, 1])
+    run_parity(W.make_workload(5, scale=1 / 16, n_layers=2), path=kv.PATH_HYBRID, kernel=k, streams=4, tuning={"stage_chunk_bytes": 2 << 20})
+    run_parity(W.make_workload(4, scale=1 / 16, n_layers=2), path=kv.PATH_HYBRID, kernel=k, dev_flags=[0, HBM, 0, 0, HBM, 0])
+    _retrieve_ranges("hybrid", kernel, {"stage_chunk_bytes": 2 << 20}, None)
 
 
 @pytest.mark.parametrize("path", ["staged", "zerocopy"])
@@ -850,6 +864,28 @@ def test_hbm_type_pool_devices_batched_groups_and_ranges(kernel):
             pool.destroy()
 
 
+@pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs a second GPU: the peer (NVLink / NVSwitch) branch of HBM-type pool devices")
+@pytest.mark.parametrize("path", ["staged", "zerocopy", "auto"])
+def test_hbm_type_pool_device_on_a_peer_gpu(path):
+    """SURVEY.md 8(f) row 2 on real hardware, the day a box with two GPUs runs this suite: pool devices in the HBM of GPU 1
+    (cudaDeviceEnablePeerAccess from GPU 0; the kernels reach the stripes by peer loads / stores), alone and mixed with a host
+    buffer — same oracle parity as every other pool, and the GLT says where each stripe lives."""
+    wl = W.make_workload(4, scale=1 / 16, n_layers=3)
+    g = wl.geom
+    caps = [wl.moved_bytes() + (64 << 20)] * 3
+    with kv.KvPool([1.0, 8.0, 8.0], caps, n_layers=g.n_layers, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, dev_flags=[0, HBM, HBM],
+                   gpus=[-1, 1, 1], link_groups=[0, 1, 1]) as pool:
+        assert pool.device_type(1) == (kv.TYPE_HBM, 1) and pool.device_type(2) == (kv.TYPE_HBM, 1)
+        peer = pool.measure_bandwidth(1, kv.MEASURE_KERNEL_RETRIEVE, 64 << 20, 3)
+        host = pool.measure_bandwidth(0, kv.MEASURE_RETRIEVE, 64 << 20, 3)
+        assert peer > 2 * host                                                     # NVLink, not the host link
+    for flags, gpus in (([HBM, HBM], [1, 1]), ([0, HBM], [-1, 1]), ([HBM, 0, HBM], [1, -1, 0])):
+        n = len(flags)
+        wl_n = _custom(g, wl.nphys, [wl.layer_table(0, 0)], n, tuple(float(1 + (i % 2) * 3) for i in range(n)))
+        out = run_parity(wl_n, path=PATHS[path], kernel=kv.KERNEL_VEC16, dev_flags=flags, gpus=gpus)
+        assert out["bytes_compared"] == wl_n.moved_bytes()
+
+
 def test_hbm_type_pool_device_introspection_bandwidth_and_errors():
     g = dict(n_layers=1, n_kv_heads=2, head_dim=64)
     with pytest.raises(kv.KvPoolError) as e:                                       # HBM excludes the host-memory flags
@@ -865,6 +901,18 @@ def test_hbm_type_pool_device_introspection_bandwidth_and_errors():
         host = pool.measure_bandwidth(0, 0, 32 << 20, 3)
         hbm_r, hbm_w = pool.measure_bandwidth(1, 0, 64 << 20, 3), pool.measure_bandwidth(1, 1, 64 << 20, 3)
         assert hbm_r > 5 * host and hbm_w > 5 * host                               # a device-to-device copy, not the host link
+        # the same devices measured with the library's own gather / scatter kernel (what reaches the stripes of such a pool)
+        k_host = [pool.measure_bandwidth(0, d, 32 << 20, 3) for d in (kv.MEASURE_KERNEL_RETRIEVE, kv.MEASURE_KERNEL_OFFLOAD)]
+        k_hbm = [pool.measure_bandwidth(1, d, 64 << 20, 3) for d in (kv.MEASURE_KERNEL_RETRIEVE, kv.MEASURE_KERNEL_OFFLOAD)]
+        assert all(0.5 * host < x < 1.2 * host for x in k_host) and all(x > 5 * host for x in k_hbm)
+        with pytest.raises(kv.KvPoolError) as e:
+            pool.measure_bandwidth(0, 4, 32 << 20, 3)
+        assert e.value.code == kv.EINVAL
+        # kvpool_calibrate: measure, divide what link groups share (none here), install; Eq. 1's weights follow
+        b = pool.calibrate(kv.MEASURE_KERNEL_RETRIEVE, 32 << 20, 3)
+        assert np.array_equal(pool.bandwidths()[0], b) and list(pool.bandwidths()[1]) == [0, 0]
+        assert np.array_equal(pool.weights(), oracle.weights(list(b)))
+        pool.set_bandwidth([50.0, 1500.0])
         pl = pool.place([31])
         c = pl.counts(0)
         assert list(c) == [1, 30]                                                   # 50 : 1500 of 31 blocks
