@@ -78,6 +78,10 @@ def parse_args():
     ap.add_argument("--duplex", action="store_true",
                     help="offload of one request concurrent with retrieve of another (PCIe is full duplex): per-direction and aggregate "
                          "GB/s against simultaneous cudaMemcpyAsync in both directions")
+    ap.add_argument("--profile-range", choices=["staged", "hybrid", "zerocopy"], default=None,
+                    help="--duplex: run only this path and bracket ONE duplex pass (offload of A interleaved with retrieve of B) with "
+                         "cudaProfilerStart / cudaProfilerStop, for `ncu --replay-mode app-range` (concurrent kernels and "
+                         "copies stay concurrent inside a range; per-kernel profiling would serialise them)")
     ap.add_argument("--hostalloc", action="store_true", help="pool buffers from cudaHostAlloc (KVPOOL_DEV_CUDA_HOSTALLOC) instead of the default "
                     "huge-page mapping + cudaHostRegister; main run and --duplex")
     ap.add_argument("--compute-us", type=float, default=0.0, help="--blocked-io: extra calibrated compute per layer (kvpool_spin), microseconds")
@@ -1114,6 +1118,34 @@ def run_duplex(args) -> None:
     src_k, src_v, dst_k, dst_v = [x[0] for x in src], [x[1] for x in src], [x[0] for x in dst], [x[1] for x in dst]
     sa, sb = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
 
+    if args.profile_range:
+        pool.set_path({"staged": kv.PATH_STAGED, "hybrid": kv.PATH_HYBRID, "zerocopy": kv.PATH_ZEROCOPY}[args.profile_range])
+        if args.link_ctas:
+            pool.set_tuning(link_ctas=args.link_ctas)
+        for it in range(3):
+            pa, pb = pool.place(bpl), pool.place(bpl)
+            pool.offload_layers(pb, 0, src_k, src_v, g.kvb, tables, sb)
+            pool.wait_offloads(pb, sb)
+            torch.cuda.synchronize()
+            pool.synchronize()
+            if it == 2:
+                torch.cuda.profiler.start()
+            t0 = time.perf_counter()
+            for l in range(L):
+                pool.offload(pa, l, src[l][0], src[l][1], g.kvb, tables[l], sa)
+                pool.retrieve(pb, l, dst[l][0], dst[l][1], g.kvb, tables[l], sb)
+            pool.wait_offloads(pa, sa)
+            torch.cuda.synchronize()
+            pool.synchronize()
+            t1 = time.perf_counter()
+            if it == 2:
+                torch.cuda.profiler.stop()
+            print(f"# --profile-range {args.profile_range}: pass {it}: {2 * moved / 2**20:.0f} MiB both ways in {1e3 * (t1 - t0):.2f} ms = {2 * moved / (t1 - t0) / 1e9:.1f} GB/s aggregate", flush=True)
+            pa.release()
+            pb.release()
+        pool.destroy()
+        return
+
     # duplex peak of the link: simultaneous H2D and D2H copies of 1 GiB each
     hd, dd = torch.empty(1 << 30, dtype=torch.uint8).pin_memory(), torch.empty(1 << 30, dtype=torch.uint8, device=dev)
     hu, du = torch.empty(1 << 30, dtype=torch.uint8).pin_memory(), torch.empty(1 << 30, dtype=torch.uint8, device=dev)
@@ -1208,7 +1240,8 @@ def run_blocked_io(args) -> None:
             share = np.array(bw) / np.sum(bw)
             moved = wl.moved_bytes()
             caps = [int(moved * sh * 1.25) + (L + 4) * (g.payload + 4096) for sh in share]
-            pool = kv.KvPool(bw, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim)
+            pool = kv.KvPool(bw, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim,
+                             link_groups=[1] * len(bw) if args.link_groups == "shared" else None)
             bpl = wl.blocks_per_layer(0)
             pl = pool.place(bpl)
             elems = g.kvb // 2
