@@ -252,9 +252,12 @@ def test_kv_stream_is_identical_on_cpu_and_gpu():
 
 # (cfg, path, kernel): every BASELINE.json configuration at its FULL size on the default path and kernel — what bench.py
 # times — plus the hand-written link path with the cp.async.bulk kernel on the two largest per-layer launches (config 4,
-# the headline, and config 6, 512 MiB per layer) and the two remaining path x kernel combinations on the headline config.
+# the headline, and config 6, 512 MiB per layer), the two remaining path x kernel combinations on the headline config, and the
+# hybrid path on config 6 (whose 512 MiB layers retrieve through DEVICE-MAJOR chunks, as on the default path: the ring's
+# slots hold 256 MiB).
 FULL_SIZE_CASES = [(2, "auto", "vec16"), (3, "auto", "vec16"), (4, "auto", "vec16"), (5, "auto", "vec16"), (6, "auto", "vec16"),
-                   (4, "zerocopy", "bulk"), (6, "zerocopy", "bulk"), (4, "auto", "bulk"), (4, "zerocopy", "vec16"), (3, "zerocopy", "bulk")]
+                   (4, "zerocopy", "bulk"), (6, "zerocopy", "bulk"), (4, "auto", "bulk"), (4, "zerocopy", "vec16"), (3, "zerocopy", "bulk"),
+                   (6, "hybrid", "bulk")]
 
 
 @pytest.mark.parametrize("cfg,path,kernel", FULL_SIZE_CASES)
@@ -1233,12 +1236,13 @@ def test_red_zones_around_planes_stripes_and_staging_stay_intact(kernel):
 
 
 @pytest.mark.parametrize("kernel", list(KERNELS))
-@pytest.mark.parametrize("path", ["staged", "zerocopy"])
+@pytest.mark.parametrize("path", ["staged", "zerocopy", "staged-chunked"])
 def test_device_side_table_check_skips_and_counts_bad_entries(path, kernel):
     """kvpool_set_table_check (R12, opt-in): table entries outside [0, nphys) are skipped — nothing outside the
     planes is read or written (red zones intact), the other blocks move exactly as the oracle says — and counted; with
     a clean table the check changes nothing."""
-    p, k = PATHS[path], KERNELS[kernel]
+    # staged-chunked: a slot holds 5 blocks, so the layer travels in device-major chunks (launches that walk the inverse map)
+    p, k, chunked = PATHS[path.split("-")[0]], KERNELS[kernel], path.endswith("chunked")
     rng = np.random.default_rng(71)
     dev = torch.device("cuda:0")
     g = W.Geometry(n_layers=1, n_kv_heads=2, head_dim=80)                 # kvb = 5120 B, ragged against the 4 KiB piece
@@ -1253,7 +1257,7 @@ def test_device_side_table_check_skips_and_counts_bad_entries(path, kernel):
     pool = make_pool(wl)
     try:
         pool.set_path(p)
-        pool.set_tuning(kernel=k, link_kernel=k)
+        pool.set_tuning(kernel=k, link_kernel=k, **({"stage_chunk_bytes": 5 * 2 * g.kvb} if chunked else {}))
         pool.set_table_check(nphys)
         pl = pool.place([K])
 
