@@ -55,6 +55,14 @@ def _load():
         lib.orc_checksum.argtypes = [vp, vp, u64, u64, vp, u64]
         lib.orc_layer_parallel.restype = ctypes.c_int
         lib.orc_layer_parallel.argtypes = [ctypes.c_int, vp, vp, u64, u64, vp, u64, vp, vp, vp, u32]
+        lib.orc_lba_range_len.restype = u64
+        lib.orc_lba_range_len.argtypes = [u64, u64, u64]
+        lib.orc_ssd_direct_store.restype = u64
+        lib.orc_ssd_direct_store.argtypes = [vp, u64, u64, u64, vp, u64, u64]
+        lib.orc_ssd_location.restype = None
+        lib.orc_ssd_location.argtypes = [u64, u64, u64, u64, vp, vp]
+        lib.orc_ssd_direct_retrieve.restype = None
+        lib.orc_ssd_direct_retrieve.argtypes = [vp, u64, u64, u64, vp, u64]
         _lib = lib
     return _lib
 
@@ -184,3 +192,37 @@ def checksum(kv_layer: np.ndarray, table: np.ndarray) -> int:
     kp, vp_, stride, kvb = _planes(kv_layer)
     table = np.ascontiguousarray(table, dtype=np.int32)
     return int(_load().orc_checksum(kp, vp_, stride, kvb, _ptr(table), table.shape[0]))
+
+
+# ---- KV-passthrough: the SSD as an array of sectors ------------------------------------------------
+def lba_range_len(set_size: int, kv_size: int, sector_size: int) -> int:
+    """ceil(|offload_set| * KV_size / sector_size) sectors (PAPER.md:183)."""
+    return int(_load().orc_lba_range_len(int(set_size), int(kv_size), int(sector_size)))
+
+
+def ssd_direct_store(disk: np.ndarray, sector_size: int, first_lba: int, stripe: np.ndarray, kv_size: int) -> int:
+    """SSD_Direct_Store of one offload set (`stripe`: its payloads in slot order) into `disk` (uint8, a whole number of
+    sectors) at first_lba; returns the range length in sectors."""
+    assert disk.dtype == np.uint8 and disk.flags["C_CONTIGUOUS"] and disk.nbytes % sector_size == 0
+    stripe = np.ascontiguousarray(stripe, dtype=np.uint8)
+    assert stripe.nbytes % kv_size == 0
+    n = int(_load().orc_ssd_direct_store(_ptr(disk), disk.nbytes // sector_size, int(sector_size), int(first_lba),
+                                         _ptr(stripe) if stripe.size else None, stripe.nbytes // kv_size, int(kv_size)))
+    if n == 2 ** 64 - 1:
+        raise ValueError("the LBA range does not fit the disk")
+    return n
+
+
+def ssd_location(first_lba: int, slot: int, kv_size: int, sector_size: int) -> Tuple[int, int]:
+    """GLT location of KV cache `slot` of a set stored at first_lba: (LBA, byte inside that sector)."""
+    lba, off = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    _load().orc_ssd_location(int(first_lba), int(slot), int(kv_size), int(sector_size), ctypes.addressof(lba), ctypes.addressof(off))
+    return int(lba.value), int(off.value)
+
+
+def ssd_direct_retrieve(disk: np.ndarray, sector_size: int, lba: int, byte_in_sector: int, kv_size: int) -> np.ndarray:
+    """SSD_Direct_Retrieve of one KV cache by its GLT location."""
+    assert disk.dtype == np.uint8 and disk.flags["C_CONTIGUOUS"]
+    out = np.empty(int(kv_size), dtype=np.uint8)
+    _load().orc_ssd_direct_retrieve(_ptr(disk), int(sector_size), int(lba), int(byte_in_sector), _ptr(out), int(kv_size))
+    return out

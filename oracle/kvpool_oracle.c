@@ -25,7 +25,12 @@
  *                             indexing into the range's slots; stripe bytes outside the range's slots keep their fill
  *   orc_checksum            — closed form n_words^2 * c for constant words, python big-int restatement, sensitivity
  *                             to swapping two blocks
- *   stripe offsets inside a pool buffer: PARITY UNPINNED (implementation detail; not produced here).
+ *   orc_lba_range_len       — the paper's own formula against hand-worked values (tests/golden/
+ *                             worked_lba_ranges.txt), the defining inequality of a ceiling, exact rationals
+ *   orc_ssd_direct_store / orc_ssd_direct_retrieve / orc_ssd_location
+ *                           — numpy slicing of the sector array, sector-multiple KV sizes reduce to whole-sector
+ *                             copies, zero padding and untouched neighbours, brute-force byte addresses, round trip
+ *   stripe offsets inside a pool buffer and the FIRST LBA of a range: PARITY UNPINNED (allocator detail; not produced here).
  *
  * Build: gcc -O2 -shared -fPIC -pthread -o liboracle.so kvpool_oracle.c   (oracle/__init__.py does it)
  */
@@ -235,4 +240,50 @@ int orc_layer_parallel(int retrieve, uint8_t *k_plane, uint8_t *v_plane, uint64_
     }
     for (uint32_t i = 0; i < n; ++i) pthread_join(th[i], NULL);
     return 0;
+}
+
+/* ---- KV-passthrough, SSD branch of Algorithm 1 (l.20-21) and of the retrieval -----------
+ * The SSD is an array of sectors addressed by logical block address (LBA): `disk` holds disk_sectors * sector_size
+ * bytes, sector x at disk + x*sector_size.
+ *
+ * SSD_Direct_Store: "allocates a contiguous LBA range on the target device and writes the KV caches to that range ...
+ * The LBA range length is ceil(|offload_set_i| * KV_size / sector_size) blocks". */
+uint64_t orc_lba_range_len(uint64_t set_size, uint64_t kv_size, uint64_t sector_size) {
+    unsigned __int128 bytes = (unsigned __int128)set_size * kv_size;
+    uint64_t len = (uint64_t)(bytes / sector_size);
+    if (bytes % sector_size) len += 1;          /* ceiling */
+    return len;
+}
+
+/* The offload set (already in the order MEMSTORE would lay it out: slot 0, 1, ... — `set` holds set_size payloads of
+ * kv_size bytes) is written to the range starting at first_lba, payloads back to back; what is left of the last sector
+ * is zero (the paper does not say what fills it: DESIGN.md R18).  Sectors outside the range are not touched.  Returns
+ * the range length in sectors, or UINT64_MAX if the range does not fit the disk. */
+uint64_t orc_ssd_direct_store(uint8_t *disk, uint64_t disk_sectors, uint64_t sector_size, uint64_t first_lba,
+                              const uint8_t *set, uint64_t set_size, uint64_t kv_size) {
+    uint64_t len = orc_lba_range_len(set_size, kv_size, sector_size);
+    if (first_lba > disk_sectors || len > disk_sectors - first_lba) return UINT64_MAX;
+    uint8_t *at = disk + first_lba * sector_size;
+    uint64_t bytes = set_size * kv_size;
+    for (uint64_t s = 0; s < set_size; ++s) memcpy(at + s * kv_size, set + s * kv_size, kv_size);
+    memset(at + bytes, 0, len * sector_size - bytes);
+    return len;
+}
+
+/* "The resulting LBA information is returned to the bandwidth-aware KV allocator and stored in the GLT";
+ * Table I: location = LBA for type SSD.  KV cache number `slot` of a set stored at first_lba starts in sector
+ * first_lba + floor(slot*KV_size / sector_size), at byte (slot*KV_size) mod sector_size of that sector (0 whenever
+ * KV_size is a multiple of the sector size, as for every model shape of the paper; R18). */
+void orc_ssd_location(uint64_t first_lba, uint64_t slot, uint64_t kv_size, uint64_t sector_size, uint64_t *lba,
+                      uint64_t *byte_in_sector) {
+    unsigned __int128 off = (unsigned __int128)slot * kv_size;
+    *lba = first_lba + (uint64_t)(off / sector_size);
+    *byte_in_sector = (uint64_t)(off % sector_size);
+}
+
+/* SSD_Direct_Retrieve: "reads back a KV cache from SSD using the device_idx and location fields stored in the GLT"
+ * (PAPER.md:185): kv_size bytes starting at (lba, byte_in_sector). */
+void orc_ssd_direct_retrieve(const uint8_t *disk, uint64_t sector_size, uint64_t lba, uint64_t byte_in_sector,
+                             uint8_t *payload_out, uint64_t kv_size) {
+    memcpy(payload_out, disk + lba * sector_size + byte_in_sector, kv_size);
 }

@@ -417,3 +417,92 @@ def test_checksum_closed_form_python_restatement_and_sensitivity():
     assert oracle.checksum(kv, t2) != oracle.checksum(kv, table)
     assert oracle.checksum(np.ascontiguousarray(kv[::-1]), table) != oracle.checksum(kv, table)
     assert oracle.checksum(kv, table[:0]) == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# KV-passthrough: LBA range length, SSD_Direct_Store, GLT location, SSD_Direct_Retrieve
+# ------------------------------------------------------------------------------------------------
+def test_lba_range_length_hand_worked_values_and_the_definition_of_a_ceiling(golden_dir):
+    rows = list(_golden_rows(golden_dir, "worked_lba_ranges.txt"))
+    assert len(rows) == 10
+    for n, kv, sec, want, _how in rows:
+        assert oracle.lba_range_len(int(n), int(kv), int(sec)) == int(want), (n, kv, sec)
+    # the defining property of ceil(x) for x = n*kv/sec, in exact rationals: len - 1 < x <= len
+    # (a floor, a "+1 always" or a rounding to nearest each break one side of it)
+    rng = np.random.default_rng(21)
+    for _ in range(2000):
+        n, kv = int(rng.integers(0, 5000)), int(rng.integers(1, 70000))
+        sec = int(rng.choice([512, 520, 4096, 4160, 1, 7]))
+        got, x = oracle.lba_range_len(n, kv, sec), Fraction(n * kv, sec)
+        assert got - 1 < x <= got
+    # no 64-bit overflow in set_size * kv_size (a 16 EiB product still divides exactly)
+    assert oracle.lba_range_len(2 ** 40, 2 ** 30, 4096) == 2 ** 58
+
+
+def test_ssd_direct_store_is_a_slice_assignment_of_the_sector_array_zero_padded():
+    rng = np.random.default_rng(22)
+    for kv, sec, n, first, sectors in [(96, 512, 17, 3, 16), (65536, 512, 5, 100, 800), (1536, 4096, 5, 1, 4), (48, 512, 1, 0, 1), (512, 512, 9, 7, 16)]:
+        stripe = rng.integers(0, 256, size=n * kv, dtype=np.uint8)
+        disk = np.full(sectors * sec, 0xA5, dtype=np.uint8)
+        length = oracle.ssd_direct_store(disk, sec, first, stripe, kv)
+        assert length == oracle.lba_range_len(n, kv, sec)
+        rows = disk.reshape(sectors, sec)
+        flat = rows[first:first + length].reshape(-1)
+        assert np.array_equal(flat[:n * kv], stripe)                       # payloads back to back from the first sector on
+        assert not flat[n * kv:].any()                                     # the rest of the last sector is zero
+        assert (rows[:first] == 0xA5).all() and (rows[first + length:] == 0xA5).all()   # neighbours untouched
+        if kv % sec == 0:                                                  # sector-multiple payloads: whole-sector copies, no padding
+            assert length * sec == n * kv
+    with pytest.raises(ValueError):                                        # a range that runs off the disk is refused, nothing written
+        disk = np.full(4 * 512, 0xA5, dtype=np.uint8)
+        oracle.ssd_direct_store(disk, 512, 3, np.zeros(2 * 512, dtype=np.uint8), 512)
+    assert (disk == 0xA5).all()
+    # the empty set writes nothing
+    disk = np.full(4 * 512, 0xA5, dtype=np.uint8)
+    assert oracle.ssd_direct_store(disk, 512, 2, np.zeros(0, dtype=np.uint8), 64) == 0 and (disk == 0xA5).all()
+
+
+def test_ssd_location_and_direct_retrieve_find_every_kv_cache_by_its_byte_address():
+    rng = np.random.default_rng(23)
+    for kv, sec, n, first in [(96, 512, 40, 5), (65536, 4096, 6, 2), (1536, 4096, 9, 0), (512, 512, 12, 3), (700, 520, 11, 1)]:
+        stripe = rng.integers(0, 256, size=n * kv, dtype=np.uint8)
+        sectors = first + oracle.lba_range_len(n, kv, sec) + 2
+        disk = np.full(sectors * sec, 0x5A, dtype=np.uint8)
+        oracle.ssd_direct_store(disk, sec, first, stripe, kv)
+        seen = set()
+        for s in range(n):
+            lba, off = oracle.ssd_location(first, s, kv, sec)
+            # the location is the byte address of the payload, split into (sector, byte inside it): brute force over the
+            # candidates instead of trusting the division
+            want = [(a, b) for a in range(sectors) for b in range(sec) if a * sec + b == first * sec + s * kv]
+            assert [(lba, off)] == want
+            assert 0 <= off < sec and (off == 0 or kv % sec)
+            seen.add((lba, off))
+            assert np.array_equal(oracle.ssd_direct_retrieve(disk, sec, lba, off, kv), stripe[s * kv:(s + 1) * kv])
+        assert len(seen) == n                                              # distinct KV caches, distinct locations
+        if kv % sec == 0:                                                  # LBA advances by KV_size / sector_size per cache
+            assert [oracle.ssd_location(first, s, kv, sec)[0] for s in range(n)] == [first + s * (kv // sec) for s in range(n)]
+
+
+def test_ssd_store_then_retrieve_reproduces_an_offloaded_layer():
+    # MEMSTORE's stripe order is what SSD_Direct_Store writes (Alg. 1 l.18 / l.21 differ only in the medium): store the
+    # pinned orc_offload_layer's stripes on two "SSDs", read every KV cache back through its location, scatter it
+    rng = np.random.default_rng(24)
+    nphys, kvb, K, sec = 23, 96, 17, 512
+    kv = _tiny_layer(rng, nphys, kvb)
+    table = rng.permutation(nphys)[:K].astype(np.int32)
+    pl = oracle.place([3.0, 1.0], [K])[0]
+    stripes = oracle.offload_layer(kv, table, pl)
+    disks, first = [], [4, 1]
+    for i in range(2):
+        d = np.full(64 * sec, 0xEE, dtype=np.uint8)
+        assert oracle.ssd_direct_store(d, sec, first[i], stripes[i], 2 * kvb) == oracle.lba_range_len(int(pl.counts[i]), 2 * kvb, sec)
+        disks.append(d)
+    back = np.full_like(kv, 0x7FC1)
+    for j in range(K):
+        i, s = int(pl.dev[j]), int(pl.slot[j])
+        payload = oracle.ssd_direct_retrieve(disks[i], sec, *oracle.ssd_location(first[i], s, 2 * kvb, sec), 2 * kvb).view(np.uint16)
+        back[0, table[j]], back[1, table[j]] = payload[:kvb // 2], payload[kvb // 2:]
+    ref = np.full_like(kv, 0x7FC1)
+    ref[:, table] = kv[:, table]
+    assert np.array_equal(back, ref)
