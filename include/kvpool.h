@@ -48,7 +48,8 @@ enum {
   KVPOOL_ECUDA = -3,  /* a CUDA runtime call failed (message has the CUDA error string) */
   KVPOOL_ENUMA = -4,  /* KVPOOL_DEV_NUMA_STRICT and the pages could not be bound to the requested node */
   KVPOOL_ESTATE = -5, /* retrieve of a layer that was never offloaded; set_bandwidth while placements are live; ... */
-  KVPOOL_ENOENT = -6  /* kvpool_glt_find: no KV cache with that identifier */
+  KVPOOL_ENOENT = -6, /* kvpool_glt_find: no KV cache with that identifier */
+  KVPOOL_EIO = -7     /* an SSD-type pool device could not be opened, or a store / retrieve command on it failed */
 };
 
 /* pool-device flags */
@@ -62,6 +63,15 @@ enum {
                                         peer of the pool's GPU, or that GPU itself.  Its stripes are reached
                                         by the kernels directly (peer loads / stores); no staging, no copy engine.            */
 
+#define KVPOOL_DEV_SSD 16u           /* the pool device is block storage addressed by LBA (the paper's SSD type, KV-passthrough,
+                                        PAPER.md:179-185): `path` names a block device (/dev/nvme0n1, a partition) or a
+                                        file standing in for one.  It is opened O_DIRECT - the kernel's page cache and the
+                                        file system's data path are bypassed; on a raw block device there is no file system
+                                        at all - and driven by the device's own worker thread through asynchronous store /
+                                        retrieve commands; GPU streams and the worker hand bounce lanes to each other with
+                                        stream write-value / wait-value operations, no host callback and no
+                                        synchronisation.  Excludes every other flag.               */
+
 #define KVPOOL_MEASURE_KERNEL_RETRIEVE 2 /* kvpool_measure_bandwidth / kvpool_calibrate `direction`, see there */
 #define KVPOOL_MEASURE_KERNEL_OFFLOAD 3
 
@@ -70,7 +80,7 @@ enum {
 /* pool-device types (GLT `type`, Table I) */
 enum {
   KVPOOL_TYPE_MEM = 0, /* pinned host memory; location = host pointer                                     */
-  KVPOOL_TYPE_SSD = 1, /* the paper's second type (location = LBA); not built: no NVMe on the box         */
+  KVPOOL_TYPE_SSD = 1, /* block storage (KVPOOL_DEV_SSD); location = logical block address (LBA)          */
   KVPOOL_TYPE_HBM = 2  /* GPU memory (KVPOOL_DEV_HBM); location = device pointer valid on the pool's GPU  */
 };
 
@@ -114,7 +124,14 @@ typedef struct {           /* one pool device (Table I)           
                            /* paper's "independent I/O streams", are per independent      */
                            /* resource: copies that share a link only slow each other down, and layer   */
                            /* l+1's copies would delay layer l's), and kvpool_calibrate divides what    */
-                           /* they share.  Placement (Eq. 1-2) is untouched: only b_i changes           */
+                           /* they share.  Placement (Eq. 1-2) is untouched: only b_i changes.  An SSD-   */
+                           /* type device always has I/O streams of its own (a stream that waits for a   */
+                           /* disk must not hold up the copies of a host buffer)                         */
+  const char* path;        /* SSD: block device or file (host string, copied); NULL otherwise           */
+  uint32_t sector_bytes;   /* SSD: sector size LBAs count in - a power of two in 512..65536 and a       */
+                           /* multiple of the device's logical sector; 0 = ask the block device, 4096   */
+                           /* for a file.  Otherwise 0                                                  */
+  uint32_t reserved;       /* 0                                                                         */
 } kvpool_device_desc;
 
 typedef struct { /* geometry of one paged KV block */
@@ -143,7 +160,10 @@ typedef struct {         /* kvpool_set_tuning; 0 in any field = library default 
                             without chunking.  UINT64_MAX: no cap (a slot holds the largest layer); at least one block per chunk */
   uint32_t pdl;          /* programmatic dependent launch of the library's kernels (the next layer's launch latency and
                             ramp hide under the current layer's kernel): 1 = on (default), 2 = off                          */
-  uint32_t reserved;     /* 0                                                                                             */
+  uint32_t ssd_lanes;    /* SSD-type devices: bounce lanes per device and direction (default 4): a lane is one store /
+                            retrieve command in flight - pinned host memory for the disk's DMA plus a device staging piece */
+  uint64_t ssd_chunk_bytes; /* SSD-type devices: bytes per command (default 8 MiB; at least one KV cache plus two sectors).
+                            ssd_lanes / ssd_chunk_bytes are fixed by the first kvpool_place: ESTATE afterwards           */
 } kvpool_tuning;
 
 /* ---- pure host arithmetic (no CUDA, no pool) --------------------------------------------------------
@@ -156,6 +176,11 @@ KVPOOL_API int kvpool_plan_weights(const double* bandwidth_gbps /*host[n]*/, uin
  * NULL (counts only).                                                                                  */
 KVPOOL_API int kvpool_plan_layer(const uint64_t* w /*host[n]*/, uint32_t n, uint64_t K, uint32_t* counts_out /*host[n]*/,
                       uint8_t* dev_out /*host[K] or NULL*/, uint32_t* slot_out /*host[K] or NULL*/);
+
+/* KV-passthrough: the length, in sectors, of the contiguous LBA range SSD_Direct_Store allocates for an
+ * offload set of set_size KV caches of kv_size bytes: ceil(set_size * kv_size / sector_bytes).  EINVAL if sector_bytes
+ * is 0 or the result does not fit 64 bits.                                                                          */
+KVPOOL_API int kvpool_plan_lba_range(uint64_t set_size, uint64_t kv_size, uint32_t sector_bytes, uint64_t* n_sectors_out /*host*/);
 
 /* The caller's contract on a block table (R12), checked on a HOST copy: K entries, each in [0, nphys), no
  * physical block named twice (a duplicate would make two KV caches race for one block at retrieve).  The hot path
@@ -351,6 +376,23 @@ KVPOOL_API int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint3
  * blocking cudaMemcpy for HBM).  The caller must have waited for the offload (kvpool_wait_offloads + stream sync).
  * For inspection and tests; not a hot-path call.                                                                 */
 KVPOOL_API int kvpool_stripe_read(kvpool_t* pool, const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, void* dst_host, uint64_t nbytes);
+/* SSD-type pool devices (GLT `type` = KVPOOL_TYPE_SSD, `location` = LBA; Table I).  For such a device
+ * kvpool_stripe returns the first LBA of the stripe's range (cast to a pointer-sized integer) and kvpool_lookup the LBA
+ * of the sector in which the KV cache's payload starts; kvpool_device_info's host_base is NULL.
+ * kvpool_ssd_range: the contiguous LBA range SSD_Direct_Store allocated for the offload set of (layer, dev):
+ *   n_sectors = ceil(c_{l,dev} * P / sector_bytes), first_lba in units of sector_bytes.  The payloads
+ *   follow each other in slot order from the first byte of the range; the rest of the last sector is zero.
+ * kvpool_ssd_location: where KV cache `block` of `layer` lives: LBA = first_lba + floor(slot*P / sector_bytes) and the
+ *   byte inside that sector (0 whenever P is a multiple of the sector size).  EINVAL if the block's device is not SSD.
+ * kvpool_ssd_info: sector size, whether the device is open with direct I/O (0 = the file system refused O_DIRECT and
+ *   the library fell back to buffered I/O), whether it is a block device (0 = a file standing in for one), and the
+ *   store / retrieve commands its worker has completed.  Any out pointer may be NULL.                               */
+KVPOOL_API int kvpool_ssd_range(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, uint64_t* first_lba, uint64_t* n_sectors,
+                     uint32_t* sector_bytes);
+KVPOOL_API int kvpool_ssd_location(const kvpool_placement_t* pl, uint32_t layer, uint32_t block, uint64_t* lba, uint32_t* byte_in_sector);
+KVPOOL_API int kvpool_ssd_info(const kvpool_t* pool, uint32_t dev, uint32_t* sector_bytes, int32_t* direct_io, int32_t* block_device,
+                    uint64_t* stores_completed, uint64_t* retrieves_completed);
+
 /* Keyed GLT (Table I `key` = "hash of the KV cache identifier"): give the K_l KV caches of a layer
  * caller-chosen 64-bit identifiers (e.g. the prefix-hash of the tokens a block covers, mixed with the layer), after
  * which any of them is found by identifier alone, across placements — what cross-request prefix reuse needs.

@@ -16,18 +16,18 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libkvpool.so")
 
 MAX_DEVICES = 32
-OK, EINVAL, ENOMEM, ECUDA, ENUMA, ESTATE, ENOENT = 0, -1, -2, -3, -4, -5, -6
-DEV_WRITE_COMBINED, DEV_NUMA_STRICT, DEV_HBM, DEV_CUDA_HOSTALLOC = 1, 2, 4, 8
+OK, EINVAL, ENOMEM, ECUDA, ENUMA, ESTATE, ENOENT, EIO = 0, -1, -2, -3, -4, -5, -6, -7
+DEV_WRITE_COMBINED, DEV_NUMA_STRICT, DEV_HBM, DEV_CUDA_HOSTALLOC, DEV_SSD = 1, 2, 4, 8, 16
 TYPE_MEM, TYPE_SSD, TYPE_HBM = 0, 1, 2
 NUMA_AUTO = -2
 MEASURE_RETRIEVE, MEASURE_OFFLOAD, MEASURE_KERNEL_RETRIEVE, MEASURE_KERNEL_OFFLOAD = 0, 1, 2, 3
 PROFILE_OFF, PROFILE_SIDE, PROFILE_INSTREAM = 0, 1, 2
 PATH_AUTO, PATH_STAGED, PATH_ZEROCOPY, PATH_HYBRID = 0, 1, 2, 3
 KERNEL_VEC16, KERNEL_BULK = 0, 1
-_ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA", ESTATE: "ESTATE", ENOENT: "ENOENT"}
+_ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA", ESTATE: "ESTATE", ENOENT: "ENOENT", EIO: "EIO"}
 
 EXPORTS = [
-    "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
+    "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_plan_lba_range", "kvpool_ssd_range", "kvpool_ssd_location", "kvpool_ssd_info", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
     "kvpool_measure_bandwidth", "kvpool_share_bandwidth", "kvpool_calibrate", "kvpool_bandwidths", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release", "kvpool_set_tables",
     "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
@@ -37,7 +37,7 @@ EXPORTS = [
 
 class DeviceDesc(ctypes.Structure):
     _fields_ = [("bandwidth_gbps", c_double), ("capacity_bytes", c_uint64), ("numa_node", c_int32), ("flags", c_uint32),
-                ("gpu", c_int32), ("link_group", c_uint32)]
+                ("gpu", c_int32), ("link_group", c_uint32), ("path", c_char_p), ("sector_bytes", c_uint32), ("reserved", c_uint32)]
 
 
 class Geometry(ctypes.Structure):
@@ -49,7 +49,7 @@ class Tuning(ctypes.Structure):
     _fields_ = [("kernel", c_uint32), ("link_kernel", c_uint32), ("hbm_ctas", c_uint32), ("link_ctas", c_uint32), ("bulk_chunk", c_uint32),
                 ("bulk_stages", c_uint32), ("bulk_warps", c_uint32), ("stage_slots", c_uint32),
                 ("vec_threads", c_uint32), ("vec_unroll", c_uint32), ("auto_threshold_bytes", c_uint64), ("group_bytes", c_uint64),
-                ("stage_chunk_bytes", c_uint64), ("pdl", c_uint32), ("reserved", c_uint32)]
+                ("stage_chunk_bytes", c_uint64), ("pdl", c_uint32), ("ssd_lanes", c_uint32), ("ssd_chunk_bytes", c_uint64)]
 
 
 class KvPoolError(RuntimeError):
@@ -75,6 +75,10 @@ def lib():
         sig = {
             "kvpool_plan_weights": [vp, c_uint32, vp],
             "kvpool_plan_layer": [vp, c_uint32, c_uint64, vp, vp, vp],
+            "kvpool_plan_lba_range": [c_uint64, c_uint64, c_uint32, POINTER(c_uint64)],
+            "kvpool_ssd_range": [vp, c_uint32, c_uint32, POINTER(c_uint64), POINTER(c_uint64), POINTER(c_uint32)],
+            "kvpool_ssd_location": [vp, c_uint32, c_uint32, POINTER(c_uint64), POINTER(c_uint32)],
+            "kvpool_ssd_info": [vp, c_uint32, POINTER(c_uint32), POINTER(c_int32), POINTER(c_int32), POINTER(c_uint64), POINTER(c_uint64)],
             "kvpool_validate_table": [vp, c_uint64, c_uint64],
             "kvpool_set_table_check": [vp, c_uint64],
             "kvpool_table_errors": [vp, vp],
@@ -187,6 +191,12 @@ def kvpool_plan_layer(w: Sequence[int], K: int, with_map: bool = True):
     return (counts, dev, slot) if with_map else counts
 
 
+def kvpool_plan_lba_range(set_size: int, kv_size: int, sector_bytes: int) -> int:
+    n = c_uint64()
+    _ck(lib().kvpool_plan_lba_range(int(set_size), int(kv_size), int(sector_bytes), byref(n)))
+    return n.value
+
+
 def kvpool_share_bandwidth(alone_gbps: Sequence[float], link_group: Sequence[int]) -> np.ndarray:
     a = np.ascontiguousarray(alone_gbps, dtype=np.float64)
     g = np.ascontiguousarray(link_group, dtype=np.uint32)
@@ -231,15 +241,27 @@ class Placement:
 
     def stripe(self, layer: int, dev: int) -> np.ndarray:
         """The stripe's bytes as uint8: a numpy VIEW of the pinned pool buffer for a MEM device (no copy), a host
-        copy made by kvpool_stripe_read for an HBM device."""
+        copy made by kvpool_stripe_read for an HBM or SSD device."""
         loc, n = self.stripe_location(layer, dev)
         if n == 0:
             return np.zeros(0, dtype=np.uint8)
-        if self.pool.device_type(dev)[0] == TYPE_HBM:
+        if self.pool.device_type(dev)[0] != TYPE_MEM:
             out = np.empty(n, dtype=np.uint8)
             _ck(lib().kvpool_stripe_read(self.pool.handle, self.handle, layer, dev, out.ctypes.data, n))
             return out
         return np.ctypeslib.as_array(ctypes.cast(loc, POINTER(c_uint8)), shape=(n,))
+
+    def ssd_range(self, layer: int, dev: int) -> Tuple[int, int, int]:
+        """(first LBA, sectors, sector bytes) of the stripe's LBA range on an SSD-type device."""
+        a, n, sec = c_uint64(), c_uint64(), c_uint32()
+        _ck(lib().kvpool_ssd_range(self.handle, layer, dev, byref(a), byref(n), byref(sec)))
+        return a.value, n.value, sec.value
+
+    def ssd_location(self, layer: int, block: int) -> Tuple[int, int]:
+        """(LBA, byte inside that sector) of a KV cache that lives on an SSD-type device."""
+        a, b = c_uint64(), c_uint32()
+        _ck(lib().kvpool_ssd_location(self.handle, layer, block, byref(a), byref(b)))
+        return a.value, b.value
 
     def release(self) -> None:
         if self.handle:
@@ -253,13 +275,15 @@ class KvPool:
     def __init__(self, bandwidth_gbps: Sequence[float], capacity_bytes: Sequence[int], *, n_layers: int, n_kv_heads: int,
                  head_dim: int, block_tokens: int = 16, elem_bytes: int = 2, cuda_device: int = 0,
                  numa_nodes: Optional[Sequence[int]] = None, dev_flags: Optional[Sequence[int]] = None,
-                 gpus: Optional[Sequence[int]] = None, link_groups: Optional[Sequence[int]] = None):
+                 gpus: Optional[Sequence[int]] = None, link_groups: Optional[Sequence[int]] = None,
+                 paths: Optional[Sequence[Optional[str]]] = None, sector_bytes: Optional[Sequence[int]] = None):
         n = len(bandwidth_gbps)
         descs = (DeviceDesc * n)()
         for i in range(n):
             descs[i] = DeviceDesc(float(bandwidth_gbps[i]), int(capacity_bytes[i]), int(numa_nodes[i]) if numa_nodes else -1,
                                   int(dev_flags[i]) if dev_flags else 0, int(gpus[i]) if gpus else -1,
-                                  int(link_groups[i]) if link_groups else 0)
+                                  int(link_groups[i]) if link_groups else 0,
+                                  os.fsencode(paths[i]) if paths and paths[i] else None, int(sector_bytes[i]) if sector_bytes else 0, 0)
         self.geometry = Geometry(n_layers, block_tokens, n_kv_heads, head_dim, elem_bytes)
         self.kvb = block_tokens * n_kv_heads * head_dim * elem_bytes
         self.payload = 2 * self.kvb
@@ -431,10 +455,15 @@ class KvPool:
         return {"host_base": base.value, "capacity": cap.value, "used": used.value, "numa_node": node.value}
 
     def device_type(self, dev: int) -> Tuple[int, int]:
-        """(TYPE_MEM | TYPE_HBM, CUDA ordinal holding an HBM device or -1)."""
+        """(TYPE_MEM | TYPE_SSD | TYPE_HBM, CUDA ordinal holding an HBM device or -1)."""
         t, g = c_uint32(), c_int32()
         _ck(lib().kvpool_device_type(self.handle, dev, byref(t), byref(g)))
         return t.value, g.value
+
+    def ssd_info(self, dev: int) -> dict:
+        sec, direct, blk, st, rt = c_uint32(), c_int32(), c_int32(), c_uint64(), c_uint64()
+        _ck(lib().kvpool_ssd_info(self.handle, dev, byref(sec), byref(direct), byref(blk), byref(st), byref(rt)))
+        return {"sector_bytes": sec.value, "direct_io": bool(direct.value), "block_device": bool(blk.value), "stores": st.value, "retrieves": rt.value}
 
     def set_table_check(self, nphys: int) -> None:
         _ck(lib().kvpool_set_table_check(self.handle, int(nphys)))

@@ -42,6 +42,8 @@ void default_tuning(kvpool* p) {
   p->tune.group_bytes = 64ull << 20;
   p->tune.auto_threshold_bytes = 8ull << 20;
   p->tune.pdl = 1;
+  p->tune.ssd_lanes = 4;
+  p->tune.ssd_chunk_bytes = 8ull << 20;
 }
 
 void free_slots(kvpool* p) {
@@ -191,6 +193,7 @@ LaunchCfg launch_cfg(const kvpool* p, bool link_bound, bool pack) {
 
 // Does a transfer of `host_bytes` to / from host-memory devices go through the staging ring and the copy engines?
 bool use_staged(const kvpool* p, bool pack, uint64_t host_bytes) {
+  if (p->ssd_mask) return true;   // a pool with an SSD-type device moves device-major on every path (kvpool_ssd.cu)
   if (all_hbm(p)) return false;   // nothing to stage: every stripe is reached in place (one kernel, HBM grid)
   if (host_bytes == 0) return false;  // all of its blocks went to HBM-type devices (tiny K, large weights)
   switch (p->path) {
@@ -276,8 +279,12 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
   for (uint32_t i = 0; i < n_devs; ++i) {
     bw[i] = devs[i].bandwidth_gbps;
     if (devs[i].capacity_bytes == 0) return fail(KVPOOL_EINVAL, "create: device %u has zero capacity", i);
-    if (devs[i].flags & ~(KVPOOL_DEV_WRITE_COMBINED | KVPOOL_DEV_NUMA_STRICT | KVPOOL_DEV_HBM | KVPOOL_DEV_CUDA_HOSTALLOC)) return fail(KVPOOL_EINVAL, "create: device %u unknown flags", i);
+    if (devs[i].flags & ~(KVPOOL_DEV_WRITE_COMBINED | KVPOOL_DEV_NUMA_STRICT | KVPOOL_DEV_HBM | KVPOOL_DEV_CUDA_HOSTALLOC | KVPOOL_DEV_SSD)) return fail(KVPOOL_EINVAL, "create: device %u unknown flags", i);
     if ((devs[i].flags & KVPOOL_DEV_HBM) && (devs[i].flags & ~KVPOOL_DEV_HBM)) return fail(KVPOOL_EINVAL, "create: device %u: KVPOOL_DEV_HBM excludes the host-memory flags", i);
+    if ((devs[i].flags & KVPOOL_DEV_SSD) && (devs[i].flags & ~KVPOOL_DEV_SSD)) return fail(KVPOOL_EINVAL, "create: device %u: KVPOOL_DEV_SSD excludes every other flag", i);
+    if ((devs[i].flags & KVPOOL_DEV_SSD) && (!devs[i].path || !*devs[i].path)) return fail(KVPOOL_EINVAL, "create: device %u: an SSD-type device needs a path", i);
+    if (!(devs[i].flags & KVPOOL_DEV_SSD) && (devs[i].path || devs[i].sector_bytes)) return fail(KVPOOL_EINVAL, "create: device %u: path / sector_bytes are for SSD-type devices", i);
+    if (devs[i].reserved) return fail(KVPOOL_EINVAL, "create: device %u: reserved must be 0", i);
     if (devs[i].numa_node < KVPOOL_NUMA_AUTO) return fail(KVPOOL_EINVAL, "create: device %u: numa_node %d", i, devs[i].numa_node);
   }
   if (!quantise_weights(bw.data(), n_devs, w.data())) return fail(KVPOOL_EINVAL, "create: bandwidth must be positive (>= 0.0005 GB/s)");
@@ -303,6 +310,7 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
   p->w = w;
   default_tuning(p.get());
   auto cleanup = [&]() {
+    ssd_close_all(p.get());
     for (auto& b : p->bufs) host_buffer_free(&b);
     for (auto s : p->own_streams) cudaStreamDestroy(s);
     if (p->table_arena) cudaFree(p->table_arena);
@@ -311,8 +319,16 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     if (p->join_out) cudaStreamDestroy(p->join_out);
   };
   p->bufs.resize(n_devs);
+  p->ssd.resize(n_devs);
   for (uint32_t i = 0; i < n_devs; ++i) {
     std::string err;
+    if (devs[i].flags & KVPOOL_DEV_SSD) {  // block storage: no buffer; LBAs are handed out in units of its sector size
+      const int rc = ssd_open(p.get(), i, devs[i]);
+      if (rc != KVPOOL_OK) { const std::string keep = last_error_message(); cleanup(); return fail(rc, "%s", keep.c_str()); }
+      p->bufs[i].bytes = p->ssd[i]->io.capacity();
+      p->alloc.emplace_back(p->bufs[i].bytes, std::max<uint64_t>(4096, p->ssd[i]->io.sector()));
+      continue;
+    }
     const bool hbm = devs[i].flags & KVPOOL_DEV_HBM;
     const int rc = hbm ? device_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes, devs[i].gpu < 0 ? cuda_device : devs[i].gpu, cuda_device, &err)
                        : host_buffer_alloc(&p->bufs[i], devs[i].capacity_bytes,
@@ -333,8 +349,8 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
   for (uint32_t i = 0; i < n_devs; ++i) {
     p->link_group[i] = devs[i].link_group;
     uint32_t first = i;
-    for (uint32_t j = 0; j < i && devs[i].link_group; ++j)
-      if (devs[j].link_group == devs[i].link_group) { first = j; break; }
+    for (uint32_t j = 0; j < i && devs[i].link_group && !is_ssd(p.get(), i); ++j)  // (an SSD-type device keeps streams of its own)
+      if (devs[j].link_group == devs[i].link_group && !is_ssd(p.get(), j)) { first = j; break; }
     if (first != i) { p->io[i] = p->io[first]; p->io_out[i] = p->io_out[first]; continue; }
     for (auto* v : {&p->io, &p->io_out}) {
       cudaError_t e = cudaStreamCreateWithFlags(&(*v)[i], cudaStreamNonBlocking);
@@ -365,6 +381,7 @@ int kvpool_destroy(kvpool_t* p) {
   cudaDeviceSynchronize();
   for (auto* pl : p->live) destroy_placement(p, pl);
   p->live.clear();
+  ssd_close_all(p);  // (after the device-wide synchronize above: every command has had the GPU's half)
   free_slots(p);
   for (auto s : p->own_streams) cudaStreamDestroy(s);
   for (auto& b : p->bufs) host_buffer_free(&b);
@@ -399,6 +416,7 @@ int kvpool_measure_bandwidth(kvpool_t* p, uint32_t dev, int direction, uint64_t 
     return fail(KVPOOL_EINVAL, "measure_bandwidth: bad arguments");
   if (bytes > p->bufs[dev].bytes) return fail(KVPOOL_EINVAL, "measure_bandwidth: %llu bytes exceed the pool buffer", (unsigned long long)bytes);
   if (!p->live.empty()) return fail(KVPOOL_ESTATE, "measure_bandwidth: %zu placements are live", p->live.size());
+  if (is_ssd(p, dev)) return ssd_measure(p, dev, direction == 1 || direction == KVPOOL_MEASURE_KERNEL_OFFLOAD, bytes, iters, gbps_out);
   DeviceGuard guard(p->cuda_device);
   struct Scratch {  // whatever the measurement allocates goes away on every return path
     void* buf = nullptr;
@@ -537,6 +555,13 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
   if (t->auto_threshold_bytes) d.auto_threshold_bytes = t->auto_threshold_bytes;
   if (t->group_bytes) d.group_bytes = t->group_bytes;
   if (t->stage_chunk_bytes) d.stage_chunk_bytes = t->stage_chunk_bytes == ~0ull ? 0 : t->stage_chunk_bytes;
+  if ((t->ssd_lanes && t->ssd_lanes != d.ssd_lanes) || (t->ssd_chunk_bytes && t->ssd_chunk_bytes != d.ssd_chunk_bytes)) {
+    if (t->ssd_lanes > 64) return fail(KVPOOL_EINVAL, "set_tuning: ssd_lanes must be <= 64");
+    for (auto& S : p->ssd)
+      if (S && S->n_lanes) return fail(KVPOOL_ESTATE, "set_tuning: ssd_lanes / ssd_chunk_bytes are fixed by the first kvpool_place");
+    if (t->ssd_lanes) d.ssd_lanes = t->ssd_lanes;
+    if (t->ssd_chunk_bytes) d.ssd_chunk_bytes = t->ssd_chunk_bytes;
+  }
   if (t->stage_slots && t->stage_slots != d.stage_slots) {
     DeviceGuard guard(p->cuda_device);
     d.stage_slots = t->stage_slots;
@@ -554,7 +579,7 @@ int kvpool_set_tuning(kvpool_t* p, const kvpool_tuning* t) {
 int kvpool_reserve_staging(kvpool_t* p, uint64_t bytes) {
   PoolLock lock__(p);
   if (!p) return fail(KVPOOL_EINVAL, "reserve_staging: null pool");
-  if (all_hbm(p)) return KVPOOL_OK;  // nothing is ever staged
+  if (!has_mem(p)) return KVPOOL_OK;  // nothing is ever staged (HBM-type stripes are reached in place, SSD-type devices have lanes)
   DeviceGuard guard(p->cuda_device);
   return ensure_slots(p, bytes + static_cast<uint64_t>(p->n) * 256 * (kMaxBatch + 1));
 }
@@ -595,7 +620,7 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
       m->order.resize(K);
       for (uint64_t j = 0; j < K; ++j) m->order[m->start[m->dev[j]] + m->slot[j]] = static_cast<uint32_t>(j);
       for (uint32_t i = 0; i < N; ++i)
-        if (!is_hbm(p, i)) m->host_blocks += m->counts[i];
+        if (is_mem(p, i)) m->host_blocks += m->counts[i];
       table_bytes += (2 + (p->hbm_mask && !all_hbm(p) ? 1 : 0)) * ((K * 4 + 255) / 256 * 256) + (K + 255) / 256 * 256;
       it = by_k.emplace(K, std::move(m)).first;
     }
@@ -609,15 +634,17 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
   // a4: stripe allocation, all or nothing.  Each pool device gets ONE contiguous region per placement in which the
   // layers' stripes follow each other in layer order (256-byte aligned), so that a run of consecutive layers is also
   // one contiguous span per device — what lets the batched calls move several small layers with one copy per device.
-  constexpr uint64_t kStripeAlign = 256;
+  // (on an SSD-type device a stripe is an LBA range: it starts on a sector boundary)
   pl->region_off.assign(N, 0);
   pl->region_bytes.assign(N, 0);
   for (uint32_t l = 0; l < L; ++l) {
     auto& Ls = pl->layers[l];
     Ls.stripe_off.assign(N, 0);
+    if (p->ssd_mask) { Ls.ssd_last_lane.assign(N, 0); Ls.ssd_last_use.assign(N, 0); }
     for (uint32_t i = 0; i < N; ++i) {
+      const uint64_t align = is_ssd(p, i) ? std::max<uint64_t>(256, p->ssd[i]->io.sector()) : 256;
       Ls.stripe_off[i] = pl->region_bytes[i];  // relative for now
-      pl->region_bytes[i] += (static_cast<uint64_t>(Ls.map->counts[i]) * p->payload + kStripeAlign - 1) / kStripeAlign * kStripeAlign;
+      pl->region_bytes[i] += (static_cast<uint64_t>(Ls.map->counts[i]) * p->payload + align - 1) / align * align;
     }
   }
   bool ok = true;
@@ -696,7 +723,11 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
     cudaError_t e = take_event(p, &Ls.landed);
     if (e != cudaSuccess) { rollback(); return fail(KVPOOL_ECUDA, "place: cudaEventCreate: %s", cudaGetErrorString(e)); }
   }
-  if (p->path != KVPOOL_PATH_ZEROCOPY && !all_hbm(p)) {
+  if (p->ssd_mask) {
+    const int rc = ssd_ensure_lanes(p);
+    if (rc != KVPOOL_OK) { rollback(); return rc; }
+  }
+  if ((p->path != KVPOOL_PATH_ZEROCOPY || p->ssd_mask) && has_mem(p)) {
     // a slot holds the largest layer, or a group of small layers (plus the 256-byte alignment gaps between stripes)
     const uint64_t total_bytes = std::accumulate(pl->region_bytes.begin(), pl->region_bytes.end(), uint64_t{0});
     const uint64_t group_cap = std::min<uint64_t>(std::max<uint64_t>(max_layer_bytes, p->tune.group_bytes), total_bytes);
@@ -716,9 +747,11 @@ int kvpool_release(kvpool_t* p, kvpool_placement_t* pl) {
   auto it = std::find(p->live.begin(), p->live.end(), pl);
   if (it == p->live.end()) return fail(KVPOOL_EINVAL, "release: placement does not belong to this pool");
   DeviceGuard guard(p->cuda_device);
-  const int rc = sync_pool_streams(p);  // the library's own transfers for it must be over
+  int rc = sync_pool_streams(p);  // the library's own transfers for it must be over
   if (rc != KVPOOL_OK) return rc;
   for (auto& u : pl->last_use) CU(cudaEventSynchronize(u.second));  // and so must the kernels it put on the caller's streams
+  rc = p->ssd_mask ? ssd_drain(p) : KVPOOL_OK;  // and the store commands of the SSD-type devices (a failed one: EIO, the placement stays)
+  if (rc != KVPOOL_OK) return rc;
   p->live.erase(it);
   destroy_placement(p, pl);
   return KVPOOL_OK;
@@ -762,9 +795,13 @@ int kvpool_lookup(const kvpool_placement_t* pl, uint32_t layer, uint32_t block, 
   if (block >= L.map->K) return fail(KVPOOL_EINVAL, "lookup: block %u out of range (K %llu)", block, (unsigned long long)L.map->K);
   const uint32_t d = L.map->dev[block], s = L.map->slot[block];
   if (device_id) *device_id = d;
-  if (type) *type = is_hbm(pl->pool, d) ? KVPOOL_TYPE_HBM : KVPOOL_TYPE_MEM;
+  if (type) *type = is_ssd(pl->pool, d) ? KVPOOL_TYPE_SSD : is_hbm(pl->pool, d) ? KVPOOL_TYPE_HBM : KVPOOL_TYPE_MEM;
   if (slot) *slot = s;
-  if (host_ptr) *host_ptr = pool_bytes(pl->pool, d) + L.stripe_off[d] + static_cast<uint64_t>(s) * pl->pool->payload;
+  if (host_ptr) {
+    if (is_ssd(pl->pool, d))  // Table I: location = LBA (of the sector the payload starts in; kvpool_ssd_location has the byte)
+      *host_ptr = reinterpret_cast<void*>(static_cast<uintptr_t>((L.stripe_off[d] + static_cast<uint64_t>(s) * pl->pool->payload) / pl->pool->ssd[d]->io.sector()));
+    else *host_ptr = pool_bytes(pl->pool, d) + L.stripe_off[d] + static_cast<uint64_t>(s) * pl->pool->payload;
+  }
   return KVPOOL_OK;
 }
 
@@ -772,7 +809,10 @@ int kvpool_stripe(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, vo
   if (!pl || layer >= pl->layers.size() || dev >= pl->pool->n) return fail(KVPOOL_EINVAL, "stripe: bad arguments");
   const LayerState& L = pl->layers[layer];
   const uint64_t bytes = static_cast<uint64_t>(L.map->counts[dev]) * pl->pool->payload;
-  if (host_ptr) *host_ptr = bytes ? pool_bytes(pl->pool, dev) + L.stripe_off[dev] : nullptr;
+  if (host_ptr) {
+    if (is_ssd(pl->pool, dev)) *host_ptr = reinterpret_cast<void*>(static_cast<uintptr_t>(L.stripe_off[dev] / pl->pool->ssd[dev]->io.sector()));  // first LBA
+    else *host_ptr = bytes ? pool_bytes(pl->pool, dev) + L.stripe_off[dev] : nullptr;
+  }
   if (nbytes) *nbytes = bytes;
   return KVPOOL_OK;
 }
@@ -785,6 +825,10 @@ int kvpool_stripe_read(kvpool_t* p, const kvpool_placement_t* pl, uint32_t layer
   if (nbytes > bytes) return fail(KVPOOL_EINVAL, "stripe_read: %llu bytes exceed the stripe's %llu", (unsigned long long)nbytes, (unsigned long long)bytes);
   if (nbytes == 0) return KVPOOL_OK;
   if (!dst_host) return fail(KVPOOL_EINVAL, "stripe_read: null destination");
+  if (is_ssd(p, dev)) {  // wait for the device's worker, then read the LBA range with plain preads
+    const int rc = ssd_drain(p);
+    return rc != KVPOOL_OK ? rc : ssd_read(p, dev, L.stripe_off[dev], dst_host, nbytes);
+  }
   const uint8_t* src = pool_bytes(p, dev) + L.stripe_off[dev];
   if (is_hbm(p, dev)) {
     DeviceGuard guard(p->cuda_device);
@@ -798,8 +842,49 @@ int kvpool_stripe_read(kvpool_t* p, const kvpool_placement_t* pl, uint32_t layer
 
 int kvpool_device_type(const kvpool_t* p, uint32_t dev, uint32_t* type, int32_t* gpu) {
   if (!p || dev >= p->n) return fail(KVPOOL_EINVAL, "device_type: bad arguments");
-  if (type) *type = is_hbm(p, dev) ? KVPOOL_TYPE_HBM : KVPOOL_TYPE_MEM;
+  if (type) *type = is_ssd(p, dev) ? KVPOOL_TYPE_SSD : is_hbm(p, dev) ? KVPOOL_TYPE_HBM : KVPOOL_TYPE_MEM;
   if (gpu) *gpu = p->bufs[dev].gpu;
+  return KVPOOL_OK;
+}
+
+int kvpool_plan_lba_range(uint64_t set_size, uint64_t kv_size, uint32_t sector_bytes, uint64_t* n_sectors_out) {
+  if (!n_sectors_out || !lba_range_len(set_size, kv_size, sector_bytes, n_sectors_out))
+    return fail(KVPOOL_EINVAL, "plan_lba_range: null output, zero sector size or a range beyond 2^64 sectors");
+  return KVPOOL_OK;
+}
+
+int kvpool_ssd_range(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, uint64_t* first_lba, uint64_t* n_sectors, uint32_t* sector_bytes) {
+  if (!pl || layer >= pl->layers.size() || dev >= pl->pool->n) return fail(KVPOOL_EINVAL, "ssd_range: bad arguments");
+  if (!is_ssd(pl->pool, dev)) return fail(KVPOOL_EINVAL, "ssd_range: pool device %u is not an SSD-type device", dev);
+  const LayerState& L = pl->layers[layer];
+  const uint32_t sec = pl->pool->ssd[dev]->io.sector();
+  if (first_lba) *first_lba = L.stripe_off[dev] / sec;
+  if (n_sectors) lba_range_len(L.map->counts[dev], pl->pool->payload, sec, n_sectors);
+  if (sector_bytes) *sector_bytes = sec;
+  return KVPOOL_OK;
+}
+
+int kvpool_ssd_location(const kvpool_placement_t* pl, uint32_t layer, uint32_t block, uint64_t* lba, uint32_t* byte_in_sector) {
+  if (!pl || layer >= pl->layers.size()) return fail(KVPOOL_EINVAL, "ssd_location: bad arguments");
+  const LayerState& L = pl->layers[layer];
+  if (block >= L.map->K) return fail(KVPOOL_EINVAL, "ssd_location: block %u out of range (K %llu)", block, (unsigned long long)L.map->K);
+  const uint32_t d = L.map->dev[block];
+  if (!is_ssd(pl->pool, d)) return fail(KVPOOL_EINVAL, "ssd_location: block %u lives on pool device %u, which is not an SSD-type device", block, d);
+  const uint64_t sec = pl->pool->ssd[d]->io.sector(), at = L.stripe_off[d] + static_cast<uint64_t>(L.map->slot[block]) * pl->pool->payload;
+  if (lba) *lba = at / sec;
+  if (byte_in_sector) *byte_in_sector = static_cast<uint32_t>(at % sec);
+  return KVPOOL_OK;
+}
+
+int kvpool_ssd_info(const kvpool_t* p, uint32_t dev, uint32_t* sector_bytes, int32_t* direct_io, int32_t* block_device, uint64_t* stores, uint64_t* retrieves) {
+  if (!p || dev >= p->n) return fail(KVPOOL_EINVAL, "ssd_info: bad arguments");
+  if (!is_ssd(p, dev)) return fail(KVPOOL_EINVAL, "ssd_info: pool device %u is not an SSD-type device", dev);
+  const SsdDevice& io = p->ssd[dev]->io;
+  if (sector_bytes) *sector_bytes = io.sector();
+  if (direct_io) *direct_io = io.direct();
+  if (block_device) *block_device = io.block_device();
+  if (stores) *stores = io.completed(1);
+  if (retrieves) *retrieves = io.completed(0);
   return KVPOOL_OK;
 }
 

@@ -127,6 +127,7 @@ static int naive_layer(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, bool
   int rc = check_layer_call(p, pl, layer, k_base, v_base, stride, table_host);
   if (rc != KVPOOL_OK) return rc;
   LayerState& L = pl->layers[layer];
+  if (p->ssd_mask) return fail(KVPOOL_EINVAL, "the per-block memcpy baseline has no SSD branch");
   if (!pack && !L.offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", layer);
   if (pack) { L.offloaded = true; L.have.clear(); }
   DeviceGuard guard(p->cuda_device);

@@ -20,6 +20,7 @@
 #include "kernels.cuh"
 #include "placement.hpp"
 #include "pool_mem.hpp"
+#include "ssd_io.hpp"
 
 static_assert(KVPOOL_MAX_DEVICES == kvp::kMaxDevices && KVPOOL_MAX_DEVICES == kvp::kMaxDev, "device limit mismatch");
 
@@ -80,6 +81,10 @@ struct LayerState {
   std::vector<uint64_t> have;        // else, once a partial offload has happened: bit j = logical block j is in the pool
   cudaEvent_t landed = nullptr;      // recorded when the layer's stripes are complete in the pool
   bool landed_pending = false;
+  // SSD-type devices: the store command that completes this layer's stripe on device i = use ssd_last_use[i] of offload
+  // lane ssd_last_lane[i] (bit i of ssd_stored says there is one); its completion is the worker's cpu_seq flag, not an event
+  uint32_t ssd_stored = 0;
+  std::vector<uint32_t> ssd_last_lane, ssd_last_use;
 };
 
 struct ProfRec {  // one profiled kernel launch
@@ -98,6 +103,29 @@ struct StageSlot {
                                               // unpack, so kernel_done alone covers them
   std::vector<cudaEvent_t> copy_done;         // [N] last memcpy per pool stream that read/wrote the slot
 };
+
+// One store / retrieve command in flight on an SSD-type device: pinned bounce memory for the disk's DMA, a device staging
+// piece of the same size for the pack / unpack kernel, and the events that recycle them.
+struct SsdLane {
+  uint8_t* bounce = nullptr;
+  uint8_t* stage = nullptr;
+  cudaEvent_t copy_done = nullptr;    // last copy between stage and bounce
+  cudaEvent_t kernel_done = nullptr;  // last kernel that read / wrote stage
+  uint32_t uses = 0;                  // sequence number of the lane's latest use (the value its flags are compared with)
+};
+struct SsdState {  // one SSD-type pool device (KV-passthrough)
+  SsdDevice io;
+  uint8_t* bounce_base = nullptr;  // pinned host memory: [direction][lane] x lane_bytes
+  uint8_t* stage_base = nullptr;   // device memory, same layout
+  uint32_t* flags = nullptr;       // pinned + mapped: per direction and lane, gpu_seq (written by a stream write-value, polled
+  uint64_t flags_dev = 0;          // by the worker) and cpu_seq (written by the worker, awaited by a stream wait-value)
+  uint64_t lane_bytes = 0;
+  uint32_t n_lanes = 0;
+  std::vector<SsdLane> lane[2];    // [0] retrieve (SSD -> GPU), [1] offload (GPU -> SSD)
+  uint32_t cursor[2] = {0, 0};
+  uint8_t* scratch = nullptr;      // aligned host memory for kvpool_stripe_read / kvpool_measure_bandwidth
+};
+constexpr uint64_t kSsdScratchBytes = 4ull << 20;
 
 }  // namespace kvp
 
@@ -144,6 +172,8 @@ struct kvpool {
   std::vector<kvp::HostBuffer> bufs;
   std::vector<uint32_t> link_group;  // [N] kvpool_device_desc.link_group: devices of one group share io / io_out streams
   std::vector<cudaStream_t> own_streams;  // every stream created for io / io_out, once (members of a group alias one)
+  uint32_t ssd_mask = 0;  // bit i: pool device i is block storage (KVPOOL_DEV_SSD): its share of a layer moves through bounce lanes
+  std::vector<std::unique_ptr<kvp::SsdState>> ssd;  // [N], null for the other types
   uint32_t hbm_mask = 0;  // bit i: pool device i is GPU memory (KVPOOL_DEV_HBM): reached by the kernels directly, never staged or copied
   std::vector<kvp::StripeAllocator> alloc;
   std::vector<cudaStream_t> io;      // one I/O stream per pool device ("independent I/O streams"): host -> GPU copies
@@ -209,6 +239,20 @@ inline bool is_hbm(const kvpool* p, uint32_t i) { return (p->hbm_mask >> i) & 1u
 inline uint8_t* pool_bytes(const kvpool* p, uint32_t i) {
   return static_cast<uint8_t*>(is_hbm(p, i) ? p->bufs[i].dev_alias : p->bufs[i].host);
 }
+inline bool is_ssd(const kvpool* p, uint32_t i) { return (p->ssd_mask >> i) & 1u; }
+inline bool is_mem(const kvpool* p, uint32_t i) { return !is_hbm(p, i) && !is_ssd(p, i); }
+inline bool has_mem(const kvpool* p) { return ((p->hbm_mask | p->ssd_mask) & (p->n >= 32 ? 0xFFFFFFFFu : (1u << p->n) - 1u)) != (p->n >= 32 ? 0xFFFFFFFFu : (1u << p->n) - 1u); }
+// kvpool_ssd.cu: SSD-type pool devices
+int ssd_open(kvpool* p, uint32_t i, const kvpool_device_desc& d);  // kvpool_create
+void ssd_close_all(kvpool* p);                                      // kvpool_destroy / failed create
+int ssd_ensure_lanes(kvpool* p);                                    // kvpool_place: bounce lanes, staging pieces, flags, workers
+// slots [lo, hi) of layer L's stripe on SSD device i, offload (pack) or retrieve, in lane-sized commands; `a` carries the
+// paged side of the launch (bases, stride, table)
+int ssd_move(kvpool* p, LayerState& L, uint32_t i, uint32_t lo, uint32_t hi, bool pack, LayerArgs a, cudaStream_t s);
+int ssd_wait_stored(kvpool* p, const LayerState& L, cudaStream_t s);  // `s` waits until the layer's store commands have completed
+int ssd_drain(kvpool* p);                                           // host waits for every worker; EIO if a command failed
+int ssd_read(kvpool* p, uint32_t i, uint64_t off, void* dst, uint64_t n);  // after ssd_drain
+int ssd_measure(kvpool* p, uint32_t i, bool write, uint64_t bytes, uint32_t iters, double* gbps);
 inline bool all_hbm(const kvpool* p) { return p->hbm_mask == (p->n >= 32 ? 0xFFFFFFFFu : (1u << p->n) - 1u); }
 
 }  // namespace kvp

@@ -1,0 +1,261 @@
+// libkvpool.so: SSD-type pool devices — KV-passthrough, GPU side.  DESIGN.md section 14.
+//
+// An SSD-type device's share of a layer moves in lane-sized commands, DEVICE-MAJOR (runs of consecutive slots of its
+// stripe = consecutive bytes of its LBA range, reached through the device's inverse map like the chunks of kvpool_xfer.cu):
+//
+//   store    (Alg. 1 l.20-21, SSD_Direct_Store):    pack kernel -> lane.stage (HBM) -> D2H copy -> lane.bounce (pinned)
+//                                                    -> the device's worker writes the LBA range (ssd_io.cpp)
+//   retrieve (SSD_Direct_Retrieve):   worker reads the LBA range -> lane.bounce -> H2D copy -> lane.stage
+//                                                    -> unpack kernel
+//
+// The GPU streams and the worker never synchronise with the host: each lane and direction has two 32-bit sequence flags in
+// mapped pinned memory — gpu_seq, raised by a stream write-value behind the lane's copy, and cpu_seq, raised by the worker
+// behind its pread / pwrite — and each side waits for the other with a stream wait-value / a poll.  The API call only
+// enqueues: stream operations on the GPU side, one command on the worker's queue.
+#include "kvpool_internal.hpp"
+
+namespace kvp {
+namespace {
+
+// cuStreamWaitValue32 / cuStreamWriteValue32 (driver API), reached through the runtime's entry-point query so that the
+// library links against cudart only.  CUstream = cudaStream_t, CUdeviceptr = unsigned long long, CUresult 0 = success.
+using MemOpFn = int (*)(cudaStream_t, unsigned long long, unsigned int, unsigned int);
+MemOpFn g_wait_value = nullptr, g_write_value = nullptr;
+constexpr unsigned int kWaitGeq = 0x0, kWriteDefault = 0x0;  // CU_STREAM_WAIT_VALUE_GEQ (wrap-aware), CU_STREAM_WRITE_VALUE_DEFAULT (fenced)
+
+int memops_init() {
+  if (g_wait_value && g_write_value) return KVPOOL_OK;
+  void *w = nullptr, *r = nullptr;
+  cudaDriverEntryPointQueryResult qw, qr;
+  CU(cudaGetDriverEntryPointByVersion("cuStreamWaitValue32", &w, 12000, cudaEnableDefault, &qw));
+  CU(cudaGetDriverEntryPointByVersion("cuStreamWriteValue32", &r, 12000, cudaEnableDefault, &qr));
+  if (!w || !r || qw != cudaDriverEntryPointSuccess || qr != cudaDriverEntryPointSuccess)
+    return fail(KVPOOL_ECUDA, "this driver has no stream memory operations (cuStreamWaitValue32 / cuStreamWriteValue32)");
+  g_wait_value = reinterpret_cast<MemOpFn>(w);
+  g_write_value = reinterpret_cast<MemOpFn>(r);
+  return KVPOOL_OK;
+}
+
+#define DRV(call)                                                                         \
+  do {                                                                                    \
+    const int r__ = (call);                                                               \
+    if (r__ != 0) return fail(KVPOOL_ECUDA, "%s: driver error %d", #call, r__);           \
+  } while (0)
+
+// Flags of lane k, direction d: 32 words per lane (gpu_seq at word 0, cpu_seq at word 16: separate cache lines).
+constexpr uint32_t kFlagStride = 32;
+inline uint32_t flag_word(const SsdState& S, int d, uint32_t lane, bool cpu) { return (static_cast<uint32_t>(d) * S.n_lanes + lane) * kFlagStride + (cpu ? 16u : 0u); }
+inline unsigned long long flag_dev(const SsdState& S, int d, uint32_t lane, bool cpu) { return S.flags_dev + 4ull * flag_word(S, d, lane, cpu); }
+
+void free_lanes(SsdState& S) {
+  S.io.stop();
+  for (auto& v : S.lane) {
+    for (auto& ln : v) {
+      if (ln.copy_done) cudaEventDestroy(ln.copy_done);
+      if (ln.kernel_done) cudaEventDestroy(ln.kernel_done);
+    }
+    v.clear();
+  }
+  if (S.bounce_base) cudaFreeHost(S.bounce_base);
+  if (S.stage_base) cudaFree(S.stage_base);
+  if (S.flags) cudaFreeHost(S.flags);
+  S.bounce_base = S.stage_base = nullptr;
+  S.flags = nullptr;
+  S.n_lanes = 0;
+}
+
+uint64_t gcd64(uint64_t a, uint64_t b) {
+  while (b) { const uint64_t t = a % b; a = b; b = t; }
+  return a;
+}
+
+}  // namespace
+
+int ssd_open(kvpool* p, uint32_t i, const kvpool_device_desc& d) {
+  int rc = memops_init();
+  if (rc != KVPOOL_OK) return rc;
+  std::unique_ptr<SsdState> S(new SsdState);
+  std::string err;
+  rc = S->io.open(d.path, d.capacity_bytes, d.sector_bytes, &err);
+  if (rc != KVPOOL_OK) return fail(rc, "create: pool device %u: %s", i, err.c_str());
+  S->scratch = static_cast<uint8_t*>(aligned_alloc(4096, kSsdScratchBytes));
+  if (!S->scratch) return fail(KVPOOL_ENOMEM, "create: pool device %u: out of memory", i);
+  p->ssd[i] = std::move(S);
+  p->ssd_mask |= 1u << i;
+  return KVPOOL_OK;
+}
+
+void ssd_close_all(kvpool* p) {
+  for (auto& S : p->ssd) {
+    if (!S) continue;
+    free_lanes(*S);
+    S->io.close();
+    free(S->scratch);
+    S.reset();
+  }
+  p->ssd_mask = 0;
+}
+
+int ssd_ensure_lanes(kvpool* p) {
+  for (uint32_t i = 0; i < p->n; ++i) {
+    if (!is_ssd(p, i)) continue;
+    SsdState& S = *p->ssd[i];
+    if (S.n_lanes) continue;
+    const uint64_t sec = S.io.sector();
+    // a command carries at least one KV cache, displaced by up to a sector and rounded up to one
+    const uint64_t least = (p->payload + sec - 1) / sec * sec + 2 * sec;
+    S.lane_bytes = (std::max<uint64_t>(p->tune.ssd_chunk_bytes, least) + 4095) / 4096 * 4096;
+    const uint32_t n = std::max<uint32_t>(p->tune.ssd_lanes, 1);
+    const uint64_t total = 2ull * n * S.lane_bytes;
+    cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&S.bounce_base), total, cudaHostAllocPortable);
+    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&S.stage_base), total);
+    if (e == cudaSuccess) e = cudaHostAlloc(reinterpret_cast<void**>(&S.flags), 2ull * n * kFlagStride * 4, cudaHostAllocMapped | cudaHostAllocPortable);
+    void* fd = nullptr;
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer(&fd, S.flags, 0);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      free_lanes(S);
+      return fail(KVPOOL_ENOMEM, "place: bounce lanes of SSD-type device %u (%llu bytes pinned + as many on the GPU): %s", i, (unsigned long long)total, cudaGetErrorString(e));
+    }
+    memset(S.flags, 0, 2ull * n * kFlagStride * 4);
+    S.flags_dev = reinterpret_cast<uint64_t>(fd);
+    S.n_lanes = n;
+    for (int d = 0; d < 2; ++d) {
+      S.lane[d].resize(n);
+      for (uint32_t k = 0; k < n; ++k) {
+        SsdLane& ln = S.lane[d][k];
+        ln.bounce = S.bounce_base + (static_cast<uint64_t>(d) * n + k) * S.lane_bytes;
+        ln.stage = S.stage_base + (static_cast<uint64_t>(d) * n + k) * S.lane_bytes;
+        CU(cudaEventCreateWithFlags(&ln.copy_done, cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&ln.kernel_done, cudaEventDisableTiming));
+      }
+    }
+    uint8_t* const bounce[2] = {S.lane[0][0].bounce, S.lane[1][0].bounce};
+    volatile uint32_t* const gpu[2] = {S.flags + flag_word(S, 0, 0, false), S.flags + flag_word(S, 1, 0, false)};
+    volatile uint32_t* const cpu[2] = {S.flags + flag_word(S, 0, 0, true), S.flags + flag_word(S, 1, 0, true)};
+    S.io.start(n, S.lane_bytes, bounce, gpu, cpu, kFlagStride);
+  }
+  return KVPOOL_OK;
+}
+
+int ssd_move(kvpool* p, LayerState& L, uint32_t i, uint32_t lo, uint32_t hi, bool pack, LayerArgs a, cudaStream_t s) {
+  SsdState& S = *p->ssd[i];
+  if (!S.n_lanes) return fail(KVPOOL_ESTATE, "SSD-type device %u has no bounce lanes", i);
+  const uint64_t P = p->payload, sec = S.io.sector();
+  const int d = pack ? 1 : 0;
+  cudaStream_t io = pack ? p->io_out[i] : p->io[i];
+  const uint64_t unit = sec / gcd64(P, sec);  // every `unit` KV caches the stripe is back on a sector boundary
+  a.order = L.map->order_d;
+  a.visit = nullptr;
+  for (uint32_t x = lo; x < hi;) {
+    const uint64_t byte0 = L.stripe_off[i] + static_cast<uint64_t>(x) * P;
+    const uint64_t at = byte0 / sec * sec;
+    const uint32_t head = static_cast<uint32_t>(byte0 - at);
+    uint32_t n = static_cast<uint32_t>(std::min<uint64_t>(hi - x, (S.lane_bytes - sec - head) / P));
+    if (unit > 1 && x + n < hi) {  // ragged KV size: end the command on a sector boundary when one is within reach
+      const uint64_t end = (static_cast<uint64_t>(x) + n) / unit * unit;
+      if (end > x) n = static_cast<uint32_t>(end - x);
+    }
+    const uint32_t k = S.cursor[d]++ % S.n_lanes;
+    SsdLane& ln = S.lane[d][k];
+    const uint32_t u = ++ln.uses;
+    const uint64_t bytes = static_cast<uint64_t>(n) * P;
+    a.j0 = L.map->start[i] + x;
+    a.K = n;
+    a.pool_base[0] = reinterpret_cast<uint64_t>(ln.stage);
+    // If enqueueing fails half way, both flags of this use are raised from the host so that no later use of the lane
+    // (and no worker) waits for a hand-over that will never come.
+    auto abandon = [&](int rc) {
+      __atomic_store_n(S.flags + flag_word(S, d, k, false), u, __ATOMIC_RELEASE);
+      __atomic_store_n(S.flags + flag_word(S, d, k, true), u, __ATOMIC_RELEASE);
+      return rc;
+    };
+    auto cu = [&](cudaError_t e, const char* what) { return e == cudaSuccess ? KVPOOL_OK : fail(KVPOOL_ECUDA, "%s: %s", what, cudaGetErrorString(e)); };
+    int rc;
+    if (pack) {
+      // SSD_Direct_Store: gather into the lane's staging piece, copy it out to the bounce memory once the lane's previous
+      // command has been written (cpu_seq >= u-1), tell the worker (gpu_seq = u); the worker writes the LBA range
+      if ((rc = cu(cudaStreamWaitEvent(s, ln.copy_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
+      if ((rc = launch_counted(p, a, true, false, s)) != KVPOOL_OK) return abandon(rc);
+      if ((rc = cu(cudaEventRecord(ln.kernel_done, s), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
+      if ((rc = cu(cudaStreamWaitEvent(io, ln.kernel_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
+      if (g_wait_value(io, flag_dev(S, d, k, true), u - 1, kWaitGeq) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed"));
+      if ((rc = cu(cudaMemcpyAsync(ln.bounce + head, ln.stage, bytes, cudaMemcpyDeviceToHost, io), "cudaMemcpyAsync")) != KVPOOL_OK) return abandon(rc);
+      p->n_memcpys++;
+      if (g_write_value(io, flag_dev(S, d, k, false), u, kWriteDefault) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed"));
+      if ((rc = cu(cudaEventRecord(ln.copy_done, io), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
+      S.io.submit(SsdCmd{SsdCmd::kWrite, x + n == L.map->counts[i], k, u, at, head, bytes});
+      L.ssd_last_lane[i] = k;
+      L.ssd_last_use[i] = u;
+      L.ssd_stored |= 1u << i;
+    } else {
+      // SSD_Direct_Retrieve: the worker reads the LBA range into the bounce memory once the lane's previous command has
+      // been drained (gpu_seq >= u-1) and raises cpu_seq = u; the copy waits for that, the unpack for the copy
+      S.io.submit(SsdCmd{SsdCmd::kRead, false, k, u, at, head, bytes});
+      if (g_wait_value(io, flag_dev(S, d, k, true), u, kWaitGeq) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed"));
+      if ((rc = cu(cudaStreamWaitEvent(io, ln.kernel_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
+      if ((rc = cu(cudaMemcpyAsync(ln.stage, ln.bounce + head, bytes, cudaMemcpyHostToDevice, io), "cudaMemcpyAsync")) != KVPOOL_OK) return abandon(rc);
+      p->n_memcpys++;
+      if (g_write_value(io, flag_dev(S, d, k, false), u, kWriteDefault) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed"));
+      if ((rc = cu(cudaEventRecord(ln.copy_done, io), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
+      if ((rc = cu(cudaStreamWaitEvent(s, ln.copy_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return rc;
+      if ((rc = launch_counted(p, a, false, false, s)) != KVPOOL_OK) return rc;
+      if ((rc = cu(cudaEventRecord(ln.kernel_done, s), "cudaEventRecord")) != KVPOOL_OK) return rc;
+    }
+    x += n;
+  }
+  return KVPOOL_OK;
+}
+
+int ssd_wait_stored(kvpool* p, const LayerState& L, cudaStream_t s) {
+  for (uint32_t i = 0; i < p->n; ++i) {
+    if (!(L.ssd_stored >> i & 1u)) continue;
+    const SsdState& S = *p->ssd[i];
+    if (seq_reached(S.flags + flag_word(S, 1, L.ssd_last_lane[i], true), L.ssd_last_use[i])) continue;  // already on the disk
+    DRV(g_wait_value(s, flag_dev(S, 1, L.ssd_last_lane[i], true), L.ssd_last_use[i], kWaitGeq));
+  }
+  return KVPOOL_OK;
+}
+
+int ssd_drain(kvpool* p) {
+  int err = 0;
+  for (auto& S : p->ssd) {
+    if (!S) continue;
+    if (S->io.running()) S->io.drain();
+    const int e = S->io.take_error();
+    if (e && !err) err = e;
+  }
+  return err ? fail(KVPOOL_EIO, "an SSD-type pool device failed a store / retrieve command: %s", strerror(err)) : KVPOOL_OK;
+}
+
+int ssd_read(kvpool* p, uint32_t i, uint64_t off, void* dst, uint64_t n) {
+  SsdState& S = *p->ssd[i];
+  const int e = S.io.read_bytes(off, dst, n, S.scratch, kSsdScratchBytes);
+  return e ? fail(KVPOOL_EIO, "read of SSD-type device %u: %s", i, strerror(e)) : KVPOOL_OK;
+}
+
+// "Measured bandwidth" of an SSD-type device: sequential commands of the scratch size over the first
+// `bytes` of the device, on the calling thread, median of `iters` passes by the host's clock.  The region is written
+// once first, so that a sparse stand-in file has its blocks.  The disk side only: the PCIe hop of a lane overlaps it.
+int ssd_measure(kvpool* p, uint32_t i, bool write, uint64_t bytes, uint32_t iters, double* gbps) {
+  SsdState& S = *p->ssd[i];
+  const uint64_t sec = S.io.sector();
+  bytes = bytes / sec * sec;
+  if (bytes == 0) return fail(KVPOOL_EINVAL, "measure_bandwidth: fewer bytes than one sector");
+  memset(S.scratch, 0x5a, kSsdScratchBytes);
+  int e = S.io.io_span(true, 0, bytes, S.scratch, kSsdScratchBytes);
+  std::vector<double> sec_s(iters);
+  for (uint32_t it = 0; it < iters && !e; ++it) {
+    timespec t0, t1;
+    clock_gettime(CLOCK_MONOTONIC, &t0);
+    e = S.io.io_span(write, 0, bytes, S.scratch, kSsdScratchBytes);
+    clock_gettime(CLOCK_MONOTONIC, &t1);
+    sec_s[it] = (t1.tv_sec - t0.tv_sec) + 1e-9 * (t1.tv_nsec - t0.tv_nsec);
+  }
+  if (e) return fail(KVPOOL_EIO, "measure_bandwidth: SSD-type device %u: %s", i, strerror(e));
+  std::sort(sec_s.begin(), sec_s.end());
+  *gbps = static_cast<double>(bytes) / (sec_s[iters / 2] * 1.0e9);
+  return KVPOOL_OK;
+}
+
+}  // namespace kvp

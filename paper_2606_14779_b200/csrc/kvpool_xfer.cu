@@ -48,7 +48,7 @@ struct ChunkPlan {
   uint32_t lo[KVPOOL_MAX_DEVICES], hi[KVPOOL_MAX_DEVICES];
   uint64_t off[KVPOOL_MAX_DEVICES];  // byte offset of device i's share inside the slot
   uint64_t host_bytes = 0;           // what the chunk moves to / from host-memory devices
-  bool host_blocks = false, hbm_blocks = false;
+  bool host_blocks = false, hbm_blocks = false, ssd_blocks = false;
 };
 static ChunkPlan plan_chunk(const kvpool* p, const LayerState& L, uint32_t first, uint32_t n) {
   ChunkPlan c;
@@ -58,6 +58,7 @@ static ChunkPlan plan_chunk(const kvpool* p, const LayerState& L, uint32_t first
     c.off[i] = acc;
     if (c.hi[i] == c.lo[i]) continue;
     if (is_hbm(p, i)) { c.hbm_blocks = true; continue; }
+    if (is_ssd(p, i)) { c.ssd_blocks = true; continue; }  // through the device's bounce lanes, never through a staging slot
     c.host_blocks = true;
     acc += static_cast<uint64_t>(c.hi[i] - c.lo[i]) * p->payload;
   }
@@ -118,19 +119,24 @@ int kvpool_offload_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, ui
   // staged: pack kernel -> device staging slot, then one D2H copy per device on the per-device I/O streams; `stream` is
   // released as soon as the last pack is enqueued.  A layer larger than a slot travels in chunks of logical blocks.
   const uint64_t per_slot = p->slots.empty() ? 0 : blocks_per_slot(p);
-  if (per_slot == 0) return fail(KVPOOL_ESTATE, "offload: no staging slot (the placement was made while the path was zero-copy)");
+  if (per_slot == 0 && whole.host_blocks) return fail(KVPOOL_ESTATE, "offload: no staging slot (the placement was made while the path was zero-copy)");
   // `landed` must mean "all stripes complete": it is recorded on a stream of the pool's own that carries no copies and only
   // gathers every chunk's kernel and copies — the per-device I/O streams never wait for one another
   cudaStream_t lead = p->join_out;
   if (L.landed_pending) CU(cudaStreamWaitEvent(lead, L.landed, 0));  // `landed` keeps covering what was offloaded before
   // an earlier offload of this layer may still be writing the HBM-type stripes the kernel stores into
   if (whole.hbm_blocks && L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
-  if (n_blocks > per_slot) {
+  if (n_blocks > per_slot || p->ssd_mask) {
     // DEVICE-MAJOR chunks: a chunk is a run of consecutive slots of one device's stripe, gathered by a launch that finds its
     // logical blocks through that device's inverse map, and leaves the slot as ONE copy.  An HBM-type device's share is
-    // gathered in place by one launch.
+    // gathered in place by one launch; an SSD-type device's share goes through that device's bounce lanes (SSD_Direct_Store,
+    // Alg. 1 l.20-21), which is why a pool with such a device always moves device-major.
     a.order = L.map->order_d;
     for (uint32_t i = 0; i < N; ++i) {
+      if (is_ssd(p, i)) {
+        if (whole.hi[i] > whole.lo[i] && (rc = ssd_move(p, L, i, whole.lo[i], whole.hi[i], true, a, s)) != KVPOOL_OK) return rc;
+        continue;
+      }
       for (uint32_t lo = whole.lo[i]; lo < whole.hi[i];) {
         const uint32_t n = is_hbm(p, i) ? whole.hi[i] - lo : static_cast<uint32_t>(std::min<uint64_t>(per_slot, whole.hi[i] - lo));
         a.j0 = L.map->start[i] + lo;
@@ -248,13 +254,18 @@ int kvpool_retrieve_range(kvpool_t* p, kvpool_placement_t* pl, uint32_t layer, u
   // ahead of `stream` — then the unpack kernel on `stream` once all of them have landed in the staging slot.  A range
   // larger than a slot travels in chunks of logical blocks: the copies of chunk c+1 overlap the unpack of chunk c.
   const uint64_t per_slot = p->slots.empty() ? 0 : blocks_per_slot(p);
-  if (per_slot == 0) return fail(KVPOOL_ESTATE, "retrieve: no staging slot (the placement was made while the path was zero-copy)");
+  if (per_slot == 0 && whole.host_blocks) return fail(KVPOOL_ESTATE, "retrieve: no staging slot (the placement was made while the path was zero-copy)");
   if (whole.hbm_blocks && L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));  // HBM-type stripes are read in place
-  if (n_blocks > per_slot) {
+  if (n_blocks > per_slot || p->ssd_mask) {
     // DEVICE-MAJOR chunks (see kvpool_offload_range): one copy fills a slot with a run of one device's slots, one launch
-    // scatters them through that device's inverse map; the copy of the next chunk overlaps it
+    // scatters them through that device's inverse map; the copy of the next chunk overlaps it.  SSD-type devices first: their
+    // retrieve commands (SSD_Direct_Retrieve) go to the workers before anything is enqueued for the faster
+    // devices, so that the disks read while the link moves the host-memory devices' share.
     a.order = L.map->order_d;
+    for (uint32_t i = 0; i < N; ++i)
+      if (is_ssd(p, i) && whole.hi[i] > whole.lo[i] && (rc = ssd_move(p, L, i, whole.lo[i], whole.hi[i], false, a, s)) != KVPOOL_OK) return rc;
     for (uint32_t i = 0; i < N; ++i) {
+      if (is_ssd(p, i)) continue;
       for (uint32_t lo = whole.lo[i]; lo < whole.hi[i];) {
         const uint32_t n = is_hbm(p, i) ? whole.hi[i] - lo : static_cast<uint32_t>(std::min<uint64_t>(per_slot, whole.hi[i] - lo));
         a.j0 = L.map->start[i] + lo;
@@ -391,6 +402,7 @@ int issue_zero_copy_group(const BatchCall& c, const LayerGroup& g) {
 // not fit a staging slot (the caller then falls back to per-layer calls).
 int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   kvpool* p = c.p;
+  if (p->ssd_mask) return 1;  // a pool with an SSD-type device moves layer by layer, device-major
   const uint32_t N = p->n;
   const std::vector<cudaStream_t>& ios = c.pack ? p->io_out : p->io;  // the copy streams of this direction
   const LayerState& A = c.pl->layers[c.first + g.q[0]];
@@ -635,8 +647,13 @@ int kvpool_wait_offloads(kvpool_t* p, kvpool_placement_t* pl, void* cuda_stream)
   if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "wait_offloads: bad arguments");
   DeviceGuard guard(p->cuda_device);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  for (auto& L : pl->layers)
+  for (auto& L : pl->layers) {
     if (L.landed_pending) CU(cudaStreamWaitEvent(s, L.landed, 0));
+    if (L.ssd_stored) {  // the store commands of SSD-type devices complete on their workers: wait for the flags they raise
+      const int rc = ssd_wait_stored(p, L, s);
+      if (rc != KVPOOL_OK) return rc;
+    }
+  }
   return KVPOOL_OK;
 }
 
@@ -644,7 +661,8 @@ int kvpool_synchronize(kvpool_t* p) {
   PoolLock lock__(p);
   if (!p) return fail(KVPOOL_EINVAL, "synchronize: null pool");
   DeviceGuard guard(p->cuda_device);
-  const int rc = sync_pool_streams(p);
+  int rc = sync_pool_streams(p);
+  if (rc == KVPOOL_OK && p->ssd_mask) rc = ssd_drain(p);  // and the workers of the SSD-type devices; EIO if a command failed
   if (rc != KVPOOL_OK) return rc;
   // offloads that have landed by now need no stream waits any more: later calls on those layers enqueue nothing but
   // their own work (which is what makes a zero-copy retrieve capturable into a CUDA graph)

@@ -22,7 +22,7 @@ extern int cudaDeviceSynchronize(void);
 
 static int gpu_round_trip(void) {
     enum { NPHYS = 96, K0 = 64, K1 = 3, KVB = 16 * 2 * 64 * 2, PLANE = NPHYS * KVB };
-    kvpool_device_desc d[2] = {{2.0, 8u << 20, -1, 0, -1, 0}, {1.0, 8u << 20, -1, KVPOOL_DEV_HBM, -1, 0}};
+    kvpool_device_desc d[2] = {{2.0, 8u << 20, -1, 0, -1, 0, NULL, 0, 0}, {1.0, 8u << 20, -1, KVPOOL_DEV_HBM, -1, 0, NULL, 0, 0}};
     kvpool_geometry g = {2, 16, 2, 64, 2};
     kvpool_t *pool = NULL;
     kvpool_placement_t *pl = NULL;

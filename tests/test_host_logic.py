@@ -207,3 +207,24 @@ def test_stripe_allocator_against_a_page_bitmap_model(tmp_path):
                     os.path.join(ROOT, "paper_2606_14779_b200", "csrc", "placement.cpp"), "-o", exe], check=True)
     out = subprocess.run([exe], capture_output=True, text=True)
     assert out.returncode == 0 and out.stdout.strip() == "stripe allocator ok", out.stdout
+
+
+def test_plan_lba_range_matches_oracle_and_rejects_bad_arguments(golden_dir):
+    """KV-passthrough's range length as the library computes it against the oracle's, on the hand-worked rows
+    and on random sizes up to products beyond 2^64."""
+    with open(os.path.join(golden_dir, "worked_lba_ranges.txt")) as f:
+        rows = [[c.strip() for c in ln.split("|")] for ln in f if ln.strip() and not ln.startswith("#")]
+    for n, kvs, sec, want, _ in rows:
+        assert kv.kvpool_plan_lba_range(int(n), int(kvs), int(sec)) == int(want) == oracle.lba_range_len(int(n), int(kvs), int(sec))
+    rng = np.random.default_rng(31)
+    for _ in range(3000):
+        n, kvs = int(rng.integers(0, 2 ** 33)), int(rng.integers(1, 2 ** 31))
+        sec = int(rng.choice([512, 1024, 4096, 65536, 520, 1, 3]))
+        assert kv.kvpool_plan_lba_range(n, kvs, sec) == oracle.lba_range_len(n, kvs, sec)
+    assert kv.kvpool_plan_lba_range(2 ** 40, 2 ** 30, 4096) == 2 ** 58          # the product does not fit 64 bits, the result does
+    with pytest.raises(kv.KvPoolError) as e:
+        kv.kvpool_plan_lba_range(1, 1, 0)
+    assert e.value.code == kv.EINVAL
+    with pytest.raises(kv.KvPoolError) as e:                                     # more than 2^64 sectors
+        kv.kvpool_plan_lba_range(2 ** 63, 2 ** 63, 1)
+    assert e.value.code == kv.EINVAL
