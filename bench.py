@@ -75,6 +75,10 @@ def parse_args():
     ap.add_argument("--mixed-pool", action="store_true",
                     help="HBM-type pool devices (KVPOOL_DEV_HBM; the pool's own GPU standing in for an NVLink peer) next to a pinned "
                          "host device: bandwidth-proportional split by measured weights, offload / retrieve GB/s (DESIGN.md §11)")
+    ap.add_argument("--ssd-pool", action="store_true",
+                    help="side mode: pools with SSD-type devices (KV-passthrough, PAPER.md:179-185) - files under --ssd-dir opened O_DIRECT stand in "
+                         "for NVMe namespaces: one SSD alone, host memory + one SSD, host memory + two SSDs (the paper's mix); text table")
+    ap.add_argument("--ssd-dir", default="/dev/shm", help="--ssd-pool: directory that holds the stand-in files (or pass block devices, comma separated)")
     ap.add_argument("--duplex", action="store_true",
                     help="offload of one request concurrent with retrieve of another (PCIe is full duplex): per-direction and aggregate "
                          "GB/s against simultaneous cudaMemcpyAsync in both directions")
@@ -1104,6 +1108,89 @@ def run_mixed_pool(args) -> None:
         pool.destroy()
 
 
+def run_ssd_pool(args) -> None:
+    """Unified pooling over host memory AND block storage: Eq. 1-2 split every layer between a pinned
+    host buffer and one or two SSD-type devices in proportion to kvpool_calibrate's figures (cudaMemcpyAsync for the host
+    buffer, the device's own sequential commands for an SSD; all devices name one link group because every byte crosses this
+    GPU's single PCIe link).  Whole request (8 layers of --config), batched calls, legs timed apart with CUDA events on the
+    caller's stream — the offload leg ends when kvpool_wait_offloads lets the stream go, i.e. when the store commands are on
+    the disk; every run is verified bit-exact against the source.  Text table on stdout."""
+    import torch
+    from paper_2606_14779_b200 import binding as kv
+    from paper_2606_14779_b200 import workloads as W
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    L = 8
+    wl = W.make_workload(args.config, n_layers=L)
+    wl.sliding_layers = ()
+    g = wl.geom
+    bpl = wl.blocks_per_layer(0)
+    K, moved = int(bpl[0]), int(bpl.sum()) * g.payload
+    elems = g.kvb // 2
+    src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+    dst = [W.poison_torch((2, wl.nphys, elems), dev) for l in range(L)]
+    tables = [torch.from_numpy(np.ascontiguousarray(wl.layer_table(0, l))).to(dev) for l in range(L)]
+    src_k, src_v, dst_k, dst_v = [x[0] for x in src], [x[1] for x in src], [x[0] for x in dst], [x[1] for x in dst]
+    s = torch.cuda.Stream(device=dev)
+    torch.cuda.synchronize()
+    cap = (moved + (L + 4) * (g.payload + 65536) + 65535) // 65536 * 65536
+    given = [x for x in args.ssd_dir.split(",") if x]
+    blockdevs = all(os.path.exists(x) and not os.path.isdir(x) for x in given)
+    print(f"# bench.py --ssd-pool --config {args.config} --ssd-dir {args.ssd_dir}: {wl.name} cut to {L} layers, {moved / 2**20:.0f} MiB per leg ({K} blocks of "
+          f"{g.payload} B per layer); SSD-type devices = {'the block devices given' if blockdevs else 'files under ' + given[0] + ' opened O_DIRECT (no NVMe on this box)'}; "
+          "weights = kvpool_calibrate (256 MiB per device, one link group); median of 3; 8 MiB commands on 4 lanes per device and direction")
+    print(f"{'pool':30s} {'weights (GB/s)':>20s} {'blocks per layer':>18s} {'offload GB/s':>12s} {'retrieve GB/s':>13s} {'sum of weights':>14s} {'of sum':>11s} {'stores':>7s} {'retrieves':>9s} {'direct':>6s}   (stores / retrieves: commands per leg)")
+    for name, types in (("1 host buffer", "m"), ("1 SSD", "s"), ("1 host buffer + 1 SSD", "ms"), ("1 host buffer + 2 SSDs", "mss")):
+        n = len(types)
+        n_ssd = types.count("s")
+        if blockdevs and n_ssd > len(given):
+            continue
+        paths, k = [], 0
+        for t in types:
+            paths.append(None if t == "m" else (given[k] if blockdevs else os.path.join(given[0], f"kvpool_ssd_{os.getpid()}_{k}.img")))
+            k += t == "s"
+        pool = kv.KvPool([1.0] * n, [cap] * n, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim,
+                         dev_flags=[kv.DEV_SSD if t == "s" else 0 for t in types], link_groups=[1] * n, paths=paths)
+        try:
+            bw = list(pool.calibrate(kv.MEASURE_RETRIEVE, 256 << 20, 5))
+            ssds = [i for i, t in enumerate(types) if t == "s"]
+            before = [pool.ssd_info(i) for i in ssds]                      # (the calibration's own commands are not the request's)
+            offs, rets = [], []
+            for it in range(4):
+                for d in dst:
+                    d.fill_(np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item())
+                pl = pool.place(bpl)
+                counts = list(pl.counts(0))
+                torch.cuda.synchronize()
+                ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+                ev[0].record(s)
+                pool.offload_layers(pl, 0, src_k, src_v, g.kvb, tables, s)
+                pool.wait_offloads(pl, s)
+                ev[1].record(s)
+                s.synchronize()
+                pool.synchronize()
+                ev[2].record(s)
+                pool.retrieve_layers(pl, 0, dst_k, dst_v, g.kvb, tables, s)
+                ev[3].record(s)
+                s.synchronize()
+                pl.release()
+                if it > 0:
+                    offs.append(ev[0].elapsed_time(ev[1]))
+                    rets.append(ev[2].elapsed_time(ev[3]))
+            for l in range(L):
+                if not torch.equal(dst[l][:, tables[l].long()], src[l][:, tables[l].long()]):
+                    raise RuntimeError(f"{name}: retrieved KV differs from the source")
+            o, r = moved / statistics.median(offs) / 1e6, moved / statistics.median(rets) / 1e6
+            infos = [pool.ssd_info(i) for i in ssds]
+            print(f"{name:30s} {'/'.join(f'{b:.1f}' for b in bw):>20s} {'/'.join(str(c) for c in counts):>18s} {o:12.2f} {r:13.2f} {sum(bw):14.1f} "
+                  f"{o / sum(bw):5.2f}/{r / sum(bw):5.2f} {sum(i['stores'] - j['stores'] for i, j in zip(infos, before)) // 4:7d} "
+                  f"{sum(i['retrieves'] - j['retrieves'] for i, j in zip(infos, before)) // 4:9d} "
+                  f"{'/'.join('yes' if i['direct_io'] else 'no' for i in infos) or '-':>6s}", flush=True)
+        finally:
+            pool.destroy()
+
+
 def run_duplex(args) -> None:
     """A serving engine evicts one request's KV while it fetches another's.  Request A is offloaded on one stream while
     request B (offloaded beforehand) is retrieved on another; both legs are timed with CUDA events on their own stream and
@@ -1359,6 +1446,9 @@ def main():
         return
     if args.mixed_pool:
         run_mixed_pool(args)
+        return
+    if args.ssd_pool:
+        run_ssd_pool(args)
         return
     if args.duplex:
         run_duplex(args)

@@ -1,8 +1,9 @@
 /*
  * kvpool.h — C ABI of the B200-native unified KV pooling hot path (arxiv 2606.14779).
  *
- * The library moves a request's *paged* KV cache between GPU HBM and a pool of pinned host buffers
- * ("pool devices"), assigning each layer's KV blocks to pool devices in proportion to
+ * The library moves a request's *paged* KV cache between GPU HBM and a pool of "pool devices" — pinned
+ * host buffers (type MEM), block storage addressed by LBA (type SSD, KV-passthrough) and GPU memory of
+ * NVLink peers (type HBM) —, assigning each layer's KV blocks to pool devices in proportion to
  * their measured bandwidth (Eq. 1-2; Algorithm 1) and retrieving
  * them through a dense global lookup table (Table I; retrieval).
  *
@@ -70,7 +71,7 @@ enum {
                                         at all - and driven by the device's own worker thread through asynchronous store /
                                         retrieve commands; GPU streams and the worker hand bounce lanes to each other with
                                         stream write-value / wait-value operations, no host callback and no
-                                        synchronisation (DESIGN.md section 14).  Excludes every other flag.               */
+                                        synchronisation (DESIGN.md section 13).  Excludes every other flag.               */
 
 #define KVPOOL_MEASURE_KERNEL_RETRIEVE 2 /* kvpool_measure_bandwidth / kvpool_calibrate `direction`, see there */
 #define KVPOOL_MEASURE_KERNEL_OFFLOAD 3

@@ -113,7 +113,7 @@ struct SsdLane {
   cudaEvent_t kernel_done = nullptr;  // last kernel that read / wrote stage
   uint32_t uses = 0;                  // sequence number of the lane's latest use (the value its flags are compared with)
 };
-struct SsdState {  // one SSD-type pool device (KV-passthrough, PAPER.md:179-185; DESIGN.md section 14)
+struct SsdState {  // one SSD-type pool device (KV-passthrough, PAPER.md:179-185; DESIGN.md section 13)
   SsdDevice io;
   uint8_t* bounce_base = nullptr;  // pinned host memory: [direction][lane] x lane_bytes
   uint8_t* stage_base = nullptr;   // device memory, same layout

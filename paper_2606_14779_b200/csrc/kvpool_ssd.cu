@@ -1,4 +1,4 @@
-// libkvpool.so: SSD-type pool devices — KV-passthrough, GPU side.  DESIGN.md section 14.
+// libkvpool.so: SSD-type pool devices — KV-passthrough, GPU side.  DESIGN.md section 13.
 //
 // An SSD-type device's share of a layer moves in lane-sized commands, DEVICE-MAJOR (runs of consecutive slots of its
 // stripe = consecutive bytes of its LBA range, reached through the device's inverse map like the chunks of kvpool_xfer.cu):
@@ -138,69 +138,94 @@ int ssd_ensure_lanes(kvpool* p) {
   return KVPOOL_OK;
 }
 
+namespace {
+
+// One command of device i: `bytes` at byte offset `byte0` of the device travel between its LBA range and the staging piece of
+// the next lane of that direction.  `launch(stage)` enqueues on `s` whatever fills (store) or drains (retrieve) the piece —
+// the pack / unpack launch — and returns a KVPOOL code.  *lane_out / *use_out name the command (for ssd_wait_stored).
+template <class Launch>
+int ssd_command(kvpool* p, uint32_t i, bool pack, uint64_t byte0, uint64_t bytes, bool zero_tail, cudaStream_t s, Launch&& launch,
+                uint32_t* lane_out, uint32_t* use_out) {
+  SsdState& S = *p->ssd[i];
+  const uint64_t sec = S.io.sector();
+  const int d = pack ? 1 : 0;
+  cudaStream_t io = pack ? p->io_out[i] : p->io[i];
+  const uint64_t at = byte0 / sec * sec;
+  const uint32_t head = static_cast<uint32_t>(byte0 - at);
+  const uint32_t k = S.cursor[d]++ % S.n_lanes;
+  SsdLane& ln = S.lane[d][k];
+  const uint32_t u = ++ln.uses;
+  *lane_out = k;
+  *use_out = u;
+  // If enqueueing fails half way, both flags of this use are raised from the host so that no later use of the lane (and no
+  // worker) waits for a hand-over that will never come.
+  auto abandon = [&](int rc) {
+    __atomic_store_n(S.flags + flag_word(S, d, k, false), u, __ATOMIC_RELEASE);
+    __atomic_store_n(S.flags + flag_word(S, d, k, true), u, __ATOMIC_RELEASE);
+    return rc;
+  };
+  auto cu = [&](cudaError_t e, const char* what) { return e == cudaSuccess ? KVPOOL_OK : fail(KVPOOL_ECUDA, "%s: %s", what, cudaGetErrorString(e)); };
+  int rc;
+  if (pack) {
+    // SSD_Direct_Store: gather into the lane's staging piece, copy it out to the bounce memory once the lane's previous
+    // command has been written (cpu_seq >= u-1), tell the worker (gpu_seq = u); the worker writes the LBA range
+    if ((rc = cu(cudaStreamWaitEvent(s, ln.copy_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
+    if ((rc = launch(ln.stage)) != KVPOOL_OK) return abandon(rc);
+    if ((rc = cu(cudaEventRecord(ln.kernel_done, s), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
+    if ((rc = cu(cudaStreamWaitEvent(io, ln.kernel_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
+    if (g_wait_value(io, flag_dev(S, d, k, true), u - 1, kWaitGeq) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed"));
+    if ((rc = cu(cudaMemcpyAsync(ln.bounce + head, ln.stage, bytes, cudaMemcpyDeviceToHost, io), "cudaMemcpyAsync")) != KVPOOL_OK) return abandon(rc);
+    p->n_memcpys++;
+    if (g_write_value(io, flag_dev(S, d, k, false), u, kWriteDefault) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed"));
+    if ((rc = cu(cudaEventRecord(ln.copy_done, io), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
+    S.io.submit(SsdCmd{SsdCmd::kWrite, zero_tail, k, u, at, head, bytes});
+    return KVPOOL_OK;
+  }
+  // SSD_Direct_Retrieve: the worker reads the LBA range into the bounce memory once the lane's previous command has been
+  // drained (gpu_seq >= u-1) and raises cpu_seq = u; the copy waits for that, the unpack for the copy
+  S.io.submit(SsdCmd{SsdCmd::kRead, false, k, u, at, head, bytes});
+  if (g_wait_value(io, flag_dev(S, d, k, true), u, kWaitGeq) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed"));
+  if ((rc = cu(cudaStreamWaitEvent(io, ln.kernel_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
+  if ((rc = cu(cudaMemcpyAsync(ln.stage, ln.bounce + head, bytes, cudaMemcpyHostToDevice, io), "cudaMemcpyAsync")) != KVPOOL_OK) return abandon(rc);
+  p->n_memcpys++;
+  if (g_write_value(io, flag_dev(S, d, k, false), u, kWriteDefault) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed"));
+  if ((rc = cu(cudaEventRecord(ln.copy_done, io), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
+  if ((rc = cu(cudaStreamWaitEvent(s, ln.copy_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return rc;
+  if ((rc = launch(ln.stage)) != KVPOOL_OK) return rc;
+  return cu(cudaEventRecord(ln.kernel_done, s), "cudaEventRecord");
+}
+
+}  // namespace
+
 int ssd_move(kvpool* p, LayerState& L, uint32_t i, uint32_t lo, uint32_t hi, bool pack, LayerArgs a, cudaStream_t s) {
   SsdState& S = *p->ssd[i];
   if (!S.n_lanes) return fail(KVPOOL_ESTATE, "SSD-type device %u has no bounce lanes", i);
   const uint64_t P = p->payload, sec = S.io.sector();
-  const int d = pack ? 1 : 0;
-  cudaStream_t io = pack ? p->io_out[i] : p->io[i];
   const uint64_t unit = sec / gcd64(P, sec);  // every `unit` KV caches the stripe is back on a sector boundary
   a.order = L.map->order_d;
   a.visit = nullptr;
   for (uint32_t x = lo; x < hi;) {
     const uint64_t byte0 = L.stripe_off[i] + static_cast<uint64_t>(x) * P;
-    const uint64_t at = byte0 / sec * sec;
-    const uint32_t head = static_cast<uint32_t>(byte0 - at);
+    const uint32_t head = static_cast<uint32_t>(byte0 % sec);
     uint32_t n = static_cast<uint32_t>(std::min<uint64_t>(hi - x, (S.lane_bytes - sec - head) / P));
     if (unit > 1 && x + n < hi) {  // ragged KV size: end the command on a sector boundary when one is within reach
       const uint64_t end = (static_cast<uint64_t>(x) + n) / unit * unit;
       if (end > x) n = static_cast<uint32_t>(end - x);
     }
-    const uint32_t k = S.cursor[d]++ % S.n_lanes;
-    SsdLane& ln = S.lane[d][k];
-    const uint32_t u = ++ln.uses;
-    const uint64_t bytes = static_cast<uint64_t>(n) * P;
     a.j0 = L.map->start[i] + x;
     a.K = n;
-    a.pool_base[0] = reinterpret_cast<uint64_t>(ln.stage);
-    // If enqueueing fails half way, both flags of this use are raised from the host so that no later use of the lane
-    // (and no worker) waits for a hand-over that will never come.
-    auto abandon = [&](int rc) {
-      __atomic_store_n(S.flags + flag_word(S, d, k, false), u, __ATOMIC_RELEASE);
-      __atomic_store_n(S.flags + flag_word(S, d, k, true), u, __ATOMIC_RELEASE);
-      return rc;
-    };
-    auto cu = [&](cudaError_t e, const char* what) { return e == cudaSuccess ? KVPOOL_OK : fail(KVPOOL_ECUDA, "%s: %s", what, cudaGetErrorString(e)); };
-    int rc;
+    uint32_t lane = 0, use = 0;
+    const int rc = ssd_command(p, i, pack, byte0, static_cast<uint64_t>(n) * P, x + n == L.map->counts[i], s,
+                               [&](uint8_t* stage) {
+                                 a.pool_base[0] = reinterpret_cast<uint64_t>(stage);
+                                 return launch_counted(p, a, pack, false, s);
+                               },
+                               &lane, &use);
+    if (rc != KVPOOL_OK) return rc;
     if (pack) {
-      // SSD_Direct_Store: gather into the lane's staging piece, copy it out to the bounce memory once the lane's previous
-      // command has been written (cpu_seq >= u-1), tell the worker (gpu_seq = u); the worker writes the LBA range
-      if ((rc = cu(cudaStreamWaitEvent(s, ln.copy_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
-      if ((rc = launch_counted(p, a, true, false, s)) != KVPOOL_OK) return abandon(rc);
-      if ((rc = cu(cudaEventRecord(ln.kernel_done, s), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
-      if ((rc = cu(cudaStreamWaitEvent(io, ln.kernel_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
-      if (g_wait_value(io, flag_dev(S, d, k, true), u - 1, kWaitGeq) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed"));
-      if ((rc = cu(cudaMemcpyAsync(ln.bounce + head, ln.stage, bytes, cudaMemcpyDeviceToHost, io), "cudaMemcpyAsync")) != KVPOOL_OK) return abandon(rc);
-      p->n_memcpys++;
-      if (g_write_value(io, flag_dev(S, d, k, false), u, kWriteDefault) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed"));
-      if ((rc = cu(cudaEventRecord(ln.copy_done, io), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
-      S.io.submit(SsdCmd{SsdCmd::kWrite, x + n == L.map->counts[i], k, u, at, head, bytes});
-      L.ssd_last_lane[i] = k;
-      L.ssd_last_use[i] = u;
+      L.ssd_last_lane[i] = lane;
+      L.ssd_last_use[i] = use;
       L.ssd_stored |= 1u << i;
-    } else {
-      // SSD_Direct_Retrieve: the worker reads the LBA range into the bounce memory once the lane's previous command has
-      // been drained (gpu_seq >= u-1) and raises cpu_seq = u; the copy waits for that, the unpack for the copy
-      S.io.submit(SsdCmd{SsdCmd::kRead, false, k, u, at, head, bytes});
-      if (g_wait_value(io, flag_dev(S, d, k, true), u, kWaitGeq) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed"));
-      if ((rc = cu(cudaStreamWaitEvent(io, ln.kernel_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
-      if ((rc = cu(cudaMemcpyAsync(ln.stage, ln.bounce + head, bytes, cudaMemcpyHostToDevice, io), "cudaMemcpyAsync")) != KVPOOL_OK) return abandon(rc);
-      p->n_memcpys++;
-      if (g_write_value(io, flag_dev(S, d, k, false), u, kWriteDefault) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed"));
-      if ((rc = cu(cudaEventRecord(ln.copy_done, io), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
-      if ((rc = cu(cudaStreamWaitEvent(s, ln.copy_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return rc;
-      if ((rc = launch_counted(p, a, false, false, s)) != KVPOOL_OK) return rc;
-      if ((rc = cu(cudaEventRecord(ln.kernel_done, s), "cudaEventRecord")) != KVPOOL_OK) return rc;
     }
     x += n;
   }
@@ -234,25 +259,36 @@ int ssd_read(kvpool* p, uint32_t i, uint64_t off, void* dst, uint64_t n) {
   return e ? fail(KVPOOL_EIO, "read of SSD-type device %u: %s", i, strerror(e)) : KVPOOL_OK;
 }
 
-// "Measured bandwidth" of an SSD-type device: sequential commands of the scratch size over the first
-// `bytes` of the device, on the calling thread, median of `iters` passes by the host's clock.  The region is written
-// once first, so that a sparse stand-in file has its blocks.  The disk side only: the PCIe hop of a lane overlaps it.
+// "Measured bandwidth" of an SSD-type device, with the mechanism that moves the bytes: the first `bytes` of
+// the device travel through the device's own lanes — worker, bounce memory, copy engine, staging piece — exactly as a
+// retrieve (or an offload) moves them, without the pack / unpack launch; median of `iters` passes by the host's clock
+// around enqueue + completion.  (A plain pread loop into a cache-resident buffer reads 10-15 % fast.)  The region is
+// written once first, so that a sparse stand-in file has its blocks.
 int ssd_measure(kvpool* p, uint32_t i, bool write, uint64_t bytes, uint32_t iters, double* gbps) {
+  int rc = ssd_ensure_lanes(p);
+  if (rc != KVPOOL_OK) return rc;
   SsdState& S = *p->ssd[i];
-  const uint64_t sec = S.io.sector();
+  DeviceGuard guard(p->cuda_device);
+  const uint64_t sec = S.io.sector(), piece = (S.lane_bytes - 2 * sec) / sec * sec;
   bytes = bytes / sec * sec;
   if (bytes == 0) return fail(KVPOOL_EINVAL, "measure_bandwidth: fewer bytes than one sector");
-  memset(S.scratch, 0x5a, kSsdScratchBytes);
-  int e = S.io.io_span(true, 0, bytes, S.scratch, kSsdScratchBytes);
+  cudaStream_t s = p->upload, io = write ? p->io_out[i] : p->io[i];
   std::vector<double> sec_s(iters);
-  for (uint32_t it = 0; it < iters && !e; ++it) {
+  for (uint32_t it = 0; it < iters + 1; ++it) {  // pass 0 writes the region (and warms up)
+    const bool w = write || it == 0;
     timespec t0, t1;
     clock_gettime(CLOCK_MONOTONIC, &t0);
-    e = S.io.io_span(write, 0, bytes, S.scratch, kSsdScratchBytes);
+    for (uint64_t off = 0; off < bytes; off += piece) {
+      uint32_t lane, use;
+      rc = ssd_command(p, i, w, off, std::min(piece, bytes - off), false, s, [](uint8_t*) { return KVPOOL_OK; }, &lane, &use);
+      if (rc != KVPOOL_OK) return rc;
+    }
+    CU(cudaStreamSynchronize(s));
+    CU(cudaStreamSynchronize(w ? p->io_out[i] : io));
+    if ((rc = ssd_drain(p)) != KVPOOL_OK) return rc;
     clock_gettime(CLOCK_MONOTONIC, &t1);
-    sec_s[it] = (t1.tv_sec - t0.tv_sec) + 1e-9 * (t1.tv_nsec - t0.tv_nsec);
+    if (it > 0) sec_s[it - 1] = (t1.tv_sec - t0.tv_sec) + 1e-9 * (t1.tv_nsec - t0.tv_nsec);
   }
-  if (e) return fail(KVPOOL_EIO, "measure_bandwidth: SSD-type device %u: %s", i, strerror(e));
   std::sort(sec_s.begin(), sec_s.end());
   *gbps = static_cast<double>(bytes) / (sec_s[iters / 2] * 1.0e9);
   return KVPOOL_OK;

@@ -1,6 +1,6 @@
 """GPU parity of SSD-type pool devices (KV-passthrough; Algorithm 1 l.20-21) against the CPU oracle.
 
-There is no NVMe device on the GPU box, so the "SSD" is a file opened O_DIRECT (R19, section 14); what is compared
+There is no NVMe device on the GPU box, so the "SSD" is a file opened O_DIRECT (R19, section 13); what is compared
 does not depend on the medium: the placement, the LBA range of every offload set (length = the paper's ceil formula), the
 bytes of every sector of those ranges — read back from the file with plain Python file I/O, never through the library —
 against orc_ssd_direct_store, every KV cache's GLT location against orc_ssd_location, and the retrieved paged tensors.
