@@ -816,6 +816,19 @@ def run_kvpool(args) -> dict:
             shapes[other.wl.name] = side_line(other, 9 if other.moved < (8 << 30) else 5, 3, link_h2d, link_d2h)
             other.close()
 
+    pools = {}
+    if world == 1 and args.config == 4 and args.path == "auto" and not args.no_extras:
+        # unified pooling over host memory AND block storage: a pinned host buffer plus one SSD-type
+        # device (a file opened O_DIRECT stands in: no NVMe on this box), 8 layers of this configuration, bit-verified
+        try:
+            lines = ssd_pool_lines(4, args.ssd_dir, ["ms"])
+            head = next(lines)
+            for r in lines:
+                pools["host+ssd"] = dict(r, medium=head["medium"], layers=head["layers"], moved_bytes_per_leg=head["moved_bytes_per_leg"],
+                                         frac_of_link=r["retrieve_gbps"] / link_h2d, offload_frac_of_link=r["offload_gbps"] / link_d2h)
+        except Exception as e:                         # (a box without a writable --ssd-dir: say so instead of losing the headline)
+            pools["host+ssd"] = {"unavailable": f"{type(e).__name__}: {e}"}
+
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "warmup_extra_steps": settle["extra_steps"], "ms_per_step": step_ms,
@@ -847,6 +860,8 @@ def run_kvpool(args) -> dict:
         out["paths"] = paths
     if shapes:
         out["shapes"] = shapes
+    if pools:
+        out["pools"] = pools
     if layer_rows:
         out["retrieve_layer_ms"] = layer_stats(layer_rows)
     if args.detail and rank == 0:
@@ -1108,13 +1123,12 @@ def run_mixed_pool(args) -> None:
         pool.destroy()
 
 
-def run_ssd_pool(args) -> None:
-    """Unified pooling over host memory AND block storage (PAPER.md:132, 179-185): Eq. 1-2 split every layer between a pinned
-    host buffer and one or two SSD-type devices in proportion to kvpool_calibrate's figures (cudaMemcpyAsync for the host
-    buffer, the device's own sequential commands for an SSD; all devices name one link group because every byte crosses this
-    GPU's single PCIe link).  Whole request (8 layers of --config), batched calls, legs timed apart with CUDA events on the
-    caller's stream — the offload leg ends when kvpool_wait_offloads lets the stream go, i.e. when the store commands are on
-    the disk; every run is verified bit-exact against the source.  Text table on stdout."""
+def ssd_pool_lines(cfg: int, ssd_dir: str, kinds):
+    """Generator behind --ssd-pool and the `pools` side line of the default run: for every pool in `kinds` (a string per pool,
+    'm' = pinned host buffer, 's' = SSD-type device) one dict with the calibrated weights, the split and the bit-verified
+    offload / retrieve GB/s of a whole request (8 layers of config `cfg`, batched calls, legs timed apart with CUDA events on
+    the caller's stream - the offload leg ends when kvpool_wait_offloads lets the stream go, i.e. when the store commands
+    are on the disk).  The first item yielded is the header dict."""
     import torch
     from paper_2606_14779_b200 import binding as kv
     from paper_2606_14779_b200 import workloads as W
@@ -1122,7 +1136,7 @@ def run_ssd_pool(args) -> None:
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
     L = 8
-    wl = W.make_workload(args.config, n_layers=L)
+    wl = W.make_workload(cfg, n_layers=L)
     wl.sliding_layers = ()
     g = wl.geom
     bpl = wl.blocks_per_layer(0)
@@ -1135,16 +1149,13 @@ def run_ssd_pool(args) -> None:
     s = torch.cuda.Stream(device=dev)
     torch.cuda.synchronize()
     cap = (moved + (L + 4) * (g.payload + 65536) + 65535) // 65536 * 65536
-    given = [x for x in args.ssd_dir.split(",") if x]
+    given = [x for x in ssd_dir.split(",") if x]
     blockdevs = all(os.path.exists(x) and not os.path.isdir(x) for x in given)
-    print(f"# bench.py --ssd-pool --config {args.config} --ssd-dir {args.ssd_dir}: {wl.name} cut to {L} layers, {moved / 2**20:.0f} MiB per leg ({K} blocks of "
-          f"{g.payload} B per layer); SSD-type devices = {'the block devices given' if blockdevs else 'files under ' + given[0] + ' opened O_DIRECT (no NVMe on this box)'}; "
-          "weights = kvpool_calibrate (256 MiB per device, one link group); median of 3; 8 MiB commands on 4 lanes per device and direction")
-    print(f"{'pool':30s} {'weights (GB/s)':>20s} {'blocks per layer':>18s} {'offload GB/s':>12s} {'retrieve GB/s':>13s} {'sum of weights':>14s} {'of sum':>11s} {'stores':>7s} {'retrieves':>9s} {'direct':>6s}   (stores / retrieves: commands per leg)")
-    for name, types in (("1 host buffer", "m"), ("1 SSD", "s"), ("1 host buffer + 1 SSD", "ms"), ("1 host buffer + 2 SSDs", "mss")):
+    yield {"workload": wl.name, "layers": L, "moved_bytes_per_leg": moved, "blocks_per_layer": K, "payload": g.payload,
+           "medium": "the block devices given" if blockdevs else f"files under {given[0]} opened O_DIRECT (no NVMe on this box)"}
+    for types in kinds:
         n = len(types)
-        n_ssd = types.count("s")
-        if blockdevs and n_ssd > len(given):
+        if blockdevs and types.count("s") > len(given):
             continue
         paths, k = [], 0
         for t in types:
@@ -1161,7 +1172,7 @@ def run_ssd_pool(args) -> None:
                 for d in dst:
                     d.fill_(np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item())
                 pl = pool.place(bpl)
-                counts = list(pl.counts(0))
+                counts = [int(c) for c in pl.counts(0)]
                 torch.cuda.synchronize()
                 ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
                 ev[0].record(s)
@@ -1180,15 +1191,34 @@ def run_ssd_pool(args) -> None:
                     rets.append(ev[2].elapsed_time(ev[3]))
             for l in range(L):
                 if not torch.equal(dst[l][:, tables[l].long()], src[l][:, tables[l].long()]):
-                    raise RuntimeError(f"{name}: retrieved KV differs from the source")
-            o, r = moved / statistics.median(offs) / 1e6, moved / statistics.median(rets) / 1e6
+                    raise RuntimeError(f"pool {types}: retrieved KV differs from the source")
             infos = [pool.ssd_info(i) for i in ssds]
-            print(f"{name:30s} {'/'.join(f'{b:.1f}' for b in bw):>20s} {'/'.join(str(c) for c in counts):>18s} {o:12.2f} {r:13.2f} {sum(bw):14.1f} "
-                  f"{o / sum(bw):5.2f}/{r / sum(bw):5.2f} {sum(i['stores'] - j['stores'] for i, j in zip(infos, before)) // 4:7d} "
-                  f"{sum(i['retrieves'] - j['retrieves'] for i, j in zip(infos, before)) // 4:9d} "
-                  f"{'/'.join('yes' if i['direct_io'] else 'no' for i in infos) or '-':>6s}", flush=True)
+            yield {"pool": types, "bandwidth_gbps": [round(float(b), 2) for b in bw], "blocks_per_layer": counts,
+                   "offload_gbps": moved / statistics.median(offs) / 1e6, "retrieve_gbps": moved / statistics.median(rets) / 1e6,
+                   "sum_of_weights_gbps": float(sum(bw)), "stores_per_leg": sum(i["stores"] - j["stores"] for i, j in zip(infos, before)) // 4,
+                   "retrieves_per_leg": sum(i["retrieves"] - j["retrieves"] for i, j in zip(infos, before)) // 4,
+                   "direct_io": [i["direct_io"] for i in infos], "verified_bit_exact_round_trip": True}
         finally:
             pool.destroy()
+
+
+def run_ssd_pool(args) -> None:
+    """Unified pooling over host memory AND block storage (PAPER.md:132, 179-185): Eq. 1-2 split every layer between a pinned
+    host buffer and one or two SSD-type devices in proportion to kvpool_calibrate's figures (cudaMemcpyAsync for the host
+    buffer, the device's own lanes for an SSD; all devices name one link group because every byte crosses this GPU's single
+    PCIe link).  Text table on stdout; ssd_pool_lines has the procedure."""
+    names = {"m": "1 host buffer", "s": "1 SSD", "ms": "1 host buffer + 1 SSD", "mss": "1 host buffer + 2 SSDs"}
+    lines = ssd_pool_lines(args.config, args.ssd_dir, list(names))
+    h = next(lines)
+    print(f"# bench.py --ssd-pool --config {args.config} --ssd-dir {args.ssd_dir}: {h['workload']} cut to {h['layers']} layers, {h['moved_bytes_per_leg'] / 2**20:.0f} MiB per leg "
+          f"({h['blocks_per_layer']} blocks of {h['payload']} B per layer); SSD-type devices = {h['medium']}; "
+          "weights = kvpool_calibrate (256 MiB per device, one link group); median of 3; 8 MiB commands on 4 lanes per device and direction")
+    print(f"{'pool':30s} {'weights (GB/s)':>20s} {'blocks per layer':>18s} {'offload GB/s':>12s} {'retrieve GB/s':>13s} {'sum of weights':>14s} {'of sum':>11s} {'stores':>7s} {'retrieves':>9s} {'direct':>6s}   (stores / retrieves: commands per leg)")
+    for r in lines:
+        sw = r["sum_of_weights_gbps"]
+        print(f"{names[r['pool']]:30s} {'/'.join(f'{b:.1f}' for b in r['bandwidth_gbps']):>20s} {'/'.join(str(c) for c in r['blocks_per_layer']):>18s} "
+              f"{r['offload_gbps']:12.2f} {r['retrieve_gbps']:13.2f} {sw:14.1f} {r['offload_gbps'] / sw:5.2f}/{r['retrieve_gbps'] / sw:5.2f} "
+              f"{r['stores_per_leg']:7d} {r['retrieves_per_leg']:9d} {'/'.join('yes' if d else 'no' for d in r['direct_io']) or '-':>6s}", flush=True)
 
 
 def run_duplex(args) -> None:

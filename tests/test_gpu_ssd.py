@@ -387,3 +387,69 @@ def test_measure_bandwidth_and_calibrate_with_an_ssd(tmp_path):
         pl.release()
     finally:
         pool.destroy()
+
+
+@pytest.mark.timeout(1200)
+def test_full_size_config4_with_two_ssd_devices_every_byte_against_oracle(tmp_path):
+    """BASELINE.json's headline configuration at its FULL size (Qwen3-30B-A3B-shaped KV at 128K: 48 layers x 8192 blocks, 12 GiB
+    per leg, weights 4:4:2:2:1:1) with the two slowest pool devices made SSD-type: 585 blocks of every layer (18.3 MiB, three
+    8 MiB commands) go to each, 1.7 GiB in all through the lanes.  Batched calls as in bench.py; compared with the oracle
+    BYTE FOR BYTE, streamed layer by layer: every stripe, every sector of every LBA range (read from the files with plain file
+    I/O), the whole retrieved tensor."""
+    wl = W.make_workload(4)
+    g, dev, L = wl.geom, torch.device("cuda:0"), wl.geom.n_layers
+    bw = list(wl.default_weights())
+    types = ["mem"] * 4 + ["ssd"] * 2
+    share = np.array(bw) / np.sum(bw)
+    caps = [(int(wl.moved_bytes() * s * 1.1) + (L + 4) * (g.payload + 8192) + 65535) // 65536 * 65536 for s in share]
+    files = [str(tmp_path / f"ssd{i}.img") if t == "ssd" else None for i, t in enumerate(types)]
+    pool = kv.KvPool(bw, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, dev_flags=[kv.DEV_SSD if t == "ssd" else 0 for t in types],
+                     paths=files, sector_bytes=[4096 if t == "ssd" else 0 for t in types], link_groups=[1] * 6)
+    try:
+        bpl = wl.blocks_per_layer(0)
+        pl, opl = pool.place(bpl), oracle.place(bw, bpl)
+        table_np = [np.ascontiguousarray(wl.layer_table(0, l)) for l in range(L)]
+        tables = [torch.from_numpy(t).to(dev) for t in table_np]
+        src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+        dst = [W.poison_torch((2, wl.nphys, g.kvb // 2), dev) for _ in range(L)]
+        torch.cuda.synchronize()
+        s = torch.cuda.Stream()
+        pool.offload_layers(pl, 0, [x[0] for x in src], [x[1] for x in src], g.kvb, tables, s)
+        pool.wait_offloads(pl, s)
+        s.synchronize()
+        pool.synchronize()
+        pool.retrieve_layers(pl, 0, [d[0] for d in dst], [d[1] for d in dst], g.kvb, tables, s)
+        s.synchronize()
+        pool.synchronize()
+        shape = (2, wl.nphys, g.kvb // 2)
+        pin_src, pin_got = torch.empty(shape, dtype=torch.int16).pin_memory(), torch.empty(shape, dtype=torch.int16).pin_memory()
+        ref = np.empty(shape, dtype=np.uint16)
+        stripe_bytes = sector_bytes = 0
+        for l in range(L):
+            assert np.array_equal(pl.counts(l), opl[l].counts) and list(opl[l].counts) == [2341, 2341, 1170, 1170, 585, 585]
+            d_, s_ = pl.layer_map(l)
+            assert np.array_equal(d_.astype(np.uint32), opl[l].dev) and np.array_equal(s_, opl[l].slot)
+            pin_src.copy_(src[l], non_blocking=True)
+            pin_got.copy_(dst[l], non_blocking=True)
+            torch.cuda.synchronize()
+            src_cpu, got = pin_src.numpy().view(np.uint16), pin_got.numpy().view(np.uint16)
+            want = oracle.offload_layer(src_cpu, table_np[l], opl[l], parallel=True)
+            for i, t in enumerate(types):
+                assert np.array_equal(pl.stripe(l, i), want[i]), f"stripe bytes differ: layer {l} device {i}"
+                stripe_bytes += want[i].nbytes
+                if t == "ssd":
+                    first, n_sec, sec = pl.ssd_range(l, i)
+                    assert n_sec == oracle.lba_range_len(585, g.payload, sec) == 585 * 8
+                    disk = np.empty(n_sec * sec, dtype=np.uint8)
+                    oracle.ssd_direct_store(disk, sec, 0, want[i], g.payload)
+                    assert np.array_equal(_read_file(files[i], first * sec, n_sec * sec), disk), f"sectors differ: layer {l} device {i}"
+                    sector_bytes += disk.nbytes
+            ref[...] = W.POISON_BITS
+            oracle.retrieve_layer(ref, table_np[l], opl[l], want, parallel=True)
+            assert np.array_equal(got, ref), f"retrieved layer {l} differs from the oracle's"
+        assert stripe_bytes == wl.moved_bytes() and sector_bytes == 2 * 48 * 585 * g.payload
+        info = pool.ssd_info(5)
+        assert info["stores"] >= 48 * 3 and info["retrieves"] >= 48 * 3
+        pl.release()
+    finally:
+        pool.destroy()
