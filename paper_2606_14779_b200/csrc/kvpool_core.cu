@@ -378,7 +378,11 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
 int kvpool_destroy(kvpool_t* p) {
   if (!p) return fail(KVPOOL_EINVAL, "destroy: null pool");
   DeviceGuard guard(p->cuda_device);
-  cudaDeviceSynchronize();
+  if (cudaDeviceSynchronize() != cudaSuccess) {  // a dead GPU never delivers its half of the pending SSD commands
+    cudaGetLastError();
+    for (auto& S : p->ssd)
+      if (S) S->io.abort();
+  }
   for (auto* pl : p->live) destroy_placement(p, pl);
   p->live.clear();
   ssd_close_all(p);  // (after the device-wide synchronize above: every command has had the GPU's half)

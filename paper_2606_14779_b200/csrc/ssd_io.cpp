@@ -125,8 +125,8 @@ void SsdDevice::drain() {
 }
 
 // Poll for the GPU's half of a command (the paper polls NVMe completions on a dedicated core; here the
-// worker polls the flag a stream write-value raises): spin briefly, then poll every 20 us.  Gives up after two minutes
-// (a GPU that never delivers must not hang the process): the command then fails with ETIMEDOUT.
+// worker polls the flag a stream write-value raises): spin briefly, then poll every 20 us.  Gives up when the pool says
+// the GPU is gone (abort(), from kvpool_destroy after a failed device synchronize) and, as a backstop, after ten minutes.
 bool SsdDevice::wait_flag(const volatile uint32_t* f, uint32_t v) {
   for (int i = 0; i < 4096; ++i) {
     if (seq_reached(f, v)) return true;
@@ -136,8 +136,9 @@ bool SsdDevice::wait_flag(const volatile uint32_t* f, uint32_t v) {
   const timespec nap{0, 20000};
   for (uint64_t n = 0;; ++n) {
     if (seq_reached(f, v)) return true;
+    if (abort_.load(std::memory_order_relaxed)) return false;
     nanosleep(&nap, nullptr);
-    if ((n & 1023) == 1023 && std::chrono::steady_clock::now() - t0 > std::chrono::seconds(120)) return false;
+    if ((n & 1023) == 1023 && std::chrono::steady_clock::now() - t0 > std::chrono::minutes(10)) return false;
   }
 }
 
@@ -166,11 +167,11 @@ void SsdDevice::execute(const SsdCmd& c) {
   if (total > lane_bytes_ || c.file_off % sector_ || c.file_off + total > capacity_) e = EINVAL;
   if (c.op == SsdCmd::kRead) {
     // SSD_Direct_Retrieve: the lane is free once the GPU has drained its previous use; read the LBA range into it
-    if (!wait_flag(gpu, c.use - 1)) e = e ? e : ETIMEDOUT;
+    if (!wait_flag(gpu, c.use - 1)) e = e ? e : (abort_.load() ? ECANCELED : ETIMEDOUT);
     if (!e) e = rw_full(false, c.file_off, buf, total);
   } else {
     // SSD_Direct_Store: wait for the GPU's copy into the lane, complete the first / last sector, write the LBA range
-    if (!wait_flag(gpu, c.use)) e = e ? e : ETIMEDOUT;
+    if (!wait_flag(gpu, c.use)) e = e ? e : (abort_.load() ? ECANCELED : ETIMEDOUT);
     if (!e && c.head) {  // the range starts inside a sector that holds a neighbour's bytes: keep them
       e = rw_full(false, c.file_off, edge_, sector_);
       if (!e) memcpy(buf, edge_, c.head);

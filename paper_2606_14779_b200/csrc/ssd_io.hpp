@@ -48,6 +48,7 @@ class SsdDevice {
   void stop();  // drains, then joins the worker
   void submit(const SsdCmd& c);
   void drain();  // block until every submitted command has completed
+  void abort() { abort_.store(true); }  // the GPU is gone: commands still waiting for its half fail with ECANCELED instead of polling on
   // first I/O error since the last call (an errno value; 0 = none).  A failed command still completes its handshake,
   // so that no stream waits for ever.
   int take_error() { return error_.exchange(0); }
@@ -86,6 +87,7 @@ class SsdDevice {
   uint64_t submitted_ = 0, finished_ = 0;
   bool stopping_ = false;
   std::atomic<int> error_{0};
+  std::atomic<bool> abort_{false};
   std::atomic<uint64_t> done_[2] = {{0}, {0}};
 };
 

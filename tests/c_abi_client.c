@@ -3,8 +3,13 @@
  * run by tests/test_host_logic.py).  With the argument "gpu" (tests/test_gpu_parity.py) it also moves bytes: it creates
  * a pool of one pinned host device and one HBM-type device, places a request, offloads a small paged layer it filled
  * itself, retrieves it into a poisoned copy and compares — the round trip, the untouched blocks, and one payload on
- * each pool device located through kvpool_lookup (Table I `location`).  It links the library and the CUDA runtime
- * only: no oracle, no Python. */
+ * each pool device located through kvpool_lookup (Table I `location`).  With a file name as second argument the pool gets
+ * a third, SSD-type device backed by that file (KV-passthrough): its payloads are found by LBA
+ * (kvpool_ssd_location) and read back with plain pread.  It links the library and the CUDA runtime only: no oracle, no
+ * Python. */
+#define _XOPEN_SOURCE 700
+#include <fcntl.h>
+#include <unistd.h>
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
@@ -20,13 +25,18 @@ extern int cudaDeviceSynchronize(void);
 
 #define CHECK(x) do { if ((x) != 0) { fprintf(stderr, "%s failed: %s\n", #x, kvpool_last_error()); return 3; } } while (0)
 
-static int gpu_round_trip(void) {
+static int gpu_round_trip(const char *ssd_path) {
     enum { NPHYS = 96, K0 = 64, K1 = 3, KVB = 16 * 2 * 64 * 2, PLANE = NPHYS * KVB };
-    kvpool_device_desc d[2] = {{2.0, 8u << 20, -1, 0, -1, 0, NULL, 0, 0}, {1.0, 8u << 20, -1, KVPOOL_DEV_HBM, -1, 0, NULL, 0, 0}};
+    kvpool_device_desc d[3] = {{2.0, 8u << 20, -1, 0, -1, 0, NULL, 0, 0}, {1.0, 8u << 20, -1, KVPOOL_DEV_HBM, -1, 0, NULL, 0, 0},
+                               {1.0, 8u << 20, -1, KVPOOL_DEV_SSD, -1, 0, NULL, 512, 0}};
+    const uint32_t n_dev = ssd_path ? 3 : 2;
+    uint64_t lba = 0;
+    uint32_t in_sector = 0, sector = 0;
+    int fd = -1;
     kvpool_geometry g = {2, 16, 2, 64, 2};
     kvpool_t *pool = NULL;
     kvpool_placement_t *pl = NULL;
-    uint32_t bpl[2] = {K0, K1}, id, type, s, x = 14779u, seen[2] = {0, 0};
+    uint32_t bpl[2] = {K0, K1}, id, type, s, x = 14779u, seen[3] = {0, 0, 0};
     int32_t table[K0];
     unsigned char *src = malloc(2 * PLANE), *back = malloc(2 * PLANE), *payload = malloc(2 * KVB);
     void *src_d = NULL, *dst_d = NULL, *table_d = NULL, *ptr = NULL;
@@ -36,7 +46,8 @@ static int gpu_round_trip(void) {
     for (i = 0; i < 2 * (size_t)PLANE; ++i) { x = x * 1664525u + 1013904223u; src[i] = (unsigned char)(x >> 24); }
     for (j = 0; j < K0; ++j) table[j] = (j * 37 + 11) % NPHYS; /* 37 is coprime with 96: distinct physical blocks */
     CHECK(kvpool_validate_table(table, K0, NPHYS));
-    CHECK(kvpool_create(d, 2, &g, 0, 0, &pool));
+    d[2].path = ssd_path;
+    CHECK(kvpool_create(d, n_dev, &g, 0, 0, &pool));
     CHECK(kvpool_place(pool, bpl, &pl));
     CHECK(kvpool_lookup(pl, 0, 63, &id, &type, &s, &ptr));
     printf("glt block 63: device %u type %u slot %u ptr %s\n", id, type, s, ptr ? "set" : "null");
@@ -57,9 +68,16 @@ static int gpu_round_trip(void) {
     /* Table I: every block's payload (K block then V block) sits at its `location` */
     for (j = 0; j < K0; ++j) {
         CHECK(kvpool_lookup(pl, 0, (uint32_t)j, &id, &type, &s, &ptr));
-        if (id > 1 || type != (id ? (uint32_t)KVPOOL_TYPE_HBM : (uint32_t)KVPOOL_TYPE_MEM) || !ptr) return 4;
+        if (id >= n_dev || type != (id == 2 ? (uint32_t)KVPOOL_TYPE_SSD : id ? (uint32_t)KVPOOL_TYPE_HBM : (uint32_t)KVPOOL_TYPE_MEM)) return 4;
         if (type == KVPOOL_TYPE_MEM) memcpy(payload, ptr, 2 * KVB);
-        else CHECK(cudaMemcpy(payload, ptr, 2 * KVB, 2));
+        else if (type == KVPOOL_TYPE_HBM) CHECK(cudaMemcpy(payload, ptr, 2 * KVB, 2));
+        else { /* Table I: type SSD, location = LBA; SSD_Direct_Retrieve by hand */
+            CHECK(kvpool_ssd_location(pl, 0, (uint32_t)j, &lba, &in_sector));
+            CHECK(kvpool_ssd_range(pl, 0, id, NULL, NULL, &sector));
+            if ((uint64_t)(size_t)ptr != lba) return 4;
+            if (fd < 0 && (fd = open(ssd_path, O_RDONLY)) < 0) return 4;
+            if (pread(fd, payload, 2 * KVB, (off_t)(lba * sector + in_sector)) != 2 * KVB) return 4;
+        }
         if (memcmp(payload, src + (size_t)table[j] * KVB, KVB) || memcmp(payload + KVB, src + PLANE + (size_t)table[j] * KVB, KVB)) {
             fprintf(stderr, "payload of block %d differs from the paged K/V block\n", j);
             return 4;
@@ -67,6 +85,8 @@ static int gpu_round_trip(void) {
         seen[id]++;
     }
     printf("payloads ok: %u on the host device, %u on the HBM device\n", seen[0], seen[1]);
+    if (ssd_path) printf("payloads ok: %u on the SSD device (%u-byte sectors)\n", seen[2], sector);
+    if (fd >= 0) close(fd);
     /* retrieve into the poisoned copy */
     CHECK(kvpool_retrieve(pool, pl, 0, dst_d, (char *)dst_d + PLANE, KVB, table_d, NULL));
     CHECK(cudaDeviceSynchronize());
@@ -103,6 +123,6 @@ int main(int argc, char **argv) {
     printf("error \"%s\"\n", kvpool_last_error());
     printf("%s\n", kvpool_version());
     printf("sizeof %u %u %u\n", (unsigned)sizeof(kvpool_device_desc), (unsigned)sizeof(kvpool_geometry), (unsigned)sizeof(kvpool_tuning));
-    if (argc > 1 && strcmp(argv[1], "gpu") == 0) return gpu_round_trip();
+    if (argc > 1 && strcmp(argv[1], "gpu") == 0) return gpu_round_trip(argc > 2 ? argv[2] : NULL);
     return 0;
 }

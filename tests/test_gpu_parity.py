@@ -740,6 +740,14 @@ def test_plain_c_client_creates_a_pool_on_the_gpu(tmp_path):
     assert f"glt block 2: device {int(d[2])} type {2 * int(d[2])} slot {int(s[2])} ptr set" in out
     assert f"payloads ok: {int(c[0])} on the host device, {int(c[1])} on the HBM device" in out
     assert out[-1] == "round trip ok: 64 blocks of 8192 bytes, 32 other blocks untouched"
+    # the same program with a third, SSD-type device backed by a file: payloads found by LBA and read with plain pread
+    run = subprocess.run([exe, "gpu", str(tmp_path / "ssd.img")], capture_output=True, text=True, timeout=120)
+    assert run.returncode == 0, run.stderr
+    out = run.stdout.splitlines()
+    c = oracle.counts([2000, 1000, 1000], 64)
+    assert f"payloads ok: {int(c[0])} on the host device, {int(c[1])} on the HBM device" in out
+    assert f"payloads ok: {int(c[2])} on the SSD device (512-byte sectors)" in out
+    assert out[-1] == "round trip ok: 64 blocks of 8192 bytes, 32 other blocks untouched" and not (tmp_path / "ssd.img").exists()
 
 
 def test_keyed_glt_finds_blocks_across_placements_and_forgets_them_on_release():

@@ -228,3 +228,39 @@ def test_plan_lba_range_matches_oracle_and_rejects_bad_arguments(golden_dir):
     with pytest.raises(kv.KvPoolError) as e:                                     # more than 2^64 sectors
         kv.kvpool_plan_lba_range(2 ** 63, 2 ** 63, 1)
     assert e.value.code == kv.EINVAL
+
+
+@pytest.mark.parametrize("sector,kv_size,slots,lane_bytes", [(512, 1536, 333, 32 << 10), (4096, 1536, 333, 32 << 10), (512, 96, 777, 4096 + 2 * 512),
+                                                            (4096, 65536, 21, 1 << 20), (4096, 5120, 57, 16 << 10)])
+def test_ssd_worker_stores_and_retrieves_lba_ranges_like_the_oracle(tmp_path, sector, kv_size, slots, lane_bytes):
+    """The host side of KV-passthrough (csrc/ssd_io.cpp: the device's worker thread, read-modify-write of edge sectors, zero
+    padding, lane hand-over) without a GPU: tests/ssd_io_check.cpp plays the GPU's half of every command; the backing file
+    must equal orc_ssd_direct_store's sector array — after the set has arrived in out-of-order instalments that start and
+    end inside sectors — and the read-back must equal the set (orc_ssd_direct_retrieve of every KV cache)."""
+    import subprocess
+    exe = str(tmp_path / "ssd_io_check")
+    csrc = os.path.join(ROOT, "paper_2606_14779_b200", "csrc")
+    subprocess.run(["g++", "-std=c++17", "-O1", "-pthread", "-Wall", "-Wextra", "-Werror", os.path.join(ROOT, "tests", "ssd_io_check.cpp"),
+                    os.path.join(csrc, "ssd_io.cpp"), "-o", exe], check=True)
+    rng = np.random.default_rng(sector + kv_size)
+    stripe = rng.integers(0, 256, size=slots * kv_size, dtype=np.uint8)
+    first = 3
+    n_sec = oracle.lba_range_len(slots, kv_size, sector)
+    disk_path, fill = str(tmp_path / "disk.img"), 0xC3
+    with open(disk_path, "wb") as f:
+        f.write(bytes([fill]) * ((first + n_sec + 4) * sector))
+    stripe.tofile(str(tmp_path / "stripe.bin"))
+    cuts = sorted({0, slots, *[int(x) for x in rng.integers(1, slots, size=5)]})
+    spans = [f"{a}:{b}" for a, b in zip(cuts, cuts[1:])]
+    spans = [spans[i] for i in rng.permutation(len(spans))]                        # instalments arrive out of order
+    out = subprocess.run([exe, disk_path, str(sector), str(kv_size), str(first), str(lane_bytes), "3", str(tmp_path / "stripe.bin"),
+                          str(tmp_path / "out.bin")] + spans, capture_output=True, text=True, timeout=120)
+    assert out.returncode == 0 and out.stdout.startswith("ssd io ok"), out.stdout + out.stderr
+    want = np.full((first + n_sec + 4) * sector, fill, dtype=np.uint8)
+    assert oracle.ssd_direct_store(want, sector, first, stripe, kv_size) == n_sec
+    assert np.array_equal(np.fromfile(disk_path, dtype=np.uint8), want)             # every sector, padding and neighbours included
+    back = np.fromfile(str(tmp_path / "out.bin"), dtype=np.uint8)
+    for s in [0, slots - 1] + [int(x) for x in rng.integers(0, slots, size=16)]:
+        lba, off = oracle.ssd_location(first, s, kv_size, sector)
+        assert np.array_equal(back[s * kv_size:(s + 1) * kv_size], oracle.ssd_direct_retrieve(want, sector, lba, off, kv_size))
+    assert np.array_equal(back, stripe)
