@@ -78,7 +78,7 @@ def parse_args():
     ap.add_argument("--ssd-pool", action="store_true",
                     help="side mode: pools with SSD-type devices (KV-passthrough, PAPER.md:179-185) - files under --ssd-dir opened O_DIRECT stand in "
                          "for NVMe namespaces: one SSD alone, host memory + one SSD, host memory + two SSDs (the paper's mix); text table")
-    ap.add_argument("--ssd-dir", default="/dev/shm", help="--ssd-pool: directory that holds the stand-in files (or pass block devices, comma separated)")
+    ap.add_argument("--ssd-dir", default="/tmp", help="--ssd-pool: directory that holds the stand-in files (or pass block devices, comma separated)")
     ap.add_argument("--duplex", action="store_true",
                     help="offload of one request concurrent with retrieve of another (PCIe is full duplex): per-direction and aggregate "
                          "GB/s against simultaneous cudaMemcpyAsync in both directions")
@@ -1197,7 +1197,7 @@ def ssd_pool_lines(cfg: int, ssd_dir: str, kinds):
                    "offload_gbps": moved / statistics.median(offs) / 1e6, "retrieve_gbps": moved / statistics.median(rets) / 1e6,
                    "sum_of_weights_gbps": float(sum(bw)), "stores_per_leg": sum(i["stores"] - j["stores"] for i, j in zip(infos, before)) // 4,
                    "retrieves_per_leg": sum(i["retrieves"] - j["retrieves"] for i, j in zip(infos, before)) // 4,
-                   "direct_io": [i["direct_io"] for i in infos], "verified_bit_exact_round_trip": True}
+                   "direct_io": [i["direct_io"] for i in infos], "queue_depth": [i["queue_depth"] for i in infos], "verified_bit_exact_round_trip": True}
         finally:
             pool.destroy()
 
@@ -1213,12 +1213,12 @@ def run_ssd_pool(args) -> None:
     print(f"# bench.py --ssd-pool --config {args.config} --ssd-dir {args.ssd_dir}: {h['workload']} cut to {h['layers']} layers, {h['moved_bytes_per_leg'] / 2**20:.0f} MiB per leg "
           f"({h['blocks_per_layer']} blocks of {h['payload']} B per layer); SSD-type devices = {h['medium']}; "
           "weights = kvpool_calibrate (256 MiB per device, one link group); median of 3; 8 MiB commands on 4 lanes per device and direction")
-    print(f"{'pool':30s} {'weights (GB/s)':>20s} {'blocks per layer':>18s} {'offload GB/s':>12s} {'retrieve GB/s':>13s} {'sum of weights':>14s} {'of sum':>11s} {'stores':>7s} {'retrieves':>9s} {'direct':>6s}   (stores / retrieves: commands per leg)")
+    print(f"{'pool':30s} {'weights (GB/s)':>20s} {'blocks per layer':>18s} {'offload GB/s':>12s} {'retrieve GB/s':>13s} {'sum of weights':>14s} {'of sum':>11s} {'stores':>7s} {'retrieves':>9s} {'direct':>6s} {'depth':>5s}   (stores / retrieves: commands per leg; depth: commands in flight per device, io_uring)")
     for r in lines:
         sw = r["sum_of_weights_gbps"]
         print(f"{names[r['pool']]:30s} {'/'.join(f'{b:.1f}' for b in r['bandwidth_gbps']):>20s} {'/'.join(str(c) for c in r['blocks_per_layer']):>18s} "
               f"{r['offload_gbps']:12.2f} {r['retrieve_gbps']:13.2f} {sw:14.1f} {r['offload_gbps'] / sw:5.2f}/{r['retrieve_gbps'] / sw:5.2f} "
-              f"{r['stores_per_leg']:7d} {r['retrieves_per_leg']:9d} {'/'.join('yes' if d else 'no' for d in r['direct_io']) or '-':>6s}", flush=True)
+              f"{r['stores_per_leg']:7d} {r['retrieves_per_leg']:9d} {'/'.join('yes' if d else 'no' for d in r['direct_io']) or '-':>6s} {'/'.join(str(q) for q in r['queue_depth']) or '-':>5s}", flush=True)
 
 
 def run_duplex(args) -> None:

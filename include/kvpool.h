@@ -387,12 +387,14 @@ KVPOOL_API int kvpool_stripe_read(kvpool_t* pool, const kvpool_placement_t* pl, 
  *   byte inside that sector (0 whenever P is a multiple of the sector size).  EINVAL if the block's device is not SSD.
  * kvpool_ssd_info: sector size, whether the device is open with direct I/O (0 = the file system refused O_DIRECT and
  *   the library fell back to buffered I/O), whether it is a block device (0 = a file standing in for one), and the
- *   store / retrieve commands its worker has completed.  Any out pointer may be NULL.                               */
+ *   store / retrieve commands its worker has completed, and how many commands the worker keeps in flight on the device
+ *   (io_uring; 1 = the synchronous fall-back, 0 = no worker yet: it starts with the first kvpool_place or measurement).
+ *   Any out pointer may be NULL.                                                                                   */
 KVPOOL_API int kvpool_ssd_range(const kvpool_placement_t* pl, uint32_t layer, uint32_t dev, uint64_t* first_lba, uint64_t* n_sectors,
                      uint32_t* sector_bytes);
 KVPOOL_API int kvpool_ssd_location(const kvpool_placement_t* pl, uint32_t layer, uint32_t block, uint64_t* lba, uint32_t* byte_in_sector);
 KVPOOL_API int kvpool_ssd_info(const kvpool_t* pool, uint32_t dev, uint32_t* sector_bytes, int32_t* direct_io, int32_t* block_device,
-                    uint64_t* stores_completed, uint64_t* retrieves_completed);
+                    uint64_t* stores_completed, uint64_t* retrieves_completed, uint32_t* queue_depth);
 
 /* Keyed GLT (Table I `key` = "hash of the KV cache identifier"): give the K_l KV caches of a layer
  * caller-chosen 64-bit identifiers (e.g. the prefix-hash of the tokens a block covers, mixed with the layer), after

@@ -78,7 +78,7 @@ def lib():
             "kvpool_plan_lba_range": [c_uint64, c_uint64, c_uint32, POINTER(c_uint64)],
             "kvpool_ssd_range": [vp, c_uint32, c_uint32, POINTER(c_uint64), POINTER(c_uint64), POINTER(c_uint32)],
             "kvpool_ssd_location": [vp, c_uint32, c_uint32, POINTER(c_uint64), POINTER(c_uint32)],
-            "kvpool_ssd_info": [vp, c_uint32, POINTER(c_uint32), POINTER(c_int32), POINTER(c_int32), POINTER(c_uint64), POINTER(c_uint64)],
+            "kvpool_ssd_info": [vp, c_uint32, POINTER(c_uint32), POINTER(c_int32), POINTER(c_int32), POINTER(c_uint64), POINTER(c_uint64), POINTER(c_uint32)],
             "kvpool_validate_table": [vp, c_uint64, c_uint64],
             "kvpool_set_table_check": [vp, c_uint64],
             "kvpool_table_errors": [vp, vp],
@@ -461,9 +461,10 @@ class KvPool:
         return t.value, g.value
 
     def ssd_info(self, dev: int) -> dict:
-        sec, direct, blk, st, rt = c_uint32(), c_int32(), c_int32(), c_uint64(), c_uint64()
-        _ck(lib().kvpool_ssd_info(self.handle, dev, byref(sec), byref(direct), byref(blk), byref(st), byref(rt)))
-        return {"sector_bytes": sec.value, "direct_io": bool(direct.value), "block_device": bool(blk.value), "stores": st.value, "retrieves": rt.value}
+        sec, direct, blk, st, rt, qd = c_uint32(), c_int32(), c_int32(), c_uint64(), c_uint64(), c_uint32()
+        _ck(lib().kvpool_ssd_info(self.handle, dev, byref(sec), byref(direct), byref(blk), byref(st), byref(rt), byref(qd)))
+        return {"sector_bytes": sec.value, "direct_io": bool(direct.value), "block_device": bool(blk.value), "stores": st.value, "retrieves": rt.value,
+                "queue_depth": qd.value}
 
     def set_table_check(self, nphys: int) -> None:
         _ck(lib().kvpool_set_table_check(self.handle, int(nphys)))

@@ -880,7 +880,8 @@ int kvpool_ssd_location(const kvpool_placement_t* pl, uint32_t layer, uint32_t b
   return KVPOOL_OK;
 }
 
-int kvpool_ssd_info(const kvpool_t* p, uint32_t dev, uint32_t* sector_bytes, int32_t* direct_io, int32_t* block_device, uint64_t* stores, uint64_t* retrieves) {
+int kvpool_ssd_info(const kvpool_t* p, uint32_t dev, uint32_t* sector_bytes, int32_t* direct_io, int32_t* block_device, uint64_t* stores, uint64_t* retrieves,
+                    uint32_t* queue_depth) {
   if (!p || dev >= p->n) return fail(KVPOOL_EINVAL, "ssd_info: bad arguments");
   if (!is_ssd(p, dev)) return fail(KVPOOL_EINVAL, "ssd_info: pool device %u is not an SSD-type device", dev);
   const SsdDevice& io = p->ssd[dev]->io;
@@ -889,6 +890,7 @@ int kvpool_ssd_info(const kvpool_t* p, uint32_t dev, uint32_t* sector_bytes, int
   if (block_device) *block_device = io.block_device();
   if (stores) *stores = io.completed(1);
   if (retrieves) *retrieves = io.completed(0);
+  if (queue_depth) *queue_depth = io.running() ? io.queue_depth() : 0;
   return KVPOOL_OK;
 }
 

@@ -5,7 +5,10 @@
 #include <errno.h>
 #include <fcntl.h>
 #include <linux/fs.h>
+#include <linux/io_uring.h>
 #include <sys/ioctl.h>
+#include <sys/mman.h>
+#include <sys/syscall.h>
 #include <sys/stat.h>
 #include <time.h>
 #include <unistd.h>
@@ -28,6 +31,100 @@ bool lba_range_len(uint64_t set_size, uint64_t kv_size, uint64_t sector, uint64_
   return true;
 }
 
+// ---- io_uring with raw system calls ----------------------------------------------------------------------------------
+bool Uring::open(unsigned entries) {
+  close();
+  io_uring_params prm;
+  memset(&prm, 0, sizeof prm);
+  fd_ = static_cast<int>(syscall(__NR_io_uring_setup, entries, &prm));
+  if (fd_ < 0) { fd_ = -1; return false; }
+  entries_ = prm.sq_entries;
+  sq_ring_bytes_ = prm.sq_off.array + prm.sq_entries * sizeof(unsigned);
+  cq_ring_bytes_ = prm.cq_off.cqes + prm.cq_entries * sizeof(io_uring_cqe);
+  const bool single = prm.features & IORING_FEAT_SINGLE_MMAP;
+  if (single) sq_ring_bytes_ = cq_ring_bytes_ = std::max(sq_ring_bytes_, cq_ring_bytes_);
+  sq_ring_ = mmap(nullptr, sq_ring_bytes_, PROT_READ | PROT_WRITE, MAP_SHARED | MAP_POPULATE, fd_, IORING_OFF_SQ_RING);
+  cq_ring_ = single ? sq_ring_ : mmap(nullptr, cq_ring_bytes_, PROT_READ | PROT_WRITE, MAP_SHARED | MAP_POPULATE, fd_, IORING_OFF_CQ_RING);
+  sqes_bytes_ = prm.sq_entries * sizeof(io_uring_sqe);
+  sqes_ = mmap(nullptr, sqes_bytes_, PROT_READ | PROT_WRITE, MAP_SHARED | MAP_POPULATE, fd_, IORING_OFF_SQES);
+  if (sq_ring_ == MAP_FAILED || cq_ring_ == MAP_FAILED || sqes_ == MAP_FAILED) {
+    if (sq_ring_ == MAP_FAILED) sq_ring_ = nullptr;
+    if (cq_ring_ == MAP_FAILED) cq_ring_ = nullptr;
+    if (sqes_ == MAP_FAILED) sqes_ = nullptr;
+    close();
+    return false;
+  }
+  auto at = [](void* base, unsigned off) { return reinterpret_cast<unsigned*>(static_cast<char*>(base) + off); };
+  sq_head_ = at(sq_ring_, prm.sq_off.head);
+  sq_tail_ = at(sq_ring_, prm.sq_off.tail);
+  sq_mask_ = at(sq_ring_, prm.sq_off.ring_mask);
+  sq_array_ = at(sq_ring_, prm.sq_off.array);
+  cq_head_ = at(cq_ring_, prm.cq_off.head);
+  cq_tail_ = at(cq_ring_, prm.cq_off.tail);
+  cq_mask_ = at(cq_ring_, prm.cq_off.ring_mask);
+  cqes_ = static_cast<char*>(cq_ring_) + prm.cq_off.cqes;
+  to_submit_ = 0;
+  return true;
+}
+
+void Uring::close() {
+  if (sqes_) munmap(sqes_, sqes_bytes_);
+  if (cq_ring_ && cq_ring_ != sq_ring_) munmap(cq_ring_, cq_ring_bytes_);
+  if (sq_ring_) munmap(sq_ring_, sq_ring_bytes_);
+  sqes_ = cq_ring_ = sq_ring_ = nullptr;
+  if (fd_ >= 0) ::close(fd_);
+  fd_ = -1;
+}
+
+bool Uring::queue(bool write, int file, void* buf, uint32_t len, uint64_t off, uint64_t user_data) {
+  const unsigned tail = *sq_tail_, head = __atomic_load_n(sq_head_, __ATOMIC_ACQUIRE);
+  if (tail - head >= entries_) return false;
+  const unsigned idx = tail & *sq_mask_;
+  io_uring_sqe* e = static_cast<io_uring_sqe*>(sqes_) + idx;
+  memset(e, 0, sizeof *e);
+  e->opcode = write ? IORING_OP_WRITE : IORING_OP_READ;
+  e->fd = file;
+  e->off = off;
+  e->addr = reinterpret_cast<uint64_t>(buf);
+  e->len = len;
+  e->user_data = user_data;
+  sq_array_[idx] = idx;
+  __atomic_store_n(sq_tail_, tail + 1, __ATOMIC_RELEASE);
+  ++to_submit_;
+  return true;
+}
+
+int Uring::flush() {
+  while (to_submit_) {
+    const long r = syscall(__NR_io_uring_enter, fd_, to_submit_, 0, 0, nullptr, 0);
+    if (r < 0) {
+      if (errno == EINTR || errno == EAGAIN || errno == EBUSY) continue;
+      return errno;
+    }
+    to_submit_ -= static_cast<unsigned>(r);
+  }
+  return 0;
+}
+
+bool Uring::reap(uint64_t* user_data, int32_t* res) {
+  const unsigned head = *cq_head_;
+  if (head == __atomic_load_n(cq_tail_, __ATOMIC_ACQUIRE)) return false;
+  const io_uring_cqe* c = static_cast<const io_uring_cqe*>(cqes_) + (head & *cq_mask_);
+  *user_data = c->user_data;
+  *res = c->res;
+  __atomic_store_n(cq_head_, head + 1, __ATOMIC_RELEASE);
+  return true;
+}
+
+int Uring::wait_one() {
+  for (;;) {
+    const long r = syscall(__NR_io_uring_enter, fd_, 0, 1, IORING_ENTER_GETEVENTS, nullptr, 0);
+    if (r >= 0) return 0;
+    if (errno != EINTR) return errno;
+  }
+}
+
+// ---- the device ------------------------------------------------------------------------------------------------------
 int SsdDevice::open(const char* path, uint64_t capacity, uint32_t sector, std::string* err) {
   close();
   if (!path || !*path) { *err = "an SSD-type pool device needs a path (block device or file)"; return KVPOOL_EINVAL; }
@@ -96,7 +193,10 @@ void SsdDevice::start(uint32_t n_lanes, uint64_t lane_bytes, uint8_t* const boun
   stride_ = stride;
   for (int d = 0; d < 2; ++d) { bounce_[d] = bounce[d]; gpu_seq_[d] = gpu_seq[d]; cpu_seq_[d] = cpu_seq[d]; }
   stopping_ = false;
-  worker_ = std::thread([this] { run(); });
+  const char* sync = getenv("KVPOOL_SSD_SYNC");
+  depth_ = 1;
+  if (!(sync && *sync == '1') && ring_.open(std::max(8u, 4 * n_lanes))) depth_ = std::max(2u, 2 * n_lanes);
+  worker_ = depth_ > 1 ? std::thread([this] { run_async(); }) : std::thread([this] { run(); });
 }
 
 void SsdDevice::stop() {
@@ -108,6 +208,7 @@ void SsdDevice::stop() {
   }
   cv_.notify_all();
   worker_.join();
+  ring_.close();
 }
 
 void SsdDevice::submit(const SsdCmd& c) {
@@ -157,40 +258,55 @@ int SsdDevice::rw_full(bool write, uint64_t off, uint8_t* buf, uint64_t n) {
   return 0;
 }
 
-void SsdDevice::execute(const SsdCmd& c) {
+bool SsdDevice::gpu_half_arrived(const SsdCmd& c) const {
   const int d = c.op == SsdCmd::kWrite ? 1 : 0;
-  uint8_t* const buf = bounce_[d] + static_cast<uint64_t>(c.lane) * lane_bytes_;
-  volatile uint32_t* const gpu = gpu_seq_[d] + static_cast<uint64_t>(c.lane) * stride_;
-  volatile uint32_t* const cpu = cpu_seq_[d] + static_cast<uint64_t>(c.lane) * stride_;
+  const volatile uint32_t* gpu = gpu_seq_[d] + static_cast<uint64_t>(c.lane) * stride_;
+  // a store needs the GPU's copy into the lane (gpu_seq >= use); a retrieve needs the lane drained of its previous use
+  return seq_reached(gpu, c.op == SsdCmd::kWrite ? c.use : c.use - 1);
+}
+
+int SsdDevice::prepare_store(const SsdCmd& c) {
+  uint8_t* const buf = bounce_[1] + static_cast<uint64_t>(c.lane) * lane_bytes_;
   const uint64_t body = c.head + c.len, total = (body + sector_ - 1) / sector_ * sector_;
   int e = 0;
-  if (total > lane_bytes_ || c.file_off % sector_ || c.file_off + total > capacity_) e = EINVAL;
-  if (c.op == SsdCmd::kRead) {
-    // SSD_Direct_Retrieve: the lane is free once the GPU has drained its previous use; read the LBA range into it
-    if (!wait_flag(gpu, c.use - 1)) e = e ? e : (abort_.load() ? ECANCELED : ETIMEDOUT);
-    if (!e) e = rw_full(false, c.file_off, buf, total);
-  } else {
-    // SSD_Direct_Store: wait for the GPU's copy into the lane, complete the first / last sector, write the LBA range
-    if (!wait_flag(gpu, c.use)) e = e ? e : (abort_.load() ? ECANCELED : ETIMEDOUT);
-    if (!e && c.head) {  // the range starts inside a sector that holds a neighbour's bytes: keep them
-      e = rw_full(false, c.file_off, edge_, sector_);
-      if (!e) memcpy(buf, edge_, c.head);
-    }
-    if (!e && total > body) {
-      if (c.zero_tail) memset(buf + body, 0, total - body);
-      else {
-        e = rw_full(false, c.file_off + total - sector_, edge_, sector_);
-        if (!e) memcpy(buf + body, edge_ + (sector_ - (total - body)), total - body);
-      }
-    }
-    if (!e) e = rw_full(true, c.file_off, buf, total);
+  if (c.head) {  // the range starts inside a sector that holds a neighbour's bytes: keep them
+    e = rw_full(false, c.file_off, edge_, sector_);
+    if (!e) memcpy(buf, edge_, c.head);
   }
+  if (!e && total > body) {
+    if (c.zero_tail) memset(buf + body, 0, total - body);
+    else {
+      e = rw_full(false, c.file_off + total - sector_, edge_, sector_);
+      if (!e) memcpy(buf + body, edge_ + (sector_ - (total - body)), total - body);
+    }
+  }
+  return e;
+}
+
+void SsdDevice::complete(const SsdCmd& c, int e) {
+  const int d = c.op == SsdCmd::kWrite ? 1 : 0;
   if (e) {
     int none = 0;
     error_.compare_exchange_strong(none, e);
   }
-  __atomic_store_n(cpu, c.use, __ATOMIC_RELEASE);  // the handshake completes even on failure: no stream waits for ever
+  // the hand-over completes even on failure: no stream waits for ever
+  __atomic_store_n(cpu_seq_[d] + static_cast<uint64_t>(c.lane) * stride_, c.use, __ATOMIC_RELEASE);
   done_[d].fetch_add(1);
+}
+
+void SsdDevice::execute(const SsdCmd& c) {
+  const int d = c.op == SsdCmd::kWrite ? 1 : 0;
+  uint8_t* const buf = bounce_[d] + static_cast<uint64_t>(c.lane) * lane_bytes_;
+  volatile uint32_t* const gpu = gpu_seq_[d] + static_cast<uint64_t>(c.lane) * stride_;
+  const uint64_t body = c.head + c.len, total = (body + sector_ - 1) / sector_ * sector_;
+  int e = 0;
+  if (total > lane_bytes_ || c.file_off % sector_ || c.file_off + total > capacity_) e = EINVAL;
+  // SSD_Direct_Retrieve: the lane is free once the GPU has drained its previous use; read the LBA range into it.
+  // SSD_Direct_Store: wait for the GPU's copy into the lane, complete the first / last sector, write the LBA range.
+  if (!wait_flag(gpu, c.op == SsdCmd::kWrite ? c.use : c.use - 1)) e = e ? e : (abort_.load() ? ECANCELED : ETIMEDOUT);
+  if (!e && c.op == SsdCmd::kWrite) e = prepare_store(c);
+  if (!e) e = rw_full(c.op == SsdCmd::kWrite, c.file_off, buf, total);
+  complete(c, e);
 }
 
 void SsdDevice::run() {
@@ -209,6 +325,117 @@ void SsdDevice::run() {
       ++finished_;
     }
     cv_done_.notify_all();
+  }
+}
+
+// The asynchronous worker.  Commands leave the queue in submission order into a small window (`depth_`); a command's disk
+// I/O is submitted to the ring as soon as the GPU's half has arrived AND no earlier command still in the window touches
+// the same sectors with a write on either side (a retrieve after a store of the same range, a store's read-modify-write of
+// a sector it shares with its neighbour); completions are reaped from the ring in whatever order the device finishes them.
+struct SsdDevice::Active {
+  SsdCmd c;
+  uint64_t lo, hi;  // byte range of whole sectors the command touches
+  uint64_t id;
+  enum { kWaiting, kInFlight } state;
+  std::chrono::steady_clock::time_point since;
+};
+
+void SsdDevice::run_async() {
+  std::vector<Active> win;
+  uint64_t next_id = 1;
+  unsigned idle = 0;
+  for (;;) {
+    bool progress = false;
+    {  // take commands off the queue, in order, while the window has room
+      std::unique_lock<std::mutex> l(mu_);
+      if (win.empty()) {
+        cv_.wait(l, [this] { return stopping_ || !q_.empty(); });
+        if (q_.empty()) return;
+      }
+      while (!q_.empty() && win.size() < depth_) {
+        Active a;
+        a.c = q_.front();
+        q_.pop_front();
+        const uint64_t total = (a.c.head + a.c.len + sector_ - 1) / sector_ * sector_;
+        a.lo = a.c.file_off;
+        a.hi = a.c.file_off + total;
+        a.id = next_id++;
+        a.state = Active::kWaiting;
+        a.since = std::chrono::steady_clock::now();
+        win.push_back(a);
+        progress = true;
+      }
+    }
+    unsigned finished = 0;
+    for (size_t k = 0; k < win.size(); ++k) {
+      Active& a = win[k];
+      if (a.state != Active::kWaiting) continue;
+      bool blocked = false;  // an earlier command of the window overlaps and one of the two writes
+      for (size_t j = 0; j < k && !blocked; ++j)
+        blocked = win[j].lo < a.hi && a.lo < win[j].hi && (win[j].c.op == SsdCmd::kWrite || a.c.op == SsdCmd::kWrite);
+      if (blocked) continue;
+      int e = 0;
+      const uint64_t total = a.hi - a.lo;
+      if (total > lane_bytes_ || a.lo % sector_ || a.hi > capacity_ || total > 0x7fffffffull) e = EINVAL;
+      if (!e && !gpu_half_arrived(a.c)) {
+        if (abort_.load(std::memory_order_relaxed)) e = ECANCELED;
+        else if (std::chrono::steady_clock::now() - a.since > std::chrono::minutes(10)) e = ETIMEDOUT;
+        else continue;
+      }
+      const int d = a.c.op == SsdCmd::kWrite ? 1 : 0;
+      uint8_t* const buf = bounce_[d] + static_cast<uint64_t>(a.c.lane) * lane_bytes_;
+      if (!e && d == 1) e = prepare_store(a.c);
+      if (!e && !ring_.queue(d == 1, fd_, buf, static_cast<uint32_t>(total), a.lo, a.id)) continue;  // ring full: next round
+      progress = true;
+      if (e) {
+        complete(a.c, e);
+        a.id = 0;  // done
+        ++finished;
+      } else {
+        a.state = Active::kInFlight;
+      }
+    }
+    if (int e = ring_.flush()) {  // the kernel refused the submission: fail what was queued
+      for (auto& a : win)
+        if (a.state == Active::kInFlight) { complete(a.c, e); a.id = 0; ++finished; }
+    }
+    uint64_t id;
+    int32_t res;
+    while (ring_.reap(&id, &res)) {
+      progress = true;
+      for (auto& a : win) {
+        if (a.id != id || a.state != Active::kInFlight) continue;
+        int e = res < 0 ? -res : 0;
+        const uint64_t total = a.hi - a.lo;
+        if (!e && static_cast<uint64_t>(res) < total) {  // short transfer: finish it synchronously
+          const int d = a.c.op == SsdCmd::kWrite ? 1 : 0;
+          uint8_t* const buf = bounce_[d] + static_cast<uint64_t>(a.c.lane) * lane_bytes_;
+          e = res == 0 ? EIO : rw_full(d == 1, a.lo + static_cast<uint64_t>(res), buf + res, total - static_cast<uint64_t>(res));
+        }
+        complete(a.c, e);
+        a.id = 0;
+        ++finished;
+        break;
+      }
+    }
+    if (finished) {
+      win.erase(std::remove_if(win.begin(), win.end(), [](const Active& a) { return a.id == 0; }), win.end());
+      {
+        std::lock_guard<std::mutex> l(mu_);
+        finished_ += finished;
+      }
+      cv_done_.notify_all();
+    }
+    if (progress) { idle = 0; continue; }
+    // nothing moved: every command of the window waits for the GPU or for the disk
+    bool waiting_for_gpu = false;
+    for (auto& a : win) waiting_for_gpu |= a.state == Active::kWaiting;
+    if (!waiting_for_gpu && !win.empty()) { ring_.wait_one(); continue; }  // only the disk: sleep in the kernel until it completes one
+    if (++idle < 2048) __builtin_ia32_pause();
+    else {
+      const timespec nap{0, 20000};
+      nanosleep(&nap, nullptr);
+    }
   }
 }
 

@@ -1,7 +1,11 @@
 // KV-passthrough, host side: one SSD-type pool device = a block device (or a file standing in for one)
 // opened O_DIRECT and addressed by LBA, a queue of asynchronous store / retrieve commands, and the device's own worker
 // thread ("each pool device has its own worker thread") that polls for the GPU's half of each command and
-// completes it with pread / pwrite — submission (the API call) is decoupled from completion (the worker).
+// completes it — submission (the API call) is decoupled from completion (the worker).  The worker drives the disk through
+// an io_uring of its own (raw system calls, no liburing): it submits the read / write of every command whose GPU half has
+// arrived and reaps completions from the ring, so that several commands of one device are in flight at once (as many as
+// it has lanes) while commands that touch the same sectors keep their order; where the kernel has no io_uring (or with
+// KVPOOL_SSD_SYNC=1 in the environment) it falls back to one synchronous pread / pwrite at a time.
 // Pure C++17, no CUDA: the bounce memory and the GPU<->CPU sequence flags are handed in by kvpool_ssd.cu.
 #pragma once
 #include <atomic>
@@ -11,6 +15,7 @@
 #include <mutex>
 #include <string>
 #include <thread>
+#include <vector>
 
 namespace kvp {
 
@@ -30,6 +35,28 @@ struct SsdCmd {
   uint64_t file_off;  // byte offset of the first sector touched (a multiple of the sector size)
   uint32_t head;      // the payload starts `head` bytes into that sector (0 whenever KV_size is a multiple of the sector)
   uint64_t len;       // payload bytes, at bounce + head
+};
+
+// The kernel's asynchronous I/O rings, set up and driven with raw system calls (io_uring_setup / io_uring_enter + mmap).
+class Uring {
+ public:
+  ~Uring() { close(); }
+  bool open(unsigned entries);  // false: io_uring is not available here
+  void close();
+  bool ok() const { return fd_ >= 0; }
+  // queue one read / write of `len` bytes (false: the submission ring is full); flush() hands queued entries to the kernel
+  bool queue(bool write, int file, void* buf, uint32_t len, uint64_t off, uint64_t user_data);
+  int flush();
+  bool reap(uint64_t* user_data, int32_t* res);  // one completion, if any
+  int wait_one();                                // sleep in the kernel until a completion is there
+ private:
+  int fd_ = -1;
+  unsigned entries_ = 0, to_submit_ = 0;
+  void *sq_ring_ = nullptr, *cq_ring_ = nullptr, *sqes_ = nullptr;
+  size_t sq_ring_bytes_ = 0, cq_ring_bytes_ = 0, sqes_bytes_ = 0;
+  unsigned *sq_head_ = nullptr, *sq_tail_ = nullptr, *sq_mask_ = nullptr, *sq_array_ = nullptr;
+  unsigned *cq_head_ = nullptr, *cq_tail_ = nullptr, *cq_mask_ = nullptr;
+  void* cqes_ = nullptr;
 };
 
 class SsdDevice {
@@ -62,9 +89,15 @@ class SsdDevice {
   bool block_device() const { return blockdev_; }
   uint64_t completed(int write) const { return done_[write ? 1 : 0].load(); }
   bool running() const { return worker_.joinable(); }
+  unsigned queue_depth() const { return depth_; }  // commands the worker keeps in flight (1 = the synchronous fall-back)
 
  private:
   void run();
+  void run_async();
+  struct Active;  // a command the asynchronous worker has taken off the queue
+  bool gpu_half_arrived(const SsdCmd& c) const;
+  int prepare_store(const SsdCmd& c);  // first / last sector of a store: keep the neighbours' bytes, or zero the padding
+  void complete(const SsdCmd& c, int err);
   bool wait_flag(const volatile uint32_t* f, uint32_t v);
   int rw_full(bool write, uint64_t off, uint8_t* buf, uint64_t n);
   void execute(const SsdCmd& c);
@@ -88,6 +121,8 @@ class SsdDevice {
   bool stopping_ = false;
   std::atomic<int> error_{0};
   std::atomic<bool> abort_{false};
+  Uring ring_;
+  unsigned depth_ = 1;
   std::atomic<uint64_t> done_[2] = {{0}, {0}};
 };
 

@@ -169,6 +169,7 @@ def test_host_memory_plus_ssd_pool_llama_1k(tmp_path, path, kernel):
     assert out["ssd_bytes"] == 4 * 21 * wl.geom.payload              # device 1 holds 21 of the 64 blocks of every layer
     info = out["info"][1]
     assert info["sector_bytes"] == 512 and not info["block_device"] and info["stores"] >= 4 and info["retrieves"] >= 4
+    assert info["queue_depth"] in (1, 8)                             # io_uring with 2 x 4 lanes in flight, or the synchronous fall-back
 
 
 @pytest.mark.parametrize("sector", [512, 4096])
@@ -453,3 +454,12 @@ def test_full_size_config4_with_two_ssd_devices_every_byte_against_oracle(tmp_pa
         pl.release()
     finally:
         pool.destroy()
+
+
+def test_synchronous_fallback_of_the_worker(tmp_path, monkeypatch):
+    """KVPOOL_SSD_SYNC=1 (or a kernel without io_uring): one pread / pwrite at a time instead of a ring of commands in flight;
+    same bytes."""
+    monkeypatch.setenv("KVPOOL_SSD_SYNC", "1")
+    wl = W.make_workload(1, n_layers=2)
+    out = _run(wl, ["mem", "ssd"], tmp_path, tuning={"ssd_lanes": 2, "ssd_chunk_bytes": 256 << 10})
+    assert out["info"][1]["queue_depth"] == 1
