@@ -69,8 +69,9 @@ enum {
                                         file standing in for one.  It is opened O_DIRECT - the kernel's page cache and the
                                         file system's data path are bypassed; on a raw block device there is no file system
                                         at all - and driven by the device's own worker thread through asynchronous store /
-                                        retrieve commands; GPU streams and the worker hand bounce lanes to each other with
-                                        stream write-value / wait-value operations, no host callback and no
+                                        retrieve commands (io_uring); the pack / unpack kernels reach the pinned bounce lanes
+                                        over the link, and GPU streams and the worker hand lanes to each other with stream
+                                        write-value / wait-value operations: no copy engine, no host callback, no
                                         synchronisation.  Excludes every other flag.               */
 
 #define KVPOOL_MEASURE_KERNEL_RETRIEVE 2 /* kvpool_measure_bandwidth / kvpool_calibrate `direction`, see there */
@@ -126,8 +127,8 @@ typedef struct {           /* one pool device (Table I)           
                            /* resource: copies that share a link only slow each other down, and layer   */
                            /* l+1's copies would delay layer l's), and kvpool_calibrate divides what    */
                            /* they share.  Placement (Eq. 1-2) is untouched: only b_i changes.  An SSD-   */
-                           /* type device always has I/O streams of its own (a stream that waits for a   */
-                           /* disk must not hold up the copies of a host buffer)                         */
+                           /* type device moves its share on kernel streams of its own, whatever its     */
+                           /* group (a stream that waits for a disk must hold up nothing else)           */
   const char* path;        /* SSD: block device or file (host string, copied); NULL otherwise           */
   uint32_t sector_bytes;   /* SSD: sector size LBAs count in - a power of two in 512..65536 and a       */
                            /* multiple of the device's logical sector; 0 = ask the block device, 4096   */
@@ -162,7 +163,8 @@ typedef struct {         /* kvpool_set_tuning; 0 in any field = library default 
   uint32_t pdl;          /* programmatic dependent launch of the library's kernels (the next layer's launch latency and
                             ramp hide under the current layer's kernel): 1 = on (default), 2 = off                          */
   uint32_t ssd_lanes;    /* SSD-type devices: bounce lanes per device and direction (default 4): a lane is one store /
-                            retrieve command in flight - pinned host memory for the disk's DMA plus a device staging piece */
+                            retrieve command in flight - pinned, GPU-mapped host memory: the disk's DMA target on one side,
+                            read / written by the pack / unpack kernel over the link on the other                          */
   uint64_t ssd_chunk_bytes; /* SSD-type devices: bytes per command (default 8 MiB; at least one KV cache plus two sectors).
                             ssd_lanes / ssd_chunk_bytes are fixed by the first kvpool_place: ESTATE afterwards           */
 } kvpool_tuning;

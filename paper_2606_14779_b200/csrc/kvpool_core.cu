@@ -171,9 +171,10 @@ LayerArgs base_args(const kvpool* p, const LayerState& L, const void* k_base, co
 }
 
 
-LaunchCfg launch_cfg(const kvpool* p, bool link_bound, bool pack) {
+LaunchCfg launch_cfg(const kvpool* p, bool link_bound, bool pack, bool lane) {
   // a zero-copy launch over a pool with HBM devices moves most of its bytes at HBM / NVLink rates: give it the HBM grid
-  if (p->hbm_mask) link_bound = false;
+  // (not a launch on an SSD-type device's lane: that one touches nothing but the lane's mapped host memory)
+  if (p->hbm_mask && !lane) link_bound = false;
   LaunchCfg c{};
   c.kernel = link_bound ? p->tune.link_kernel : p->tune.kernel;
   c.ctas = link_bound ? p->tune.link_ctas : p->tune.hbm_ctas;

@@ -83,7 +83,7 @@ int prof_end(kvpool* p, ProfRec* r, cudaStream_t s) {
 }  // namespace
 
 // Launch one layer kernel, counted and (when profiling) bracketed by an event pair.
-int launch_counted(kvpool* p, const LayerArgs& a, bool pack, bool link_bound, cudaStream_t s) {
+int launch_counted(kvpool* p, const LayerArgs& a, bool pack, bool link_bound, cudaStream_t s, bool lane) {
   ProfRec r;
   if (p->profiling) {
     r.bytes = static_cast<uint64_t>(a.K) * p->payload;
@@ -93,7 +93,7 @@ int launch_counted(kvpool* p, const LayerArgs& a, bool pack, bool link_bound, cu
   }
   LayerArgs timed = a;
   if (p->profiling) timed.span = take_span(p, &r);
-  CU(launch_layer_copy(timed, pack, launch_cfg(p, link_bound, pack), s));
+  CU(launch_layer_copy(timed, pack, launch_cfg(p, link_bound, pack, lane), s));
   p->n_kernels++;
   if (p->profiling) return prof_end(p, &r, s);
   return KVPOOL_OK;

@@ -104,25 +104,27 @@ struct StageSlot {
   std::vector<cudaEvent_t> copy_done;         // [N] last memcpy per pool stream that read/wrote the slot
 };
 
-// One store / retrieve command in flight on an SSD-type device: pinned bounce memory for the disk's DMA, a device staging
-// piece of the same size for the pack / unpack kernel, and the events that recycle them.
+// One store / retrieve command in flight on an SSD-type device: pinned, GPU-mapped bounce memory — the disk's DMA target on
+// one side, read / written by the pack / unpack kernel over the link on the other.
 struct SsdLane {
-  uint8_t* bounce = nullptr;
-  uint8_t* stage = nullptr;
-  cudaEvent_t copy_done = nullptr;    // last copy between stage and bounce
-  cudaEvent_t kernel_done = nullptr;  // last kernel that read / wrote stage
+  uint8_t* bounce = nullptr;          // CPU address (the worker's pread / pwrite buffer)
+  uint8_t* bounce_dev = nullptr;      // the GPU's address of the same bytes
   uint32_t uses = 0;                  // sequence number of the lane's latest use (the value its flags are compared with)
 };
 struct SsdState {  // one SSD-type pool device (KV-passthrough)
   SsdDevice io;
-  uint8_t* bounce_base = nullptr;  // pinned host memory: [direction][lane] x lane_bytes
-  uint8_t* stage_base = nullptr;   // device memory, same layout
+  uint8_t* bounce_base = nullptr;  // pinned + mapped host memory: [direction][lane] x lane_bytes
   uint32_t* flags = nullptr;       // pinned + mapped: per direction and lane, gpu_seq (written by a stream write-value, polled
   uint64_t flags_dev = 0;          // by the worker) and cpu_seq (written by the worker, awaited by a stream wait-value)
   uint64_t lane_bytes = 0;
   uint32_t n_lanes = 0;
   std::vector<SsdLane> lane[2];    // [0] retrieve (SSD -> GPU), [1] offload (GPU -> SSD)
   uint32_t cursor[2] = {0, 0};
+  // The device's pack / unpack launches run on streams of its own, forked from and joined back to the caller's stream: a
+  // launch that waits for a lane (i.e. for the disk) must not hold up the faster devices' launches queued behind it
+  cudaStream_t kstream[2] = {nullptr, nullptr};
+  cudaEvent_t fork[2] = {nullptr, nullptr}, join[2] = {nullptr, nullptr};
+  bool join_pending = false;       // a batched offload joins its pack launches once, at the end of the call
   uint8_t* scratch = nullptr;      // aligned host memory for kvpool_stripe_read / kvpool_measure_bandwidth
 };
 constexpr uint64_t kSsdScratchBytes = 4ull << 20;
@@ -172,6 +174,7 @@ struct kvpool {
   std::vector<kvp::HostBuffer> bufs;
   std::vector<uint32_t> link_group;  // [N] kvpool_device_desc.link_group: devices of one group share io / io_out streams
   std::vector<cudaStream_t> own_streams;  // every stream created for io / io_out, once (members of a group alias one)
+  bool ssd_defer_join = false;  // inside kvpool_offload_layers: see SsdState::join_pending
   uint32_t ssd_mask = 0;  // bit i: pool device i is block storage (KVPOOL_DEV_SSD): its share of a layer moves through bounce lanes
   std::vector<std::unique_ptr<kvp::SsdState>> ssd;  // [N], null for the other types
   uint32_t hbm_mask = 0;  // bit i: pool device i is GPU memory (KVPOOL_DEV_HBM): reached by the kernels directly, never staged or copied
@@ -222,12 +225,12 @@ void destroy_placement(kvpool* p, kvpool_placement* pl);
 int check_layer_call(kvpool* p, kvpool_placement* pl, uint32_t layer, const void* k_base, const void* v_base, uint64_t stride,
                      const int32_t* table);
 LayerArgs base_args(const kvpool* p, const LayerState& L, const void* k_base, const void* v_base, uint64_t stride, const int32_t* table);
-LaunchCfg launch_cfg(const kvpool* p, bool link_bound, bool pack = false);
+LaunchCfg launch_cfg(const kvpool* p, bool link_bound, bool pack = false, bool lane = false);
 bool use_staged(const kvpool* p, bool pack, uint64_t host_bytes);
 int wait_slot_free(kvpool* p, StageSlot& slot, cudaStream_t s);
 void settle_landed(LayerState& L);
 // kvpool_dev.cu: launches counted for kvpool_stats and, while profiling is on, bracketed by an event pair and a device-clock span
-int launch_counted(kvpool* p, const LayerArgs& a, bool pack, bool link_bound, cudaStream_t s);
+int launch_counted(kvpool* p, const LayerArgs& a, bool pack, bool link_bound, cudaStream_t s, bool lane = false);
 int launch_multi_counted(kvpool* p, const MultiArgs& ma, bool pack, bool link_bound, cudaStream_t s);
 
 // The layer's block table on the device: the caller's, or (null) the one kvpool_set_tables uploaded.
@@ -249,6 +252,7 @@ int ssd_ensure_lanes(kvpool* p);                                    // kvpool_pl
 // slots [lo, hi) of layer L's stripe on SSD device i, offload (pack) or retrieve, in lane-sized commands; `a` carries the
 // paged side of the launch (bases, stride, table)
 int ssd_move(kvpool* p, LayerState& L, uint32_t i, uint32_t lo, uint32_t hi, bool pack, LayerArgs a, cudaStream_t s);
+int ssd_join_deferred(kvpool* p, cudaStream_t s);  // end of a batched offload: `s` waits for the pack launches of the SSD-type devices
 int ssd_wait_stored(kvpool* p, const LayerState& L, cudaStream_t s);  // `s` waits until the layer's store commands have completed
 int ssd_drain(kvpool* p);                                           // host waits for every worker; EIO if a command failed
 int ssd_read(kvpool* p, uint32_t i, uint64_t off, void* dst, uint64_t n);  // after ssd_drain

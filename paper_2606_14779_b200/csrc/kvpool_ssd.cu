@@ -3,15 +3,23 @@
 // An SSD-type device's share of a layer moves in lane-sized commands, DEVICE-MAJOR (runs of consecutive slots of its
 // stripe = consecutive bytes of its LBA range, reached through the device's inverse map like the chunks of kvpool_xfer.cu):
 //
-//   store    (Alg. 1 l.20-21, SSD_Direct_Store):    pack kernel -> lane.stage (HBM) -> D2H copy -> lane.bounce (pinned)
+//   store    (Alg. 1 l.20-21, SSD_Direct_Store):    pack kernel -> lane.bounce (mapped pinned memory, written over the link)
 //                                                    -> the device's worker writes the LBA range (ssd_io.cpp)
-//   retrieve (SSD_Direct_Retrieve):   worker reads the LBA range -> lane.bounce -> H2D copy -> lane.stage
-//                                                    -> unpack kernel
+//   retrieve (SSD_Direct_Retrieve):   worker reads the LBA range -> lane.bounce -> unpack kernel (reads it
+//                                                    over the link)
 //
 // The GPU streams and the worker never synchronise with the host: each lane and direction has two 32-bit sequence flags in
-// mapped pinned memory — gpu_seq, raised by a stream write-value behind the lane's copy, and cpu_seq, raised by the worker
-// behind its pread / pwrite — and each side waits for the other with a stream wait-value / a poll.  The API call only
+// mapped pinned memory — gpu_seq, raised by a stream write-value behind the lane's kernel, and cpu_seq, raised by the worker
+// behind its read / write — and each side waits for the other with a stream wait-value / a poll.  The API call only
 // enqueues: stream operations on the GPU side, one command on the worker's queue.
+//
+// No copy engine on this path, on purpose.  A first version staged every lane through an HBM piece and a cudaMemcpyAsync
+// (pack -> HBM -> D2H -> bounce), with the wait-value in front of the copy.  A wait-value that precedes a copy sits on the
+// copy engine's channel, and while it waits for the disk it holds up the copies of OTHER streams on that engine: next to a
+// host-memory device's 200 MiB copies the lanes' 8 MiB copies fell from 5 to 0.2-2.9 GB/s (an offload of host + SSD moved
+// 25-45 GB/s instead of 54), and two pools on two host threads stopped making progress altogether.  On a compute stream a
+// waiting wait-value holds up nothing but its own stream.  The disk is ten times slower than SM-issued transfers over the
+// link (51 GB/s), so the kernels lose nothing by reaching the bounce memory themselves.
 #include "kvpool_internal.hpp"
 
 namespace kvp {
@@ -49,17 +57,17 @@ inline unsigned long long flag_dev(const SsdState& S, int d, uint32_t lane, bool
 
 void free_lanes(SsdState& S) {
   S.io.stop();
-  for (auto& v : S.lane) {
-    for (auto& ln : v) {
-      if (ln.copy_done) cudaEventDestroy(ln.copy_done);
-      if (ln.kernel_done) cudaEventDestroy(ln.kernel_done);
-    }
-    v.clear();
+  for (auto& v : S.lane) v.clear();
+  for (int d = 0; d < 2; ++d) {
+    if (S.kstream[d]) cudaStreamDestroy(S.kstream[d]);
+    if (S.fork[d]) cudaEventDestroy(S.fork[d]);
+    if (S.join[d]) cudaEventDestroy(S.join[d]);
+    S.kstream[d] = nullptr;
+    S.fork[d] = S.join[d] = nullptr;
   }
   if (S.bounce_base) cudaFreeHost(S.bounce_base);
-  if (S.stage_base) cudaFree(S.stage_base);
   if (S.flags) cudaFreeHost(S.flags);
-  S.bounce_base = S.stage_base = nullptr;
+  S.bounce_base = nullptr;
   S.flags = nullptr;
   S.n_lanes = 0;
 }
@@ -107,27 +115,29 @@ int ssd_ensure_lanes(kvpool* p) {
     S.lane_bytes = (std::max<uint64_t>(p->tune.ssd_chunk_bytes, least) + 4095) / 4096 * 4096;
     const uint32_t n = std::max<uint32_t>(p->tune.ssd_lanes, 1);
     const uint64_t total = 2ull * n * S.lane_bytes;
-    cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&S.bounce_base), total, cudaHostAllocPortable);
-    if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void**>(&S.stage_base), total);
+    cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&S.bounce_base), total, cudaHostAllocPortable | cudaHostAllocMapped);
+    void* bd = nullptr;
+    if (e == cudaSuccess) e = cudaHostGetDevicePointer(&bd, S.bounce_base, 0);
     if (e == cudaSuccess) e = cudaHostAlloc(reinterpret_cast<void**>(&S.flags), 2ull * n * kFlagStride * 4, cudaHostAllocMapped | cudaHostAllocPortable);
     void* fd = nullptr;
     if (e == cudaSuccess) e = cudaHostGetDevicePointer(&fd, S.flags, 0);
     if (e != cudaSuccess) {
       cudaGetLastError();
       free_lanes(S);
-      return fail(KVPOOL_ENOMEM, "place: bounce lanes of SSD-type device %u (%llu bytes pinned + as many on the GPU): %s", i, (unsigned long long)total, cudaGetErrorString(e));
+      return fail(KVPOOL_ENOMEM, "place: bounce lanes of SSD-type device %u (%llu bytes pinned): %s", i, (unsigned long long)total, cudaGetErrorString(e));
     }
     memset(S.flags, 0, 2ull * n * kFlagStride * 4);
     S.flags_dev = reinterpret_cast<uint64_t>(fd);
     S.n_lanes = n;
     for (int d = 0; d < 2; ++d) {
+      CU(cudaStreamCreateWithFlags(&S.kstream[d], cudaStreamNonBlocking));
+      CU(cudaEventCreateWithFlags(&S.fork[d], cudaEventDisableTiming));
+      CU(cudaEventCreateWithFlags(&S.join[d], cudaEventDisableTiming));
       S.lane[d].resize(n);
       for (uint32_t k = 0; k < n; ++k) {
         SsdLane& ln = S.lane[d][k];
         ln.bounce = S.bounce_base + (static_cast<uint64_t>(d) * n + k) * S.lane_bytes;
-        ln.stage = S.stage_base + (static_cast<uint64_t>(d) * n + k) * S.lane_bytes;
-        CU(cudaEventCreateWithFlags(&ln.copy_done, cudaEventDisableTiming));
-        CU(cudaEventCreateWithFlags(&ln.kernel_done, cudaEventDisableTiming));
+        ln.bounce_dev = static_cast<uint8_t*>(bd) + (static_cast<uint64_t>(d) * n + k) * S.lane_bytes;
       }
     }
     uint8_t* const bounce[2] = {S.lane[0][0].bounce, S.lane[1][0].bounce};
@@ -140,16 +150,15 @@ int ssd_ensure_lanes(kvpool* p) {
 
 namespace {
 
-// One command of device i: `bytes` at byte offset `byte0` of the device travel between its LBA range and the staging piece of
-// the next lane of that direction.  `launch(stage)` enqueues on `s` whatever fills (store) or drains (retrieve) the piece —
-// the pack / unpack launch — and returns a KVPOOL code.  *lane_out / *use_out name the command (for ssd_wait_stored).
+// One command of device i: `bytes` at byte offset `byte0` of the device travel between its LBA range and the bounce memory of
+// the next lane of that direction.  `launch(at)` enqueues on `s` the launch that fills (store) or drains (retrieve) the lane
+// at its GPU address `at` and returns a KVPOOL code.  *lane_out / *use_out name the command (for ssd_wait_stored).
 template <class Launch>
 int ssd_command(kvpool* p, uint32_t i, bool pack, uint64_t byte0, uint64_t bytes, bool zero_tail, cudaStream_t s, Launch&& launch,
                 uint32_t* lane_out, uint32_t* use_out) {
   SsdState& S = *p->ssd[i];
   const uint64_t sec = S.io.sector();
   const int d = pack ? 1 : 0;
-  cudaStream_t io = pack ? p->io_out[i] : p->io[i];
   const uint64_t at = byte0 / sec * sec;
   const uint32_t head = static_cast<uint32_t>(byte0 - at);
   const uint32_t k = S.cursor[d]++ % S.n_lanes;
@@ -164,35 +173,26 @@ int ssd_command(kvpool* p, uint32_t i, bool pack, uint64_t byte0, uint64_t bytes
     __atomic_store_n(S.flags + flag_word(S, d, k, true), u, __ATOMIC_RELEASE);
     return rc;
   };
-  auto cu = [&](cudaError_t e, const char* what) { return e == cudaSuccess ? KVPOOL_OK : fail(KVPOOL_ECUDA, "%s: %s", what, cudaGetErrorString(e)); };
   int rc;
+  // The kernel itself moves the bytes between the paged blocks and the lane's mapped bounce memory over the link; the two
+  // hand-overs are stream memory operations on the kernel's own stream.
+  uint8_t* const at_dev = ln.bounce_dev + head;
   if (pack) {
-    // SSD_Direct_Store: gather into the lane's staging piece, copy it out to the bounce memory once the lane's previous
-    // command has been written (cpu_seq >= u-1), tell the worker (gpu_seq = u); the worker writes the LBA range
-    if ((rc = cu(cudaStreamWaitEvent(s, ln.copy_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
-    if ((rc = launch(ln.stage)) != KVPOOL_OK) return abandon(rc);
-    if ((rc = cu(cudaEventRecord(ln.kernel_done, s), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
-    if ((rc = cu(cudaStreamWaitEvent(io, ln.kernel_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
-    if (g_wait_value(io, flag_dev(S, d, k, true), u - 1, kWaitGeq) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed"));
-    if ((rc = cu(cudaMemcpyAsync(ln.bounce + head, ln.stage, bytes, cudaMemcpyDeviceToHost, io), "cudaMemcpyAsync")) != KVPOOL_OK) return abandon(rc);
-    p->n_memcpys++;
-    if (g_write_value(io, flag_dev(S, d, k, false), u, kWriteDefault) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed"));
-    if ((rc = cu(cudaEventRecord(ln.copy_done, io), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
+    // SSD_Direct_Store: once the lane's previous command is on the disk (cpu_seq >= u-1) gather into the bounce memory,
+    // then tell the worker (gpu_seq = u, fenced: the kernel's stores are visible to the CPU first)
+    if (g_wait_value(s, flag_dev(S, d, k, true), u - 1, kWaitGeq) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed"));
+    if ((rc = launch(at_dev)) != KVPOOL_OK) return abandon(rc);
+    if (g_write_value(s, flag_dev(S, d, k, false), u, kWriteDefault) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed"));
     S.io.submit(SsdCmd{SsdCmd::kWrite, zero_tail, k, u, at, head, bytes});
     return KVPOOL_OK;
   }
   // SSD_Direct_Retrieve: the worker reads the LBA range into the bounce memory once the lane's previous command has been
-  // drained (gpu_seq >= u-1) and raises cpu_seq = u; the copy waits for that, the unpack for the copy
+  // scattered (gpu_seq >= u-1) and raises cpu_seq = u; the unpack waits for that and frees the lane (gpu_seq = u)
   S.io.submit(SsdCmd{SsdCmd::kRead, false, k, u, at, head, bytes});
-  if (g_wait_value(io, flag_dev(S, d, k, true), u, kWaitGeq) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed"));
-  if ((rc = cu(cudaStreamWaitEvent(io, ln.kernel_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return abandon(rc);
-  if ((rc = cu(cudaMemcpyAsync(ln.stage, ln.bounce + head, bytes, cudaMemcpyHostToDevice, io), "cudaMemcpyAsync")) != KVPOOL_OK) return abandon(rc);
-  p->n_memcpys++;
-  if (g_write_value(io, flag_dev(S, d, k, false), u, kWriteDefault) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed"));
-  if ((rc = cu(cudaEventRecord(ln.copy_done, io), "cudaEventRecord")) != KVPOOL_OK) return abandon(rc);
-  if ((rc = cu(cudaStreamWaitEvent(s, ln.copy_done, 0), "cudaStreamWaitEvent")) != KVPOOL_OK) return rc;
-  if ((rc = launch(ln.stage)) != KVPOOL_OK) return rc;
-  return cu(cudaEventRecord(ln.kernel_done, s), "cudaEventRecord");
+  if (g_wait_value(s, flag_dev(S, d, k, true), u, kWaitGeq) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed"));
+  if ((rc = launch(at_dev)) != KVPOOL_OK) return abandon(rc);
+  if (g_write_value(s, flag_dev(S, d, k, false), u, kWriteDefault) != 0) return abandon(fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed"));
+  return KVPOOL_OK;
 }
 
 }  // namespace
@@ -204,6 +204,13 @@ int ssd_move(kvpool* p, LayerState& L, uint32_t i, uint32_t lo, uint32_t hi, boo
   const uint64_t unit = sec / gcd64(P, sec);  // every `unit` KV caches the stripe is back on a sector boundary
   a.order = L.map->order_d;
   a.visit = nullptr;
+  // The launches go to the device's own kernel stream, which first catches up with the caller's stream (the source blocks /
+  // the destination tensor are whatever `s` has made of them so far) and is joined back below.  On `s` itself they would
+  // sit, waiting for lanes the disk frees at its own pace, in front of the next launches of the host-memory devices.
+  const int d = pack ? 1 : 0;
+  cudaStream_t k = S.kstream[d];
+  CU(cudaEventRecord(S.fork[d], s));
+  CU(cudaStreamWaitEvent(k, S.fork[d], 0));
   for (uint32_t x = lo; x < hi;) {
     const uint64_t byte0 = L.stripe_off[i] + static_cast<uint64_t>(x) * P;
     const uint32_t head = static_cast<uint32_t>(byte0 % sec);
@@ -215,10 +222,10 @@ int ssd_move(kvpool* p, LayerState& L, uint32_t i, uint32_t lo, uint32_t hi, boo
     a.j0 = L.map->start[i] + x;
     a.K = n;
     uint32_t lane = 0, use = 0;
-    const int rc = ssd_command(p, i, pack, byte0, static_cast<uint64_t>(n) * P, x + n == L.map->counts[i], s,
-                               [&](uint8_t* stage) {
-                                 a.pool_base[0] = reinterpret_cast<uint64_t>(stage);
-                                 return launch_counted(p, a, pack, false, s);
+    const int rc = ssd_command(p, i, pack, byte0, static_cast<uint64_t>(n) * P, x + n == L.map->counts[i], k,
+                               [&](uint8_t* at) {
+                                 a.pool_base[0] = reinterpret_cast<uint64_t>(at);
+                                 return launch_counted(p, a, pack, true, k, true);  // a link-bound launch: 4 CTAs fill the link
                                },
                                &lane, &use);
     if (rc != KVPOOL_OK) return rc;
@@ -228,6 +235,21 @@ int ssd_move(kvpool* p, LayerState& L, uint32_t i, uint32_t lo, uint32_t hi, boo
       L.ssd_stored |= 1u << i;
     }
     x += n;
+  }
+  // join: a retrieve is complete in `s` order (kvpool.h), and work enqueued on `s` after an offload may overwrite the source
+  // blocks - per layer for the per-layer calls, once at the end of a batched offload (the source blocks of all its layers
+  // stay as they are until the call's last launch anyway)
+  CU(cudaEventRecord(S.join[d], k));
+  if (pack && p->ssd_defer_join) S.join_pending = true;
+  else CU(cudaStreamWaitEvent(s, S.join[d], 0));
+  return KVPOOL_OK;
+}
+
+int ssd_join_deferred(kvpool* p, cudaStream_t s) {
+  for (auto& S : p->ssd) {
+    if (!S || !S->join_pending) continue;
+    S->join_pending = false;
+    CU(cudaStreamWaitEvent(s, S->join[1], 0));
   }
   return KVPOOL_OK;
 }
@@ -260,19 +282,46 @@ int ssd_read(kvpool* p, uint32_t i, uint64_t off, void* dst, uint64_t n) {
 }
 
 // "Measured bandwidth" of an SSD-type device, with the mechanism that moves the bytes: the first `bytes` of
-// the device travel through the device's own lanes — worker, bounce memory, copy engine, staging piece — exactly as a
-// retrieve (or an offload) moves them, without the pack / unpack launch; median of `iters` passes by the host's clock
-// around enqueue + completion.  (A plain pread loop into a cache-resident buffer reads 10-15 % fast.)  The region is
-// written once first, so that a sparse stand-in file has its blocks.
+// the device travel through the device's own lanes — worker, bounce memory, link, gather / scatter kernel — exactly as a
+// retrieve (or an offload) moves them, between the disk and a scratch paged layout whose block table and inverse map are
+// the identity; median of `iters` passes by the host's clock around enqueue + completion.  (A plain pread loop into a
+// cache-resident buffer reads 10-15 % fast.)  The region is written once first, so that a sparse stand-in file has its blocks.
 int ssd_measure(kvpool* p, uint32_t i, bool write, uint64_t bytes, uint32_t iters, double* gbps) {
   int rc = ssd_ensure_lanes(p);
   if (rc != KVPOOL_OK) return rc;
   SsdState& S = *p->ssd[i];
   DeviceGuard guard(p->cuda_device);
-  const uint64_t sec = S.io.sector(), piece = (S.lane_bytes - 2 * sec) / sec * sec;
-  bytes = bytes / sec * sec;
-  if (bytes == 0) return fail(KVPOOL_EINVAL, "measure_bandwidth: fewer bytes than one sector");
-  cudaStream_t s = p->upload, io = write ? p->io_out[i] : p->io[i];
+  const uint64_t P = p->payload, sec = S.io.sector();
+  const uint64_t unit = sec / gcd64(P, sec);                             // KV caches per sector-aligned run
+  const uint64_t K = (S.lane_bytes - 2 * sec) / (unit * P) * unit;       // KV caches per command: a whole number of sectors
+  if (K == 0 || K > 0x7fffffffull) return fail(KVPOOL_EINVAL, "measure_bandwidth: the lanes of SSD-type device %u are too small for a sector-aligned run of KV caches", i);
+  const uint64_t piece = K * P;
+  bytes = bytes / piece * piece;
+  if (bytes == 0) return fail(KVPOOL_EINVAL, "measure_bandwidth: fewer bytes than one command (%llu)", (unsigned long long)piece);
+  struct Scratch {
+    void* buf = nullptr;
+    uint32_t* ident = nullptr;
+    ~Scratch() {
+      if (buf) cudaFree(buf);
+      if (ident) cudaFree(ident);
+    }
+  } m;
+  CU(cudaMalloc(&m.buf, piece));
+  CU(cudaMalloc(reinterpret_cast<void**>(&m.ident), K * 4));
+  std::vector<uint32_t> h(K);
+  std::iota(h.begin(), h.end(), 0u);
+  cudaStream_t s = p->upload;
+  CU(cudaMemcpyAsync(m.ident, h.data(), K * 4, cudaMemcpyHostToDevice, s));
+  CU(cudaMemsetAsync(m.buf, 0x5a, piece, s));
+  CU(cudaStreamSynchronize(s));
+  LayerArgs a{};
+  a.k_base = static_cast<uint8_t*>(m.buf);
+  a.v_base = static_cast<uint8_t*>(m.buf) + K * p->kvb;
+  a.stride = p->kvb;
+  a.table = reinterpret_cast<const int32_t*>(m.ident);
+  a.order = m.ident;
+  a.K = static_cast<uint32_t>(K);
+  a.kvb = static_cast<uint32_t>(p->kvb);
   std::vector<double> sec_s(iters);
   for (uint32_t it = 0; it < iters + 1; ++it) {  // pass 0 writes the region (and warms up)
     const bool w = write || it == 0;
@@ -280,11 +329,15 @@ int ssd_measure(kvpool* p, uint32_t i, bool write, uint64_t bytes, uint32_t iter
     clock_gettime(CLOCK_MONOTONIC, &t0);
     for (uint64_t off = 0; off < bytes; off += piece) {
       uint32_t lane, use;
-      rc = ssd_command(p, i, w, off, std::min(piece, bytes - off), false, s, [](uint8_t*) { return KVPOOL_OK; }, &lane, &use);
+      rc = ssd_command(p, i, w, off, piece, false, s,
+                       [&](uint8_t* at) {
+                         a.pool_base[0] = reinterpret_cast<uint64_t>(at);
+                         return launch_counted(p, a, w, true, s, true);
+                       },
+                       &lane, &use);
       if (rc != KVPOOL_OK) return rc;
     }
     CU(cudaStreamSynchronize(s));
-    CU(cudaStreamSynchronize(w ? p->io_out[i] : io));
     if ((rc = ssd_drain(p)) != KVPOOL_OK) return rc;
     clock_gettime(CLOCK_MONOTONIC, &t1);
     if (it > 0) sec_s[it - 1] = (t1.tv_sec - t0.tv_sec) + 1e-9 * (t1.tv_nsec - t0.tv_nsec);

@@ -525,10 +525,30 @@ int issue_group_work(const BatchCall& c, const LayerGroup& g) {
 // Layers [first, first+n) in one call.  Consecutive layers are gathered into groups of at least tune.group_bytes (a
 // layer at least that large travels with whatever small layers precede it); each group moves as one unit: one fused
 // zero-copy launch, or one pack/unpack launch plus one copy per pool device.
+static int layers_batched_locked(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32_t first, uint32_t n, const void* const* k_bases,
+                                 const void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream,
+                                 void* const* ready);
+
 static int layers_batched(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32_t first, uint32_t n, const void* const* k_bases,
                           const void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream,
                           void* const* ready = nullptr) {
   PoolLock lock__(p);
+  if (!p || !pack || !p->ssd_mask) return layers_batched_locked(p, pl, pack, first, n, k_bases, v_bases, stride, tables, cuda_stream, ready);
+  // a batched offload over a pool with SSD-type devices: their pack launches (kvpool_ssd.cu) are joined back to `stream`
+  // once, here, instead of after every layer, so that the launches of the host-memory devices never queue behind a disk
+  p->ssd_defer_join = true;
+  int rc = layers_batched_locked(p, pl, pack, first, n, k_bases, v_bases, stride, tables, cuda_stream, ready);
+  p->ssd_defer_join = false;
+  DeviceGuard guard(p->cuda_device);
+  const int rc2 = ssd_join_deferred(p, static_cast<cudaStream_t>(cuda_stream));  // (also after an error: the launches made so far still read the source)
+  if (rc == KVPOOL_OK) rc = rc2;
+  if (rc == KVPOOL_OK && pl) rc = note_use(p, pl, static_cast<cudaStream_t>(cuda_stream));
+  return rc;
+}
+
+static int layers_batched_locked(kvpool_t* p, kvpool_placement_t* pl, bool pack, uint32_t first, uint32_t n, const void* const* k_bases,
+                                 const void* const* v_bases, uint64_t stride, const int32_t* const* tables, void* cuda_stream,
+                                 void* const* ready) {
   if (!p || !pl || pl->pool != p || !is_live(p, pl)) return fail(KVPOOL_EINVAL, "layers: bad pool or placement");
   if (static_cast<uint64_t>(first) + n > p->geom.n_layers) return fail(KVPOOL_EINVAL, "layers [%u, %u) out of range (n_layers %u)", first, first + n, p->geom.n_layers);
   if (n == 0) return KVPOOL_OK;
