@@ -78,6 +78,7 @@ def parse_args():
     ap.add_argument("--ssd-pool", action="store_true",
                     help="side mode: pools with SSD-type devices (KV-passthrough, PAPER.md:179-185) - files under --ssd-dir opened O_DIRECT stand in "
                          "for NVMe namespaces: one SSD alone, host memory + one SSD, host memory + two SSDs (the paper's mix); text table")
+    ap.add_argument("--ssd-kinds", default="m,s,ms,mss", help="--ssd-pool: the pools to run, comma separated; m = a pinned host buffer, s = an SSD-type device")
     ap.add_argument("--ssd-dir", default="/tmp", help="--ssd-pool: directory that holds the stand-in files (or pass block devices, comma separated)")
     ap.add_argument("--duplex", action="store_true",
                     help="offload of one request concurrent with retrieve of another (PCIe is full duplex): per-direction and aggregate "
@@ -1208,7 +1209,7 @@ def run_ssd_pool(args) -> None:
     buffer, the device's own lanes for an SSD; all devices name one link group because every byte crosses this GPU's single
     PCIe link).  Text table on stdout; ssd_pool_lines has the procedure."""
     names = {"m": "1 host buffer", "s": "1 SSD", "ms": "1 host buffer + 1 SSD", "mss": "1 host buffer + 2 SSDs"}
-    lines = ssd_pool_lines(args.config, args.ssd_dir, list(names))
+    lines = ssd_pool_lines(args.config, args.ssd_dir, [k for k in args.ssd_kinds.split(",") if k in names])
     h = next(lines)
     print(f"# bench.py --ssd-pool --config {args.config} --ssd-dir {args.ssd_dir}: {h['workload']} cut to {h['layers']} layers, {h['moved_bytes_per_leg'] / 2**20:.0f} MiB per leg "
           f"({h['blocks_per_layer']} blocks of {h['payload']} B per layer); SSD-type devices = {h['medium']}; "
