@@ -463,3 +463,74 @@ def test_synchronous_fallback_of_the_worker(tmp_path, monkeypatch):
     wl = W.make_workload(1, n_layers=2)
     out = _run(wl, ["mem", "ssd"], tmp_path, tuning={"ssd_lanes": 2, "ssd_chunk_bytes": 256 << 10})
     assert out["info"][1]["queue_depth"] == 1
+
+
+@pytest.mark.timeout(180)
+def test_ssd_pool_makes_progress_next_to_another_pools_copy_engine_traffic(tmp_path):
+    """Two pools on two host threads: one streams a host-memory pool's 128 MiB layers through the copy engines without a
+    pause, the other offloads and retrieves through an SSD-type device.  The SSD pool's lanes use no copy engine and their
+    stream wait-values sit on compute streams, so they neither starve nor stall the other pool (a first version that staged
+    lanes through cudaMemcpyAsync stopped making progress in exactly this set-up: kvpool_ssd.cu).  Results against the
+    oracle; the whole test must finish in seconds."""
+    import threading
+    import time
+    wl = W.make_workload(2, scale=1 / 4, n_layers=4)                     # LLaMA-shaped, 512 blocks of 64 KiB per layer = 32 MiB
+    g, dev, L = wl.geom, torch.device("cuda:0"), 4
+    big = W.make_workload(2, n_layers=2)                                 # the other pool's request: 2 layers of 128 MiB
+    bpl_big = big.blocks_per_layer(0)
+    mem = kv.KvPool([1.0], [big.moved_bytes() + (1 << 20)], n_layers=2, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim)
+    pool, bw, files = _ssd_pool(_custom(g, wl.nphys, [wl.requests[0].table], 1, (1.0,), cfg=2), ["ssd"], tmp_path, sector=4096)
+    stop, rounds, errors = threading.Event(), [0], []
+    try:
+        big_src = [W.kv_layer_torch(big, l, dev) for l in range(2)]
+        big_tab = [torch.from_numpy(np.ascontiguousarray(big.layer_table(0, l))).to(dev) for l in range(2)]
+        plm = mem.place(bpl_big)
+        s2 = torch.cuda.Stream()
+        mem.offload_layers(plm, 0, [x[0] for x in big_src], [x[1] for x in big_src], g.kvb, big_tab, s2)
+        mem.wait_offloads(plm, s2)
+        s2.synchronize()
+
+        def background():
+            try:
+                while not stop.is_set():
+                    mem.offload_layers(plm, 0, [x[0] for x in big_src], [x[1] for x in big_src], g.kvb, big_tab, s2)
+                    mem.retrieve_layers(plm, 0, [x[0] for x in big_src], [x[1] for x in big_src], g.kvb, big_tab, s2)   # (a round trip onto itself)
+                    s2.synchronize()
+                    rounds[0] += 1
+            except Exception as e:                                         # pragma: no cover
+                errors.append(e)
+
+        th = threading.Thread(target=background)
+        th.start()
+        time.sleep(0.05)
+        t0 = time.perf_counter()
+        bpl = wl.blocks_per_layer(0)
+        pl, opl = pool.place(bpl), oracle.place([1.0], bpl)
+        s1 = torch.cuda.Stream()
+        tables_np = [np.ascontiguousarray(wl.layer_table(0, l)) for l in range(L)]
+        tables = [torch.from_numpy(t).to(dev) for t in tables_np]
+        for rep in range(3):
+            src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+            dst = [W.poison_torch((2, wl.nphys, g.kvb // 2), dev) for _ in range(L)]
+            torch.cuda.current_stream().synchronize()
+            pool.offload_layers(pl, 0, [x[0] for x in src], [x[1] for x in src], g.kvb, tables, s1)
+            pool.retrieve_layers(pl, 0, [x[0] for x in dst], [x[1] for x in dst], g.kvb, tables, s1)
+            s1.synchronize()
+            for l in range(L):
+                want = oracle.offload_layer(W.kv_layer_numpy(wl, l), tables_np[l], opl[l])
+                ref = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+                oracle.retrieve_layer(ref, tables_np[l], opl[l], want)
+                assert np.array_equal(dst[l].cpu().numpy().view(np.uint16), ref), (rep, l)
+        took = time.perf_counter() - t0
+        stop.set()
+        th.join(60)
+        assert not th.is_alive() and not errors, errors
+        assert rounds[0] >= 2                                              # the other pool kept streaming meanwhile
+        assert took < 60, took                                             # 768 MiB through the "disk" and back: seconds, not a stall
+        pool.synchronize()
+        pl.release()
+        plm.release()
+    finally:
+        stop.set()
+        pool.destroy()
+        mem.destroy()
