@@ -301,7 +301,8 @@ KVPOOL_API int kvpool_offload(kvpool_t* pool, kvpool_placement_t* pl, uint32_t l
 KVPOOL_API int kvpool_retrieve(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, void* k_base /*device*/, void* v_base /*device*/,
                     uint64_t block_stride_bytes, const int32_t* block_table_dev, void* cuda_stream);
 /* Batched forms: layers [first_layer, first_layer + n_layers) in one call, equivalent to the per-layer calls in
- * ascending order.  k_bases / v_bases / block_tables are HOST arrays of n_layers DEVICE pointers (entries of layers
+ * ascending order provided the paged tensors of different layers do not overlap (the library lets the launches of one
+ * call overlap each other's ends).  k_bases / v_bases / block_tables are HOST arrays of n_layers DEVICE pointers (entries of layers
  * with K_l = 0 may be NULL).  Consecutive layers are gathered into groups of at least `group_bytes` (default 64 MiB,
  * at most 64 layers; a large layer travels with the small ones before it) and each group moves as one unit: one
  * fused kernel launch on the zero-copy path, or one pack/unpack launch plus ONE cudaMemcpyAsync per pool device on

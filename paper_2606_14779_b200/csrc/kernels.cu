@@ -60,6 +60,20 @@ __device__ __forceinline__ void span_end(unsigned long long* span) {
 __device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// The three orderings of kernels.cuh (kChain*).
+__device__ __forceinline__ void chain_enter(uint32_t chain) {
+  if (chain == kChainHead) {
+    griddep_wait();
+    griddep_launch_dependents();
+  } else {
+    griddep_launch_dependents();
+    if (chain != kChainFollower) griddep_wait();
+  }
+}
+__device__ __forceinline__ void chain_exit(uint32_t chain) {
+  if (chain == kChainFollower) griddep_wait();
+}
+
 // Decode work item t of a layer split into `pieces` pieces per K (or V) block of `piece_bytes` bytes.
 struct Piece {
   uint8_t* paged;
@@ -140,8 +154,7 @@ __global__ void __launch_bounds__(kVecMaxThreads) kv_copy_vec16(const __grid_con
   const uint64_t nwarps = static_cast<uint64_t>(gridDim.x) * warps_per_cta;
   const uint32_t pieces = (a.kvb + kVecPiece - 1) / kVecPiece;
   const uint64_t total = static_cast<uint64_t>(units(a)) * 2u * pieces;
-  griddep_launch_dependents();
-  griddep_wait();
+  chain_enter(a.chain);
   if (threadIdx.x == 0) span_begin(a.span);
   for (uint64_t t = static_cast<uint64_t>(blockIdx.x) * warps_per_cta + (threadIdx.x >> 5); t < total; t += nwarps) {
     const Piece p = decode(a, t, pieces, kVecPiece);
@@ -169,6 +182,7 @@ __global__ void __launch_bounds__(kVecMaxThreads) kv_copy_vec16(const __grid_con
     __syncthreads();
     if (threadIdx.x == 0) span_end(a.span);
   }
+  chain_exit(a.chain);
 }
 
 // ---- cp.async.bulk / mbarrier primitives (PTX ISA 8.x, sm_90+; SASS: UBLKCP, SYNCS) ------------------
@@ -215,10 +229,11 @@ __global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Args
   const uint32_t warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
   const uint32_t bar0 = smem_u32(smem) + warp * stages * 8u;
   const uint32_t buf0 = smem_u32(smem) + kBulkBarrierBytes + warp * stages * chunk;
-  griddep_launch_dependents();
+  if (a.chain != kChainHead) griddep_launch_dependents();
   for (uint32_t s = 0; s < stages; ++s) mbar_init(bar0 + 8u * s, 1);
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  griddep_wait();
+  if (a.chain != kChainFollower) griddep_wait();
+  if (a.chain == kChainHead) griddep_launch_dependents();
   span_begin(a.span);
 
   const uint32_t pieces = a.kvb / chunk;  // host guarantees chunk | kvb
@@ -249,6 +264,7 @@ __global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Args
   }
   bulk_wait_all();
   span_end(a.span);
+  chain_exit(a.chain);
 }
 
 // ---- consumer stand-in: position-weighted 64-bit checksum of the blocks named by a table ---------------------------

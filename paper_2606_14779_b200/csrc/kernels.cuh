@@ -36,8 +36,18 @@ struct LayerArgs {
   unsigned long long* span;  // profiling only (else null): device {min start, max end} of the launch in %globaltimer ns
   unsigned long long* bad;   // table check only (else null): counts table entries outside [0, nphys_check)
   uint32_t nphys_check;      // 0 = the table is trusted (R12); else entries >= this (or negative) are skipped and counted
+  uint32_t chain;            // kChain*: how the launch orders itself against the kernel before it on the stream (below)
   uint64_t pool_base[kMaxDev];
 };
+
+// Programmatic dependent launch, three ways (kernels.cu).  kChainNone: let the successor become resident at once, touch
+// memory only once the predecessor grid has completed — right for a launch that may depend on anything before it.
+// A run of launches that do NOT depend on each other (the layers of one batched retrieve: other stripes, other paged
+// tensors) can overlap each launch's first transfers with its predecessor's tail instead: the HEAD of the run waits for
+// everything before it and only then lets its successor go; a FOLLOWER starts moving bytes at once — whatever the head
+// waited for is complete, and the launches between the head and itself are its independent siblings — and waits for its
+// predecessor just before it exits, so that grids still complete in stream order and whatever follows the run sees all of it.
+constexpr uint32_t kChainNone = 0, kChainHead = 1, kChainFollower = 2;
 
 // Several layers in one launch (tiny layers: one launch latency and one pipeline ramp for the whole batch).  Units are
 // numbered across the batch; layer i owns units [first_unit, first_unit + K).  pool_base points at N device-visible
@@ -58,7 +68,7 @@ struct MultiArgs {
   uint32_t kvb;
   uint32_t n;            // layers in this launch, <= kMaxBatch
   uint32_t total_units;  // sum of K
-  uint32_t pad;
+  uint32_t chain;        // kChain*, as in LayerArgs
   unsigned long long* span;  // as in LayerArgs
   unsigned long long* bad;   // as in LayerArgs
   uint32_t nphys_check, pad2;

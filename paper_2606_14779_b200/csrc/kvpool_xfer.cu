@@ -351,7 +351,20 @@ struct BatchCall {
   uint64_t stride;
   cudaStream_t s;
   void* const* ready;  // optional: caller-owned cudaEvent_t per layer of the call, recorded on `s` when that layer is complete
+  bool* chain_run;     // the launch enqueued last on `s` by this call heads / follows a run of chained launches (kernels.cuh)
+  std::vector<LayerState*>* landed_later;  // offloads of a chained run: their `landed` events are recorded behind the run
 };
+
+// Record the `landed` events a chained run of offload launches has put off (an event record between two launches would
+// undo the chaining): behind the run's last launch every one of its layers is complete in the pool.
+int flush_landed(const BatchCall& c) {
+  for (LayerState* L : *c.landed_later) {
+    CU(cudaEventRecord(L->landed, c.s));
+    L->landed_pending = true;
+  }
+  c.landed_later->clear();
+  return KVPOOL_OK;
+}
 
 void fill_descs(const BatchCall& c, const LayerGroup& g, MultiArgs* ma) {
   ma->stride = c.stride;
@@ -380,10 +393,24 @@ int issue_zero_copy_group(const BatchCall& c, const LayerGroup& g) {
   kvpool* p = c.p;
   MultiArgs ma{};
   fill_descs(c, g, &ma);
+  bool waited = false;
   for (uint32_t b = 0; b < g.n; ++b) {
     LayerState& L = c.pl->layers[c.first + g.q[b]];
-    if (L.landed_pending) CU(cudaStreamWaitEvent(c.s, L.landed, 0));  // settled (no wait) after kvpool_synchronize
+    if (L.landed_pending) { CU(cudaStreamWaitEvent(c.s, L.landed, 0)); waited = true; }  // settled (no wait) after kvpool_synchronize
   }
+  // Retrieves of one batched call in a pool with HBM-type devices: the launches are independent of each other (other
+  // stripes, other paged tensors) and last ~90 us each, of which the first microseconds are the link's first-byte latency
+  // and the ramp: chain them (kernels.cuh), so that a launch's host-memory blocks are already on the link while its
+  // predecessor's last wave drains.  Only where the launches are back to back on the stream (no event wait or record
+  // between them, no profiling markers) and many waves long (the HBM grid; a 4-CTA link launch would let the whole
+  // request start at once and lose the layer order).
+  const bool chain = p->hbm_mask && !c.ready && !waited && !p->profiling && p->tune.pdl != 2;
+  ma.chain = !chain ? kChainNone : (*c.chain_run ? kChainFollower : kChainHead);
+  if (!chain) {
+    const int frc = flush_landed(c);
+    if (frc != KVPOOL_OK) return frc;
+  }
+  *c.chain_run = chain;
   const int rc = launch_multi_counted(p, ma, c.pack, true, c.s);
   if (rc != KVPOOL_OK) return rc;
   if (c.pack)
@@ -391,6 +418,7 @@ int issue_zero_copy_group(const BatchCall& c, const LayerGroup& g) {
       LayerState& L = c.pl->layers[c.first + g.q[b]];
       L.offloaded = true;
       L.have.clear();
+      if (chain) { c.landed_later->push_back(&L); continue; }
       CU(cudaEventRecord(L.landed, c.s));
       L.landed_pending = true;
     }
@@ -402,6 +430,8 @@ int issue_zero_copy_group(const BatchCall& c, const LayerGroup& g) {
 // not fit a staging slot (the caller then falls back to per-layer calls).
 int issue_staged_group(const BatchCall& c, const LayerGroup& g) {
   kvpool* p = c.p;
+  *c.chain_run = false;
+  if (const int frc = flush_landed(c)) return frc;
   if (p->ssd_mask) return 1;  // a pool with an SSD-type device moves layer by layer, device-major
   const uint32_t N = p->n;
   const std::vector<cudaStream_t>& ios = c.pack ? p->io_out : p->io;  // the copy streams of this direction
@@ -512,6 +542,8 @@ int issue_group_work(const BatchCall& c, const LayerGroup& g) {
     const int rc = issue_staged_group(c, g);
     if (rc != 1) return rc;
   }
+  *c.chain_run = false;
+  if (const int frc = flush_landed(c)) return frc;
   for (uint32_t b = 0; b < g.n; ++b) {  // a single layer, or a group too large for a staging slot: the per-layer path
     const uint32_t q = g.q[b], layer = c.first + q;
     const int rc = c.pack ? kvpool_offload(p, c.pl, layer, c.k_bases[q], c.v_bases[q], c.stride, c.tables ? c.tables[q] : nullptr, c.s)
@@ -560,7 +592,13 @@ static int layers_batched_locked(kvpool_t* p, kvpool_placement_t* pl, bool pack,
     if (!pack && !pl->layers[first + q].offloaded) return fail(KVPOOL_ESTATE, "retrieve: layer %u was never offloaded", first + q);
   }
   DeviceGuard guard(p->cuda_device);
-  const BatchCall c{p, pl, pack, first, k_bases, v_bases, tables, stride, static_cast<cudaStream_t>(cuda_stream), ready};
+  bool chain_run = false;
+  std::vector<LayerState*> landed_later;
+  const BatchCall c{p, pl, pack, first, k_bases, v_bases, tables, stride, static_cast<cudaStream_t>(cuda_stream), ready, &chain_run, &landed_later};
+  struct Flush {  // whatever path leaves the call: the events put off so far are recorded
+    const BatchCall& c;
+    ~Flush() { flush_landed(c); }
+  } flush_on_exit{c};
   uint64_t cap = std::max<uint64_t>(p->tune.group_bytes, 1);
   if (ready) {
     // a consumer follows behind the per-layer events: a request so small that it would travel as ONE group (all layers
@@ -597,7 +635,8 @@ static int layers_batched_locked(kvpool_t* p, kvpool_placement_t* pl, bool pack,
       units = 0;
     }
   }
-  const int rc = issue_group(c, g);
+  int rc = issue_group(c, g);
+  if (rc == KVPOOL_OK) rc = flush_landed(c);
   return rc == KVPOOL_OK ? note_use(p, pl, c.s) : rc;
 }
 
