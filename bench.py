@@ -829,6 +829,15 @@ def run_kvpool(args) -> dict:
                                          frac_of_link=r["retrieve_gbps"] / link_h2d, offload_frac_of_link=r["offload_gbps"] / link_d2h)
         except Exception as e:                         # (a box without a writable --ssd-dir: say so instead of losing the headline)
             pools["host+ssd"] = {"unavailable": f"{type(e).__name__}: {e}"}
+        # ... and over host memory and GPU memory (HBM-type pool device; this GPU's own memory stands in for
+        # an NVLink peer's: one GPU per box), 8 layers of this configuration, bit-verified
+        lines = mixed_pool_lines(4, (("host+hbm", [0, kv.DEV_HBM]),), L=8)
+        head = next(lines)
+        for r in lines:
+            pools["host+hbm"] = dict(r, layers=head["layers"], moved_bytes_per_leg=head["moved_bytes_per_leg"],
+                                     hbm_device="this GPU's own memory standing in for an NVLink peer's (one GPU per box)",
+                                     frac_of_sum_of_weights=r["retrieve_gbps"] / r["sum_of_weights_gbps"],
+                                     offload_frac_of_sum_of_weights=r["offload_gbps"] / r["sum_of_weights_gbps"])
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -1054,18 +1063,17 @@ def time_under_dma(torch, s, o, fn, bg, launches: int = 16, reps: int = 4):
     return best
 
 
-def run_mixed_pool(args) -> None:
-    """Eq. 1-2 at work on devices of very different speed: one pinned host buffer (PCIe) and one HBM-type device, alone and
-    together, weights = kvpool_measure_bandwidth of each.  Whole request (16 layers of --config), batched calls, legs
-    timed apart with CUDA events; every run is verified bit-exact against the source.  Text table on stdout."""
+def mixed_pool_lines(cfg: int, pools, L: int = 16):
+    """Generator behind --mixed-pool and the `pools.host+hbm` side line of the default run: for every (name, flags) in `pools`
+    one dict with the calibrated weights, the split and the bit-verified offload / retrieve GB/s of a whole request (L layers
+    of config `cfg`, batched calls, legs timed apart with CUDA events).  The first item yielded is the header dict."""
     import torch
     from paper_2606_14779_b200 import binding as kv
     from paper_2606_14779_b200 import workloads as W
 
     dev = torch.device("cuda", 0)
     torch.cuda.set_device(dev)
-    L = 16
-    wl = W.make_workload(args.config, n_layers=L)
+    wl = W.make_workload(cfg, n_layers=L)
     wl.sliding_layers = ()
     g = wl.geom
     bpl = wl.blocks_per_layer(0)
@@ -1078,50 +1086,66 @@ def run_mixed_pool(args) -> None:
     s = torch.cuda.Stream(device=dev)
     torch.cuda.synchronize()
     cap = moved + (L + 4) * (g.payload + 4096)
-    print(f"# bench.py --mixed-pool --config {args.config}: {wl.name} cut to {L} layers, {moved / 2**20:.0f} MiB per leg ({K} blocks of {g.payload} B per layer); "
-          "weights = kvpool_calibrate (256 MiB per device: cudaMemcpyAsync for the host-only pool, the gather kernel itself for pools with HBM-type devices; link groups "
-          "share; payload GB/s); median of 3; HBM-type device = this GPU's own memory")
-    print(f"{'pool':34s} {'weights (GB/s)':>22s} {'blocks per layer':>18s} {'offload GB/s':>12s} {'retrieve GB/s':>13s} {'sum of weights':>14s} {'kernels':>8s} {'memcpys':>8s}")
-    for name, flags in (("1 host buffer", [0]), ("1 host buffer + 1 HBM device", [0, kv.DEV_HBM]), ("2 host buffers + 2 HBM devices", [0, 0, kv.DEV_HBM, kv.DEV_HBM]),
-                        ("1 HBM device", [kv.DEV_HBM])):
+    yield {"workload": wl.name, "layers": L, "moved_bytes_per_leg": moved, "blocks_per_layer": K, "payload": g.payload}
+    for name, flags in pools:
         n = len(flags)
         # devices behind ONE shared resource name one link group (the host buffers behind this GPU's single PCIe link: 1; the
         # HBM-type devices inside one GPU: 2): kvpool_calibrate measures every device and divides what a group shares.  A pool
         # with HBM-type devices is measured with the library's own kernel, which is what reaches every stripe there.
         pool = kv.KvPool([1.0] * n, [cap] * n, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, dev_flags=flags,
                          link_groups=[2 if f else 1 for f in flags])
-        bw = list(pool.calibrate(kv.MEASURE_KERNEL_RETRIEVE if any(flags) else kv.MEASURE_RETRIEVE, 256 << 20, 5))
-        offs, rets = [], []
-        k0, m0 = pool.stats()
-        for it in range(4):
-            for d in dst:
-                d.fill_(np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item())
-            pl = pool.place(bpl)
-            counts = list(pl.counts(0))
-            torch.cuda.synchronize()
-            ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
-            ev[0].record(s)
-            pool.offload_layers(pl, 0, src_k, src_v, g.kvb, tables, s)
-            pool.wait_offloads(pl, s)
-            ev[1].record(s)
-            s.synchronize()
-            pool.synchronize()
-            ev[2].record(s)
-            pool.retrieve_layers(pl, 0, dst_k, dst_v, g.kvb, tables, s)
-            ev[3].record(s)
-            s.synchronize()
-            pl.release()
-            if it > 0:
-                offs.append(ev[0].elapsed_time(ev[1]))
-                rets.append(ev[2].elapsed_time(ev[3]))
-        k1, m1 = pool.stats()
-        for l in range(L):
-            if not torch.equal(dst[l][:, tables[l].long()], src[l][:, tables[l].long()]):
-                raise RuntimeError(f"{name}: retrieved KV differs from the source")
-        o, r = moved / statistics.median(offs) / 1e6, moved / statistics.median(rets) / 1e6
-        print(f"{name:34s} {'/'.join(f'{b:.0f}' for b in bw):>22s} {'/'.join(str(c) for c in counts):>18s} {o:12.1f} {r:13.1f} {sum(bw):14.0f} "
-              f"{(k1 - k0) // 4:8d} {(m1 - m0) // 4:8d}", flush=True)
-        pool.destroy()
+        try:
+            bw = list(pool.calibrate(kv.MEASURE_KERNEL_RETRIEVE if any(flags) else kv.MEASURE_RETRIEVE, 256 << 20, 5))
+            offs, rets = [], []
+            k0, m0 = pool.stats()
+            for it in range(4):
+                for d in dst:
+                    d.fill_(np.int16(np.uint16(W.POISON_BITS).view(np.int16)).item())
+                pl = pool.place(bpl)
+                counts = [int(c) for c in pl.counts(0)]
+                torch.cuda.synchronize()
+                ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+                ev[0].record(s)
+                pool.offload_layers(pl, 0, src_k, src_v, g.kvb, tables, s)
+                pool.wait_offloads(pl, s)
+                ev[1].record(s)
+                s.synchronize()
+                pool.synchronize()
+                ev[2].record(s)
+                pool.retrieve_layers(pl, 0, dst_k, dst_v, g.kvb, tables, s)
+                ev[3].record(s)
+                s.synchronize()
+                pl.release()
+                if it > 0:
+                    offs.append(ev[0].elapsed_time(ev[1]))
+                    rets.append(ev[2].elapsed_time(ev[3]))
+            k1, m1 = pool.stats()
+            for l in range(L):
+                if not torch.equal(dst[l][:, tables[l].long()], src[l][:, tables[l].long()]):
+                    raise RuntimeError(f"{name}: retrieved KV differs from the source")
+            yield {"pool": name, "bandwidth_gbps": [round(float(b), 1) for b in bw], "blocks_per_layer": counts,
+                   "offload_gbps": moved / statistics.median(offs) / 1e6, "retrieve_gbps": moved / statistics.median(rets) / 1e6,
+                   "sum_of_weights_gbps": float(sum(bw)), "kernels_per_step": (k1 - k0) // 4, "memcpys_per_step": (m1 - m0) // 4,
+                   "verified_bit_exact_round_trip": True}
+        finally:
+            pool.destroy()
+
+
+def run_mixed_pool(args) -> None:
+    """Eq. 1-2 at work on devices of very different speed: one pinned host buffer (PCIe) and one HBM-type device, alone and
+    together, weights = kvpool_calibrate.  Whole request (16 layers of --config), batched calls, legs timed apart with CUDA
+    events; every run is verified bit-exact against the source.  Text table on stdout; mixed_pool_lines has the procedure."""
+    from paper_2606_14779_b200 import binding as kv
+    lines = mixed_pool_lines(args.config, (("1 host buffer", [0]), ("1 host buffer + 1 HBM device", [0, kv.DEV_HBM]),
+                                           ("2 host buffers + 2 HBM devices", [0, 0, kv.DEV_HBM, kv.DEV_HBM]), ("1 HBM device", [kv.DEV_HBM])))
+    h = next(lines)
+    print(f"# bench.py --mixed-pool --config {args.config}: {h['workload']} cut to {h['layers']} layers, {h['moved_bytes_per_leg'] / 2**20:.0f} MiB per leg ({h['blocks_per_layer']} blocks of {h['payload']} B per layer); "
+          "weights = kvpool_calibrate (256 MiB per device: cudaMemcpyAsync for the host-only pool, the gather kernel itself for pools with HBM-type devices; link groups "
+          "share; payload GB/s); median of 3; HBM-type device = this GPU's own memory")
+    print(f"{'pool':34s} {'weights (GB/s)':>22s} {'blocks per layer':>18s} {'offload GB/s':>12s} {'retrieve GB/s':>13s} {'sum of weights':>14s} {'kernels':>8s} {'memcpys':>8s}")
+    for r in lines:
+        print(f"{r['pool']:34s} {'/'.join(f'{b:.0f}' for b in r['bandwidth_gbps']):>22s} {'/'.join(str(c) for c in r['blocks_per_layer']):>18s} {r['offload_gbps']:12.1f} "
+              f"{r['retrieve_gbps']:13.1f} {r['sum_of_weights_gbps']:14.0f} {r['kernels_per_step']:8d} {r['memcpys_per_step']:8d}", flush=True)
 
 
 def ssd_pool_lines(cfg: int, ssd_dir: str, kinds):
@@ -1196,6 +1220,7 @@ def ssd_pool_lines(cfg: int, ssd_dir: str, kinds):
             infos = [pool.ssd_info(i) for i in ssds]
             yield {"pool": types, "bandwidth_gbps": [round(float(b), 2) for b in bw], "blocks_per_layer": counts,
                    "offload_gbps": moved / statistics.median(offs) / 1e6, "retrieve_gbps": moved / statistics.median(rets) / 1e6,
+                   "offload_gbps_best": moved / min(offs) / 1e6, "retrieve_gbps_best": moved / min(rets) / 1e6,
                    "sum_of_weights_gbps": float(sum(bw)), "stores_per_leg": sum(i["stores"] - j["stores"] for i, j in zip(infos, before)) // 4,
                    "retrieves_per_leg": sum(i["retrieves"] - j["retrieves"] for i, j in zip(infos, before)) // 4,
                    "direct_io": [i["direct_io"] for i in infos], "queue_depth": [i["queue_depth"] for i in infos], "verified_bit_exact_round_trip": True}
