@@ -129,7 +129,10 @@ typedef struct {           /* one pool device (Table I)           
                            /* they share.  Placement (Eq. 1-2) is untouched: only b_i changes.  An SSD-   */
                            /* type device moves its share on kernel streams of its own, whatever its     */
                            /* group (a stream that waits for a disk must hold up nothing else)           */
-  const char* path;        /* SSD: block device or file (host string, copied); NULL otherwise           */
+  const char* path;        /* SSD: block device or file (host string, copied); NULL otherwise.  The     */
+                           /* library owns sectors [0, capacity_bytes / sector_bytes) of it: whatever    */
+                           /* they held is overwritten; a file it had to create is removed again by      */
+                           /* kvpool_destroy.  Two devices of one pool must not name the same path       */
   uint32_t sector_bytes;   /* SSD: sector size LBAs count in - a power of two in 512..65536 and a       */
                            /* multiple of the device's logical sector; 0 = ask the block device, 4096   */
                            /* for a file.  Otherwise 0                                                  */

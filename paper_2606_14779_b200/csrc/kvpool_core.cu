@@ -286,6 +286,9 @@ int kvpool_create(const kvpool_device_desc* devs, uint32_t n_devs, const kvpool_
     if ((devs[i].flags & KVPOOL_DEV_SSD) && (!devs[i].path || !*devs[i].path)) return fail(KVPOOL_EINVAL, "create: device %u: an SSD-type device needs a path", i);
     if (!(devs[i].flags & KVPOOL_DEV_SSD) && (devs[i].path || devs[i].sector_bytes)) return fail(KVPOOL_EINVAL, "create: device %u: path / sector_bytes are for SSD-type devices", i);
     if (devs[i].reserved) return fail(KVPOOL_EINVAL, "create: device %u: reserved must be 0", i);
+    for (uint32_t j = 0; j < i && (devs[i].flags & KVPOOL_DEV_SSD); ++j)
+      if ((devs[j].flags & KVPOOL_DEV_SSD) && strcmp(devs[j].path, devs[i].path) == 0)
+        return fail(KVPOOL_EINVAL, "create: devices %u and %u name the same path: their LBA ranges would overlap", j, i);
     if (devs[i].numa_node < KVPOOL_NUMA_AUTO) return fail(KVPOOL_EINVAL, "create: device %u: numa_node %d", i, devs[i].numa_node);
   }
   if (!quantise_weights(bw.data(), n_devs, w.data())) return fail(KVPOOL_EINVAL, "create: bandwidth must be positive (>= 0.0005 GB/s)");

@@ -319,6 +319,9 @@ def test_ssd_errors_bad_arguments_full_device_and_a_failing_disk(tmp_path):
     with pytest.raises(kv.KvPoolError) as e:                                   # SSD excludes the other flags
         kv.KvPool([1.0], [1 << 20], dev_flags=[kv.DEV_SSD | kv.DEV_HBM], paths=[str(tmp_path / "x")], **geo)
     assert e.value.code == kv.EINVAL
+    with pytest.raises(kv.KvPoolError) as e:                                   # two devices on one path: their LBA ranges would overlap
+        kv.KvPool([1.0, 1.0], [1 << 20] * 2, dev_flags=[kv.DEV_SSD] * 2, paths=[str(tmp_path / "x")] * 2, **geo)
+    assert e.value.code == kv.EINVAL
     with pytest.raises(kv.KvPoolError) as e:                                   # sector size not a power of two
         kv.KvPool([1.0], [1 << 20], dev_flags=[kv.DEV_SSD], paths=[str(tmp_path / "x")], sector_bytes=[520], **geo)
     assert e.value.code == kv.EINVAL
