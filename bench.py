@@ -89,6 +89,7 @@ def parse_args():
                          "copies stay concurrent inside a range; per-kernel profiling would serialise them)")
     ap.add_argument("--hostalloc", action="store_true", help="pool buffers from cudaHostAlloc (KVPOOL_DEV_CUDA_HOSTALLOC) instead of the default "
                     "huge-page mapping + cudaHostRegister; main run and --duplex")
+    ap.add_argument("--contexts", default="1024,4096,16384,32768,65536,131072", help="--blocked-io: the context lengths to run, comma separated")
     ap.add_argument("--compute-us", type=float, default=0.0, help="--blocked-io: extra calibrated compute per layer (kvpool_spin), microseconds")
     ap.add_argument("--detail", default=None, help="write per-layer latencies and side measurements to this JSON file")
     return ap.parse_args()
@@ -1387,11 +1388,11 @@ def run_blocked_io(args) -> None:
           f"{' + kvpool_spin' if spin_ns else ''}; times in ms; blocked = total - consumer-alone (PAPER.md:72)")
     print("# serial = retrieve(l); consume(l); host sync, layer by layer (Fig. 2a).  pipelined = all retrieves enqueued on one stream, "
           "consume(l) on another after layer l's event (Fig. 2b).  batched = the same pipeline through ONE kvpool_retrieve_layers_signal call "
-          "(the library records the per-layer events; small layers move in groups)")
+          "(the library records the per-layer events; small layers move in groups) with the consumers enqueued by ONE kvpool_checksum_layers call")
     print(f"{'shape':22s} {'ctx':>7s} {'MiB':>8s} {'io_alone':>9s} {'consume':>8s} {'serial':>8s} {'blocked':>8s} {'pipelined':>9s} {'blocked':>8s} {'GB/s':>6s} {'batched':>9s} {'blocked':>8s} {'GB/s':>6s}")
     rows = []
     for cfg in (6, 3, 4):
-        for ctx in (1024, 4096, 16384, 32768, 65536, 131072):
+        for ctx in [int(x) for x in args.contexts.split(",")]:
             wl = W.make_workload(cfg, scale=ctx / 131072)
             g, L = wl.geom, wl.geom.n_layers
             bw = list(wl.default_weights())
@@ -1400,6 +1401,8 @@ def run_blocked_io(args) -> None:
             caps = [int(moved * sh * 1.25) + (L + 4) * (g.payload + 4096) for sh in share]
             pool = kv.KvPool(bw, caps, n_layers=L, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim,
                              link_groups=[1] * len(bw) if args.link_groups == "shared" else None)
+            if args.link_ctas:
+                pool.set_tuning(link_ctas=args.link_ctas)
             bpl = wl.blocks_per_layer(0)
             pl = pool.place(bpl)
             elems = g.kvb // 2
@@ -1458,12 +1461,15 @@ def run_blocked_io(args) -> None:
                     sb.wait_event(e)
                     consume(l, 2, sb)
 
-            def pipelined_batched():        # ONE host call for the request; small layers travel in groups and become ready together
-                sums[3].zero_()
+            def pipelined_batched():        # ONE host call for the request; small layers travel in groups and become ready together;
+                sums[3].zero_()             # the consumer side is one host call too (the layer loop of an engine is not Python)
                 pool.retrieve_layers_signal(pl, 0, dst_k, dst_v, g.kvb, tables, ready, sa)
-                for l in range(L):
-                    sb.wait_event(ready[l])
-                    consume(l, 3, sb)
+                if spin_ns:
+                    for l in range(L):
+                        sb.wait_event(ready[l])
+                        consume(l, 3, sb)
+                else:
+                    pool.checksum_layers(dst_k, dst_v, g.kvb, tables, bpl, ready, sums[3], sb)
 
             t_io, t_c = wall(io_alone), wall(consume_alone)
             t_ser, t_pipe, t_pb = wall(serial), wall(pipelined), wall(pipelined_batched)

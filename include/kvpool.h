@@ -319,12 +319,16 @@ KVPOOL_API int kvpool_retrieve_layers(kvpool_t* pool, kvpool_placement_t* pl, ui
                            void* const* k_bases /*host[n_layers]*/, void* const* v_bases /*host[n_layers]*/,
                            uint64_t block_stride_bytes, const int32_t* const* block_tables /*host[n_layers]*/, void* cuda_stream);
 /* kvpool_retrieve_layers for a consumer on ANOTHER stream (layerwise pipelining): layer_ready is a HOST
- * array of n_layers caller-owned cudaEvent_t (entries may be NULL); layer_ready[q] is recorded on `stream` as soon as layer
+ * array of n_layers caller-owned cudaEvent_t (entries may be NULL); layer_ready[q] is recorded as soon as layer
  * first_layer + q is complete in the paged layout, so the consumer does cudaStreamWaitEvent(consumer, layer_ready[q]) and
  * computes layer q while the pool is still moving layers q+1, ... (the staged path's host->GPU copies run up to
- * `stage_slots` layers ahead).  Layers that travel as one group (small layers, see above) become ready together (a request
- * smaller than one group is cut into two groups here, so that the consumer of the first overlaps the second); a layer
- * with K_l = 0 is ready at once.  One host call per request instead of one per layer.                                 */
+ * `stage_slots` layers ahead).  Layers that travel as one group (small layers, see above) become ready together — except
+ * in a request of less than two groups' worth of bytes on KVPOOL_PATH_ZEROCOPY: that one moves as ONE launch
+ * whose kernel raises a flag as each layer's last byte lands, and a stream of the library's own turns the flags into the
+ * caller's events (stream wait-value, then event record), so every layer is handed over by itself although no launch and
+ * no copy is spent on it alone; such events are recorded on that stream, not on `stream`.  (On the other paths such a
+ * request is cut into two groups, so that the consumer of the first overlaps the second.)  A layer with K_l = 0 is ready
+ * at once.  One host call per request instead of one per layer.                                                       */
 KVPOOL_API int kvpool_retrieve_layers_signal(kvpool_t* pool, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers,
                                   void* const* k_bases /*host[n_layers]*/, void* const* v_bases /*host[n_layers]*/,
                                   uint64_t block_stride_bytes, const int32_t* const* block_tables /*host[n_layers]*/,

@@ -37,6 +37,15 @@ KVPOOL_API int kvpool_retrieve_naive(kvpool_t* pool, kvpool_placement_t* pl, uin
  * (n_blocks*P bytes of HBM reads).  kvb must be a multiple of 16.  Ordered on `stream`.                          */
 KVPOOL_API int kvpool_checksum(kvpool_t* pool, const void* k_base /*device*/, const void* v_base /*device*/, uint64_t block_stride_bytes,
                     const int32_t* block_table_dev, uint32_t n_blocks, uint64_t* sum_dev /*device*/, void* cuda_stream);
+/* The consumer side of kvpool_retrieve_layers_signal in one host call (what a serving engine's C++ layer loop does; a Python
+ * loop of 2 x n_layers calls costs more host time than a 1K-token request takes to arrive): for q = 0 .. n_layers-1,
+ * `stream` waits for layer_ready[q] (cudaEvent_t; NULL = no wait) and then runs kvpool_checksum over layer q's
+ * n_blocks[q] blocks into sums_dev[q].  k_bases / v_bases / block_tables_dev / layer_ready / n_blocks are HOST arrays of
+ * n_layers entries; sums_dev is a device array of n_layers uint64 the caller has zeroed.                            */
+KVPOOL_API int kvpool_checksum_layers(kvpool_t* pool, uint32_t n_layers, const void* const* k_bases /*host[n] of device*/,
+                           const void* const* v_bases, uint64_t block_stride_bytes, const int32_t* const* block_tables_dev,
+                           const uint32_t* n_blocks /*host[n]*/, void* const* layer_ready /*host[n] of cudaEvent_t, or NULL*/,
+                           uint64_t* sums_dev /*device[n]*/, void* cuda_stream);
 /* Occupy `stream` for `nanoseconds` with a one-thread kernel (calibrated compute stand-in).                        */
 KVPOOL_API int kvpool_spin(kvpool_t* pool, uint64_t nanoseconds, void* cuda_stream);
 

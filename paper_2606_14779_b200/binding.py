@@ -29,7 +29,7 @@ _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA",
 EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_plan_lba_range", "kvpool_ssd_range", "kvpool_ssd_location", "kvpool_ssd_info", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
     "kvpool_measure_bandwidth", "kvpool_share_bandwidth", "kvpool_calibrate", "kvpool_bandwidths", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release", "kvpool_set_tables",
-    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_spin",
+    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_checksum_layers", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
     "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_validate_table", "kvpool_set_table_check", "kvpool_table_errors", "kvpool_last_error", "kvpool_version",
 ]
@@ -110,6 +110,7 @@ def lib():
             "kvpool_pack": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp, vp],
             "kvpool_unpack": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp, vp],
             "kvpool_checksum": [vp, vp, vp, c_uint64, vp, c_uint32, vp, vp],
+            "kvpool_checksum_layers": [vp, c_uint32, vp, vp, c_uint64, vp, vp, vp, vp, vp],
             "kvpool_spin": [vp, c_uint64, vp],
             "kvpool_n_devices": [vp, POINTER(c_uint32)],
             "kvpool_weights": [vp, vp],
@@ -423,6 +424,15 @@ class KvPool:
     def checksum(self, k_base, v_base, block_stride_bytes: int, block_table_dev, n_blocks: int, sum_dev, stream=None) -> None:
         _ck(lib().kvpool_checksum(self.handle, _addr(k_base), _addr(v_base), block_stride_bytes, _addr(block_table_dev), n_blocks,
                                   _addr(sum_dev), _stream(stream)))
+
+    def checksum_layers(self, k_bases, v_bases, block_stride_bytes: int, block_tables, n_blocks, layer_ready, sums_dev, stream=None) -> None:
+        """For every layer q: `stream` waits for layer_ready[q] (torch event / handle / None), then checksums the layer into sums_dev[q]."""
+        n = len(k_bases)
+        ka, va, ta = self._ptr_array(k_bases), self._ptr_array(v_bases), self._ptr_array(block_tables)
+        nb = (c_uint32 * n)(*[int(x) for x in n_blocks])
+        ea = (c_void_p * n)(*[_event(e) for e in layer_ready]) if layer_ready is not None else None
+        _ck(lib().kvpool_checksum_layers(self.handle, n, ctypes.addressof(ka), ctypes.addressof(va), block_stride_bytes, ctypes.addressof(ta),
+                                         ctypes.addressof(nb), ctypes.addressof(ea) if ea is not None else None, _addr(sums_dev), _stream(stream)))
 
     def spin(self, nanoseconds: int, stream=None) -> None:
         _ck(lib().kvpool_spin(self.handle, int(nanoseconds), _stream(stream)))

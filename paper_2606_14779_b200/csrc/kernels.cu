@@ -79,6 +79,7 @@ struct Piece {
   uint8_t* paged;
   uint8_t* pooled;
   uint32_t bytes;
+  uint32_t layer;  // MultiArgs: index of the piece's layer in the launch
 };
 // Table check (opt-in, kvpool_set_table_check): a table entry outside the paged pool must neither be read nor written.
 // The piece is turned into a copy of the pool-side bytes onto themselves (harmless in both directions, and the bulk ring
@@ -111,6 +112,7 @@ __device__ __forceinline__ Piece decode(const LayerArgs& a, uint64_t t, uint32_t
   p.paged = (half ? a.v_base : a.k_base) + static_cast<uint64_t>(phys) * a.stride + off;
   p.pooled = reinterpret_cast<uint8_t*>(a.pool_base[d]) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;
   p.bytes = min(piece_bytes, a.kvb - off);
+  p.layer = 0;
   if constexpr (CHECK)
     if (a.nphys_check && static_cast<uint32_t>(phys) >= a.nphys_check) reject(p, a.bad, r == 0);
   return p;
@@ -139,6 +141,7 @@ __device__ __forceinline__ Piece decode(const MultiArgs& a, uint64_t t, uint32_t
   p.paged = (half ? L.v_base : L.k_base) + static_cast<uint64_t>(phys) * a.stride + off;
   p.pooled = reinterpret_cast<uint8_t*>(__ldg(L.pool_base + d) + a.delta[d]) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;
   p.bytes = min(piece_bytes, a.kvb - off);
+  p.layer = lo;
   if constexpr (CHECK)
     if (a.nphys_check && static_cast<uint32_t>(phys) >= a.nphys_check) reject(p, a.bad, r == 0);
   return p;
@@ -146,7 +149,20 @@ __device__ __forceinline__ Piece decode(const MultiArgs& a, uint64_t t, uint32_t
 __device__ __forceinline__ uint32_t units(const LayerArgs& a) { return a.K; }
 __device__ __forceinline__ uint32_t units(const MultiArgs& a) { return a.total_units; }
 
-template <bool PACK, int kVecUnroll, class Args>
+// SIGNAL (MultiArgs only): per-layer completion flags, see kernels.cuh.
+__device__ __forceinline__ void signal_piece(const MultiArgs& a, const Piece& p, uint32_t pieces, uint32_t lane) {
+  __threadfence();  // this lane's stores of the piece are visible device-wide ...
+  __syncwarp();     // ... and so are the other lanes' before lane 0 counts the piece
+  if (lane != 0) return;
+  const uint32_t want = a.d[p.layer].K * 2u * pieces;
+  if (atomicAdd(a.sig_count + p.layer, 1u) + 1u == want) {
+    a.sig_count[p.layer] = 0;  // clean for the next launch that is given this set of flags
+    __threadfence();
+    atomicExch(a.sig_flag + p.layer, a.sig_seq);
+  }
+}
+
+template <bool PACK, int kVecUnroll, class Args, bool SIGNAL = false>
 __global__ void __launch_bounds__(kVecMaxThreads) kv_copy_vec16(const __grid_constant__ Args a) {
   constexpr uint32_t kVecPiece = kVecUnroll * 32 * 16;  // bytes per warp iteration (4 KiB at unroll 8)
   const uint32_t lane = threadIdx.x & 31u;
@@ -174,6 +190,7 @@ __global__ void __launch_bounds__(kVecMaxThreads) kv_copy_vec16(const __grid_con
       for (int u = 0; u < kVecUnroll; ++u)
         if (u * 512u + lane * 16u < p.bytes) st_stream(dst + u * 512, v[u]);
     }
+    if constexpr (SIGNAL) signal_piece(a, p, pieces, lane);
   }
   if (a.span) {  // uniform across the grid
     // The end of the launch is set by the CTAs that retire last; only those wait for their stores to land (a fence in
@@ -410,7 +427,20 @@ cudaError_t launch_layer_copy(const LayerArgs& a, bool pack, const LaunchCfg& cf
   return launch_copy(a, a.K, pack, cfg, stream);
 }
 
+// A retrieve that raises a flag per layer (MultiArgs::sig_flag): the 16-byte kernel, whose stores are plain and can be
+// fenced piece by piece (the bulk kernel's asynchronous stores retire in groups).
+static cudaError_t launch_multi_signal(const MultiArgs& a, const LaunchCfg& cfg, cudaStream_t stream) {
+  if (a.total_units == 0) return cudaSuccess;
+  const uint32_t threads = cfg.vec_threads ? cfg.vec_threads : kVecMaxThreads;
+  const uint32_t pieces = (a.kvb + 4095u) / 4096u;
+  const uint64_t total = static_cast<uint64_t>(a.total_units) * 2u * pieces;
+  const uint64_t want = (total + (threads / 32) - 1) / (threads / 32);
+  const uint32_t grid = static_cast<uint32_t>(want < cfg.ctas ? want : cfg.ctas);
+  return launch_ex(kv_copy_vec16<false, 8, MultiArgs, true>, grid, threads, 0, stream, cfg.pdl, a);
+}
+
 cudaError_t launch_multi_copy(const MultiArgs& a, bool pack, const LaunchCfg& cfg, cudaStream_t stream) {
+  if (a.sig_flag && !pack) return launch_multi_signal(a, cfg, stream);
   return launch_copy(a, a.total_units, pack, cfg, stream);
 }
 

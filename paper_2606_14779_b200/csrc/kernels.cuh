@@ -71,7 +71,14 @@ struct MultiArgs {
   uint32_t chain;        // kChain*, as in LayerArgs
   unsigned long long* span;  // as in LayerArgs
   unsigned long long* bad;   // as in LayerArgs
-  uint32_t nphys_check, pad2;
+  uint32_t nphys_check;
+  // Per-layer completion signals (retrieve only; null = none): the warp that finishes the last piece of layer i of the launch
+  // raises sig_flag[i] = sig_seq once every store of that layer is visible device-wide (sig_count[i] counts the pieces and
+  // is left at zero again).  A stream wait-value on the flag then stands where an event record after a launch of that
+  // layer alone would: ONE launch moves many small layers and still hands them over one by one (kvpool_retrieve_layers_signal).
+  uint32_t sig_seq;
+  uint32_t* sig_count;
+  uint32_t* sig_flag;
   uint64_t delta[kMaxDev];  // added (mod 2^64) to pool_base[i]: 0 for the mapped host stripes themselves, or the
                             // displacement that maps device i's span of stripes onto its copy in a staging slot
   MultiDesc d[kMaxBatch];

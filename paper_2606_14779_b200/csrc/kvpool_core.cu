@@ -392,6 +392,10 @@ int kvpool_destroy(kvpool_t* p) {
   ssd_close_all(p);  // (after the device-wide synchronize above: every command has had the GPU's half)
   free_slots(p);
   for (auto s : p->own_streams) cudaStreamDestroy(s);
+  for (auto& x : p->sig) {  // (their streams are in own_streams)
+    if (x.mem_d) cudaFree(x.mem_d);
+    if (x.done) cudaEventDestroy(x.done);
+  }
   for (auto& b : p->bufs) host_buffer_free(&b);
   if (p->table_arena) cudaFree(p->table_arena);
   if (p->table_arena_host) cudaFreeHost(p->table_arena_host);

@@ -110,7 +110,10 @@ int launch_multi_counted(kvpool* p, const MultiArgs& ma, bool pack, bool link_bo
   }
   MultiArgs timed = ma;
   if (p->profiling) timed.span = take_span(p, &r);
-  CU(launch_multi_copy(timed, pack, launch_cfg(p, link_bound, pack), s));
+  LaunchCfg cfg = launch_cfg(p, link_bound, pack);
+  // a signalled retrieve runs the 16-byte kernel (kernels.cu): 8 CTAs of it fill the link (profiles/r1_sweep_link.txt)
+  if (ma.sig_flag && link_bound && !p->hbm_mask) cfg.ctas = std::max<uint32_t>(cfg.ctas, 8);
+  CU(launch_multi_copy(timed, pack, cfg, s));
   p->n_kernels++;
   if (p->profiling) return prof_end(p, &r, s);
   return KVPOOL_OK;
@@ -178,6 +181,21 @@ int kvpool_checksum(kvpool_t* p, const void* k_base, const void* v_base, uint64_
                      static_cast<uint32_t>(p->kvb), reinterpret_cast<unsigned long long*>(sum_dev), p->tune.hbm_ctas,
                      static_cast<cudaStream_t>(cuda_stream)));
   p->n_kernels++;
+  return KVPOOL_OK;
+}
+
+int kvpool_checksum_layers(kvpool_t* p, uint32_t n_layers, const void* const* k_bases, const void* const* v_bases, uint64_t stride,
+                           const int32_t* const* tables, const uint32_t* n_blocks, void* const* layer_ready, uint64_t* sums_dev,
+                           void* cuda_stream) {
+  PoolLock lock__(p);
+  if (!p || !k_bases || !v_bases || !tables || !n_blocks || !sums_dev) return fail(KVPOOL_EINVAL, "checksum_layers: null argument");
+  DeviceGuard guard(p->cuda_device);
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  for (uint32_t q = 0; q < n_layers; ++q) {
+    if (layer_ready && layer_ready[q]) CU(cudaStreamWaitEvent(s, static_cast<cudaEvent_t>(layer_ready[q]), 0));
+    const int rc = kvpool_checksum(p, k_bases[q], v_bases[q], stride, tables[q], n_blocks[q], sums_dev + q, s);
+    if (rc != KVPOOL_OK) return rc;
+  }
   return KVPOOL_OK;
 }
 

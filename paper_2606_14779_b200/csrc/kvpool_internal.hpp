@@ -129,6 +129,16 @@ struct SsdState {  // one SSD-type pool device (KV-passthrough, PAPER.md:179-185
 };
 constexpr uint64_t kSsdScratchBytes = 4ull << 20;
 
+// Per-layer completion flags of one signalled multi-layer retrieve (kernels.cuh, MultiArgs::sig_flag) and the stream that
+// turns them into the caller's per-layer events: [wait-value(flag of layer 0)] [record ready[0]] [wait-value(flag 1)] ...
+struct SignalSet {
+  uint32_t* mem_d = nullptr;       // device: kMaxBatch piece counters, then kMaxBatch flags
+  cudaStream_t stream = nullptr;   // a stream per set: a launch held up on its own stream delays nobody else's events
+  cudaEvent_t done = nullptr;      // the launch that used the set last has completed (its counters are back at zero)
+  uint32_t seq = 0;                // flags of the set's latest launch read >= seq
+};
+constexpr uint32_t kSignalSets = 8;
+
 }  // namespace kvp
 
 struct GltHash {  // Table I `key`: splitmix64 finaliser of the identifier
@@ -174,6 +184,8 @@ struct kvpool {
   std::vector<kvp::HostBuffer> bufs;
   std::vector<uint32_t> link_group;  // [N] kvpool_device_desc.link_group: devices of one group share io / io_out streams
   std::vector<cudaStream_t> own_streams;  // every stream created for io / io_out, once (members of a group alias one)
+  std::vector<kvp::SignalSet> sig;  // made on first use
+  uint32_t sig_cursor = 0;
   bool ssd_defer_join = false;  // inside kvpool_offload_layers: see SsdState::join_pending
   uint32_t ssd_mask = 0;  // bit i: pool device i is block storage (KVPOOL_DEV_SSD): its share of a layer moves through bounce lanes
   std::vector<std::unique_ptr<kvp::SsdState>> ssd;  // [N], null for the other types
@@ -245,6 +257,10 @@ inline uint8_t* pool_bytes(const kvpool* p, uint32_t i) {
 inline bool is_ssd(const kvpool* p, uint32_t i) { return (p->ssd_mask >> i) & 1u; }
 inline bool is_mem(const kvpool* p, uint32_t i) { return !is_hbm(p, i) && !is_ssd(p, i); }
 inline bool has_mem(const kvpool* p) { return ((p->hbm_mask | p->ssd_mask) & (p->n >= 32 ? 0xFFFFFFFFu : (1u << p->n) - 1u)) != (p->n >= 32 ? 0xFFFFFFFFu : (1u << p->n) - 1u); }
+// kvpool_ssd.cu: stream memory operations (cuStreamWaitValue32 / cuStreamWriteValue32 through the runtime's entry-point query)
+int memops_init();                                                        // ECUDA where the driver has none
+int stream_wait_geq(cudaStream_t s, uint64_t dev_addr, uint32_t value);  // `s` waits until (int32)(*addr - value) >= 0
+int stream_write(cudaStream_t s, uint64_t dev_addr, uint32_t value);     // fenced: earlier writes of `s` are visible first
 // kvpool_ssd.cu: SSD-type pool devices
 int ssd_open(kvpool* p, uint32_t i, const kvpool_device_desc& d);  // kvpool_create
 void ssd_close_all(kvpool* p);                                      // kvpool_destroy / failed create

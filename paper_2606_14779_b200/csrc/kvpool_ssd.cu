@@ -31,6 +31,15 @@ using MemOpFn = int (*)(cudaStream_t, unsigned long long, unsigned int, unsigned
 MemOpFn g_wait_value = nullptr, g_write_value = nullptr;
 constexpr unsigned int kWaitGeq = 0x0, kWriteDefault = 0x0;  // CU_STREAM_WAIT_VALUE_GEQ (wrap-aware), CU_STREAM_WRITE_VALUE_DEFAULT (fenced)
 
+}  // namespace
+
+int stream_wait_geq(cudaStream_t s, uint64_t dev_addr, uint32_t value) {
+  return g_wait_value(s, dev_addr, value, kWaitGeq) == 0 ? KVPOOL_OK : fail(KVPOOL_ECUDA, "cuStreamWaitValue32 failed");
+}
+int stream_write(cudaStream_t s, uint64_t dev_addr, uint32_t value) {
+  return g_write_value(s, dev_addr, value, kWriteDefault) == 0 ? KVPOOL_OK : fail(KVPOOL_ECUDA, "cuStreamWriteValue32 failed");
+}
+
 int memops_init() {
   if (g_wait_value && g_write_value) return KVPOOL_OK;
   void *w = nullptr, *r = nullptr;
@@ -43,6 +52,8 @@ int memops_init() {
   g_write_value = reinterpret_cast<MemOpFn>(r);
   return KVPOOL_OK;
 }
+
+namespace {
 
 #define DRV(call)                                                                         \
   do {                                                                                    \

@@ -353,7 +353,30 @@ struct BatchCall {
   void* const* ready;  // optional: caller-owned cudaEvent_t per layer of the call, recorded on `s` when that layer is complete
   bool* chain_run;     // the launch enqueued last on `s` by this call heads / follows a run of chained launches (kernels.cuh)
   std::vector<LayerState*>* landed_later;  // offloads of a chained run: their `landed` events are recorded behind the run
+  bool signal;         // a small request with a consumer behind per-layer events: groups move zero-copy, ONE launch that
+                       // raises a flag per layer (kernels.cuh); *signalled says the group's ready events are taken care of
+  bool* signalled;
 };
+
+// The next set of per-layer flags (round-robin over kSignalSets, made on first use); `s` waits for the launch that used it last.
+int take_signal_set(kvpool* p, cudaStream_t s, SignalSet** out) {
+  if (p->sig.empty()) {
+    std::vector<SignalSet> v(kSignalSets);
+    for (auto& x : v) {
+      CU(cudaMalloc(reinterpret_cast<void**>(&x.mem_d), 2ull * kMaxBatch * sizeof(uint32_t)));
+      CU(cudaMemsetAsync(x.mem_d, 0, 2ull * kMaxBatch * sizeof(uint32_t), p->upload));
+      CU(cudaStreamCreateWithFlags(&x.stream, cudaStreamNonBlocking));
+      CU(cudaEventCreateWithFlags(&x.done, cudaEventDisableTiming));
+      p->own_streams.push_back(x.stream);  // kvpool_release / kvpool_synchronize wait for them too
+    }
+    CU(cudaStreamSynchronize(p->upload));
+    p->sig = std::move(v);
+  }
+  SignalSet& x = p->sig[p->sig_cursor++ % p->sig.size()];
+  CU(cudaStreamWaitEvent(s, x.done, 0));
+  *out = &x;
+  return KVPOOL_OK;
+}
 
 // Record the `landed` events a chained run of offload launches has put off (an event record between two launches would
 // undo the chaining): behind the run's last launch every one of its layers is complete in the pool.
@@ -404,6 +427,27 @@ int issue_zero_copy_group(const BatchCall& c, const LayerGroup& g) {
   // predecessor's last wave drains.  Only where the launches are back to back on the stream (no event wait or record
   // between them, no profiling markers) and many waves long (the HBM grid; a 4-CTA link launch would let the whole
   // request start at once and lose the layer order).
+  if (c.signal && !c.pack && g.n > 1) {
+    // ONE launch for the group, and still one hand-over per layer: the kernel raises a flag when a layer's last piece has
+    // landed; a stream of the flag set's own waits for the flags in layer order and records the caller's events behind them
+    SignalSet* x = nullptr;
+    int rc = take_signal_set(p, c.s, &x);
+    if (rc != KVPOOL_OK) return rc;
+    ma.sig_count = x->mem_d;
+    ma.sig_flag = x->mem_d + kMaxBatch;
+    ma.sig_seq = ++x->seq;
+    *c.chain_run = false;
+    if ((rc = flush_landed(c)) != KVPOOL_OK) return rc;
+    if ((rc = launch_multi_counted(p, ma, false, true, c.s)) != KVPOOL_OK) return rc;
+    CU(cudaEventRecord(x->done, c.s));
+    for (uint32_t b = 0; b < g.n; ++b) {
+      if (!c.ready[g.q[b]]) continue;
+      if ((rc = stream_wait_geq(x->stream, reinterpret_cast<uint64_t>(ma.sig_flag + b), ma.sig_seq)) != KVPOOL_OK) return rc;
+      CU(cudaEventRecord(static_cast<cudaEvent_t>(c.ready[g.q[b]]), x->stream));
+    }
+    *c.signalled = true;
+    return KVPOOL_OK;
+  }
   const bool chain = p->hbm_mask && !c.ready && !waited && !p->profiling && p->tune.pdl != 2;
   ma.chain = !chain ? kChainNone : (*c.chain_run ? kChainFollower : kChainHead);
   if (!chain) {
@@ -528,8 +572,9 @@ int issue_group_work(const BatchCall& c, const LayerGroup& g);
 // Move one group, then tell the caller's per-layer events: the layers of a group become ready together.
 int issue_group(const BatchCall& c, const LayerGroup& g) {
   if (g.n == 0) return KVPOOL_OK;
+  *c.signalled = false;
   const int rc = issue_group_work(c, g);
-  if (rc != KVPOOL_OK || !c.ready) return rc;
+  if (rc != KVPOOL_OK || !c.ready || *c.signalled) return rc;
   for (uint32_t b = 0; b < g.n; ++b)
     if (c.ready[g.q[b]]) CU(cudaEventRecord(static_cast<cudaEvent_t>(c.ready[g.q[b]]), c.s));
   return KVPOOL_OK;
@@ -537,7 +582,7 @@ int issue_group(const BatchCall& c, const LayerGroup& g) {
 
 int issue_group_work(const BatchCall& c, const LayerGroup& g) {
   kvpool* p = c.p;
-  if (!use_staged(p, c.pack, g.host_bytes)) return issue_zero_copy_group(c, g);
+  if ((c.signal && !p->ssd_mask) || !use_staged(p, c.pack, g.host_bytes)) return issue_zero_copy_group(c, g);
   if (g.n > 1) {
     const int rc = issue_staged_group(c, g);
     if (rc != 1) return rc;
@@ -594,20 +639,29 @@ static int layers_batched_locked(kvpool_t* p, kvpool_placement_t* pl, bool pack,
   DeviceGuard guard(p->cuda_device);
   bool chain_run = false;
   std::vector<LayerState*> landed_later;
-  const BatchCall c{p, pl, pack, first, k_bases, v_bases, tables, stride, static_cast<cudaStream_t>(cuda_stream), ready, &chain_run, &landed_later};
+  uint64_t cap = std::max<uint64_t>(p->tune.group_bytes, 1);
+  bool signal = false, signalled = false;
+  if (ready) {
+    // A consumer follows behind the per-layer events.  On the zero-copy path a request so small that it would travel as
+    // one or two groups (all of a group's layers ready together: the consumer hardly overlapped) moves as ONE launch that
+    // signals every layer as it completes, so that the consumer of layer l runs under the transfer of layer l+1.  (Not
+    // the default for such requests: through the copy engines the link runs 8 % faster than under SM-issued reads, and two
+    // staged groups beat the signalled launch — GPT-OSS-shaped KV at 1K context, 27 MiB: 0.566 against 0.594 ms.)
+    uint64_t total = 0;
+    for (uint32_t q = 0; q < n; ++q) total += pl->layers[first + q].map->K * p->payload;
+    if (!pack && total < 2 * cap && p->path == KVPOOL_PATH_ZEROCOPY && !p->ssd_mask && memops_init() == KVPOOL_OK) {
+      signal = true;
+      cap = std::max<uint64_t>(total, 1);
+    } else if (total < cap) {
+      cap = std::max<uint64_t>((total + 1) / 2, 1);  // else cut it in two, so that the first half's consumer runs under the second half's transfer
+    }
+  }
+  const BatchCall c{p, pl, pack, first, k_bases, v_bases, tables, stride, static_cast<cudaStream_t>(cuda_stream), ready, &chain_run, &landed_later,
+                    signal, &signalled};
   struct Flush {  // whatever path leaves the call: the events put off so far are recorded
     const BatchCall& c;
     ~Flush() { flush_landed(c); }
   } flush_on_exit{c};
-  uint64_t cap = std::max<uint64_t>(p->tune.group_bytes, 1);
-  if (ready) {
-    // a consumer follows behind the per-layer events: a request so small that it would travel as ONE group (all layers
-    // ready together, the consumer not overlapped at all) is cut in two, so that the consumer of the first half runs
-    // under the transfer of the second (GPT-OSS-shaped KV at 1K context: 27 MiB; profiles/r2_blocked_io.txt)
-    uint64_t total = 0;
-    for (uint32_t q = 0; q < n; ++q) total += pl->layers[first + q].map->K * p->payload;
-    if (total < cap) cap = std::max<uint64_t>((total + 1) / 2, 1);
-  }
   LayerGroup g;
   uint64_t units = 0;
   for (uint32_t q = 0; q < n; ++q) {

@@ -402,6 +402,10 @@ def test_checksum_consumer_matches_oracle_and_detects_round_trip():
             out = torch.zeros(3, dtype=torch.int64, device=dev)
             pool.checksum(src[0], src[1], wl.geom.kvb, table, n, out[0:1])
             pool.checksum(src[0], src[1], wl.geom.kvb, table, n // 2, out[1:2])
+            both = torch.zeros(2, dtype=torch.int64, device=dev)                 # the same two through the one-call layer loop
+            pool.checksum_layers([src[0], src[0]], [src[1], src[1]], wl.geom.kvb, [table, table], [n, n // 2], None, both)
+            torch.cuda.synchronize()
+            assert torch.equal(both, out[0:2])
             want = oracle.checksum(W.kv_layer_numpy(wl, 0), table_np)
             want_half = oracle.checksum(W.kv_layer_numpy(wl, 0), table_np[:n // 2])
             pl = pool.place(wl.blocks_per_layer(0))

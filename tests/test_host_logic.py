@@ -27,7 +27,7 @@ def test_library_exports_every_symbol_declared_in_header():
     product = set(re.findall(pat, open(os.path.join(ROOT, "include", "kvpool.h")).read()))
     devel = set(re.findall(pat, open(os.path.join(ROOT, "include", "kvpool_dev.h")).read()))
     # the product header is the boundary SURVEY.md 8(b) lists; baselines, stand-ins, counters and profiling live apart
-    assert devel == {"kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_checksum", "kvpool_spin", "kvpool_stats",
+    assert devel == {"kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_checksum", "kvpool_checksum_layers", "kvpool_spin", "kvpool_stats",
                      "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock"} and not (devel & product)
     declared = sorted(product | devel)
     assert len(declared) >= 27 and "kvpool_create" in declared and "kvpool_retrieve" in declared
