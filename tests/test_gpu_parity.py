@@ -603,6 +603,62 @@ def test_layer_ready_events_fire_layer_by_layer_not_at_the_end_of_the_request(pa
         pool.destroy()
 
 
+@pytest.mark.parametrize("kernel", list(KERNELS))
+def test_one_signalled_launch_hands_small_layers_over_one_by_one(kernel):
+    """Zero-copy path, a request of 32 layers x 2 MiB (less than two groups' worth): kvpool_retrieve_layers_signal moves it
+    with ONE kernel launch whose kernel raises a flag per layer; the per-layer events, recorded behind stream wait-values on
+    those flags, fire in layer order and spread over the launch (ready[0] long before ready[31]); a consumer that waits on
+    nothing but the events reads the oracle's bytes."""
+    dev = torch.device("cuda:0")
+    wl = W.make_workload(4, scale=1 / 128, n_layers=32)    # 64 blocks x 32 KiB = 2 MiB per layer, 6 buffers 4:4:2:2:1:1
+    g, L = wl.geom, wl.geom.n_layers
+    bw = list(wl.default_weights())
+    pool = make_pool(wl)
+    try:
+        pool.set_path(kv.PATH_ZEROCOPY)
+        pool.set_tuning(kernel=KERNELS[kernel], link_kernel=KERNELS[kernel])
+        bpl = wl.blocks_per_layer(0)
+        pl, opl = pool.place(bpl), oracle.place(bw, bpl)
+        tables_np = [np.ascontiguousarray(wl.layer_table(0, l)) for l in range(L)]
+        tables = [torch.from_numpy(t).to(dev) for t in tables_np]
+        src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+        torch.cuda.synchronize()
+        io, consumer = torch.cuda.Stream(), torch.cuda.Stream()
+        pool.offload_layers(pl, 0, [x[0] for x in src], [x[1] for x in src], g.kvb, tables, io)
+        pool.wait_offloads(pl, io)
+        io.synchronize()
+        pool.synchronize()
+        for attempt in range(3):                           # the flag sets are reused round-robin; the last pass is the measured one
+            dst = [W.poison_torch((2, wl.nphys, g.kvb // 2), dev) for l in range(L)]
+            sums = torch.zeros(L, dtype=torch.int64, device=dev)
+            torch.cuda.synchronize()
+            ready = [torch.cuda.Event() for _ in range(L)]
+            stamps = [torch.cuda.Event(enable_timing=True) for _ in range(L)]
+            k0, m0 = pool.stats()
+            pool.retrieve_layers_signal(pl, 0, [d[0] for d in dst], [d[1] for d in dst], g.kvb, tables, ready, io)
+            k1, m1 = pool.stats()
+            assert (k1 - k0, m1 - m0) == (1, 0)             # one launch, no copy
+            for l in range(L):                             # the consumer never synchronises with `io` except through the events
+                consumer.wait_event(ready[l])
+                stamps[l].record(consumer)
+                pool.checksum(dst[l][0], dst[l][1], g.kvb, tables[l], int(bpl[l]), sums[l:l + 1], consumer)
+            consumer.synchronize()
+            got = [int(x) % 2 ** 64 for x in sums.cpu().tolist()]
+            assert got == [oracle.checksum(W.kv_layer_numpy(wl, l), tables_np[l]) for l in range(L)]
+            io.synchronize()
+        at = [stamps[0].elapsed_time(stamps[l]) for l in range(L)]
+        assert all(b >= a - 0.01 for a, b in zip(at, at[1:])), at          # in layer order
+        assert at[L - 1] > 0.6 and at[L // 2] > 0.25 * at[L - 1], at        # 62 MiB behind layer 0 take > 1 ms on the link: spread over the launch
+        for l in range(L):
+            stripes = oracle.offload_layer(W.kv_layer_numpy(wl, l), tables_np[l], opl[l])
+            ref = W.poison_numpy((2, wl.nphys, g.kvb // 2))
+            oracle.retrieve_layer(ref, tables_np[l], opl[l], stripes)
+            assert np.array_equal(dst[l].cpu().numpy().view(np.uint16), ref), f"retrieved layer {l} differs"
+        pl.release()
+    finally:
+        pool.destroy()
+
+
 def test_release_waits_for_work_still_queued_on_the_callers_stream():
     """kvpool_release must not hand stripes back to the allocator while a kernel on a caller's stream still uses them: a
     zero-copy retrieve queued behind 80 ms of other work is still pending when release is called; release returns only
