@@ -239,7 +239,11 @@ int ssd_move(kvpool* p, LayerState& L, uint32_t i, uint32_t lo, uint32_t hi, boo
                                  return launch_counted(p, a, pack, true, k, true);  // a link-bound launch: 4 CTAs fill the link
                                },
                                &lane, &use);
-    if (rc != KVPOOL_OK) return rc;
+    if (rc != KVPOOL_OK) {  // what has been launched so far still reads / writes the caller's blocks: join it before giving up
+      if (cudaEventRecord(S.join[d], k) == cudaSuccess) cudaStreamWaitEvent(s, S.join[d], 0);
+      cudaGetLastError();
+      return rc;
+    }
     if (pack) {
       L.ssd_last_lane[i] = lane;
       L.ssd_last_use[i] = use;

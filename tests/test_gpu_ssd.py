@@ -537,3 +537,36 @@ def test_ssd_pool_makes_progress_next_to_another_pools_copy_engine_traffic(tmp_p
         stop.set()
         pool.destroy()
         mem.destroy()
+
+
+def test_per_layer_events_with_an_ssd_in_the_pool(tmp_path):
+    """kvpool_retrieve_layers_signal over host memory + an SSD-type device (layerwise pipelining): a layer's
+    event fires once the host buffer's share AND the SSD's share of that layer are in the paged layout; a consumer that waits
+    on nothing but the events reads the oracle's bytes."""
+    wl = W.make_workload(1, n_layers=6)
+    g, dev, L = wl.geom, torch.device("cuda:0"), 6
+    pool, bw, files = _ssd_pool(wl, ["mem", "ssd"], tmp_path, tuning={"ssd_lanes": 2, "ssd_chunk_bytes": 512 << 10})
+    try:
+        bpl = wl.blocks_per_layer(0)
+        pl = pool.place(bpl)
+        tables_np = [np.ascontiguousarray(wl.layer_table(0, l)) for l in range(L)]
+        tables = [torch.from_numpy(t).to(dev) for t in tables_np]
+        src = [W.kv_layer_torch(wl, l, dev) for l in range(L)]
+        dst = [W.poison_torch((2, wl.nphys, g.kvb // 2), dev) for _ in range(L)]
+        sums = torch.zeros(L, dtype=torch.int64, device=dev)
+        torch.cuda.synchronize()
+        io, consumer = torch.cuda.Stream(), torch.cuda.Stream()
+        pool.offload_layers(pl, 0, [x[0] for x in src], [x[1] for x in src], g.kvb, tables, io)
+        ready = [torch.cuda.Event() for _ in range(L)]
+        pool.retrieve_layers_signal(pl, 0, [d[0] for d in dst], [d[1] for d in dst], g.kvb, tables, ready, io)   # (no wait in between)
+        pool.checksum_layers([d[0] for d in dst], [d[1] for d in dst], g.kvb, tables, bpl, ready, sums, consumer)
+        consumer.synchronize()
+        got = [int(x) % 2 ** 64 for x in sums.cpu().tolist()]
+        assert got == [oracle.checksum(W.kv_layer_numpy(wl, l), tables_np[l]) for l in range(L)]
+        io.synchronize()
+        for l in range(L):
+            assert torch.equal(dst[l][:, tables[l].long()], src[l][:, tables[l].long()])
+        pool.synchronize()
+        pl.release()
+    finally:
+        pool.destroy()
