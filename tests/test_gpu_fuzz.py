@@ -1,5 +1,6 @@
 """Randomised choreography test: seeded random sequences of place / offload / re-offload / retrieve / range retrieve /
-batched calls / release over ONE pool, several live placements each on its own stream, random pool flavours (host and
+batched calls (half of the batched retrieves through kvpool_retrieve_layers_signal, with a consumer behind the per-layer
+events) / release over ONE pool, several live placements each on its own stream, random pool flavours (host and
 HBM-type devices), random paths and tuning (1-3 staging slots, small groups), no synchronisation between operations
 except at checkpoints.  Everything the library overlaps — staging-slot recycling, per-device I/O streams, landed events,
 region reuse after release — must still produce the oracle's bytes: every retrieve lands in a fresh poison-filled tensor
@@ -80,6 +81,8 @@ def test_random_sequences_match_the_oracle(seed, ssd, tmp_path):
     kvb = ELEMS * 2
     pending = []                                                               # (dst tensor, expected numpy, description)
     reqs = []
+    signal_rng = np.random.default_rng(4242 + seed)                            # (its own generator: the operation sequences of the seeds stay what they were)
+    consumer = torch.cuda.Stream(device=dev)
 
     def stripes_of(r, l, v=None):
         v = r.version[l] if v is None else v
@@ -177,7 +180,19 @@ def test_random_sequences_match_the_oracle(seed, ssd, tmp_path):
                 if n == 0:
                     continue
                 dsts = [fresh_dst(r) for _ in range(n)]
-                pool.retrieve_layers(r.pl, a, [d[0] for d in dsts], [d[1] for d in dsts], kvb, [r.table] * n, r.stream)
+                if signal_rng.random() < 0.5:
+                    # the same through kvpool_retrieve_layers_signal: a consumer stream that waits on NOTHING but the per-layer
+                    # events snapshots each layer as soon as its event fires; the snapshots must hold the oracle's bytes (on the
+                    # zero-copy path small requests move as one launch that raises a flag per layer, kernels.cuh)
+                    ready = [torch.cuda.Event() for _ in range(n)]
+                    pool.retrieve_layers_signal(r.pl, a, [d[0] for d in dsts], [d[1] for d in dsts], kvb, [r.table] * n, ready, r.stream)
+                    for q, l in enumerate(range(a, a + n)):
+                        consumer.wait_event(ready[q])
+                        with torch.cuda.stream(consumer):
+                            snap = dsts[q].clone()
+                        pending.append((snap, expect(r, l, r.version[l]), ("retrieve_layers_signal snapshot", seed, step, l)))
+                else:
+                    pool.retrieve_layers(r.pl, a, [d[0] for d in dsts], [d[1] for d in dsts], kvb, [r.table] * n, r.stream)
                 for q, l in enumerate(range(a, a + n)):
                     pending.append((dsts[q], expect(r, l, r.version[l]), ("retrieve_layers", seed, step, l)))
             elif op < 0.91:
