@@ -111,7 +111,8 @@ typedef struct kvpool_placement kvpool_placement_t; /* opaque: one request's GLT
 typedef struct {           /* one pool device (Table I)                                    */
   double bandwidth_gbps;   /* b_i of Eq. 1, measured, in 1e9 B/s; > 0                                   */
   uint64_t capacity_bytes; /* size of the buffer the library allocates (pinned + mapped host memory, or */
-                           /* device memory with KVPOOL_DEV_HBM); > 0                                   */
+                           /* device memory with KVPOOL_DEV_HBM), or how much of `path` an SSD-type      */
+                           /* device may use; > 0                                                        */
   int32_t numa_node;       /* MEM: -1 = no preference (the pages land on the nodes of the cores that    */
                            /* fault them in: on a multi-socket host prefer KVPOOL_NUMA_AUTO);           */
                            /* KVPOOL_NUMA_AUTO = the node the pool's GPU hangs off (sysfs; no           */
