@@ -41,8 +41,28 @@ def _backing_file(path, nbytes):
     return str(path)
 
 
-def _ssd_pool(wl, types, tmp_path, *, sector=512, slack=1.5, tuning=None, path=kv.PATH_AUTO, kernel=kv.KERNEL_VEC16, bandwidth=None):
-    """types[i] in {"mem", "ssd", "hbm"}; returns (pool, bw, files) with files[i] the backing file of SSD device i."""
+_LOOPS = []                                       # loop devices attached by _ssd_pool(blockdev=True), detached by _detach_loops
+
+
+def _attach_loop(path):
+    """A loop device over `path` (direct I/O to the backing file): a real block device node for the S_ISBLK branch."""
+    import subprocess
+    r = subprocess.run(["losetup", "-f", "--show", "--direct-io=on", str(path)], capture_output=True, text=True)
+    if r.returncode != 0:
+        pytest.skip(f"no loop device to be had here: {r.stderr.strip()}")
+    _LOOPS.append(r.stdout.strip())
+    return r.stdout.strip()
+
+
+def _detach_loops():
+    import subprocess
+    while _LOOPS:
+        subprocess.run(["losetup", "-d", _LOOPS.pop()], capture_output=True)
+
+
+def _ssd_pool(wl, types, tmp_path, *, sector=512, slack=1.5, tuning=None, path=kv.PATH_AUTO, kernel=kv.KERNEL_VEC16, bandwidth=None, blockdev=False):
+    """types[i] in {"mem", "ssd", "hbm"}; returns (pool, bw, files) with files[i] the backing file of SSD device i (with
+    blockdev: the loop device attached to it, which is then what the pool opens)."""
     g = wl.geom
     bw = list(bandwidth) if bandwidth is not None else list(wl.default_weights())
     share = np.array(bw) / np.sum(bw)
@@ -50,6 +70,8 @@ def _ssd_pool(wl, types, tmp_path, *, sector=512, slack=1.5, tuning=None, path=k
     caps = [(c + 65535) // 65536 * 65536 for c in caps]
     flags = [{"mem": 0, "ssd": kv.DEV_SSD, "hbm": kv.DEV_HBM}[t] for t in types]
     files = [_backing_file(tmp_path / f"ssd{i}.img", caps[i]) if t == "ssd" else None for i, t in enumerate(types)]
+    if blockdev:
+        files = [_attach_loop(f) if f else None for f in files]
     pool = kv.KvPool(bw, caps, n_layers=g.n_layers, n_kv_heads=g.n_kv_heads, head_dim=g.head_dim, block_tokens=g.block_tokens,
                      elem_bytes=g.elem_bytes, dev_flags=flags, paths=files, sector_bytes=[sector if t == "ssd" else 0 for t in types])
     pool.set_path(path)
@@ -83,10 +105,11 @@ def _check_ssd_stripe(pool, pl, l, i, path, want_stripe, payload, opl_l, seen_ra
     return first, n_sec, sec, have, lo
 
 
-def _run(wl, types, tmp_path, *, path="auto", kernel="vec16", sector=512, tuning=None, bandwidth=None, batched=False):
+def _run(wl, types, tmp_path, *, path="auto", kernel="vec16", sector=512, tuning=None, bandwidth=None, batched=False, blockdev=False):
     dev = torch.device("cuda:0")
     g = wl.geom
-    pool, bw, files = _ssd_pool(wl, types, tmp_path, sector=sector, tuning=tuning, path=PATHS[path], kernel=KERNELS[kernel], bandwidth=bandwidth)
+    pool, bw, files = _ssd_pool(wl, types, tmp_path, sector=sector, tuning=tuning, path=PATHS[path], kernel=KERNELS[kernel], bandwidth=bandwidth,
+                                blockdev=blockdev)
     try:
         for i, t in enumerate(types):
             assert pool.device_type(i)[0] == {"mem": kv.TYPE_MEM, "ssd": kv.TYPE_SSD, "hbm": kv.TYPE_HBM}[t]
@@ -158,6 +181,7 @@ def _run(wl, types, tmp_path, *, path="auto", kernel="vec16", sector=512, tuning
         return {"ssd_bytes": n_ssd_bytes, "info": infos}
     finally:
         pool.destroy()
+        _detach_loops()
 
 
 @pytest.mark.parametrize("kernel", list(KERNELS))
@@ -570,3 +594,25 @@ def test_per_layer_events_with_an_ssd_in_the_pool(tmp_path):
         pl.release()
     finally:
         pool.destroy()
+
+
+@pytest.mark.parametrize("sector", [0, 4096])
+def test_ssd_type_device_on_a_block_device_node(tmp_path, sector):
+    """The S_ISBLK branch (no NVMe on the box: a loop device, itself doing direct I/O to its backing file, is the block device
+    node): capacity checked against BLKGETSIZE64, the sector size taken from BLKSSZGET when the caller gives none, no file
+    system between the library and the device's sectors — which are read back here through the device node, never through
+    the library, and compared with orc_ssd_direct_store."""
+    wl = W.make_workload(1, n_layers=3)
+    out = _run(wl, ["mem", "ssd"], tmp_path, sector=sector, blockdev=True, batched=True, tuning={"ssd_lanes": 3, "ssd_chunk_bytes": 512 << 10})
+    info = out["info"][1]
+    assert info["block_device"] and info["sector_bytes"] == (sector or 512) and info["stores"] >= 3
+    # a capacity beyond the device is refused
+    f = _backing_file(tmp_path / "small.img", 1 << 20)
+    loop = _attach_loop(f)
+    try:
+        with pytest.raises(kv.KvPoolError) as e:
+            kv.KvPool([1.0], [2 << 20], dev_flags=[kv.DEV_SSD], paths=[loop], n_layers=1, n_kv_heads=8, head_dim=128)
+        assert e.value.code == kv.EINVAL
+    finally:
+        _detach_loops()
+    assert os.path.exists(f)                                                   # the library never removes what it did not create
