@@ -269,7 +269,8 @@ KVPOOL_API int kvpool_place(kvpool_t* pool, const uint32_t* blocks_per_layer /*h
 /* Frees the stripes and tables.  Waits first (host-blocking) for the library's own transfers and for the last work
  * each hot-path call enqueued with this placement on the caller's streams, so the stripes cannot be handed to another
  * request while a kernel still reads or writes them.  (Calls made while a stream was being captured into a CUDA graph
- * are not tracked: a graph that names the placement must not be launched after the release.)                       */
+ * are not tracked: a graph that names the placement must not be launched after the release.)  EIO, the placement still
+ * live, if a command of an SSD-type device has failed (see kvpool_synchronize): release again to let it go.            */
 KVPOOL_API int kvpool_release(kvpool_t* pool, kvpool_placement_t* pl);
 
 /* A request's block tables in ONE upload (a 1K-token request moves 4 MiB per layer: a separate table copy per layer costs
@@ -351,13 +352,16 @@ KVPOOL_API int kvpool_retrieve_range(kvpool_t* pool, kvpool_placement_t* pl, uin
 KVPOOL_API int kvpool_offload_range(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, uint32_t first_block, uint32_t n_blocks,
                          const void* k_base /*device*/, const void* v_base /*device*/, uint64_t block_stride_bytes,
                          const int32_t* block_table_dev /*device[K_l]*/, void* cuda_stream);
-/* Make `stream` wait until every offload enqueued so far with `pl` has landed in the pool.             */
+/* Make `stream` wait until every offload enqueued so far with `pl` has landed in the pool (on an SSD-type device: until
+ * its store commands have been written — a stream wait-value on the flag the device's worker raises).                */
 KVPOOL_API int kvpool_wait_offloads(kvpool_t* pool, kvpool_placement_t* pl, void* cuda_stream);
 /* Block the host until all work the pool enqueued on its own streams is done (not the caller's), and note which
  * offloads have landed.  After the caller has also synchronised its own streams, later zero-copy calls on those layers
  * enqueue exactly one kernel on `cuda_stream` and nothing else (no event waits or queries), so a zero-copy
  * kvpool_retrieve / kvpool_retrieve_layers / kvpool_retrieve_range can be captured into a CUDA graph and replayed
- * (profiling off; the placement and the tables must outlive the graph).                                           */
+ * (profiling off; the placement and the tables must outlive the graph).  Also waits for the workers of SSD-type devices;
+ * EIO (once) if a store / retrieve command has failed since the last call — the bytes of that command are lost, every
+ * hand-over has completed all the same.                                                                             */
 KVPOOL_API int kvpool_synchronize(kvpool_t* pool);
 
 /* In-device halves alone (a5 / a8): gather the layer's blocks into `stage_dev` (device, K_l*P bytes) in
