@@ -329,7 +329,8 @@ KVPOOL_API int kvpool_retrieve_layers(kvpool_t* pool, kvpool_placement_t* pl, ui
  * whose kernel raises a flag as each layer's last byte lands, and a stream of the library's own turns the flags into the
  * caller's events (stream wait-value, then event record), so every layer is handed over by itself although no launch and
  * no copy is spent on it alone; such events are recorded on that stream, not on `stream`.  (On the other paths such a
- * request is cut into two groups, so that the consumer of the first overlaps the second.)  A layer with K_l = 0 is ready
+ * request is cut into two groups, so that the consumer of the first overlaps the second, and the last eighth of any small
+ * request travels as a short group of its own, so that few consumers are left behind the last byte.)  A layer with K_l = 0 is ready
  * at once.  One host call per request instead of one per layer.                                                       */
 KVPOOL_API int kvpool_retrieve_layers_signal(kvpool_t* pool, kvpool_placement_t* pl, uint32_t first_layer, uint32_t n_layers,
                                   void* const* k_bases /*host[n_layers]*/, void* const* v_bases /*host[n_layers]*/,

@@ -641,6 +641,7 @@ static int layers_batched_locked(kvpool_t* p, kvpool_placement_t* pl, bool pack,
   std::vector<LayerState*> landed_later;
   uint64_t cap = std::max<uint64_t>(p->tune.group_bytes, 1);
   bool signal = false, signalled = false;
+  uint64_t tail_start = ~0ull;  // bytes of the call in front of its last, short group (below)
   if (ready) {
     // A consumer follows behind the per-layer events.  On the zero-copy path a request so small that it would travel as
     // one or two groups (all of a group's layers ready together: the consumer hardly overlapped) moves as ONE launch that
@@ -655,6 +656,11 @@ static int layers_batched_locked(kvpool_t* p, kvpool_placement_t* pl, bool pack,
     } else if (total < cap) {
       cap = std::max<uint64_t>((total + 1) / 2, 1);  // else cut it in two, so that the first half's consumer runs under the second half's transfer
     }
+    // ... and whatever the size: the layers of the call's LAST group become ready together when the last byte has arrived,
+    // and their consumers then run with nothing left to hide under (a dozen small launches: 40-60 us behind a 0.5-2.5 ms
+    // request).  So the last eighth of a small request (at most a quarter of a group) travels as a short group of its own:
+    // one more set of copies (~10 us of ramps) for a tail of two or three consumers instead of twelve or sixteen.
+    if (!signal) tail_start = total - std::min(total / 8, cap / 4);
   }
   const BatchCall c{p, pl, pack, first, k_bases, v_bases, tables, stride, static_cast<cudaStream_t>(cuda_stream), ready, &chain_run, &landed_later,
                     signal, &signalled};
@@ -663,7 +669,8 @@ static int layers_batched_locked(kvpool_t* p, kvpool_placement_t* pl, bool pack,
     ~Flush() { flush_landed(c); }
   } flush_on_exit{c};
   LayerGroup g;
-  uint64_t units = 0;
+  uint64_t units = 0, before = 0;  // before: bytes of the call's layers in front of layer q
+  bool tail_open = false;
   for (uint32_t q = 0; q < n; ++q) {
     LayerState& L = pl->layers[first + q];
     if (L.map->K == 0) {  // nothing to move: ready in stream order right away
@@ -672,6 +679,16 @@ static int layers_batched_locked(kvpool_t* p, kvpool_placement_t* pl, bool pack,
       continue;
     }
     const uint64_t bytes = L.map->K * p->payload;
+    if (!tail_open && before >= tail_start) {  // the short last group starts here
+      tail_open = true;
+      if (g.n) {
+        const int rc = issue_group(c, g);
+        if (rc != KVPOOL_OK) return rc;
+        g = LayerGroup{};
+        units = 0;
+      }
+    }
+    before += bytes;
     if (g.n && (g.n == kMaxBatch || units + L.map->K > 0x7fffffffull || g.bytes + bytes > std::max(cap, bytes))) {
       const int rc = issue_group(c, g);
       if (rc != KVPOOL_OK) return rc;
