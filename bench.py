@@ -831,8 +831,8 @@ def run_kvpool(args) -> dict:
         except Exception as e:                         # (a box without a writable --ssd-dir: say so instead of losing the headline)
             pools["host+ssd"] = {"unavailable": f"{type(e).__name__}: {e}"}
         # ... and over host memory and GPU memory (HBM-type pool device; this GPU's own memory stands in for
-        # an NVLink peer's: one GPU per box), 8 layers of this configuration, bit-verified
-        lines = mixed_pool_lines(4, (("host+hbm", [0, kv.DEV_HBM]),), L=8)
+        # an NVLink peer's: one GPU per box), 16 layers of this configuration, bit-verified
+        lines = mixed_pool_lines(4, (("host+hbm", [0, kv.DEV_HBM]),), L=16)
         head = next(lines)
         for r in lines:
             pools["host+hbm"] = dict(r, layers=head["layers"], moved_bytes_per_leg=head["moved_bytes_per_leg"],
