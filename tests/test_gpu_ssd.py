@@ -47,7 +47,10 @@ _LOOPS = []                                       # loop devices attached by _ss
 def _attach_loop(path):
     """A loop device over `path` (direct I/O to the backing file): a real block device node for the S_ISBLK branch."""
     import subprocess
-    r = subprocess.run(["losetup", "-f", "--show", "--direct-io=on", str(path)], capture_output=True, text=True)
+    try:
+        r = subprocess.run(["losetup", "-f", "--show", "--direct-io=on", str(path)], capture_output=True, text=True, timeout=30)
+    except (OSError, subprocess.TimeoutExpired) as e:
+        pytest.skip(f"no losetup here: {e}")
     if r.returncode != 0:
         pytest.skip(f"no loop device to be had here: {r.stderr.strip()}")
     _LOOPS.append(r.stdout.strip())
