@@ -232,7 +232,8 @@ def test_plan_lba_range_matches_oracle_and_rejects_bad_arguments(golden_dir):
 
 @pytest.mark.parametrize("sector,kv_size,slots,lane_bytes", [(512, 1536, 333, 32 << 10), (4096, 1536, 333, 32 << 10), (512, 96, 777, 4096 + 2 * 512),
                                                             (4096, 65536, 21, 1 << 20), (4096, 5120, 57, 16 << 10)])
-def test_ssd_worker_stores_and_retrieves_lba_ranges_like_the_oracle(tmp_path, sector, kv_size, slots, lane_bytes):
+@pytest.mark.parametrize("engine", ["io_uring", "sync"])
+def test_ssd_worker_stores_and_retrieves_lba_ranges_like_the_oracle(tmp_path, sector, kv_size, slots, lane_bytes, engine):
     """The host side of KV-passthrough (csrc/ssd_io.cpp: the device's worker thread, read-modify-write of edge sectors, zero
     padding, lane hand-over) without a GPU: tests/ssd_io_check.cpp plays the GPU's half of every command; the backing file
     must equal orc_ssd_direct_store's sector array — after the set has arrived in out-of-order instalments that start and
@@ -254,7 +255,8 @@ def test_ssd_worker_stores_and_retrieves_lba_ranges_like_the_oracle(tmp_path, se
     spans = [f"{a}:{b}" for a, b in zip(cuts, cuts[1:])]
     spans = [spans[i] for i in rng.permutation(len(spans))]                        # instalments arrive out of order
     out = subprocess.run([exe, disk_path, str(sector), str(kv_size), str(first), str(lane_bytes), "3", str(tmp_path / "stripe.bin"),
-                          str(tmp_path / "out.bin")] + spans, capture_output=True, text=True, timeout=120)
+                          str(tmp_path / "out.bin")] + spans, capture_output=True, text=True, timeout=120,
+                         env=dict(os.environ, KVPOOL_SSD_SYNC="1" if engine == "sync" else "0"))   # both engines of the worker
     assert out.returncode == 0 and out.stdout.startswith("ssd io ok"), out.stdout + out.stderr
     want = np.full((first + n_sec + 4) * sector, fill, dtype=np.uint8)
     assert oracle.ssd_direct_store(want, sector, first, stripe, kv_size) == n_sec
