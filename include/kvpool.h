@@ -373,6 +373,30 @@ KVPOOL_API int kvpool_pack(kvpool_t* pool, kvpool_placement_t* pl, uint32_t laye
 KVPOOL_API int kvpool_unpack(kvpool_t* pool, kvpool_placement_t* pl, uint32_t layer, void* k_base, void* v_base,
                   uint64_t block_stride_bytes, const int32_t* block_table_dev, const void* stage_dev, void* cuda_stream);
 
+/* kvpool_pack for callers that must not allocate GPU memory — code running inside a serving engine that has given nearly
+ * all of HBM to its own KV allocator (a cudaMalloc made later can fail) and whose decode loop cannot afford the
+ * device-wide wait cudaMalloc / cudaFree imply.  No pool, no placement: the call itself works out where Algorithm 1 puts
+ * the K blocks of one layer over n pool devices of integer weights w (as from kvpool_plan_weights; Eq. 1-2, Alg. 1
+ * l.4-16 — the same counts and the same weighted round-robin as kvpool_plan_layer / kvpool_place) and gathers them into
+ * stage_dev (device, K*P bytes, 16-byte aligned) in stripe order, byte for byte what kvpool_pack writes.  The dev / slot
+ * maps the gather reads, which kvpool_place keeps in cudaMalloc'd memory, live here in one fixed array inside the
+ * library's own device image: 160 KiB of HBM on every GPU that loads the library, held until the process exits.  The call
+ * makes no cudaMalloc, cudaFree or other allocating CUDA call; it enqueues two kernels on `cuda_stream` (one fills the
+ * maps on the GPU, one gathers) and returns.
+ *   - K > KVPOOL_STATIC_MAX_BLOCKS (a 512K-token layer at 16-token blocks): EINVAL, nothing enqueued.  K = 0 is a no-op.
+ *   - cuda_device: the CUDA ordinal the pointers and the stream belong to (0..63).  The FIRST call on a GPU also looks up
+ *     the array's address on that GPU (and thereby has the runtime load the library's device code there): make that first
+ *     call at start-up, before any stream capture.
+ *   - All calls on one GPU share the array.  Calls on one stream are ordered and safe.  Calls whose kernels may overlap on
+ *     the GPU (different streams with no event between them, or several host threads doing so) RACE on it and give wrong
+ *     bytes: order them.  The array keeps the last call's maps; no call depends on what it finds there.
+ *   - geom->n_layers is ignored.  EINVAL for n = 0, n > KVPOOL_MAX_DEVICES, a zero weight, a block size or a pointer /
+ *     stride that is not a multiple of 16; ECUDA if a CUDA call fails.  The table is not validated (R12).      */
+#define KVPOOL_STATIC_MAX_BLOCKS 32768u
+KVPOOL_API int kvpool_pack_static(const uint64_t* w /*host[n]*/, uint32_t n, const kvpool_geometry* geom /*host*/, uint32_t K,
+                       const void* k_base /*device*/, const void* v_base /*device*/, uint64_t block_stride_bytes,
+                       const int32_t* block_table_dev /*device[K]*/, void* stage_dev /*device*/, int cuda_device, void* cuda_stream);
+
 /* ---- introspection (GLT, Table I) -----------------------------------------------------------------------*/
 KVPOOL_API int kvpool_n_devices(const kvpool_t* pool, uint32_t* n_out);
 KVPOOL_API int kvpool_weights(const kvpool_t* pool, uint64_t* w_out /*host[n_devs]*/);

@@ -29,7 +29,7 @@ _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA",
 EXPORTS = [
     "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_plan_lba_range", "kvpool_ssd_range", "kvpool_ssd_location", "kvpool_ssd_info", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
     "kvpool_measure_bandwidth", "kvpool_share_bandwidth", "kvpool_calibrate", "kvpool_bandwidths", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release", "kvpool_set_tables",
-    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_checksum", "kvpool_checksum_layers", "kvpool_spin",
+    "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_pack_static", "kvpool_checksum", "kvpool_checksum_layers", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
     "kvpool_glt_bind", "kvpool_glt_find", "kvpool_layer_map", "kvpool_stats", "kvpool_set_profiling", "kvpool_profile_read", "kvpool_profile_read_clock", "kvpool_validate_table", "kvpool_set_table_check", "kvpool_table_errors", "kvpool_last_error", "kvpool_version",
 ]
@@ -109,6 +109,7 @@ def lib():
             "kvpool_synchronize": [vp],
             "kvpool_pack": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp, vp],
             "kvpool_unpack": [vp, vp, c_uint32, vp, vp, c_uint64, vp, vp, vp],
+            "kvpool_pack_static": [vp, c_uint32, POINTER(Geometry), c_uint32, vp, vp, c_uint64, vp, vp, c_int, vp],
             "kvpool_checksum": [vp, vp, vp, c_uint64, vp, c_uint32, vp, vp],
             "kvpool_checksum_layers": [vp, c_uint32, vp, vp, c_uint64, vp, vp, vp, vp, vp],
             "kvpool_spin": [vp, c_uint64, vp],
@@ -190,6 +191,21 @@ def kvpool_plan_layer(w: Sequence[int], K: int, with_map: bool = True):
     _ck(lib().kvpool_plan_layer(w.ctypes.data, w.shape[0], int(K), counts.ctypes.data,
                                 dev.ctypes.data if with_map else None, slot.ctypes.data if with_map else None))
     return (counts, dev, slot) if with_map else counts
+
+
+STATIC_MAX_BLOCKS = 32768
+
+
+def kvpool_pack_static(w: Sequence[int], K: int, k_base, v_base, block_stride_bytes: int, block_table_dev, stage_dev, *,
+                       n_kv_heads: int, head_dim: int, block_tokens: int = 16, elem_bytes: int = 2, cuda_device: int = 0, stream=None) -> None:
+    """kvpool_pack without a pool and without any GPU allocation by the library (for code that runs inside an engine which
+    owns all of HBM and cannot stall on cudaMalloc): places the K blocks of one layer over the devices of integer weights
+    `w` and gathers them into `stage_dev` in stripe order.  The maps live in a fixed array inside the library, shared by
+    every call on the GPU: K <= STATIC_MAX_BLOCKS, and calls that could overlap on the GPU must be ordered by the caller."""
+    wa = np.ascontiguousarray(w, dtype=np.uint64)
+    geom = Geometry(1, block_tokens, n_kv_heads, head_dim, elem_bytes)
+    _ck(lib().kvpool_pack_static(wa.ctypes.data, wa.shape[0], byref(geom), int(K), _addr(k_base), _addr(v_base), int(block_stride_bytes),
+                                 _addr(block_table_dev), _addr(stage_dev), int(cuda_device), _stream(stream)))
 
 
 def kvpool_plan_lba_range(set_size: int, kv_size: int, sector_bytes: int) -> int:

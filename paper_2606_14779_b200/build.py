@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkvpool.so")
-SOURCES = ["kvpool_core.cu", "kvpool_xfer.cu", "kvpool_dev.cu", "kvpool_ssd.cu", "kernels.cu", "placement.cpp", "pool_mem.cpp", "ssd_io.cpp"]
+SOURCES = ["kvpool_core.cu", "kvpool_xfer.cu", "kvpool_dev.cu", "kvpool_ssd.cu", "kvpool_static.cu", "kernels.cu", "placement.cpp", "pool_mem.cpp", "ssd_io.cpp"]
 HEADERS = ["kvpool_internal.hpp", "kernels.cuh", "placement.hpp", "pool_mem.hpp", "ssd_io.hpp", os.path.join("..", "..", "include", "kvpool.h"),
            os.path.join("..", "..", "include", "kvpool_dev.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--shared",
