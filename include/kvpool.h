@@ -436,6 +436,16 @@ KVPOOL_API int kvpool_ssd_location(const kvpool_placement_t* pl, uint32_t layer,
 KVPOOL_API int kvpool_ssd_info(const kvpool_t* pool, uint32_t dev, uint32_t* sector_bytes, int32_t* direct_io, int32_t* block_device,
                     uint64_t* stores_completed, uint64_t* retrieves_completed, uint32_t* queue_depth);
 
+/* Store / retrieve commands of the pool's SSD-type devices that have failed since kvpool_create (a count that only grows;
+ * 0 for a pool without such devices).  Non-blocking and lock-free - it reads the workers' counters - so an engine that
+ * pipelines on per-layer events can poll it (before and after a request, say) instead of waiting for the EIO of the next
+ * kvpool_synchronize / kvpool_release.  What a failed command leaves behind: a failed RETRIEVE command still hands its
+ * bytes over, so that no stream waits for ever and the layer's events fire, but the KV caches it covered arrive as ZERO
+ * bytes - never as whatever the shared bounce lane held before, which could be another request's KV; a failed STORE
+ * command leaves its LBA range unwritten.  A count that moved while a request was in flight means: do not use that
+ * request's KV.                                                                                                      */
+KVPOOL_API int kvpool_io_errors(const kvpool_t* pool, uint64_t* failed_out /*host*/);
+
 /* Keyed GLT (Table I `key` = "hash of the KV cache identifier"): give the K_l KV caches of a layer
  * caller-chosen 64-bit identifiers (e.g. the prefix-hash of the tokens a block covers, mixed with the layer), after
  * which any of them is found by identifier alone, across placements — what cross-request prefix reuse needs.

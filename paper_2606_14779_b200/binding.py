@@ -27,7 +27,7 @@ KERNEL_VEC16, KERNEL_BULK = 0, 1
 _ERRNAMES = {EINVAL: "EINVAL", ENOMEM: "ENOMEM", ECUDA: "ECUDA", ENUMA: "ENUMA", ESTATE: "ESTATE", ENOENT: "ENOENT", EIO: "EIO"}
 
 EXPORTS = [
-    "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_plan_lba_range", "kvpool_ssd_range", "kvpool_ssd_location", "kvpool_ssd_info", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
+    "kvpool_plan_weights", "kvpool_plan_layer", "kvpool_plan_lba_range", "kvpool_ssd_range", "kvpool_ssd_location", "kvpool_ssd_info", "kvpool_io_errors", "kvpool_create", "kvpool_destroy", "kvpool_set_bandwidth",
     "kvpool_measure_bandwidth", "kvpool_share_bandwidth", "kvpool_calibrate", "kvpool_bandwidths", "kvpool_set_path", "kvpool_set_tuning", "kvpool_get_tuning", "kvpool_reserve_staging", "kvpool_place", "kvpool_release", "kvpool_set_tables",
     "kvpool_offload", "kvpool_retrieve", "kvpool_retrieve_range", "kvpool_offload_range", "kvpool_offload_layers", "kvpool_retrieve_layers", "kvpool_retrieve_layers_signal", "kvpool_offload_naive", "kvpool_retrieve_naive", "kvpool_wait_offloads", "kvpool_synchronize", "kvpool_pack", "kvpool_unpack", "kvpool_pack_static", "kvpool_checksum", "kvpool_checksum_layers", "kvpool_spin",
     "kvpool_n_devices", "kvpool_weights", "kvpool_device_info", "kvpool_device_type", "kvpool_counts", "kvpool_lookup", "kvpool_stripe", "kvpool_stripe_read",
@@ -116,6 +116,7 @@ def lib():
             "kvpool_n_devices": [vp, POINTER(c_uint32)],
             "kvpool_weights": [vp, vp],
             "kvpool_device_info": [vp, c_uint32, POINTER(vp), POINTER(c_uint64), POINTER(c_uint64), POINTER(c_int32)],
+            "kvpool_io_errors": [vp, POINTER(c_uint64)],
             "kvpool_counts": [vp, c_uint32, vp],
             "kvpool_lookup": [vp, c_uint32, c_uint32, POINTER(c_uint32), POINTER(c_uint32), POINTER(c_uint32), POINTER(vp)],
             "kvpool_stripe": [vp, c_uint32, c_uint32, POINTER(vp), POINTER(c_uint64)],
@@ -469,6 +470,12 @@ class KvPool:
         _ck(lib().kvpool_glt_find(self.handle, int(ident), byref(key), byref(d), byref(t), byref(loc), byref(ph), byref(layer), byref(block)))
         return {"key": key.value, "device_id": d.value, "type": t.value, "location": loc.value or 0, "placement": ph.value,
                 "layer": layer.value, "block": block.value}
+
+    def io_errors(self) -> int:
+        """Failed store / retrieve commands of the pool's SSD-type devices since create (non-blocking)."""
+        n = c_uint64()
+        _ck(lib().kvpool_io_errors(self.handle, byref(n)))
+        return n.value
 
     def weights(self) -> np.ndarray:
         w = np.zeros(self.n_devices, dtype=np.uint64)

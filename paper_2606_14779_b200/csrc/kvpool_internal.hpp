@@ -81,10 +81,13 @@ struct LayerState {
   std::vector<uint64_t> have;        // else, once a partial offload has happened: bit j = logical block j is in the pool
   cudaEvent_t landed = nullptr;      // recorded when the layer's stripes are complete in the pool
   bool landed_pending = false;
-  // SSD-type devices: the store command that completes this layer's stripe on device i = use ssd_last_use[i] of offload
-  // lane ssd_last_lane[i] (bit i of ssd_stored says there is one); its completion is the worker's cpu_seq flag, not an event
+  // SSD-type devices: ssd_lane_use[i][k] = the latest use of offload lane k of device i that carried a store command of this
+  // layer (0 = none; bit i of ssd_stored says there is one).  A stripe larger than a lane is several commands on several
+  // lanes, instalments (kvpool_offload_range) add more, and the worker reaps completions in any order: the layer's stripe is
+  // on the device once EVERY such lane's cpu_seq flag has reached its entry (uses of one lane complete in order).  The
+  // completion is the worker's flag, not an event
   uint32_t ssd_stored = 0;
-  std::vector<uint32_t> ssd_last_lane, ssd_last_use;
+  std::vector<std::vector<uint32_t>> ssd_lane_use;
 };
 
 struct ProfRec {  // one profiled kernel launch

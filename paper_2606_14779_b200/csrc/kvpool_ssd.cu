@@ -139,11 +139,19 @@ int ssd_ensure_lanes(kvpool* p) {
     }
     memset(S.flags, 0, 2ull * n * kFlagStride * 4);
     S.flags_dev = reinterpret_cast<uint64_t>(fd);
-    S.n_lanes = n;
+    S.n_lanes = n;  // (flag_word needs it) every failure below goes through free_lanes, which takes it back to 0:
+                    // n_lanes != 0 on return means lanes, streams and a running worker
+    for (int d = 0; d < 2 && e == cudaSuccess; ++d) {
+      e = cudaStreamCreateWithFlags(&S.kstream[d], cudaStreamNonBlocking);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&S.fork[d], cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&S.join[d], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) {  // nothing half-made is left behind: the next kvpool_place starts over
+      cudaGetLastError();
+      free_lanes(S);
+      return fail(KVPOOL_ECUDA, "place: streams / events of SSD-type device %u: %s", i, cudaGetErrorString(e));
+    }
     for (int d = 0; d < 2; ++d) {
-      CU(cudaStreamCreateWithFlags(&S.kstream[d], cudaStreamNonBlocking));
-      CU(cudaEventCreateWithFlags(&S.fork[d], cudaEventDisableTiming));
-      CU(cudaEventCreateWithFlags(&S.join[d], cudaEventDisableTiming));
       S.lane[d].resize(n);
       for (uint32_t k = 0; k < n; ++k) {
         SsdLane& ln = S.lane[d][k];
@@ -178,10 +186,18 @@ int ssd_command(kvpool* p, uint32_t i, bool pack, uint64_t byte0, uint64_t bytes
   *lane_out = k;
   *use_out = u;
   // If enqueueing fails half way, both flags of this use are raised from the host so that no later use of the lane (and no
-  // worker) waits for a hand-over that will never come.
+  // worker) waits for a hand-over that will never come.  Earlier uses of the lane may still be pending, and their own
+  // hand-overs (a stream write-value of u-1, the worker's store of u-1) land later: a plain store here could be overwritten
+  // by them and the flag would read u-1 for ever.  So the host first waits until both flags have reached u-1 — the earlier
+  // uses are enqueued and complete by themselves — and only then raises them to u; flags never go backwards.  (If the GPU
+  // itself is gone the wait gives up after two seconds and the pool's abort path takes over at kvpool_destroy.)
   auto abandon = [&](int rc) {
-    __atomic_store_n(S.flags + flag_word(S, d, k, false), u, __ATOMIC_RELEASE);
-    __atomic_store_n(S.flags + flag_word(S, d, k, true), u, __ATOMIC_RELEASE);
+    for (int cpu = 0; cpu < 2; ++cpu) {
+      volatile uint32_t* f = S.flags + flag_word(S, d, k, cpu != 0);
+      const timespec nap{0, 50000};
+      for (int spins = 0; spins < 40000 && !seq_reached(f, u - 1); ++spins) nanosleep(&nap, nullptr);
+      __atomic_store_n(f, u, __ATOMIC_RELEASE);
+    }
     return rc;
   };
   int rc;
@@ -245,8 +261,9 @@ int ssd_move(kvpool* p, LayerState& L, uint32_t i, uint32_t lo, uint32_t hi, boo
       return rc;
     }
     if (pack) {
-      L.ssd_last_lane[i] = lane;
-      L.ssd_last_use[i] = use;
+      auto& uses = L.ssd_lane_use[i];
+      if (uses.size() < S.n_lanes) uses.resize(S.n_lanes, 0);
+      uses[lane] = use;  // uses of a lane only grow
       L.ssd_stored |= 1u << i;
     }
     x += n;
@@ -273,8 +290,11 @@ int ssd_wait_stored(kvpool* p, const LayerState& L, cudaStream_t s) {
   for (uint32_t i = 0; i < p->n; ++i) {
     if (!(L.ssd_stored >> i & 1u)) continue;
     const SsdState& S = *p->ssd[i];
-    if (seq_reached(S.flags + flag_word(S, 1, L.ssd_last_lane[i], true), L.ssd_last_use[i])) continue;  // already on the disk
-    DRV(g_wait_value(s, flag_dev(S, 1, L.ssd_last_lane[i], true), L.ssd_last_use[i], kWaitGeq));
+    const auto& uses = L.ssd_lane_use[i];
+    for (uint32_t k = 0; k < uses.size(); ++k) {  // every lane that carried a piece of the stripe, not just the last one
+      if (uses[k] == 0 || seq_reached(S.flags + flag_word(S, 1, k, true), uses[k])) continue;  // none, or already on the disk
+      DRV(g_wait_value(s, flag_dev(S, 1, k, true), uses[k], kWaitGeq));
+    }
   }
   return KVPOOL_OK;
 }

@@ -94,6 +94,13 @@ bool Uring::queue(bool write, int file, void* buf, uint32_t len, uint64_t off, u
   return true;
 }
 
+unsigned Uring::drop_unsubmitted() {
+  const unsigned n = to_submit_;
+  __atomic_store_n(sq_tail_, *sq_tail_ - n, __ATOMIC_RELEASE);  // no SQPOLL: the kernel reads the tail only inside io_uring_enter
+  to_submit_ = 0;
+  return n;
+}
+
 int Uring::flush() {
   while (to_submit_) {
     const long r = syscall(__NR_io_uring_enter, fd_, to_submit_, 0, 0, nullptr, 0);
@@ -226,20 +233,20 @@ void SsdDevice::drain() {
 }
 
 // Poll for the GPU's half of a command (the paper polls NVMe completions on a dedicated core; here the
-// worker polls the flag a stream write-value raises): spin briefly, then poll every 20 us.  Gives up when the pool says
-// the GPU is gone (abort(), from kvpool_destroy after a failed device synchronize) and, as a backstop, after ten minutes.
+// worker polls the flag a stream write-value raises): spin briefly, then poll every 20 us.  Gives up only when the pool says
+// the GPU is gone (abort(), from kvpool_destroy after a failed device synchronize) — never by the clock: a stream that is
+// legitimately held up (long work in front of it, an external event) hands its lane over late, and a command that had
+// given up by then would leave the layer marked as stored with nothing written.
 bool SsdDevice::wait_flag(const volatile uint32_t* f, uint32_t v) {
   for (int i = 0; i < 4096; ++i) {
     if (seq_reached(f, v)) return true;
     __builtin_ia32_pause();
   }
-  const auto t0 = std::chrono::steady_clock::now();
   const timespec nap{0, 20000};
-  for (uint64_t n = 0;; ++n) {
+  for (;;) {
     if (seq_reached(f, v)) return true;
     if (abort_.load(std::memory_order_relaxed)) return false;
     nanosleep(&nap, nullptr);
-    if ((n & 1023) == 1023 && std::chrono::steady_clock::now() - t0 > std::chrono::minutes(10)) return false;
   }
 }
 
@@ -283,11 +290,18 @@ int SsdDevice::prepare_store(const SsdCmd& c) {
   return e;
 }
 
-void SsdDevice::complete(const SsdCmd& c, int e) {
+void SsdDevice::complete(const SsdCmd& c, int e, bool lane_is_ours) {
   const int d = c.op == SsdCmd::kWrite ? 1 : 0;
   if (e) {
     int none = 0;
     error_.compare_exchange_strong(none, e);
+    failed_.fetch_add(1);
+    // A failed retrieve still hands its lane over (no stream may wait for ever), and the unpack kernel then scatters
+    // whatever the lane holds into the caller's paged KV.  The lanes are shared by all requests and keep their last
+    // contents, so that must not be the lane as it stands: the caller gets zeroes, never another request's KV.  (Not when
+    // the GPU's half never arrived — the GPU is gone, and its previous kernel may formally still own the lane.)
+    if (d == 0 && lane_is_ours)
+      memset(bounce_[0] + static_cast<uint64_t>(c.lane) * lane_bytes_, 0, static_cast<size_t>(std::min<uint64_t>(c.head + c.len, lane_bytes_)));
   }
   // the hand-over completes even on failure: no stream waits for ever
   __atomic_store_n(cpu_seq_[d] + static_cast<uint64_t>(c.lane) * stride_, c.use, __ATOMIC_RELEASE);
@@ -303,10 +317,11 @@ void SsdDevice::execute(const SsdCmd& c) {
   if (total > lane_bytes_ || c.file_off % sector_ || c.file_off + total > capacity_) e = EINVAL;
   // SSD_Direct_Retrieve: the lane is free once the GPU has drained its previous use; read the LBA range into it.
   // SSD_Direct_Store: wait for the GPU's copy into the lane, complete the first / last sector, write the LBA range.
-  if (!wait_flag(gpu, c.op == SsdCmd::kWrite ? c.use : c.use - 1)) e = e ? e : (abort_.load() ? ECANCELED : ETIMEDOUT);
+  bool ours = true;
+  if (!wait_flag(gpu, c.op == SsdCmd::kWrite ? c.use : c.use - 1)) { ours = false; e = e ? e : ECANCELED; }
   if (!e && c.op == SsdCmd::kWrite) e = prepare_store(c);
   if (!e) e = rw_full(c.op == SsdCmd::kWrite, c.file_off, buf, total);
-  complete(c, e);
+  complete(c, e, ours);
 }
 
 void SsdDevice::run() {
@@ -337,7 +352,6 @@ struct SsdDevice::Active {
   uint64_t lo, hi;  // byte range of whole sectors the command touches
   uint64_t id;
   enum { kWaiting, kInFlight } state;
-  std::chrono::steady_clock::time_point since;
 };
 
 void SsdDevice::run_async() {
@@ -361,12 +375,12 @@ void SsdDevice::run_async() {
         a.hi = a.c.file_off + total;
         a.id = next_id++;
         a.state = Active::kWaiting;
-        a.since = std::chrono::steady_clock::now();
         win.push_back(a);
         progress = true;
       }
     }
     unsigned finished = 0;
+    std::vector<uint64_t> queued;  // ids handed to the ring in this round, in order
     for (size_t k = 0; k < win.size(); ++k) {
       Active& a = win[k];
       if (a.state != Active::kWaiting) continue;
@@ -376,28 +390,34 @@ void SsdDevice::run_async() {
       if (blocked) continue;
       int e = 0;
       const uint64_t total = a.hi - a.lo;
-      if (total > lane_bytes_ || a.lo % sector_ || a.hi > capacity_ || total > 0x7fffffffull) e = EINVAL;
-      if (!e && !gpu_half_arrived(a.c)) {
-        if (abort_.load(std::memory_order_relaxed)) e = ECANCELED;
-        else if (std::chrono::steady_clock::now() - a.since > std::chrono::minutes(10)) e = ETIMEDOUT;
+      if (!gpu_half_arrived(a.c)) {  // (checked first, so that a command that fails for another reason fails owning its lane)
+        if (abort_.load(std::memory_order_relaxed)) e = ECANCELED;  // the GPU is gone; never by the clock (wait_flag)
         else continue;
       }
+      const bool ours = e == 0;
+      if (!e && (total > lane_bytes_ || a.lo % sector_ || a.hi > capacity_ || total > 0x7fffffffull)) e = EINVAL;
       const int d = a.c.op == SsdCmd::kWrite ? 1 : 0;
       uint8_t* const buf = bounce_[d] + static_cast<uint64_t>(a.c.lane) * lane_bytes_;
       if (!e && d == 1) e = prepare_store(a.c);
       if (!e && !ring_.queue(d == 1, fd_, buf, static_cast<uint32_t>(total), a.lo, a.id)) continue;  // ring full: next round
       progress = true;
       if (e) {
-        complete(a.c, e);
+        complete(a.c, e, ours);
         a.id = 0;  // done
         ++finished;
       } else {
         a.state = Active::kInFlight;
+        queued.push_back(a.id);
       }
     }
-    if (int e = ring_.flush()) {  // the kernel refused the submission: fail what was queued
-      for (auto& a : win)
-        if (a.state == Active::kInFlight) { complete(a.c, e); a.id = 0; ++finished; }
+    if (int e = ring_.flush()) {
+      // The kernel refused the submission: fail the entries of THIS round it did not accept (the last `left` queued) and take
+      // them off the ring.  Commands it accepted, now or in earlier rounds, are on the disk's side: their lanes stay theirs
+      // until their completions are reaped.
+      const unsigned left = ring_.drop_unsubmitted();
+      for (size_t q = queued.size() - std::min<size_t>(left, queued.size()); q < queued.size(); ++q)
+        for (auto& a : win)
+          if (a.id == queued[q] && a.state == Active::kInFlight) { complete(a.c, e, true); a.id = 0; ++finished; break; }
     }
     uint64_t id;
     int32_t res;
@@ -412,7 +432,7 @@ void SsdDevice::run_async() {
           uint8_t* const buf = bounce_[d] + static_cast<uint64_t>(a.c.lane) * lane_bytes_;
           e = res == 0 ? EIO : rw_full(d == 1, a.lo + static_cast<uint64_t>(res), buf + res, total - static_cast<uint64_t>(res));
         }
-        complete(a.c, e);
+        complete(a.c, e, true);
         a.id = 0;
         ++finished;
         break;

@@ -47,6 +47,7 @@ class Uring {
   // queue one read / write of `len` bytes (false: the submission ring is full); flush() hands queued entries to the kernel
   bool queue(bool write, int file, void* buf, uint32_t len, uint64_t off, uint64_t user_data);
   int flush();
+  unsigned drop_unsubmitted();  // after a failed flush(): take the entries the kernel did not accept off the ring; how many
   bool reap(uint64_t* user_data, int32_t* res);  // one completion, if any
   int wait_one();                                // sleep in the kernel until a completion is there
  private:
@@ -79,6 +80,8 @@ class SsdDevice {
   // first I/O error since the last call (an errno value; 0 = none).  A failed command still completes its handshake,
   // so that no stream waits for ever.
   int take_error() { return error_.exchange(0); }
+  // commands that have failed since start (never reset; readable at any time from any thread)
+  uint64_t failed() const { return failed_.load(); }
   // Synchronous helpers for inspection / measurement (call after drain()): whole sectors are moved through `scratch`
   // (4 KiB-aligned, scratch_bytes a multiple of the sector size).
   int read_bytes(uint64_t off, void* dst, uint64_t n, uint8_t* scratch, uint64_t scratch_bytes);
@@ -97,7 +100,7 @@ class SsdDevice {
   struct Active;  // a command the asynchronous worker has taken off the queue
   bool gpu_half_arrived(const SsdCmd& c) const;
   int prepare_store(const SsdCmd& c);  // first / last sector of a store: keep the neighbours' bytes, or zero the padding
-  void complete(const SsdCmd& c, int err);
+  void complete(const SsdCmd& c, int err, bool lane_is_ours);  // lane_is_ours: the GPU's half of the command had arrived
   bool wait_flag(const volatile uint32_t* f, uint32_t v);
   int rw_full(bool write, uint64_t off, uint8_t* buf, uint64_t n);
   void execute(const SsdCmd& c);
@@ -120,6 +123,7 @@ class SsdDevice {
   uint64_t submitted_ = 0, finished_ = 0;
   bool stopping_ = false;
   std::atomic<int> error_{0};
+  std::atomic<uint64_t> failed_{0};
   std::atomic<bool> abort_{false};
   Uring ring_;
   unsigned depth_ = 1;

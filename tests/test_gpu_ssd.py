@@ -388,14 +388,66 @@ def test_ssd_errors_bad_arguments_full_device_and_a_failing_disk(tmp_path):
         pool.wait_offloads(pl)
         torch.cuda.synchronize()
         pool.synchronize()
+        assert pool.io_errors() == 0
+        # leave recognisable bytes in the retrieve lanes: a retrieve that works, of KV that is all 0x77
+        marker = torch.full((2, wl.nphys, wl.geom.kvb), 0x77, dtype=torch.uint8, device=dev)
+        pool.offload(pl, 0, marker[0], marker[1], wl.geom.kvb, table)
+        pool.wait_offloads(pl)
+        pool.retrieve(pl, 0, marker[0], marker[1], wl.geom.kvb, table)
+        pool.offload(pl, 0, src[0], src[1], wl.geom.kvb, table)
+        pool.wait_offloads(pl)
+        torch.cuda.synchronize()
+        pool.synchronize()
+        assert pool.io_errors() == 0
         os.truncate(files[0], 0)                                               # the device loses its sectors
         dst = W.poison_torch((2, wl.nphys, wl.geom.kvb // 2), dev)
         pool.retrieve(pl, 0, dst[0], dst[1], wl.geom.kvb, table)
         torch.cuda.synchronize()                                               # returns: the failed reads still release their lanes
+        assert pool.io_errors() > 0                                            # visible without blocking, before any synchronize
+        # what the failed commands handed over is zero bytes: neither the lanes' last contents (0x77) nor anything else
+        got = dst.view(torch.uint8).reshape(2, wl.nphys, wl.geom.kvb)[:, table.long()]
+        assert int(got.count_nonzero()) == 0
         with pytest.raises(kv.KvPoolError) as e:
             pool.synchronize()
         assert e.value.code == kv.EIO
         pool.synchronize()                                                     # reported once
+        pl.release()
+    finally:
+        pool.destroy()
+
+
+def test_wait_offloads_covers_every_command_of_a_stripe_and_every_instalment(tmp_path):
+    """A stripe much larger than a lane is many store commands spread over the lanes, an instalment offload adds more, and
+    the worker completes them in whatever order the disk does: after kvpool_wait_offloads + a sync of THAT stream (no
+    kvpool_synchronize, no stripe read through the library, both of which would wait for the worker) every sector of the
+    stripe must already be in the file."""
+    base = W.make_workload(1, n_layers=8)                                       # 64 KV caches of 64 KiB per layer
+    wl = _custom(base.geom, base.nphys, [base.requests[0].table], 1, (1.0,))
+    g = wl.geom
+    dev = torch.device("cuda:0")
+    pool, bw, files = _ssd_pool(wl, ["ssd"], tmp_path, bandwidth=[1.0], tuning={"ssd_chunk_bytes": 3 * g.payload, "ssd_lanes": 4})
+    try:
+        bpl = wl.blocks_per_layer(0)
+        pl = pool.place(bpl)
+        opl = oracle.place(bw, bpl)
+        stream = torch.cuda.Stream()
+        srcs = [W.kv_layer_torch(wl, l, dev) for l in range(g.n_layers)]
+        tables_np = [np.ascontiguousarray(wl.layer_table(0, l)) for l in range(g.n_layers)]
+        tables = [torch.from_numpy(t).to(dev) for t in tables_np]
+        torch.cuda.synchronize()
+        for l in range(g.n_layers):
+            K = int(bpl[l])
+            cuts = [0, K] if l % 2 == 0 else [0, K // 3, K // 3 + 5, K]           # odd layers arrive in three instalments
+            for a, b in zip(cuts, cuts[1:]):
+                pool.offload_range(pl, l, a, b - a, srcs[l][0], srcs[l][1], g.kvb, tables[l], stream)
+            pool.wait_offloads(pl, stream)
+            stream.synchronize()
+            first, n_sec, sec = pl.ssd_range(l, 0)
+            want = oracle.offload_layer(W.kv_layer_numpy(wl, l), tables_np[l], opl[l])[0]
+            have = _read_file(files[0], first * sec, want.nbytes)
+            assert np.array_equal(have, want), f"layer {l}: wait_offloads returned before every store command was on the disk"
+        assert pool.ssd_info(0)["stores"] >= g.n_layers * 20                      # really many commands per stripe
+        pool.synchronize()
         pl.release()
     finally:
         pool.destroy()
