@@ -22,7 +22,7 @@ namespace kvp {
 namespace {
 
 constexpr int kVecMaxThreads = 512;
-constexpr uint32_t kBulkBarrierBytes = 1024;          // room for warps*stages mbarriers in front of the ring
+constexpr uint32_t kBulkBarrierBytes = 1024;          // in front of the ring: 512 B of mbarriers (warps*stages <= 64), 512 B of destination pointers
 
 __device__ __forceinline__ int4 ld_stream(const void* p) {
   int4 r;
@@ -89,40 +89,46 @@ __device__ __forceinline__ void reject(Piece& p, unsigned long long* bad, bool f
   if (first_piece && (threadIdx.x & 31u) == 0 && bad) atomicAdd(bad, 1ull);
 }
 
-template <bool CHECK = true>
-__device__ __forceinline__ Piece decode(const LayerArgs& a, uint64_t t, uint32_t pieces, uint32_t piece_bytes) {
-  const uint32_t per_unit = 2u * pieces;
-  const uint32_t local = static_cast<uint32_t>(t / per_unit);
-  const uint32_t r = static_cast<uint32_t>(t - static_cast<uint64_t>(local) * per_unit);
-  const uint32_t half = r >= pieces ? 1u : 0u;  // 0: K block, 1: V block
-  const uint32_t c = r - half * pieces;
-  const uint32_t off = c * piece_bytes;
-  uint32_t j, d, s;
+// A piece is decoded in two steps, so that a caller that knows its next piece early (the single issuing lane of the bulk
+// kernel) can have the table reads in flight while it waits for something else: decode_load issues the global loads for
+// piece r of unit `local` and does no arithmetic on their results; decode_finish turns them into addresses.
+struct RawPiece {
+  int32_t phys;
+  uint32_t d, s, r;
+  uint32_t layer;  // MultiArgs only
+};
+__device__ __forceinline__ RawPiece decode_load(const LayerArgs& a, uint32_t local, uint32_t r) {
+  RawPiece m;
+  uint32_t j;
   if (a.order) {  // device-major chunk: unit `local` of one device's slot range (uniform across the launch)
     j = __ldg(a.order + a.j0 + local);
-    d = 0;
-    s = local;
+    m.d = 0;
+    m.s = local;
   } else {
     j = a.visit ? __ldg(a.visit + a.j0 + local) : a.j0 + local;
-    d = __ldg(a.dev + j);
-    s = __ldg(a.slot + j);
+    m.d = __ldg(a.dev + j);
+    m.s = __ldg(a.slot + j);
   }
-  const int32_t phys = __ldg(a.table + j);
+  m.phys = __ldg(a.table + j);
+  m.r = r;
+  m.layer = 0;
+  return m;
+}
+template <bool CHECK = true>
+__device__ __forceinline__ Piece decode_finish(const LayerArgs& a, const RawPiece& m, uint32_t pieces, uint32_t piece_bytes) {
+  const uint32_t half = m.r >= pieces ? 1u : 0u;  // 0: K block, 1: V block
+  const uint32_t off = (m.r - half * pieces) * piece_bytes;
   Piece p;
-  p.paged = (half ? a.v_base : a.k_base) + static_cast<uint64_t>(phys) * a.stride + off;
-  p.pooled = reinterpret_cast<uint8_t*>(a.pool_base[d]) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;
+  p.paged = (half ? a.v_base : a.k_base) + static_cast<uint64_t>(m.phys) * a.stride + off;
+  p.pooled = reinterpret_cast<uint8_t*>(a.pool_base[m.d]) + (static_cast<uint64_t>(m.s) * 2u + half) * a.kvb + off;
   p.bytes = min(piece_bytes, a.kvb - off);
   p.layer = 0;
   if constexpr (CHECK)
-    if (a.nphys_check && static_cast<uint32_t>(phys) >= a.nphys_check) reject(p, a.bad, r == 0);
+    if (a.nphys_check && static_cast<uint32_t>(m.phys) >= a.nphys_check) reject(p, a.bad, m.r == 0);
   return p;
 }
 
-template <bool CHECK = true>
-__device__ __forceinline__ Piece decode(const MultiArgs& a, uint64_t t, uint32_t pieces, uint32_t piece_bytes) {
-  const uint32_t per_unit = 2u * pieces;
-  const uint32_t unit = static_cast<uint32_t>(t / per_unit);
-  const uint32_t r = static_cast<uint32_t>(t - static_cast<uint64_t>(unit) * per_unit);
+__device__ __forceinline__ RawPiece decode_load(const MultiArgs& a, uint32_t unit, uint32_t r) {
   uint32_t lo = 0, hi = a.n;  // last layer with first_unit <= unit
   while (hi - lo > 1) {
     const uint32_t mid = (lo + hi) >> 1;
@@ -131,20 +137,36 @@ __device__ __forceinline__ Piece decode(const MultiArgs& a, uint64_t t, uint32_t
   }
   const MultiDesc& L = a.d[lo];
   const uint32_t j = unit - L.first_unit;
-  const uint32_t half = r >= pieces ? 1u : 0u;
-  const uint32_t c = r - half * pieces;
-  const int32_t phys = __ldg(L.table + j);
-  const uint32_t d = __ldg(L.dev + j);
-  const uint32_t s = __ldg(L.slot + j);
-  const uint32_t off = c * piece_bytes;
+  RawPiece m;
+  m.phys = __ldg(L.table + j);
+  m.d = __ldg(L.dev + j);
+  m.s = __ldg(L.slot + j);
+  m.r = r;
+  m.layer = lo;
+  return m;
+}
+template <bool CHECK = true>
+__device__ __forceinline__ Piece decode_finish(const MultiArgs& a, const RawPiece& m, uint32_t pieces, uint32_t piece_bytes) {
+  const MultiDesc& L = a.d[m.layer];
+  const uint32_t half = m.r >= pieces ? 1u : 0u;
+  const uint32_t off = (m.r - half * pieces) * piece_bytes;
   Piece p;
-  p.paged = (half ? L.v_base : L.k_base) + static_cast<uint64_t>(phys) * a.stride + off;
-  p.pooled = reinterpret_cast<uint8_t*>(__ldg(L.pool_base + d) + a.delta[d]) + (static_cast<uint64_t>(s) * 2u + half) * a.kvb + off;
+  p.paged = (half ? L.v_base : L.k_base) + static_cast<uint64_t>(m.phys) * a.stride + off;
+  p.pooled = reinterpret_cast<uint8_t*>(__ldg(L.pool_base + m.d) + a.delta[m.d]) + (static_cast<uint64_t>(m.s) * 2u + half) * a.kvb + off;
   p.bytes = min(piece_bytes, a.kvb - off);
-  p.layer = lo;
+  p.layer = m.layer;
   if constexpr (CHECK)
-    if (a.nphys_check && static_cast<uint32_t>(phys) >= a.nphys_check) reject(p, a.bad, r == 0);
+    if (a.nphys_check && static_cast<uint32_t>(m.phys) >= a.nphys_check) reject(p, a.bad, m.r == 0);
   return p;
+}
+
+// Work item t of a launch whose K (or V) blocks are split into `pieces` pieces of `piece_bytes` bytes.
+template <bool CHECK = true, class Args>
+__device__ __forceinline__ Piece decode(const Args& a, uint64_t t, uint32_t pieces, uint32_t piece_bytes) {
+  const uint32_t per_unit = 2u * pieces;
+  const uint32_t unit = static_cast<uint32_t>(t / per_unit);
+  const uint32_t r = static_cast<uint32_t>(t - static_cast<uint64_t>(unit) * per_unit);
+  return decode_finish<CHECK>(a, decode_load(a, unit, r), pieces, piece_bytes);
 }
 __device__ __forceinline__ uint32_t units(const LayerArgs& a) { return a.K; }
 __device__ __forceinline__ uint32_t units(const MultiArgs& a) { return a.total_units; }
@@ -254,29 +276,54 @@ __global__ void __launch_bounds__(256) kv_copy_bulk(const __grid_constant__ Args
   span_begin(a.span);
 
   const uint32_t pieces = a.kvb / chunk;  // host guarantees chunk | kvb
-  const uint64_t total = static_cast<uint64_t>(units(a)) * 2u * pieces;
+  const uint32_t per_unit = 2u * pieces;
+  const uint64_t total = static_cast<uint64_t>(units(a)) * per_unit;
   const uint64_t gw = static_cast<uint64_t>(blockIdx.x) * nw + warp, ngw = static_cast<uint64_t>(gridDim.x) * nw;
   const uint64_t mine = gw < total ? (total - gw + ngw - 1) / ngw : 0;
 
-  uint64_t issued = 0;
-  uint8_t* out_ring[8];  // destination of the chunk sitting in each stage (stages <= 8)
-  auto issue = [&](uint64_t n) {
-    const uint32_t s = static_cast<uint32_t>(n % stages);
-    const Piece p = decode<CHECK>(a, gw + n * ngw, pieces, chunk);
-    out_ring[s] = PACK ? p.pooled : p.paged;
-    mbar_arrive_expect_tx(bar0 + 8u * s, chunk);
-    bulk_g2s(buf0 + s * chunk, PACK ? p.paged : p.pooled, chunk, bar0 + 8u * s);
+  // The lane is the only issue slot of its ring, so nothing slow may sit between two of its cp.async.bulk: its pieces
+  // gw, gw + ngw, ... are walked as (unit, piece in unit) with a carry (no division in the loop), stage indices and the
+  // barrier parity are counters, the stages' destinations sit in shared memory, and the table reads of the NEXT piece are
+  // issued before the lane goes to wait for the oldest load, so that they have landed when it comes back to issue.
+  uint32_t unit = static_cast<uint32_t>(gw / per_unit), r = static_cast<uint32_t>(gw % per_unit);
+  const uint32_t du = static_cast<uint32_t>(ngw / per_unit), dr = static_cast<uint32_t>(ngw % per_unit);
+  auto advance = [&] {
+    unit += du;
+    r += dr;
+    if (r >= per_unit) { r -= per_unit; ++unit; }
   };
-  for (; issued < mine && issued + 1 < stages; ++issued) issue(issued);
+  uint8_t** const out_ring = reinterpret_cast<uint8_t**>(smem + kBulkBarrierBytes / 2) + warp * stages;  // destination of the chunk in each stage
+  uint32_t s_issue = 0;
+  auto issue = [&](const RawPiece& m) {
+    const Piece p = decode_finish<CHECK>(a, m, pieces, chunk);
+    out_ring[s_issue] = PACK ? p.pooled : p.paged;
+    mbar_arrive_expect_tx(bar0 + 8u * s_issue, chunk);
+    bulk_g2s(buf0 + s_issue * chunk, PACK ? p.paged : p.pooled, chunk, bar0 + 8u * s_issue);
+    if (++s_issue == stages) s_issue = 0;
+  };
+  uint64_t issued = 0;
+  RawPiece next{};
+  if (mine) next = decode_load(a, unit, r);
+  while (issued < mine && issued + 1 < stages) {
+    const RawPiece cur = next;
+    ++issued;
+    advance();
+    if (issued < mine) next = decode_load(a, unit, r);
+    issue(cur);
+  }
+  uint32_t s_cons = 0, parity = 0;
   for (uint64_t i = 0; i < mine; ++i) {
-    const uint32_t s = static_cast<uint32_t>(i % stages);
-    mbar_wait(bar0 + 8u * s, static_cast<uint32_t>(i / stages) & 1u);
-    bulk_s2g(out_ring[s], buf0 + s * chunk, chunk);
+    mbar_wait(bar0 + 8u * s_cons, parity);
+    bulk_s2g(out_ring[s_cons], buf0 + s_cons * chunk, chunk);
     bulk_commit();
+    if (++s_cons == stages) { s_cons = 0; parity ^= 1u; }
     if (issued < mine) {
       bulk_wait_read_1();  // the store issued one iteration ago has drained its stage: refill that stage
-      issue(issued);
+      const RawPiece cur = next;
       ++issued;
+      advance();
+      if (issued < mine) next = decode_load(a, unit, r);
+      issue(cur);
     }
   }
   bulk_wait_all();

@@ -32,9 +32,9 @@ void default_tuning(kvpool* p) {
   p->tune.link_kernel = KVPOOL_KERNEL_BULK;  // 2 CTAs already saturate the link (profiles/r1_sweep_link.txt)
   p->tune.hbm_ctas = 16u * p->sm_count;  // many short CTAs balance the tail better than a persistent grid here (profiles/r1_sweep_hbm.txt)
   p->tune.link_ctas = 4;
-  p->tune.bulk_chunk = 16384;
-  p->tune.bulk_stages = 6;
-  p->tune.bulk_warps = 2;
+  p->tune.bulk_chunk = 16384;  // 3 issuing lanes per SM x 4 stages x 16 KiB = 192 KiB of shared memory, 144 KiB of loads in flight per SM:
+  p->tune.bulk_stages = 4;     // 6.2 / 6.3 TB/s pack / unpack in-device; 2 lanes x 6 stages (more bytes in flight, fewer issue slots)
+  p->tune.bulk_warps = 3;      // reads 5.9 / 5.8 (profiles/r3_sweep_bulk.txt)
   p->tune.stage_slots = 2;                   // one slot fills while the other drains; the kernels take ~2 % of a copy's time
   p->tune.stage_chunk_bytes = 256ull << 20;  // ring <= 512 MiB whatever the context length (larger layers: device-major chunks)
   p->tune.vec_threads = 512;
@@ -652,7 +652,7 @@ int kvpool_place(kvpool_t* p, const uint32_t* blocks_per_layer, kvpool_placement
   for (uint32_t l = 0; l < L; ++l) {
     auto& Ls = pl->layers[l];
     Ls.stripe_off.assign(N, 0);
-    if (p->ssd_mask) { Ls.ssd_last_lane.assign(N, 0); Ls.ssd_last_use.assign(N, 0); }
+    if (p->ssd_mask) Ls.ssd_lane_use.assign(N, {});
     for (uint32_t i = 0; i < N; ++i) {
       const uint64_t align = is_ssd(p, i) ? std::max<uint64_t>(256, p->ssd[i]->io.sector()) : 256;
       Ls.stripe_off[i] = pl->region_bytes[i];  // relative for now
@@ -885,6 +885,15 @@ int kvpool_ssd_location(const kvpool_placement_t* pl, uint32_t layer, uint32_t b
   const uint64_t sec = pl->pool->ssd[d]->io.sector(), at = L.stripe_off[d] + static_cast<uint64_t>(L.map->slot[block]) * pl->pool->payload;
   if (lba) *lba = at / sec;
   if (byte_in_sector) *byte_in_sector = static_cast<uint32_t>(at % sec);
+  return KVPOOL_OK;
+}
+
+int kvpool_io_errors(const kvpool_t* p, uint64_t* failed_out) {
+  if (!p || !failed_out) return fail(KVPOOL_EINVAL, "io_errors: bad arguments");
+  uint64_t n = 0;  // no pool lock: the counters are atomics of the workers, the device list is fixed at create
+  for (const auto& S : p->ssd)
+    if (S) n += S->io.failed();
+  *failed_out = n;
   return KVPOOL_OK;
 }
 
