@@ -61,12 +61,18 @@ def parse_args():
                          "pair per pool device (the paper's literal 'independent I/O streams', PAPER.md:177)")
     ap.add_argument("--per-layer", action="store_true",
                     help="issue one kvpool_offload / kvpool_retrieve call per layer in the timed step instead of the batched *_layers calls")
+    ap.add_argument("--lockstep", action="store_true",
+                    help="several requests (config 5): issue LAYER-major - layer l of every request before layer l+1 of any, one per-layer "
+                         "call per request and layer on the request's own stream - as a batch decode that runs its requests in lock-step "
+                         "needs them; default: request-major batched calls")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the side lines printed beside the headline (paths.zerocopy / paths.hybrid on the "
                                                               "same workload, shapes.* = the other two 128K shapes)")
     ap.add_argument("--settle-s", type=float, default=60.0, help="upper bound on the untimed host-settle phase before the timed steps (0 = off)")
     ap.add_argument("--sweep", choices=["hbm", "link"], default=None,
                     help="tuning sweep instead of the benchmark: in-device pack/unpack (hbm) or zero-copy transfer (link) GB/s over launch shapes")
+    ap.add_argument("--sweep-kernels", choices=["all", "vec16", "bulk"], default="all", help="--sweep hbm: which kernel's launch shapes to run")
+    ap.add_argument("--bulk-shape", default=None, help="--sweep hbm: run only this bulk launch shape: warps,stages,chunk,ctas")
     ap.add_argument("--variants", action="store_true",
                     help="time the transfer variants side by side on --config (default 2): per-block cudaMemcpyAsync, staged, zero-copy")
     ap.add_argument("--blocked-io", action="store_true",
@@ -91,6 +97,9 @@ def parse_args():
                     "huge-page mapping + cudaHostRegister; main run and --duplex")
     ap.add_argument("--contexts", default="1024,4096,16384,32768,65536,131072", help="--blocked-io: the context lengths to run, comma separated")
     ap.add_argument("--compute-us", type=float, default=0.0, help="--blocked-io: extra calibrated compute per layer (kvpool_spin), microseconds")
+    ap.add_argument("--launch-only", action="store_true",
+                    help="start the ranks of --gpus N, have them meet (gloo, no GPU needed), print {\"launched_ranks\": N} from rank 0 and exit: "
+                         "checks the launcher by itself")
     ap.add_argument("--detail", default=None, help="write per-layer latencies and side measurements to this JSON file")
     return ap.parse_args()
 
@@ -245,7 +254,7 @@ def run_reference(args) -> dict:
         sys.exit(0)
     st = oracle_setup(args.config)
     wl = st[1]
-    layers_per_step = 4
+    layers_per_step = wl.geom.n_layers          # a step = the whole request, as in the CUDA arm (config 4: 48 layers, 12 GiB per leg)
     for _ in range(args.warmup):
         oracle_time_layers(st, 1, True)
     t_ret = t_all = 0.0
@@ -316,6 +325,7 @@ class Rig:
             tune["stage_chunk_bytes"] = int(args.stage_chunk_mib * 2**20) if args.stage_chunk_mib > 0 else 2**64 - 1
         if tune:
             pool.set_tuning(**tune)
+        self.lockstep = bool(args.lockstep) and R > 1
         self.set_path(path)
         self.tn = pool.get_tuning()
         self.numa_actual = [pool.device_info(i)["numa_node"] for i in range(N)]
@@ -367,7 +377,10 @@ class Rig:
     def do_offload(self, pls, own_tables: bool = False):
         pool, g = self.pool, self.g
         self.fork()
-        for r in range(self.R):
+        for l in range(self.L) if self.lockstep else ():
+            for r in range(self.R):
+                pool.offload(pls[r], l, self.src_k[l], self.src_v[l], g.kvb, None if own_tables else self.tables[r][l], self.stream_of(r))
+        for r in range(self.R) if not self.lockstep else ():
             tb = None if own_tables else self.tables[r]
             if self.args.per_layer:
                 for l in range(self.L):
@@ -383,7 +396,14 @@ class Rig:
         records when a layer is complete in the paged layout."""
         pool, g = self.pool, self.g
         self.fork()
-        for r in range(self.R):
+        # lock-step (SURVEY 8(d) config 5): the link's I/O stream serves transfers in issue order, so layer-major issue hands
+        # every request its layer l before any request gets layer l+1
+        for l in range(self.L) if self.lockstep else ():
+            for r in range(self.R):
+                pool.retrieve(pls[r], l, self.dst_k[l], self.dst_v[l], g.kvb, None if own_tables else self.tables[r][l], self.stream_of(r))
+                if ready is not None:
+                    ready[r][l].record(self.stream_of(r))
+        for r in range(self.R) if not self.lockstep else ():
             s, tb = self.stream_of(r), (None if own_tables else self.tables[r])
             if self.args.per_layer:
                 for l in range(self.L):
@@ -755,6 +775,11 @@ def run_kvpool(args) -> dict:
     link_roof = {"bound": "host_link", "what": "retrieve leg (all layers back to back)", "achieved": value / world, "peak": link_h2d,
                  "unit": "GB/s", "frac": value / world / link_h2d, "offload_achieved": moved / (off_ms * 1e6), "offload_peak": link_d2h,
                  "offload_frac": moved / (off_ms * 1e6) / link_d2h, "peak_source": "1 GiB pinned cudaMemcpyAsync measured in this run"}
+    # the step itself is bound by the host link, not by the dominant kernel: the link figures sit inside the object the driver parses
+    roof["link"] = {"achieved": link_roof["achieved"], "peak": link_h2d, "frac": link_roof["frac"], "unit": "GB/s",
+                    "what": "the metric: retrieve leg of the step against the cudaMemcpyAsync H2D peak measured in this run"}
+    roof["frac_is"] = ("event pairs around each launch inside the timed step (the contract's clock; reads long under a concurrent DMA); "
+                       "frac_kernel_clock is the same launches by the kernel's own %globaltimer span, roofline_hbm.*_back_to_back the kernel alone")
     best_unpack = max(hbm["unpack_vec16_back_to_back_gbps"], hbm["unpack_bulk_back_to_back_gbps"])
     best_pack = max(hbm["pack_vec16_back_to_back_gbps"], hbm["pack_bulk_back_to_back_gbps"])
     hbm_roof = {"bound": "hbm", "what": f"in-device pack/unpack of one {Kbig * g.payload / 2**20:.0f} MiB layer launched alone, 2*bytes/time; "
@@ -818,6 +843,22 @@ def run_kvpool(args) -> dict:
             shapes[other.wl.name] = side_line(other, 9 if other.moved < (8 << 30) else 5, 3, link_h2d, link_d2h)
             other.close()
 
+    concurrency = None
+    if world == 1 and args.config == 4 and args.path == "auto" and not args.no_extras:
+        # config 5 (BASELINE.json configs[4]): four requests of 32K..128K on four streams in LOCK-STEP - layer l of
+        # every request before layer l+1 of any (960 MiB per layer round).  retrieve_layer_ms = the interval between consecutive
+        # layer-ready events of ONE request, i.e. what a batch-4 decode waits per layer; the floor is 960 MiB / link peak.
+        try:
+            conc = Rig(args, 5, "auto", local, world)
+            conc.lockstep = True
+            concurrency = side_line(conc, 3, 1, link_h2d, link_d2h)
+            per_round = sum(int(conc.bpl[r].max()) for r in range(conc.R)) * conc.g.payload
+            concurrency.update(issue_order="layer-major (lock-step), one per-layer call per request and layer, 4 streams",
+                               layer_round_bytes=per_round, layer_round_floor_ms=per_round / (link_h2d * 1e6))
+            conc.close()
+        except Exception as e:                         # (a host without ~50 GiB to pin: say so instead of losing the headline)
+            concurrency = {"error": f"{type(e).__name__}: {e}"}
+
     pools = {}
     if world == 1 and args.config == 4 and args.path == "auto" and not args.no_extras:
         # unified pooling over host memory AND block storage: a pinned host buffer plus one SSD-type
@@ -871,6 +912,8 @@ def run_kvpool(args) -> dict:
         out["paths"] = paths
     if shapes:
         out["shapes"] = shapes
+    if concurrency:
+        out["concurrency"] = concurrency
     if pools:
         out["pools"] = pools
     if layer_rows:
@@ -928,13 +971,18 @@ def run_sweep(args) -> None:
     if args.sweep == "hbm":
         print("# in-device pack / unpack, GB/s = 2*bytes/time, 8 launches per event pair, median of 6; measured HBM copy peak "
               f"{measured_peaks()['hbm_gbs']:.0f} GB/s")
-        for threads, unroll, ctas in itertools.product((128, 256, 512), (4, 8, 16), (148, 296, 592, 1184, 2368, 4736)):
+        vec_grid = itertools.product((128, 256, 512), (4, 8, 16), (148, 296, 592, 1184, 2368, 4736)) if args.sweep_kernels in ("all", "vec16") else ()
+        for threads, unroll, ctas in vec_grid:
             pool.set_tuning(kernel=kv.KERNEL_VEC16, vec_threads=threads, vec_unroll=unroll, hbm_ctas=ctas)
             p = timed(lambda l: pool.pack(pl, l, src[l][0], src[l][1], g.kvb, tables[l], stage, main_s), 8, 8)
             u = timed(lambda l: pool.unpack(pl, l, src[l][0], src[l][1], g.kvb, tables[l], stage, main_s), 8, 8)
             print(f"vec16 threads {threads:4d} unroll {unroll:2d} ctas {ctas:5d}: pack {2 * nbytes / p / 1e6:6.0f}  unpack {2 * nbytes / u / 1e6:6.0f}", flush=True)
-        for warps, stages, chunk, ctas in [(1, 8, 16384, 148), (2, 6, 16384, 148), (2, 4, 16384, 148), (4, 6, 8192, 148), (4, 4, 8192, 296),
-                                           (2, 3, 16384, 296), (2, 3, 32768, 148), (4, 3, 16384, 148), (8, 3, 8192, 148), (8, 6, 4096, 148)]:
+        only = [tuple(int(x) for x in args.bulk_shape.split(","))] if args.bulk_shape else None
+        for warps, stages, chunk, ctas in only or [(1, 8, 16384, 148), (2, 6, 16384, 148), (2, 4, 16384, 148), (4, 6, 8192, 148), (4, 4, 8192, 296),
+                                           (2, 3, 16384, 296), (2, 3, 32768, 148), (4, 3, 16384, 148), (8, 3, 8192, 148), (8, 6, 4096, 148),
+                                           (3, 4, 16384, 148), (4, 4, 8192, 148), (6, 4, 8192, 148), (4, 5, 8192, 148), (3, 5, 8192, 148), (5, 4, 8192, 148),
+                                           (7, 3, 8192, 148), (3, 3, 16384, 148), (3, 2, 32768, 148), (5, 2, 16384, 148), (6, 2, 16384, 148), (3, 8, 8192, 148),
+                                           (3, 4, 16384, 296)] if args.sweep_kernels in ("all", "bulk") else []:
             pool.set_tuning(kernel=kv.KERNEL_BULK, bulk_warps=warps, bulk_stages=stages, bulk_chunk=chunk, hbm_ctas=ctas)
             p = timed(lambda l: pool.pack(pl, l, src[l][0], src[l][1], g.kvb, tables[l], stage, main_s), 8, 8)
             u = timed(lambda l: pool.unpack(pl, l, src[l][0], src[l][1], g.kvb, tables[l], stage, main_s), 8, 8)
@@ -1492,8 +1540,58 @@ def run_blocked_io(args) -> None:
             json.dump(rows, f, indent=1)
 
 
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` by itself (no torchrun around it: WORLD_SIZE unset) starts the N ranks here: one process per
+    GPU, each a copy of this command line with RANK / LOCAL_RANK / WORLD_SIZE / MASTER_ADDR / MASTER_PORT set, exactly what
+    torchrun would hand them.  Rank 0 inherits stdout and prints the one JSON line; every rank's stderr passes through.  Fewer
+    visible GPUs than ranks is an error, never a silent N = 1.  Returns the worst exit code."""
+    import socket
+    n = args.gpus
+    if args.impl == "kvpool" and not args.launch_only:
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < n:
+            log(f"bench.py --gpus {n}: only {have} CUDA device(s) visible - refusing to run fewer ranks than asked for")
+            return 2
+    with socket.socket() as sock:
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+    procs = []
+    for r in range(n):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(n), LOCAL_WORLD_SIZE=str(n), MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        env.setdefault("NCCL_DEBUG", "INFO" if r == 0 else "WARN")   # rank 0's NCCL log names the ranks and the transport
+        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__)] + sys.argv[1:], env=env,
+                                      stdout=None if r == 0 else subprocess.DEVNULL))
+    log(f"bench.py: started {n} ranks (one per GPU), rendezvous 127.0.0.1:{port}")
+    rcs = [p.wait() for p in procs]
+    return max(abs(rc) for rc in rcs)
+
+
+def launch_only(args) -> None:
+    import torch
+    import torch.distributed as dist
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    if world > 1:
+        dist.init_process_group("gloo")
+    t = torch.ones(1, dtype=torch.int64)
+    if world > 1:
+        dist.all_reduce(t)
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"launched_ranks": int(t.item()), "n_gpus": args.gpus}), flush=True)
+
+
 def main():
     args = parse_args()
+    world = os.environ.get("WORLD_SIZE")
+    if args.gpus > 1 and world is None and (args.impl == "kvpool" or args.launch_only):
+        sys.exit(spawn_ranks(args))
+    if world is not None and int(world) != args.gpus:
+        log(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE={world} ranks")
+        sys.exit(2)
+    if args.launch_only:
+        launch_only(args)
+        return
     if args.impl == "reference":
         print(json.dumps(run_reference(args)), flush=True)
         return
